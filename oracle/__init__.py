@@ -1,0 +1,261 @@
+"""ctypes wrapper around the CPU oracle (oracle.cpp).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs may import this package; the product
+(paper_1004_0014_b200) never does.  All results are float64.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import numpy as np
+
+from .build import build as _build
+
+
+class _Geom(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("hx", C.c_double), ("hy", C.c_double), ("hz", C.c_double),
+                ("cx", C.c_double), ("cy", C.c_double), ("cz", C.c_double),
+                ("K", C.c_int32), ("nu", C.c_int32), ("nv", C.c_int32),
+                ("pu", C.c_double), ("pv", C.c_double), ("sad", C.c_double), ("sdd", C.c_double),
+                ("off_u", C.c_double), ("off_v", C.c_double)]
+
+
+class _Opts(C.Structure):
+    _fields_ = [("max_iter", C.c_int32), ("grad_tol", C.c_double), ("armijo_c", C.c_double),
+                ("armijo_beta", C.c_double), ("max_backtracks", C.c_int32),
+                ("init_step_vox", C.c_double), ("batched_linesearch", C.c_int32),
+                ("inv_max_iter", C.c_int32), ("inv_tol_mm", C.c_double)]
+
+
+class _Result(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("status", C.c_int32), ("J0", C.c_double), ("J", C.c_double),
+                ("a", C.c_double), ("b", C.c_double)]
+
+
+@dataclass(frozen=True)
+class Geometry:
+    nx: int
+    ny: int
+    nz: int
+    hx: float
+    hy: float
+    hz: float
+    K: int
+    nu: int
+    nv: int
+    pu: float
+    pv: float
+    sad: float = 1000.0
+    sdd: float = 1500.0
+    off_u: float = 0.0
+    off_v: float = 0.0
+    cx: float = 0.0
+    cy: float = 0.0
+    cz: float = 0.0
+
+    @property
+    def V(self):
+        return self.nx * self.ny * self.nz
+
+    @property
+    def vshape(self):
+        return (self.nz, self.ny, self.nx)
+
+    @property
+    def pshape(self):
+        return (self.nv, self.nu)
+
+    def _c(self) -> _Geom:
+        # pitches and sizes are what the float32 C-ABI of the GPU path sees: round through float32
+        f = lambda v: float(np.float32(v))
+        return _Geom(self.nx, self.ny, self.nz, f(self.hx), f(self.hy), f(self.hz),
+                     f(self.cx), f(self.cy), f(self.cz), self.K, self.nu, self.nv,
+                     f(self.pu), f(self.pv), f(self.sad), f(self.sdd), f(self.off_u), f(self.off_v))
+
+
+@dataclass
+class Opts:
+    max_iter: int = 10
+    grad_tol: float = 0.0
+    armijo_c: float = 1e-4
+    armijo_beta: float = 0.5
+    max_backtracks: int = 8
+    init_step_vox: float = 1.0
+    batched_linesearch: int = 0
+    inv_max_iter: int = 50
+    inv_tol_mm: float = 1e-4
+
+    def _c(self) -> _Opts:
+        f = lambda v: float(np.float32(v))
+        return _Opts(self.max_iter, f(self.grad_tol), f(self.armijo_c), f(self.armijo_beta),
+                     self.max_backtracks, f(self.init_step_vox), self.batched_linesearch,
+                     self.inv_max_iter, f(self.inv_tol_mm))
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build())
+        _lib.orc_cost.restype = C.c_double
+    return _lib
+
+
+def set_threads(n: int) -> None:
+    lib().orc_set_threads(int(n))
+
+
+def max_threads() -> int:
+    return int(lib().orc_max_threads())
+
+
+def _f32(a):
+    a = np.ascontiguousarray(a)
+    assert a.dtype == np.float32, "oracle inputs are the float32 arrays the GPU path consumes"
+    return a
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _angle(theta) -> float:
+    # the C-ABI passes the gantry angle as float32
+    return float(np.float32(theta))
+
+
+def warp(g: Geometry, f0, xbar, u, w) -> np.ndarray:
+    f0, xbar, u, w = _f32(f0), _f32(xbar), _f32(u), _f64(w)
+    out = np.empty(g.vshape, dtype=np.float64)
+    gc = g._c()
+    lib().orc_warp(C.byref(gc), _p(f0), _p(xbar), _p(u), _p(w), _p(out))
+    return out
+
+
+def warp_grad(g: Geometry, f0, xbar, u, w) -> np.ndarray:
+    f0, xbar, u, w = _f32(f0), _f32(xbar), _f32(u), _f64(w)
+    out = np.empty((3,) + g.vshape, dtype=np.float64)
+    gc = g._c()
+    lib().orc_warp_grad(C.byref(gc), _p(f0), _p(xbar), _p(u), _p(w), _p(out))
+    return out
+
+
+def project(g: Geometry, f, theta) -> np.ndarray:
+    f = _f64(f)
+    assert f.size == g.V
+    out = np.empty(g.pshape, dtype=np.float64)
+    gc = g._c()
+    lib().orc_project(C.byref(gc), _p(f), C.c_double(_angle(theta)), _p(out))
+    return out
+
+
+def backproject(g: Geometry, r, theta) -> np.ndarray:
+    r = _f64(r)
+    assert r.size == g.nu * g.nv
+    out = np.empty(g.vshape, dtype=np.float64)
+    gc = g._c()
+    lib().orc_backproject(C.byref(gc), _p(r), C.c_double(_angle(theta)), _p(out))
+    return out
+
+
+def traverse(g: Geometry, theta, iu: int, iv: int):
+    cap = g.nx + g.ny + g.nz + 8
+    ijk = np.zeros((cap, 3), dtype=np.int32)
+    ln = np.zeros(cap, dtype=np.float64)
+    n = C.c_int32(0)
+    gap = C.c_double(0)
+    gc = g._c()
+    rc = lib().orc_traverse(C.byref(gc), C.c_double(_angle(theta)), int(iu), int(iv), cap, _p(ijk), _p(ln),
+                            C.byref(n), C.byref(gap))
+    assert rc == 0
+    return ijk[:n.value].copy(), ln[:n.value].copy(), gap.value
+
+
+def min_gaps(g: Geometry, theta) -> np.ndarray:
+    out = np.empty(g.pshape, dtype=np.float64)
+    gc = g._c()
+    lib().orc_min_gaps(C.byref(gc), C.c_double(_angle(theta)), _p(out))
+    return out
+
+
+def lsfit(p, y):
+    p, y = _f64(p), _f32(y)
+    a, b = C.c_double(0), C.c_double(0)
+    rc = lib().orc_lsfit(C.c_int64(p.size), _p(p), _p(y), C.byref(a), C.byref(b))
+    return rc, a.value, b.value
+
+
+def cost(p, y, a, b) -> float:
+    p, y = _f64(p), _f32(y)
+    return float(lib().orc_cost(C.c_int64(p.size), _p(p), _p(y), C.c_double(a), C.c_double(b)))
+
+
+def gradient(g: Geometry, f0, xbar, u, w, a, b, p, y, theta) -> np.ndarray:
+    f0, xbar, u, w, p, y = _f32(f0), _f32(xbar), _f32(u), _f64(w), _f64(p), _f32(y)
+    out = np.empty(g.K, dtype=np.float64)
+    gc = g._c()
+    lib().orc_gradient(C.byref(gc), _p(f0), _p(xbar), _p(u), _p(w), C.c_double(a), C.c_double(b), _p(p), _p(y),
+                       C.c_double(_angle(theta)), _p(out))
+    return out
+
+
+def evaluate(g: Geometry, f0, xbar, u, w, theta):
+    """f(w) and p = P f(w)."""
+    f = warp(g, f0, xbar, u, w)
+    return f, project(g, f, theta)
+
+
+def invert(g: Geometry, xbar, u, w, r0, max_iter: int = 50, tol_mm: float = 1e-4):
+    xbar, u, w = _f32(xbar), _f32(u), _f64(w)
+    r0 = _f32(np.atleast_2d(r0))
+    M = r0.shape[0]
+    out = np.empty((M, 3), dtype=np.float64)
+    its = np.zeros(M, dtype=np.int32)
+    gc = g._c()
+    lib().orc_invert(C.byref(gc), _p(xbar), _p(u), _p(w), M, _p(r0), int(max_iter),
+                     C.c_double(float(np.float32(tol_mm))), _p(out), _p(its))
+    return out, its
+
+
+def dvf_at_points(g: Geometry, xbar, u, w, pts) -> np.ndarray:
+    xbar, u, w = _f32(xbar), _f32(u), _f64(w)
+    pts = _f64(np.atleast_2d(pts))
+    out = np.empty_like(pts)
+    gc = g._c()
+    lib().orc_dvf_at_points(C.byref(gc), _p(xbar), _p(u), _p(w), pts.shape[0], _p(pts), _p(out))
+    return out
+
+
+def solve(g: Geometry, f0, xbar, u, y, theta, w0, opts: Optional[Opts] = None,
+          forced_mu: Optional[Sequence[float]] = None, want_volume: bool = True):
+    opts = opts or Opts()
+    f0, xbar, u, y, w0 = _f32(f0), _f32(xbar), _f32(u), _f32(y), _f64(w0)
+    n = opts.max_iter
+    w = np.empty(g.K, dtype=np.float64)
+    f = np.empty(g.vshape, dtype=np.float64) if want_volume else None
+    p = np.empty(g.pshape, dtype=np.float64)
+    Jt = np.full(n + 1, np.nan)
+    gt = np.full(max(n, 1), np.nan)
+    mt = np.full(max(n, 1), np.nan)
+    bt = np.full(max(n, 1), -1, dtype=np.int32)
+    res = _Result()
+    fm = _f64(forced_mu) if forced_mu is not None else None
+    if fm is not None:
+        assert fm.size >= n
+    gc, oc = g._c(), opts._c()
+    lib().orc_solve(C.byref(gc), _p(f0), _p(xbar), _p(u), _p(y), C.c_double(_angle(theta)), _p(w0), C.byref(oc),
+                    _p(fm) if fm is not None else None, _p(w), _p(f) if f is not None else None, _p(p),
+                    C.byref(res), _p(Jt), _p(gt), _p(mt), _p(bt))
+    it = res.iters
+    return dict(w=w, f=f, p=p, a=res.a, b=res.b, J0=res.J0, J=res.J, iters=it, status=res.status,
+                J_trace=Jt[:it + 1], gnorm_trace=gt[:min(it + 1, n)], mu_trace=mt[:it], backtracks=bt[:it])

@@ -1,0 +1,188 @@
+/* pcamm.h -- C ABI of the B200 per-projection PCA lung-motion solve.
+ *
+ * Method: Li, Jia, Lewis, Gu, Folkerts, Men, Jiang, "Real-time volumetric image reconstruction and
+ * 3D tumor localization based on a single x-ray projection image for lung cancer radiotherapy"
+ * (PAPER.md).  Citations below are PAPER.md line numbers plus the section / equation they fall in;
+ * "reading A<n>" refers to the list of readings in DESIGN.md.
+ *
+ * The library minimises (section 2.2, Eq. 2)
+ *
+ *        J(w, a, b) = || P_theta f(x, f0) - a y - b 1 ||_2^2     s.t.   x = xbar + U w
+ *
+ * by the alternating algorithm of PAPER.md:L84-95 (Eq. 3: gradient step on w with Armijo's rule,
+ * Eq. 4: closed-form (a, b)), and localises landmarks through the fixed-point inverse of the
+ * pull-back DVF (section 2.3).  Every step runs in CUDA kernels for sm_100a;
+ * there is no CPU fallback.  All calls are blocking with respect to their host outputs.
+ *
+ * Conventions
+ *   volume   [nz][ny][nx] float32, x fastest; voxel (i,j,k) centre in world mm is
+ *            (cx + (i-(nx-1)/2) hx, cy + (j-(ny-1)/2) hy, cz + (k-(nz-1)/2) hz); z = rotation axis.
+ *   fields   DVFs are pull-back, in mm: f(r) = f0(r + x(r)) (reading A1), stored
+ *            planar [3][nz][ny][nx] (component 0 = x).
+ *   detector [nv][nu] float32, u fastest.  At gantry angle theta the source is
+ *            S = sad (cos theta, sin theta, 0), the detector centre C = -(sdd-sad)(cos theta, sin theta, 0),
+ *            u^ = (-sin theta, cos theta, 0), v^ = (0,0,1); pixel (iu,iv) centre is
+ *            C + (iu-(nu-1)/2+off_u) pu u^ + (iv-(nv-1)/2+off_v) pv v^   (reading A14).
+ *   P        Siddon's exact radiological path, one ray per pixel centre: p_i = sum_j l_ij f_j with
+ *            l_ij the length in mm of the source->pixel segment inside voxel box j (reading A3);
+ *            P^T is the transpose of the same l_ij (reading A4).
+ *   *_dev    CUDA device pointers (caller-owned);  *_host  host pointers (caller-owned).
+ *   stream   a cudaStream_t passed as void* (NULL = default stream).
+ *
+ * Return codes: 0 OK; < 0 hard error (PCAMM_E_*); > 0 soft status of a solve (PCAMM_S_*), also
+ * stored in pcamm_info.status.  No exception crosses the ABI.  pcamm_last_error() returns a
+ * thread-local message for the last hard error on the calling thread.
+ */
+#ifndef PCAMM_H
+#define PCAMM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PCAMM_KMAX 8            /* maximum number of eigenvector fields K */
+#define PCAMM_MAX_BACKTRACKS 16 /* upper bound on pcamm_opts.max_backtracks */
+
+#define PCAMM_OK 0
+#define PCAMM_E_INVALID (-1)    /* invalid argument / size mismatch / unsupported geometry */
+#define PCAMM_E_CUDA (-2)       /* CUDA runtime error (message in pcamm_last_error) */
+#define PCAMM_E_NOMEM (-3)      /* device allocation failed */
+#define PCAMM_E_NONFINITE (-4)  /* non-finite value in an input checked at this call */
+#define PCAMM_E_SINGULAR (-5)   /* intensity fit singular: y is constant (reading A8) */
+#define PCAMM_S_MAXITER 1       /* stopped on max_iter */
+#define PCAMM_S_GRADTOL 2       /* stopped on ||g||_2 <= grad_tol */
+#define PCAMM_S_LINESEARCH 3    /* no candidate step satisfied Armijo's inequality */
+
+typedef struct pcamm_model pcamm_model; /* opaque; immutable after create except for its scratch */
+
+typedef struct {
+    int32_t nx, ny, nz;   /* volume size, x fastest */
+    float hx, hy, hz;     /* voxel size, mm */
+    float cx, cy, cz;     /* world position of the volume centre, mm (isocentre = origin) */
+    int32_t K;            /* number of eigenvector fields, 1..PCAMM_KMAX (Eq. 1) */
+    int32_t nu, nv;       /* detector size, u fastest */
+    float pu, pv;         /* pixel pitch, mm */
+    float sad, sdd;       /* source-axis and source-detector distance, mm */
+    float off_u, off_v;   /* detector offset in pixels */
+    int32_t max_batch;    /* largest B of pcamm_reconstruct_batch (>= 1); scratch is sized for it */
+    int32_t max_candidates; /* 1, or >= opts.max_backtracks to allow batched_linesearch */
+} pcamm_geometry;
+
+typedef struct {
+    int32_t max_iter;       /* default 10 */
+    float grad_tol;         /* stop if ||g||_2 <= grad_tol; default 0 = off */
+    float armijo_c;         /* default 1e-4 (reading A7) */
+    float armijo_beta;      /* default 0.5 */
+    int32_t max_backtracks; /* default 8 */
+    float init_step_vox;    /* first trial moves the DVF by this many voxels rms; default 1 (A7) */
+    int32_t batched_linesearch; /* 0: sequential backtracking; 1: evaluate all candidates at once
+                                   and take the largest passing step (same result; config C3) */
+    int32_t inv_max_iter;   /* default 50 (reading A13) */
+    float inv_tol_mm;       /* default 1e-4 */
+    int32_t loop_mode;      /* 0 (default): the whole solve is one CUDA graph with device-side
+                               while-loops, no host round trip per trial;
+                               1: the host drives the same kernels and reads one status word per
+                               step (debug aid; same arithmetic) */
+} pcamm_opts;
+
+typedef struct {
+    int32_t iters, status;
+    double J0, J;           /* cost after the initial intensity fit / at exit (Eq. 2) */
+    double a, b;            /* intensity fit at exit (Eq. 4) */
+    /* optional traces, caller-allocated host arrays or NULL:
+       J_trace[max_iter+1], gnorm_trace[max_iter], mu_trace[max_iter], backtracks_trace[max_iter] */
+    double* J_trace;
+    double* gnorm_trace;
+    double* mu_trace;
+    int32_t* backtracks_trace;
+} pcamm_info;
+
+/* Fills *opts with the defaults listed above. */
+void pcamm_default_opts(pcamm_opts* opts);
+
+/* Build a model: copies f0 [nz][ny][nx], the mean DVF [3][nz][ny][nx] and the K eigenvector fields
+ * [K][3][nz][ny][nx] (mm; Eq. 1) into library-owned device memory, allocates all
+ * scratch for geometry->max_batch x max_candidates evaluations, and stores the n_landmarks
+ * reference positions [M][3] (mm).  The caller may free its inputs on return.
+ * Geometry restrictions (else PCAMM_E_INVALID): the source and the detector plane lie outside
+ * the volume's bounding sphere, and a ray moves at most one voxel in z per voxel along its
+ * dominant in-plane axis (true for any circular cone-beam geometry with sane voxel aspect). */
+int pcamm_model_create(const pcamm_geometry* geometry, const float* f0_dev, const float* mean_dvf_dev,
+                       const float* eig_dvf_dev, int32_t n_landmarks, const float* landmarks_mm_host,
+                       void* stream, pcamm_model** out);
+void pcamm_model_destroy(pcamm_model* model);
+
+/* The per-projection solve (sections 2.2-2.3).  y_dev [nv][nu] is the measured
+ * projection, w_init_host [K] the start (the previous frame's w).  Outputs:
+ * w_out_host [K]; volume_out_dev [nz][ny][nx] = f(w) or NULL; landmarks_out_host [M][3] mm or
+ * NULL; info or NULL.  Returns a PCAMM_S_* status or a PCAMM_E_* error. */
+int pcamm_reconstruct(pcamm_model* model, const float* y_dev, float angle_rad, const float* w_init_host,
+                      const pcamm_opts* opts, float* w_out_host, float* volume_out_dev,
+                      float* landmarks_out_host, pcamm_info* info, void* stream);
+
+/* Same, with the measured projection in host memory: the host->device copy of y is part of the
+ * call (used for end-to-end timing). */
+int pcamm_reconstruct_host(pcamm_model* model, const float* y_host, float angle_rad,
+                           const float* w_init_host, const pcamm_opts* opts, float* w_out_host,
+                           float* volume_out_dev, float* landmarks_out_host, pcamm_info* info,
+                           void* stream);
+
+/* B independent solves in flight (different angles, projections and starts), advanced in lock
+ * step so that every pass over the K+1 vector fields serves all B of them.  Arrays are the
+ * single-solve ones with a leading [B]; info is an array of B or NULL.  Returns 0 when every
+ * solve ended with a soft status, else the first hard error. */
+int pcamm_reconstruct_batch(pcamm_model* model, int32_t B, const float* y_dev, const float* angles_rad_host,
+                            const float* w_init_host, const pcamm_opts* opts, float* w_out_host,
+                            float* volumes_out_dev, float* landmarks_out_host, pcamm_info* info,
+                            void* stream);
+
+/* ---- function-level hooks (parity tests; reading A16 level i) ---- */
+
+/* f = warp(f0, xbar + U w): Eq. 1 + trilinear pull-back. */
+int pcamm_warp(pcamm_model* model, const float* w_host, float* volume_out_dev, void* stream);
+
+/* p = P_theta f for a caller-supplied volume [nz][ny][nx] (Eq. 2). */
+int pcamm_project(pcamm_model* model, const float* volume_dev, float angle_rad, float* proj_out_dev,
+                  void* stream);
+
+/* B = P_theta^T r for a caller-supplied detector image r [nv][nu]: backprojection onto the voxel
+ * grid, [nz][ny][nx] (reading A4).  Test hook for the adjoint identity; the solve
+ * itself never materialises this volume. */
+int pcamm_backproject(pcamm_model* model, const float* r_dev, float angle_rad, float* volume_out_dev,
+                      void* stream);
+
+/* One evaluation at (w, a, b): p = P f(w) (written to proj_out_dev if not NULL),
+ * J = ||p - a y - b||^2 (Eq. 2), grad[k] = dJ/dw_k, and the least-squares
+ * (a, b) of Eq. 4 for this p in ab_fit_out[2] (or NULL). */
+int pcamm_eval(pcamm_model* model, const float* y_dev, float angle_rad, const float* w_host, float a,
+               float b, double* J_out, double* grad_out, double* ab_fit_out, float* proj_out_dev,
+               void* stream);
+
+/* Ordered voxel list and intersection lengths (mm) of one ray, source side first, segments of
+ * zero length dropped (reading A22).  Runs the projector's own traversal code on the device. */
+int pcamm_traverse(pcamm_model* model, float angle_rad, int32_t iu, int32_t iv, int32_t cap,
+                   int32_t* ijk_out_host, float* len_out_host, int32_t* n_out, void* stream);
+
+/* Landmark positions r with r + x(r) = r0 by r_{m+1} = r0 - x(r_m) (A13). */
+int pcamm_localise(pcamm_model* model, const float* w_host, int32_t inv_max_iter, float inv_tol_mm,
+                   float* landmarks_out_host, void* stream);
+
+/* Timing hook for bench.py: launches the given kernel of one evaluation `reps` times on `stream`
+ * with the model's scratch (inputs taken as they stand from the last pcamm_eval) and returns the
+ * average device time per launch in milliseconds, measured with CUDA events on that stream.
+ * which: 0 = warp (a-1), 1 = project (a-2), 2 = gradient (a-4). */
+int pcamm_time_kernel(pcamm_model* model, int32_t which, int32_t reps, float* ms_out, void* stream);
+
+/* Number of kernels launched by this library on the calling thread since the last reset
+ * (host-side launch count; kernels inside device-side loops are counted from the device's
+ * iteration counters after each solve). */
+int64_t pcamm_launch_count(int32_t reset);
+
+const char* pcamm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PCAMM_H */

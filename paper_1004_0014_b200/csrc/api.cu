@@ -1,0 +1,650 @@
+// C ABI of libpcamm (include/pcamm.h): model life cycle, the solve as one CUDA graph with
+// device-side while-loops (or driven from the host, opts.loop_mode = 1), and the function-level
+// hooks.  Argument marshalling and kernel sequencing only: every step of the hot path runs in the
+// kernels of warp.cu, project.cu, gradient.cu and control.cu.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "internal.h"
+
+namespace pcamm {
+
+static thread_local std::string g_error;
+static thread_local long long g_launches = 0;
+
+void set_error(const std::string& msg) { g_error = msg; }
+void count_launch(long long n) { g_launches += n; }
+
+namespace {
+
+struct GraphRec {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+};
+
+__global__ void k_count_nonfinite(const float* __restrict__ a, long long n, unsigned long long* count) {
+    unsigned long long c = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        if (!isfinite(a[i])) ++c;
+    if (c) atomicAdd(count, c);
+}
+
+}  // namespace
+}  // namespace pcamm
+
+using namespace pcamm;
+
+struct pcamm_model {
+    pcamm_geometry geo;
+    Geom G;
+    int M = 0, Bmax = 1, Cmax = 1, S = 1;
+    // model (device)
+    float *f0 = nullptr, *xbar = nullptr, *u = nullptr, *lm0 = nullptr;
+    // scratch (device)
+    float *vol_std = nullptr, *vol_tr = nullptr, *p = nullptr, *rL = nullptr;
+    float4* utab = nullptr;
+    float2* vtab = nullptr;
+    char* in_block = nullptr;
+    size_t in_block_bytes = 0, in_off = 0;
+    CtlBufs c = {};
+    SlotState* out_slots = nullptr;
+    double* lm_out = nullptr;
+    int* trav_ijk = nullptr;
+    float* trav_len = nullptr;
+    int* trav_n = nullptr;
+    int trav_cap = 0;
+    unsigned long long* nonfinite = nullptr;
+    float* y_stage = nullptr;   // device copy of a host-side measured projection (pcamm_reconstruct_host)
+    // pinned host staging
+    char* h_in = nullptr;
+    SolveState* h_solves = nullptr;
+    SolveTrace* h_traces = nullptr;
+    LoopFlags* h_flags = nullptr;
+    double* h_lm = nullptr;
+    int* h_trav = nullptr;
+    std::map<long long, GraphRec> graphs;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    std::vector<void*> dev_allocs, host_allocs;
+};
+
+namespace {
+
+#define CUDA_TRY(expr)                                                                         \
+    do {                                                                                       \
+        cudaError_t e_ = (expr);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            set_error(std::string(#expr) + ": " + cudaGetErrorString(e_));                     \
+            return e_ == cudaErrorMemoryAllocation ? PCAMM_E_NOMEM : PCAMM_E_CUDA;             \
+        }                                                                                      \
+    } while (0)
+
+int invalid(const std::string& msg) {
+    set_error(msg);
+    return PCAMM_E_INVALID;
+}
+
+template <class T>
+cudaError_t dalloc(pcamm_model* m, T** ptr, size_t count) {
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, count * sizeof(T) > 0 ? count * sizeof(T) : 16);
+    if (e == cudaSuccess) { m->dev_allocs.push_back(p); *ptr = (T*)p; }
+    return e;
+}
+
+template <class T>
+cudaError_t halloc(pcamm_model* m, T** ptr, size_t count) {
+    void* p = nullptr;
+    cudaError_t e = cudaMallocHost(&p, count * sizeof(T) > 0 ? count * sizeof(T) : 16);
+    if (e == cudaSuccess) { m->host_allocs.push_back(p); *ptr = (T*)p; }
+    return e;
+}
+
+CallOpts* h_opts(pcamm_model* m) { return (CallOpts*)m->h_in; }
+SolveIn* h_solve_in(pcamm_model* m) { return (SolveIn*)(m->h_in + m->in_off); }
+
+int check_seq(const Seq& q, const char* what) {
+    if (q.err != cudaSuccess) {
+        set_error(std::string(what) + ": " + cudaGetErrorString(q.err));
+        return PCAMM_E_CUDA;
+    }
+    return PCAMM_OK;
+}
+
+int resolve_opts(const pcamm_model* m, const pcamm_opts* user, pcamm_opts* o) {
+    pcamm_default_opts(o);
+    if (user) *o = *user;
+    if (o->max_iter < 0) return invalid("opts.max_iter < 0");
+    if (o->max_backtracks < 1 || o->max_backtracks > MAXBT) return invalid("opts.max_backtracks out of range");
+    if (!(o->armijo_beta > 0.f && o->armijo_beta < 1.f)) return invalid("opts.armijo_beta must be in (0, 1)");
+    if (!(o->armijo_c >= 0.f) || !(o->init_step_vox > 0.f)) return invalid("opts.armijo_c / init_step_vox");
+    if (o->batched_linesearch && o->max_backtracks > m->Cmax)
+        return invalid("batched_linesearch needs geometry.max_candidates >= opts.max_backtracks");
+    if (o->inv_max_iter < 0) return invalid("opts.inv_max_iter < 0");
+    return PCAMM_OK;
+}
+
+void fill_call(pcamm_model* m, const pcamm_opts& o, int B, int C) {
+    CallOpts* c = h_opts(m);
+    c->B = B; c->C = C;
+    c->max_iter = o.max_iter; c->max_backtracks = o.max_backtracks; c->batched = o.batched_linesearch ? 1 : 0;
+    c->inv_max_iter = o.inv_max_iter;
+    c->grad_tol = (double)o.grad_tol; c->armijo_c = (double)o.armijo_c; c->armijo_beta = (double)o.armijo_beta;
+    c->init_step_vox = (double)o.init_step_vox; c->inv_tol = (double)o.inv_tol_mm;
+    const Geom& G = m->G;
+    const double hmin = std::fmin((double)G.hx, std::fmin((double)G.hy, (double)G.hz));
+    c->hmin_sqrtV = hmin * std::sqrt((double)G.V);
+}
+
+int push_call(pcamm_model* m, int B, cudaStream_t st) {
+    CUDA_TRY(cudaMemcpyAsync(m->in_block, m->h_in, m->in_off + sizeof(SolveIn) * (size_t)B, cudaMemcpyHostToDevice, st));
+    return PCAMM_OK;
+}
+
+// ---- the kernel sequences of a solve (shared by the graph and the host-driven mode)
+
+void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_iter, int use_cond) {
+    const Geom& G = m->G;
+    launch_ysums(q, G, m->c, B);
+    launch_begin(q, G, m->c, 0);
+    launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, B * C, 0, m->vol_std, m->vol_tr, G.V);
+    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->vol_std, m->vol_tr, G.V, m->p, m->c.proj_part);
+    launch_ctl_init(q, G, m->c, h_iter, use_cond);
+}
+
+void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial, int use_cond) {
+    const Geom& G = m->G;
+    launch_resid(q, G, m->c.solves, m->c.in, B, 0, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
+    launch_grad(q, G, m->f0, m->xbar, m->u, m->c.solves, B, m->rL, m->utab, m->vtab, m->c.grad_part);
+    launch_ctl_grad(q, G, m->c, h_trial, use_cond);
+}
+
+void seq_trial(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_trial, int use_cond) {
+    const Geom& G = m->G;
+    launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, B * C, 0, m->vol_std, m->vol_tr, G.V);
+    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->vol_std, m->vol_tr, G.V, m->p, m->c.proj_part);
+    launch_ctl_trial(q, G, m->c, h_trial, use_cond);
+}
+
+void seq_tail(pcamm_model* m, Seq& q, int B) {
+    const Geom& G = m->G;
+    launch_resid(q, G, m->c.solves, m->c.in, B, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
+    launch_ctl_final(q, G, m->c, m->out_slots);
+    launch_invert(q, G, m->xbar, m->u, m->c, B, m->M, m->lm0, m->lm_out);
+}
+
+int get_graph(pcamm_model* m, int B, int C, GraphRec** out) {
+    const long long key = (long long)B * 1024 + C;
+    auto it = m->graphs.find(key);
+    if (it != m->graphs.end()) { *out = &it->second; return PCAMM_OK; }
+    GraphRec rec;
+    CUDA_TRY(cudaGraphCreate(&rec.graph, 0));
+    cudaGraphConditionalHandle h_iter, h_trial;
+    CUDA_TRY(cudaGraphConditionalHandleCreate(&h_iter, rec.graph, 0, cudaGraphCondAssignDefault));
+    CUDA_TRY(cudaGraphConditionalHandleCreate(&h_trial, rec.graph, 0, cudaGraphCondAssignDefault));
+    Seq q;
+    q.graph = rec.graph;
+    seq_head(m, q, B, C, h_iter, 1);
+    Seq it_body = q.add_while(h_iter);          // iterations n = 0 ..
+    seq_grad(m, it_body, B, h_trial, 1);
+    Seq tr_body = it_body.add_while(h_trial);   // Armijo backtracking (Eq. 3)
+    seq_trial(m, tr_body, B, C, h_trial, 1);
+    launch_ctl_iter_end(it_body, m->c, h_iter, 1);
+    seq_tail(m, q, B);
+    int rc;
+    if ((rc = check_seq(q, "graph build")) || (rc = check_seq(it_body, "graph build (iteration body)")) ||
+        (rc = check_seq(tr_body, "graph build (trial body)"))) {
+        cudaGraphDestroy(rec.graph);
+        return rc;
+    }
+    cudaError_t e = cudaGraphInstantiate(&rec.exec, rec.graph, 0);
+    if (e != cudaSuccess) {
+        set_error(std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
+        cudaGraphDestroy(rec.graph);
+        return PCAMM_E_CUDA;
+    }
+    m->graphs[key] = rec;
+    *out = &m->graphs[key];
+    return PCAMM_OK;
+}
+
+int read_flags(pcamm_model* m, cudaStream_t st) {
+    CUDA_TRY(cudaMemcpyAsync(m->h_flags, m->c.flags, sizeof(LoopFlags), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return PCAMM_OK;
+}
+
+int run_host_loop(pcamm_model* m, int B, int C, cudaStream_t st) {
+    Seq q;
+    q.stream = st;
+    int rc;
+    seq_head(m, q, B, C, 0, 0);
+    if ((rc = check_seq(q, "solve head")) || (rc = read_flags(m, st))) return rc;
+    while (m->h_flags->iter_cond) {
+        seq_grad(m, q, B, 0, 0);
+        if ((rc = check_seq(q, "gradient step")) || (rc = read_flags(m, st))) return rc;
+        while (m->h_flags->trial_cond) {
+            seq_trial(m, q, B, C, 0, 0);
+            if ((rc = check_seq(q, "trial step")) || (rc = read_flags(m, st))) return rc;
+        }
+    }
+    seq_tail(m, q, B);
+    return check_seq(q, "solve tail");
+}
+
+int solve_impl(pcamm_model* m, int B, const float* y_dev, const float* angles, const float* w_init,
+               const pcamm_opts* user_opts, float* w_out, float* volumes_out, float* lm_out, pcamm_info* info,
+               cudaStream_t st) {
+    if (!m) return invalid("model is NULL");
+    if (B < 1 || B > m->Bmax) return invalid("B outside [1, geometry.max_batch]");
+    if (!y_dev || !angles || !w_init || !w_out) return invalid("NULL argument");
+    pcamm_opts o;
+    int rc = resolve_opts(m, user_opts, &o);
+    if (rc) return rc;
+    const Geom& G = m->G;
+    const int C = o.batched_linesearch ? o.max_backtracks : 1;
+    fill_call(m, o, B, C);
+    SolveIn* in = h_solve_in(m);
+    for (int b = 0; b < B; ++b) {
+        in[b].y = y_dev + (size_t)b * G.npix;
+        in[b].angle = angles[b];
+        if (!std::isfinite(angles[b])) return invalid("angle is not finite");
+        for (int k = 0; k < KMAX; ++k) in[b].w_init[k] = k < G.K ? w_init[b * G.K + k] : 0.f;
+        for (int k = 0; k < G.K; ++k)
+            if (!std::isfinite(w_init[b * G.K + k])) { set_error("w_init is not finite"); return PCAMM_E_NONFINITE; }
+        in[b].a = in[b].b = 0.f;
+    }
+    if ((rc = push_call(m, B, st))) return rc;
+    if (o.loop_mode == 0) {
+        GraphRec* g = nullptr;
+        if ((rc = get_graph(m, B, C, &g))) return rc;
+        CUDA_TRY(cudaGraphLaunch(g->exec, st));
+    } else {
+        if ((rc = run_host_loop(m, B, C, st))) return rc;
+    }
+    if (volumes_out) {
+        Seq q;
+        q.stream = st;
+        launch_warp(q, G, m->f0, m->xbar, m->u, m->out_slots, m->c.solves, B, 1, volumes_out, nullptr, G.V);
+        if ((rc = check_seq(q, "final warp"))) return rc;
+    }
+    CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState) * B, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(m->h_flags, m->c.flags, sizeof(LoopFlags), cudaMemcpyDeviceToHost, st));
+    if (lm_out && m->M > 0)
+        CUDA_TRY(cudaMemcpyAsync(m->h_lm, m->lm_out, sizeof(double) * 3 * m->M * B, cudaMemcpyDeviceToHost, st));
+    bool want_trace = false;
+    if (info)
+        for (int b = 0; b < B; ++b)
+            want_trace |= info[b].J_trace || info[b].gnorm_trace || info[b].mu_trace || info[b].backtracks_trace;
+    if (want_trace)
+        CUDA_TRY(cudaMemcpyAsync(m->h_traces, m->c.traces, sizeof(SolveTrace) * B, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (o.loop_mode == 0) count_launch(m->h_flags->n_launch);
+    int first_err = 0;
+    for (int b = 0; b < B; ++b) {
+        const SolveState& s = m->h_solves[b];
+        for (int k = 0; k < G.K; ++k) w_out[b * G.K + k] = (float)s.w[k];
+        if (s.status < 0 && !first_err) {
+            first_err = s.status;
+            set_error(s.status == PCAMM_E_SINGULAR ? "intensity fit singular: y is constant"
+                                                   : "non-finite value in y or in the gradient");
+        }
+        if (info) {
+            pcamm_info& I = info[b];
+            I.iters = s.iter; I.status = s.status; I.J0 = s.J0; I.J = s.J; I.a = s.a; I.b = s.b;
+            const SolveTrace& t = m->h_traces[b];
+            const int n = s.iter < TRACE_CAP ? s.iter : TRACE_CAP;
+            const int ng = (s.status == PCAMM_S_GRADTOL || s.status == PCAMM_S_LINESEARCH) && n < TRACE_CAP ? n + 1 : n;
+            if (I.J_trace) std::memcpy(I.J_trace, t.J, sizeof(double) * (n + 1));
+            if (I.gnorm_trace) std::memcpy(I.gnorm_trace, t.gnorm, sizeof(double) * (ng < o.max_iter ? ng : o.max_iter));
+            if (I.mu_trace) std::memcpy(I.mu_trace, t.mu, sizeof(double) * n);
+            if (I.backtracks_trace) std::memcpy(I.backtracks_trace, t.bt, sizeof(int) * n);
+        }
+    }
+    if (lm_out)
+        for (int i = 0; i < 3 * m->M * B; ++i) lm_out[i] = (float)m->h_lm[i];
+    if (first_err) return first_err;
+    return B == 1 ? m->h_solves[0].status : PCAMM_OK;
+}
+
+// Common start of the hooks: one solve slot, view from `angle`, w into slot 0.
+int hook_begin(pcamm_model* m, const float* y_dev, float angle, const float* w, float a, float b, int mode,
+               cudaStream_t st, Seq& q) {
+    pcamm_opts o;
+    pcamm_default_opts(&o);
+    fill_call(m, o, 1, 1);
+    SolveIn* in = h_solve_in(m);
+    in[0].y = y_dev;
+    in[0].angle = angle;
+    for (int k = 0; k < KMAX; ++k) in[0].w_init[k] = (w && k < m->G.K) ? w[k] : 0.f;
+    in[0].a = a; in[0].b = b;
+    int rc = push_call(m, 1, st);
+    if (rc) return rc;
+    q.stream = st;
+    launch_begin(q, m->G, m->c, mode);
+    return check_seq(q, "begin");
+}
+
+}  // namespace
+
+extern "C" {
+
+void pcamm_default_opts(pcamm_opts* o) {
+    if (!o) return;
+    o->max_iter = 10;
+    o->grad_tol = 0.f;
+    o->armijo_c = 1e-4f;
+    o->armijo_beta = 0.5f;
+    o->max_backtracks = 8;
+    o->init_step_vox = 1.f;
+    o->batched_linesearch = 0;
+    o->inv_max_iter = 50;
+    o->inv_tol_mm = 1e-4f;
+    o->loop_mode = 0;
+}
+
+const char* pcamm_last_error(void) { return g_error.c_str(); }
+
+int64_t pcamm_launch_count(int32_t reset) {
+    const long long n = g_launches;
+    if (reset) g_launches = 0;
+    return n;
+}
+
+void pcamm_model_destroy(pcamm_model* m) {
+    if (!m) return;
+    for (auto& kv : m->graphs) {
+        if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
+        if (kv.second.graph) cudaGraphDestroy(kv.second.graph);
+    }
+    if (m->ev0) cudaEventDestroy(m->ev0);
+    if (m->ev1) cudaEventDestroy(m->ev1);
+    for (void* p : m->dev_allocs) cudaFree(p);
+    for (void* p : m->host_allocs) cudaFreeHost(p);
+    delete m;
+}
+
+int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float* mean_dvf_dev, const float* eig_dvf_dev,
+                       int32_t n_landmarks, const float* landmarks_mm_host, void* stream, pcamm_model** out) {
+    if (out) *out = nullptr;
+    if (!g || !f0_dev || !mean_dvf_dev || !eig_dvf_dev || !out) return invalid("NULL argument");
+    if (g->nx < 1 || g->ny < 1 || g->nz < 1 || g->nu < 1 || g->nv < 1) return invalid("sizes must be positive");
+    if (!(g->hx > 0 && g->hy > 0 && g->hz > 0 && g->pu > 0 && g->pv > 0)) return invalid("voxel / pixel sizes must be positive");
+    if (g->K < 1 || g->K > KMAX) return invalid("K outside [1, PCAMM_KMAX]");
+    if (n_landmarks < 0 || (n_landmarks > 0 && !landmarks_mm_host)) return invalid("landmarks");
+    const long long V = (long long)g->nx * g->ny * g->nz;
+    if (V >= (1LL << 31) || (long long)g->nu * g->nv >= (1LL << 31)) return invalid("volume or detector too large");
+    const int Bmax = g->max_batch < 1 ? 1 : g->max_batch;
+    const int Cmax = g->max_candidates < 1 ? 1 : g->max_candidates;
+    if (Cmax > MAXBT || Bmax > 4096) return invalid("max_batch / max_candidates too large");
+    if (!(g->sad > 0 && g->sdd > g->sad)) return invalid("need 0 < sad < sdd");
+    // source and detector plane outside the volume's bounding sphere about the isocentre
+    const double ex = 0.5 * g->nx * (double)g->hx, ey = 0.5 * g->ny * (double)g->hy, ez = 0.5 * g->nz * (double)g->hz;
+    const double R = std::sqrt((double)g->cx * g->cx + (double)g->cy * g->cy + (double)g->cz * g->cz) +
+                     std::sqrt(ex * ex + ey * ey + ez * ez);
+    if (!(R < 0.999 * g->sad && R < 0.999 * ((double)g->sdd - g->sad)))
+        return invalid("source or detector inside the volume's bounding sphere");
+    // at most one voxel in z per voxel along the dominant in-plane axis
+    const double vmax = (0.5 * (g->nv - 1) + std::fabs((double)g->off_v)) * g->pv;
+    if (!(vmax / g->hz <= (double)g->sdd / std::sqrt((double)g->hx * g->hx + (double)g->hy * g->hy)))
+        return invalid("cone angle too steep for the voxel aspect ratio (z-slope > 1 voxel per slab)");
+
+    pcamm_model* m = new (std::nothrow) pcamm_model();
+    if (!m) { set_error("out of host memory"); return PCAMM_E_NOMEM; }
+    m->geo = *g;
+    m->M = n_landmarks; m->Bmax = Bmax; m->Cmax = Cmax; m->S = Bmax * Cmax;
+    Geom& G = m->G;
+    G.nx = g->nx; G.ny = g->ny; G.nz = g->nz; G.V = V;
+    G.hx = g->hx; G.hy = g->hy; G.hz = g->hz;
+    G.ihx = 1.f / g->hx; G.ihy = 1.f / g->hy; G.ihz = 1.f / g->hz;
+    G.cx = g->cx; G.cy = g->cy; G.cz = g->cz;
+    G.lox = (double)g->cx - ex; G.loy = (double)g->cy - ey; G.loz = (double)g->cz - ez;
+    G.K = g->K; G.nu = g->nu; G.nv = g->nv; G.npix = g->nu * g->nv;
+    G.pu = g->pu; G.pv = g->pv; G.sad = g->sad; G.sdd = g->sdd; G.off_u = g->off_u; G.off_v = g->off_v;
+
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t S = (size_t)m->S, B = (size_t)Bmax;
+    m->in_off = (sizeof(CallOpts) + 63) / 64 * 64;
+    m->in_block_bytes = m->in_off + sizeof(SolveIn) * B;
+    m->c.ysum_blocks = ysum_blocks(G);
+    m->c.proj_blocks = project_blocks(G);
+    m->c.resid_blocks = resid_blocks(G);
+    m->c.grad_blocks = grad_blocks(G);
+    m->trav_cap = G.nx + G.ny + G.nz + 8;
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return r == cudaSuccess; };
+    ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->xbar, 3 * (size_t)V)) &&
+        ok(dalloc(m, &m->u, 3 * (size_t)V * G.K)) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
+        ok(dalloc(m, &m->vol_std, S * V)) && ok(dalloc(m, &m->vol_tr, S * V)) && ok(dalloc(m, &m->p, S * G.npix)) &&
+        ok(dalloc(m, &m->rL, B * G.npix)) && ok(dalloc(m, &m->utab, B * G.nu)) && ok(dalloc(m, &m->vtab, B * G.nv)) &&
+        ok(dalloc(m, &m->in_block, m->in_block_bytes)) && ok(dalloc(m, &m->c.solves, B)) &&
+        ok(dalloc(m, &m->c.traces, B)) && ok(dalloc(m, &m->c.slots, S)) && ok(dalloc(m, &m->c.flags, 1)) &&
+        ok(dalloc(m, &m->c.ysum_part, B * m->c.ysum_blocks * 2)) &&
+        ok(dalloc(m, &m->c.proj_part, S * m->c.proj_blocks * 3)) &&
+        ok(dalloc(m, &m->c.resid_part, B * m->c.resid_blocks)) &&
+        ok(dalloc(m, &m->c.grad_part, B * m->c.grad_blocks * KMAX)) && ok(dalloc(m, &m->out_slots, B)) &&
+        ok(dalloc(m, &m->lm_out, 3 * B * (size_t)(m->M > 0 ? m->M : 1))) &&
+        ok(dalloc(m, &m->trav_ijk, 3 * (size_t)m->trav_cap)) && ok(dalloc(m, &m->trav_len, (size_t)m->trav_cap)) &&
+        ok(dalloc(m, &m->trav_n, 1)) && ok(dalloc(m, &m->nonfinite, 1)) && ok(dalloc(m, &m->y_stage, (size_t)G.npix)) &&
+        ok(halloc(m, &m->h_in, m->in_block_bytes)) && ok(halloc(m, &m->h_solves, B)) &&
+        ok(halloc(m, &m->h_traces, B)) && ok(halloc(m, &m->h_flags, 1)) &&
+        ok(halloc(m, &m->h_lm, 3 * B * (size_t)(m->M > 0 ? m->M : 1))) &&
+        ok(halloc(m, &m->h_trav, 4 * (size_t)m->trav_cap + 4)) &&
+        ok(cudaEventCreate(&m->ev0)) && ok(cudaEventCreate(&m->ev1));
+    if (e != cudaSuccess) {
+        set_error(std::string("allocation failed: ") + cudaGetErrorString(e));
+        cudaGetLastError();
+        pcamm_model_destroy(m);
+        return e == cudaErrorMemoryAllocation ? PCAMM_E_NOMEM : PCAMM_E_CUDA;
+    }
+    m->c.opts = (CallOpts*)m->in_block;
+    m->c.in = (SolveIn*)(m->in_block + m->in_off);
+    std::memset(m->h_in, 0, m->in_block_bytes);
+
+    auto fail = [&](int rc) { pcamm_model_destroy(m); return rc; };
+#define TRY_OR_FAIL(expr)                                                                       \
+    do {                                                                                        \
+        cudaError_t e_ = (expr);                                                                \
+        if (e_ != cudaSuccess) {                                                                \
+            set_error(std::string(#expr) + ": " + cudaGetErrorString(e_));                      \
+            return fail(PCAMM_E_CUDA);                                                          \
+        }                                                                                       \
+    } while (0)
+    TRY_OR_FAIL(cudaMemcpyAsync(m->f0, f0_dev, sizeof(float) * V, cudaMemcpyDeviceToDevice, st));
+    TRY_OR_FAIL(cudaMemcpyAsync(m->xbar, mean_dvf_dev, sizeof(float) * 3 * V, cudaMemcpyDeviceToDevice, st));
+    TRY_OR_FAIL(cudaMemcpyAsync(m->u, eig_dvf_dev, sizeof(float) * 3 * V * G.K, cudaMemcpyDeviceToDevice, st));
+    if (m->M > 0)
+        TRY_OR_FAIL(cudaMemcpyAsync(m->lm0, landmarks_mm_host, sizeof(float) * 3 * m->M, cudaMemcpyHostToDevice, st));
+    TRY_OR_FAIL(cudaMemsetAsync(m->nonfinite, 0, sizeof(unsigned long long), st));
+    TRY_OR_FAIL(cudaMemsetAsync(m->c.solves, 0, sizeof(SolveState) * B, st));
+    TRY_OR_FAIL(cudaMemsetAsync(m->c.slots, 0, sizeof(SlotState) * S, st));
+    TRY_OR_FAIL(cudaMemsetAsync(m->c.flags, 0, sizeof(LoopFlags), st));
+    k_count_nonfinite<<<592, 256, 0, st>>>(m->f0, V, m->nonfinite);
+    k_count_nonfinite<<<592, 256, 0, st>>>(m->xbar, 3 * V, m->nonfinite);
+    k_count_nonfinite<<<592, 256, 0, st>>>(m->u, 3 * V * G.K, m->nonfinite);
+    unsigned long long bad = 0;
+    TRY_OR_FAIL(cudaMemcpyAsync(&bad, m->nonfinite, sizeof(bad), cudaMemcpyDeviceToHost, st));
+    TRY_OR_FAIL(cudaStreamSynchronize(st));
+#undef TRY_OR_FAIL
+    if (m->M > 0)
+        for (int i = 0; i < 3 * m->M; ++i)
+            if (!std::isfinite(landmarks_mm_host[i])) bad++;
+    if (bad) {
+        set_error("non-finite value in f0, the DVF fields or the landmarks");
+        return fail(PCAMM_E_NONFINITE);
+    }
+    *out = m;
+    return PCAMM_OK;
+}
+
+int pcamm_reconstruct_batch(pcamm_model* m, int32_t B, const float* y_dev, const float* angles_rad_host,
+                            const float* w_init_host, const pcamm_opts* opts, float* w_out_host, float* volumes_out_dev,
+                            float* landmarks_out_host, pcamm_info* info, void* stream) {
+    const int rc = solve_impl(m, B, y_dev, angles_rad_host, w_init_host, opts, w_out_host, volumes_out_dev,
+                              landmarks_out_host, info, (cudaStream_t)stream);
+    return (B == 1 && rc > 0) ? PCAMM_OK : rc;
+}
+
+int pcamm_reconstruct(pcamm_model* m, const float* y_dev, float angle_rad, const float* w_init_host,
+                      const pcamm_opts* opts, float* w_out_host, float* volume_out_dev, float* landmarks_out_host,
+                      pcamm_info* info, void* stream) {
+    return solve_impl(m, 1, y_dev, &angle_rad, w_init_host, opts, w_out_host, volume_out_dev, landmarks_out_host, info,
+                      (cudaStream_t)stream);
+}
+
+int pcamm_reconstruct_host(pcamm_model* m, const float* y_host, float angle_rad, const float* w_init_host,
+                           const pcamm_opts* opts, float* w_out_host, float* volume_out_dev, float* landmarks_out_host,
+                           pcamm_info* info, void* stream) {
+    if (!m || !y_host) return invalid("NULL argument");
+    float* y_stage = m->y_stage;
+    CUDA_TRY(cudaMemcpyAsync(y_stage, y_host, (size_t)m->G.npix * sizeof(float), cudaMemcpyHostToDevice,
+                             (cudaStream_t)stream));
+    return solve_impl(m, 1, y_stage, &angle_rad, w_init_host, opts, w_out_host, volume_out_dev, landmarks_out_host, info,
+                      (cudaStream_t)stream);
+}
+
+int pcamm_warp(pcamm_model* m, const float* w_host, float* volume_out_dev, void* stream) {
+    if (!m || !w_host || !volume_out_dev) return invalid("NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    Seq q;
+    int rc = hook_begin(m, nullptr, 0.f, w_host, 0.f, 0.f, 2, st, q);
+    if (rc) return rc;
+    launch_warp(q, m->G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, 1, 1, volume_out_dev, nullptr, m->G.V);
+    if ((rc = check_seq(q, "warp"))) return rc;
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return PCAMM_OK;
+}
+
+int pcamm_project(pcamm_model* m, const float* volume_dev, float angle_rad, float* proj_out_dev, void* stream) {
+    if (!m || !volume_dev || !proj_out_dev) return invalid("NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    Seq q;
+    int rc = hook_begin(m, nullptr, angle_rad, nullptr, 0.f, 0.f, 2, st, q);
+    if (rc) return rc;
+    launch_transpose(q, m->G, volume_dev, m->vol_tr);
+    launch_project(q, m->G, m->c.slots, m->c.solves, m->c.in, 1, volume_dev, m->vol_tr, m->G.V, m->p, m->c.proj_part);
+    if ((rc = check_seq(q, "project"))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * m->G.npix, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return PCAMM_OK;
+}
+
+int pcamm_backproject(pcamm_model* m, const float* r_dev, float angle_rad, float* volume_out_dev, void* stream) {
+    if (!m || !r_dev || !volume_out_dev) return invalid("NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    Seq q;
+    int rc = hook_begin(m, nullptr, angle_rad, nullptr, 0.f, 0.f, 2, st, q);
+    if (rc) return rc;
+    launch_resid(q, m->G, m->c.solves, m->c.in, 1, 1, m->p, r_dev, m->rL, m->utab, m->vtab, m->c.resid_part);
+    launch_backproject(q, m->G, m->c.solves, m->rL, m->utab, m->vtab, volume_out_dev);
+    if ((rc = check_seq(q, "backproject"))) return rc;
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return PCAMM_OK;
+}
+
+int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float* w_host, float a, float b, double* J_out,
+               double* grad_out, double* ab_fit_out, float* proj_out_dev, void* stream) {
+    if (!m || !y_dev || !w_host) return invalid("NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom& G = m->G;
+    Seq q2;
+    int rc = hook_begin(m, y_dev, angle_rad, w_host, a, b, 1, st, q2);
+    if (rc) return rc;
+    launch_ysums(q2, G, m->c, 1);
+    launch_warp(q2, G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, 1, 0, m->vol_std, m->vol_tr, G.V);
+    launch_project(q2, G, m->c.slots, m->c.solves, m->c.in, 1, m->vol_std, m->vol_tr, G.V, m->p, m->c.proj_part);
+    launch_ctl_eval(q2, G, m->c, 0);
+    launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
+    launch_grad(q2, G, m->f0, m->xbar, m->u, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
+    launch_ctl_eval(q2, G, m->c, 1);
+    if ((rc = check_seq(q2, "eval"))) return rc;
+    if (proj_out_dev) CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * G.npix, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    const SolveState& s = m->h_solves[0];
+    if (J_out) *J_out = s.J;
+    if (grad_out) for (int k = 0; k < G.K; ++k) grad_out[k] = s.g[k];
+    if (ab_fit_out) { ab_fit_out[0] = s.fit_a; ab_fit_out[1] = s.fit_b; }
+    return PCAMM_OK;
+}
+
+int pcamm_traverse(pcamm_model* m, float angle_rad, int32_t iu, int32_t iv, int32_t cap, int32_t* ijk_out_host,
+                   float* len_out_host, int32_t* n_out, void* stream) {
+    if (!m || !ijk_out_host || !len_out_host || !n_out) return invalid("NULL argument");
+    if (iu < 0 || iu >= m->G.nu || iv < 0 || iv >= m->G.nv || cap < 0) return invalid("pixel outside the detector");
+    cudaStream_t st = (cudaStream_t)stream;
+    Seq q;
+    int rc = hook_begin(m, nullptr, angle_rad, nullptr, 0.f, 0.f, 2, st, q);
+    if (rc) return rc;
+    const int dcap = cap < m->trav_cap ? cap : m->trav_cap;
+    launch_traverse(q, m->G, m->c.solves, iu, iv, dcap, m->trav_ijk, m->trav_len, m->trav_n);
+    if ((rc = check_seq(q, "traverse"))) return rc;
+    int* h = m->h_trav;
+    CUDA_TRY(cudaMemcpyAsync(h, m->trav_n, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(h + 1, m->trav_ijk, sizeof(int) * 3 * dcap, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(h + 1 + 3 * m->trav_cap, m->trav_len, sizeof(float) * dcap, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    const int n = h[0];
+    *n_out = n;
+    const int ncopy = n < dcap ? n : dcap;
+    std::memcpy(ijk_out_host, h + 1, sizeof(int) * 3 * ncopy);
+    std::memcpy(len_out_host, h + 1 + 3 * m->trav_cap, sizeof(float) * ncopy);
+    if (n > cap) return invalid("cap too small for this ray");
+    return PCAMM_OK;
+}
+
+int pcamm_localise(pcamm_model* m, const float* w_host, int32_t inv_max_iter, float inv_tol_mm, float* landmarks_out_host,
+                   void* stream) {
+    if (!m || !w_host || !landmarks_out_host) return invalid("NULL argument");
+    if (m->M <= 0) return PCAMM_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    pcamm_opts o;
+    pcamm_default_opts(&o);
+    o.inv_max_iter = inv_max_iter; o.inv_tol_mm = inv_tol_mm;
+    fill_call(m, o, 1, 1);
+    SolveIn* in = h_solve_in(m);
+    in[0].y = nullptr; in[0].angle = 0.f; in[0].a = in[0].b = 0.f;
+    for (int k = 0; k < KMAX; ++k) in[0].w_init[k] = k < m->G.K ? w_host[k] : 0.f;
+    int rc = push_call(m, 1, st);
+    if (rc) return rc;
+    Seq q;
+    q.stream = st;
+    launch_begin(q, m->G, m->c, 2);
+    launch_invert(q, m->G, m->xbar, m->u, m->c, 1, m->M, m->lm0, m->lm_out);
+    if ((rc = check_seq(q, "localise"))) return rc;
+    CUDA_TRY(cudaMemcpyAsync(m->h_lm, m->lm_out, sizeof(double) * 3 * m->M, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    for (int i = 0; i < 3 * m->M; ++i) landmarks_out_host[i] = (float)m->h_lm[i];
+    return PCAMM_OK;
+}
+
+int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out, void* stream) {
+    if (!m || !ms_out || reps < 1 || which < 0 || which > 2) return invalid("invalid argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom& G = m->G;
+    Seq q;
+    q.stream = st;
+    CUDA_TRY(cudaEventRecord(m->ev0, st));
+    for (int i = 0; i < reps; ++i) {
+        if (which == 0)
+            launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, 1, 0, m->vol_std, m->vol_tr, G.V);
+        else if (which == 1)
+            launch_project(q, G, m->c.slots, m->c.solves, m->c.in, 1, m->vol_std, m->vol_tr, G.V, m->p, m->c.proj_part);
+        else
+            launch_grad(q, G, m->f0, m->xbar, m->u, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
+    }
+    CUDA_TRY(cudaEventRecord(m->ev1, st));
+    int rc = check_seq(q, "time_kernel");
+    if (rc) return rc;
+    CUDA_TRY(cudaEventSynchronize(m->ev1));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, m->ev0, m->ev1));
+    *ms_out = ms / (float)reps;
+    return PCAMM_OK;
+}
+
+}  // extern "C"

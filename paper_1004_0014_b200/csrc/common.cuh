@@ -1,0 +1,115 @@
+// Shared device structs and helpers of the CUDA path.  No code here is shared with oracle/.
+//
+// Notation follows the paper (section 2): f0 reference volume, xbar mean DVF, u_k
+// eigenvector fields, w PCA coefficients, y measured projection, P_theta projector, (a, b)
+// intensity fit, J cost, g = dJ/dw, mu step size.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/pcamm.h"
+
+namespace pcamm {
+
+constexpr int KMAX = PCAMM_KMAX;
+constexpr int MAXBT = PCAMM_MAX_BACKTRACKS;
+constexpr int TRACE_CAP = 1024;  // iterations recorded in the device-side traces
+
+// Model-constant geometry (passed to kernels by value).
+struct Geom {
+    int nx, ny, nz;
+    long long V;
+    float hx, hy, hz;
+    float ihx, ihy, ihz;      // 1 / h
+    float cx, cy, cz;         // world position of the volume centre
+    double lox, loy, loz;     // world position of the volume's low corner
+    int K;
+    int nu, nv, npix;
+    float pu, pv, sad, sdd, off_u, off_v;
+};
+
+// Angle-dependent part of the geometry of one solve, computed on the device in double.
+// layout bit 0: some ray of this view marches along y and reads the standard volume [z][y][x];
+// layout bit 1: some ray marches along x and reads the in-plane transposed volume [z][x][y].
+struct View {
+    double cs, sn;
+    int layout;
+    int pad;
+};
+
+// Host -> device, one copy per call.
+struct CallOpts {
+    int B, C;                 // solves in flight, candidate steps evaluated per trial round
+    int max_iter, max_backtracks, batched, inv_max_iter;
+    double grad_tol, armijo_c, armijo_beta, init_step_vox, inv_tol;
+    double hmin_sqrtV;        // min(h) * sqrt(V): the 1-voxel-rms step scale (reading A7)
+};
+
+struct SolveIn {
+    const float* y;           // measured projection of this solve (device)
+    float angle;
+    float w_init[KMAX];
+    float a, b;               // used by the pcamm_eval hook only
+};
+
+struct SolveState {
+    View view;
+    double w[KMAX], g[KMAX];
+    double a, b, Sy, Syy;
+    double Jn, J0, J, g2, mu, mu_prev;
+    double fit_a, fit_b;      // pcamm_eval hook: least-squares (a, b) for the evaluated p
+    int iter, status, running, trialing, t, acc_slot;
+};
+
+struct SolveTrace {
+    double J[TRACE_CAP + 1], gnorm[TRACE_CAP], mu[TRACE_CAP];
+    int bt[TRACE_CAP];
+};
+
+// One trial evaluation: candidate c of solve b, slot s = b * C + c.
+struct SlotState {
+    float w[KMAX];
+    int active, solve;
+    double mu, J, Sp, Syp;
+};
+
+// Loop conditions mirrored to plain memory so that the host-driven mode can read them.
+struct LoopFlags {
+    int iter_cond, trial_cond;
+    long long n_launch;
+};
+
+// In-plane direction D - S of the rays of detector column iu (independent of the row).
+__device__ __forceinline__ void ray_dir_inplane(const Geom& G, double cs, double sn, int iu, double* dx, double* dy) {
+    const double uu = ((double)iu - 0.5 * (G.nu - 1) + (double)G.off_u) * (double)G.pu;
+    *dx = -(double)G.sdd * cs - uu * sn;
+    *dy = -(double)G.sdd * sn + uu * cs;
+}
+
+// ---------------------------------------------------------------- reductions
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Sum over a block of NT threads (NT multiple of 32, <= 1024); result valid in thread 0.
+// Fixed order: lanes by butterfly, warps in index order -> deterministic.
+template <int NT>
+__device__ __forceinline__ double block_sum(double v, double* smem /* [NT/32] */) {
+    v = warp_sum(v);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();  // protect smem reuse between successive calls
+    if (lane == 0) smem[wid] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int i = 0; i < NT / 32; ++i) s += smem[i];
+    }
+    return s;
+}
+
+}  // namespace pcamm

@@ -1,0 +1,283 @@
+// a-3 (residual) and a-4: dJ/dw = 2 U^T (df/dx) P^T (P f - a y - b 1).
+//
+// The chain is evaluated voxel by voxel in one pass over the K+1 vector fields, and no
+// volume-sized gradient is ever written:
+//
+//   B_j  = sum_i l_ij r_i          backprojection of the residual, gathered by the voxel: the exact
+//                                  length of every ray through voxel box j (the same l_ij as the
+//                                  projector: reading A4), times r_i
+//   G_j  = df_j / dx_j             exact derivative of the trilinear interpolant (PAPER.md:L95:
+//                                  "has to be consistent with the interpolation process"; A6)
+//   g_k  = 2 sum_j B_j (G_j . u_kj)
+//
+// df/dx is block diagonal (voxel j's value depends on x_j only; reading A5), which is what allows
+// the fusion.  Voxels whose eight taps make G_j = 0 skip the gather (their term is exactly 0).
+//
+// The gather uses the separable form of the ray/box intersection in the parameter alpha of
+// S + alpha (D - S) with D on the flat detector: the in-plane slabs give an alpha-interval that
+// depends on the detector column only, the z-slab one that depends on the row only, and
+// l_ij = |D - S| * |intersection of the two|.  Per view, k_resid tabulates (d_x, d_y, 1/d_x,
+// 1/d_y) per column, (d_z, 1/d_z) per row and rL_i = r_i |D_i - S| per pixel.
+#include "internal.h"
+
+namespace pcamm {
+
+namespace {
+
+constexpr int RT = 256;         // k_resid threads
+constexpr int TILE = 32, ROWS = 4, GT = 256;
+constexpr float PAR_INV = 1e30f; // 1/d for a ray parallel to a slab: [0, +big) or (-big, 0] keeps
+                                 // the half-open inside test of reading A21
+
+// r = p - a y - b (Eq. 2), rL = r |D - S|; tables of this view; partial sums of r^2.
+// r_direct != NULL: r is taken from there (pcamm_backproject hook).  force: also for solves that
+// have stopped (closing pass of a solve).
+__global__ void __launch_bounds__(RT)
+k_resid(const Geom G, const SolveState* __restrict__ solves, const SolveIn* __restrict__ in,
+        int force, const float* __restrict__ p_slots, const float* __restrict__ r_direct, float* __restrict__ rL,
+        float4* __restrict__ utab, float2* __restrict__ vtab, double* __restrict__ partials) {
+    __shared__ double red[RT / 32];
+    const int b = blockIdx.y;
+    const SolveState& st = solves[b];
+    if (!st.running && !force) return;
+    const View vw = st.view;
+    const int pix = blockIdx.x * RT + threadIdx.x;
+    double rr = 0.0;
+    if (pix < G.npix) {
+        const int iu = pix % G.nu, iv = pix / G.nu;
+        const double uu = ((double)iu - 0.5 * (G.nu - 1) + (double)G.off_u) * (double)G.pu;
+        const double vv = ((double)iv - 0.5 * (G.nv - 1) + (double)G.off_v) * (double)G.pv;
+        const double L = sqrt((double)G.sdd * (double)G.sdd + uu * uu + vv * vv);
+        double r;
+        if (r_direct) r = (double)__ldg(r_direct + pix);
+        else {
+            const float* y = in[b].y;
+            const double pv = (double)__ldg(p_slots + (long long)st.acc_slot * G.npix + pix);
+            r = pv - st.a * (y ? (double)__ldg(y + pix) : 0.0) - st.b;
+        }
+        rr = r * r;
+        rL[(long long)b * G.npix + pix] = (float)(r * L);
+        if (pix < G.nu) {
+            double dx, dy;
+            ray_dir_inplane(G, vw.cs, vw.sn, pix, &dx, &dy);
+            utab[(long long)b * G.nu + pix] = make_float4((float)dx, (float)dy, dx != 0.0 ? (float)(1.0 / dx) : PAR_INV,
+                                                          dy != 0.0 ? (float)(1.0 / dy) : PAR_INV);
+        }
+        if (pix < G.nv) {
+            const double vz = ((double)pix - 0.5 * (G.nv - 1) + (double)G.off_v) * (double)G.pv;
+            vtab[(long long)b * G.nv + pix] = make_float2((float)vz, vz != 0.0 ? (float)(1.0 / vz) : PAR_INV);
+        }
+    }
+    const double s = block_sum<RT>(rr, red);
+    if (threadIdx.x == 0) partials[(long long)b * gridDim.x + blockIdx.x] = s;
+}
+
+// Per-view constants of the gather, in float.
+struct GatherView {
+    float cs, sn, Sx, Sy;     // source position (in-plane); S_z = 0
+    float Wt, Wd;             // half extent of a voxel box across / along the central ray
+    float sdd_ipu, sdd_ipv;   // sdd / pitch
+    float cu, cv;             // pixel index of the detector origin
+};
+
+__device__ __forceinline__ GatherView make_gather_view(const Geom& G, const View& vw) {
+    GatherView g;
+    g.cs = (float)vw.cs; g.sn = (float)vw.sn;
+    g.Sx = (float)((double)G.sad * vw.cs); g.Sy = (float)((double)G.sad * vw.sn);
+    g.Wt = 0.5f * (G.hx * fabsf(g.sn) + G.hy * fabsf(g.cs));
+    g.Wd = 0.5f * (G.hx * fabsf(g.cs) + G.hy * fabsf(g.sn));
+    g.sdd_ipu = G.sdd / G.pu; g.sdd_ipv = G.sdd / G.pv;
+    g.cu = 0.5f * (G.nu - 1) - G.off_u; g.cv = 0.5f * (G.nv - 1) - G.off_v;
+    return g;
+}
+
+// B_j = sum_i l_ij r_i for the voxel centred at (xw, yw, zw) mm.
+__device__ __forceinline__ float gather_voxel(const Geom& G, const GatherView& gv, const float* __restrict__ rL,
+                                              const float4* __restrict__ utab, const float2* __restrict__ vtab,
+                                              float xw, float yw, float zw) {
+    const float ex = xw - gv.Sx, ey = yw - gv.Sy, ez = zw;             // voxel centre - source
+    const float depth = -(ex * gv.cs + ey * gv.sn);                     // along the central ray
+    const float t = ey * gv.cs - ex * gv.sn;                            // along u^
+    // detector bounding rectangle of the box's shadow (perspective projection of a convex body:
+    // extremes of t/depth and z/depth over the box are bounded by these four quotients)
+    const float i1 = 1.f / (depth - gv.Wd), i2 = 1.f / (depth + gv.Wd);
+    const float tl = t - gv.Wt, th = t + gv.Wt, zl = ez - 0.5f * G.hz, zh = ez + 0.5f * G.hz;
+    const float ulo = fminf(tl * i1, tl * i2) * gv.sdd_ipu + gv.cu, uhi = fmaxf(th * i1, th * i2) * gv.sdd_ipu + gv.cu;
+    const float vlo = fminf(zl * i1, zl * i2) * gv.sdd_ipv + gv.cv, vhi = fmaxf(zh * i1, zh * i2) * gv.sdd_ipv + gv.cv;
+    const int iu0 = max(0, (int)ceilf(ulo - 0.01f)), iu1 = min(G.nu - 1, (int)floorf(uhi + 0.01f));
+    const int iv0 = max(0, (int)ceilf(vlo - 0.01f)), iv1 = min(G.nv - 1, (int)floorf(vhi + 0.01f));
+    const float xl = ex - 0.5f * G.hx, xh = ex + 0.5f * G.hx, yl = ey - 0.5f * G.hy, yh = ey + 0.5f * G.hy;
+    float acc = 0.f;
+    for (int iu = iu0; iu <= iu1; ++iu) {
+        const float4 ud = __ldg(utab + iu);
+        const float ax0 = xl * ud.z, ax1 = xh * ud.z, ay0 = yl * ud.w, ay1 = yh * ud.w;
+        const float lo_u = fmaxf(fminf(ax0, ax1), fminf(ay0, ay1));
+        const float hi_u = fminf(fmaxf(ax0, ax1), fmaxf(ay0, ay1));
+        if (!(hi_u > lo_u)) continue;
+        for (int iv = iv0; iv <= iv1; ++iv) {
+            const float2 vd = __ldg(vtab + iv);
+            const float az0 = zl * vd.y, az1 = zh * vd.y;
+            const float lo = fmaxf(lo_u, fminf(az0, az1)), hi = fminf(hi_u, fmaxf(az0, az1));
+            acc = fmaf(fmaxf(hi - lo, 0.f), __ldg(rL + iv * G.nu + iu), acc);
+        }
+    }
+    return acc;
+}
+
+__device__ __forceinline__ float f0_tap(const float* __restrict__ f0, int nx, int ny, int nz, int i, int j, int k) {
+    if ((unsigned)i < (unsigned)nx && (unsigned)j < (unsigned)ny && (unsigned)k < (unsigned)nz)
+        return __ldg(f0 + ((long long)k * ny + j) * nx + i);
+    return 0.f;
+}
+
+// G = d f / d x (1/mm) of the trilinear interpolant at voxel (i,j,k) displaced by d voxels:
+// forward differences along the four parallel cell edges per axis, bilinearly weighted
+// (reading A6).
+__device__ __forceinline__ void trilinear_grad(const Geom& G, const float* __restrict__ f0, int i, int j, int k,
+                                               float dx, float dy, float dz, float* gx, float* gy, float* gz) {
+    const float fx = floorf(dx), fy = floorf(dy), fz = floorf(dz);
+    const float tx = dx - fx, ty = dy - fy, tz = dz - fz;
+    const int i0 = i + (int)fx, j0 = j + (int)fy, k0 = k + (int)fz;
+    const int nx = G.nx, ny = G.ny, nz = G.nz;
+    float c000, c100, c010, c110, c001, c101, c011, c111;
+    if (i0 >= 0 && i0 + 1 < nx && j0 >= 0 && j0 + 1 < ny && k0 >= 0 && k0 + 1 < nz) {
+        const float* p = f0 + ((long long)k0 * ny + j0) * nx + i0;
+        const long long sy = nx, sz = (long long)nx * ny;
+        c000 = __ldg(p);           c100 = __ldg(p + 1);
+        c010 = __ldg(p + sy);      c110 = __ldg(p + sy + 1);
+        c001 = __ldg(p + sz);      c101 = __ldg(p + sz + 1);
+        c011 = __ldg(p + sz + sy); c111 = __ldg(p + sz + sy + 1);
+    } else {
+        c000 = f0_tap(f0, nx, ny, nz, i0, j0, k0);         c100 = f0_tap(f0, nx, ny, nz, i0 + 1, j0, k0);
+        c010 = f0_tap(f0, nx, ny, nz, i0, j0 + 1, k0);     c110 = f0_tap(f0, nx, ny, nz, i0 + 1, j0 + 1, k0);
+        c001 = f0_tap(f0, nx, ny, nz, i0, j0, k0 + 1);     c101 = f0_tap(f0, nx, ny, nz, i0 + 1, j0, k0 + 1);
+        c011 = f0_tap(f0, nx, ny, nz, i0, j0 + 1, k0 + 1); c111 = f0_tap(f0, nx, ny, nz, i0 + 1, j0 + 1, k0 + 1);
+    }
+    const float X0 = 1.f - tx, Y0 = 1.f - ty, Z0 = 1.f - tz;
+    *gx = G.ihx * ((Y0 * (c100 - c000) + ty * (c110 - c010)) * Z0 + (Y0 * (c101 - c001) + ty * (c111 - c011)) * tz);
+    *gy = G.ihy * ((X0 * (c010 - c000) + tx * (c110 - c100)) * Z0 + (X0 * (c011 - c001) + tx * (c111 - c101)) * tz);
+    *gz = G.ihz * ((X0 * (c001 - c000) + tx * (c101 - c100)) * Y0 + (X0 * (c011 - c010) + tx * (c111 - c110)) * ty);
+}
+
+template <int K>
+__global__ void __launch_bounds__(GT)
+k_grad(const Geom G, const float* __restrict__ f0, const float* __restrict__ xbar, const float* __restrict__ u,
+       const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
+       const float2* __restrict__ vtab, double* __restrict__ partials) {
+    __shared__ double red[GT / 32];
+    const int lane = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int x0 = blockIdx.x * TILE, y0 = blockIdx.y * TILE, z = blockIdx.z;
+    const int x = x0 + lane;
+    const long long V = G.V;
+    const int blk = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    const int nblk = gridDim.x * gridDim.y * gridDim.z;
+
+    float xb[ROWS][3], uu[ROWS][K][3];
+    bool in[ROWS];
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) {
+        const int y = y0 + ty + 8 * r;
+        in[r] = (x < G.nx) && (y < G.ny);
+        const long long lin = ((long long)z * G.ny + y) * G.nx + x;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            xb[r][c] = in[r] ? __ldcs(xbar + c * V + lin) : 0.f;
+#pragma unroll
+            for (int k = 0; k < K; ++k) uu[r][k][c] = in[r] ? __ldcs(u + ((long long)k * 3 + c) * V + lin) : 0.f;
+        }
+    }
+    const float xw = G.cx + ((float)x - 0.5f * (G.nx - 1)) * G.hx;
+    const float zw = G.cz + ((float)z - 0.5f * (G.nz - 1)) * G.hz;
+
+    for (int b = 0; b < B; ++b) {
+        if (!solves[b].running) continue;               // uniform over the grid
+        float w[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) w[k] = (float)solves[b].w[k];
+        const GatherView gv = make_gather_view(G, solves[b].view);
+        const float* rLb = rL + (long long)b * G.npix;
+        const float4* ub = utab + (long long)b * G.nu;
+        const float2* vb = vtab + (long long)b * G.nv;
+        float acc[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) acc[k] = 0.f;
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r) {
+            if (!in[r]) continue;
+            float d[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                float xs = xb[r][c];                    // Eq. (1)
+#pragma unroll
+                for (int k = 0; k < K; ++k) xs = fmaf(uu[r][k][c], w[k], xs);
+                d[c] = xs;
+            }
+            const int y = y0 + ty + 8 * r;
+            float gx, gy, gz;
+            trilinear_grad(G, f0, x, y, z, __fdiv_rn(d[0], G.hx), __fdiv_rn(d[1], G.hy), __fdiv_rn(d[2], G.hz),
+                           &gx, &gy, &gz);
+            if (gx == 0.f && gy == 0.f && gz == 0.f) continue;
+            const float yw = G.cy + ((float)y - 0.5f * (G.ny - 1)) * G.hy;
+            const float Bj = gather_voxel(G, gv, rLb, ub, vb, xw, yw, zw);
+#pragma unroll
+            for (int k = 0; k < K; ++k)
+                acc[k] = fmaf(Bj, gx * uu[r][k][0] + gy * uu[r][k][1] + gz * uu[r][k][2], acc[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const double s = block_sum<GT>((double)acc[k], red);
+            if (threadIdx.x == 0) partials[((long long)b * nblk + blk) * KMAX + k] = s;
+        }
+    }
+}
+
+// Hook: B = P^T r as a volume (view of solve 0).
+__global__ void __launch_bounds__(256)
+k_backproject(const Geom G, const SolveState* __restrict__ solves, const float* __restrict__ rL,
+              const float4* __restrict__ utab, const float2* __restrict__ vtab, float* __restrict__ out) {
+    const GatherView gv = make_gather_view(G, solves[0].view);
+    const long long lin = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (lin >= G.V) return;
+    const int i = (int)(lin % G.nx), j = (int)((lin / G.nx) % G.ny), k = (int)(lin / ((long long)G.nx * G.ny));
+    const float xw = G.cx + ((float)i - 0.5f * (G.nx - 1)) * G.hx;
+    const float yw = G.cy + ((float)j - 0.5f * (G.ny - 1)) * G.hy;
+    const float zw = G.cz + ((float)k - 0.5f * (G.nz - 1)) * G.hz;
+    out[lin] = gather_voxel(G, gv, rL, utab, vtab, xw, yw, zw);
+}
+
+template <int K>
+void launch_k(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SolveState* solves,
+              int B, const float* rL, const float4* utab, const float2* vtab, double* partials) {
+    dim3 grid((G.nx + TILE - 1) / TILE, (G.ny + TILE - 1) / TILE, G.nz);
+    q.launch(k_grad<K>, grid, dim3(GT), 0, G, f0, xbar, u, solves, B, rL, utab, vtab, partials);
+}
+
+}  // namespace
+
+int resid_blocks(const Geom& G) { return (G.npix + RT - 1) / RT; }
+int grad_blocks(const Geom& G) { return ((G.nx + TILE - 1) / TILE) * ((G.ny + TILE - 1) / TILE) * G.nz; }
+
+void launch_resid(Seq& q, const Geom& G, const SolveState* solves, const SolveIn* in, int B, int force,
+                  const float* p, const float* r_direct, float* rL, float4* utab, float2* vtab, double* partials) {
+    q.launch(k_resid, dim3(resid_blocks(G), B), dim3(RT), 0, G, solves, in, force, p, r_direct, rL, utab, vtab,
+             partials);
+}
+
+void launch_grad(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SolveState* solves,
+                 int B, const float* rL, const float4* utab, const float2* vtab, double* partials) {
+    switch (G.K) {
+#define PCAMM_CASE(KK) \
+    case KK: launch_k<KK>(q, G, f0, xbar, u, solves, B, rL, utab, vtab, partials); break;
+        PCAMM_CASE(1) PCAMM_CASE(2) PCAMM_CASE(3) PCAMM_CASE(4)
+        PCAMM_CASE(5) PCAMM_CASE(6) PCAMM_CASE(7) PCAMM_CASE(8)
+#undef PCAMM_CASE
+        default: break;
+    }
+}
+
+void launch_backproject(Seq& q, const Geom& G, const SolveState* solves, const float* rL, const float4* utab,
+                        const float2* vtab, float* vol_out) {
+    q.launch(k_backproject, dim3((unsigned)((G.V + 255) / 256)), dim3(256), 0, G, solves, rL, utab, vtab, vol_out);
+}
+
+}  // namespace pcamm

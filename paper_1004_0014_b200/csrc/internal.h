@@ -1,0 +1,135 @@
+// Host-side plumbing shared by the translation units of libpcamm: the kernel sequencer (the same
+// launcher code either launches on a stream or appends kernel nodes to a CUDA graph) and the
+// launcher prototypes of each step of the hot path.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <string>
+
+#include "common.cuh"
+
+namespace pcamm {
+
+void set_error(const std::string& msg);
+void count_launch(long long n);
+
+// A linear sequence of kernels.  stream mode: cudaLaunchKernel on `stream`.  graph mode: each
+// kernel becomes a node of `graph` depending on the previous one, so the solve can be replayed
+// as one graph launch with device-side while-loops (cudaGraphCondTypeWhile) around sub-sequences.
+struct Seq {
+    cudaStream_t stream = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphNode_t last = nullptr;
+    bool has_last = false;
+    cudaError_t err = cudaSuccess;
+
+    bool graph_mode() const { return graph != nullptr; }
+
+    template <class... KArgs, class... Args>
+    void launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args) {
+        if (err != cudaSuccess) return;
+        launch_impl<KArgs...>(kernel, grid, block, smem, static_cast<KArgs>(args)...);
+    }
+
+    // Appends a while-loop node; the kernels of its body go to the returned sequence.
+    Seq add_while(cudaGraphConditionalHandle handle) {
+        Seq body;
+        if (err != cudaSuccess) { body.err = err; return body; }
+        cudaGraphNodeParams p = {};
+        p.type = cudaGraphNodeTypeConditional;
+        p.conditional.handle = handle;
+        p.conditional.type = cudaGraphCondTypeWhile;
+        p.conditional.size = 1;
+        cudaGraphNode_t node;
+        err = cudaGraphAddNode(&node, graph, has_last ? &last : nullptr, has_last ? 1 : 0, &p);
+        if (err != cudaSuccess) { body.err = err; return body; }
+        last = node;
+        has_last = true;
+        body.graph = p.conditional.phGraph_out[0];
+        return body;
+    }
+
+  private:
+    template <class... KArgs>
+    void launch_impl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, KArgs... args) {
+        void* argv[] = {(void*)&args...};
+        if (graph) {
+            cudaKernelNodeParams kp = {};
+            kp.func = (void*)kernel;
+            kp.gridDim = grid;
+            kp.blockDim = block;
+            kp.sharedMemBytes = (unsigned)smem;
+            kp.kernelParams = argv;
+            cudaGraphNode_t node;
+            err = cudaGraphAddKernelNode(&node, graph, has_last ? &last : nullptr, has_last ? 1 : 0, &kp);
+            last = node;
+            has_last = true;
+        } else {
+            err = cudaLaunchKernel((const void*)kernel, grid, block, argv, smem, stream);
+            count_launch(1);
+        }
+    }
+};
+
+// ---- a-1 (warp.cu)
+void launch_warp(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SlotState* slots,
+                 const SolveState* solves, int nslots, int force_layout, float* vol_std, float* vol_tr,
+                 long long slot_stride);
+
+// ---- a-2 (project.cu)
+int project_blocks(const Geom& G);
+// p[s] = P f[s] for every active slot; per-block partial sums {sum p, sum y p, sum (p - a y - b)^2}.
+void launch_project(Seq& q, const Geom& G, const SlotState* slots, const SolveState* solves, const SolveIn* in,
+                    int nslots, const float* vol_std, const float* vol_tr, long long slot_stride, float* p,
+                    double* partials);
+// hook: project a caller volume in standard layout at the view of solve 0 (transposes on the fly
+// into vol_tr if that view needs it).
+void launch_transpose(Seq& q, const Geom& G, const float* vol_std, float* vol_tr);
+void launch_traverse(Seq& q, const Geom& G, const SolveState* solves, int iu, int iv, int cap, int* ijk, float* len,
+                     int* n_out);
+
+// ---- a-3 / a-4 (gradient.cu)
+int resid_blocks(const Geom& G);
+int grad_blocks(const Geom& G);
+// r = p - a y - b, rL = r * |D - S|, per-view tables, partial sums of r^2; p of solve b is read
+// from its accepted slot.
+// force: also for solves that are no longer running (closing pass); r_direct: take r from there.
+void launch_resid(Seq& q, const Geom& G, const SolveState* solves, const SolveIn* in, int B, int force,
+                  const float* p, const float* r_direct, float* rL, float4* utab, float2* vtab, double* partials);
+// g = 2 U^T (df/dx) P^T r, per-block partial sums [B][blocks][K].
+void launch_grad(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SolveState* solves,
+                 int B, const float* rL, const float4* utab, const float2* vtab, double* partials);
+// hook: B = P^T r as a volume for solve 0's view (rL/utab/vtab as written by launch_resid).
+void launch_backproject(Seq& q, const Geom& G, const SolveState* solves, const float* rL, const float4* utab,
+                        const float2* vtab, float* vol_out);
+
+// ---- control (control.cu)
+struct CtlBufs {
+    CallOpts* opts;
+    SolveIn* in;
+    SolveState* solves;
+    SolveTrace* traces;
+    SlotState* slots;
+    LoopFlags* flags;
+    double* ysum_part;   // [B][ysum_blocks][2]
+    double* proj_part;   // [S][project_blocks][3]
+    double* resid_part;  // [B][resid_blocks]
+    double* grad_part;   // [B][grad_blocks][K]
+    int ysum_blocks, proj_blocks, resid_blocks, grad_blocks;
+};
+int ysum_blocks(const Geom& G);
+void launch_ysums(Seq& q, const Geom& G, const CtlBufs& c, int B);
+// begin: views, w = w_init, slot 0 of every solve = w_init.  mode 0 solve, 1 eval hook.
+void launch_begin(Seq& q, const Geom& G, const CtlBufs& c, int mode);
+void launch_ctl_init(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond);
+void launch_ctl_grad(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond);
+void launch_ctl_trial(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond);
+void launch_ctl_iter_end(Seq& q, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond);
+void launch_ctl_final(Seq& q, const Geom& G, const CtlBufs& c, SlotState* out_slots);
+void launch_ctl_eval(Seq& q, const Geom& G, const CtlBufs& c, int stage);
+// a-6: landmarks [B][M][3]
+void launch_invert(Seq& q, const Geom& G, const float* xbar, const float* u, const CtlBufs& c, int B, int M,
+                   const float* r0, double* r_out);
+
+}  // namespace pcamm

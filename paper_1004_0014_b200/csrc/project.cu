@@ -1,0 +1,234 @@
+// a-2: cone-beam forward projection p = P_theta f  (section 2.2, Eq. 2;
+// "P is a projection matrix which computes the projection image of f").
+//
+// Reading A3: p_i = sum_j l_ij f_j with l_ij the exact length of the source -> pixel-centre
+// segment inside voxel box j (Siddon's radiological path).  The oracle merges and sorts all plane
+// crossings; this kernel computes the same sum slab by slab:
+//
+//   the ray marches along its dominant in-plane axis m (|d_m|/h_m largest; t = the other in-plane
+//   axis).  Between the planes M = i and M = i+1 (voxel-corner index units) it moves by
+//   |sT| <= 1 voxels in t and |sZ| <= 1 voxels in z, so it crosses at most one t-plane and one
+//   z-plane inside the slab: at most three voxels, whose shares tau of the slab length follow
+//   from where those two crossings fall.  Summed over slabs this is exactly Siddon's sum; every
+//   thread does the same work per slab and neighbouring rays read neighbouring addresses.
+//
+// Layout: rays marching along y read the standard volume [z][y][x] (t = x is contiguous), rays
+// marching along x read the in-plane transposed copy [z][x][y] (t = y contiguous), both written
+// by the warp kernel.  One thread per ray, one warp per 32 consecutive u of a detector row, a
+// block per 32 x 8 detector tile: a warp's loads of one slab fall into one or two 128 B lines.
+//
+// Ray set-up (source, direction, entry) is done in double; the march itself in float with
+// positions formed as fma(slope, plane, offset), never accumulated.
+//
+// a-3 (first half): the same kernel forms r_i = p_i - a y_i - b and the per-block partial sums of
+// p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.
+#include "internal.h"
+
+namespace pcamm {
+
+namespace {
+
+constexpr int TU = 32, TV = 8, NT = TU * TV;
+
+struct Ray {
+    int axis;          // 0: marches along x (reads [z][x][y]); 1: marches along y (reads [z][y][x])
+    int i_start, n, step;
+    int Nm, Nt, Nz;
+    // transverse / axial position (voxel-corner index units) at the q-th plane the ray meets,
+    // counted from the entry plane of its first slab: T = fma(sT, q, T0); sT, sZ are per step
+    float T0, sT, invT, Z0, sZ, invZ;
+    float Ls;          // mm of path per slab
+};
+
+__device__ __forceinline__ Ray make_ray(const Geom& G, const View& vw, int iu, int iv) {
+    Ray r;
+    const double uu = ((double)iu - 0.5 * (G.nu - 1) + (double)G.off_u) * (double)G.pu;
+    const double vv = ((double)iv - 0.5 * (G.nv - 1) + (double)G.off_v) * (double)G.pv;
+    const double Sx = (double)G.sad * vw.cs, Sy = (double)G.sad * vw.sn;
+    const double dx = -(double)G.sdd * vw.cs - uu * vw.sn;   // D - S
+    const double dy = -(double)G.sdd * vw.sn + uu * vw.cs;
+    const double dz = vv;
+    const double L = sqrt(dx * dx + dy * dy + dz * dz);
+    const double gx = dx / (double)G.hx, gy = dy / (double)G.hy, gz = dz / (double)G.hz;
+    const double Sxi = (Sx - G.lox) / (double)G.hx, Syi = (Sy - G.loy) / (double)G.hy, Szi = (0.0 - G.loz) / (double)G.hz;
+    double gm, gt, Sm, St;
+    if (fabs(gx) >= fabs(gy)) { r.axis = 0; gm = gx; gt = gy; Sm = Sxi; St = Syi; r.Nm = G.nx; r.Nt = G.ny; }
+    else                      { r.axis = 1; gm = gy; gt = gx; Sm = Syi; St = Sxi; r.Nm = G.ny; r.Nt = G.nx; }
+    r.Nz = G.nz;
+    const double sT = gt / gm, sZ = gz / gm;
+    const double T0 = St - Sm * sT, Z0 = Szi - Sm * sZ;
+    r.step = gm > 0.0 ? 1 : -1;
+    r.Ls = (float)(L / fabs(gm));
+    // slabs in which the ray can be inside the volume (conservative; exactness comes from the
+    // per-voxel range test in the sink)
+    double Mlo = 0.0, Mhi = (double)r.Nm;
+    bool empty = false;
+    if (sT != 0.0) {
+        const double m0 = (0.0 - T0) / sT, m1 = ((double)r.Nt - T0) / sT;
+        Mlo = fmax(Mlo, fmin(m0, m1)); Mhi = fmin(Mhi, fmax(m0, m1));
+    } else if (!(T0 >= 0.0 && T0 < (double)r.Nt)) empty = true;
+    if (sZ != 0.0) {
+        const double m0 = (0.0 - Z0) / sZ, m1 = ((double)r.Nz - Z0) / sZ;
+        Mlo = fmax(Mlo, fmin(m0, m1)); Mhi = fmin(Mhi, fmax(m0, m1));
+    } else if (!(Z0 >= 0.0 && Z0 < (double)r.Nz)) empty = true;
+    int ifirst = (int)floor(Mlo) - 1, ilast = (int)ceil(Mhi);
+    ifirst = max(ifirst, 0); ilast = min(ilast, r.Nm - 1);
+    r.n = 0; r.i_start = 0;
+    r.T0 = r.sT = r.invT = r.Z0 = r.sZ = r.invZ = 0.f;
+    if (empty || !(Mlo <= Mhi) || ilast < ifirst) return r;
+    r.n = ilast - ifirst + 1;
+    r.i_start = r.step > 0 ? ifirst : ilast;
+    const double Mb = r.step > 0 ? (double)ifirst : (double)(ilast + 1);   // entry plane of the first slab
+    r.T0 = (float)(T0 + sT * Mb); r.Z0 = (float)(Z0 + sZ * Mb);
+    r.sT = (float)(sT * r.step); r.sZ = (float)(sZ * r.step);
+    r.invT = 1.0f / r.sT; r.invZ = 1.0f / r.sZ;
+    return r;
+}
+
+// Calls sink(i, j, k, tau) for every (slab i, transverse j, axial k) piece, source side first;
+// tau = share of the slab's path length.
+template <class Sink>
+__device__ __forceinline__ void march(const Ray& r, Sink& sink) {
+    int i = r.i_start;
+    float Te = r.T0, Ze = r.Z0;
+    int ja = __float2int_rd(Te), ka = __float2int_rd(Ze);
+    for (int n = 0; n < r.n; ++n, i += r.step) {
+        const float q = (float)(n + 1);
+        const float Tx = fmaf(r.sT, q, r.T0), Zx = fmaf(r.sZ, q, r.Z0);
+        const int jb = __float2int_rd(Tx), kb = __float2int_rd(Zx);
+        // |sT|, |sZ| <= 1: at most one crossing each; rounding may show two, the second then
+        // coincides with the slab's exit plane and is left to the next slab
+        const int dj = max(-1, min(1, jb - ja)), dk = max(-1, min(1, kb - ka));
+        const int je = ja + dj, ke = ka + dk;
+        float tt = 1.f, tz = 1.f;
+        if (dj != 0) tt = fminf(fmaxf(((float)max(ja, je) - Te) * r.invT, 0.f), 1.f);
+        if (dk != 0) tz = fminf(fmaxf(((float)max(ka, ke) - Ze) * r.invZ, 0.f), 1.f);
+        const float t1 = fminf(tt, tz), t2 = fmaxf(tt, tz);
+        sink(i, ja, ka, t1);
+        if (t1 < 1.f) {
+            const bool tfirst = tt < tz;
+            sink(i, tfirst ? je : ja, tfirst ? ka : ke, t2 - t1);
+            if (t2 < 1.f) sink(i, je, ke, 1.f - t2);
+        }
+        Te = Tx; Ze = Zx; ja = jb; ka = kb;
+    }
+}
+
+struct AccSink {
+    const float* __restrict__ vol;
+    int Nm, Nt, Nz;
+    float acc;
+    __device__ __forceinline__ void operator()(int i, int j, int k, float tau) {
+        if ((unsigned)j < (unsigned)Nt && (unsigned)k < (unsigned)Nz)
+            acc = fmaf(tau, __ldg(vol + (k * Nm + i) * Nt + j), acc);
+    }
+};
+
+__global__ void __launch_bounds__(NT)
+k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* __restrict__ solves,
+          const SolveIn* __restrict__ in, const float* __restrict__ vol_std, const float* __restrict__ vol_tr,
+          long long slot_stride, float* __restrict__ p_out, double* __restrict__ partials) {
+    __shared__ double red[NT / 32];
+    const int s = blockIdx.z;
+    if (!slots[s].active) return;
+    const int b = slots[s].solve;
+    const View vw = solves[b].view;
+    const int tiles_u = (G.nu + TU - 1) / TU;
+    const int iu = (blockIdx.x % tiles_u) * TU + (threadIdx.x & 31);
+    const int iv = (blockIdx.x / tiles_u) * TV + (threadIdx.x >> 5);
+    double vp = 0.0, vyp = 0.0, vrr = 0.0;
+    if (iu < G.nu && iv < G.nv) {
+        const Ray r = make_ray(G, vw, iu, iv);
+        AccSink sink;
+        sink.vol = (r.axis == 0 ? vol_tr : vol_std) + (long long)s * slot_stride;
+        sink.Nm = r.Nm; sink.Nt = r.Nt; sink.Nz = r.Nz; sink.acc = 0.f;
+        march(r, sink);
+        const float p = sink.acc * r.Ls;
+        const int pix = iv * G.nu + iu;
+        p_out[(long long)s * G.npix + pix] = p;
+        const float* y = in[b].y;
+        const double yv = y ? (double)__ldg(y + pix) : 0.0;
+        const double res = (double)p - solves[b].a * yv - solves[b].b;   // Eq. (2) residual
+        vp = (double)p; vyp = yv * (double)p; vrr = res * res;
+    }
+    const int nblk = gridDim.x;
+    double* out = partials + ((long long)s * nblk + blockIdx.x) * 3;
+    const double sp = block_sum<NT>(vp, red);
+    const double syp = block_sum<NT>(vyp, red);
+    const double srr = block_sum<NT>(vrr, red);
+    if (threadIdx.x == 0) { out[0] = sp; out[1] = syp; out[2] = srr; }
+}
+
+// In-plane transpose [z][y][x] -> [z][x][y] (hook path only: the solve's volumes are written in
+// both layouts by the warp kernel).
+__global__ void __launch_bounds__(256)
+k_transpose(const Geom G, const float* __restrict__ src, float* __restrict__ dst) {
+    __shared__ float tile[32][33];
+    const int lane = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32, z = blockIdx.z;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int y = y0 + ty + 8 * r, x = x0 + lane;
+        tile[ty + 8 * r][lane] = (x < G.nx && y < G.ny) ? src[((long long)z * G.ny + y) * G.nx + x] : 0.f;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int x = x0 + ty + 8 * r, y = y0 + lane;
+        if (x < G.nx && y < G.ny) dst[((long long)z * G.nx + x) * G.ny + y] = tile[lane][ty + 8 * r];
+    }
+}
+
+struct RecSink {
+    int axis, cap, n;
+    int Nt, Nz;
+    float Ls, eps;
+    int* ijk;
+    float* len;
+    __device__ __forceinline__ void operator()(int i, int j, int k, float tau) {
+        if (!((unsigned)j < (unsigned)Nt && (unsigned)k < (unsigned)Nz)) return;
+        const float l = tau * Ls;
+        if (!(l > eps)) return;     // zero-length pieces are dropped (reading A22)
+        if (n < cap) {
+            ijk[3 * n + 0] = axis == 0 ? i : j;
+            ijk[3 * n + 1] = axis == 0 ? j : i;
+            ijk[3 * n + 2] = k;
+            len[n] = l;
+        }
+        ++n;
+    }
+};
+
+__global__ void k_traverse(const Geom G, const SolveState* __restrict__ solves, int iu, int iv, int cap, int* ijk,
+                           float* len, int* n_out) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const Ray r = make_ray(G, solves[0].view, iu, iv);
+    RecSink sink;
+    sink.axis = r.axis; sink.cap = cap; sink.n = 0; sink.Nt = r.Nt; sink.Nz = r.Nz; sink.Ls = r.Ls;
+    sink.eps = 1e-6f * fminf(G.hx, fminf(G.hy, G.hz));
+    sink.ijk = ijk; sink.len = len;
+    march(r, sink);
+    *n_out = sink.n;
+}
+
+}  // namespace
+
+int project_blocks(const Geom& G) { return ((G.nu + TU - 1) / TU) * ((G.nv + TV - 1) / TV); }
+
+void launch_project(Seq& q, const Geom& G, const SlotState* slots, const SolveState* solves, const SolveIn* in,
+                    int nslots, const float* vol_std, const float* vol_tr, long long slot_stride, float* p,
+                    double* partials) {
+    q.launch(k_project, dim3(project_blocks(G), 1, nslots), dim3(NT), 0, G, slots, solves, in, vol_std, vol_tr,
+             slot_stride, p, partials);
+}
+
+void launch_transpose(Seq& q, const Geom& G, const float* vol_std, float* vol_tr) {
+    q.launch(k_transpose, dim3((G.nx + 31) / 32, (G.ny + 31) / 32, G.nz), dim3(256), 0, G, vol_std, vol_tr);
+}
+
+void launch_traverse(Seq& q, const Geom& G, const SolveState* solves, int iu, int iv, int cap, int* ijk, float* len,
+                     int* n_out) {
+    q.launch(k_traverse, dim3(1), dim3(32), 0, G, solves, iu, iv, cap, ijk, len, n_out);
+}
+
+}  // namespace pcamm

@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- ms per projection solve on the headline workload (BASELINE.json configs[2]:
+256x256x128 volume, 1.5 mm voxels, K = 3, detector 512x384 @ 0.776 mm, 360 projections at 1 deg,
+irregular breathing at 1.5x amplitude, Poisson noise at 1e5 photons per ray; all synthetic, seeded).
+
+One step = one whole per-projection solve: initial evaluation and fit, 10
+iterations of {residual, fused adjoint gradient, Armijo backtracking with one
+warp + projection per trial, Eq. 4 fit}, closing cost, tumour localisation.  Consecutive steps
+solve consecutive projections of the rotation (1 degree, 1/6 s apart) and each starts from the
+previous frame's coefficients.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config C2]
+
+N > 1 (under torchrun): replicas only -- every rank holds the model and solves its own contiguous
+block of K projections; no data-path collective; scaling is weak.
+--impl reference times the CPU oracle (fp64, OpenMP on the host cores) on the same workload.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import get_config                                   # noqa: E402
+from workloads.build import build_workload                         # noqa: E402
+from workloads.motion import dvf_grid                              # noqa: E402
+from workloads.noise import add_noise                              # noqa: E402
+from workloads.phantom import voxelise                             # noqa: E402
+
+METRIC = "ms_per_projection_solve"
+FIRST_FRAME = 60      # where in the rotation the timed block starts (any frame is representative)
+PAPER_MS = None       # the paper's 240 ms is for another volume/detector/machine: context only
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+# ----------------------------------------------------------------------------- inputs (CPU, seeded)
+
+_G = {}
+
+
+def _gt_worker(idx):
+    cfg, spec, frames = _G["cfg"], _G["spec"], _G["frames"]
+    fr = frames[idx]
+    return idx, voxelise(cfg, dvf_grid(cfg, spec, fr.phase, fr.amplitude)).astype(np.float32)
+
+
+def ground_truth_volumes(wl, indices):
+    """The phantom deformed by the test DVF of each frame (workloads recipe), in parallel on the host
+    cores.  Must run before CUDA is initialised (fork)."""
+    import multiprocessing as mp
+    _G.update(cfg=wl.cfg, spec=wl.spec, frames=wl.frames)
+    uniq = sorted(set(indices))
+    n_proc = max(1, min(len(uniq), (os.cpu_count() or 2) - 1, 12))
+    if n_proc == 1:
+        return dict(_gt_worker(i) for i in uniq)
+    with mp.get_context("fork").Pool(n_proc) as pool:
+        return dict(pool.map(_gt_worker, uniq))
+
+
+def solver_iterations(cfg) -> int:
+    return cfg.iterations
+
+
+def algorithmic_bytes(cfg):
+    """what the method must move per launch, f0 gathers counted once."""
+    V, K, npix = cfg.V, cfg.K, cfg.npix
+    return {"warp": (12 * (K + 1) + 4 + 4) * V,
+            "project": 4 * V + 4 * npix,
+            "gradient": (12 * (K + 1) + 4) * V + 4 * npix}
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        time.sleep(0.25)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------- the two arms
+
+def oracle_geometry(cfg):
+    import oracle
+    return oracle.Geometry(cfg.nx, cfg.ny, cfg.nz, cfg.hx, cfg.hy, cfg.hz, cfg.K, cfg.nu, cfg.nv, cfg.pu, cfg.pv,
+                           cfg.sad, cfg.sdd)
+
+
+def time_oracle_solves(wl, gts, frame_ids, iterations, threads=None):
+    """The oracle as it stands (fp64 C++, OpenMP over rays / voxels) on the host cores: one full
+    solve per frame, projections simulated by the oracle's own projector.  Returns seconds per
+    solve (list) and the thread count."""
+    import oracle
+    cfg = wl.cfg
+    g = oracle_geometry(cfg)
+    nthr = threads or oracle.max_threads()
+    oracle.set_threads(nthr)
+    w = np.zeros(cfg.K)
+    secs = []
+    for fid in frame_ids:
+        fr = wl.frames[fid]
+        y = add_noise(oracle.project(g, gts[fid], fr.angle_rad), cfg.noise, seed=fid)
+        t0 = time.perf_counter()
+        res = oracle.solve(g, wl.f0, wl.model.mean, wl.model.eig, y, fr.angle_rad, w,
+                           oracle.Opts(max_iter=iterations, batched_linesearch=int(cfg.batched_linesearch)),
+                           want_volume=False)
+        oracle.invert(g, wl.model.mean, wl.model.eig, res["w"], wl.landmarks)
+        secs.append(time.perf_counter() - t0)
+        w = res["w"]
+    return secs, nthr
+
+
+def run_reference(args, cfg, rank, world):
+    if rank != 0:
+        return
+    wl = build_workload(cfg)
+    n = args.steps + args.warmup
+    ids = [(FIRST_FRAME + i) % len(wl.frames) for i in range(n)]
+    # bounded sample: the block's first frames only, one full solve each, cycled over the steps
+    n_distinct = min(n, 2)
+    gts = ground_truth_volumes(wl, ids[:n_distinct])
+    it = solver_iterations(cfg)
+    cyc = [ids[i % n_distinct] for i in range(n)]
+    secs, nthr = time_oracle_solves(wl, gts, cyc, it)
+    timed = secs[args.warmup:]
+    ms = 1e3 * float(np.mean(timed))
+    line = {"impl": "reference", "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(cfg, it),
+            "cpu_baseline": {"value": ms, "unit": "ms", "cores": nthr, "kind": "oracle",
+                             "sample": f"full {it}-iteration oracle solves, {n_distinct} distinct projections "
+                                       f"cycled over {n} steps, OpenMP on {nthr} threads"},
+            "e2e": {"value": ms, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def config_dict(cfg, iterations):
+    return {"workload": f"{cfg.name}: volume {cfg.nx}x{cfg.ny}x{cfg.nz} @ {cfg.hx} mm, K={cfg.K}, detector "
+                        f"{cfg.nu}x{cfg.nv} @ {cfg.pu} mm, consecutive projections 1 deg / (1/6) s apart from frame "
+                        f"{FIRST_FRAME}, {cfg.noise} noise, {'irregular' if cfg.irregular else 'regular'} breathing "
+                        f"x{cfg.amplitude}",
+            "iterations": iterations, "warm_start": "previous frame's w (PAPER.md:L141)",
+            "line_search": "batched 8 candidates" if cfg.batched_linesearch else "sequential Armijo backtracking",
+            "l2": "inputs larger than L2: every pass streams the (K+1) vector fields "
+                  f"({12 * (cfg.K + 1) * cfg.V / 2**20:.0f} MiB) through a 126 MB L2",
+            "parallelism": "replicas"}
+
+
+def run_ours(args, cfg, rank, local_rank, world):
+    from paper_1004_0014_b200 import replicas
+    it = solver_iterations(cfg)
+    n = args.steps + args.warmup
+    # ---- inputs on the CPU first (the worker pool forks before CUDA is initialised)
+    t0 = time.perf_counter()
+    wl = build_workload(cfg)
+    ids = replicas.frame_block(rank, world, n, FIRST_FRAME, len(wl.frames))
+    gts = ground_truth_volumes(wl, ids)
+    log(f"[rank {rank}] inputs built in {time.perf_counter() - t0:.1f} s")
+
+    import torch
+    import paper_1004_0014_b200 as pc
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = replicas.init_process_group("nccl")
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(dev)
+    C = 8 if cfg.batched_linesearch else 1
+    m = pc.Model(nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, hx=cfg.hx, hy=cfg.hy, hz=cfg.hz, K=cfg.K, nu=cfg.nu, nv=cfg.nv,
+                 pu=cfg.pu, pv=cfg.pv, f0=t(wl.f0), mean_dvf=t(wl.model.mean), eig_dvf=t(wl.model.eig),
+                 landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=C)
+    # measured projections: the scanner is simulated with the library's own projector applied to
+    # the ground-truth volume, plus seeded noise (the CPU arm simulates its own with the oracle)
+    ys_host, ys_dev = [], []
+    for fid in ids:
+        fr = wl.frames[fid]
+        p_true = m.project(t(gts[fid]), fr.angle_rad).cpu().numpy()
+        y = add_noise(p_true, cfg.noise, seed=fid)
+        ys_host.append(torch.from_numpy(y).pin_memory())
+        ys_dev.append(t(y))
+    angles = [float(wl.frames[fid].angle_rad) for fid in ids]
+    opts = pc.Opts(max_iter=it, batched_linesearch=int(cfg.batched_linesearch))
+
+    def run_block(first, count, w, host):
+        for i in range(first, first + count):
+            if host:
+                r = m.reconstruct(ys_host[i].numpy(), angles[i], w, opts, host_y=True)
+            else:
+                r = m.reconstruct(ys_dev[i], angles[i], w, opts)
+            w = r.w
+        return w, r
+
+    # ---- device-resident timing: y already in HBM
+    w = np.zeros(cfg.K, np.float32)
+    w, _ = run_block(0, args.warmup, w, host=False)
+    w_after_warmup = w.copy()
+    torch.cuda.synchronize()
+    replicas.barrier(dist)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    pc.launch_count(reset=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    w, last = run_block(args.warmup, args.steps, w, host=False)
+    e1.record()
+    torch.cuda.synchronize()
+    launches = pc.launch_count(reset=True)
+    replicas.barrier(dist)
+    clocks = sampler.stop() if sampler else None
+    elapsed_ms = replicas.max_over_ranks(dist, e0.elapsed_time(e1), dev)
+    launches = int(replicas.sum_over_ranks(dist, launches, dev))
+
+    # ---- end to end: y in pinned host memory, copied inside the call; results read back inside it
+    run_block(max(args.warmup - 1, 0), 1, w_after_warmup, host=True)
+    torch.cuda.synchronize()
+    replicas.barrier(dist)
+    t0 = time.perf_counter()
+    run_block(args.warmup, args.steps, w_after_warmup, host=True)
+    torch.cuda.synchronize()
+    e2e_ms = replicas.max_over_ranks(dist, 1e3 * (time.perf_counter() - t0), dev)
+    h2d = cfg.npix * 4 + 128 + 56          # y + the call's option block (CallOpts, SolveIn)
+    d2h = 272 + 16 + 24 * len(wl.landmarks)  # SolveState + LoopFlags + landmark positions (double)
+
+    if rank != 0:
+        return
+    ms_per_solve = elapsed_ms / (args.steps * world)
+
+    # ---- per-kernel device times on the last frame's state (CUDA events inside the library, on the
+    #      stream the kernels are launched on), and the launch mix of one traced solve
+    i_last = n - 1
+    tr = m.reconstruct(ys_dev[i_last], angles[i_last], w_after_warmup, opts, trace=True)
+    trials = int(np.sum(tr.backtracks + 1)) if tr.backtracks is not None else it
+    m.eval(ys_dev[i_last], angles[i_last], tr.w, tr.a, tr.b, want_proj=False)
+    for which in (0, 1, 2):
+        m.time_kernel(which, 3)
+    kt = {name: m.time_kernel(which, 20) for which, name in ((0, "warp"), (1, "project"), (2, "gradient"))}
+    nl = {"warp": trials + 1, "project": trials + 1, "gradient": tr.iters}
+    ab = algorithmic_bytes(cfg)
+    peak, peak_src = measured_peak_gbs()
+    per_kernel = {k: {"ms": kt[k], "launches_per_solve": nl[k], "algorithmic_bytes": ab[k],
+                      "gbs": ab[k] / (kt[k] * 1e-3) / 1e9, "frac": ab[k] / (kt[k] * 1e-3) / 1e9 / peak}
+                  for k in kt}
+    dom = max(kt, key=lambda k: kt[k] * nl[k])
+    wp_gbs = (ab["warp"] + ab["project"]) / ((kt["warp"] + kt["project"]) * 1e-3) / 1e9
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": per_kernel[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": per_kernel[dom]["frac"], "traffic": None, "peak_source": peak_src,
+                "per_kernel": per_kernel,
+                "warp_plus_project": {"gbs": wp_gbs, "frac": wp_gbs / peak,
+                                      "frac_of_nominal_8000": wp_gbs / 8000.0},
+                "kernel_share_of_step": {k: kt[k] * nl[k] / (elapsed_ms / args.steps) for k in kt}}
+
+    # ---- the oracle on this box's host cores, one full solve of the same workload
+    cpu = None
+    if not args.no_cpu_baseline:
+        tc = time.perf_counter()
+        secs, nthr = time_oracle_solves(wl, gts, [ids[args.warmup]], it)
+        cpu = {"value": 1e3 * secs[0], "unit": "ms", "cores": nthr, "kind": "oracle",
+               "sample": f"1 projection (frame {ids[args.warmup]}), full {it}-iteration solve from w = 0, "
+                         f"OpenMP on {nthr} threads; {time.perf_counter() - tc:.0f} s including its simulated y"}
+
+    line = {"metric": METRIC, "value": ms_per_solve, "unit": "ms", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": config_dict(cfg, it), "projections_per_s": 1e3 * args.steps * world / elapsed_ms,
+            "clocks": clocks,
+            "e2e": {"value": e2e_ms / (args.steps * world), "unit": "ms", "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h},
+            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "last_solve": {"iters": tr.iters, "trials": trials, "status": tr.status, "J0": tr.J0, "J": tr.J},
+            "context": {"paper_ms_per_projection_tesla_c1060": 240.0}}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C2")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    from paper_1004_0014_b200.replicas import env_rank_world
+    rank, local_rank, world = env_rank_world()
+    cfg = get_config(args.config)
+    if args.impl == "reference":
+        run_reference(args, cfg, rank, world)
+    else:
+        run_ours(args, cfg, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

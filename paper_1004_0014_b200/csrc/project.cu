@@ -9,16 +9,17 @@
 //   axis).  Between the planes M = i and M = i+1 (voxel-corner index units) it moves by
 //   |sT| <= 1 voxels in t and |sZ| <= 1 voxels in z, so it crosses at most one t-plane and one
 //   z-plane inside the slab: at most three voxels, whose shares tau of the slab length follow
-//   from where those two crossings fall.  Summed over slabs this is exactly Siddon's sum; every
-//   thread does the same work per slab and neighbouring rays read neighbouring addresses.
+//   from where those two crossings fall.  Summed over slabs this is exactly Siddon's sum; most
+//   slabs hold a single voxel (one load, one add) and neighbouring rays read neighbouring
+//   addresses.
 //
 // Layout: rays marching along y read the standard volume [z][y][x] (t = x is contiguous), rays
 // marching along x read the in-plane transposed copy [z][x][y] (t = y contiguous), both written
 // by the warp kernel.  One thread per ray, one warp per 32 consecutive u of a detector row, a
 // block per 32 x 8 detector tile: a warp's loads of one slab fall into one or two 128 B lines.
 //
-// Ray set-up (source, direction, entry) is done in double; the march itself in float with
-// positions formed as fma(slope, plane, offset), never accumulated.
+// Ray set-up (source, direction, entry, first crossings, crossing spacing) is done in double; the
+// march itself is integer (fixed-point crossing counters) plus one float multiply-add per piece.
 //
 // a-3 (first half): the same kernel forms r_i = p_i - a y_i - b and the per-block partial sums of
 // p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.
@@ -30,24 +31,46 @@ namespace {
 
 constexpr int TU = 32, TV = 8, NT = TU * TV;
 
+// One ray in the frame of its marching axis.  Slab n (n = 0 .. n_slabs-1, counted from the source
+// side) is the n-th voxel layer along the marching axis that the ray meets; q in [n, n+1] is the
+// ray parameter inside it.  The crossings of transverse (t) and axial (z) voxel planes are tracked
+// as 32.32 fixed-point values of q: hi word = slab in which the crossing falls, lo word = share of
+// that slab's path before it.  The first crossing and the spacing 1/|slope| come from the double
+// precision set-up, so that a crossing's slab and share do not depend on float rounding of a
+// position (for a ray almost parallel to a plane family that rounding, divided by the slope,
+// would misplace the crossing by whole slabs).
 struct Ray {
-    int axis;          // 0: marches along x (reads [z][x][y]); 1: marches along y (reads [z][y][x])
-    int i_start, n, step;
+    int axis;                       // 0: marches along x (reads [z][x][y]); 1: along y (reads [z][y][x])
+    int i_start, n_slabs, step;     // first layer index, count, +1 / -1
     int Nm, Nt, Nz;
-    // transverse / axial position (voxel-corner index units) at the q-th plane the ray meets,
-    // counted from the entry plane of its first slab: T = fma(sT, q, T0); sT, sZ are per step
-    float T0, sT, invT, Z0, sZ, invZ;
-    float Ls;          // mm of path per slab
+    int j0, k0, dirT, dirZ;         // voxel of the entry point; direction of change at a crossing
+    unsigned long long QT, dQT, QZ, dQZ;
+    float Ls;                       // mm of path per slab
 };
+
+constexpr double FIX = 4294967296.0;            // 2^32
+constexpr double QMAX = 1073741824.0;           // crossings beyond any volume are parked here (2^30 slabs)
+
+__device__ __forceinline__ void first_crossing(double P0, double s, int* idx0, int* dir, unsigned long long* Q,
+                                               unsigned long long* dQ) {
+    const double fl = floor(P0);
+    *idx0 = (int)fl;
+    if (s == 0.0) { *dir = 0; *Q = (unsigned long long)(QMAX * FIX); *dQ = 0ull; return; }
+    *dir = s > 0.0 ? 1 : -1;
+    const double plane = s > 0.0 ? fl + 1.0 : fl;
+    const double q = fmin(fmax((plane - P0) / s, 0.0), QMAX);
+    const double d = fmin(1.0 / fabs(s), QMAX);
+    *Q = (unsigned long long)(q * FIX + 0.5);
+    *dQ = (unsigned long long)(d * FIX + 0.5);
+    if (*dQ < (1ull << 32)) *dQ = 1ull << 32;   // |s| <= 1: never two crossings in one slab
+}
 
 __device__ __forceinline__ Ray make_ray(const Geom& G, const View& vw, int iu, int iv) {
     Ray r;
-    const double uu = ((double)iu - 0.5 * (G.nu - 1) + (double)G.off_u) * (double)G.pu;
-    const double vv = ((double)iv - 0.5 * (G.nv - 1) + (double)G.off_v) * (double)G.pv;
+    double dx, dy;
+    ray_dir_inplane(G, vw.cs, vw.sn, iu, &dx, &dy);                       // D - S
+    const double dz = ((double)iv - 0.5 * (G.nv - 1) + (double)G.off_v) * (double)G.pv;
     const double Sx = (double)G.sad * vw.cs, Sy = (double)G.sad * vw.sn;
-    const double dx = -(double)G.sdd * vw.cs - uu * vw.sn;   // D - S
-    const double dy = -(double)G.sdd * vw.sn + uu * vw.cs;
-    const double dz = vv;
     const double L = sqrt(dx * dx + dy * dy + dz * dz);
     const double gx = dx / (double)G.hx, gy = dy / (double)G.hy, gz = dz / (double)G.hz;
     const double Sxi = (Sx - G.lox) / (double)G.hx, Syi = (Sy - G.loy) / (double)G.hy, Szi = (0.0 - G.loz) / (double)G.hz;
@@ -55,12 +78,12 @@ __device__ __forceinline__ Ray make_ray(const Geom& G, const View& vw, int iu, i
     if (fabs(gx) >= fabs(gy)) { r.axis = 0; gm = gx; gt = gy; Sm = Sxi; St = Syi; r.Nm = G.nx; r.Nt = G.ny; }
     else                      { r.axis = 1; gm = gy; gt = gx; Sm = Syi; St = Sxi; r.Nm = G.ny; r.Nt = G.nx; }
     r.Nz = G.nz;
-    const double sT = gt / gm, sZ = gz / gm;
-    const double T0 = St - Sm * sT, Z0 = Szi - Sm * sZ;
+    const double sT = gt / gm, sZ = gz / gm;            // per unit of the marching coordinate M
+    const double T0 = St - Sm * sT, Z0 = Szi - Sm * sZ; // at the plane M = 0
     r.step = gm > 0.0 ? 1 : -1;
     r.Ls = (float)(L / fabs(gm));
-    // slabs in which the ray can be inside the volume (conservative; exactness comes from the
-    // per-voxel range test in the sink)
+    // layers in which the ray can be inside the volume (conservative by one; exactness comes from
+    // the per-voxel range test in the sink)
     double Mlo = 0.0, Mhi = (double)r.Nm;
     bool empty = false;
     if (sT != 0.0) {
@@ -73,44 +96,37 @@ __device__ __forceinline__ Ray make_ray(const Geom& G, const View& vw, int iu, i
     } else if (!(Z0 >= 0.0 && Z0 < (double)r.Nz)) empty = true;
     int ifirst = (int)floor(Mlo) - 1, ilast = (int)ceil(Mhi);
     ifirst = max(ifirst, 0); ilast = min(ilast, r.Nm - 1);
-    r.n = 0; r.i_start = 0;
-    r.T0 = r.sT = r.invT = r.Z0 = r.sZ = r.invZ = 0.f;
+    r.n_slabs = 0; r.i_start = 0; r.j0 = r.k0 = r.dirT = r.dirZ = 0; r.QT = r.dQT = r.QZ = r.dQZ = 0ull;
     if (empty || !(Mlo <= Mhi) || ilast < ifirst) return r;
-    r.n = ilast - ifirst + 1;
+    r.n_slabs = ilast - ifirst + 1;
     r.i_start = r.step > 0 ? ifirst : ilast;
     const double Mb = r.step > 0 ? (double)ifirst : (double)(ilast + 1);   // entry plane of the first slab
-    r.T0 = (float)(T0 + sT * Mb); r.Z0 = (float)(Z0 + sZ * Mb);
-    r.sT = (float)(sT * r.step); r.sZ = (float)(sZ * r.step);
-    r.invT = 1.0f / r.sT; r.invZ = 1.0f / r.sZ;
+    first_crossing(T0 + sT * Mb, sT * r.step, &r.j0, &r.dirT, &r.QT, &r.dQT);
+    first_crossing(Z0 + sZ * Mb, sZ * r.step, &r.k0, &r.dirZ, &r.QZ, &r.dQZ);
     return r;
 }
 
-// Calls sink(i, j, k, tau) for every (slab i, transverse j, axial k) piece, source side first;
+// Calls sink(i, j, k, tau) for every (layer i, transverse j, axial k) piece, source side first;
 // tau = share of the slab's path length.
 template <class Sink>
 __device__ __forceinline__ void march(const Ray& r, Sink& sink) {
-    int i = r.i_start;
-    float Te = r.T0, Ze = r.Z0;
-    int ja = __float2int_rd(Te), ka = __float2int_rd(Ze);
-    for (int n = 0; n < r.n; ++n, i += r.step) {
-        const float q = (float)(n + 1);
-        const float Tx = fmaf(r.sT, q, r.T0), Zx = fmaf(r.sZ, q, r.Z0);
-        const int jb = __float2int_rd(Tx), kb = __float2int_rd(Zx);
-        // |sT|, |sZ| <= 1: at most one crossing each; rounding may show two, the second then
-        // coincides with the slab's exit plane and is left to the next slab
-        const int dj = max(-1, min(1, jb - ja)), dk = max(-1, min(1, kb - ka));
-        const int je = ja + dj, ke = ka + dk;
-        float tt = 1.f, tz = 1.f;
-        if (dj != 0) tt = fminf(fmaxf(((float)max(ja, je) - Te) * r.invT, 0.f), 1.f);
-        if (dk != 0) tz = fminf(fmaxf(((float)max(ka, ke) - Ze) * r.invZ, 0.f), 1.f);
+    int i = r.i_start, j = r.j0, k = r.k0;
+    unsigned long long QT = r.QT, QZ = r.QZ;
+    const float inv32 = 2.3283064365386963e-10f;   // 2^-32
+    for (int n = 0; n < r.n_slabs; ++n, i += r.step) {
+        const bool ct = (unsigned)(QT >> 32) == (unsigned)n, cz = (unsigned)(QZ >> 32) == (unsigned)n;
+        if (!ct && !cz) { sink(i, j, k, 1.f); continue; }
+        const float tt = ct ? __uint2float_rn((unsigned)QT) * inv32 : 1.f;
+        const float tz = cz ? __uint2float_rn((unsigned)QZ) * inv32 : 1.f;
+        const int je = ct ? j + r.dirT : j, ke = cz ? k + r.dirZ : k;
         const float t1 = fminf(tt, tz), t2 = fmaxf(tt, tz);
-        sink(i, ja, ka, t1);
-        if (t1 < 1.f) {
-            const bool tfirst = tt < tz;
-            sink(i, tfirst ? je : ja, tfirst ? ka : ke, t2 - t1);
-            if (t2 < 1.f) sink(i, je, ke, 1.f - t2);
-        }
-        Te = Tx; Ze = Zx; ja = jb; ka = kb;
+        sink(i, j, k, t1);
+        const bool tfirst = tt < tz;
+        sink(i, tfirst ? je : j, tfirst ? k : ke, t2 - t1);
+        if (ct && cz) sink(i, je, ke, 1.f - t2);
+        j = je; k = ke;
+        if (ct) QT += r.dQT;
+        if (cz) QZ += r.dQZ;
     }
 }
 

@@ -130,8 +130,9 @@ def test_uniform_volume_gives_box_chords():
 @pytest.mark.parametrize("theta", [0.0, 0.37, np.pi / 4, 1.3, np.pi / 2, 2.5, 4.4, 5.9])
 def test_traversal_index_sets_are_bit_exact(theta):
     """north_star: bit-exact ray/voxel index sets.  Isocentre shifted by an irrational fraction of a
-    voxel (reading A22); rays whose smallest crossing gap is < 1e-3 min(h) are degenerate and are
-    compared on length only."""
+    voxel (reading A22); rays whose smallest crossing gap is < 1e-5 min(h) are degenerate and are
+    compared on total length only (crossing positions are carried in 32.32 fixed point from a
+    double-precision set-up, so the order of crossings is resolved far below that gap)."""
     g = _geom(n=(24, 20, 12), det=(30, 14), pitch=(4.0, 4.0))
     f0, xbar, u, scale, m = _model(g)
     n_deg = n_cmp = 0
@@ -140,13 +141,13 @@ def test_traversal_index_sets_are_bit_exact(theta):
             ijk_o, len_o, gap = oracle.traverse(g, theta, iu, iv)
             ijk_g, len_g = m.traverse(theta, iu, iv)
             assert abs(len_g.sum() - len_o.sum()) <= 1e-4
-            if gap < 1e-3 * min(g.hx, g.hy, g.hz):
+            if gap < 1e-5 * min(g.hx, g.hy, g.hz):
                 n_deg += 1
                 continue
             n_cmp += 1
             assert np.array_equal(ijk_g, ijk_o), (iu, iv, ijk_g, ijk_o)
             np.testing.assert_allclose(len_g, len_o, rtol=0, atol=2e-4)
-    assert n_cmp > 50 and n_deg <= 0.02 * (n_cmp + n_deg) + 1
+    assert n_cmp > 50 and n_deg <= 0.01 * (n_cmp + n_deg) + 1
 
 
 def test_traversal_golden_central_ray():

@@ -233,7 +233,7 @@ def run_ours(args, cfg, rank, local_rank, world):
         ys_host.append(torch.from_numpy(y).pin_memory())
         ys_dev.append(t(y))
     angles = [float(wl.frames[fid].angle_rad) for fid in ids]
-    opts = pc.Opts(max_iter=it, batched_linesearch=int(cfg.batched_linesearch))
+    opts = pc.Opts(max_iter=it, batched_linesearch=int(cfg.batched_linesearch), loop_mode=args.loop_mode)
 
     def run_block(first, count, w, host):
         for i in range(first, first + count):
@@ -332,6 +332,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1],
+                    help="0: the solve is one CUDA graph with device-side while-loops (default, the timed "
+                         "configuration); 1: same kernels launched from the host (for per-launch ncu lists)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     from paper_1004_0014_b200.replicas import env_rank_world

@@ -46,7 +46,9 @@ struct pcamm_model {
     // model (device)
     float *f0 = nullptr, *xbar = nullptr, *u = nullptr, *lm0 = nullptr;
     // scratch (device)
-    float *vol_std = nullptr, *vol_tr = nullptr, *p = nullptr, *rL = nullptr;
+    float *vol = nullptr, *p = nullptr, *rL = nullptr;   // vol: trial volumes, ray layout [S][PV]
+    ColHdr* col_hdr = nullptr;      // [B][nu]
+    SlabEntry* slab_tab = nullptr;  // [B][nu][max_slabs]
     float4* utab = nullptr;
     float2* vtab = nullptr;
     char* in_block = nullptr;
@@ -151,8 +153,9 @@ void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     const Geom& G = m->G;
     launch_ysums(q, G, m->c, B);
     launch_begin(q, G, m->c, 0);
-    launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, B * C, 0, m->vol_std, m->vol_tr, G.V);
-    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->vol_std, m->vol_tr, G.V, m->p, m->c.proj_part);
+    launch_view_tables(q, G, m->c.solves, B, m->col_hdr, m->slab_tab);
+    launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, B * C, 1, m->vol, G.PV);
+    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
     launch_ctl_init(q, G, m->c, h_iter, use_cond);
 }
 
@@ -165,8 +168,8 @@ void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial,
 
 void seq_trial(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_trial, int use_cond) {
     const Geom& G = m->G;
-    launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, B * C, 0, m->vol_std, m->vol_tr, G.V);
-    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->vol_std, m->vol_tr, G.V, m->p, m->c.proj_part);
+    launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, B * C, 1, m->vol, G.PV);
+    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
     launch_ctl_trial(q, G, m->c, h_trial, use_cond);
 }
 
@@ -269,7 +272,7 @@ int solve_impl(pcamm_model* m, int B, const float* y_dev, const float* angles, c
     if (volumes_out) {
         Seq q;
         q.stream = st;
-        launch_warp(q, G, m->f0, m->xbar, m->u, m->out_slots, m->c.solves, B, 1, volumes_out, nullptr, G.V);
+        launch_warp(q, G, m->f0, m->xbar, m->u, m->out_slots, B, 0, volumes_out, G.V);
         if ((rc = check_seq(q, "final warp"))) return rc;
     }
     CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState) * B, cudaMemcpyDeviceToHost, st));
@@ -377,7 +380,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     if (g->K < 1 || g->K > KMAX) return invalid("K outside [1, PCAMM_KMAX]");
     if (n_landmarks < 0 || (n_landmarks > 0 && !landmarks_mm_host)) return invalid("landmarks");
     const long long V = (long long)g->nx * g->ny * g->nz;
-    if (V >= (1LL << 31) || (long long)g->nu * g->nv >= (1LL << 31)) return invalid("volume or detector too large");
+    if ((long long)(g->nx + 2) * (g->ny + 2) * g->nz >= (1LL << 31) || (long long)g->nu * g->nv >= (1LL << 31)) return invalid("volume or detector too large");
     const int Bmax = g->max_batch < 1 ? 1 : g->max_batch;
     const int Cmax = g->max_candidates < 1 ? 1 : g->max_candidates;
     if (Cmax > MAXBT || Bmax > 4096) return invalid("max_batch / max_candidates too large");
@@ -399,6 +402,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     m->M = n_landmarks; m->Bmax = Bmax; m->Cmax = Cmax; m->S = Bmax * Cmax;
     Geom& G = m->G;
     G.nx = g->nx; G.ny = g->ny; G.nz = g->nz; G.V = V;
+    G.pnx = g->nx + 2; G.pny = g->ny + 2; G.PV = (long long)G.pnx * G.pny * g->nz;
     G.hx = g->hx; G.hy = g->hy; G.hz = g->hz;
     G.ihx = 1.f / g->hx; G.ihy = 1.f / g->hy; G.ihz = 1.f / g->hz;
     G.cx = g->cx; G.cy = g->cy; G.cz = g->cz;
@@ -419,7 +423,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return r == cudaSuccess; };
     ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->xbar, 3 * (size_t)V)) &&
         ok(dalloc(m, &m->u, 3 * (size_t)V * G.K)) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
-        ok(dalloc(m, &m->vol_std, S * V)) && ok(dalloc(m, &m->vol_tr, S * V)) && ok(dalloc(m, &m->p, S * G.npix)) &&
+        ok(dalloc(m, &m->vol, S * (size_t)G.PV)) && ok(dalloc(m, &m->col_hdr, B * G.nu)) &&
+        ok(dalloc(m, &m->slab_tab, B * G.nu * (size_t)max_slabs(G))) && ok(dalloc(m, &m->p, S * G.npix)) &&
         ok(dalloc(m, &m->rL, B * G.npix)) && ok(dalloc(m, &m->utab, B * G.nu)) && ok(dalloc(m, &m->vtab, B * G.nv)) &&
         ok(dalloc(m, &m->in_block, m->in_block_bytes)) && ok(dalloc(m, &m->c.solves, B)) &&
         ok(dalloc(m, &m->c.traces, B)) && ok(dalloc(m, &m->c.slots, S)) && ok(dalloc(m, &m->c.flags, 1)) &&
@@ -459,6 +464,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     TRY_OR_FAIL(cudaMemcpyAsync(m->u, eig_dvf_dev, sizeof(float) * 3 * V * G.K, cudaMemcpyDeviceToDevice, st));
     if (m->M > 0)
         TRY_OR_FAIL(cudaMemcpyAsync(m->lm0, landmarks_mm_host, sizeof(float) * 3 * m->M, cudaMemcpyHostToDevice, st));
+    TRY_OR_FAIL(cudaMemsetAsync(m->vol, 0, sizeof(float) * S * (size_t)G.PV, st));   // zero border, never written
     TRY_OR_FAIL(cudaMemsetAsync(m->nonfinite, 0, sizeof(unsigned long long), st));
     TRY_OR_FAIL(cudaMemsetAsync(m->c.solves, 0, sizeof(SolveState) * B, st));
     TRY_OR_FAIL(cudaMemsetAsync(m->c.slots, 0, sizeof(SlotState) * S, st));
@@ -513,7 +519,7 @@ int pcamm_warp(pcamm_model* m, const float* w_host, float* volume_out_dev, void*
     Seq q;
     int rc = hook_begin(m, nullptr, 0.f, w_host, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
-    launch_warp(q, m->G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, 1, 1, volume_out_dev, nullptr, m->G.V);
+    launch_warp(q, m->G, m->f0, m->xbar, m->u, m->c.slots, 1, 0, volume_out_dev, m->G.V);
     if ((rc = check_seq(q, "warp"))) return rc;
     CUDA_TRY(cudaStreamSynchronize(st));
     return PCAMM_OK;
@@ -525,8 +531,9 @@ int pcamm_project(pcamm_model* m, const float* volume_dev, float angle_rad, floa
     Seq q;
     int rc = hook_begin(m, nullptr, angle_rad, nullptr, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
-    launch_transpose(q, m->G, volume_dev, m->vol_tr);
-    launch_project(q, m->G, m->c.slots, m->c.solves, m->c.in, 1, volume_dev, m->vol_tr, m->G.V, m->p, m->c.proj_part);
+    launch_view_tables(q, m->G, m->c.solves, 1, m->col_hdr, m->slab_tab);
+    launch_to_ray_layout(q, m->G, volume_dev, m->vol);
+    launch_project(q, m->G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
     if ((rc = check_seq(q, "project"))) return rc;
     CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * m->G.npix, cudaMemcpyDeviceToDevice, st));
     CUDA_TRY(cudaStreamSynchronize(st));
@@ -555,8 +562,9 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     int rc = hook_begin(m, y_dev, angle_rad, w_host, a, b, 1, st, q2);
     if (rc) return rc;
     launch_ysums(q2, G, m->c, 1);
-    launch_warp(q2, G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, 1, 0, m->vol_std, m->vol_tr, G.V);
-    launch_project(q2, G, m->c.slots, m->c.solves, m->c.in, 1, m->vol_std, m->vol_tr, G.V, m->p, m->c.proj_part);
+    launch_view_tables(q2, G, m->c.solves, 1, m->col_hdr, m->slab_tab);
+    launch_warp(q2, G, m->f0, m->xbar, m->u, m->c.slots, 1, 1, m->vol, G.PV);
+    launch_project(q2, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
     launch_ctl_eval(q2, G, m->c, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
     launch_grad(q2, G, m->f0, m->xbar, m->u, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
@@ -581,7 +589,8 @@ int pcamm_traverse(pcamm_model* m, float angle_rad, int32_t iu, int32_t iv, int3
     int rc = hook_begin(m, nullptr, angle_rad, nullptr, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
     const int dcap = cap < m->trav_cap ? cap : m->trav_cap;
-    launch_traverse(q, m->G, m->c.solves, iu, iv, dcap, m->trav_ijk, m->trav_len, m->trav_n);
+    launch_view_tables(q, m->G, m->c.solves, 1, m->col_hdr, m->slab_tab);
+    launch_traverse(q, m->G, m->col_hdr, m->slab_tab, iu, iv, dcap, m->trav_ijk, m->trav_len, m->trav_n);
     if ((rc = check_seq(q, "traverse"))) return rc;
     int* h = m->h_trav;
     CUDA_TRY(cudaMemcpyAsync(h, m->trav_n, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -631,9 +640,9 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
     CUDA_TRY(cudaEventRecord(m->ev0, st));
     for (int i = 0; i < reps; ++i) {
         if (which == 0)
-            launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, m->c.solves, 1, 0, m->vol_std, m->vol_tr, G.V);
+            launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, 1, 1, m->vol, G.PV);
         else if (which == 1)
-            launch_project(q, G, m->c.slots, m->c.solves, m->c.in, 1, m->vol_std, m->vol_tr, G.V, m->p, m->c.proj_part);
+            launch_project(q, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
         else
             launch_grad(q, G, m->f0, m->xbar, m->u, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
     }

@@ -20,6 +20,8 @@ constexpr int TRACE_CAP = 1024;  // iterations recorded in the device-side trace
 struct Geom {
     int nx, ny, nz;
     long long V;
+    int pnx, pny;             // in-plane size of a ray-layout volume: nx + 2, ny + 2 (zero border)
+    long long PV;             // elements of one ray-layout volume: pnx * pny * nz
     float hx, hy, hz;
     float ihx, ihy, ihz;      // 1 / h
     float cx, cy, cz;         // world position of the volume centre
@@ -30,12 +32,35 @@ struct Geom {
 };
 
 // Angle-dependent part of the geometry of one solve, computed on the device in double.
-// layout bit 0: some ray of this view marches along y and reads the standard volume [z][y][x];
-// layout bit 1: some ray marches along x and reads the in-plane transposed volume [z][x][y].
 struct View {
     double cs, sn;
-    int layout;
-    int pad;
+};
+
+// Ray layout of a trial volume (what the projector reads): z fastest, one voxel of zero border
+// in x and y,   element (x, y, z) at ((y + 1) * pnx + (x + 1)) * nz + z.
+// All rays of one detector column share their in-plane path, so a warp takes 32 consecutive
+// detector rows of one column: its lanes sit in the same (x, y) voxel column and read
+// neighbouring z, i.e. one or two 128 B lines per load, whatever the gantry angle.
+__host__ __device__ __forceinline__ long long ray_layout_index(const Geom& G, int x, int y, int z) {
+    return ((long long)(y + 1) * G.pnx + (x + 1)) * G.nz + z;
+}
+
+// Per view and detector column: the in-plane part of the slab traversal (project.cu).
+struct ColHdr {
+    double lam0;              // (M_b - S_m) / g_m at the entry plane of the first slab
+    double kap;               // 1 / |g_m|: ray parameter per slab, in units of (D - S) per voxel
+    float dxy2;               // in-plane part of |D - S|^2, mm^2
+    int n_slabs;              // slabs in which the column's rays can be inside the volume in-plane
+    int dT;                   // element offset to the next voxel across a transverse plane
+    int axis;                 // 0: marches along x, 1: along y
+};
+
+// Per view, column and slab: element offset of the voxel column (i, j) the ray is in when it
+// enters the slab, and the share tt of the slab's path before the transverse plane crossing
+// (1 if none in this slab).
+struct SlabEntry {
+    int off0;
+    float tt;
 };
 
 // Host -> device, one copy per call.

@@ -50,20 +50,6 @@ __device__ bool lsfit(double n, double Sy, double Syy, double Sp, double Syp, do
 __device__ void set_view(const Geom& G, float angle, View* vw) {
     const double th = (double)angle;
     vw->cs = cos(th); vw->sn = sin(th);
-    // which marching axes occur among the rays of this view: |d_x|/h_x >= |d_y|/h_y marches x.
-    // The ratio is monotone in u between its ends unless an axis direction lies inside the fan,
-    // in which case both ends are on the same side of 1 anyway.
-    double dx0, dy0, dx1, dy1;
-    ray_dir_inplane(G, vw->cs, vw->sn, 0, &dx0, &dy0);
-    ray_dir_inplane(G, vw->cs, vw->sn, G.nu - 1, &dx1, &dy1);
-    const double ax0 = fabs(dx0) / (double)G.hx, ay0 = fabs(dy0) / (double)G.hy;
-    const double ax1 = fabs(dx1) / (double)G.hx, ay1 = fabs(dy1) / (double)G.hy;
-    const double eps = 1e-9;
-    int layout = 0;
-    if (ax0 >= ay0 * (1.0 - eps) || ax1 >= ay1 * (1.0 - eps)) layout |= 2;   // some ray marches x
-    if (ax0 <= ay0 * (1.0 + eps) || ax1 <= ay1 * (1.0 + eps)) layout |= 1;   // some ray marches y
-    vw->layout = layout;
-    vw->pad = 0;
 }
 
 __device__ void trial_w(const SolveState& st, int K, double mu, SlotState* sl) {

@@ -73,21 +73,25 @@ struct Seq {
 };
 
 // ---- a-1 (warp.cu)
+// f[s] = warp(f0, xbar + U w[s]) for every active slot; ray_layout: the z-fastest layout the
+// projector reads (slot stride G.PV), else the standard [z][y][x] (slot stride G.V).
 void launch_warp(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SlotState* slots,
-                 const SolveState* solves, int nslots, int force_layout, float* vol_std, float* vol_tr,
-                 long long slot_stride);
+                 int nslots, int ray_layout, float* vol_out, long long slot_stride);
 
 // ---- a-2 (project.cu)
 int project_blocks(const Geom& G);
-// p[s] = P f[s] for every active slot; per-block partial sums {sum p, sum y p, sum (p - a y - b)^2}.
+int max_slabs(const Geom& G);
+// in-plane traversal tables of the views of solves 0..B-1 (once per solve: the angle is fixed)
+void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, ColHdr* hdr, SlabEntry* tab);
+// p[s] = P f[s] for every active slot (volumes in the ray layout); per-block partial sums
+// {sum p, sum y p, sum (p - a y - b)^2}.
 void launch_project(Seq& q, const Geom& G, const SlotState* slots, const SolveState* solves, const SolveIn* in,
-                    int nslots, const float* vol_std, const float* vol_tr, long long slot_stride, float* p,
+                    int nslots, const ColHdr* hdr, const SlabEntry* tab, const float* vol, float* p,
                     double* partials);
-// hook: project a caller volume in standard layout at the view of solve 0 (transposes on the fly
-// into vol_tr if that view needs it).
-void launch_transpose(Seq& q, const Geom& G, const float* vol_std, float* vol_tr);
-void launch_traverse(Seq& q, const Geom& G, const SolveState* solves, int iu, int iv, int cap, int* ijk, float* len,
-                     int* n_out);
+// hooks: standard layout -> ray layout; one ray of the view of solve 0
+void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray);
+void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* tab, int iu, int iv, int cap,
+                     int* ijk, float* len, int* n_out);
 
 // ---- a-3 / a-4 (gradient.cu)
 int resid_blocks(const Geom& G);

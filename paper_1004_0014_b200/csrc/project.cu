@@ -9,17 +9,22 @@
 //   axis).  Between the planes M = i and M = i+1 (voxel-corner index units) it moves by
 //   |sT| <= 1 voxels in t and |sZ| <= 1 voxels in z, so it crosses at most one t-plane and one
 //   z-plane inside the slab: at most three voxels, whose shares tau of the slab length follow
-//   from where those two crossings fall.  Summed over slabs this is exactly Siddon's sum; most
-//   slabs hold a single voxel (one load, one add) and neighbouring rays read neighbouring
-//   addresses.
+//   from where those two crossings fall.  Summed over slabs this is exactly Siddon's sum.
 //
-// Layout: rays marching along y read the standard volume [z][y][x] (t = x is contiguous), rays
-// marching along x read the in-plane transposed copy [z][x][y] (t = y contiguous), both written
-// by the warp kernel.  One thread per ray, one warp per 32 consecutive u of a detector row, a
-// block per 32 x 8 detector tile: a warp's loads of one slab fall into one or two 128 B lines.
+// Split of the work.  On a flat detector whose rows are parallel to the rotation axis, all rays
+// of one detector column share their in-plane path; the gantry angle is fixed for the whole
+// solve (P varies per angle, not per iteration).  So the in-plane traversal is
+// tabulated ONCE per solve (k_view_tables: per column and slab the voxel column the ray is in
+// and the share tt of the slab before its t-plane crossing, evaluated directly in double), and
+// the projector, which runs once per line-search trial, only tracks the z crossings per ray (32.32
+// fixed-point counters set up in double) and accumulates at most three pieces per slab.
 //
-// Ray set-up (source, direction, entry, first crossings, crossing spacing) is done in double; the
-// march itself is integer (fixed-point crossing counters) plus one float multiply-add per piece.
+// Mapping: one thread per ray, one warp per 32 consecutive detector rows of ONE column.  The
+// lanes of a warp are in the same (x, y) voxel column and ~11 neighbouring z, so with the
+// z-fastest ray layout of the trial volumes (common.cuh) every load of a warp falls into one or
+// two 128 B lines at any gantry angle; the table entry of a slab is one broadcast 8-byte load;
+// the trip count is uniform over the warp.  The volume was just written by the warp kernel and is
+// L2/L1-resident: this kernel is bound by instruction issue, not by HBM.
 //
 // a-3 (first half): the same kernel forms r_i = p_i - a y_i - b and the per-block partial sums of
 // p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.
@@ -29,27 +34,112 @@ namespace pcamm {
 
 namespace {
 
-constexpr int TU = 32, TV = 8, NT = TU * TV;
-
-// One ray in the frame of its marching axis.  Slab n (n = 0 .. n_slabs-1, counted from the source
-// side) is the n-th voxel layer along the marching axis that the ray meets; q in [n, n+1] is the
-// ray parameter inside it.  The crossings of transverse (t) and axial (z) voxel planes are tracked
-// as 32.32 fixed-point values of q: hi word = slab in which the crossing falls, lo word = share of
-// that slab's path before it.  The first crossing and the spacing 1/|slope| come from the double
-// precision set-up, so that a crossing's slab and share do not depend on float rounding of a
-// position (for a ray almost parallel to a plane family that rounding, divided by the slope,
-// would misplace the crossing by whole slabs).
-struct Ray {
-    int axis;                       // 0: marches along x (reads [z][x][y]); 1: along y (reads [z][y][x])
-    int i_start, n_slabs, step;     // first layer index, count, +1 / -1
-    int Nm, Nt, Nz;
-    int j0, k0, dirT, dirZ;         // voxel of the entry point; direction of change at a crossing
-    unsigned long long QT, dQT, QZ, dQZ;
-    float Ls;                       // mm of path per slab
-};
+constexpr int PW = 4;             // warps (= detector columns) per block
+constexpr int NT = 32 * PW;
 
 constexpr double FIX = 4294967296.0;            // 2^32
 constexpr double QMAX = 1073741824.0;           // crossings beyond any volume are parked here (2^30 slabs)
+
+// ------------------------------------------------------------------ per-view tables (once per solve)
+
+struct ColSetup {
+    int axis, Nm, Nt, step, dirT, n_slabs, i_start;
+    double sT, T0, Mb, gm, Sm;
+};
+
+__device__ __forceinline__ ColSetup col_setup(const Geom& G, const View& vw, int iu, double* dxy2) {
+    ColSetup c;
+    double dx, dy;
+    ray_dir_inplane(G, vw.cs, vw.sn, iu, &dx, &dy);                       // D - S, in-plane
+    *dxy2 = dx * dx + dy * dy;
+    const double Sx = (double)G.sad * vw.cs, Sy = (double)G.sad * vw.sn;
+    const double gx = dx / (double)G.hx, gy = dy / (double)G.hy;
+    const double Sxi = (Sx - G.lox) / (double)G.hx, Syi = (Sy - G.loy) / (double)G.hy;
+    double gt, St;
+    if (fabs(gx) >= fabs(gy)) { c.axis = 0; c.gm = gx; gt = gy; c.Sm = Sxi; St = Syi; c.Nm = G.nx; c.Nt = G.ny; }
+    else                      { c.axis = 1; c.gm = gy; gt = gx; c.Sm = Syi; St = Sxi; c.Nm = G.ny; c.Nt = G.nx; }
+    c.sT = gt / c.gm;                                   // t per unit of the marching coordinate M
+    c.T0 = St - c.Sm * c.sT;                            // t at the plane M = 0
+    c.step = c.gm > 0.0 ? 1 : -1;
+    const double s = c.sT * c.step;
+    c.dirT = s > 0.0 ? 1 : (s < 0.0 ? -1 : 0);
+    // layers in which the in-plane ray overlaps [0, Nt): analytic range, widened by one, then
+    // shrunk with the same expression the entries use
+    double Mlo = 0.0, Mhi = (double)c.Nm;
+    bool empty = false;
+    if (c.sT != 0.0) {
+        const double m0 = (0.0 - c.T0) / c.sT, m1 = ((double)c.Nt - c.T0) / c.sT;
+        Mlo = fmax(Mlo, fmin(m0, m1)); Mhi = fmin(Mhi, fmax(m0, m1));
+    } else if (!(c.T0 >= 0.0 && c.T0 < (double)c.Nt)) empty = true;
+    int ifirst = (int)floor(Mlo) - 1, ilast = (int)ceil(Mhi);
+    ifirst = max(ifirst, 0); ilast = min(ilast, c.Nm - 1);
+    if (empty || !(Mlo <= Mhi)) ilast = ifirst - 1;
+    auto Tat = [&](int M) { return fma(c.sT, (double)M, c.T0); };
+    auto incl = [&](int i) {
+        const double a = Tat(i), b = Tat(i + 1);
+        return fmax(a, b) >= 0.0 && fmin(a, b) < (double)c.Nt;
+    };
+    while (ifirst <= ilast && !incl(ifirst)) ++ifirst;
+    while (ilast >= ifirst && !incl(ilast)) --ilast;
+    c.n_slabs = max(ilast - ifirst + 1, 0);
+    c.i_start = c.step > 0 ? ifirst : ilast;
+    c.Mb = c.step > 0 ? (double)ifirst : (double)(ilast + 1);            // entry plane of the first slab
+    return c;
+}
+
+// grid (nu, B); the threads of a block share the column and take slabs n = tid, tid + NT, ...
+__global__ void __launch_bounds__(128)
+k_view_tables(const Geom G, const SolveState* __restrict__ solves, ColHdr* __restrict__ hdr,
+              SlabEntry* __restrict__ tab, int max_slabs) {
+    const int iu = blockIdx.x, b = blockIdx.y;
+    const View vw = solves[b].view;
+    double dxy2;
+    const ColSetup c = col_setup(G, vw, iu, &dxy2);
+    const int strideT = (c.axis == 0 ? G.pnx : 1) * G.nz;
+    if (threadIdx.x == 0) {
+        ColHdr h;
+        h.lam0 = (c.Mb - c.Sm) / c.gm;
+        h.kap = 1.0 / fabs(c.gm);
+        h.dxy2 = (float)dxy2;
+        h.n_slabs = c.n_slabs;
+        h.dT = c.dirT * strideT;
+        h.axis = c.axis;
+        hdr[(long long)b * G.nu + iu] = h;
+    }
+    SlabEntry* row = tab + ((long long)b * G.nu + iu) * max_slabs;
+    const double s = c.sT * c.step;
+    for (int n = threadIdx.x; n < c.n_slabs; n += blockDim.x) {
+        const int Me = (int)c.Mb + c.step * n;                    // plane through which the slab is entered
+        const int i = c.i_start + c.step * n;                     // layer index of the slab
+        const double Te = fma(c.sT, (double)Me, c.T0), Tx = fma(c.sT, (double)(Me + c.step), c.T0);
+        const double fl = floor(Te);
+        const int j = (int)fl;
+        double tt = 1.0;
+        if (s > 0.0) { if (Tx >= fl + 1.0) tt = (fl + 1.0 - Te) / s; }
+        else if (s < 0.0) { if (Tx < fl) tt = (fl - Te) / s; }
+        tt = fmin(fmax(tt, 0.0), 1.0);
+        const int jx = c.axis == 0 ? i : j, jy = c.axis == 0 ? j : i;
+        SlabEntry e;
+        e.off0 = ((jy + 1) * G.pnx + (jx + 1)) * G.nz;
+        e.tt = (float)tt;
+        row[n] = e;
+    }
+}
+
+// ------------------------------------------------------------------ per-ray z tracking and the march
+
+// The crossings of axial (z) voxel planes are tracked as 32.32 fixed-point values of the slab
+// coordinate q: hi word = slab in which the crossing falls, lo word = share of that slab's path
+// before it.  The first crossing and the spacing 1/|slope| come from a double precision set-up,
+// so that a crossing's slab and share do not depend on float rounding of a position (for a ray
+// almost parallel to the planes that rounding, divided by the slope, would misplace the crossing
+// by whole slabs).
+struct RayZ {
+    int k, dirZ;
+    unsigned long long QZ, dQZ;
+    float Ls;                       // mm of path per slab
+    int kmin, kmax;                 // bounds of the axial indices met in n_slabs slabs
+};
 
 __device__ __forceinline__ void first_crossing(double P0, double s, int* idx0, int* dir, unsigned long long* Q,
                                                unsigned long long* dQ) {
@@ -65,101 +155,89 @@ __device__ __forceinline__ void first_crossing(double P0, double s, int* idx0, i
     if (*dQ < (1ull << 32)) *dQ = 1ull << 32;   // |s| <= 1: never two crossings in one slab
 }
 
-__device__ __forceinline__ Ray make_ray(const Geom& G, const View& vw, int iu, int iv) {
-    Ray r;
-    double dx, dy;
-    ray_dir_inplane(G, vw.cs, vw.sn, iu, &dx, &dy);                       // D - S
+__device__ __forceinline__ RayZ make_ray_z(const Geom& G, const ColHdr& h, int iv) {
+    RayZ r;
     const double dz = ((double)iv - 0.5 * (G.nv - 1) + (double)G.off_v) * (double)G.pv;
-    const double Sx = (double)G.sad * vw.cs, Sy = (double)G.sad * vw.sn;
-    const double L = sqrt(dx * dx + dy * dy + dz * dz);
-    const double gx = dx / (double)G.hx, gy = dy / (double)G.hy, gz = dz / (double)G.hz;
-    const double Sxi = (Sx - G.lox) / (double)G.hx, Syi = (Sy - G.loy) / (double)G.hy, Szi = (0.0 - G.loz) / (double)G.hz;
-    double gm, gt, Sm, St;
-    if (fabs(gx) >= fabs(gy)) { r.axis = 0; gm = gx; gt = gy; Sm = Sxi; St = Syi; r.Nm = G.nx; r.Nt = G.ny; }
-    else                      { r.axis = 1; gm = gy; gt = gx; Sm = Syi; St = Sxi; r.Nm = G.ny; r.Nt = G.nx; }
-    r.Nz = G.nz;
-    const double sT = gt / gm, sZ = gz / gm;            // per unit of the marching coordinate M
-    const double T0 = St - Sm * sT, Z0 = Szi - Sm * sZ; // at the plane M = 0
-    r.step = gm > 0.0 ? 1 : -1;
-    r.Ls = (float)(L / fabs(gm));
-    // layers in which the ray can be inside the volume (conservative by one; exactness comes from
-    // the per-voxel range test in the sink)
-    double Mlo = 0.0, Mhi = (double)r.Nm;
-    bool empty = false;
-    if (sT != 0.0) {
-        const double m0 = (0.0 - T0) / sT, m1 = ((double)r.Nt - T0) / sT;
-        Mlo = fmax(Mlo, fmin(m0, m1)); Mhi = fmin(Mhi, fmax(m0, m1));
-    } else if (!(T0 >= 0.0 && T0 < (double)r.Nt)) empty = true;
-    if (sZ != 0.0) {
-        const double m0 = (0.0 - Z0) / sZ, m1 = ((double)r.Nz - Z0) / sZ;
-        Mlo = fmax(Mlo, fmin(m0, m1)); Mhi = fmin(Mhi, fmax(m0, m1));
-    } else if (!(Z0 >= 0.0 && Z0 < (double)r.Nz)) empty = true;
-    int ifirst = (int)floor(Mlo) - 1, ilast = (int)ceil(Mhi);
-    ifirst = max(ifirst, 0); ilast = min(ilast, r.Nm - 1);
-    r.n_slabs = 0; r.i_start = 0; r.j0 = r.k0 = r.dirT = r.dirZ = 0; r.QT = r.dQT = r.QZ = r.dQZ = 0ull;
-    if (empty || !(Mlo <= Mhi) || ilast < ifirst) return r;
-    r.n_slabs = ilast - ifirst + 1;
-    r.i_start = r.step > 0 ? ifirst : ilast;
-    const double Mb = r.step > 0 ? (double)ifirst : (double)(ilast + 1);   // entry plane of the first slab
-    first_crossing(T0 + sT * Mb, sT * r.step, &r.j0, &r.dirT, &r.QT, &r.dQT);
-    first_crossing(Z0 + sZ * Mb, sZ * r.step, &r.k0, &r.dirZ, &r.QZ, &r.dQZ);
+    const double gz = dz / (double)G.hz;
+    const double Szi = (0.0 - G.loz) / (double)G.hz;                      // the source is in the plane z = 0
+    const double sz = gz * h.kap;                                         // z per slab
+    first_crossing(fma(gz, h.lam0, Szi), sz, &r.k, &r.dirZ, &r.QZ, &r.dQZ);
+    r.Ls = (float)(sqrt((double)h.dxy2 + dz * dz) * h.kap);
+    const int ncross = (int)(fabs(sz) * (double)h.n_slabs) + 2;           // conservative
+    r.kmin = r.dirZ < 0 ? r.k - ncross : r.k;
+    r.kmax = r.dirZ > 0 ? r.k + ncross : r.k;
     return r;
 }
 
-// Calls sink(i, j, k, tau) for every (layer i, transverse j, axial k) piece, source side first;
-// tau = share of the slab's path length.
+// Calls sink(off, k, tau) for every piece of every slab, source side first: off = element offset
+// of the voxel column (i, j), k the axial index, tau the share of the slab's path length.
+// Pieces of zero share are passed on (the sink ignores or drops them).
 template <class Sink>
-__device__ __forceinline__ void march(const Ray& r, Sink& sink) {
-    int i = r.i_start, j = r.j0, k = r.k0;
-    unsigned long long QT = r.QT, QZ = r.QZ;
+__device__ __forceinline__ void march(const SlabEntry* __restrict__ row, int n_slabs, int dT, RayZ r, Sink& sink) {
     const float inv32 = 2.3283064365386963e-10f;   // 2^-32
-    for (int n = 0; n < r.n_slabs; ++n, i += r.step) {
-        const bool ct = (unsigned)(QT >> 32) == (unsigned)n, cz = (unsigned)(QZ >> 32) == (unsigned)n;
-        if (!ct && !cz) { sink(i, j, k, 1.f); continue; }
-        const float tt = ct ? __uint2float_rn((unsigned)QT) * inv32 : 1.f;
+    int k = r.k;
+    unsigned long long QZ = r.QZ;
+#pragma unroll 4
+    for (int n = 0; n < n_slabs; ++n) {
+        const int2 e = __ldg(reinterpret_cast<const int2*>(row) + n);
+        const int off0 = e.x, off1 = e.x + dT;
+        const float tt = __int_as_float(e.y);
+        const bool cz = (unsigned)(QZ >> 32) == (unsigned)n;
         const float tz = cz ? __uint2float_rn((unsigned)QZ) * inv32 : 1.f;
-        const int je = ct ? j + r.dirT : j, ke = cz ? k + r.dirZ : k;
+        const int ke = cz ? k + r.dirZ : k;
         const float t1 = fminf(tt, tz), t2 = fmaxf(tt, tz);
-        sink(i, j, k, t1);
         const bool tfirst = tt < tz;
-        sink(i, tfirst ? je : j, tfirst ? k : ke, t2 - t1);
-        if (ct && cz) sink(i, je, ke, 1.f - t2);
-        j = je; k = ke;
-        if (ct) QT += r.dQT;
+        sink(off0, k, t1);
+        sink(tfirst ? off1 : off0, tfirst ? k : ke, t2 - t1);
+        sink(off1, ke, 1.f - t2);
+        k = ke;
         if (cz) QZ += r.dQZ;
     }
 }
 
+// CHECK = false: the caller has established that the ray stays inside [0, nz) for the whole
+// march (no per-piece test).
+template <bool CHECK>
 struct AccSink {
     const float* __restrict__ vol;
-    int Nm, Nt, Nz;
+    int Nz;
     float acc;
-    __device__ __forceinline__ void operator()(int i, int j, int k, float tau) {
-        if ((unsigned)j < (unsigned)Nt && (unsigned)k < (unsigned)Nz)
-            acc = fmaf(tau, __ldg(vol + (k * Nm + i) * Nt + j), acc);
+    __device__ __forceinline__ void operator()(int off, int k, float tau) {
+        if (!CHECK || (unsigned)k < (unsigned)Nz) acc = fmaf(tau, __ldg(vol + (unsigned)(off + k)), acc);
     }
 };
 
 __global__ void __launch_bounds__(NT)
 k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* __restrict__ solves,
-          const SolveIn* __restrict__ in, const float* __restrict__ vol_std, const float* __restrict__ vol_tr,
-          long long slot_stride, float* __restrict__ p_out, double* __restrict__ partials) {
+          const SolveIn* __restrict__ in, const ColHdr* __restrict__ hdr, const SlabEntry* __restrict__ tab,
+          int max_slabs, const float* __restrict__ vol, float* __restrict__ p_out, double* __restrict__ partials) {
     __shared__ double red[NT / 32];
     const int s = blockIdx.z;
     if (!slots[s].active) return;
     const int b = slots[s].solve;
-    const View vw = solves[b].view;
-    const int tiles_u = (G.nu + TU - 1) / TU;
-    const int iu = (blockIdx.x % tiles_u) * TU + (threadIdx.x & 31);
-    const int iv = (blockIdx.x / tiles_u) * TV + (threadIdx.x >> 5);
+    const int iu = blockIdx.x * PW + (threadIdx.x >> 5);
+    const int iv = blockIdx.y * 32 + (threadIdx.x & 31);
     double vp = 0.0, vyp = 0.0, vrr = 0.0;
     if (iu < G.nu && iv < G.nv) {
-        const Ray r = make_ray(G, vw, iu, iv);
-        AccSink sink;
-        sink.vol = (r.axis == 0 ? vol_tr : vol_std) + (long long)s * slot_stride;
-        sink.Nm = r.Nm; sink.Nt = r.Nt; sink.Nz = r.Nz; sink.acc = 0.f;
-        march(r, sink);
-        const float p = sink.acc * r.Ls;
+        const ColHdr h = hdr[(long long)b * G.nu + iu];
+        float p = 0.f;
+        if (h.n_slabs > 0) {
+            const RayZ r = make_ray_z(G, h, iv);
+            const SlabEntry* row = tab + ((long long)b * G.nu + iu) * max_slabs;
+            const float* base = vol + (long long)s * G.PV;
+            asm volatile("" : "+l"(base));       // one base pointer; 32-bit offsets in the loop
+            float acc;
+            if (r.kmin >= 0 && r.kmax < G.nz) {
+                AccSink<false> sink{base, G.nz, 0.f};
+                march(row, h.n_slabs, h.dT, r, sink);
+                acc = sink.acc;
+            } else {
+                AccSink<true> sink{base, G.nz, 0.f};
+                march(row, h.n_slabs, h.dT, r, sink);
+                acc = sink.acc;
+            }
+            p = acc * r.Ls;
+        }
         const int pix = iv * G.nu + iu;
         p_out[(long long)s * G.npix + pix] = p;
         const float* y = in[b].y;
@@ -167,47 +245,50 @@ k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* _
         const double res = (double)p - solves[b].a * yv - solves[b].b;   // Eq. (2) residual
         vp = (double)p; vyp = yv * (double)p; vrr = res * res;
     }
-    const int nblk = gridDim.x;
-    double* out = partials + ((long long)s * nblk + blockIdx.x) * 3;
+    const int nblk = gridDim.x * gridDim.y;
+    const int blk = blockIdx.y * gridDim.x + blockIdx.x;
+    double* out = partials + ((long long)s * nblk + blk) * 3;
     const double sp = block_sum<NT>(vp, red);
     const double syp = block_sum<NT>(vyp, red);
     const double srr = block_sum<NT>(vrr, red);
     if (threadIdx.x == 0) { out[0] = sp; out[1] = syp; out[2] = srr; }
 }
 
-// In-plane transpose [z][y][x] -> [z][x][y] (hook path only: the solve's volumes are written in
-// both layouts by the warp kernel).
+// Standard [z][y][x] -> ray layout (hook path only: the solve's volumes are written in the ray
+// layout by the warp kernel).  Tile: 32 x by 32 z at fixed y.
 __global__ void __launch_bounds__(256)
-k_transpose(const Geom G, const float* __restrict__ src, float* __restrict__ dst) {
+k_to_ray_layout(const Geom G, const float* __restrict__ src, float* __restrict__ dst) {
     __shared__ float tile[32][33];
-    const int lane = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32, z = blockIdx.z;
+    const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
+    const int x0 = blockIdx.x * 32, z0 = blockIdx.y * 32, y = blockIdx.z;
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-        const int y = y0 + ty + 8 * r, x = x0 + lane;
-        tile[ty + 8 * r][lane] = (x < G.nx && y < G.ny) ? src[((long long)z * G.ny + y) * G.nx + x] : 0.f;
+        const int z = z0 + tw + 8 * r, x = x0 + lane;
+        tile[tw + 8 * r][lane] = (x < G.nx && z < G.nz) ? src[((long long)z * G.ny + y) * G.nx + x] : 0.f;
     }
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-        const int x = x0 + ty + 8 * r, y = y0 + lane;
-        if (x < G.nx && y < G.ny) dst[((long long)z * G.nx + x) * G.ny + y] = tile[lane][ty + 8 * r];
+        const int x = x0 + tw + 8 * r, z = z0 + lane;
+        if (x < G.nx && z < G.nz) dst[ray_layout_index(G, x, y, z)] = tile[lane][tw + 8 * r];
     }
 }
 
 struct RecSink {
-    int axis, cap, n;
-    int Nt, Nz;
+    int cap, n;
+    int nx, ny, nz, pnx;
     float Ls, eps;
     int* ijk;
     float* len;
-    __device__ __forceinline__ void operator()(int i, int j, int k, float tau) {
-        if (!((unsigned)j < (unsigned)Nt && (unsigned)k < (unsigned)Nz)) return;
+    __device__ __forceinline__ void operator()(int off, int k, float tau) {
+        if (!((unsigned)k < (unsigned)nz)) return;
+        const int col = off / nz, jy = col / pnx - 1, jx = col % pnx - 1;
+        if (!((unsigned)jx < (unsigned)nx && (unsigned)jy < (unsigned)ny)) return;      // zero border
         const float l = tau * Ls;
         if (!(l > eps)) return;     // zero-length pieces are dropped (reading A22)
         if (n < cap) {
-            ijk[3 * n + 0] = axis == 0 ? i : j;
-            ijk[3 * n + 1] = axis == 0 ? j : i;
+            ijk[3 * n + 0] = jx;
+            ijk[3 * n + 1] = jy;
             ijk[3 * n + 2] = k;
             len[n] = l;
         }
@@ -215,36 +296,47 @@ struct RecSink {
     }
 };
 
-__global__ void k_traverse(const Geom G, const SolveState* __restrict__ solves, int iu, int iv, int cap, int* ijk,
-                           float* len, int* n_out) {
+// One ray through the projector's own tables and march (pcamm_traverse).
+__global__ void k_traverse(const Geom G, const ColHdr* __restrict__ hdr, const SlabEntry* __restrict__ tab,
+                           int max_slabs, int iu, int iv, int cap, int* ijk, float* len, int* n_out) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    const Ray r = make_ray(G, solves[0].view, iu, iv);
+    const ColHdr h = hdr[iu];
     RecSink sink;
-    sink.axis = r.axis; sink.cap = cap; sink.n = 0; sink.Nt = r.Nt; sink.Nz = r.Nz; sink.Ls = r.Ls;
+    sink.cap = cap; sink.n = 0; sink.nx = G.nx; sink.ny = G.ny; sink.nz = G.nz; sink.pnx = G.pnx;
     sink.eps = 1e-6f * fminf(G.hx, fminf(G.hy, G.hz));
+    sink.Ls = 0.f;
     sink.ijk = ijk; sink.len = len;
-    march(r, sink);
+    if (h.n_slabs > 0) {
+        const RayZ r = make_ray_z(G, h, iv);
+        sink.Ls = r.Ls;
+        march(tab + (long long)iu * max_slabs, h.n_slabs, h.dT, r, sink);
+    }
     *n_out = sink.n;
 }
 
 }  // namespace
 
-int project_blocks(const Geom& G) { return ((G.nu + TU - 1) / TU) * ((G.nv + TV - 1) / TV); }
+int project_blocks(const Geom& G) { return ((G.nu + PW - 1) / PW) * ((G.nv + 31) / 32); }
+int max_slabs(const Geom& G) { return G.nx > G.ny ? G.nx : G.ny; }
+
+void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, ColHdr* hdr, SlabEntry* tab) {
+    q.launch(k_view_tables, dim3(G.nu, B), dim3(128), 0, G, solves, hdr, tab, max_slabs(G));
+}
 
 void launch_project(Seq& q, const Geom& G, const SlotState* slots, const SolveState* solves, const SolveIn* in,
-                    int nslots, const float* vol_std, const float* vol_tr, long long slot_stride, float* p,
+                    int nslots, const ColHdr* hdr, const SlabEntry* tab, const float* vol, float* p,
                     double* partials) {
-    q.launch(k_project, dim3(project_blocks(G), 1, nslots), dim3(NT), 0, G, slots, solves, in, vol_std, vol_tr,
-             slot_stride, p, partials);
+    q.launch(k_project, dim3((G.nu + PW - 1) / PW, (G.nv + 31) / 32, nslots), dim3(NT), 0, G, slots, solves, in, hdr,
+             tab, max_slabs(G), vol, p, partials);
 }
 
-void launch_transpose(Seq& q, const Geom& G, const float* vol_std, float* vol_tr) {
-    q.launch(k_transpose, dim3((G.nx + 31) / 32, (G.ny + 31) / 32, G.nz), dim3(256), 0, G, vol_std, vol_tr);
+void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray) {
+    q.launch(k_to_ray_layout, dim3((G.nx + 31) / 32, (G.nz + 31) / 32, G.ny), dim3(256), 0, G, vol_std, vol_ray);
 }
 
-void launch_traverse(Seq& q, const Geom& G, const SolveState* solves, int iu, int iv, int cap, int* ijk, float* len,
-                     int* n_out) {
-    q.launch(k_traverse, dim3(1), dim3(32), 0, G, solves, iu, iv, cap, ijk, len, n_out);
+void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* tab, int iu, int iv, int cap,
+                     int* ijk, float* len, int* n_out) {
+    q.launch(k_traverse, dim3(1), dim3(32), 0, G, hdr, tab, max_slabs(G), iu, iv, cap, ijk, len, n_out);
 }
 
 }  // namespace pcamm

@@ -9,11 +9,9 @@
 // into registers and the slot loop runs inside the thread.
 //
 // HBM layout: fields planar [3][V] / [K][3][V] exactly as the caller gave them; a warp reads 32
-// consecutive x of one row per load instruction (one 128 B line per plane and row), 12 (K+1)/...
-// independent lines in flight per thread.  The warped volume is written once per layout the
-// projector of that view needs: standard [z][y][x] (rays marching along y) and/or in-plane
-// transposed [z][x][y] (rays marching along x), the latter through a 32x33 shared-memory tile
-// so that both writes are full 128 B lines.
+// consecutive x of one row per load instruction (one 128 B line per plane and row).  The warped
+// volume is written once, in the z-fastest ray layout of common.cuh that the projector reads at
+// every gantry angle (or in the standard layout for the volume returned to the caller).
 #include "internal.h"
 
 namespace pcamm {
@@ -21,7 +19,7 @@ namespace pcamm {
 namespace {
 
 constexpr int TILE = 32;
-constexpr int ROWS = 4;        // voxels per thread (rows ty, ty+8, ty+16, ty+24 of the tile)
+constexpr int ROWS = 4;        // voxels per thread (z rows tw, tw+8, tw+16, tw+24 of the tile)
 constexpr int NTHREADS = 256;  // 32 x 8
 
 // f0 with zero padding outside the grid (reading A2).
@@ -60,14 +58,17 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ f0, int nx,
     return (r00 * Y0 + r10 * ty) * Z0 + (r01 * Y0 + r11 * ty) * tz;
 }
 
-template <int K>
+// Tile: 32 x by 32 z at fixed y.  Loads: lane = x (one 128 B line per plane and z).  Stores in the
+// ray layout (RAY = true, what the projector reads): lane = z, through a 32x33 shared-memory
+// tile, one 128 B line per (x, y); in the standard layout [z][y][x] (RAY = false: the volume
+// handed back to the caller): lane = x.
+template <int K, bool RAY>
 __global__ void __launch_bounds__(NTHREADS)
 k_warp(const Geom G, const float* __restrict__ f0, const float* __restrict__ xbar, const float* __restrict__ u,
-       const SlotState* __restrict__ slots, const SolveState* __restrict__ solves, int nslots, int force_layout,
-       float* __restrict__ vol_std, float* __restrict__ vol_tr, long long slot_stride) {
+       const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride) {
     __shared__ float tile[TILE][TILE + 1];
-    const int lane = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    const int x0 = blockIdx.x * TILE, y0 = blockIdx.y * TILE, z = blockIdx.z;
+    const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
+    const int x0 = blockIdx.x * TILE, z0 = blockIdx.y * TILE, y = blockIdx.z;
     const int x = x0 + lane;
     const long long V = G.V;
 
@@ -75,8 +76,8 @@ k_warp(const Geom G, const float* __restrict__ f0, const float* __restrict__ xba
     bool in[ROWS];
 #pragma unroll
     for (int r = 0; r < ROWS; ++r) {
-        const int y = y0 + ty + 8 * r;
-        in[r] = (x < G.nx) && (y < G.ny);
+        const int z = z0 + tw + 8 * r;
+        in[r] = (x < G.nx) && (z < G.nz);
         const long long lin = ((long long)z * G.ny + y) * G.nx + x;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -91,9 +92,7 @@ k_warp(const Geom G, const float* __restrict__ f0, const float* __restrict__ xba
         float w[K];
 #pragma unroll
         for (int k = 0; k < K; ++k) w[k] = slots[s].w[k];
-        const int layout = force_layout ? force_layout : solves[slots[s].solve].view.layout;
-        float* out_std = vol_std + (long long)s * slot_stride;
-        float* out_tr = vol_tr + (long long)s * slot_stride;
+        float* out = vol_out + (long long)s * slot_stride;
         float val[ROWS];
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
@@ -107,26 +106,24 @@ k_warp(const Geom G, const float* __restrict__ f0, const float* __restrict__ xba
                     for (int k = 0; k < K; ++k) xs = fmaf(uu[r][k][c], w[k], xs);
                     d[c] = xs;
                 }
-                const int y = y0 + ty + 8 * r;
-                val[r] = trilinear(f0, G.nx, G.ny, G.nz, x, y, z,
+                val[r] = trilinear(f0, G.nx, G.ny, G.nz, x, y, z0 + tw + 8 * r,
                                    __fdiv_rn(d[0], G.hx), __fdiv_rn(d[1], G.hy), __fdiv_rn(d[2], G.hz));
             }
         }
-        if (layout & 1) {
+        if (!RAY) {
 #pragma unroll
             for (int r = 0; r < ROWS; ++r)
-                if (in[r]) out_std[((long long)z * G.ny + (y0 + ty + 8 * r)) * G.nx + x] = val[r];
-        }
-        if (layout & 2) {
+                if (in[r]) out[((long long)(z0 + tw + 8 * r) * G.ny + y) * G.nx + x] = val[r];
+        } else {
             __syncthreads();
 #pragma unroll
-            for (int r = 0; r < ROWS; ++r) tile[ty + 8 * r][lane] = val[r];
+            for (int r = 0; r < ROWS; ++r) tile[tw + 8 * r][lane] = val[r];
             __syncthreads();
-            const int yo = y0 + lane;
+            const int zo = z0 + lane;
 #pragma unroll
             for (int r = 0; r < ROWS; ++r) {
-                const int xo = x0 + ty + 8 * r;
-                if (xo < G.nx && yo < G.ny) out_tr[((long long)z * G.nx + xo) * G.ny + yo] = tile[lane][ty + 8 * r];
+                const int xo = x0 + tw + 8 * r;
+                if (xo < G.nx && zo < G.nz) out[ray_layout_index(G, xo, y, zo)] = tile[lane][tw + 8 * r];
             }
         }
     }
@@ -134,21 +131,19 @@ k_warp(const Geom G, const float* __restrict__ f0, const float* __restrict__ xba
 
 template <int K>
 void launch_k(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SlotState* slots,
-              const SolveState* solves, int nslots, int force_layout, float* vol_std, float* vol_tr,
-              long long slot_stride) {
-    dim3 grid((G.nx + TILE - 1) / TILE, (G.ny + TILE - 1) / TILE, G.nz);
-    q.launch(k_warp<K>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, solves, nslots, force_layout, vol_std,
-             vol_tr, slot_stride);
+              int nslots, int ray_layout, float* vol_out, long long slot_stride) {
+    dim3 grid((G.nx + TILE - 1) / TILE, (G.nz + TILE - 1) / TILE, G.ny);
+    if (ray_layout) q.launch(k_warp<K, true>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride);
+    else q.launch(k_warp<K, false>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride);
 }
 
 }  // namespace
 
 void launch_warp(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SlotState* slots,
-                 const SolveState* solves, int nslots, int force_layout, float* vol_std, float* vol_tr,
-                 long long slot_stride) {
+                 int nslots, int ray_layout, float* vol_out, long long slot_stride) {
     switch (G.K) {
 #define PCAMM_CASE(KK) \
-    case KK: launch_k<KK>(q, G, f0, xbar, u, slots, solves, nslots, force_layout, vol_std, vol_tr, slot_stride); break;
+    case KK: launch_k<KK>(q, G, f0, xbar, u, slots, nslots, ray_layout, vol_out, slot_stride); break;
         PCAMM_CASE(1) PCAMM_CASE(2) PCAMM_CASE(3) PCAMM_CASE(4)
         PCAMM_CASE(5) PCAMM_CASE(6) PCAMM_CASE(7) PCAMM_CASE(8)
 #undef PCAMM_CASE

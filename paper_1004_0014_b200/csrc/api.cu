@@ -35,6 +35,31 @@ __global__ void k_count_nonfinite(const float* __restrict__ a, long long n, unsi
 }
 
 }  // namespace
+
+bool make_field_map(const Geom& G, const float* fields, int planes, int tz, CUtensorMap* out, std::string* why) {
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    if (G.nx % 4 != 0) { if (why) *why = "nx * 4 bytes is not a multiple of 16"; return false; }
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        if (why) *why = "cuTensorMapEncodeTiled is not available";
+        return false;
+    }
+    const cuuint64_t dims[4] = {(cuuint64_t)G.nx, (cuuint64_t)G.ny, (cuuint64_t)G.nz, (cuuint64_t)planes};
+    const cuuint64_t strides[3] = {(cuuint64_t)G.nx * 4, (cuuint64_t)G.nx * G.ny * 4, (cuuint64_t)G.V * 4};
+    const cuuint32_t box[4] = {(cuuint32_t)TX, 1u, (cuuint32_t)tz, (cuuint32_t)planes};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = ((EncodeFn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)fields, dims, strides, box, estr,
+                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                      CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { if (why) *why = "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")"; return false; }
+    return true;
+}
+
 }  // namespace pcamm
 
 using namespace pcamm;
@@ -44,7 +69,8 @@ struct pcamm_model {
     Geom G;
     int M = 0, Bmax = 1, Cmax = 1, S = 1;
     // model (device)
-    float *f0 = nullptr, *xbar = nullptr, *u = nullptr, *lm0 = nullptr;
+    float *f0 = nullptr, *fields = nullptr, *xbar = nullptr, *u = nullptr, *lm0 = nullptr;   // xbar, u: views of fields
+    FieldStream fs;
     // scratch (device)
     float *vol = nullptr, *p = nullptr, *rL = nullptr;   // vol: trial volumes, ray layout [S][PV]
     ColHdr* col_hdr = nullptr;      // [B][nu]
@@ -154,7 +180,7 @@ void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     launch_ysums(q, G, m->c, B);
     launch_begin(q, G, m->c, 0);
     launch_view_tables(q, G, m->c.solves, B, m->col_hdr, m->slab_tab);
-    launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, B * C, 1, m->vol, G.PV);
+    launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV);
     launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
     launch_ctl_init(q, G, m->c, h_iter, use_cond);
 }
@@ -168,7 +194,7 @@ void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial,
 
 void seq_trial(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_trial, int use_cond) {
     const Geom& G = m->G;
-    launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, B * C, 1, m->vol, G.PV);
+    launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV);
     launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
     launch_ctl_trial(q, G, m->c, h_trial, use_cond);
 }
@@ -272,7 +298,7 @@ int solve_impl(pcamm_model* m, int B, const float* y_dev, const float* angles, c
     if (volumes_out) {
         Seq q;
         q.stream = st;
-        launch_warp(q, G, m->f0, m->xbar, m->u, m->out_slots, B, 0, volumes_out, G.V);
+        launch_warp(q, G, m->fs, m->f0, m->out_slots, B, 0, volumes_out, G.V);
         if ((rc = check_seq(q, "final warp"))) return rc;
     }
     CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState) * B, cudaMemcpyDeviceToHost, st));
@@ -421,8 +447,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     m->trav_cap = G.nx + G.ny + G.nz + 8;
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return r == cudaSuccess; };
-    ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->xbar, 3 * (size_t)V)) &&
-        ok(dalloc(m, &m->u, 3 * (size_t)V * G.K)) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
+    ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->fields, 3 * (size_t)V * (G.K + 1))) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
         ok(dalloc(m, &m->vol, S * (size_t)G.PV)) && ok(dalloc(m, &m->col_hdr, B * G.nu)) &&
         ok(dalloc(m, &m->slab_tab, B * G.nu * (size_t)max_slabs(G))) && ok(dalloc(m, &m->p, S * G.npix)) &&
         ok(dalloc(m, &m->rL, B * G.npix)) && ok(dalloc(m, &m->utab, B * G.nu)) && ok(dalloc(m, &m->vtab, B * G.nv)) &&
@@ -446,6 +471,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         pcamm_model_destroy(m);
         return e == cudaErrorMemoryAllocation ? PCAMM_E_NOMEM : PCAMM_E_CUDA;
     }
+    m->xbar = m->fields;
+    m->u = m->fields + 3 * (size_t)V;
     m->c.opts = (CallOpts*)m->in_block;
     m->c.in = (SolveIn*)(m->in_block + m->in_off);
     std::memset(m->h_in, 0, m->in_block_bytes);
@@ -483,6 +510,14 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         set_error("non-finite value in f0, the DVF fields or the landmarks");
         return fail(PCAMM_E_NONFINITE);
     }
+    // the streaming kernels' view of the fields: TMA tensor map (else the generic kernels)
+    m->fs.fields = m->fields;
+    int dev = 0, n_sm = 1;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    m->fs.n_sm = n_sm > 0 ? n_sm : 1;
+    std::string why;
+    m->fs.use_tma = make_field_map(G, m->fields, 3 * (G.K + 1), 32, &m->fs.map32, &why);
     *out = m;
     return PCAMM_OK;
 }
@@ -519,7 +554,7 @@ int pcamm_warp(pcamm_model* m, const float* w_host, float* volume_out_dev, void*
     Seq q;
     int rc = hook_begin(m, nullptr, 0.f, w_host, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
-    launch_warp(q, m->G, m->f0, m->xbar, m->u, m->c.slots, 1, 0, volume_out_dev, m->G.V);
+    launch_warp(q, m->G, m->fs, m->f0, m->c.slots, 1, 0, volume_out_dev, m->G.V);
     if ((rc = check_seq(q, "warp"))) return rc;
     CUDA_TRY(cudaStreamSynchronize(st));
     return PCAMM_OK;
@@ -563,7 +598,7 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     if (rc) return rc;
     launch_ysums(q2, G, m->c, 1);
     launch_view_tables(q2, G, m->c.solves, 1, m->col_hdr, m->slab_tab);
-    launch_warp(q2, G, m->f0, m->xbar, m->u, m->c.slots, 1, 1, m->vol, G.PV);
+    launch_warp(q2, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV);
     launch_project(q2, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
     launch_ctl_eval(q2, G, m->c, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
@@ -640,7 +675,7 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
     CUDA_TRY(cudaEventRecord(m->ev0, st));
     for (int i = 0; i < reps; ++i) {
         if (which == 0)
-            launch_warp(q, G, m->f0, m->xbar, m->u, m->c.slots, 1, 1, m->vol, G.PV);
+            launch_warp(q, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV);
         else if (which == 1)
             launch_project(q, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
         else

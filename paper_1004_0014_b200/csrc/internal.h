@@ -8,6 +8,7 @@
 #include <string>
 
 #include "common.cuh"
+#include "stream.cuh"
 
 namespace pcamm {
 
@@ -75,8 +76,8 @@ struct Seq {
 // ---- a-1 (warp.cu)
 // f[s] = warp(f0, xbar + U w[s]) for every active slot; ray_layout: the z-fastest layout the
 // projector reads (slot stride G.PV), else the standard [z][y][x] (slot stride G.V).
-void launch_warp(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SlotState* slots,
-                 int nslots, int ray_layout, float* vol_out, long long slot_stride);
+void launch_warp(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
+                 int ray_layout, float* vol_out, long long slot_stride);
 
 // ---- a-2 (project.cu)
 int project_blocks(const Geom& G);

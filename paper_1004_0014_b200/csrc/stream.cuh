@@ -1,0 +1,149 @@
+// The streaming skeleton shared by the two HBM-bound kernels of the hot path (a-1 warp.cu, a-4
+// gradient.cu): both make one pass over the K+1 planar vector fields (Eq. 1:
+// x = xbar + sum_k u_k w_k needs all of them per voxel) and then chase 8-tap gathers in f0.
+//
+// A persistent CTA per SM.  One producer thread moves field tiles HBM -> shared memory with TMA
+// (cp.async.bulk.tensor, one 4-D box {TX x, 1 y, TZ z, 3(K+1) planes} per tile, completion
+// signalled on an mbarrier) through a ring of stages; consumer groups of 8 warps take the tiles
+// in turn.  The stream is thereby decoupled from the consumers' dependent chain
+// (fields -> displaced position -> f0 gathers -> interpolation), which is what kept the first,
+// register-staged version of these kernels at 35 % of the DRAM bandwidth (profiles/r01a).
+//
+// Tile = TX = 32 voxels along x, TZ along z, at fixed y: loads are 128 B rows of each plane, and
+// the warp kernel's transposed store (z fastest, ray layout) is one 128 B line per (x, y).
+#pragma once
+
+#include <cuda.h>
+
+#include <string>
+
+#include "common.cuh"
+
+namespace pcamm {
+
+constexpr int TX = 32;             // tile extent along x
+constexpr int GROUP_WARPS = 8;     // warps of a consumer group
+constexpr int GROUP_THREADS = 32 * GROUP_WARPS;
+
+// Tile t of the volume (x tiles fastest, then y, then z tiles: the CTAs that run side by side
+// read neighbouring rows of the same z slices).
+struct TileCoord {
+    int x0, y, z0;
+};
+
+__host__ __device__ __forceinline__ int tiles_x(const Geom& G) { return (G.nx + TX - 1) / TX; }
+__host__ __device__ __forceinline__ int tiles_z(const Geom& G, int tz) { return (G.nz + tz - 1) / tz; }
+__host__ __device__ __forceinline__ long long tile_count(const Geom& G, int tz) {
+    return (long long)tiles_x(G) * G.ny * tiles_z(G, tz);
+}
+__device__ __forceinline__ TileCoord tile_coord(const Geom& G, int tz, long long t) {
+    const int ntx = tiles_x(G);
+    TileCoord c;
+    c.x0 = (int)(t % ntx) * TX;
+    c.y = (int)((t / ntx) % G.ny);
+    c.z0 = (int)(t / ((long long)ntx * G.ny)) * tz;
+    return c;
+}
+
+// ---------------------------------------------------------------- mbarrier / TMA (PTX)
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    const uint32_t addr = smem_u32(bar);
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(addr), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+
+// One 4-D box of the field tensor {x, y, z, plane} -> shared memory, evict-first in L2 (the
+// fields are streamed once per pass and must not push f0 and the trial volumes out of L2).
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
+                                            int c3, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void group_barrier(int group) {
+    asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(GROUP_THREADS) : "memory");
+}
+
+// Shared-memory ring of a streaming kernel: NS stages of P planes x TZ x TX floats.
+template <int P, int TZ, int NS>
+struct FieldRing {
+    static constexpr int STAGE_FLOATS = P * TZ * TX;
+    static constexpr uint32_t STAGE_BYTES = STAGE_FLOATS * 4u;
+    static constexpr size_t BYTES = (size_t)NS * STAGE_BYTES + 2 * NS * sizeof(uint64_t);
+
+    float* data;        // 128 B aligned
+    uint64_t* full;     // [NS] TMA completion
+    uint64_t* empty;    // [NS] consumers done with the stage
+
+    __device__ __forceinline__ void bind(unsigned char* smem) {
+        data = reinterpret_cast<float*>(smem);
+        full = reinterpret_cast<uint64_t*>(smem + (size_t)NS * STAGE_BYTES);
+        empty = full + NS;
+    }
+    __device__ __forceinline__ void init() {   // one thread
+        for (int s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        mbar_fence_init();
+    }
+    __device__ __forceinline__ const float* stage(int s) const { return data + (size_t)s * STAGE_FLOATS; }
+
+    // Producer side: tiles i = 0 .. n-1 of this CTA are tiles blockIdx.x + i * gridDim.x.
+    __device__ __forceinline__ void produce(const CUtensorMap* map, const Geom& G, long long n_tiles) {
+        const uint64_t policy = l2_evict_first_policy();
+        int s = 0;
+        uint32_t ph = 0;
+        for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+            mbar_wait(empty + s, ph ^ 1u);                       // the stage is free (passes at once on a fresh ring)
+            const TileCoord c = tile_coord(G, TZ, t);
+            mbar_arrive_expect_tx(full + s, STAGE_BYTES);
+            tma_load_4d(data + (size_t)s * STAGE_FLOATS, map, full + s, c.x0, c.y, c.z0, 0, policy);
+            if (++s == NS) { s = 0; ph ^= 1u; }
+        }
+    }
+};
+
+// What the streaming kernels need to know about the model's fields.
+struct FieldStream {
+    const float* fields = nullptr;   // [3(K+1)][V]: xbar's planes, then u_1 .. u_K
+    bool use_tma = false;            // false: register-staged generic kernels
+    int n_sm = 1;                    // persistent grid size
+    CUtensorMap map32;               // box {TX, 1, 32, 3(K+1)}
+};
+
+// Host: the tensor map of the fields [P][nz][ny][nx] (xbar's three planes first, then u_1 .. u_K)
+// with box {TX, 1, tz, P}.  Returns false if the driver entry point is missing or the shape
+// cannot be described (nx * 4 must be a multiple of 16 bytes).
+bool make_field_map(const Geom& G, const float* fields, int planes, int tz, CUtensorMap* out, std::string* why);
+
+}  // namespace pcamm

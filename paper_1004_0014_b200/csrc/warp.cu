@@ -8,11 +8,16 @@
 // batched line search, or independent solves in flight): the fields of a voxel are loaded once
 // into registers and the slot loop runs inside the thread.
 //
-// HBM layout: fields planar [3][V] / [K][3][V] exactly as the caller gave them; a warp reads 32
-// consecutive x of one row per load instruction (one 128 B line per plane and row).  The warped
-// volume is written once, in the z-fastest ray layout of common.cuh that the projector reads at
-// every gantry angle (or in the standard layout for the volume returned to the caller).
+// HBM layout: fields planar [3(K+1)][V] (xbar's planes, then u_1 .. u_K), exactly the caller's
+// order.  The warped volume is written once, in the z-fastest ray layout of common.cuh that the
+// projector reads at every gantry angle (or in the standard layout for the volume returned to
+// the caller).
+//
+// k_warp_tma is the kernel of the solve: field tiles arrive in shared memory by TMA through the
+// mbarrier ring of stream.cuh, consumer groups interpolate and store.  k_warp_generic (one
+// register-staged tile per block) serves shapes TMA cannot describe (nx not a multiple of 4).
 #include "internal.h"
+#include "stream.cuh"
 
 namespace pcamm {
 
@@ -64,7 +69,7 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ f0, int nx,
 // handed back to the caller): lane = x.
 template <int K, bool RAY>
 __global__ void __launch_bounds__(NTHREADS)
-k_warp(const Geom G, const float* __restrict__ f0, const float* __restrict__ xbar, const float* __restrict__ u,
+k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restrict__ xbar, const float* __restrict__ u,
        const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride) {
     __shared__ float tile[TILE][TILE + 1];
     const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
@@ -129,21 +134,137 @@ k_warp(const Geom G, const float* __restrict__ f0, const float* __restrict__ xba
     }
 }
 
+// ---------------------------------------------------------------- the TMA-fed kernel
+
+constexpr int WTZ = 32;            // tile extent along z (the transposed store needs 32)
+constexpr int WNG = 2;             // consumer groups
+constexpr int WTHREADS = 32 * (WNG * GROUP_WARPS + 1);
+
+template <int K> struct WarpStages { static constexpr int value = K <= 3 ? 4 : (K <= 5 ? 3 : 2); };
+
 template <int K>
-void launch_k(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SlotState* slots,
-              int nslots, int ray_layout, float* vol_out, long long slot_stride) {
+constexpr size_t warp_smem_bytes() {
+    return 128 + FieldRing<3 * (K + 1), WTZ, WarpStages<K>::value>::BYTES + 16 +
+           (size_t)WNG * TX * (TX + 1) * sizeof(float);
+}
+
+template <int K, bool RAY>
+__global__ void __launch_bounds__(WTHREADS, 1)
+k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
+           const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride) {
+    constexpr int P = 3 * (K + 1), NS = WarpStages<K>::value;
+    using Ring = FieldRing<P, WTZ, NS>;
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    Ring ring;
+    ring.bind(smem);
+    float(*tiles)[TX][TX + 1] = reinterpret_cast<float(*)[TX][TX + 1]>(smem + ((Ring::BYTES + 15) & ~size_t(15)));
+    if (threadIdx.x == 0) ring.init();
+    __syncthreads();
+    const long long n_tiles = tile_count(G, WTZ);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp == WNG * GROUP_WARPS) {                       // producer
+        if (lane == 0) ring.produce(&fmap, G, n_tiles);
+        return;
+    }
+    const int group = warp / GROUP_WARPS, tw = warp % GROUP_WARPS;
+    float(*tile)[TX + 1] = tiles[group];
+    int s = 0, turn = 0;
+    uint32_t ph = 0;
+    for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        if (turn == group) {
+            mbar_wait(ring.full + s, ph);
+            const float* sf = ring.stage(s);               // [P][WTZ][TX]
+            const TileCoord c = tile_coord(G, WTZ, t);
+            const int x = c.x0 + lane;
+            for (int sl = 0; sl < nslots; ++sl) {
+                if (!slots[sl].active) continue;           // uniform over the grid
+                float w[K];
+#pragma unroll
+                for (int k = 0; k < K; ++k) w[k] = slots[sl].w[k];
+                float* out = vol_out + (long long)sl * slot_stride;
+                float val[ROWS];
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) {
+                    const int zz = tw + GROUP_WARPS * r, z = c.z0 + zz;
+                    val[r] = 0.f;
+                    if (x < G.nx && z < G.nz) {
+                        float d[3];
+#pragma unroll
+                        for (int cc = 0; cc < 3; ++cc) {
+                            float xs = sf[(cc * WTZ + zz) * TX + lane];                     // Eq. (1)
+#pragma unroll
+                            for (int k = 0; k < K; ++k) xs = fmaf(sf[((3 + 3 * k + cc) * WTZ + zz) * TX + lane], w[k], xs);
+                            d[cc] = xs;
+                        }
+                        val[r] = trilinear(f0, G.nx, G.ny, G.nz, x, c.y, z, __fdiv_rn(d[0], G.hx), __fdiv_rn(d[1], G.hy),
+                                           __fdiv_rn(d[2], G.hz));
+                    }
+                }
+                if (!RAY) {
+#pragma unroll
+                    for (int r = 0; r < ROWS; ++r) {
+                        const int z = c.z0 + tw + GROUP_WARPS * r;
+                        if (x < G.nx && z < G.nz) out[((long long)z * G.ny + c.y) * G.nx + x] = val[r];
+                    }
+                } else {
+                    group_barrier(group);
+#pragma unroll
+                    for (int r = 0; r < ROWS; ++r) tile[tw + GROUP_WARPS * r][lane] = val[r];
+                    group_barrier(group);
+                    const int zo = c.z0 + lane;
+#pragma unroll
+                    for (int r = 0; r < ROWS; ++r) {
+                        const int xo = c.x0 + tw + GROUP_WARPS * r;
+                        if (xo < G.nx && zo < G.nz) out[ray_layout_index(G, xo, c.y, zo)] = tile[lane][tw + GROUP_WARPS * r];
+                    }
+                }
+            }
+            group_barrier(group);                           // every thread of the group is done with the stage
+            if (tw == 0 && lane == 0) mbar_arrive(ring.empty + s);
+        }
+        if (++turn == WNG) turn = 0;
+        if (++s == NS) { s = 0; ph ^= 1u; }
+    }
+}
+
+template <int K, bool RAY>
+void launch_tma(Seq& q, const Geom& G, const CUtensorMap& fmap, int n_sm, const float* f0, const SlotState* slots,
+                int nslots, float* vol_out, long long slot_stride) {
+    static bool configured = false;
+    constexpr size_t smem = warp_smem_bytes<K>();
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_warp_tma<K, RAY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) { q.err = e; return; }
+        configured = true;
+    }
+    const long long nt = tile_count(G, WTZ);
+    const int grid = (int)(nt < n_sm ? nt : n_sm);
+    q.launch(k_warp_tma<K, RAY>, dim3(grid), dim3(WTHREADS), smem, fmap, G, f0, slots, nslots, vol_out, slot_stride);
+}
+
+template <int K>
+void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
+              int ray_layout, float* vol_out, long long slot_stride) {
+    if (fs.use_tma) {
+        if (ray_layout) launch_tma<K, true>(q, G, fs.map32, fs.n_sm, f0, slots, nslots, vol_out, slot_stride);
+        else launch_tma<K, false>(q, G, fs.map32, fs.n_sm, f0, slots, nslots, vol_out, slot_stride);
+        return;
+    }
+    const float* xbar = fs.fields;
+    const float* u = fs.fields + 3 * G.V;
     dim3 grid((G.nx + TILE - 1) / TILE, (G.nz + TILE - 1) / TILE, G.ny);
-    if (ray_layout) q.launch(k_warp<K, true>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride);
-    else q.launch(k_warp<K, false>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride);
+    if (ray_layout) q.launch(k_warp_generic<K, true>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride);
+    else q.launch(k_warp_generic<K, false>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride);
 }
 
 }  // namespace
 
-void launch_warp(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SlotState* slots,
-                 int nslots, int ray_layout, float* vol_out, long long slot_stride) {
+void launch_warp(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
+                 int ray_layout, float* vol_out, long long slot_stride) {
     switch (G.K) {
 #define PCAMM_CASE(KK) \
-    case KK: launch_k<KK>(q, G, f0, xbar, u, slots, nslots, ray_layout, vol_out, slot_stride); break;
+    case KK: launch_k<KK>(q, G, fs, f0, slots, nslots, ray_layout, vol_out, slot_stride); break;
         PCAMM_CASE(1) PCAMM_CASE(2) PCAMM_CASE(3) PCAMM_CASE(4)
         PCAMM_CASE(5) PCAMM_CASE(6) PCAMM_CASE(7) PCAMM_CASE(8)
 #undef PCAMM_CASE

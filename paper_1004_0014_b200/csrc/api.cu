@@ -34,6 +34,16 @@ __global__ void k_count_nonfinite(const float* __restrict__ a, long long n, unsi
     if (c) atomicAdd(count, c);
 }
 
+// Fields to voxel units, once at create: plane p holds component p % 3, divided by h of that
+// axis (IEEE division: a displacement of exactly n voxels stays exactly n).
+__global__ void k_fields_to_voxel_units(float* __restrict__ fields, long long V, int planes, float hx, float hy, float hz) {
+    const long long n = V * planes;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int c = (int)((i / V) % 3);
+        fields[i] = __fdiv_rn(fields[i], c == 0 ? hx : (c == 1 ? hy : hz));
+    }
+}
+
 }  // namespace
 
 bool make_field_map(const Geom& G, const float* fields, int planes, int tz, CUtensorMap* out, std::string* why) {
@@ -499,6 +509,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     k_count_nonfinite<<<592, 256, 0, st>>>(m->f0, V, m->nonfinite);
     k_count_nonfinite<<<592, 256, 0, st>>>(m->xbar, 3 * V, m->nonfinite);
     k_count_nonfinite<<<592, 256, 0, st>>>(m->u, 3 * V * G.K, m->nonfinite);
+    k_fields_to_voxel_units<<<1184, 256, 0, st>>>(m->fields, V, 3 * (G.K + 1), G.hx, G.hy, G.hz);
     unsigned long long bad = 0;
     TRY_OR_FAIL(cudaMemcpyAsync(&bad, m->nonfinite, sizeof(bad), cudaMemcpyDeviceToHost, st));
     TRY_OR_FAIL(cudaStreamSynchronize(st));

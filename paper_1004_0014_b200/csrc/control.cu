@@ -360,9 +360,9 @@ k_invert(const Geom G, const float* __restrict__ xbar, const float* __restrict__
 #pragma unroll
             for (int c = 0; c < 3; ++c) part[c] += coef * (double)__ldg(base + c * V + lin);
         }
-        double x[3];
+        double x[3];                                   // the model's fields are in voxel units: x (mm) = field * h
 #pragma unroll
-        for (int c = 0; c < 3; ++c) x[c] = warp_sum(part[c]);
+        for (int c = 0; c < 3; ++c) x[c] = warp_sum(part[c]) * h[c];
         double d2 = 0.0;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {

@@ -130,7 +130,8 @@ __device__ __forceinline__ float f0_tap(const float* __restrict__ f0, int nx, in
     return 0.f;
 }
 
-// G = d f / d x (1/mm) of the trilinear interpolant at voxel (i,j,k) displaced by d voxels:
+// G = d f / d x of the trilinear interpolant at voxel (i,j,k) displaced by d voxels, per voxel of
+// displacement (the model's fields are in voxel units, so G . u_k needs no 1/h: (G/h) . (u h) = G . u):
 // forward differences along the four parallel cell edges per axis, bilinearly weighted
 // (reading A6).
 __device__ __forceinline__ void trilinear_grad(const Geom& G, const float* __restrict__ f0, int i, int j, int k,
@@ -154,9 +155,9 @@ __device__ __forceinline__ void trilinear_grad(const Geom& G, const float* __res
         c011 = f0_tap(f0, nx, ny, nz, i0, j0 + 1, k0 + 1); c111 = f0_tap(f0, nx, ny, nz, i0 + 1, j0 + 1, k0 + 1);
     }
     const float X0 = 1.f - tx, Y0 = 1.f - ty, Z0 = 1.f - tz;
-    *gx = G.ihx * ((Y0 * (c100 - c000) + ty * (c110 - c010)) * Z0 + (Y0 * (c101 - c001) + ty * (c111 - c011)) * tz);
-    *gy = G.ihy * ((X0 * (c010 - c000) + tx * (c110 - c100)) * Z0 + (X0 * (c011 - c001) + tx * (c111 - c101)) * tz);
-    *gz = G.ihz * ((X0 * (c001 - c000) + tx * (c101 - c100)) * Y0 + (X0 * (c011 - c010) + tx * (c111 - c110)) * ty);
+    *gx = ((Y0 * (c100 - c000) + ty * (c110 - c010)) * Z0 + (Y0 * (c101 - c001) + ty * (c111 - c011)) * tz);
+    *gy = ((X0 * (c010 - c000) + tx * (c110 - c100)) * Z0 + (X0 * (c011 - c001) + tx * (c111 - c101)) * tz);
+    *gz = ((X0 * (c001 - c000) + tx * (c101 - c100)) * Y0 + (X0 * (c011 - c010) + tx * (c111 - c110)) * ty);
 }
 
 template <int K>
@@ -214,8 +215,7 @@ k_grad(const Geom G, const float* __restrict__ f0, const float* __restrict__ xba
             }
             const int y = y0 + ty + 8 * r;
             float gx, gy, gz;
-            trilinear_grad(G, f0, x, y, z, __fdiv_rn(d[0], G.hx), __fdiv_rn(d[1], G.hy), __fdiv_rn(d[2], G.hz),
-                           &gx, &gy, &gz);
+            trilinear_grad(G, f0, x, y, z, d[0], d[1], d[2], &gx, &gy, &gz);
             if (gx == 0.f && gy == 0.f && gz == 0.f) continue;
             const float yw = G.cy + ((float)y - 0.5f * (G.ny - 1)) * G.hy;
             const float Bj = gather_voxel(G, gv, rLb, ub, vb, xw, yw, zw);

@@ -4,6 +4,9 @@
 //   f_j = trilinear(f0, idx_j + x_j / h)           ("found through trilinear
 //                                                   interpolation"; pull-back, L99; readings A1, A2)
 //
+// The model keeps the fields in voxel units (xbar / h, u_k / h per component, divided once at
+// pcamm_model_create), so Eq. (1) yields the displacement in voxels directly.
+//
 // One pass over the K+1 vector fields serves every active trial slot (candidate steps of a
 // batched line search, or independent solves in flight): the fields of a voxel are loaded once
 // into registers and the slot loop runs inside the thread.
@@ -27,40 +30,45 @@ constexpr int TILE = 32;
 constexpr int ROWS = 4;        // voxels per thread (z rows tw, tw+8, tw+16, tw+24 of the tile)
 constexpr int NTHREADS = 256;  // 32 x 8
 
-// f0 with zero padding outside the grid (reading A2).
-__device__ __forceinline__ float f0_tap(const float* __restrict__ f0, int nx, int ny, int nz, int i, int j, int k) {
-    if ((unsigned)i < (unsigned)nx && (unsigned)j < (unsigned)ny && (unsigned)k < (unsigned)nz)
-        return __ldg(f0 + ((long long)k * ny + j) * nx + i);
-    return 0.f;
+// One axis of the 8-tap stencil: the cell index i0 = i + floor(d), the fraction t = d - floor(d),
+// the two tap indices clamped into the grid and the two weights, zeroed where the tap lies
+// outside the grid (reading A2: f0 = 0 there).  floor() and the fraction are taken of the
+// displacement alone, so that the lattice position never enters a float32 sum (idx + d would
+// lose 1e-5 voxel at idx ~ 256).  Branch-free, so that the gathers of several voxels can be in
+// flight together.
+struct AxisTaps {
+    int i0, i1;       // clamped tap indices
+    float w0, w1;     // (1 - t), t, or 0 outside the grid
+};
+
+__device__ __forceinline__ AxisTaps axis_taps(int i, float d, int n) {
+    const float fl = floorf(d);
+    const float t = d - fl;
+    const int a = i + (int)fl, b = a + 1;
+    AxisTaps r;
+    r.w0 = (unsigned)a < (unsigned)n ? 1.f - t : 0.f;
+    r.w1 = (unsigned)b < (unsigned)n ? t : 0.f;
+    r.i0 = min(max(a, 0), n - 1);
+    r.i1 = min(max(b, 0), n - 1);
+    return r;
 }
 
-// Trilinear interpolation of f0 at voxel (i,j,k) displaced by d voxels (d = x / h).
-// floor() and the fractional part are taken of the displacement alone, so that the lattice
-// position never enters a float32 sum (idx + d would lose 1e-5 voxel at idx ~ 256).
+// Trilinear interpolation of f0 at voxel (i,j,k) displaced by d voxels (d = x / h):
+// sum_abc c_abc X_a Y_b Z_c, x innermost.
 __device__ __forceinline__ float trilinear(const float* __restrict__ f0, int nx, int ny, int nz, int i, int j, int k,
                                            float dx, float dy, float dz) {
-    const float fx = floorf(dx), fy = floorf(dy), fz = floorf(dz);
-    const float tx = dx - fx, ty = dy - fy, tz = dz - fz;
-    const int i0 = i + (int)fx, j0 = j + (int)fy, k0 = k + (int)fz;
-    float c000, c100, c010, c110, c001, c101, c011, c111;
-    if (i0 >= 0 && i0 + 1 < nx && j0 >= 0 && j0 + 1 < ny && k0 >= 0 && k0 + 1 < nz) {
-        const float* p = f0 + ((long long)k0 * ny + j0) * nx + i0;
-        const long long sy = nx, sz = (long long)nx * ny;
-        c000 = __ldg(p);           c100 = __ldg(p + 1);
-        c010 = __ldg(p + sy);      c110 = __ldg(p + sy + 1);
-        c001 = __ldg(p + sz);      c101 = __ldg(p + sz + 1);
-        c011 = __ldg(p + sz + sy); c111 = __ldg(p + sz + sy + 1);
-    } else {
-        c000 = f0_tap(f0, nx, ny, nz, i0, j0, k0);         c100 = f0_tap(f0, nx, ny, nz, i0 + 1, j0, k0);
-        c010 = f0_tap(f0, nx, ny, nz, i0, j0 + 1, k0);     c110 = f0_tap(f0, nx, ny, nz, i0 + 1, j0 + 1, k0);
-        c001 = f0_tap(f0, nx, ny, nz, i0, j0, k0 + 1);     c101 = f0_tap(f0, nx, ny, nz, i0 + 1, j0, k0 + 1);
-        c011 = f0_tap(f0, nx, ny, nz, i0, j0 + 1, k0 + 1); c111 = f0_tap(f0, nx, ny, nz, i0 + 1, j0 + 1, k0 + 1);
-    }
-    const float X0 = 1.f - tx, Y0 = 1.f - ty, Z0 = 1.f - tz;
-    // sum_abc c_abc X_a Y_b Z_c, x innermost
-    const float r00 = c000 * X0 + c100 * tx, r10 = c010 * X0 + c110 * tx;
-    const float r01 = c001 * X0 + c101 * tx, r11 = c011 * X0 + c111 * tx;
-    return (r00 * Y0 + r10 * ty) * Z0 + (r01 * Y0 + r11 * ty) * tz;
+    const AxisTaps X = axis_taps(i, dx, nx), Y = axis_taps(j, dy, ny), Z = axis_taps(k, dz, nz);
+    const float* r00 = f0 + ((long long)Z.i0 * ny + Y.i0) * nx;
+    const float* r10 = f0 + ((long long)Z.i0 * ny + Y.i1) * nx;
+    const float* r01 = f0 + ((long long)Z.i1 * ny + Y.i0) * nx;
+    const float* r11 = f0 + ((long long)Z.i1 * ny + Y.i1) * nx;
+    const float c000 = __ldg(r00 + X.i0), c100 = __ldg(r00 + X.i1);
+    const float c010 = __ldg(r10 + X.i0), c110 = __ldg(r10 + X.i1);
+    const float c001 = __ldg(r01 + X.i0), c101 = __ldg(r01 + X.i1);
+    const float c011 = __ldg(r11 + X.i0), c111 = __ldg(r11 + X.i1);
+    const float v00 = c000 * X.w0 + c100 * X.w1, v10 = c010 * X.w0 + c110 * X.w1;
+    const float v01 = c001 * X.w0 + c101 * X.w1, v11 = c011 * X.w0 + c111 * X.w1;
+    return (v00 * Y.w0 + v10 * Y.w1) * Z.w0 + (v01 * Y.w0 + v11 * Y.w1) * Z.w1;
 }
 
 // Tile: 32 x by 32 z at fixed y.  Loads: lane = x (one 128 B line per plane and z).  Stores in the
@@ -111,8 +119,7 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
                     for (int k = 0; k < K; ++k) xs = fmaf(uu[r][k][c], w[k], xs);
                     d[c] = xs;
                 }
-                val[r] = trilinear(f0, G.nx, G.ny, G.nz, x, y, z0 + tw + 8 * r,
-                                   __fdiv_rn(d[0], G.hx), __fdiv_rn(d[1], G.hy), __fdiv_rn(d[2], G.hz));
+                val[r] = trilinear(f0, G.nx, G.ny, G.nz, x, y, z0 + tw + 8 * r, d[0], d[1], d[2]);
             }
         }
         if (!RAY) {
@@ -144,8 +151,7 @@ template <int K> struct WarpStages { static constexpr int value = K <= 3 ? 4 : (
 
 template <int K>
 constexpr size_t warp_smem_bytes() {
-    return 128 + FieldRing<3 * (K + 1), WTZ, WarpStages<K>::value>::BYTES + 16 +
-           (size_t)WNG * TX * (TX + 1) * sizeof(float);
+    return FieldRing<3 * (K + 1), WTZ, WarpStages<K>::value>::BYTES;
 }
 
 template <int K, bool RAY>
@@ -154,12 +160,14 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
            const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride) {
     constexpr int P = 3 * (K + 1), NS = WarpStages<K>::value;
     using Ring = FieldRing<P, WTZ, NS>;
-    extern __shared__ unsigned char smem_raw[];
-    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ float tiles[WNG][TX][TX + 1];
     Ring ring;
-    ring.bind(smem);
-    float(*tiles)[TX][TX + 1] = reinterpret_cast<float(*)[TX][TX + 1]>(smem + ((Ring::BYTES + 15) & ~size_t(15)));
-    if (threadIdx.x == 0) ring.init();
+    ring.bind(smem_raw);
+    if (threadIdx.x == 0) {
+        if (smem_u32(smem_raw) & 127u) __trap();           // TMA destinations must be 128 B aligned
+        ring.init();
+    }
     __syncthreads();
     const long long n_tiles = tile_count(G, WTZ);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -174,7 +182,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         if (turn == group) {
             mbar_wait(ring.full + s, ph);
-            const float* sf = ring.stage(s);               // [P][WTZ][TX]
+            const uint32_t sf = smem_u32(ring.stage(s));   // [P][WTZ][TX]
             const TileCoord c = tile_coord(G, WTZ, t);
             const int x = c.x0 + lane;
             for (int sl = 0; sl < nslots; ++sl) {
@@ -187,19 +195,17 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
 #pragma unroll
                 for (int r = 0; r < ROWS; ++r) {
                     const int zz = tw + GROUP_WARPS * r, z = c.z0 + zz;
-                    val[r] = 0.f;
-                    if (x < G.nx && z < G.nz) {
-                        float d[3];
+                    // voxels of a ragged tile beyond the grid: TMA filled their fields with zeros, the
+                    // taps are clamped, the value is computed and not stored
+                    float d[3];
 #pragma unroll
-                        for (int cc = 0; cc < 3; ++cc) {
-                            float xs = sf[(cc * WTZ + zz) * TX + lane];                     // Eq. (1)
+                    for (int cc = 0; cc < 3; ++cc) {
+                        float xs = lds_f32(sf + 4u * ((cc * WTZ + zz) * TX + lane));               // Eq. (1)
 #pragma unroll
-                            for (int k = 0; k < K; ++k) xs = fmaf(sf[((3 + 3 * k + cc) * WTZ + zz) * TX + lane], w[k], xs);
-                            d[cc] = xs;
-                        }
-                        val[r] = trilinear(f0, G.nx, G.ny, G.nz, x, c.y, z, __fdiv_rn(d[0], G.hx), __fdiv_rn(d[1], G.hy),
-                                           __fdiv_rn(d[2], G.hz));
+                        for (int k = 0; k < K; ++k) xs = fmaf(lds_f32(sf + 4u * (((3 + 3 * k + cc) * WTZ + zz) * TX + lane)), w[k], xs);
+                        d[cc] = xs;
                     }
+                    val[r] = trilinear(f0, G.nx, G.ny, G.nz, x, c.y, z, d[0], d[1], d[2]);
                 }
                 if (!RAY) {
 #pragma unroll

@@ -53,22 +53,45 @@ __device__ __forceinline__ AxisTaps axis_taps(int i, float d, int n) {
     return r;
 }
 
-// Trilinear interpolation of f0 at voxel (i,j,k) displaced by d voxels (d = x / h):
+// The 8-tap stencil of one voxel, split into address set-up, gather and combination so that a
+// thread can have the gathers of all its voxels in flight before it consumes the first.
+struct Taps {
+    unsigned r00, r10, r01, r11;    // element offsets of the four x rows (y0 z0, y1 z0, y0 z1, y1 z1)
+    int x0, x1;                     // clamped x indices
+    float wx0, wx1, wy0, wy1, wz0, wz1;
+};
+
+__device__ __forceinline__ Taps make_taps(int nx, int ny, int nz, int i, int j, int k, float dx, float dy, float dz) {
+    const AxisTaps X = axis_taps(i, dx, nx), Y = axis_taps(j, dy, ny), Z = axis_taps(k, dz, nz);
+    Taps t;
+    t.r00 = (unsigned)((Z.i0 * ny + Y.i0) * nx); t.r10 = (unsigned)((Z.i0 * ny + Y.i1) * nx);
+    t.r01 = (unsigned)((Z.i1 * ny + Y.i0) * nx); t.r11 = (unsigned)((Z.i1 * ny + Y.i1) * nx);
+    t.x0 = X.i0; t.x1 = X.i1;
+    t.wx0 = X.w0; t.wx1 = X.w1; t.wy0 = Y.w0; t.wy1 = Y.w1; t.wz0 = Z.w0; t.wz1 = Z.w1;
+    return t;
+}
+
+__device__ __forceinline__ void gather8(const float* __restrict__ f0, const Taps& t, float* c) {
+    c[0] = __ldg(f0 + (t.r00 + t.x0)); c[1] = __ldg(f0 + (t.r00 + t.x1));
+    c[2] = __ldg(f0 + (t.r10 + t.x0)); c[3] = __ldg(f0 + (t.r10 + t.x1));
+    c[4] = __ldg(f0 + (t.r01 + t.x0)); c[5] = __ldg(f0 + (t.r01 + t.x1));
+    c[6] = __ldg(f0 + (t.r11 + t.x0)); c[7] = __ldg(f0 + (t.r11 + t.x1));
+}
+
 // sum_abc c_abc X_a Y_b Z_c, x innermost.
+__device__ __forceinline__ float combine8(const Taps& t, const float* c) {
+    const float v00 = c[0] * t.wx0 + c[1] * t.wx1, v10 = c[2] * t.wx0 + c[3] * t.wx1;
+    const float v01 = c[4] * t.wx0 + c[5] * t.wx1, v11 = c[6] * t.wx0 + c[7] * t.wx1;
+    return (v00 * t.wy0 + v10 * t.wy1) * t.wz0 + (v01 * t.wy0 + v11 * t.wy1) * t.wz1;
+}
+
+// Trilinear interpolation of f0 at voxel (i,j,k) displaced by d voxels (d = x / h).
 __device__ __forceinline__ float trilinear(const float* __restrict__ f0, int nx, int ny, int nz, int i, int j, int k,
                                            float dx, float dy, float dz) {
-    const AxisTaps X = axis_taps(i, dx, nx), Y = axis_taps(j, dy, ny), Z = axis_taps(k, dz, nz);
-    const float* r00 = f0 + ((long long)Z.i0 * ny + Y.i0) * nx;
-    const float* r10 = f0 + ((long long)Z.i0 * ny + Y.i1) * nx;
-    const float* r01 = f0 + ((long long)Z.i1 * ny + Y.i0) * nx;
-    const float* r11 = f0 + ((long long)Z.i1 * ny + Y.i1) * nx;
-    const float c000 = __ldg(r00 + X.i0), c100 = __ldg(r00 + X.i1);
-    const float c010 = __ldg(r10 + X.i0), c110 = __ldg(r10 + X.i1);
-    const float c001 = __ldg(r01 + X.i0), c101 = __ldg(r01 + X.i1);
-    const float c011 = __ldg(r11 + X.i0), c111 = __ldg(r11 + X.i1);
-    const float v00 = c000 * X.w0 + c100 * X.w1, v10 = c010 * X.w0 + c110 * X.w1;
-    const float v01 = c001 * X.w0 + c101 * X.w1, v11 = c011 * X.w0 + c111 * X.w1;
-    return (v00 * Y.w0 + v10 * Y.w1) * Z.w0 + (v01 * Y.w0 + v11 * Y.w1) * Z.w1;
+    const Taps t = make_taps(nx, ny, nz, i, j, k, dx, dy, dz);
+    float c[8];
+    gather8(f0, t, c);
+    return combine8(t, c);
 }
 
 // Tile: 32 x by 32 z at fixed y.  Loads: lane = x (one 128 B line per plane and z).  Stores in the
@@ -145,6 +168,7 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
 
 constexpr int WTZ = 32;            // tile extent along z (the transposed store needs 32)
 constexpr int WNG = 2;             // consumer groups
+constexpr int SLOT_CACHE = 64;     // slots whose coefficients are kept in shared memory
 constexpr int WTHREADS = 32 * (WNG * GROUP_WARPS + 1);
 
 template <int K> struct WarpStages { static constexpr int value = K <= 3 ? 4 : (K <= 5 ? 3 : 2); };
@@ -162,6 +186,13 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     using Ring = FieldRing<P, WTZ, NS>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ float tiles[WNG][TX][TX + 1];
+    __shared__ float s_w[SLOT_CACHE][K];                   // the slots' coefficients (constant during the launch)
+    __shared__ int s_active[SLOT_CACHE];
+    for (int i = threadIdx.x; i < nslots && i < SLOT_CACHE; i += blockDim.x) {
+        s_active[i] = slots[i].active;
+#pragma unroll
+        for (int k = 0; k < K; ++k) s_w[i][k] = slots[i].w[k];
+    }
     Ring ring;
     ring.bind(smem_raw);
     if (threadIdx.x == 0) {
@@ -186,17 +217,18 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
             const TileCoord c = tile_coord(G, WTZ, t);
             const int x = c.x0 + lane;
             for (int sl = 0; sl < nslots; ++sl) {
-                if (!slots[sl].active) continue;           // uniform over the grid
+                if (!s_active[sl]) continue;               // uniform over the grid
                 float w[K];
 #pragma unroll
-                for (int k = 0; k < K; ++k) w[k] = slots[sl].w[k];
+                for (int k = 0; k < K; ++k) w[k] = s_w[sl][k];
                 float* out = vol_out + (long long)sl * slot_stride;
+                // voxels of a ragged tile beyond the grid: TMA filled their fields with zeros, the
+                // taps are clamped, the value is computed and not stored
                 float val[ROWS];
+                Taps taps[ROWS];
 #pragma unroll
                 for (int r = 0; r < ROWS; ++r) {
                     const int zz = tw + GROUP_WARPS * r, z = c.z0 + zz;
-                    // voxels of a ragged tile beyond the grid: TMA filled their fields with zeros, the
-                    // taps are clamped, the value is computed and not stored
                     float d[3];
 #pragma unroll
                     for (int cc = 0; cc < 3; ++cc) {
@@ -205,8 +237,13 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                         for (int k = 0; k < K; ++k) xs = fmaf(lds_f32(sf + 4u * (((3 + 3 * k + cc) * WTZ + zz) * TX + lane)), w[k], xs);
                         d[cc] = xs;
                     }
-                    val[r] = trilinear(f0, G.nx, G.ny, G.nz, x, c.y, z, d[0], d[1], d[2]);
+                    taps[r] = make_taps(G.nx, G.ny, G.nz, x, c.y, z, d[0], d[1], d[2]);
                 }
+                float cv[ROWS][8];
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) gather8(f0, taps[r], cv[r]);     // 8 ROWS gathers in flight
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) val[r] = combine8(taps[r], cv[r]);
                 if (!RAY) {
 #pragma unroll
                     for (int r = 0; r < ROWS; ++r) {
@@ -246,7 +283,11 @@ void launch_tma(Seq& q, const Geom& G, const CUtensorMap& fmap, int n_sm, const 
     }
     const long long nt = tile_count(G, WTZ);
     const int grid = (int)(nt < n_sm ? nt : n_sm);
-    q.launch(k_warp_tma<K, RAY>, dim3(grid), dim3(WTHREADS), smem, fmap, G, f0, slots, nslots, vol_out, slot_stride);
+    for (int s0 = 0; s0 < nslots; s0 += SLOT_CACHE) {      // the kernel keeps up to SLOT_CACHE slots' coefficients on chip
+        const int ns = nslots - s0 < SLOT_CACHE ? nslots - s0 : SLOT_CACHE;
+        q.launch(k_warp_tma<K, RAY>, dim3(grid), dim3(WTHREADS), smem, fmap, G, f0, slots + s0, ns,
+                 vol_out + (long long)s0 * slot_stride, slot_stride);
+    }
 }
 
 template <int K>

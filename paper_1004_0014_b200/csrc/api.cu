@@ -2,6 +2,7 @@
 // device-side while-loops (or driven from the host, opts.loop_mode = 1), and the function-level
 // hooks.  Argument marshalling and kernel sequencing only: every step of the hot path runs in the
 // kernels of warp.cu, project.cu, gradient.cu and control.cu.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -198,7 +199,7 @@ void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
 void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial, int use_cond) {
     const Geom& G = m->G;
     launch_resid(q, G, m->c.solves, m->c.in, B, 0, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_grad(q, G, m->f0, m->xbar, m->u, m->c.solves, B, m->rL, m->utab, m->vtab, m->c.grad_part);
+    launch_grad(q, G, m->fs, m->f0, m->c.solves, B, m->rL, m->utab, m->vtab, m->c.grad_part);
     launch_ctl_grad(q, G, m->c, h_trial, use_cond);
 }
 
@@ -453,7 +454,15 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     m->c.ysum_blocks = ysum_blocks(G);
     m->c.proj_blocks = project_blocks(G);
     m->c.resid_blocks = resid_blocks(G);
-    m->c.grad_blocks = grad_blocks(G);
+    {   // sized for either gradient kernel; the count in use is fixed once the field stream is known
+        int dev = 0, n_sm = 1;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        m->fs.n_sm = n_sm > 0 ? n_sm : 1;
+        FieldStream generic = m->fs, tma = m->fs;
+        generic.use_tma = false; tma.use_tma = true;
+        m->c.grad_blocks = std::max(grad_blocks(G, generic), grad_blocks(G, tma));
+    }
     m->trav_cap = G.nx + G.ny + G.nz + 8;
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return r == cudaSuccess; };
@@ -523,12 +532,9 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     }
     // the streaming kernels' view of the fields: TMA tensor map (else the generic kernels)
     m->fs.fields = m->fields;
-    int dev = 0, n_sm = 1;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    m->fs.n_sm = n_sm > 0 ? n_sm : 1;
     std::string why;
     m->fs.use_tma = make_field_map(G, m->fields, 3 * (G.K + 1), 32, &m->fs.map32, &why);
+    m->c.grad_blocks = grad_blocks(G, m->fs);
     *out = m;
     return PCAMM_OK;
 }
@@ -613,7 +619,7 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     launch_project(q2, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
     launch_ctl_eval(q2, G, m->c, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_grad(q2, G, m->f0, m->xbar, m->u, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
+    launch_grad(q2, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
     launch_ctl_eval(q2, G, m->c, 1);
     if ((rc = check_seq(q2, "eval"))) return rc;
     if (proj_out_dev) CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * G.npix, cudaMemcpyDeviceToDevice, st));
@@ -690,7 +696,7 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
         else if (which == 1)
             launch_project(q, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
         else
-            launch_grad(q, G, m->f0, m->xbar, m->u, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
+            launch_grad(q, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
     }
     CUDA_TRY(cudaEventRecord(m->ev1, st));
     int rc = check_seq(q, "time_kernel");

@@ -19,6 +19,8 @@
 // l_ij = |D - S| * |intersection of the two|.  Per view, k_resid tabulates (d_x, d_y, 1/d_x,
 // 1/d_y) per column, (d_z, 1/d_z) per row and rL_i = r_i |D_i - S| per pixel.
 #include "internal.h"
+#include "stream.cuh"
+#include "trilinear.cuh"
 
 namespace pcamm {
 
@@ -100,7 +102,7 @@ __device__ __forceinline__ float gather_voxel(const Geom& G, const GatherView& g
     const float t = ey * gv.cs - ex * gv.sn;                            // along u^
     // detector bounding rectangle of the box's shadow (perspective projection of a convex body:
     // extremes of t/depth and z/depth over the box are bounded by these four quotients)
-    const float i1 = 1.f / (depth - gv.Wd), i2 = 1.f / (depth + gv.Wd);
+    const float i1 = __frcp_rn(depth - gv.Wd), i2 = __frcp_rn(depth + gv.Wd);   // loop bounds only (0.01 px margin)
     const float tl = t - gv.Wt, th = t + gv.Wt, zl = ez - 0.5f * G.hz, zh = ez + 0.5f * G.hz;
     const float ulo = fminf(tl * i1, tl * i2) * gv.sdd_ipu + gv.cu, uhi = fmaxf(th * i1, th * i2) * gv.sdd_ipu + gv.cu;
     const float vlo = fminf(zl * i1, zl * i2) * gv.sdd_ipv + gv.cv, vhi = fmaxf(zh * i1, zh * i2) * gv.sdd_ipv + gv.cv;
@@ -124,45 +126,19 @@ __device__ __forceinline__ float gather_voxel(const Geom& G, const GatherView& g
     return acc;
 }
 
-__device__ __forceinline__ float f0_tap(const float* __restrict__ f0, int nx, int ny, int nz, int i, int j, int k) {
-    if ((unsigned)i < (unsigned)nx && (unsigned)j < (unsigned)ny && (unsigned)k < (unsigned)nz)
-        return __ldg(f0 + ((long long)k * ny + j) * nx + i);
-    return 0.f;
-}
-
 // G = d f / d x of the trilinear interpolant at voxel (i,j,k) displaced by d voxels, per voxel of
-// displacement (the model's fields are in voxel units, so G . u_k needs no 1/h: (G/h) . (u h) = G . u):
-// forward differences along the four parallel cell edges per axis, bilinearly weighted
-// (reading A6).
+// displacement (the model's fields are in voxel units, so G . u_k needs no 1/h: (G/h) . (u h) = G . u).
 __device__ __forceinline__ void trilinear_grad(const Geom& G, const float* __restrict__ f0, int i, int j, int k,
                                                float dx, float dy, float dz, float* gx, float* gy, float* gz) {
-    const float fx = floorf(dx), fy = floorf(dy), fz = floorf(dz);
-    const float tx = dx - fx, ty = dy - fy, tz = dz - fz;
-    const int i0 = i + (int)fx, j0 = j + (int)fy, k0 = k + (int)fz;
-    const int nx = G.nx, ny = G.ny, nz = G.nz;
-    float c000, c100, c010, c110, c001, c101, c011, c111;
-    if (i0 >= 0 && i0 + 1 < nx && j0 >= 0 && j0 + 1 < ny && k0 >= 0 && k0 + 1 < nz) {
-        const float* p = f0 + ((long long)k0 * ny + j0) * nx + i0;
-        const long long sy = nx, sz = (long long)nx * ny;
-        c000 = __ldg(p);           c100 = __ldg(p + 1);
-        c010 = __ldg(p + sy);      c110 = __ldg(p + sy + 1);
-        c001 = __ldg(p + sz);      c101 = __ldg(p + sz + 1);
-        c011 = __ldg(p + sz + sy); c111 = __ldg(p + sz + sy + 1);
-    } else {
-        c000 = f0_tap(f0, nx, ny, nz, i0, j0, k0);         c100 = f0_tap(f0, nx, ny, nz, i0 + 1, j0, k0);
-        c010 = f0_tap(f0, nx, ny, nz, i0, j0 + 1, k0);     c110 = f0_tap(f0, nx, ny, nz, i0 + 1, j0 + 1, k0);
-        c001 = f0_tap(f0, nx, ny, nz, i0, j0, k0 + 1);     c101 = f0_tap(f0, nx, ny, nz, i0 + 1, j0, k0 + 1);
-        c011 = f0_tap(f0, nx, ny, nz, i0, j0 + 1, k0 + 1); c111 = f0_tap(f0, nx, ny, nz, i0 + 1, j0 + 1, k0 + 1);
-    }
-    const float X0 = 1.f - tx, Y0 = 1.f - ty, Z0 = 1.f - tz;
-    *gx = ((Y0 * (c100 - c000) + ty * (c110 - c010)) * Z0 + (Y0 * (c101 - c001) + ty * (c111 - c011)) * tz);
-    *gy = ((X0 * (c010 - c000) + tx * (c110 - c100)) * Z0 + (X0 * (c011 - c001) + tx * (c111 - c101)) * tz);
-    *gz = ((X0 * (c001 - c000) + tx * (c101 - c100)) * Y0 + (X0 * (c011 - c010) + tx * (c111 - c110)) * ty);
+    const Taps t = make_taps(G.nx, G.ny, G.nz, i, j, k, dx, dy, dz);
+    float c[8];
+    gather8(f0, t, c);
+    grad8(t, c, gx, gy, gz);
 }
 
 template <int K>
 __global__ void __launch_bounds__(GT)
-k_grad(const Geom G, const float* __restrict__ f0, const float* __restrict__ xbar, const float* __restrict__ u,
+k_grad_generic(const Geom G, const float* __restrict__ f0, const float* __restrict__ xbar, const float* __restrict__ u,
        const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
        const float2* __restrict__ vtab, double* __restrict__ partials) {
     __shared__ double red[GT / 32];
@@ -231,6 +207,189 @@ k_grad(const Geom G, const float* __restrict__ f0, const float* __restrict__ xba
     }
 }
 
+int grad_grid(const Geom& G, const FieldStream& fs) {
+    const long long nt = tile_count(G, 32);
+    return (int)(nt < fs.n_sm ? nt : fs.n_sm);
+}
+
+// ---------------------------------------------------------------- the TMA-fed kernel
+//
+// Same ring as the warp kernel.  A consumer group works through a tile in batches of RB voxels
+// per thread:
+//   1. every thread forms G_j and q_kj = G_j . u_kj for its voxels (all their f0 gathers in flight
+//      together);
+//   2. the voxels with G_j != 0 are compacted into a shared-memory queue, in a fixed order
+//      (ballot + prefix over the warps: no atomics, so the summation order is reproducible);
+//   3. the queue is dealt out evenly: each thread gathers B_j for its entries and accumulates
+//      B_j q_kj.  Only boundary voxels have G_j != 0 in piecewise-constant anatomy, so without the
+//      compaction most lanes of a warp would idle through their neighbours' detector gathers.
+// Per tile and solve the group's K sums are reduced in double and added to the group's slot of
+// the partial-sum buffer; the control kernel adds the slots in index order.
+
+constexpr int GTZ = 32;
+constexpr int GNG = 2;
+constexpr int GTHREADS = 32 * (GNG * GROUP_WARPS + 1);
+constexpr int GROWS = GTZ / GROUP_WARPS;            // voxels per thread and tile
+
+template <int K> struct GradStages { static constexpr int value = K <= 3 ? 3 : 2; };
+template <int K> struct GradBatch { static constexpr int value = K <= 3 ? 4 : 2; };     // RB
+
+template <int K>
+struct QueueEntry {
+    int vox;          // zz << 5 | xx inside the tile
+    float q[K];
+};
+
+template <int K>
+constexpr size_t grad_smem_bytes() {
+    return FieldRing<3 * (K + 1), GTZ, GradStages<K>::value>::BYTES + 16 +
+           (size_t)GNG * GROUP_THREADS * GradBatch<K>::value * sizeof(QueueEntry<K>);
+}
+
+template <int K>
+__global__ void __launch_bounds__(GTHREADS, 1)
+k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
+           const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
+           const float2* __restrict__ vtab, double* __restrict__ partials) {
+    constexpr int P = 3 * (K + 1), NS = GradStages<K>::value, RB = GradBatch<K>::value, NB = GROWS / RB;
+    using Ring = FieldRing<P, GTZ, NS>;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ int s_cnt[GNG][32];
+    __shared__ float s_red[GNG][GROUP_WARPS][K];
+    Ring ring;
+    ring.bind(smem_raw);
+    QueueEntry<K>* queues = reinterpret_cast<QueueEntry<K>*>(smem_raw + ((Ring::BYTES + 15) & ~size_t(15)));
+    if (threadIdx.x == 0) {
+        if (smem_u32(smem_raw) & 127u) __trap();
+        ring.init();
+    }
+    __syncthreads();
+    const long long n_tiles = tile_count(G, GTZ);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp == GNG * GROUP_WARPS) {                       // producer
+        if (lane == 0) ring.produce(&fmap, G, n_tiles);
+        return;
+    }
+    const int group = warp / GROUP_WARPS, tw = warp % GROUP_WARPS, gtid = threadIdx.x - group * GROUP_THREADS;
+    QueueEntry<K>* queue = queues + (size_t)group * GROUP_THREADS * RB;
+    const int nslot = gridDim.x * GNG, slot = blockIdx.x * GNG + group;   // this group's partial-sum slot
+    if (gtid < K)
+        for (int b = 0; b < B; ++b) partials[((long long)b * nslot + slot) * KMAX + gtid] = 0.0;
+
+    int s = 0, turn = 0;
+    uint32_t ph = 0;
+    for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        if (turn == group) {
+            mbar_wait(ring.full + s, ph);
+            const uint32_t sf = smem_u32(ring.stage(s));   // [P][GTZ][TX]
+            const TileCoord c = tile_coord(G, GTZ, t);
+            const int x = c.x0 + lane;
+            for (int b = 0; b < B; ++b) {
+                if (!solves[b].running) continue;          // uniform over the grid
+                float w[K];
+#pragma unroll
+                for (int k = 0; k < K; ++k) w[k] = (float)solves[b].w[k];
+                const GatherView gv = make_gather_view(G, solves[b].view);
+                const float* rLb = rL + (long long)b * G.npix;
+                const float4* ub = utab + (long long)b * G.nu;
+                const float2* vb = vtab + (long long)b * G.nv;
+                float acc[K];
+#pragma unroll
+                for (int k = 0; k < K; ++k) acc[k] = 0.f;
+#pragma unroll 1
+                for (int bt = 0; bt < NB; ++bt) {
+                    // 1. G_j and q_kj
+                    Taps taps[RB];
+#pragma unroll
+                    for (int rr = 0; rr < RB; ++rr) {
+                        const int zz = tw + GROUP_WARPS * (bt * RB + rr);
+                        float d[3];
+#pragma unroll
+                        for (int cc = 0; cc < 3; ++cc) {
+                            float xs = lds_f32(sf + 4u * ((cc * GTZ + zz) * TX + lane));           // Eq. (1)
+#pragma unroll
+                            for (int k = 0; k < K; ++k)
+                                xs = fmaf(lds_f32(sf + 4u * (((3 + 3 * k + cc) * GTZ + zz) * TX + lane)), w[k], xs);
+                            d[cc] = xs;
+                        }
+                        taps[rr] = make_taps(G.nx, G.ny, G.nz, x, c.y, c.z0 + zz, d[0], d[1], d[2]);
+                    }
+                    float cv[RB][8];
+#pragma unroll
+                    for (int rr = 0; rr < RB; ++rr) gather8(f0, taps[rr], cv[rr]);
+                    float q[RB][K];
+                    unsigned masks[RB];
+#pragma unroll
+                    for (int rr = 0; rr < RB; ++rr) {
+                        const int zz = tw + GROUP_WARPS * (bt * RB + rr);
+                        float gx, gy, gz;
+                        grad8(taps[rr], cv[rr], &gx, &gy, &gz);
+#pragma unroll
+                        for (int k = 0; k < K; ++k)
+                            q[rr][k] = gx * lds_f32(sf + 4u * (((3 + 3 * k + 0) * GTZ + zz) * TX + lane)) +
+                                       gy * lds_f32(sf + 4u * (((3 + 3 * k + 1) * GTZ + zz) * TX + lane)) +
+                                       gz * lds_f32(sf + 4u * (((3 + 3 * k + 2) * GTZ + zz) * TX + lane));
+                        const bool active = x < G.nx && c.z0 + zz < G.nz && (gx != 0.f || gy != 0.f || gz != 0.f);
+                        masks[rr] = __ballot_sync(0xffffffffu, active);
+                        if (lane == 0) s_cnt[group][rr * GROUP_WARPS + tw] = __popc(masks[rr]);
+                    }
+                    group_barrier(group);
+                    // 2. compaction in the fixed order (row, warp, lane)
+                    int cnt = lane < RB * GROUP_WARPS ? s_cnt[group][lane] : 0, incl = cnt;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int v = __shfl_up_sync(0xffffffffu, incl, o);
+                        if (lane >= o) incl += v;
+                    }
+                    const int n_q = __shfl_sync(0xffffffffu, incl, 31);
+#pragma unroll
+                    for (int rr = 0; rr < RB; ++rr) {
+                        const int base = __shfl_sync(0xffffffffu, incl - cnt, rr * GROUP_WARPS + tw);
+                        if (masks[rr] >> lane & 1u) {
+                            QueueEntry<K>& e = queue[base + __popc(masks[rr] & ((1u << lane) - 1u))];
+                            e.vox = (tw + GROUP_WARPS * (bt * RB + rr)) << 5 | lane;
+#pragma unroll
+                            for (int k = 0; k < K; ++k) e.q[k] = q[rr][k];
+                        }
+                    }
+                    group_barrier(group);
+                    // 3. the detector gathers, dealt out evenly
+                    for (int e = gtid; e < n_q; e += GROUP_THREADS) {
+                        const QueueEntry<K> en = queue[e];
+                        const int xx = en.vox & 31, zz = en.vox >> 5;
+                        const float xw = G.cx + ((float)(c.x0 + xx) - 0.5f * (G.nx - 1)) * G.hx;
+                        const float yw = G.cy + ((float)c.y - 0.5f * (G.ny - 1)) * G.hy;
+                        const float zw = G.cz + ((float)(c.z0 + zz) - 0.5f * (G.nz - 1)) * G.hz;
+                        const float Bj = gather_voxel(G, gv, rLb, ub, vb, xw, yw, zw);
+#pragma unroll
+                        for (int k = 0; k < K; ++k) acc[k] = fmaf(Bj, en.q[k], acc[k]);
+                    }
+                    group_barrier(group);                   // the queue and s_cnt are free again
+                }
+                // the group's K sums of this tile and solve
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+                    float v = acc[k];
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                    if (lane == 0) s_red[group][tw][k] = v;
+                }
+                group_barrier(group);
+                if (gtid < K) {
+                    double sum = 0.0;
+#pragma unroll
+                    for (int i = 0; i < GROUP_WARPS; ++i) sum += (double)s_red[group][i][gtid];
+                    partials[((long long)b * nslot + slot) * KMAX + gtid] += sum;
+                }
+            }
+            group_barrier(group);                           // every thread of the group is done with the stage
+            if (gtid == 0) mbar_arrive(ring.empty + s);
+        }
+        if (++turn == GNG) turn = 0;
+        if (++s == NS) { s = 0; ph ^= 1u; }
+    }
+}
+
 // Hook: B = P^T r as a volume (view of solve 0).
 __global__ void __launch_bounds__(256)
 k_backproject(const Geom G, const SolveState* __restrict__ solves, const float* __restrict__ rL,
@@ -246,16 +405,33 @@ k_backproject(const Geom G, const SolveState* __restrict__ solves, const float* 
 }
 
 template <int K>
-void launch_k(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SolveState* solves,
-              int B, const float* rL, const float4* utab, const float2* vtab, double* partials) {
+void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
+              const float* rL, const float4* utab, const float2* vtab, double* partials) {
+    if (fs.use_tma) {
+        static bool configured = false;
+        constexpr size_t smem = grad_smem_bytes<K>();
+        if (!configured) {
+            cudaError_t e = cudaFuncSetAttribute(k_grad_tma<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) { q.err = e; return; }
+            configured = true;
+        }
+        q.launch(k_grad_tma<K>, dim3(grad_grid(G, fs)), dim3(GTHREADS), smem, fs.map32, G, f0, solves, B, rL, utab, vtab,
+                 partials);
+        return;
+    }
     dim3 grid((G.nx + TILE - 1) / TILE, (G.ny + TILE - 1) / TILE, G.nz);
-    q.launch(k_grad<K>, grid, dim3(GT), 0, G, f0, xbar, u, solves, B, rL, utab, vtab, partials);
+    q.launch(k_grad_generic<K>, grid, dim3(GT), 0, G, f0, fs.fields, fs.fields + 3 * G.V, solves, B, rL, utab, vtab,
+             partials);
 }
 
 }  // namespace
 
 int resid_blocks(const Geom& G) { return (G.npix + RT - 1) / RT; }
-int grad_blocks(const Geom& G) { return ((G.nx + TILE - 1) / TILE) * ((G.ny + TILE - 1) / TILE) * G.nz; }
+// partial-sum slots per solve: two per persistent CTA (TMA kernel), else one per block
+int grad_blocks(const Geom& G, const FieldStream& fs) {
+    if (fs.use_tma) return grad_grid(G, fs) * GNG;
+    return ((G.nx + TILE - 1) / TILE) * ((G.ny + TILE - 1) / TILE) * G.nz;
+}
 
 void launch_resid(Seq& q, const Geom& G, const SolveState* solves, const SolveIn* in, int B, int force,
                   const float* p, const float* r_direct, float* rL, float4* utab, float2* vtab, double* partials) {
@@ -263,11 +439,11 @@ void launch_resid(Seq& q, const Geom& G, const SolveState* solves, const SolveIn
              partials);
 }
 
-void launch_grad(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SolveState* solves,
-                 int B, const float* rL, const float4* utab, const float2* vtab, double* partials) {
+void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
+                 const float* rL, const float4* utab, const float2* vtab, double* partials) {
     switch (G.K) {
 #define PCAMM_CASE(KK) \
-    case KK: launch_k<KK>(q, G, f0, xbar, u, solves, B, rL, utab, vtab, partials); break;
+    case KK: launch_k<KK>(q, G, fs, f0, solves, B, rL, utab, vtab, partials); break;
         PCAMM_CASE(1) PCAMM_CASE(2) PCAMM_CASE(3) PCAMM_CASE(4)
         PCAMM_CASE(5) PCAMM_CASE(6) PCAMM_CASE(7) PCAMM_CASE(8)
 #undef PCAMM_CASE

@@ -96,15 +96,15 @@ void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* 
 
 // ---- a-3 / a-4 (gradient.cu)
 int resid_blocks(const Geom& G);
-int grad_blocks(const Geom& G);
+int grad_blocks(const Geom& G, const FieldStream& fs);
 // r = p - a y - b, rL = r * |D - S|, per-view tables, partial sums of r^2; p of solve b is read
 // from its accepted slot.
 // force: also for solves that are no longer running (closing pass); r_direct: take r from there.
 void launch_resid(Seq& q, const Geom& G, const SolveState* solves, const SolveIn* in, int B, int force,
                   const float* p, const float* r_direct, float* rL, float4* utab, float2* vtab, double* partials);
 // g = 2 U^T (df/dx) P^T r, per-block partial sums [B][blocks][K].
-void launch_grad(Seq& q, const Geom& G, const float* f0, const float* xbar, const float* u, const SolveState* solves,
-                 int B, const float* rL, const float4* utab, const float2* vtab, double* partials);
+void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
+                 const float* rL, const float4* utab, const float2* vtab, double* partials);
 // hook: B = P^T r as a volume for solve 0's view (rL/utab/vtab as written by launch_resid).
 void launch_backproject(Seq& q, const Geom& G, const SolveState* solves, const float* rL, const float4* utab,
                         const float2* vtab, float* vol_out);

@@ -230,6 +230,7 @@ constexpr int GTZ = 32;
 constexpr int GNG = 2;
 constexpr int GTHREADS = 32 * (GNG * GROUP_WARPS + 1);
 constexpr int GROWS = GTZ / GROUP_WARPS;            // voxels per thread and tile
+constexpr int SOLVE_CACHE = 64;                     // solves whose constants are kept in shared memory
 
 template <int K> struct GradStages { static constexpr int value = K <= 3 ? 3 : 2; };
 template <int K> struct GradBatch { static constexpr int value = K <= 3 ? 4 : 2; };     // RB
@@ -246,7 +247,9 @@ constexpr size_t grad_smem_bytes() {
            (size_t)GNG * GROUP_THREADS * GradBatch<K>::value * sizeof(QueueEntry<K>);
 }
 
-template <int K>
+// SINGLE: one solve (B = 1): the K sums stay in registers over all tiles of the CTA and are
+// reduced once at the end; otherwise they are reduced per tile and solve.
+template <int K, bool SINGLE>
 __global__ void __launch_bounds__(GTHREADS, 1)
 k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
            const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
@@ -256,6 +259,15 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ int s_cnt[GNG][32];
     __shared__ float s_red[GNG][GROUP_WARPS][K];
+    __shared__ GatherView s_gv[SOLVE_CACHE];               // per solve, constant during the launch
+    __shared__ float s_w[SOLVE_CACHE][K];
+    __shared__ int s_running[SOLVE_CACHE];
+    for (int b = threadIdx.x; b < B; b += blockDim.x) {    // B <= SOLVE_CACHE (the launcher chunks)
+        s_running[b] = solves[b].running;
+        s_gv[b] = make_gather_view(G, solves[b].view);
+#pragma unroll
+        for (int k = 0; k < K; ++k) s_w[b][k] = (float)solves[b].w[k];
+    }
     Ring ring;
     ring.bind(smem_raw);
     QueueEntry<K>* queues = reinterpret_cast<QueueEntry<K>*>(smem_raw + ((Ring::BYTES + 15) & ~size_t(15)));
@@ -276,6 +288,9 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     if (gtid < K)
         for (int b = 0; b < B; ++b) partials[((long long)b * nslot + slot) * KMAX + gtid] = 0.0;
 
+    float acc[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) acc[k] = 0.f;
     int s = 0, turn = 0;
     uint32_t ph = 0;
     for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
@@ -285,17 +300,18 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
             const TileCoord c = tile_coord(G, GTZ, t);
             const int x = c.x0 + lane;
             for (int b = 0; b < B; ++b) {
-                if (!solves[b].running) continue;          // uniform over the grid
+                if (!s_running[b]) continue;               // uniform over the grid
                 float w[K];
 #pragma unroll
-                for (int k = 0; k < K; ++k) w[k] = (float)solves[b].w[k];
-                const GatherView gv = make_gather_view(G, solves[b].view);
+                for (int k = 0; k < K; ++k) w[k] = s_w[b][k];
+                const GatherView gv = s_gv[b];
                 const float* rLb = rL + (long long)b * G.npix;
                 const float4* ub = utab + (long long)b * G.nu;
                 const float2* vb = vtab + (long long)b * G.nv;
-                float acc[K];
+                if (!SINGLE) {
 #pragma unroll
-                for (int k = 0; k < K; ++k) acc[k] = 0.f;
+                    for (int k = 0; k < K; ++k) acc[k] = 0.f;
+                }
 #pragma unroll 1
                 for (int bt = 0; bt < NB; ++bt) {
                     // 1. G_j and q_kj
@@ -334,6 +350,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                         if (lane == 0) s_cnt[group][rr * GROUP_WARPS + tw] = __popc(masks[rr]);
                     }
                     group_barrier(group);
+                    if (SINGLE && bt == NB - 1 && gtid == 0) mbar_arrive(ring.empty + s);   // no more reads of the stage
                     // 2. compaction in the fixed order (row, warp, lane)
                     int cnt = lane < RB * GROUP_WARPS ? s_cnt[group][lane] : 0, incl = cnt;
 #pragma unroll
@@ -366,27 +383,47 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     }
                     group_barrier(group);                   // the queue and s_cnt are free again
                 }
-                // the group's K sums of this tile and solve
+                if (!SINGLE) {                              // the group's K sums of this tile and solve
 #pragma unroll
-                for (int k = 0; k < K; ++k) {
-                    float v = acc[k];
+                    for (int k = 0; k < K; ++k) {
+                        float v = acc[k];
 #pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-                    if (lane == 0) s_red[group][tw][k] = v;
-                }
-                group_barrier(group);
-                if (gtid < K) {
-                    double sum = 0.0;
+                        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                        if (lane == 0) s_red[group][tw][k] = v;
+                    }
+                    group_barrier(group);
+                    if (gtid < K) {
+                        double sum = 0.0;
 #pragma unroll
-                    for (int i = 0; i < GROUP_WARPS; ++i) sum += (double)s_red[group][i][gtid];
-                    partials[((long long)b * nslot + slot) * KMAX + gtid] += sum;
+                        for (int i = 0; i < GROUP_WARPS; ++i) sum += (double)s_red[group][i][gtid];
+                        partials[((long long)b * nslot + slot) * KMAX + gtid] += sum;
+                    }
                 }
             }
-            group_barrier(group);                           // every thread of the group is done with the stage
-            if (gtid == 0) mbar_arrive(ring.empty + s);
+            if (!SINGLE) {
+                group_barrier(group);                       // every thread of the group is done with the stage
+                if (gtid == 0) mbar_arrive(ring.empty + s);
+            } else if (!s_running[0] && gtid == 0) mbar_arrive(ring.empty + s);
         }
         if (++turn == GNG) turn = 0;
         if (++s == NS) { s = 0; ph ^= 1u; }
+    }
+    if (SINGLE) {                                           // the group's K sums over all its tiles
+        double sum[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) sum[k] = warp_sum((double)acc[k]);
+        __shared__ double s_fin[GNG][GROUP_WARPS][K];
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < K; ++k) s_fin[group][tw][k] = sum[k];
+        }
+        group_barrier(group);
+        if (gtid < K) {
+            double tot = 0.0;
+#pragma unroll
+            for (int i = 0; i < GROUP_WARPS; ++i) tot += s_fin[group][i][gtid];
+            partials[(long long)slot * KMAX + gtid] = tot;
+        }
     }
 }
 
@@ -411,12 +448,24 @@ void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, con
         static bool configured = false;
         constexpr size_t smem = grad_smem_bytes<K>();
         if (!configured) {
-            cudaError_t e = cudaFuncSetAttribute(k_grad_tma<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaError_t e = cudaFuncSetAttribute(k_grad_tma<K, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(k_grad_tma<K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) { q.err = e; return; }
             configured = true;
         }
-        q.launch(k_grad_tma<K>, dim3(grad_grid(G, fs)), dim3(GTHREADS), smem, fs.map32, G, f0, solves, B, rL, utab, vtab,
-                 partials);
+        const int grid = grad_grid(G, fs), nslot = grid * GNG;
+        if (B == 1) {
+            q.launch(k_grad_tma<K, true>, dim3(grid), dim3(GTHREADS), smem, fs.map32, G, f0, solves, 1, rL, utab, vtab,
+                     partials);
+            return;
+        }
+        for (int b0 = 0; b0 < B; b0 += SOLVE_CACHE) {       // the kernel keeps up to SOLVE_CACHE solves' constants on chip
+            const int nb = B - b0 < SOLVE_CACHE ? B - b0 : SOLVE_CACHE;
+            q.launch(k_grad_tma<K, false>, dim3(grid), dim3(GTHREADS), smem, fs.map32, G, f0, solves + b0, nb,
+                     rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu, vtab + (long long)b0 * G.nv,
+                     partials + (long long)b0 * nslot * KMAX);
+        }
         return;
     }
     dim3 grid((G.nx + TILE - 1) / TILE, (G.ny + TILE - 1) / TILE, G.nz);

@@ -143,9 +143,12 @@ def test_batch_of_solves_equals_single_solves():
     batch = m.reconstruct_batch(yd, angles, w0, opts, trace=True)
     for b in range(B):
         single = m.reconstruct(yd[b], float(angles[b]), w0[b], opts, trace=True)
-        assert np.array_equal(batch[b].w, single.w), b
-        assert batch[b].J == single.J and np.array_equal(batch[b].backtracks, single.backtracks)
-        assert np.array_equal(batch[b].landmarks, single.landmarks)
+        # same arithmetic per voxel and ray; the K gradient sums are grouped per tile in the batched
+        # kernel and per thread in the single-solve one (both fixed orders), so equality holds to
+        # float32 summation-order rounding, not bitwise
+        assert np.linalg.norm(batch[b].w - single.w) <= 1e-5 * np.linalg.norm(single.w), b
+        assert abs(batch[b].J - single.J) <= 1e-5 * single.J and np.array_equal(batch[b].backtracks, single.backtracks)
+        np.testing.assert_allclose(batch[b].landmarks, single.landmarks, rtol=0, atol=1e-4)
     _compare_with_oracle(g, f0, xbar, u, ys[2], float(angles[2]), w0[2], lm, batch[2], opts)
 
 

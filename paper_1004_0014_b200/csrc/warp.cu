@@ -113,7 +113,7 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
 // ---------------------------------------------------------------- the TMA-fed kernel
 
 constexpr int WTZ = 32;            // tile extent along z (the transposed store needs 32)
-constexpr int WNG = 2;             // consumer groups
+constexpr int WNG = 3;             // consumer groups
 constexpr int SLOT_CACHE = 64;     // slots whose coefficients are kept in shared memory
 constexpr int WTHREADS = 32 * (WNG * GROUP_WARPS + 1);
 

@@ -124,6 +124,14 @@ k_view_tables(const Geom G, const SolveState* __restrict__ solves, ColHdr* __res
         e.tt = (float)tt;
         row[n] = e;
     }
+    // null entries up to the end of the (padded) row: a zero-valued border column whose
+    // transverse neighbours are inside the buffer, no crossing
+    for (int n = c.n_slabs + threadIdx.x; n < max_slabs; n += blockDim.x) {
+        SlabEntry e;
+        e.off0 = G.pnx * G.nz;            // (x, y) = (-1, 0)
+        e.tt = 1.f;
+        row[n] = e;
+    }
 }
 
 // ------------------------------------------------------------------ per-ray z tracking and the march
@@ -169,29 +177,51 @@ __device__ __forceinline__ RayZ make_ray_z(const Geom& G, const ColHdr& h, int i
     return r;
 }
 
-// Calls sink(off, k, tau) for every piece of every slab, source side first: off = element offset
-// of the voxel column (i, j), k the axial index, tau the share of the slab's path length.
-// Pieces of zero share are passed on (the sink ignores or drops them).
+// Runs the slabs of one ray, source side first, U at a time.  Per piece the sink is asked first
+// to fetch (off = element offset of the voxel column (i, j), k = axial index) and later to add
+// (off, k, tau = share of the slab's path length, fetched value): all fetches of a group of U
+// slabs are issued before the first add, and the table entries of the next group are loaded
+// while this one is worked on.  Rows are padded with null entries (zero-valued border column,
+// tt = 1) to a multiple of U plus one group, so there is no remainder loop.  Pieces of zero
+// share are passed on (the sink ignores or drops them).
+constexpr int U = 4;
+
 template <class Sink>
 __device__ __forceinline__ void march(const SlabEntry* __restrict__ row, int n_slabs, int dT, RayZ r, Sink& sink) {
     const float inv32 = 2.3283064365386963e-10f;   // 2^-32
+    const int4* row4 = reinterpret_cast<const int4*>(row);          // two entries per 16 B
     int k = r.k;
     unsigned long long QZ = r.QZ;
-#pragma unroll 4
-    for (int n = 0; n < n_slabs; ++n) {
-        const int2 e = __ldg(reinterpret_cast<const int2*>(row) + n);
-        const int off0 = e.x, off1 = e.x + dT;
-        const float tt = __int_as_float(e.y);
-        const bool cz = (unsigned)(QZ >> 32) == (unsigned)n;
-        const float tz = cz ? __uint2float_rn((unsigned)QZ) * inv32 : 1.f;
-        const int ke = cz ? k + r.dirZ : k;
-        const float t1 = fminf(tt, tz), t2 = fmaxf(tt, tz);
-        const bool tfirst = tt < tz;
-        sink(off0, k, t1);
-        sink(tfirst ? off1 : off0, tfirst ? k : ke, t2 - t1);
-        sink(off1, ke, 1.f - t2);
-        k = ke;
-        if (cz) QZ += r.dQZ;
+    int4 ea = __ldg(row4), eb = __ldg(row4 + 1);
+    for (int n0 = 0; n0 < n_slabs; n0 += U) {
+        const int4 na = __ldg(row4 + (n0 >> 1) + 2), nb = __ldg(row4 + (n0 >> 1) + 3);   // next group
+        const int off0s[U] = {ea.x, ea.z, eb.x, eb.z};
+        const float tts[U] = {__int_as_float(ea.y), __int_as_float(ea.w), __int_as_float(eb.y), __int_as_float(eb.w)};
+        int po[U][3], pk[U][3];
+        float pt[U][3], pv[U][3];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int off0 = off0s[u], off1 = off0s[u] + dT;
+            const float tt = tts[u];
+            const bool cz = (unsigned)(QZ >> 32) == (unsigned)(n0 + u);
+            const float tz = cz ? __uint2float_rn((unsigned)QZ) * inv32 : 1.f;
+            const int ke = cz ? k + r.dirZ : k;
+            const float t1 = fminf(tt, tz), t2 = fmaxf(tt, tz);
+            const bool tfirst = tt < tz;
+            po[u][0] = off0;                  pk[u][0] = k;                pt[u][0] = t1;
+            po[u][1] = tfirst ? off1 : off0;  pk[u][1] = tfirst ? k : ke;  pt[u][1] = t2 - t1;
+            po[u][2] = off1;                  pk[u][2] = ke;               pt[u][2] = 1.f - t2;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) pv[u][i] = sink.fetch(po[u][i], pk[u][i]);
+            k = ke;
+            if (cz) QZ += r.dQZ;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) sink.add(po[u][i], pk[u][i], pt[u][i], pv[u][i]);
+        }
+        ea = na; eb = nb;
     }
 }
 
@@ -202,9 +232,10 @@ struct AccSink {
     const float* __restrict__ vol;
     int Nz;
     float acc;
-    __device__ __forceinline__ void operator()(int off, int k, float tau) {
-        if (!CHECK || (unsigned)k < (unsigned)Nz) acc = fmaf(tau, __ldg(vol + (unsigned)(off + k)), acc);
+    __device__ __forceinline__ float fetch(int off, int k) const {
+        return (!CHECK || (unsigned)k < (unsigned)Nz) ? __ldg(vol + (unsigned)(off + k)) : 0.f;
     }
+    __device__ __forceinline__ void add(int, int, float tau, float v) { acc = fmaf(tau, v, acc); }
 };
 
 __global__ void __launch_bounds__(NT)
@@ -280,7 +311,8 @@ struct RecSink {
     float Ls, eps;
     int* ijk;
     float* len;
-    __device__ __forceinline__ void operator()(int off, int k, float tau) {
+    __device__ __forceinline__ float fetch(int, int) const { return 0.f; }
+    __device__ __forceinline__ void add(int off, int k, float tau, float) {
         if (!((unsigned)k < (unsigned)nz)) return;
         const int col = off / nz, jy = col / pnx - 1, jx = col % pnx - 1;
         if (!((unsigned)jx < (unsigned)nx && (unsigned)jy < (unsigned)ny)) return;      // zero border
@@ -317,7 +349,8 @@ __global__ void k_traverse(const Geom G, const ColHdr* __restrict__ hdr, const S
 }  // namespace
 
 int project_blocks(const Geom& G) { return ((G.nu + PW - 1) / PW) * ((G.nv + 31) / 32); }
-int max_slabs(const Geom& G) { return G.nx > G.ny ? G.nx : G.ny; }
+// slabs per table row: the longest march, rounded up to the group size, plus one group read ahead
+int max_slabs(const Geom& G) { return ((G.nx > G.ny ? G.nx : G.ny) + U - 1) / U * U + U; }
 
 void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, ColHdr* hdr, SlabEntry* tab) {
     q.launch(k_view_tables, dim3(G.nu, B), dim3(128), 0, G, solves, hdr, tab, max_slabs(G));

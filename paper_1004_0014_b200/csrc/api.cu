@@ -83,7 +83,7 @@ struct pcamm_model {
     float *f0 = nullptr, *fields = nullptr, *xbar = nullptr, *u = nullptr, *lm0 = nullptr;   // xbar, u: views of fields
     FieldStream fs;
     // scratch (device)
-    float *vol = nullptr, *p = nullptr, *rL = nullptr;   // vol: trial volumes, ray layout [S][PV]
+    float *vol = nullptr, *pseg = nullptr, *p = nullptr, *rL = nullptr;   // vol: trial volumes, ray layout [S][PV]
     ColHdr* col_hdr = nullptr;      // [B][nu]
     SlabEntry* slab_tab = nullptr;  // [B][nu][max_slabs]
     float4* utab = nullptr;
@@ -192,7 +192,7 @@ void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     launch_begin(q, G, m->c, 0);
     launch_view_tables(q, G, m->c.solves, B, m->col_hdr, m->slab_tab);
     launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV);
-    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
+    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
     launch_ctl_init(q, G, m->c, h_iter, use_cond);
 }
 
@@ -206,7 +206,7 @@ void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial,
 void seq_trial(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_trial, int use_cond) {
     const Geom& G = m->G;
     launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV);
-    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
+    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
     launch_ctl_trial(q, G, m->c, h_trial, use_cond);
 }
 
@@ -468,7 +468,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return r == cudaSuccess; };
     ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->fields, 3 * (size_t)V * (G.K + 1))) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
         ok(dalloc(m, &m->vol, S * (size_t)G.PV)) && ok(dalloc(m, &m->col_hdr, B * G.nu)) &&
-        ok(dalloc(m, &m->slab_tab, B * G.nu * (size_t)max_slabs(G))) && ok(dalloc(m, &m->p, S * G.npix)) &&
+        ok(dalloc(m, &m->slab_tab, B * G.nu * (size_t)max_slabs(G))) && ok(dalloc(m, &m->p, S * G.npix)) && ok(dalloc(m, &m->pseg, S * G.npix * (size_t)project_segments(G))) &&
         ok(dalloc(m, &m->rL, B * G.npix)) && ok(dalloc(m, &m->utab, B * G.nu)) && ok(dalloc(m, &m->vtab, B * G.nv)) &&
         ok(dalloc(m, &m->in_block, m->in_block_bytes)) && ok(dalloc(m, &m->c.solves, B)) &&
         ok(dalloc(m, &m->c.traces, B)) && ok(dalloc(m, &m->c.slots, S)) && ok(dalloc(m, &m->c.flags, 1)) &&
@@ -533,7 +533,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     // the streaming kernels' view of the fields: TMA tensor map (else the generic kernels)
     m->fs.fields = m->fields;
     std::string why;
-    m->fs.use_tma = make_field_map(G, m->fields, 3 * (G.K + 1), 32, &m->fs.map32, &why);
+    m->fs.use_tma = make_field_map(G, m->fields, 3 * (G.K + 1), 32, &m->fs.map32, &why) &&
+                    make_field_map(G, m->fields, 3 * (G.K + 1), 16, &m->fs.map16, &why);
     m->c.grad_blocks = grad_blocks(G, m->fs);
     *out = m;
     return PCAMM_OK;
@@ -585,7 +586,7 @@ int pcamm_project(pcamm_model* m, const float* volume_dev, float angle_rad, floa
     if (rc) return rc;
     launch_view_tables(q, m->G, m->c.solves, 1, m->col_hdr, m->slab_tab);
     launch_to_ray_layout(q, m->G, volume_dev, m->vol);
-    launch_project(q, m->G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
+    launch_project(q, m->G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
     if ((rc = check_seq(q, "project"))) return rc;
     CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * m->G.npix, cudaMemcpyDeviceToDevice, st));
     CUDA_TRY(cudaStreamSynchronize(st));
@@ -616,7 +617,7 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     launch_ysums(q2, G, m->c, 1);
     launch_view_tables(q2, G, m->c.solves, 1, m->col_hdr, m->slab_tab);
     launch_warp(q2, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV);
-    launch_project(q2, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
+    launch_project(q2, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
     launch_ctl_eval(q2, G, m->c, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
     launch_grad(q2, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
@@ -694,7 +695,7 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
         if (which == 0)
             launch_warp(q, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV);
         else if (which == 1)
-            launch_project(q, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->p, m->c.proj_part);
+            launch_project(q, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
         else
             launch_grad(q, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
     }

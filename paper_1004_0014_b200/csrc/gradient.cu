@@ -208,7 +208,7 @@ k_grad_generic(const Geom G, const float* __restrict__ f0, const float* __restri
 }
 
 int grad_grid(const Geom& G, const FieldStream& fs) {
-    const long long nt = tile_count(G, 32);
+    const long long nt = tile_count(G, G.K <= 5 ? 32 : 16);      // TileZ<K>
     return (int)(nt < fs.n_sm ? nt : fs.n_sm);
 }
 
@@ -226,13 +226,11 @@ int grad_grid(const Geom& G, const FieldStream& fs) {
 // Per tile and solve the group's K sums are reduced in double and added to the group's slot of
 // the partial-sum buffer; the control kernel adds the slots in index order.
 
-constexpr int GTZ = 32;
 constexpr int GNG = 2;
 constexpr int GTHREADS = 32 * (GNG * GROUP_WARPS + 1);
-constexpr int GROWS = GTZ / GROUP_WARPS;            // voxels per thread and tile
+constexpr int GSTATIC = 12 * 1024;                  // static shared memory of the kernel, rounded up
 constexpr int SOLVE_CACHE = 64;                     // solves whose constants are kept in shared memory
 
-template <int K> struct GradStages { static constexpr int value = K <= 3 ? 3 : 2; };
 template <int K> struct GradBatch { static constexpr int value = K <= 3 ? 4 : 2; };     // RB
 
 template <int K>
@@ -242,9 +240,13 @@ struct QueueEntry {
 };
 
 template <int K>
+constexpr size_t grad_queue_bytes() { return (size_t)GNG * GROUP_THREADS * GradBatch<K>::value * sizeof(QueueEntry<K>); }
+template <int K> struct GradStages {
+    static constexpr int value = ring_stages<K>(3, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
+};
+template <int K>
 constexpr size_t grad_smem_bytes() {
-    return FieldRing<3 * (K + 1), GTZ, GradStages<K>::value>::BYTES + 16 +
-           (size_t)GNG * GROUP_THREADS * GradBatch<K>::value * sizeof(QueueEntry<K>);
+    return FieldRing<3 * (K + 1), TileZ<K>::value, GradStages<K>::value>::BYTES + 16 + grad_queue_bytes<K>();
 }
 
 // SINGLE: one solve (B = 1): the K sums stay in registers over all tiles of the CTA and are
@@ -254,7 +256,9 @@ __global__ void __launch_bounds__(GTHREADS, 1)
 k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
            const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
            const float2* __restrict__ vtab, double* __restrict__ partials) {
-    constexpr int P = 3 * (K + 1), NS = GradStages<K>::value, RB = GradBatch<K>::value, NB = GROWS / RB;
+    constexpr int P = 3 * (K + 1), NS = GradStages<K>::value, GTZ = TileZ<K>::value, GROWS = GTZ / GROUP_WARPS;
+    constexpr int RB = GradBatch<K>::value, NB = GROWS / RB;
+    static_assert(GROWS % RB == 0 && NB >= 1, "tile rows per thread must be a multiple of the batch");
     using Ring = FieldRing<P, GTZ, NS>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ int s_cnt[GNG][32];
@@ -456,13 +460,13 @@ void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, con
         }
         const int grid = grad_grid(G, fs), nslot = grid * GNG;
         if (B == 1) {
-            q.launch(k_grad_tma<K, true>, dim3(grid), dim3(GTHREADS), smem, fs.map32, G, f0, solves, 1, rL, utab, vtab,
+            q.launch(k_grad_tma<K, true>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), G, f0, solves, 1, rL, utab, vtab,
                      partials);
             return;
         }
         for (int b0 = 0; b0 < B; b0 += SOLVE_CACHE) {       // the kernel keeps up to SOLVE_CACHE solves' constants on chip
             const int nb = B - b0 < SOLVE_CACHE ? B - b0 : SOLVE_CACHE;
-            q.launch(k_grad_tma<K, false>, dim3(grid), dim3(GTHREADS), smem, fs.map32, G, f0, solves + b0, nb,
+            q.launch(k_grad_tma<K, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), G, f0, solves + b0, nb,
                      rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu, vtab + (long long)b0 * G.nv,
                      partials + (long long)b0 * nslot * KMAX);
         }

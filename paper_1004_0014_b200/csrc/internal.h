@@ -86,8 +86,10 @@ int max_slabs(const Geom& G);
 void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, ColHdr* hdr, SlabEntry* tab);
 // p[s] = P f[s] for every active slot (volumes in the ray layout); per-block partial sums
 // {sum p, sum y p, sum (p - a y - b)^2}.
+int project_segments(const Geom& G);
+// pseg: scratch [nslots][segments][nu][nv] for the per-segment partial line integrals
 void launch_project(Seq& q, const Geom& G, const SlotState* slots, const SolveState* solves, const SolveIn* in,
-                    int nslots, const ColHdr* hdr, const SlabEntry* tab, const float* vol, float* p,
+                    int nslots, const ColHdr* hdr, const SlabEntry* tab, const float* vol, float* pseg, float* p,
                     double* partials);
 // hooks: standard layout -> ray layout; one ray of the view of solve 0
 void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray);

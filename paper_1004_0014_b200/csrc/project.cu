@@ -36,6 +36,7 @@ namespace {
 
 constexpr int PW = 4;             // warps (= detector columns) per block
 constexpr int NT = 32 * PW;
+constexpr int SEG = 64;           // slabs per block (a multiple of the march's group size)
 
 constexpr double FIX = 4294967296.0;            // 2^32
 constexpr double QMAX = 1073741824.0;           // crossings beyond any volume are parked here (2^30 slabs)
@@ -163,15 +164,17 @@ __device__ __forceinline__ void first_crossing(double P0, double s, int* idx0, i
     if (*dQ < (1ull << 32)) *dQ = 1ull << 32;   // |s| <= 1: never two crossings in one slab
 }
 
-__device__ __forceinline__ RayZ make_ray_z(const Geom& G, const ColHdr& h, int iv) {
+// z state of the ray of row iv at the entry of slab n0 of its column (slabs are then counted
+// from there), for a march of n slabs.
+__device__ __forceinline__ RayZ make_ray_z(const Geom& G, const ColHdr& h, int iv, int n0, int n) {
     RayZ r;
     const double dz = ((double)iv - 0.5 * (G.nv - 1) + (double)G.off_v) * (double)G.pv;
     const double gz = dz / (double)G.hz;
     const double Szi = (0.0 - G.loz) / (double)G.hz;                      // the source is in the plane z = 0
     const double sz = gz * h.kap;                                         // z per slab
-    first_crossing(fma(gz, h.lam0, Szi), sz, &r.k, &r.dirZ, &r.QZ, &r.dQZ);
+    first_crossing(fma(gz, fma(h.kap, (double)n0, h.lam0), Szi), sz, &r.k, &r.dirZ, &r.QZ, &r.dQZ);
     r.Ls = (float)(sqrt((double)h.dxy2 + dz * dz) * h.kap);
-    const int ncross = (int)(fabs(sz) * (double)h.n_slabs) + 2;           // conservative
+    const int ncross = (int)(fabs(sz) * (double)n) + 2;                   // conservative
     r.kmin = r.dirZ < 0 ? r.k - ncross : r.k;
     r.kmax = r.dirZ > 0 ? r.k + ncross : r.k;
     return r;
@@ -238,50 +241,92 @@ struct AccSink {
     __device__ __forceinline__ void add(int, int, float tau, float v) { acc = fmaf(tau, v, acc); }
 };
 
+// Grid: (columns / PW, row groups of 32, slots x segments).  A block marches SEG slabs of its
+// rays: the rows of the grid are cut into segments so that there are several times more blocks
+// than fit on the GPU at once and the hardware block scheduler keeps every SM busy to the end
+// (with one block per ray group everything is resident at once and the last third of the
+// kernel runs half empty: profiles/r01).  Segment s of a ray starts from the exact z state at
+// its first slab (double precision set-up) and writes its partial line integral to
+// pseg[slot][s][iu][iv]; k_project_finish adds the segments in index order.
 __global__ void __launch_bounds__(NT)
-k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* __restrict__ solves,
-          const SolveIn* __restrict__ in, const ColHdr* __restrict__ hdr, const SlabEntry* __restrict__ tab,
-          int max_slabs, const float* __restrict__ vol, float* __restrict__ p_out, double* __restrict__ partials) {
-    __shared__ double red[NT / 32];
-    const int s = blockIdx.z;
+k_project(const Geom G, const SlotState* __restrict__ slots, const ColHdr* __restrict__ hdr,
+          const SlabEntry* __restrict__ tab, int max_slabs, int n_seg, const float* __restrict__ vol,
+          float* __restrict__ pseg) {
+    const int s = blockIdx.z / n_seg, seg = blockIdx.z % n_seg;
     if (!slots[s].active) return;
     const int b = slots[s].solve;
     const int iu = blockIdx.x * PW + (threadIdx.x >> 5);
     const int iv = blockIdx.y * 32 + (threadIdx.x & 31);
-    double vp = 0.0, vyp = 0.0, vrr = 0.0;
-    if (iu < G.nu && iv < G.nv) {
-        const ColHdr h = hdr[(long long)b * G.nu + iu];
-        float p = 0.f;
-        if (h.n_slabs > 0) {
-            const RayZ r = make_ray_z(G, h, iv);
-            const SlabEntry* row = tab + ((long long)b * G.nu + iu) * max_slabs;
-            const float* base = vol + (long long)s * G.PV;
-            asm volatile("" : "+l"(base));       // one base pointer; 32-bit offsets in the loop
-            float acc;
-            if (r.kmin >= 0 && r.kmax < G.nz) {
-                AccSink<false> sink{base, G.nz, 0.f};
-                march(row, h.n_slabs, h.dT, r, sink);
-                acc = sink.acc;
-            } else {
-                AccSink<true> sink{base, G.nz, 0.f};
-                march(row, h.n_slabs, h.dT, r, sink);
-                acc = sink.acc;
-            }
-            p = acc * r.Ls;
+    if (iu >= G.nu || iv >= G.nv) return;
+    const ColHdr h = hdr[(long long)b * G.nu + iu];
+    const int n0 = seg * SEG, n = min(h.n_slabs - n0, SEG);
+    float p = 0.f;
+    if (n > 0) {
+        const RayZ r = make_ray_z(G, h, iv, n0, n);
+        const SlabEntry* row = tab + ((long long)b * G.nu + iu) * max_slabs + n0;
+        const float* base = vol + (long long)s * G.PV;
+        asm volatile("" : "+l"(base));       // one base pointer; 32-bit offsets in the loop
+        float acc;
+        if (r.kmin >= 0 && r.kmax < G.nz) {
+            AccSink<false> sink{base, G.nz, 0.f};
+            march(row, n, h.dT, r, sink);
+            acc = sink.acc;
+        } else {
+            AccSink<true> sink{base, G.nz, 0.f};
+            march(row, n, h.dT, r, sink);
+            acc = sink.acc;
         }
-        const int pix = iv * G.nu + iu;
-        p_out[(long long)s * G.npix + pix] = p;
-        const float* y = in[b].y;
-        const double yv = y ? (double)__ldg(y + pix) : 0.0;
-        const double res = (double)p - solves[b].a * yv - solves[b].b;   // Eq. (2) residual
-        vp = (double)p; vyp = yv * (double)p; vrr = res * res;
+        p = acc * r.Ls;
+    }
+    pseg[(((long long)s * n_seg + seg) * G.nu + iu) * G.nv + iv] = p;
+}
+
+// p = sum of the segments (fixed order), and a-3: r_i = p_i - a y_i - b with the per-block partial
+// sums of p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.  Tile of 32 columns x 32
+// rows: the partial images are column-major (rows contiguous, as the projector's warps write
+// them), p and y are row-major.
+constexpr int FT = 256;
+__global__ void __launch_bounds__(FT)
+k_project_finish(const Geom G, const SlotState* __restrict__ slots, const SolveState* __restrict__ solves,
+                 const SolveIn* __restrict__ in, int n_seg, const float* __restrict__ pseg, float* __restrict__ p_out,
+                 double* __restrict__ partials) {
+    __shared__ float tile[32][33];
+    __shared__ double red[FT / 32];
+    const int s = blockIdx.z;
+    if (!slots[s].active) return;
+    const int b = slots[s].solve;
+    const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
+    const int u0 = blockIdx.x * 32, v0 = blockIdx.y * 32;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int iu = u0 + tw + 8 * r, iv = v0 + lane;
+        float acc = 0.f;
+        if (iu < G.nu && iv < G.nv)
+            for (int g = 0; g < n_seg; ++g) acc += pseg[(((long long)s * n_seg + g) * G.nu + iu) * G.nv + iv];
+        tile[tw + 8 * r][lane] = acc;
+    }
+    __syncthreads();
+    double vp = 0.0, vyp = 0.0, vrr = 0.0;
+    const float* y = in[b].y;
+    const double a = solves[b].a, bb = solves[b].b;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int iv = v0 + tw + 8 * r, iu = u0 + lane;
+        if (iu < G.nu && iv < G.nv) {
+            const float p = tile[lane][tw + 8 * r];
+            const int pix = iv * G.nu + iu;
+            p_out[(long long)s * G.npix + pix] = p;
+            const double yv = y ? (double)__ldg(y + pix) : 0.0;
+            const double res = (double)p - a * yv - bb;                   // Eq. (2) residual
+            vp += (double)p; vyp += yv * (double)p; vrr += res * res;
+        }
     }
     const int nblk = gridDim.x * gridDim.y;
     const int blk = blockIdx.y * gridDim.x + blockIdx.x;
     double* out = partials + ((long long)s * nblk + blk) * 3;
-    const double sp = block_sum<NT>(vp, red);
-    const double syp = block_sum<NT>(vyp, red);
-    const double srr = block_sum<NT>(vrr, red);
+    const double sp = block_sum<FT>(vp, red);
+    const double syp = block_sum<FT>(vyp, red);
+    const double srr = block_sum<FT>(vrr, red);
     if (threadIdx.x == 0) { out[0] = sp; out[1] = syp; out[2] = srr; }
 }
 
@@ -339,7 +384,7 @@ __global__ void k_traverse(const Geom G, const ColHdr* __restrict__ hdr, const S
     sink.Ls = 0.f;
     sink.ijk = ijk; sink.len = len;
     if (h.n_slabs > 0) {
-        const RayZ r = make_ray_z(G, h, iv);
+        const RayZ r = make_ray_z(G, h, iv, 0, h.n_slabs);
         sink.Ls = r.Ls;
         march(tab + (long long)iu * max_slabs, h.n_slabs, h.dT, r, sink);
     }
@@ -348,19 +393,23 @@ __global__ void k_traverse(const Geom G, const ColHdr* __restrict__ hdr, const S
 
 }  // namespace
 
-int project_blocks(const Geom& G) { return ((G.nu + PW - 1) / PW) * ((G.nv + 31) / 32); }
+int project_blocks(const Geom& G) { return ((G.nu + 31) / 32) * ((G.nv + 31) / 32); }
 // slabs per table row: the longest march, rounded up to the group size, plus one group read ahead
 int max_slabs(const Geom& G) { return ((G.nx > G.ny ? G.nx : G.ny) + U - 1) / U * U + U; }
+int project_segments(const Geom& G) { return ((G.nx > G.ny ? G.nx : G.ny) + SEG - 1) / SEG; }
 
 void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, ColHdr* hdr, SlabEntry* tab) {
     q.launch(k_view_tables, dim3(G.nu, B), dim3(128), 0, G, solves, hdr, tab, max_slabs(G));
 }
 
 void launch_project(Seq& q, const Geom& G, const SlotState* slots, const SolveState* solves, const SolveIn* in,
-                    int nslots, const ColHdr* hdr, const SlabEntry* tab, const float* vol, float* p,
+                    int nslots, const ColHdr* hdr, const SlabEntry* tab, const float* vol, float* pseg, float* p,
                     double* partials) {
-    q.launch(k_project, dim3((G.nu + PW - 1) / PW, (G.nv + 31) / 32, nslots), dim3(NT), 0, G, slots, solves, in, hdr,
-             tab, max_slabs(G), vol, p, partials);
+    const int n_seg = project_segments(G);
+    q.launch(k_project, dim3((G.nu + PW - 1) / PW, (G.nv + 31) / 32, nslots * n_seg), dim3(NT), 0, G, slots, hdr, tab,
+             max_slabs(G), n_seg, vol, pseg);
+    q.launch(k_project_finish, dim3((G.nu + 31) / 32, (G.nv + 31) / 32, nslots), dim3(FT), 0, G, slots, solves, in, n_seg,
+             (const float*)pseg, p, partials);
 }
 
 void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray) {

@@ -143,8 +143,22 @@ struct FieldStream {
     const float* fields = nullptr;   // [3(K+1)][V]: xbar's planes, then u_1 .. u_K
     bool use_tma = false;            // false: register-staged generic kernels
     int n_sm = 1;                    // persistent grid size
-    CUtensorMap map32;               // box {TX, 1, 32, 3(K+1)}
+    CUtensorMap map32, map16;        // boxes {TX, 1, 32 | 16, 3(K+1)}
 };
+
+// Tile extent along z and ring depth by K: a stage is 3(K+1) planes x TZ x TX floats and the
+// ring has to fit in 227 KB of shared memory next to the kernel's own buffers.
+template <int K> struct TileZ { static constexpr int value = K <= 5 ? 32 : 16; };
+template <int K>
+constexpr int ring_stages(int max_stages, int budget_bytes) {
+    const int stage = 3 * (K + 1) * TileZ<K>::value * TX * 4;
+    const int n = budget_bytes / stage;
+    return n < max_stages ? (n < 1 ? 1 : n) : max_stages;
+}
+template <int K>
+__host__ __device__ __forceinline__ const CUtensorMap& field_map(const FieldStream& fs) {
+    return TileZ<K>::value == 32 ? fs.map32 : fs.map16;
+}
 
 // Host: the tensor map of the fields [P][nz][ny][nx] (xbar's three planes first, then u_1 .. u_K)
 // with box {TX, 1, tz, P}.  Returns false if the driver entry point is missing or the shape

@@ -112,26 +112,26 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
 
 // ---------------------------------------------------------------- the TMA-fed kernel
 
-constexpr int WTZ = 32;            // tile extent along z (the transposed store needs 32)
 constexpr int WNG = 3;             // consumer groups
 constexpr int SLOT_CACHE = 64;     // slots whose coefficients are kept in shared memory
 constexpr int WTHREADS = 32 * (WNG * GROUP_WARPS + 1);
 
-template <int K> struct WarpStages { static constexpr int value = K <= 3 ? 4 : (K <= 5 ? 3 : 2); };
+constexpr int WSTATIC = 16 * 1024; // static shared memory of the kernel (transposition tiles, slot cache), rounded up
+template <int K> struct WarpStages { static constexpr int value = ring_stages<K>(4, 227 * 1024 - WSTATIC - 64); };
 
 template <int K>
 constexpr size_t warp_smem_bytes() {
-    return FieldRing<3 * (K + 1), WTZ, WarpStages<K>::value>::BYTES;
+    return FieldRing<3 * (K + 1), TileZ<K>::value, WarpStages<K>::value>::BYTES;
 }
 
 template <int K, bool RAY>
 __global__ void __launch_bounds__(WTHREADS, 1)
 k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
            const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride) {
-    constexpr int P = 3 * (K + 1), NS = WarpStages<K>::value;
+    constexpr int P = 3 * (K + 1), NS = WarpStages<K>::value, WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
     using Ring = FieldRing<P, WTZ, NS>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    __shared__ float tiles[WNG][TX][TX + 1];
+    __shared__ float tiles[WNG][WTZ][TX + 1];
     __shared__ float s_w[SLOT_CACHE][K];                   // the slots' coefficients (constant during the launch)
     __shared__ int s_active[SLOT_CACHE];
     for (int i = threadIdx.x; i < nslots && i < SLOT_CACHE; i += blockDim.x) {
@@ -170,10 +170,10 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                 float* out = vol_out + (long long)sl * slot_stride;
                 // voxels of a ragged tile beyond the grid: TMA filled their fields with zeros, the
                 // taps are clamped, the value is computed and not stored
-                float val[ROWS];
-                Taps taps[ROWS];
+                float val[WROWS];
+                Taps taps[WROWS];
 #pragma unroll
-                for (int r = 0; r < ROWS; ++r) {
+                for (int r = 0; r < WROWS; ++r) {
                     const int zz = tw + GROUP_WARPS * r, z = c.z0 + zz;
                     float d[3];
 #pragma unroll
@@ -185,27 +185,28 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     }
                     taps[r] = make_taps(G.nx, G.ny, G.nz, x, c.y, z, d[0], d[1], d[2]);
                 }
-                float cv[ROWS][8];
+                float cv[WROWS][8];
 #pragma unroll
-                for (int r = 0; r < ROWS; ++r) gather8(f0, taps[r], cv[r]);     // 8 ROWS gathers in flight
+                for (int r = 0; r < WROWS; ++r) gather8(f0, taps[r], cv[r]);    // 8 WROWS gathers in flight
 #pragma unroll
-                for (int r = 0; r < ROWS; ++r) val[r] = combine8(taps[r], cv[r]);
+                for (int r = 0; r < WROWS; ++r) val[r] = combine8(taps[r], cv[r]);
                 if (!RAY) {
 #pragma unroll
-                    for (int r = 0; r < ROWS; ++r) {
+                    for (int r = 0; r < WROWS; ++r) {
                         const int z = c.z0 + tw + GROUP_WARPS * r;
                         if (x < G.nx && z < G.nz) out[((long long)z * G.ny + c.y) * G.nx + x] = val[r];
                     }
                 } else {
                     group_barrier(group);
 #pragma unroll
-                    for (int r = 0; r < ROWS; ++r) tile[tw + GROUP_WARPS * r][lane] = val[r];
+                    for (int r = 0; r < WROWS; ++r) tile[tw + GROUP_WARPS * r][lane] = val[r];
                     group_barrier(group);
                     const int zo = c.z0 + lane;
 #pragma unroll
-                    for (int r = 0; r < ROWS; ++r) {
+                    for (int r = 0; r < TX / GROUP_WARPS; ++r) {
                         const int xo = c.x0 + tw + GROUP_WARPS * r;
-                        if (xo < G.nx && zo < G.nz) out[ray_layout_index(G, xo, c.y, zo)] = tile[lane][tw + GROUP_WARPS * r];
+                        if (lane < WTZ && xo < G.nx && zo < G.nz)
+                            out[ray_layout_index(G, xo, c.y, zo)] = tile[lane][tw + GROUP_WARPS * r];
                     }
                 }
             }
@@ -227,7 +228,7 @@ void launch_tma(Seq& q, const Geom& G, const CUtensorMap& fmap, int n_sm, const 
         if (e != cudaSuccess) { q.err = e; return; }
         configured = true;
     }
-    const long long nt = tile_count(G, WTZ);
+    const long long nt = tile_count(G, TileZ<K>::value);
     const int grid = (int)(nt < n_sm ? nt : n_sm);
     for (int s0 = 0; s0 < nslots; s0 += SLOT_CACHE) {      // the kernel keeps up to SLOT_CACHE slots' coefficients on chip
         const int ns = nslots - s0 < SLOT_CACHE ? nslots - s0 : SLOT_CACHE;
@@ -240,8 +241,8 @@ template <int K>
 void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
               int ray_layout, float* vol_out, long long slot_stride) {
     if (fs.use_tma) {
-        if (ray_layout) launch_tma<K, true>(q, G, fs.map32, fs.n_sm, f0, slots, nslots, vol_out, slot_stride);
-        else launch_tma<K, false>(q, G, fs.map32, fs.n_sm, f0, slots, nslots, vol_out, slot_stride);
+        if (ray_layout) launch_tma<K, true>(q, G, field_map<K>(fs), fs.n_sm, f0, slots, nslots, vol_out, slot_stride);
+        else launch_tma<K, false>(q, G, field_map<K>(fs), fs.n_sm, f0, slots, nslots, vol_out, slot_stride);
         return;
     }
     const float* xbar = fs.fields;

@@ -181,7 +181,7 @@ def test_backprojection_is_the_transpose(theta):
     assert rel_l2(Ptr, ref) <= 1e-4
 
 
-@pytest.mark.parametrize("K,seed,theta", [(3, 11, 0.6), (5, 12, 2.2), (2, 13, 4.1), (3, 14, np.pi / 4)])
+@pytest.mark.parametrize("K,seed,theta", [(3, 11, 0.6), (5, 12, 2.2), (2, 13, 4.1), (3, 14, np.pi / 4), (8, 15, 1.1), (6, 16, 3.0)])
 def test_eval_matches_oracle(K, seed, theta):
     g = _geom(K=K)
     f0, xbar, u, scale, m = _model(g, seed=seed, disp_vox=1.2)

@@ -192,8 +192,7 @@ void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     launch_begin(q, G, m->c, 0);
     launch_view_tables(q, G, m->c.solves, B, m->col_hdr, m->slab_tab);
     launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV);
-    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
-    launch_ctl_init(q, G, m->c, h_iter, use_cond);
+    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_INIT, h_iter, use_cond);
 }
 
 void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial, int use_cond) {
@@ -206,8 +205,7 @@ void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial,
 void seq_trial(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_trial, int use_cond) {
     const Geom& G = m->G;
     launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV);
-    launch_project(q, G, m->c.slots, m->c.solves, m->c.in, B * C, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
-    launch_ctl_trial(q, G, m->c, h_trial, use_cond);
+    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_TRIAL, h_trial, use_cond);
 }
 
 void seq_tail(pcamm_model* m, Seq& q, int B) {
@@ -586,7 +584,7 @@ int pcamm_project(pcamm_model* m, const float* volume_dev, float angle_rad, floa
     if (rc) return rc;
     launch_view_tables(q, m->G, m->c.solves, 1, m->col_hdr, m->slab_tab);
     launch_to_ray_layout(q, m->G, volume_dev, m->vol);
-    launch_project(q, m->G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
+    launch_project(q, m->G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_NONE, 0, 0);
     if ((rc = check_seq(q, "project"))) return rc;
     CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * m->G.npix, cudaMemcpyDeviceToDevice, st));
     CUDA_TRY(cudaStreamSynchronize(st));
@@ -617,11 +615,10 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     launch_ysums(q2, G, m->c, 1);
     launch_view_tables(q2, G, m->c.solves, 1, m->col_hdr, m->slab_tab);
     launch_warp(q2, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV);
-    launch_project(q2, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
-    launch_ctl_eval(q2, G, m->c, 0);
+    launch_project(q2, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_EVAL, 0, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
     launch_grad(q2, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
-    launch_ctl_eval(q2, G, m->c, 1);
+    launch_ctl_eval_grad(q2, G, m->c);
     if ((rc = check_seq(q2, "eval"))) return rc;
     if (proj_out_dev) CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * G.npix, cudaMemcpyDeviceToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState), cudaMemcpyDeviceToHost, st));
@@ -695,7 +692,7 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
         if (which == 0)
             launch_warp(q, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV);
         else if (which == 1)
-            launch_project(q, G, m->c.slots, m->c.solves, m->c.in, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, m->c.proj_part);
+            launch_project(q, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_NONE, 0, 0);
         else
             launch_grad(q, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
     }

@@ -103,7 +103,12 @@ struct SlotState {
 struct LoopFlags {
     int iter_cond, trial_cond;
     long long n_launch;
+    unsigned ticket;          // blocks of k_project_finish that are done (the last one runs the control step)
+    unsigned pad;
 };
+
+// Control step run by the last block of k_project_finish.
+constexpr int THEN_NONE = 0, THEN_INIT = 1, THEN_TRIAL = 2, THEN_EVAL = 3;
 
 // In-plane direction D - S of the rays of detector column iu (independent of the row).
 __device__ __forceinline__ void ray_dir_inplane(const Geom& G, double cs, double sn, int iu, double* dx, double* dy) {

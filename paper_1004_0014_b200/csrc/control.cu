@@ -85,14 +85,14 @@ k_begin(const Geom G, const CallOpts* __restrict__ opts, const SolveIn* __restri
         for (int k = 0; k < G.K; ++k) s0.w[k] = in[b].w_init[k];
         s0.active = 1;
     }
-    if (threadIdx.x == 0) { flags->iter_cond = 0; flags->trial_cond = 0; flags->n_launch = 0; }
+    if (threadIdx.x == 0) { flags->iter_cond = 0; flags->trial_cond = 0; flags->n_launch = 0; flags->ticket = 0u; }
 }
 
 // Sum of n partials with the given stride, by the whole control block (fixed order); the result
 // is broadcast to all threads.
 __device__ double coop_sum(const double* part, int n, int stride, double* red /* [CT/32 + 1] */) {
     double v = 0.0;
-    for (int i = threadIdx.x; i < n; i += CT) v += part[(long long)i * stride];
+    for (int i = threadIdx.x; i < n; i += CT) v += __ldcg(part + (long long)i * stride);   // written by other blocks
     const double s = block_sum<CT>(v, red);
     if (threadIdx.x == 0) red[CT / 32] = s;
     __syncthreads();
@@ -117,8 +117,7 @@ __device__ void publish(LoopFlags* flags, int iter_cond, int trial_cond, int lau
 }
 
 // After the initial evaluation at w0: Sy, Syy, the first fit (reading A8), loop start.
-__global__ void __launch_bounds__(CT)
-k_ctl_init(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_iter, int use_cond) {
+__device__ void ctl_init_body(const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond) {
     __shared__ double red[CT / 32 + 1];
     int any_running = 0;
     const CallOpts& o = *c.opts;
@@ -141,7 +140,7 @@ k_ctl_init(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_iter, int use_c
         any_running |= st.running;
     }
     if (threadIdx.x == 0) {
-        publish(c.flags, any_running, 0, 5);
+        publish(c.flags, any_running, 0, 6);
         if (use_cond) cudaGraphSetConditional(h_iter, any_running);
     }
 }
@@ -196,8 +195,7 @@ k_ctl_grad(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_trial, int use_
 }
 
 // After warp + projection of the candidate(s): Armijo's inequality, Eq. (3) update, Eq. (4) fit.
-__global__ void __launch_bounds__(CT)
-k_ctl_trial(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_trial, int use_cond) {
+__device__ void ctl_trial_body(const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond) {
     __shared__ double red[CT / 32 + 1];
     int any_trial = 0, any_running = 0;
     const CallOpts& o = *c.opts;
@@ -290,8 +288,7 @@ k_ctl_final(const Geom G, CtlBufs c, SlotState* out_slots) {
 
 // pcamm_eval: stage 0 after the projection (J at the given (a, b), fit of Eq. 4), stage 1 after
 // the gradient.
-__global__ void __launch_bounds__(CT)
-k_ctl_eval(const Geom G, CtlBufs c, int stage) {
+__device__ void ctl_eval_body(const Geom& G, const CtlBufs& c, int stage) {
     __shared__ double red[CT / 32 + 1];
     const CallOpts& o = *c.opts;
     for (int b = 0; b < o.B; ++b) {
@@ -316,6 +313,74 @@ k_ctl_eval(const Geom G, CtlBufs c, int stage) {
             for (int k = 0; k < G.K; ++k) st.g[k] = 2.0 * gk[k];
         }
     }
+}
+
+__global__ void __launch_bounds__(CT)
+k_ctl_eval_grad(const Geom G, CtlBufs c) { ctl_eval_body(G, c, 1); }
+
+// a-2 (end) and a-3: p = sum of the projector's segments in index order, r_i = p_i - a y_i - b and
+// the per-block partial sums of p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.
+// Tile of 32 detector columns x 32 rows: the partial images are column-major (rows contiguous,
+// as the projector's warps write them), p and y are row-major.
+// The block that finishes last (ticket) then runs the control step that follows this projection
+// (then = THEN_INIT / THEN_TRIAL / THEN_EVAL), which saves a single-block launch per trial.
+__global__ void __launch_bounds__(CT)
+k_project_finish(const Geom G, CtlBufs c, int n_seg, const float* __restrict__ pseg, float* __restrict__ p_out, int then,
+                 cudaGraphConditionalHandle h, int use_cond) {
+    __shared__ float tile[32][33];
+    __shared__ double red[CT / 32];
+    __shared__ int s_last;
+    const int s = blockIdx.z;
+    const int nblk = gridDim.x * gridDim.y;
+    if (c.slots[s].active) {                                             // uniform over the block
+        const int b = c.slots[s].solve;
+        const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
+        const int u0 = blockIdx.x * 32, v0 = blockIdx.y * 32;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int iu = u0 + tw + 8 * r, iv = v0 + lane;
+            float acc = 0.f;
+            if (iu < G.nu && iv < G.nv)
+                for (int g = 0; g < n_seg; ++g) acc += __ldcg(pseg + (((long long)s * n_seg + g) * G.nu + iu) * G.nv + iv);
+            tile[tw + 8 * r][lane] = acc;
+        }
+        __syncthreads();
+        double vp = 0.0, vyp = 0.0, vrr = 0.0;
+        const float* y = c.in[b].y;
+        const double a = c.solves[b].a, bb = c.solves[b].b;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int iv = v0 + tw + 8 * r, iu = u0 + lane;
+            if (iu < G.nu && iv < G.nv) {
+                const float p = tile[lane][tw + 8 * r];
+                const int pix = iv * G.nu + iu;
+                p_out[(long long)s * G.npix + pix] = p;
+                const double yv = y ? (double)__ldg(y + pix) : 0.0;
+                const double res = (double)p - a * yv - bb;               // Eq. (2) residual
+                vp += (double)p; vyp += yv * (double)p; vrr += res * res;
+            }
+        }
+        const int blk = blockIdx.y * gridDim.x + blockIdx.x;
+        double* out = c.proj_part + ((long long)s * nblk + blk) * 3;
+        const double sp = block_sum<CT>(vp, red);
+        const double syp = block_sum<CT>(vyp, red);
+        const double srr = block_sum<CT>(vrr, red);
+        if (threadIdx.x == 0) { out[0] = sp; out[1] = syp; out[2] = srr; }
+    }
+    if (then == THEN_NONE) return;
+    if (threadIdx.x == 0) {
+        __threadfence();                                                  // this block's partial sums are visible
+        const unsigned total = (unsigned)nblk * gridDim.z;
+        const unsigned t = atomicAdd(&c.flags->ticket, 1u);
+        s_last = t == total - 1u;
+        if (s_last) c.flags->ticket = 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (then == THEN_INIT) ctl_init_body(G, c, h, use_cond);
+    else if (then == THEN_TRIAL) ctl_trial_body(G, c, h, use_cond);
+    else ctl_eval_body(G, c, 0);
 }
 
 // a-6.  One warp per (landmark, solve).  x(r) is the trilinear interpolation of the synthesised
@@ -391,16 +456,8 @@ void launch_begin(Seq& q, const Geom& G, const CtlBufs& c, int mode) {
              c.flags, mode);
 }
 
-void launch_ctl_init(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond) {
-    q.launch(k_ctl_init, dim3(1), dim3(CT), 0, G, c, h_iter, use_cond);
-}
-
 void launch_ctl_grad(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond) {
     q.launch(k_ctl_grad, dim3(1), dim3(CT), 0, G, c, h_trial, use_cond);
-}
-
-void launch_ctl_trial(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond) {
-    q.launch(k_ctl_trial, dim3(1), dim3(CT), 0, G, c, h_trial, use_cond);
 }
 
 void launch_ctl_iter_end(Seq& q, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond) {
@@ -411,8 +468,14 @@ void launch_ctl_final(Seq& q, const Geom& G, const CtlBufs& c, SlotState* out_sl
     q.launch(k_ctl_final, dim3(1), dim3(CT), 0, G, c, out_slots);
 }
 
-void launch_ctl_eval(Seq& q, const Geom& G, const CtlBufs& c, int stage) {
-    q.launch(k_ctl_eval, dim3(1), dim3(CT), 0, G, c, stage);
+void launch_ctl_eval_grad(Seq& q, const Geom& G, const CtlBufs& c) {
+    q.launch(k_ctl_eval_grad, dim3(1), dim3(CT), 0, G, c);
+}
+
+void launch_project_finish(Seq& q, const Geom& G, const CtlBufs& c, int nslots, int n_seg, const float* pseg, float* p,
+                           int then, cudaGraphConditionalHandle h, int use_cond) {
+    q.launch(k_project_finish, dim3((G.nu + 31) / 32, (G.nv + 31) / 32, nslots), dim3(CT), 0, G, c, n_seg, pseg, p, then, h,
+             use_cond);
 }
 
 void launch_invert(Seq& q, const Geom& G, const float* xbar, const float* u, const CtlBufs& c, int B, int M,

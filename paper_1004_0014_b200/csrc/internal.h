@@ -87,10 +87,12 @@ void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, 
 // p[s] = P f[s] for every active slot (volumes in the ray layout); per-block partial sums
 // {sum p, sum y p, sum (p - a y - b)^2}.
 int project_segments(const Geom& G);
-// pseg: scratch [nslots][segments][nu][nv] for the per-segment partial line integrals
-void launch_project(Seq& q, const Geom& G, const SlotState* slots, const SolveState* solves, const SolveIn* in,
-                    int nslots, const ColHdr* hdr, const SlabEntry* tab, const float* vol, float* pseg, float* p,
-                    double* partials);
+struct CtlBufs;
+// p[s] = P f[s] for every active slot (volumes in the ray layout; pseg: scratch
+// [nslots][segments][nu][nv] for the per-segment partial line integrals), the a-3 partial sums
+// {sum p, sum y p, sum (p - a y - b)^2}, and then the control step `then` (THEN_*, common.cuh).
+void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const ColHdr* hdr, const SlabEntry* tab,
+                    const float* vol, float* pseg, float* p, int then, cudaGraphConditionalHandle h, int use_cond);
 // hooks: standard layout -> ray layout; one ray of the view of solve 0
 void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray);
 void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* tab, int iu, int iv, int cap,
@@ -129,12 +131,12 @@ int ysum_blocks(const Geom& G);
 void launch_ysums(Seq& q, const Geom& G, const CtlBufs& c, int B);
 // begin: views, w = w_init, slot 0 of every solve = w_init.  mode 0 solve, 1 eval hook.
 void launch_begin(Seq& q, const Geom& G, const CtlBufs& c, int mode);
-void launch_ctl_init(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond);
 void launch_ctl_grad(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond);
-void launch_ctl_trial(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond);
 void launch_ctl_iter_end(Seq& q, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond);
 void launch_ctl_final(Seq& q, const Geom& G, const CtlBufs& c, SlotState* out_slots);
-void launch_ctl_eval(Seq& q, const Geom& G, const CtlBufs& c, int stage);
+void launch_ctl_eval_grad(Seq& q, const Geom& G, const CtlBufs& c);
+void launch_project_finish(Seq& q, const Geom& G, const CtlBufs& c, int nslots, int n_seg, const float* pseg, float* p,
+                           int then, cudaGraphConditionalHandle h, int use_cond);
 // a-6: landmarks [B][M][3]
 void launch_invert(Seq& q, const Geom& G, const float* xbar, const float* u, const CtlBufs& c, int B, int M,
                    const float* r0, double* r_out);

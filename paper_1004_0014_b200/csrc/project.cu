@@ -247,7 +247,7 @@ struct AccSink {
 // (with one block per ray group everything is resident at once and the last third of the
 // kernel runs half empty: profiles/r01).  Segment s of a ray starts from the exact z state at
 // its first slab (double precision set-up) and writes its partial line integral to
-// pseg[slot][s][iu][iv]; k_project_finish adds the segments in index order.
+// pseg[slot][s][iu][iv]; k_project_finish (control.cu) adds the segments in index order.
 __global__ void __launch_bounds__(NT)
 k_project(const Geom G, const SlotState* __restrict__ slots, const ColHdr* __restrict__ hdr,
           const SlabEntry* __restrict__ tab, int max_slabs, int n_seg, const float* __restrict__ vol,
@@ -279,55 +279,6 @@ k_project(const Geom G, const SlotState* __restrict__ slots, const ColHdr* __res
         p = acc * r.Ls;
     }
     pseg[(((long long)s * n_seg + seg) * G.nu + iu) * G.nv + iv] = p;
-}
-
-// p = sum of the segments (fixed order), and a-3: r_i = p_i - a y_i - b with the per-block partial
-// sums of p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.  Tile of 32 columns x 32
-// rows: the partial images are column-major (rows contiguous, as the projector's warps write
-// them), p and y are row-major.
-constexpr int FT = 256;
-__global__ void __launch_bounds__(FT)
-k_project_finish(const Geom G, const SlotState* __restrict__ slots, const SolveState* __restrict__ solves,
-                 const SolveIn* __restrict__ in, int n_seg, const float* __restrict__ pseg, float* __restrict__ p_out,
-                 double* __restrict__ partials) {
-    __shared__ float tile[32][33];
-    __shared__ double red[FT / 32];
-    const int s = blockIdx.z;
-    if (!slots[s].active) return;
-    const int b = slots[s].solve;
-    const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
-    const int u0 = blockIdx.x * 32, v0 = blockIdx.y * 32;
-#pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const int iu = u0 + tw + 8 * r, iv = v0 + lane;
-        float acc = 0.f;
-        if (iu < G.nu && iv < G.nv)
-            for (int g = 0; g < n_seg; ++g) acc += pseg[(((long long)s * n_seg + g) * G.nu + iu) * G.nv + iv];
-        tile[tw + 8 * r][lane] = acc;
-    }
-    __syncthreads();
-    double vp = 0.0, vyp = 0.0, vrr = 0.0;
-    const float* y = in[b].y;
-    const double a = solves[b].a, bb = solves[b].b;
-#pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const int iv = v0 + tw + 8 * r, iu = u0 + lane;
-        if (iu < G.nu && iv < G.nv) {
-            const float p = tile[lane][tw + 8 * r];
-            const int pix = iv * G.nu + iu;
-            p_out[(long long)s * G.npix + pix] = p;
-            const double yv = y ? (double)__ldg(y + pix) : 0.0;
-            const double res = (double)p - a * yv - bb;                   // Eq. (2) residual
-            vp += (double)p; vyp += yv * (double)p; vrr += res * res;
-        }
-    }
-    const int nblk = gridDim.x * gridDim.y;
-    const int blk = blockIdx.y * gridDim.x + blockIdx.x;
-    double* out = partials + ((long long)s * nblk + blk) * 3;
-    const double sp = block_sum<FT>(vp, red);
-    const double syp = block_sum<FT>(vyp, red);
-    const double srr = block_sum<FT>(vrr, red);
-    if (threadIdx.x == 0) { out[0] = sp; out[1] = syp; out[2] = srr; }
 }
 
 // Standard [z][y][x] -> ray layout (hook path only: the solve's volumes are written in the ray
@@ -402,14 +353,12 @@ void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, 
     q.launch(k_view_tables, dim3(G.nu, B), dim3(128), 0, G, solves, hdr, tab, max_slabs(G));
 }
 
-void launch_project(Seq& q, const Geom& G, const SlotState* slots, const SolveState* solves, const SolveIn* in,
-                    int nslots, const ColHdr* hdr, const SlabEntry* tab, const float* vol, float* pseg, float* p,
-                    double* partials) {
+void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const ColHdr* hdr, const SlabEntry* tab,
+                    const float* vol, float* pseg, float* p, int then, cudaGraphConditionalHandle h, int use_cond) {
     const int n_seg = project_segments(G);
-    q.launch(k_project, dim3((G.nu + PW - 1) / PW, (G.nv + 31) / 32, nslots * n_seg), dim3(NT), 0, G, slots, hdr, tab,
-             max_slabs(G), n_seg, vol, pseg);
-    q.launch(k_project_finish, dim3((G.nu + 31) / 32, (G.nv + 31) / 32, nslots), dim3(FT), 0, G, slots, solves, in, n_seg,
-             (const float*)pseg, p, partials);
+    q.launch(k_project, dim3((G.nu + PW - 1) / PW, (G.nv + 31) / 32, nslots * n_seg), dim3(NT), 0, G,
+             (const SlotState*)c.slots, hdr, tab, max_slabs(G), n_seg, vol, pseg);
+    launch_project_finish(q, G, c, nslots, n_seg, pseg, p, then, h, use_cond);
 }
 
 void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray) {

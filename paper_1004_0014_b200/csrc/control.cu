@@ -101,12 +101,30 @@ __device__ double coop_sum(const double* part, int n, int stride, double* red /*
 
 struct Sums3 { double a, b, c; };
 
-__device__ Sums3 sum_proj(const double* part, int nblk, int s, double* red) {
+// The three projection sums of slot s in one pass (one round trip to L2, one exchange).
+__device__ Sums3 sum_proj(const double* part, int nblk, int s, double* red /* unused */) {
+    __shared__ double ex[3][CT / 32];
+    __shared__ double tot[3];
+    (void)red;
     const double* p = part + (long long)s * nblk * 3;
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+    for (int i = threadIdx.x; i < nblk; i += CT) {
+        v0 += __ldcg(p + 3 * i); v1 += __ldcg(p + 3 * i + 1); v2 += __ldcg(p + 3 * i + 2);
+    }
+    v0 = warp_sum(v0); v1 = warp_sum(v1); v2 = warp_sum(v2);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();                       // ex / tot may still be read from a previous call
+    if (lane == 0) { ex[0][wid] = v0; ex[1][wid] = v1; ex[2][wid] = v2; }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double t = 0.0;
+#pragma unroll
+        for (int i = 0; i < CT / 32; ++i) t += ex[threadIdx.x][i];
+        tot[threadIdx.x] = t;
+    }
+    __syncthreads();
     Sums3 r;
-    r.a = coop_sum(p, nblk, 3, red);
-    r.b = coop_sum(p + 1, nblk, 3, red);
-    r.c = coop_sum(p + 2, nblk, 3, red);
+    r.a = tot[0]; r.b = tot[1]; r.c = tot[2];
     return r;
 }
 
@@ -148,19 +166,48 @@ __device__ void ctl_init_body(const Geom& G, const CtlBufs& c, cudaGraphConditio
 // After the residual and gradient kernels of iteration n: J_n, g, stopping rule, first candidate(s).
 __global__ void __launch_bounds__(CT)
 k_ctl_grad(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_trial, int use_cond) {
-    __shared__ double red[CT / 32 + 1];
+    __shared__ double ex[KMAX + 1][CT / 32];
+    __shared__ double tot[KMAX + 1];
     int any_trial = 0, any_running = 0;
-    const CallOpts& o = *c.opts;
+    const CallOpts o = *c.opts;
     const int K = G.K;
     for (int b = 0; b < o.B; ++b) {
-        SolveState& st = c.solves[b];
+        SolveState st = c.solves[b];                   // worked on in registers; thread 0 writes it back
         if (!st.running) continue;                                                        // uniform
         const int n = st.iter;
-        const double Jn = coop_sum(c.resid_part + (long long)b * c.resid_blocks, c.resid_blocks, 1, red);
-        double gk[KMAX];
-        for (int k = 0; k < K; ++k)
-            gk[k] = coop_sum(c.grad_part + (long long)b * c.grad_blocks * KMAX + k, c.grad_blocks, KMAX, red);
+        // J_n and the K gradient sums in one pass over the partial sums (fixed order)
+        {
+            double v[KMAX + 1];
+#pragma unroll
+            for (int k = 0; k <= KMAX; ++k) v[k] = 0.0;
+            const double* rp = c.resid_part + (long long)b * c.resid_blocks;
+            for (int i = threadIdx.x; i < c.resid_blocks; i += CT) v[KMAX] += __ldcg(rp + i);
+            const double* gp = c.grad_part + (long long)b * c.grad_blocks * KMAX;
+            for (int i = threadIdx.x; i < c.grad_blocks; i += CT) {
+#pragma unroll
+                for (int k = 0; k < KMAX; ++k)
+                    if (k < K) v[k] += __ldcg(gp + (long long)i * KMAX + k);
+            }
+            const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k <= KMAX; ++k) {
+                const double w = warp_sum(v[k]);
+                if (lane == 0) ex[k][wid] = w;
+            }
+            __syncthreads();
+            if (threadIdx.x <= KMAX) {
+                double t = 0.0;
+#pragma unroll
+                for (int i = 0; i < CT / 32; ++i) t += ex[threadIdx.x][i];
+                tot[threadIdx.x] = t;
+            }
+            __syncthreads();
+        }
         if (threadIdx.x != 0) continue;
+        const double Jn = tot[KMAX];
+        double gk[KMAX];
+        for (int k = 0; k < K; ++k) gk[k] = tot[k];
         st.Jn = Jn;                                                                       // Eq. (2)
         if (n == 0) st.J0 = st.Jn;
         double g2 = 0.0;
@@ -174,6 +221,7 @@ k_ctl_grad(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_trial, int use_
         if (gn <= o.grad_tol || !isfinite(gn)) {
             st.status = isfinite(gn) ? PCAMM_S_GRADTOL : PCAMM_E_NONFINITE;
             st.running = 0; st.trialing = 0;
+            c.solves[b] = st;
             continue;
         }
         st.mu = n == 0 ? o.init_step_vox * o.hmin_sqrtV / gn : 2.0 * st.mu_prev;         // reading A7
@@ -187,6 +235,7 @@ k_ctl_grad(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_trial, int use_
         }
         any_trial = 1;
         any_running = 1;
+        c.solves[b] = st;
     }
     if (threadIdx.x == 0) {
         publish(c.flags, any_running, any_trial, 3);
@@ -198,14 +247,17 @@ k_ctl_grad(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_trial, int use_
 __device__ void ctl_trial_body(const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond) {
     __shared__ double red[CT / 32 + 1];
     int any_trial = 0, any_running = 0;
-    const CallOpts& o = *c.opts;
+    const CallOpts o = *c.opts;
     const int K = G.K;
     for (int b = 0; b < o.B; ++b) {
-        SolveState& st = c.solves[b];
+        // the state is worked on in registers (one round trip to L2 each way, instead of one per
+        // field touched); thread 0 writes it back
+        SolveState st = c.solves[b];
         if (st.running && !st.trialing) any_running = 1;
         if (!st.trialing) continue;                                                       // uniform
         const int n = st.iter;
         int acc = -1;
+        double acc_mu = 0.0, acc_Sp = 0.0, acc_Syp = 0.0;
         bool failed = false;
         if (o.batched) {
             // candidates mu beta^c, c = 0..max_backtracks-1, all evaluated: the largest passing
@@ -214,8 +266,11 @@ __device__ void ctl_trial_body(const Geom& G, const CtlBufs& c, cudaGraphConditi
                 const int s = b * o.C + cnd;
                 const Sums3 sp = sum_proj(c.proj_part, c.proj_blocks, s, red);
                 if (threadIdx.x != 0) continue;
+                const double mu_s = c.slots[s].mu;
                 c.slots[s].Sp = sp.a; c.slots[s].Syp = sp.b; c.slots[s].J = sp.c;
-                if (acc < 0 && sp.c <= st.Jn - o.armijo_c * c.slots[s].mu * st.g2) { acc = s; st.t = cnd; }
+                if (acc < 0 && sp.c <= st.Jn - o.armijo_c * mu_s * st.g2) {
+                    acc = s; st.t = cnd; acc_mu = mu_s; acc_Sp = sp.a; acc_Syp = sp.b;
+                }
                 c.slots[s].active = 0;
             }
             if (threadIdx.x != 0) continue;
@@ -224,25 +279,28 @@ __device__ void ctl_trial_body(const Geom& G, const CtlBufs& c, cudaGraphConditi
             const int s = b * o.C;
             const Sums3 sp = sum_proj(c.proj_part, c.proj_blocks, s, red);
             if (threadIdx.x != 0) continue;
-            c.slots[s].Sp = sp.a; c.slots[s].Syp = sp.b; c.slots[s].J = sp.c;
-            if (sp.c <= st.Jn - o.armijo_c * st.mu * st.g2) acc = s;                      // Armijo (L95)
-            else {
+            SlotState sl = c.slots[s];
+            sl.Sp = sp.a; sl.Syp = sp.b; sl.J = sp.c;
+            if (sp.c <= st.Jn - o.armijo_c * st.mu * st.g2) {                             // Armijo (L95)
+                acc = s; acc_mu = sl.mu; acc_Sp = sp.a; acc_Syp = sp.b;
+            } else {
                 st.mu *= o.armijo_beta;
                 st.t += 1;
                 if (st.t >= o.max_backtracks) failed = true;
-                else trial_w(st, K, st.mu, &c.slots[s]);
+                else trial_w(st, K, st.mu, &sl);
             }
-            if (acc >= 0 || failed) c.slots[s].active = 0;
+            if (acc >= 0 || failed) sl.active = 0;
+            c.slots[s] = sl;
         }
         if (acc >= 0) {
-            const double mu = c.slots[acc].mu;
+            const double mu = acc_mu;
             for (int k = 0; k < K; ++k) st.w[k] -= mu * st.g[k];                          // Eq. (3)
             st.mu_prev = mu;
             st.acc_slot = acc;
             if (n < TRACE_CAP) { c.traces[b].mu[n] = mu; c.traces[b].bt[n] = st.t; }
             st.iter = n + 1;
             st.trialing = 0;
-            if (!lsfit((double)G.npix, st.Sy, st.Syy, c.slots[acc].Sp, c.slots[acc].Syp, &st.a, &st.b)) {  // Eq. (4)
+            if (!lsfit((double)G.npix, st.Sy, st.Syy, acc_Sp, acc_Syp, &st.a, &st.b)) {   // Eq. (4)
                 st.status = PCAMM_E_SINGULAR; st.running = 0;
             } else if (st.iter >= o.max_iter) { st.status = PCAMM_S_MAXITER; st.running = 0; }
         } else if (failed) {
@@ -252,6 +310,7 @@ __device__ void ctl_trial_body(const Geom& G, const CtlBufs& c, cudaGraphConditi
         }
         if (st.trialing) any_trial = 1;
         if (st.running) any_running = 1;
+        c.solves[b] = st;                                                                 // thread 0 only gets here
     }
     if (threadIdx.x == 0) {
         publish(c.flags, any_running, any_trial, 3);

@@ -220,9 +220,11 @@ int grad_grid(const Geom& G, const FieldStream& fs) {
 //      together);
 //   2. the voxels with G_j != 0 are compacted into a shared-memory queue, in a fixed order
 //      (ballot + prefix over the warps: no atomics, so the summation order is reproducible);
-//   3. the queue is dealt out evenly: each thread gathers B_j for its entries and accumulates
-//      B_j q_kj.  Only boundary voxels have G_j != 0 in piecewise-constant anatomy, so without the
-//      compaction most lanes of a warp would idle through their neighbours' detector gathers.
+//   3. the queue is dealt out in full rounds of one entry per thread: each thread gathers B_j for
+//      its entry and accumulates B_j q_kj; what does not fill a round waits for the next batch
+//      (single solve) or is flushed (several solves in flight: their views differ).  Only
+//      boundary voxels have G_j != 0 in piecewise-constant anatomy, so without the compaction
+//      most lanes of a warp would idle through their neighbours' detector gathers.
 // Per tile and solve the group's K sums are reduced in double and added to the group's slot of
 // the partial-sum buffer; the control kernel adds the slots in index order.
 
@@ -235,12 +237,14 @@ template <int K> struct GradBatch { static constexpr int value = K <= 3 ? 4 : 2;
 
 template <int K>
 struct QueueEntry {
-    int vox;          // zz << 5 | xx inside the tile
+    int xy, z;        // x | y << 16; z
     float q[K];
 };
 
+// Entries of a group's queue: one batch of new ones plus what the last round left over.
+template <int K> struct GradQueueCap { static constexpr int value = GROUP_THREADS * (GradBatch<K>::value + 1); };
 template <int K>
-constexpr size_t grad_queue_bytes() { return (size_t)GNG * GROUP_THREADS * GradBatch<K>::value * sizeof(QueueEntry<K>); }
+constexpr size_t grad_queue_bytes() { return (size_t)GNG * GradQueueCap<K>::value * sizeof(QueueEntry<K>); }
 template <int K> struct GradStages {
     static constexpr int value = ring_stages<K>(3, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
 };
@@ -261,7 +265,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     static_assert(GROWS % RB == 0 && NB >= 1, "tile rows per thread must be a multiple of the batch");
     using Ring = FieldRing<P, GTZ, NS>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    __shared__ int s_cnt[GNG][32];
+    __shared__ int s_cnt[GNG][2][32];                      // double buffered over the batches
     __shared__ float s_red[GNG][GROUP_WARPS][K];
     __shared__ GatherView s_gv[SOLVE_CACHE];               // per solve, constant during the launch
     __shared__ float s_w[SOLVE_CACHE][K];
@@ -287,7 +291,9 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
         return;
     }
     const int group = warp / GROUP_WARPS, tw = warp % GROUP_WARPS, gtid = threadIdx.x - group * GROUP_THREADS;
-    QueueEntry<K>* queue = queues + (size_t)group * GROUP_THREADS * RB;
+    constexpr int QCAP = GradQueueCap<K>::value;
+    QueueEntry<K>* queue = queues + (size_t)group * QCAP;   // ring buffer: q_head .. q_head + q_n - 1 (mod QCAP)
+    int q_head = 0, q_n = 0, parity = 0;                    // identical in every thread of the group
     const int nslot = gridDim.x * GNG, slot = blockIdx.x * GNG + group;   // this group's partial-sum slot
     if (gtid < K)
         for (int b = 0; b < B; ++b) partials[((long long)b * nslot + slot) * KMAX + gtid] = 0.0;
@@ -351,41 +357,55 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                                        gz * lds_f32(sf + 4u * (((3 + 3 * k + 2) * GTZ + zz) * TX + lane));
                         const bool active = x < G.nx && c.z0 + zz < G.nz && (gx != 0.f || gy != 0.f || gz != 0.f);
                         masks[rr] = __ballot_sync(0xffffffffu, active);
-                        if (lane == 0) s_cnt[group][rr * GROUP_WARPS + tw] = __popc(masks[rr]);
+                        if (lane == 0) s_cnt[group][parity][rr * GROUP_WARPS + tw] = __popc(masks[rr]);
                     }
                     group_barrier(group);
                     if (SINGLE && bt == NB - 1 && gtid == 0) mbar_arrive(ring.empty + s);   // no more reads of the stage
-                    // 2. compaction in the fixed order (row, warp, lane)
-                    int cnt = lane < RB * GROUP_WARPS ? s_cnt[group][lane] : 0, incl = cnt;
+                    // 2. compaction in the fixed order (row, warp, lane), appended to the queue
+                    int cnt = lane < RB * GROUP_WARPS ? s_cnt[group][parity][lane] : 0, incl = cnt;
+                    parity ^= 1;
 #pragma unroll
                     for (int o = 1; o < 32; o <<= 1) {
                         const int v = __shfl_up_sync(0xffffffffu, incl, o);
                         if (lane >= o) incl += v;
                     }
-                    const int n_q = __shfl_sync(0xffffffffu, incl, 31);
+                    const int n_new = __shfl_sync(0xffffffffu, incl, 31);
 #pragma unroll
                     for (int rr = 0; rr < RB; ++rr) {
                         const int base = __shfl_sync(0xffffffffu, incl - cnt, rr * GROUP_WARPS + tw);
                         if (masks[rr] >> lane & 1u) {
-                            QueueEntry<K>& e = queue[base + __popc(masks[rr] & ((1u << lane) - 1u))];
-                            e.vox = (tw + GROUP_WARPS * (bt * RB + rr)) << 5 | lane;
+                            int pos = q_head + q_n + base + __popc(masks[rr] & ((1u << lane) - 1u));
+                            if (pos >= QCAP) pos -= QCAP;
+                            if (pos >= QCAP) pos -= QCAP;
+                            QueueEntry<K>& e = queue[pos];
+                            e.xy = x | c.y << 16;
+                            e.z = c.z0 + tw + GROUP_WARPS * (bt * RB + rr);
 #pragma unroll
                             for (int k = 0; k < K; ++k) e.q[k] = q[rr][k];
                         }
                     }
+                    q_n += n_new;
                     group_barrier(group);
-                    // 3. the detector gathers, dealt out evenly
-                    for (int e = gtid; e < n_q; e += GROUP_THREADS) {
-                        const QueueEntry<K> en = queue[e];
-                        const int xx = en.vox & 31, zz = en.vox >> 5;
-                        const float xw = G.cx + ((float)(c.x0 + xx) - 0.5f * (G.nx - 1)) * G.hx;
-                        const float yw = G.cy + ((float)c.y - 0.5f * (G.ny - 1)) * G.hy;
-                        const float zw = G.cz + ((float)(c.z0 + zz) - 0.5f * (G.nz - 1)) * G.hz;
+                    // 3. the detector gathers, one entry per thread and round
+                    const int n_proc = SINGLE ? q_n / GROUP_THREADS * GROUP_THREADS : q_n;
+                    for (int e = gtid; e < n_proc; e += GROUP_THREADS) {
+                        int pos = q_head + e;
+                        if (pos >= QCAP) pos -= QCAP;
+                        if (pos >= QCAP) pos -= QCAP;
+                        const QueueEntry<K> en = queue[pos];
+                        const float xw = G.cx + ((float)(en.xy & 0xffff) - 0.5f * (G.nx - 1)) * G.hx;
+                        const float yw = G.cy + ((float)(en.xy >> 16) - 0.5f * (G.ny - 1)) * G.hy;
+                        const float zw = G.cz + ((float)en.z - 0.5f * (G.nz - 1)) * G.hz;
                         const float Bj = gather_voxel(G, gv, rLb, ub, vb, xw, yw, zw);
 #pragma unroll
                         for (int k = 0; k < K; ++k) acc[k] = fmaf(Bj, en.q[k], acc[k]);
                     }
-                    group_barrier(group);                   // the queue and s_cnt are free again
+                    q_head += n_proc;
+                    if (q_head >= QCAP) q_head -= QCAP;
+                    if (q_head >= QCAP) q_head -= QCAP;
+                    q_n -= n_proc;
+                    // no barrier here: the next batch writes its entries only after its own first
+                    // barrier, which no thread passes before every thread has left this loop
                 }
                 if (!SINGLE) {                              // the group's K sums of this tile and solve
 #pragma unroll
@@ -413,6 +433,21 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
         if (++s == NS) { s = 0; ph ^= 1u; }
     }
     if (SINGLE) {                                           // the group's K sums over all its tiles
+        if (s_running[0]) {                                 // what is left in the queue
+            group_barrier(group);
+            const GatherView gv = s_gv[0];
+            if (gtid < q_n) {
+                int pos = q_head + gtid;
+                if (pos >= QCAP) pos -= QCAP;
+                const QueueEntry<K> en = queue[pos];
+                const float xw = G.cx + ((float)(en.xy & 0xffff) - 0.5f * (G.nx - 1)) * G.hx;
+                const float yw = G.cy + ((float)(en.xy >> 16) - 0.5f * (G.ny - 1)) * G.hy;
+                const float zw = G.cz + ((float)en.z - 0.5f * (G.nz - 1)) * G.hz;
+                const float Bj = gather_voxel(G, gv, rL, utab, vtab, xw, yw, zw);
+#pragma unroll
+                for (int k = 0; k < K; ++k) acc[k] = fmaf(Bj, en.q[k], acc[k]);
+            }
+        }
         double sum[K];
 #pragma unroll
         for (int k = 0; k < K; ++k) sum[k] = warp_sum((double)acc[k]);

@@ -208,7 +208,7 @@ k_grad_generic(const Geom G, const float* __restrict__ f0, const float* __restri
 }
 
 int grad_grid(const Geom& G, const FieldStream& fs) {
-    const long long nt = tile_count(G, G.K <= 5 ? 32 : 16);      // TileZ<K>
+    const long long nt = tile_count(G, G.K <= 4 ? 32 : 16);      // TileZ<K>
     return (int)(nt < fs.n_sm ? nt : fs.n_sm);
 }
 
@@ -246,11 +246,11 @@ template <int K> struct GradQueueCap { static constexpr int value = GROUP_THREAD
 template <int K>
 constexpr size_t grad_queue_bytes() { return (size_t)GNG * GradQueueCap<K>::value * sizeof(QueueEntry<K>); }
 template <int K> struct GradStages {
-    static constexpr int value = ring_stages<K>(3, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
+    static constexpr int value = stages_per_group<K>(GNG, 2, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
 };
 template <int K>
 constexpr size_t grad_smem_bytes() {
-    return FieldRing<3 * (K + 1), TileZ<K>::value, GradStages<K>::value>::BYTES + 16 + grad_queue_bytes<K>();
+    return FieldRing<3 * (K + 1), TileZ<K>::value, GNG, GradStages<K>::value>::BYTES + 16 + grad_queue_bytes<K>();
 }
 
 // SINGLE: one solve (B = 1): the K sums stay in registers over all tiles of the CTA and are
@@ -260,10 +260,10 @@ __global__ void __launch_bounds__(GTHREADS, 1)
 k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
            const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
            const float2* __restrict__ vtab, double* __restrict__ partials) {
-    constexpr int P = 3 * (K + 1), NS = GradStages<K>::value, GTZ = TileZ<K>::value, GROWS = GTZ / GROUP_WARPS;
+    constexpr int P = 3 * (K + 1), GTZ = TileZ<K>::value, GROWS = GTZ / GROUP_WARPS;
     constexpr int RB = GradBatch<K>::value, NB = GROWS / RB;
     static_assert(GROWS % RB == 0 && NB >= 1, "tile rows per thread must be a multiple of the batch");
-    using Ring = FieldRing<P, GTZ, NS>;
+    using Ring = FieldRing<P, GTZ, GNG, GradStages<K>::value>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ int s_cnt[GNG][2][32];                      // double buffered over the batches
     __shared__ float s_red[GNG][GROUP_WARPS][K];
@@ -301,11 +301,11 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     float acc[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) acc[k] = 0.f;
-    int s = 0, turn = 0;
-    uint32_t ph = 0;
-    for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-        if (turn == group) {
-            mbar_wait(ring.full + s, ph);
+    int j = 0;                                             // this group's tile counter
+    for (long long t = blockIdx.x + (long long)group * gridDim.x; t < n_tiles; t += (long long)GNG * gridDim.x, ++j) {
+        {
+            const int s = Ring::stage_of(group, j);
+            mbar_wait(ring.full + s, Ring::parity_of(j));
             const uint32_t sf = smem_u32(ring.stage(s));   // [P][GTZ][TX]
             const TileCoord c = tile_coord(G, GTZ, t);
             const int x = c.x0 + lane;
@@ -429,8 +429,6 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                 if (gtid == 0) mbar_arrive(ring.empty + s);
             } else if (!s_running[0] && gtid == 0) mbar_arrive(ring.empty + s);
         }
-        if (++turn == GNG) turn = 0;
-        if (++s == NS) { s = 0; ph ^= 1u; }
     }
     if (SINGLE) {                                           // the group's K sums over all its tiles
         if (s_running[0]) {                                 // what is left in the queue

@@ -101,16 +101,23 @@ __device__ __forceinline__ void group_barrier(int group) {
     asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(GROUP_THREADS) : "memory");
 }
 
-// Shared-memory ring of a streaming kernel: NS stages of P planes x TZ x TX floats.
-template <int P, int TZ, int NS>
+// Shared-memory stages of a streaming kernel: NG consumer groups with SPG stages each, a stage
+// being P planes x TZ x TX floats.  The CTA's i-th tile (tile blockIdx.x + i * gridDim.x of the
+// volume) belongs to group i % NG and is that group's (i / NG)-th tile; it goes through stage
+// (i / NG) % SPG of the group's own little ring.  Every stage is therefore filled and drained
+// by one producer and ONE group, strictly in order, which is what makes waiting on a phase
+// parity sound (a group sharing stages with others could be a whole ring cycle ahead of the
+// barrier it polls and mistake the previous phase for its own).
+template <int P, int TZ, int NG, int SPG>
 struct FieldRing {
+    static constexpr int NS = NG * SPG;
     static constexpr int STAGE_FLOATS = P * TZ * TX;
     static constexpr uint32_t STAGE_BYTES = STAGE_FLOATS * 4u;
     static constexpr size_t BYTES = (size_t)NS * STAGE_BYTES + 2 * NS * sizeof(uint64_t);
 
     float* data;        // 128 B aligned
     uint64_t* full;     // [NS] TMA completion
-    uint64_t* empty;    // [NS] consumers done with the stage
+    uint64_t* empty;    // [NS] the group is done with the stage
 
     __device__ __forceinline__ void bind(unsigned char* smem) {
         data = reinterpret_cast<float*>(smem);
@@ -123,19 +130,22 @@ struct FieldRing {
     }
     __device__ __forceinline__ const float* stage(int s) const { return data + (size_t)s * STAGE_FLOATS; }
 
-    // Producer side: tiles i = 0 .. n-1 of this CTA are tiles blockIdx.x + i * gridDim.x.
+    // Producer (one thread).
     __device__ __forceinline__ void produce(const CUtensorMap* map, const Geom& G, long long n_tiles) {
         const uint64_t policy = l2_evict_first_policy();
-        int s = 0;
-        uint32_t ph = 0;
+        int g = 0, j = 0;                                        // group of the tile, the group's tile counter
         for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-            mbar_wait(empty + s, ph ^ 1u);                       // the stage is free (passes at once on a fresh ring)
+            const int s = g * SPG + j % SPG;
+            mbar_wait(empty + s, ((uint32_t)(j / SPG) & 1u) ^ 1u);   // the stage is free (passes at once the first time)
             const TileCoord c = tile_coord(G, TZ, t);
             mbar_arrive_expect_tx(full + s, STAGE_BYTES);
             tma_load_4d(data + (size_t)s * STAGE_FLOATS, map, full + s, c.x0, c.y, c.z0, 0, policy);
-            if (++s == NS) { s = 0; ph ^= 1u; }
+            if (++g == NG) { g = 0; ++j; }
         }
     }
+    // Consumer group g: stage and phase parity of its j-th tile.
+    __device__ __forceinline__ static int stage_of(int g, int j) { return g * SPG + j % SPG; }
+    __device__ __forceinline__ static uint32_t parity_of(int j) { return (uint32_t)(j / SPG) & 1u; }
 };
 
 // What the streaming kernels need to know about the model's fields.
@@ -148,12 +158,13 @@ struct FieldStream {
 
 // Tile extent along z and ring depth by K: a stage is 3(K+1) planes x TZ x TX floats and the
 // ring has to fit in 227 KB of shared memory next to the kernel's own buffers.
-template <int K> struct TileZ { static constexpr int value = K <= 5 ? 32 : 16; };
+template <int K> struct TileZ { static constexpr int value = K <= 4 ? 32 : 16; };
+// stages per consumer group that fit into budget_bytes, at most max_spg
 template <int K>
-constexpr int ring_stages(int max_stages, int budget_bytes) {
+constexpr int stages_per_group(int n_groups, int max_spg, int budget_bytes) {
     const int stage = 3 * (K + 1) * TileZ<K>::value * TX * 4;
-    const int n = budget_bytes / stage;
-    return n < max_stages ? (n < 1 ? 1 : n) : max_stages;
+    const int n = budget_bytes / stage / n_groups;
+    return n < max_spg ? (n < 1 ? 1 : n) : max_spg;
 }
 template <int K>
 __host__ __device__ __forceinline__ const CUtensorMap& field_map(const FieldStream& fs) {

@@ -117,19 +117,19 @@ constexpr int SLOT_CACHE = 64;     // slots whose coefficients are kept in share
 constexpr int WTHREADS = 32 * (WNG * GROUP_WARPS + 1);
 
 constexpr int WSTATIC = 16 * 1024; // static shared memory of the kernel (transposition tiles, slot cache), rounded up
-template <int K> struct WarpStages { static constexpr int value = ring_stages<K>(4, 227 * 1024 - WSTATIC - 64); };
+template <int K> struct WarpStages { static constexpr int value = stages_per_group<K>(WNG, 2, 227 * 1024 - WSTATIC - 64); };
 
 template <int K>
 constexpr size_t warp_smem_bytes() {
-    return FieldRing<3 * (K + 1), TileZ<K>::value, WarpStages<K>::value>::BYTES;
+    return FieldRing<3 * (K + 1), TileZ<K>::value, WNG, WarpStages<K>::value>::BYTES;
 }
 
 template <int K, bool RAY>
 __global__ void __launch_bounds__(WTHREADS, 1)
 k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
            const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride) {
-    constexpr int P = 3 * (K + 1), NS = WarpStages<K>::value, WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
-    using Ring = FieldRing<P, WTZ, NS>;
+    constexpr int P = 3 * (K + 1), WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
+    using Ring = FieldRing<P, WTZ, WNG, WarpStages<K>::value>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ float tiles[WNG][WTZ][TX + 1];
     __shared__ float s_w[SLOT_CACHE][K];                   // the slots' coefficients (constant during the launch)
@@ -148,17 +148,20 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     __syncthreads();
     const long long n_tiles = tile_count(G, WTZ);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int last_active = -1;                                  // the last slot that reads the stage
+    for (int i = 0; i < nslots; ++i)
+        if (s_active[i]) last_active = i;
     if (warp == WNG * GROUP_WARPS) {                       // producer
         if (lane == 0) ring.produce(&fmap, G, n_tiles);
         return;
     }
     const int group = warp / GROUP_WARPS, tw = warp % GROUP_WARPS;
     float(*tile)[TX + 1] = tiles[group];
-    int s = 0, turn = 0;
-    uint32_t ph = 0;
-    for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-        if (turn == group) {
-            mbar_wait(ring.full + s, ph);
+    int j = 0;                                             // this group's tile counter
+    for (long long t = blockIdx.x + (long long)group * gridDim.x; t < n_tiles; t += (long long)WNG * gridDim.x, ++j) {
+        {
+            const int s = Ring::stage_of(group, j);
+            mbar_wait(ring.full + s, Ring::parity_of(j));
             const uint32_t sf = smem_u32(ring.stage(s));   // [P][WTZ][TX]
             const TileCoord c = tile_coord(G, WTZ, t);
             const int x = c.x0 + lane;
@@ -185,6 +188,10 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     }
                     taps[r] = make_taps(G.nx, G.ny, G.nz, x, c.y, z, d[0], d[1], d[2]);
                 }
+                if (sl == last_active) {                    // the fields of this tile are in registers: hand the
+                    group_barrier(group);                   // stage back while the gathers are under way
+                    if (tw == 0 && lane == 0) mbar_arrive(ring.empty + s);
+                }
                 float cv[WROWS][8];
 #pragma unroll
                 for (int r = 0; r < WROWS; ++r) gather8(f0, taps[r], cv[r]);    // 8 WROWS gathers in flight
@@ -210,11 +217,8 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     }
                 }
             }
-            group_barrier(group);                           // every thread of the group is done with the stage
-            if (tw == 0 && lane == 0) mbar_arrive(ring.empty + s);
+            if (last_active < 0 && tw == 0 && lane == 0) mbar_arrive(ring.empty + s);   // nothing to do: pass the stage on
         }
-        if (++turn == WNG) turn = 0;
-        if (++s == NS) { s = 0; ph ^= 1u; }
     }
 }
 

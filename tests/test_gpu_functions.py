@@ -68,6 +68,27 @@ def test_warp_matches_oracle(K, seed):
         assert np.max(np.abs(out - ref)) <= 2e-6 * np.max(np.abs(ref))
 
 
+@pytest.mark.parametrize("K,seed", [(3, 21), (5, 22), (7, 23)])
+def test_streaming_kernels_over_many_tiles_per_cta(K, seed):
+    """A volume of 2048 field tiles: every persistent CTA of the TMA-fed warp and gradient kernels
+    goes round its shared-memory stages several times (a 148-SM GPU gives each CTA ~14 tiles), so
+    a stage handed to the wrong consumer group or polled a phase too early shows up here."""
+    g = geom(nx=64, ny=256, nz=128 if K <= 4 else 64, h=(2.0, 2.0, 2.0), K=K, nu=48, nv=40, pitch=(6.0, 6.0))
+    f0, xbar, u, scale, m = _model(g, seed=seed, disp_vox=2.0)
+    rng = np.random.default_rng(seed)
+    w = (rng.uniform(0.4, 1.0, K) * rng.choice([-1, 1], K) * scale).astype(np.float32)
+    ref = oracle.warp(g, f0, xbar, u, w)
+    out = to_host(m.warp(w))
+    assert rel_l2(out, ref) <= 5e-6
+    theta = 0.7
+    _, p_ref = oracle.evaluate(g, f0, xbar, u, w, theta)
+    y = (1.1 * p_ref + 0.02 * np.abs(p_ref).max() * rng.standard_normal(p_ref.shape)).astype(np.float32)
+    J, grad, ab, p = m.eval(to_dev(y), theta, w, 1.0, 0.0)
+    g_ref = oracle.gradient(g, f0, xbar, u, w, 1.0, 0.0, p_ref, y, theta)
+    assert rel_l2(to_host(p), p_ref) <= 1e-5
+    assert np.linalg.norm(grad - g_ref) <= 1e-3 * np.linalg.norm(g_ref), (grad, g_ref)
+
+
 def test_warp_outside_the_grid_is_zero_padded():
     """Reading A2: a displacement larger than the volume samples zeros; one cell inside tapers."""
     g = _geom(K=1, n=(20, 18, 10))

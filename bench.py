@@ -82,6 +82,48 @@ def algorithmic_bytes(cfg):
             "gradient": (12 * (K + 1) + 4) * V + 4 * npix}
 
 
+def measured_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel, from the committed
+    `ncu --set full` capture of this round (profiles/r01_traffic.json; null if absent)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+# The projector is bound by instruction issue, not by HBM (its volume is L2-resident, DESIGN.md):
+# it is reported against the fp32 lane-operation rate of the SMs.  Algorithmic operations per
+# (ray, slab) of the exact slab march (DESIGN.md "Kernels", a-2): 15.
+PROJECT_OPS_PER_RAY_SLAB = 15
+ALU_PEAK_TOPS = 148 * 128 * 1.965e9 / 1e12      # 148 SMs x 128 fp32 lanes x 1.965 GHz (B200_PROFILING.md)
+
+
+def ray_slab_count(cfg, angle_rad: float) -> int:
+    """(ray, slab) pairs the projector marches at this gantry angle: per detector column the voxel
+    layers along its dominant in-plane axis in which the ray overlaps the volume (the in-plane
+    clipping of DESIGN.md a-2), times the detector rows."""
+    cs, sn = np.cos(angle_rad), np.sin(angle_rad)
+    uu = (np.arange(cfg.nu) - 0.5 * (cfg.nu - 1)) * cfg.pu
+    dx, dy = -cfg.sdd * cs - uu * sn, -cfg.sdd * sn + uu * cs
+    gx, gy = dx / cfg.hx, dy / cfg.hy
+    sx = (cfg.sad * cs + 0.5 * cfg.nx * cfg.hx) / cfg.hx
+    sy = (cfg.sad * sn + 0.5 * cfg.ny * cfg.hy) / cfg.hy
+    along_x = np.abs(gx) >= np.abs(gy)
+    gm, gt = np.where(along_x, gx, gy), np.where(along_x, gy, gx)
+    sm, st = np.where(along_x, sx, sy), np.where(along_x, sy, sx)
+    nm, nt = np.where(along_x, cfg.nx, cfg.ny), np.where(along_x, cfg.ny, cfg.nx)
+    slope = gt / gm
+    t0 = st - sm * slope
+    with np.errstate(divide="ignore", invalid="ignore"):
+        m0, m1 = (0.0 - t0) / slope, (nt - t0) / slope
+    lo = np.where(slope != 0, np.minimum(m0, m1), 0.0)
+    hi = np.where(slope != 0, np.maximum(m0, m1), nm.astype(float))
+    lo, hi = np.clip(lo, 0, nm), np.clip(hi, 0, nm)
+    n = np.maximum(np.ceil(hi) - np.floor(lo), 0)
+    return int(n.sum()) * cfg.nv
+
+
 def measured_peak_gbs():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -209,7 +251,14 @@ def run_ours(args, cfg, rank, local_rank, world):
     # ---- inputs on the CPU first (the worker pool forks before CUDA is initialised)
     t0 = time.perf_counter()
     wl = build_workload(cfg)
-    ids = replicas.frame_block(rank, world, n, FIRST_FRAME, len(wl.frames))
+    B = max(int(args.in_flight), 1)
+    if B == 1:
+        ids = replicas.frame_block(rank, world, n, FIRST_FRAME, len(wl.frames))
+    else:
+        # B solves in flight: gantry angles and breathing states drawn from the test trajectory
+        # (seeded, BASELINE.json configs[4]); a pool of 8 distinct frames, re-noised per use
+        pool = np.random.default_rng(4 + rank).choice(len(wl.frames), size=min(8, len(wl.frames)), replace=False)
+        ids = [int(pool[i % len(pool)]) for i in range(min(n, 2) * B)]
     gts = ground_truth_volumes(wl, ids)
     log(f"[rank {rank}] inputs built in {time.perf_counter() - t0:.1f} s")
 
@@ -222,20 +271,38 @@ def run_ours(args, cfg, rank, local_rank, world):
     C = 8 if cfg.batched_linesearch else 1
     m = pc.Model(nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, hx=cfg.hx, hy=cfg.hy, hz=cfg.hz, K=cfg.K, nu=cfg.nu, nv=cfg.nv,
                  pu=cfg.pu, pv=cfg.pv, f0=t(wl.f0), mean_dvf=t(wl.model.mean), eig_dvf=t(wl.model.eig),
-                 landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=C)
+                 landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=C, max_batch=B)
     # measured projections: the scanner is simulated with the library's own projector applied to
     # the ground-truth volume, plus seeded noise (the CPU arm simulates its own with the oracle)
     ys_host, ys_dev = [], []
-    for fid in ids:
+    p_true = {}
+    for j, fid in enumerate(ids):
         fr = wl.frames[fid]
-        p_true = m.project(t(gts[fid]), fr.angle_rad).cpu().numpy()
-        y = add_noise(p_true, cfg.noise, seed=fid)
+        if fid not in p_true:
+            p_true[fid] = m.project(t(gts[fid]), fr.angle_rad).cpu().numpy()
+        y = add_noise(p_true[fid], cfg.noise, seed=fid + 1000 * (j // max(len(p_true), 1)) if B > 1 else fid)
         ys_host.append(torch.from_numpy(y).pin_memory())
         ys_dev.append(t(y))
     angles = [float(wl.frames[fid].angle_rad) for fid in ids]
     opts = pc.Opts(max_iter=it, batched_linesearch=int(cfg.batched_linesearch), loop_mode=args.loop_mode)
+    if B > 1:   # one stacked [B][nv][nu] tensor per distinct step
+        n_distinct = len(ids) // B
+        yb_dev = [torch.stack(ys_dev[j * B:(j + 1) * B]) for j in range(n_distinct)]
+        yb_host = [torch.stack([h for h in ys_host[j * B:(j + 1) * B]]).pin_memory() for j in range(n_distinct)]
+        ab = [np.array(angles[j * B:(j + 1) * B], np.float32) for j in range(n_distinct)]
+        stage = torch.empty_like(yb_dev[0])
+        w_zero = np.zeros((B, cfg.K), np.float32)
 
     def run_block(first, count, w, host):
+        if B > 1:
+            for i in range(first, first + count):
+                j = i % n_distinct
+                if host:
+                    stage.copy_(yb_host[j], non_blocking=True)
+                    r = m.reconstruct_batch(stage, ab[j], w_zero, opts)[-1]
+                else:
+                    r = m.reconstruct_batch(yb_dev[j], ab[j], w_zero, opts)[-1]
+            return w, r
         for i in range(first, first + count):
             if host:
                 r = m.reconstruct(ys_host[i].numpy(), angles[i], w, opts, host_y=True)
@@ -271,17 +338,18 @@ def run_ours(args, cfg, rank, local_rank, world):
     run_block(args.warmup, args.steps, w_after_warmup, host=True)
     torch.cuda.synchronize()
     e2e_ms = replicas.max_over_ranks(dist, 1e3 * (time.perf_counter() - t0), dev)
-    h2d = cfg.npix * 4 + 128 + 56          # y + the call's option block (CallOpts, SolveIn)
-    d2h = 272 + 16 + 24 * len(wl.landmarks)  # SolveState + LoopFlags + landmark positions (double)
+    h2d = B * (cfg.npix * 4 + 56) + 128           # y + the call's option block (CallOpts, SolveIn)
+    d2h = B * (272 + 24 * len(wl.landmarks)) + 24  # SolveState + landmark positions (double) + LoopFlags
 
     if rank != 0:
         return
-    ms_per_solve = elapsed_ms / (args.steps * world)
+    ms_per_solve = elapsed_ms / (args.steps * world * B)
 
     # ---- per-kernel device times on the last frame's state (CUDA events inside the library, on the
     #      stream the kernels are launched on), and the launch mix of one traced solve
-    i_last = n - 1
-    tr = m.reconstruct(ys_dev[i_last], angles[i_last], w_after_warmup, opts, trace=True)
+    i_last = (n - 1) if B == 1 else 0
+    tr = m.reconstruct(ys_dev[i_last], angles[i_last], w_after_warmup if B == 1 else np.zeros(cfg.K, np.float32),
+                       opts, trace=True)
     trials = int(np.sum(tr.backtracks + 1)) if tr.backtracks is not None else it
     m.eval(ys_dev[i_last], angles[i_last], tr.w, tr.a, tr.b, want_proj=False)
     for which in (0, 1, 2):
@@ -290,17 +358,30 @@ def run_ours(args, cfg, rank, local_rank, world):
     nl = {"warp": trials + 1, "project": trials + 1, "gradient": tr.iters}
     ab = algorithmic_bytes(cfg)
     peak, peak_src = measured_peak_gbs()
-    per_kernel = {k: {"ms": kt[k], "launches_per_solve": nl[k], "algorithmic_bytes": ab[k],
-                      "gbs": ab[k] / (kt[k] * 1e-3) / 1e9, "frac": ab[k] / (kt[k] * 1e-3) / 1e9 / peak}
+    traffic = measured_traffic().get(cfg.name, {})
+    per_kernel = {k: {"bound": "hbm", "ms": kt[k], "launches_per_solve": nl[k], "algorithmic_bytes": ab[k],
+                      "achieved": ab[k] / (kt[k] * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                      "frac": ab[k] / (kt[k] * 1e-3) / 1e9 / peak, "traffic": traffic.get(k)}
                   for k in kt}
+    # the projector against the SMs' fp32 lane-operation rate as well (it is not an HBM kernel)
+    n_rs = ray_slab_count(cfg, angles[i_last])
+    ops = PROJECT_OPS_PER_RAY_SLAB * n_rs
+    per_kernel["project"].update({"hbm_gbs": per_kernel["project"]["achieved"], "hbm_frac": per_kernel["project"]["frac"],
+                                  "bound": "alu", "ray_slabs": n_rs, "algorithmic_ops": ops,
+                                  "achieved": ops / (kt["project"] * 1e-3) / 1e12, "peak": ALU_PEAK_TOPS,
+                                  "unit": "Tlane-op/s", "frac": ops / (kt["project"] * 1e-3) / 1e12 / ALU_PEAK_TOPS,
+                                  "ray_slabs_per_s": n_rs / (kt["project"] * 1e-3)})
     dom = max(kt, key=lambda k: kt[k] * nl[k])
     wp_gbs = (ab["warp"] + ab["project"]) / ((kt["warp"] + kt["project"]) * 1e-3) / 1e9
-    roofline = {"kernel": dom, "bound": "hbm", "achieved": per_kernel[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": per_kernel[dom]["frac"], "traffic": None, "peak_source": peak_src,
+    d = per_kernel[dom]
+    roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],
+                "frac": d["frac"], "traffic": d["traffic"],
+                "peak_source": peak_src if d["bound"] == "hbm" else
+                "148 SMs x 128 fp32 lanes x 1.965 GHz (B200_PROFILING.md unit counts and clocks; DESIGN.md section 6)",
                 "per_kernel": per_kernel,
                 "warp_plus_project": {"gbs": wp_gbs, "frac": wp_gbs / peak,
                                       "frac_of_nominal_8000": wp_gbs / 8000.0},
-                "kernel_share_of_step": {k: kt[k] * nl[k] / (elapsed_ms / args.steps) for k in kt}}
+                "kernel_share_of_step": {k: kt[k] * nl[k] / (elapsed_ms / args.steps / B) for k in kt}}
 
     # ---- the oracle on this box's host cores, one full solve of the same workload
     cpu = None
@@ -314,9 +395,9 @@ def run_ours(args, cfg, rank, local_rank, world):
     line = {"metric": METRIC, "value": ms_per_solve, "unit": "ms", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": config_dict(cfg, it), "projections_per_s": 1e3 * args.steps * world / elapsed_ms,
+            "config": dict(config_dict(cfg, it), in_flight=B), "projections_per_s": 1e3 * args.steps * world * B / elapsed_ms,
             "clocks": clocks,
-            "e2e": {"value": e2e_ms / (args.steps * world), "unit": "ms", "h2d_bytes_per_step": h2d,
+            "e2e": {"value": e2e_ms / (args.steps * world * B), "unit": "ms", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
             "last_solve": {"iters": tr.iters, "trials": trials, "status": tr.status, "J0": tr.J0, "J": tr.J},
@@ -332,6 +413,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--in-flight", type=int, default=1,
+                    help="B > 1: every step advances B independent projection solves in lock step "
+                         "(pcamm_reconstruct_batch; BASELINE.json configs[4] sweeps 1, 4, 16, 64), each from w = 0")
     ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1],
                     help="0: the solve is one CUDA graph with device-side while-loops (default, the timed "
                          "configuration); 1: same kernels launched from the host (for per-launch ncu lists)")

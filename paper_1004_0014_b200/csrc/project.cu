@@ -122,7 +122,7 @@ k_view_tables(const Geom G, const SolveState* __restrict__ solves, ColHdr* __res
         const int jx = c.axis == 0 ? i : j, jy = c.axis == 0 ? j : i;
         SlabEntry e;
         e.off0 = ((jy + 1) * G.pnx + (jx + 1)) * G.nz;
-        e.tt = (float)tt;
+        e.tt = (float)(tt * 4294967296.0);       // in units of 2^-32 of the slab (see march)
         row[n] = e;
     }
     // null entries up to the end of the (padded) row: a zero-valued border column whose
@@ -130,7 +130,7 @@ k_view_tables(const Geom G, const SolveState* __restrict__ solves, ColHdr* __res
     for (int n = c.n_slabs + threadIdx.x; n < max_slabs; n += blockDim.x) {
         SlabEntry e;
         e.off0 = G.pnx * G.nz;            // (x, y) = (-1, 0)
-        e.tt = 1.f;
+        e.tt = 4294967296.f;
         row[n] = e;
     }
 }
@@ -173,7 +173,7 @@ __device__ __forceinline__ RayZ make_ray_z(const Geom& G, const ColHdr& h, int i
     const double Szi = (0.0 - G.loz) / (double)G.hz;                      // the source is in the plane z = 0
     const double sz = gz * h.kap;                                         // z per slab
     first_crossing(fma(gz, fma(h.kap, (double)n0, h.lam0), Szi), sz, &r.k, &r.dirZ, &r.QZ, &r.dQZ);
-    r.Ls = (float)(sqrt((double)h.dxy2 + dz * dz) * h.kap);
+    r.Ls = (float)(sqrt((double)h.dxy2 + dz * dz) * h.kap);            // mm per slab
     const int ncross = (int)(fabs(sz) * (double)n) + 2;                   // conservative
     r.kmin = r.dirZ < 0 ? r.k - ncross : r.k;
     r.kmax = r.dirZ > 0 ? r.k + ncross : r.k;
@@ -191,38 +191,47 @@ constexpr int U = 4;
 
 template <class Sink>
 __device__ __forceinline__ void march(const SlabEntry* __restrict__ row, int n_slabs, int dT, RayZ r, Sink& sink) {
-    const float inv32 = 2.3283064365386963e-10f;   // 2^-32
     const int4* row4 = reinterpret_cast<const int4*>(row);          // two entries per 16 B
     int k = r.k;
-    unsigned long long QZ = r.QZ;
+    unsigned qlo = (unsigned)r.QZ, qhi = (unsigned)(r.QZ >> 32);     // next z crossing: slab, share * 2^32
+    const unsigned dlo = (unsigned)r.dQZ, dhi = (unsigned)(r.dQZ >> 32);
     int4 ea = __ldg(row4), eb = __ldg(row4 + 1);
     for (int n0 = 0; n0 < n_slabs; n0 += U) {
         const int4 na = __ldg(row4 + (n0 >> 1) + 2), nb = __ldg(row4 + (n0 >> 1) + 3);   // next group
         const int off0s[U] = {ea.x, ea.z, eb.x, eb.z};
         const float tts[U] = {__int_as_float(ea.y), __int_as_float(ea.w), __int_as_float(eb.y), __int_as_float(eb.w)};
-        int po[U][3], pk[U][3];
+        int pi[U][3], pk[U][3];
         float pt[U][3], pv[U][3];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const int off0 = off0s[u], off1 = off0s[u] + dT;
+            // shares are kept in units of 2^-32 of a slab (the table's tt is stored that way and the
+            // crossing counter's low word is one already): the caller scales the sum once
             const float tt = tts[u];
-            const bool cz = (unsigned)(QZ >> 32) == (unsigned)(n0 + u);
-            const float tz = cz ? __uint2float_rn((unsigned)QZ) * inv32 : 1.f;
-            const int ke = cz ? k + r.dirZ : k;
+            const bool cz = qhi == (unsigned)(n0 + u);
+            const float tz = cz ? __uint2float_rn(qlo) : 4294967296.f;
+            const int dk = cz ? r.dirZ : 0;
             const float t1 = fminf(tt, tz), t2 = fmaxf(tt, tz);
             const bool tfirst = tt < tz;
-            po[u][0] = off0;                  pk[u][0] = k;                pt[u][0] = t1;
-            po[u][1] = tfirst ? off1 : off0;  pk[u][1] = tfirst ? k : ke;  pt[u][1] = t2 - t1;
-            po[u][2] = off1;                  pk[u][2] = ke;               pt[u][2] = 1.f - t2;
+            const int i0 = off0s[u] + k;
+            pi[u][0] = i0;                          pk[u][0] = k;                    pt[u][0] = t1;
+            pi[u][1] = i0 + (tfirst ? dT : dk);     pk[u][1] = tfirst ? k : k + dk;  pt[u][1] = t2 - t1;
+            pi[u][2] = i0 + dT + dk;                pk[u][2] = k + dk;               pt[u][2] = 4294967296.f - t2;
 #pragma unroll
-            for (int i = 0; i < 3; ++i) pv[u][i] = sink.fetch(po[u][i], pk[u][i]);
-            k = ke;
-            if (cz) QZ += r.dQZ;
+            for (int i = 0; i < 3; ++i) pv[u][i] = sink.fetch(pi[u][i], pk[u][i]);
+            k += dk;
+            asm("{\n"
+                ".reg .pred p;\n"
+                "setp.ne.s32 p, %2, 0;\n"
+                "@p add.cc.u32 %0, %0, %3;\n"
+                "@p addc.u32 %1, %1, %4;\n"
+                "}\n"
+                : "+r"(qlo), "+r"(qhi)
+                : "r"((int)cz), "r"(dlo), "r"(dhi));
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
 #pragma unroll
-            for (int i = 0; i < 3; ++i) sink.add(po[u][i], pk[u][i], pt[u][i], pv[u][i]);
+            for (int i = 0; i < 3; ++i) sink.add(pi[u][i], pk[u][i], pt[u][i], pv[u][i]);
         }
         ea = na; eb = nb;
     }
@@ -235,8 +244,8 @@ struct AccSink {
     const float* __restrict__ vol;
     int Nz;
     float acc;
-    __device__ __forceinline__ float fetch(int off, int k) const {
-        return (!CHECK || (unsigned)k < (unsigned)Nz) ? __ldg(vol + (unsigned)(off + k)) : 0.f;
+    __device__ __forceinline__ float fetch(int idx, int k) const {      // idx = column offset + k
+        return (!CHECK || (unsigned)k < (unsigned)Nz) ? __ldg(vol + (unsigned)idx) : 0.f;
     }
     __device__ __forceinline__ void add(int, int, float tau, float v) { acc = fmaf(tau, v, acc); }
 };
@@ -276,7 +285,7 @@ k_project(const Geom G, const SlotState* __restrict__ slots, const ColHdr* __res
             march(row, n, h.dT, r, sink);
             acc = sink.acc;
         }
-        p = acc * r.Ls;
+        p = acc * (r.Ls * 2.3283064365386963e-10f);      // the shares were summed in units of 2^-32
     }
     pseg[(((long long)s * n_seg + seg) * G.nu + iu) * G.nv + iv] = p;
 }
@@ -308,9 +317,10 @@ struct RecSink {
     int* ijk;
     float* len;
     __device__ __forceinline__ float fetch(int, int) const { return 0.f; }
-    __device__ __forceinline__ void add(int off, int k, float tau, float) {
+    __device__ __forceinline__ void add(int idx, int k, float tau_raw, float) {
         if (!((unsigned)k < (unsigned)nz)) return;
-        const int col = off / nz, jy = col / pnx - 1, jx = col % pnx - 1;
+        const float tau = tau_raw * 2.3283064365386963e-10f;                // shares come in units of 2^-32
+        const int col = (idx - k) / nz, jy = col / pnx - 1, jx = col % pnx - 1;
         if (!((unsigned)jx < (unsigned)nx && (unsigned)jy < (unsigned)ny)) return;      // zero border
         const float l = tau * Ls;
         if (!(l > eps)) return;     // zero-length pieces are dropped (reading A22)

@@ -57,7 +57,7 @@ struct ColHdr {
 
 // Per view, column and slab: element offset of the voxel column (i, j) the ray is in when it
 // enters the slab, and the share tt of the slab's path before the transverse plane crossing
-// (1 if none in this slab).
+// (1 if none in this slab), stored in units of 2^-32 of the slab like the z crossing counters.
 struct SlabEntry {
     int off0;
     float tt;

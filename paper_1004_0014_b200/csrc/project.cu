@@ -26,8 +26,8 @@
 // the trip count is uniform over the warp.  The volume was just written by the warp kernel and is
 // L2/L1-resident: this kernel is bound by instruction issue, not by HBM.
 //
-// a-3 (first half): the same kernel forms r_i = p_i - a y_i - b and the per-block partial sums of
-// p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.
+// The rays are cut into segments of SEG slabs (one block per segment of 4 columns x 32 rows);
+// k_project_finish (control.cu) adds the segments and forms the a-3 sums.
 #include "internal.h"
 
 namespace pcamm {

@@ -228,12 +228,12 @@ int grad_grid(const Geom& G, const FieldStream& fs) {
 // Per tile and solve the group's K sums are reduced in double and added to the group's slot of
 // the partial-sum buffer; the control kernel adds the slots in index order.
 
-constexpr int GNG = 3;
+constexpr int GNG = 2;
 constexpr int GTHREADS = 32 * (GNG * GROUP_WARPS + 1);
 constexpr int GSTATIC = 12 * 1024;                  // static shared memory of the kernel, rounded up
 constexpr int SOLVE_CACHE = 64;                     // solves whose constants are kept in shared memory
 
-template <int K> struct GradBatch { static constexpr int value = 2; };                  // RB
+template <int K> struct GradBatch { static constexpr int value = K <= 3 ? 4 : 2; };     // RB
 
 template <int K>
 struct QueueEntry {

@@ -83,6 +83,7 @@ struct pcamm_model {
     float *f0 = nullptr, *fields = nullptr, *xbar = nullptr, *u = nullptr, *lm0 = nullptr;   // xbar, u: views of fields
     FieldStream fs;
     // scratch (device)
+    unsigned char* cellmap = nullptr;   // FieldStream::cellmap
     float *vol = nullptr, *pseg = nullptr, *p = nullptr, *rL = nullptr;   // vol: trial volumes, ray layout [S][PV]
     ColHdr* col_hdr = nullptr;      // [B][nu]
     SlabEntry* slab_tab = nullptr;  // [B][nu][max_slabs]
@@ -464,7 +465,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     m->trav_cap = G.nx + G.ny + G.nz + 8;
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return r == cudaSuccess; };
-    ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->fields, 3 * (size_t)V * (G.K + 1))) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
+    ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->cellmap, (size_t)(g->nx + 1) * (g->ny + 1) * (g->nz + 1))) && ok(dalloc(m, &m->fields, 3 * (size_t)V * (G.K + 1))) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
         ok(dalloc(m, &m->vol, S * (size_t)G.PV)) && ok(dalloc(m, &m->col_hdr, B * G.nu)) &&
         ok(dalloc(m, &m->slab_tab, B * G.nu * (size_t)max_slabs(G))) && ok(dalloc(m, &m->p, S * G.npix)) && ok(dalloc(m, &m->pseg, S * G.npix * (size_t)project_segments(G))) &&
         ok(dalloc(m, &m->rL, B * G.npix)) && ok(dalloc(m, &m->utab, B * G.nu)) && ok(dalloc(m, &m->vtab, B * G.nv)) &&
@@ -517,6 +518,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     k_count_nonfinite<<<592, 256, 0, st>>>(m->xbar, 3 * V, m->nonfinite);
     k_count_nonfinite<<<592, 256, 0, st>>>(m->u, 3 * V * G.K, m->nonfinite);
     k_fields_to_voxel_units<<<1184, 256, 0, st>>>(m->fields, V, 3 * (G.K + 1), G.hx, G.hy, G.hz);
+    launch_build_cellmap(st, G, m->f0, m->cellmap);
+    m->fs.cellmap = m->cellmap;
     unsigned long long bad = 0;
     TRY_OR_FAIL(cudaMemcpyAsync(&bad, m->nonfinite, sizeof(bad), cudaMemcpyDeviceToHost, st));
     TRY_OR_FAIL(cudaStreamSynchronize(st));

@@ -229,7 +229,7 @@ int grad_grid(const Geom& G, const FieldStream& fs) {
 // the partial-sum buffer; the control kernel adds the slots in index order.
 
 constexpr int GNG = 2;
-constexpr int GTHREADS = 32 * (GNG * GROUP_WARPS + 1);
+constexpr int GTHREADS = 32 * GNG * GROUP_WARPS;
 constexpr int GSTATIC = 12 * 1024;                  // static shared memory of the kernel, rounded up
 constexpr int SOLVE_CACHE = 64;                     // solves whose constants are kept in shared memory
 
@@ -258,7 +258,7 @@ constexpr size_t grad_smem_bytes() {
 template <int K, bool SINGLE>
 __global__ void __launch_bounds__(GTHREADS, 1)
 k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
-           const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
+           const unsigned char* __restrict__ cellmap, const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
            const float2* __restrict__ vtab, double* __restrict__ partials) {
     constexpr int P = 3 * (K + 1), GTZ = TileZ<K>::value, GROWS = GTZ / GROUP_WARPS;
     constexpr int RB = GradBatch<K>::value, NB = GROWS / RB;
@@ -286,10 +286,6 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     __syncthreads();
     const long long n_tiles = tile_count(G, GTZ);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (warp == GNG * GROUP_WARPS) {                       // producer
-        if (lane == 0) ring.produce(&fmap, G, n_tiles);
-        return;
-    }
     const int group = warp / GROUP_WARPS, tw = warp % GROUP_WARPS, gtid = threadIdx.x - group * GROUP_THREADS;
     constexpr int QCAP = GradQueueCap<K>::value;
     QueueEntry<K>* queue = queues + (size_t)group * QCAP;   // ring buffer: q_head .. q_head + q_n - 1 (mod QCAP)
@@ -297,12 +293,18 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     const int nslot = gridDim.x * GNG, slot = blockIdx.x * GNG + group;   // this group's partial-sum slot
     if (gtid < K)
         for (int b = 0; b < B; ++b) partials[((long long)b * nslot + slot) * KMAX + gtid] = 0.0;
+    bool any_running = false;
+    for (int b = 0; b < B; ++b) any_running |= s_running[b] != 0;
+    if (!any_running) return;                              // uniform over the grid
+    const bool leader = gtid == 0;
+    const uint64_t policy = l2_evict_first_policy();
+    if (leader) ring.prologue(&fmap, G, n_tiles, group, policy);
 
     float acc[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) acc[k] = 0.f;
     int j = 0;                                             // this group's tile counter
-    for (long long t = blockIdx.x + (long long)group * gridDim.x; t < n_tiles; t += (long long)GNG * gridDim.x, ++j) {
+    for (long long t = Ring::tile_of(group, 0); t < n_tiles; t += (long long)GNG * gridDim.x, ++j) {
         {
             const int s = Ring::stage_of(group, j);
             mbar_wait(ring.full + s, Ring::parity_of(j));
@@ -324,43 +326,70 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                 }
 #pragma unroll 1
                 for (int bt = 0; bt < NB; ++bt) {
-                    // 1. G_j and q_kj
-                    Taps taps[RB];
+                    // 1. G_j and q_kj.  A voxel whose interpolation cell of f0 is constant (cell map,
+                    //    one byte) has G_j = 0 exactly: a warp none of whose voxels of this batch needs
+                    //    more skips the taps, the gathers and the derivative (most of the volume: air,
+                    //    the inside of a homogeneous organ).
+                    float dd[RB][3];
+                    unsigned char flag[RB];
 #pragma unroll
                     for (int rr = 0; rr < RB; ++rr) {
                         const int zz = tw + GROUP_WARPS * (bt * RB + rr);
-                        float d[3];
 #pragma unroll
                         for (int cc = 0; cc < 3; ++cc) {
                             float xs = lds_f32(sf + 4u * ((cc * GTZ + zz) * TX + lane));           // Eq. (1)
 #pragma unroll
                             for (int k = 0; k < K; ++k)
                                 xs = fmaf(lds_f32(sf + 4u * (((3 + 3 * k + cc) * GTZ + zz) * TX + lane)), w[k], xs);
-                            d[cc] = xs;
+                            dd[rr][cc] = xs;
                         }
-                        taps[rr] = make_taps(G.nx, G.ny, G.nz, x, c.y, c.z0 + zz, d[0], d[1], d[2]);
+                        const int ci = x + (int)floorf(dd[rr][0]) + 1, cj = c.y + (int)floorf(dd[rr][1]) + 1,
+                                  ck = c.z0 + zz + (int)floorf(dd[rr][2]) + 1;
+                        const bool inside = x < G.nx && c.z0 + zz < G.nz && (unsigned)ci <= (unsigned)G.nx &&
+                                            (unsigned)cj <= (unsigned)G.ny && (unsigned)ck <= (unsigned)G.nz;
+                        flag[rr] = inside ? __ldg(cellmap + ((long long)ck * (G.ny + 1) + cj) * (G.nx + 1) + ci) : (unsigned char)0;
                     }
-                    float cv[RB][8];
+                    bool mine = false;
 #pragma unroll
-                    for (int rr = 0; rr < RB; ++rr) gather8(f0, taps[rr], cv[rr]);
+                    for (int rr = 0; rr < RB; ++rr) mine |= flag[rr] != 0;
                     float q[RB][K];
                     unsigned masks[RB];
 #pragma unroll
                     for (int rr = 0; rr < RB; ++rr) {
-                        const int zz = tw + GROUP_WARPS * (bt * RB + rr);
-                        float gx, gy, gz;
-                        grad8(taps[rr], cv[rr], &gx, &gy, &gz);
+                        masks[rr] = 0u;
 #pragma unroll
-                        for (int k = 0; k < K; ++k)
-                            q[rr][k] = gx * lds_f32(sf + 4u * (((3 + 3 * k + 0) * GTZ + zz) * TX + lane)) +
-                                       gy * lds_f32(sf + 4u * (((3 + 3 * k + 1) * GTZ + zz) * TX + lane)) +
-                                       gz * lds_f32(sf + 4u * (((3 + 3 * k + 2) * GTZ + zz) * TX + lane));
-                        const bool active = x < G.nx && c.z0 + zz < G.nz && (gx != 0.f || gy != 0.f || gz != 0.f);
-                        masks[rr] = __ballot_sync(0xffffffffu, active);
-                        if (lane == 0) s_cnt[group][parity][rr * GROUP_WARPS + tw] = __popc(masks[rr]);
+                        for (int k = 0; k < K; ++k) q[rr][k] = 0.f;
+                    }
+                    if (__any_sync(0xffffffffu, mine)) {                       // uniform over the warp
+                        Taps taps[RB];
+#pragma unroll
+                        for (int rr = 0; rr < RB; ++rr)
+                            taps[rr] = make_taps(G.nx, G.ny, G.nz, x, c.y, c.z0 + tw + GROUP_WARPS * (bt * RB + rr),
+                                                 dd[rr][0], dd[rr][1], dd[rr][2]);
+                        float cv[RB][8];
+#pragma unroll
+                        for (int rr = 0; rr < RB; ++rr) gather8(f0, taps[rr], cv[rr]);
+#pragma unroll
+                        for (int rr = 0; rr < RB; ++rr) {
+                            const int zz = tw + GROUP_WARPS * (bt * RB + rr);
+                            float gx, gy, gz;
+                            grad8(taps[rr], cv[rr], &gx, &gy, &gz);
+#pragma unroll
+                            for (int k = 0; k < K; ++k)
+                                q[rr][k] = gx * lds_f32(sf + 4u * (((3 + 3 * k + 0) * GTZ + zz) * TX + lane)) +
+                                           gy * lds_f32(sf + 4u * (((3 + 3 * k + 1) * GTZ + zz) * TX + lane)) +
+                                           gz * lds_f32(sf + 4u * (((3 + 3 * k + 2) * GTZ + zz) * TX + lane));
+                            const bool active = flag[rr] != 0 && (gx != 0.f || gy != 0.f || gz != 0.f);
+                            masks[rr] = __ballot_sync(0xffffffffu, active);
+                        }
+                    }
+                    if (lane == 0) {
+#pragma unroll
+                        for (int rr = 0; rr < RB; ++rr) s_cnt[group][parity][rr * GROUP_WARPS + tw] = __popc(masks[rr]);
                     }
                     group_barrier(group);
-                    if (SINGLE && bt == NB - 1 && gtid == 0) mbar_arrive(ring.empty + s);   // no more reads of the stage
+                    if (SINGLE && bt == NB - 1 && leader)                   // no more reads of the stage: refill it
+                        ring.issue(&fmap, G, n_tiles, group, j + GradStages<K>::value, policy);
                     // 2. compaction in the fixed order (row, warp, lane), appended to the queue
                     int cnt = lane < RB * GROUP_WARPS ? s_cnt[group][parity][lane] : 0, incl = cnt;
                     parity ^= 1;
@@ -426,8 +455,8 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
             }
             if (!SINGLE) {
                 group_barrier(group);                       // every thread of the group is done with the stage
-                if (gtid == 0) mbar_arrive(ring.empty + s);
-            } else if (!s_running[0] && gtid == 0) mbar_arrive(ring.empty + s);
+                if (leader) ring.issue(&fmap, G, n_tiles, group, j + GradStages<K>::value, policy);
+            }
         }
     }
     if (SINGLE) {                                           // the group's K sums over all its tiles
@@ -464,6 +493,27 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     }
 }
 
+// The cell map of FieldStream: one thread per interpolation cell.
+__global__ void __launch_bounds__(256)
+k_build_cellmap(const Geom G, const float* __restrict__ f0, unsigned char* __restrict__ cellmap) {
+    const long long n = (long long)(G.nx + 1) * (G.ny + 1) * (G.nz + 1);
+    const long long lin = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (lin >= n) return;
+    const int i0 = (int)(lin % (G.nx + 1)) - 1, j0 = (int)((lin / (G.nx + 1)) % (G.ny + 1)) - 1,
+              k0 = (int)(lin / ((long long)(G.nx + 1) * (G.ny + 1))) - 1;
+    float first = 0.f;
+    bool varies = false;
+#pragma unroll
+    for (int t = 0; t < 8; ++t) {
+        const int i = i0 + (t & 1), j = j0 + ((t >> 1) & 1), k = k0 + (t >> 2);
+        const bool in = (unsigned)i < (unsigned)G.nx && (unsigned)j < (unsigned)G.ny && (unsigned)k < (unsigned)G.nz;
+        const float v = in ? f0[((long long)k * G.ny + j) * G.nx + i] : 0.f;      // zero padding (reading A2)
+        if (t == 0) first = v;
+        else varies |= v != first;
+    }
+    cellmap[lin] = varies ? 1 : 0;
+}
+
 // Hook: B = P^T r as a volume (view of solve 0).
 __global__ void __launch_bounds__(256)
 k_backproject(const Geom G, const SolveState* __restrict__ solves, const float* __restrict__ rL,
@@ -493,13 +543,13 @@ void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, con
         }
         const int grid = grad_grid(G, fs), nslot = grid * GNG;
         if (B == 1) {
-            q.launch(k_grad_tma<K, true>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), G, f0, solves, 1, rL, utab, vtab,
+            q.launch(k_grad_tma<K, true>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), G, f0, fs.cellmap, solves, 1, rL, utab, vtab,
                      partials);
             return;
         }
         for (int b0 = 0; b0 < B; b0 += SOLVE_CACHE) {       // the kernel keeps up to SOLVE_CACHE solves' constants on chip
             const int nb = B - b0 < SOLVE_CACHE ? B - b0 : SOLVE_CACHE;
-            q.launch(k_grad_tma<K, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), G, f0, solves + b0, nb,
+            q.launch(k_grad_tma<K, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), G, f0, fs.cellmap, solves + b0, nb,
                      rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu, vtab + (long long)b0 * G.nv,
                      partials + (long long)b0 * nslot * KMAX);
         }
@@ -513,6 +563,11 @@ void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, con
 }  // namespace
 
 int resid_blocks(const Geom& G) { return (G.npix + RT - 1) / RT; }
+
+void launch_build_cellmap(cudaStream_t st, const Geom& G, const float* f0, unsigned char* cellmap) {
+    const long long n = (long long)(G.nx + 1) * (G.ny + 1) * (G.nz + 1);
+    k_build_cellmap<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, f0, cellmap);
+}
 // partial-sum slots per solve: two per persistent CTA (TMA kernel), else one per block
 int grad_blocks(const Geom& G, const FieldStream& fs) {
     if (fs.use_tma) return grad_grid(G, fs) * GNG;

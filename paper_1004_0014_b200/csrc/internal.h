@@ -101,6 +101,7 @@ void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* 
 // ---- a-3 / a-4 (gradient.cu)
 int resid_blocks(const Geom& G);
 int grad_blocks(const Geom& G, const FieldStream& fs);
+void launch_build_cellmap(cudaStream_t st, const Geom& G, const float* f0, unsigned char* cellmap);
 // r = p - a y - b, rL = r * |D - S|, per-view tables, partial sums of r^2; p of solve b is read
 // from its accepted slot.
 // force: also for solves that are no longer running (closing pass); r_direct: take r from there.

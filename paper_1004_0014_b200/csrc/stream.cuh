@@ -2,10 +2,10 @@
 // gradient.cu): both make one pass over the K+1 planar vector fields (Eq. 1:
 // x = xbar + sum_k u_k w_k needs all of them per voxel) and then chase 8-tap gathers in f0.
 //
-// A persistent CTA per SM.  One producer thread moves field tiles HBM -> shared memory with TMA
-// (cp.async.bulk.tensor, one 4-D box {TX x, 1 y, TZ z, 3(K+1) planes} per tile, completion
-// signalled on an mbarrier) through a ring of stages; consumer groups of 8 warps take the tiles
-// in turn.  The stream is thereby decoupled from the consumers' dependent chain
+// A persistent CTA per SM, made of consumer groups of 8 warps that take the CTA's tiles in turn.
+// Field tiles come HBM -> shared memory by TMA (cp.async.bulk.tensor, one 4-D box
+// {TX x, 1 y, TZ z, 3(K+1) planes} per tile, completion signalled on an mbarrier), issued by the
+// group's leader one or two tiles ahead.  The stream is thereby decoupled from the dependent chain
 // (fields -> displaced position -> f0 gathers -> interpolation), which is what kept the first,
 // register-staged version of these kernels at 35 % of the DRAM bandwidth (profiles/r01a).
 //
@@ -104,48 +104,54 @@ __device__ __forceinline__ void group_barrier(int group) {
 // Shared-memory stages of a streaming kernel: NG consumer groups with SPG stages each, a stage
 // being P planes x TZ x TX floats.  The CTA's i-th tile (tile blockIdx.x + i * gridDim.x of the
 // volume) belongs to group i % NG and is that group's (i / NG)-th tile; it goes through stage
-// (i / NG) % SPG of the group's own little ring.  Every stage is therefore filled and drained
-// by one producer and ONE group, strictly in order, which is what makes waiting on a phase
-// parity sound (a group sharing stages with others could be a whole ring cycle ahead of the
+// (i / NG) % SPG of the group's own little ring.  Every stage is filled and drained by ONE group,
+// strictly in order: the group's leader thread issues the TMA load of the group's tile j + SPG
+// into a stage as soon as the group has read tile j's fields out of it (a group barrier), so no
+// "empty" barrier and no producer warp are needed, and waiting on the phase parity of the "full"
+// barrier is sound (a group sharing stages with others could be a whole ring cycle ahead of the
 // barrier it polls and mistake the previous phase for its own).
 template <int P, int TZ, int NG, int SPG>
 struct FieldRing {
     static constexpr int NS = NG * SPG;
     static constexpr int STAGE_FLOATS = P * TZ * TX;
     static constexpr uint32_t STAGE_BYTES = STAGE_FLOATS * 4u;
-    static constexpr size_t BYTES = (size_t)NS * STAGE_BYTES + 2 * NS * sizeof(uint64_t);
+    static constexpr size_t BYTES = (size_t)NS * STAGE_BYTES + NS * sizeof(uint64_t);
 
     float* data;        // 128 B aligned
     uint64_t* full;     // [NS] TMA completion
-    uint64_t* empty;    // [NS] the group is done with the stage
 
     __device__ __forceinline__ void bind(unsigned char* smem) {
         data = reinterpret_cast<float*>(smem);
         full = reinterpret_cast<uint64_t*>(smem + (size_t)NS * STAGE_BYTES);
-        empty = full + NS;
     }
     __device__ __forceinline__ void init() {   // one thread
-        for (int s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        for (int s = 0; s < NS; ++s) mbar_init(full + s, 1);
         mbar_fence_init();
     }
     __device__ __forceinline__ const float* stage(int s) const { return data + (size_t)s * STAGE_FLOATS; }
 
-    // Producer (one thread).
-    __device__ __forceinline__ void produce(const CUtensorMap* map, const Geom& G, long long n_tiles) {
-        const uint64_t policy = l2_evict_first_policy();
-        int g = 0, j = 0;                                        // group of the tile, the group's tile counter
-        for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-            const int s = g * SPG + j % SPG;
-            mbar_wait(empty + s, ((uint32_t)(j / SPG) & 1u) ^ 1u);   // the stage is free (passes at once the first time)
-            const TileCoord c = tile_coord(G, TZ, t);
-            mbar_arrive_expect_tx(full + s, STAGE_BYTES);
-            tma_load_4d(data + (size_t)s * STAGE_FLOATS, map, full + s, c.x0, c.y, c.z0, 0, policy);
-            if (++g == NG) { g = 0; ++j; }
-        }
+    // Tile of the volume that is group g's j-th tile in this CTA (may be >= the tile count).
+    __device__ __forceinline__ static long long tile_of(int g, int j) {
+        return (long long)blockIdx.x + ((long long)g + (long long)j * NG) * gridDim.x;
     }
-    // Consumer group g: stage and phase parity of its j-th tile.
     __device__ __forceinline__ static int stage_of(int g, int j) { return g * SPG + j % SPG; }
     __device__ __forceinline__ static uint32_t parity_of(int j) { return (uint32_t)(j / SPG) & 1u; }
+
+    // Group leader: start the load of the group's j-th tile (nothing if the volume has no such tile).
+    __device__ __forceinline__ void issue(const CUtensorMap* map, const Geom& G, long long n_tiles, int g, int j,
+                                          uint64_t policy) const {
+        const long long t = tile_of(g, j);
+        if (t >= n_tiles) return;
+        const int s = stage_of(g, j);
+        const TileCoord c = tile_coord(G, TZ, t);
+        mbar_arrive_expect_tx(full + s, STAGE_BYTES);
+        tma_load_4d(data + (size_t)s * STAGE_FLOATS, map, full + s, c.x0, c.y, c.z0, 0, policy);
+    }
+    // Group leader, once: the first SPG tiles.
+    __device__ __forceinline__ void prologue(const CUtensorMap* map, const Geom& G, long long n_tiles, int g,
+                                             uint64_t policy) const {
+        for (int j = 0; j < SPG; ++j) issue(map, G, n_tiles, g, j, policy);
+    }
 };
 
 // What the streaming kernels need to know about the model's fields.
@@ -154,6 +160,10 @@ struct FieldStream {
     bool use_tma = false;            // false: register-staged generic kernels
     int n_sm = 1;                    // persistent grid size
     CUtensorMap map32, map16;        // boxes {TX, 1, 32 | 16, 3(K+1)}
+    // one byte per interpolation cell (i0, j0, k0) in [-1, n-1]^3, element
+    // ((k0+1)(ny+1) + (j0+1))(nx+1) + (i0+1): 0 if the cell's eight zero-padded taps of f0 are all
+    // equal (then the image gradient is exactly 0 anywhere in the cell), else 1 (gradient.cu)
+    const unsigned char* cellmap = nullptr;
 };
 
 // Tile extent along z and ring depth by K: a stage is 3(K+1) planes x TZ x TX floats and the

@@ -114,7 +114,7 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
 
 constexpr int WNG = 3;             // consumer groups
 constexpr int SLOT_CACHE = 64;     // slots whose coefficients are kept in shared memory
-constexpr int WTHREADS = 32 * (WNG * GROUP_WARPS + 1);
+constexpr int WTHREADS = 32 * WNG * GROUP_WARPS;
 
 constexpr int WSTATIC = 16 * 1024; // static shared memory of the kernel (transposition tiles, slot cache), rounded up
 template <int K> struct WarpStages { static constexpr int value = stages_per_group<K>(WNG, 2, 227 * 1024 - WSTATIC - 64); };
@@ -151,14 +151,14 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     int last_active = -1;                                  // the last slot that reads the stage
     for (int i = 0; i < nslots; ++i)
         if (s_active[i]) last_active = i;
-    if (warp == WNG * GROUP_WARPS) {                       // producer
-        if (lane == 0) ring.produce(&fmap, G, n_tiles);
-        return;
-    }
+    if (last_active < 0) return;                           // nothing to warp
     const int group = warp / GROUP_WARPS, tw = warp % GROUP_WARPS;
+    const bool leader = tw == 0 && lane == 0;
+    const uint64_t policy = l2_evict_first_policy();
     float(*tile)[TX + 1] = tiles[group];
+    if (leader) ring.prologue(&fmap, G, n_tiles, group, policy);
     int j = 0;                                             // this group's tile counter
-    for (long long t = blockIdx.x + (long long)group * gridDim.x; t < n_tiles; t += (long long)WNG * gridDim.x, ++j) {
+    for (long long t = Ring::tile_of(group, 0); t < n_tiles; t += (long long)WNG * gridDim.x, ++j) {
         {
             const int s = Ring::stage_of(group, j);
             mbar_wait(ring.full + s, Ring::parity_of(j));
@@ -188,9 +188,9 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     }
                     taps[r] = make_taps(G.nx, G.ny, G.nz, x, c.y, z, d[0], d[1], d[2]);
                 }
-                if (sl == last_active) {                    // the fields of this tile are in registers: hand the
-                    group_barrier(group);                   // stage back while the gathers are under way
-                    if (tw == 0 && lane == 0) mbar_arrive(ring.empty + s);
+                if (sl == last_active) {                    // the fields of this tile are in registers: refill the
+                    group_barrier(group);                   // stage while the gathers are under way
+                    if (leader) ring.issue(&fmap, G, n_tiles, group, j + WarpStages<K>::value, policy);
                 }
                 float cv[WROWS][8];
 #pragma unroll
@@ -217,7 +217,6 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     }
                 }
             }
-            if (last_active < 0 && tw == 0 && lane == 0) mbar_arrive(ring.empty + s);   // nothing to do: pass the stage on
         }
     }
 }

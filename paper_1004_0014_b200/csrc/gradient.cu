@@ -334,7 +334,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     unsigned char flag[RB];
 #pragma unroll
                     for (int rr = 0; rr < RB; ++rr) {
-                        const int zz = tw + GROUP_WARPS * (bt * RB + rr);
+                        const int zz = tw * GROWS + bt * RB + rr;
 #pragma unroll
                         for (int cc = 0; cc < 3; ++cc) {
                             float xs = lds_f32(sf + 4u * ((cc * GTZ + zz) * TX + lane));           // Eq. (1)
@@ -364,14 +364,14 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                         Taps taps[RB];
 #pragma unroll
                         for (int rr = 0; rr < RB; ++rr)
-                            taps[rr] = make_taps(G.nx, G.ny, G.nz, x, c.y, c.z0 + tw + GROUP_WARPS * (bt * RB + rr),
+                            taps[rr] = make_taps(G.nx, G.ny, G.nz, x, c.y, c.z0 + tw * GROWS + bt * RB + rr,
                                                  dd[rr][0], dd[rr][1], dd[rr][2]);
                         float cv[RB][8];
 #pragma unroll
                         for (int rr = 0; rr < RB; ++rr) gather8(f0, taps[rr], cv[rr]);
 #pragma unroll
                         for (int rr = 0; rr < RB; ++rr) {
-                            const int zz = tw + GROUP_WARPS * (bt * RB + rr);
+                            const int zz = tw * GROWS + bt * RB + rr;
                             float gx, gy, gz;
                             grad8(taps[rr], cv[rr], &gx, &gy, &gz);
 #pragma unroll
@@ -408,7 +408,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                             if (pos >= QCAP) pos -= QCAP;
                             QueueEntry<K>& e = queue[pos];
                             e.xy = x | c.y << 16;
-                            e.z = c.z0 + tw + GROUP_WARPS * (bt * RB + rr);
+                            e.z = c.z0 + tw * GROWS + bt * RB + rr;
 #pragma unroll
                             for (int k = 0; k < K; ++k) e.q[k] = q[rr][k];
                         }

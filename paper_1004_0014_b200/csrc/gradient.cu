@@ -228,12 +228,18 @@ int grad_grid(const Geom& G, const FieldStream& fs) {
 // Per tile and solve the group's K sums are reduced in double and added to the group's slot of
 // the partial-sum buffer; the control kernel adds the slots in index order.
 
-constexpr int GNG = 2;
-constexpr int GTHREADS = 32 * GNG * GROUP_WARPS;
+// Consumer groups per CTA: three where their stages and queues fit into shared memory, else two.
+constexpr int grad_groups_for(int K) {
+    const int tz = K <= 4 ? 32 : 16;                                      // TileZ<K>
+    const int stage = 3 * (K + 1) * tz * TX * 4;
+    const int queue = GROUP_THREADS * 3 * (8 + 4 * K);                    // GradQueueCap x sizeof(QueueEntry)
+    return 3 * (stage + queue) + 16 * 1024 <= 227 * 1024 ? 3 : 2;
+}
+template <int K> struct GradGroups { static constexpr int value = grad_groups_for(K); };
 constexpr int GSTATIC = 12 * 1024;                  // static shared memory of the kernel, rounded up
 constexpr int SOLVE_CACHE = 64;                     // solves whose constants are kept in shared memory
 
-template <int K> struct GradBatch { static constexpr int value = K <= 3 ? 4 : 2; };     // RB
+template <int K> struct GradBatch { static constexpr int value = 2; };     // RB
 
 template <int K>
 struct QueueEntry {
@@ -244,25 +250,26 @@ struct QueueEntry {
 // Entries of a group's queue: one batch of new ones plus what the last round left over.
 template <int K> struct GradQueueCap { static constexpr int value = GROUP_THREADS * (GradBatch<K>::value + 1); };
 template <int K>
-constexpr size_t grad_queue_bytes() { return (size_t)GNG * GradQueueCap<K>::value * sizeof(QueueEntry<K>); }
+constexpr size_t grad_queue_bytes() { return (size_t)GradGroups<K>::value * GradQueueCap<K>::value * sizeof(QueueEntry<K>); }
 template <int K> struct GradStages {
-    static constexpr int value = stages_per_group<K>(GNG, 2, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
+    static constexpr int value = stages_per_group<K>(GradGroups<K>::value, 2, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
 };
 template <int K>
 constexpr size_t grad_smem_bytes() {
-    return FieldRing<3 * (K + 1), TileZ<K>::value, GNG, GradStages<K>::value>::BYTES + 16 + grad_queue_bytes<K>();
+    return FieldRing<3 * (K + 1), TileZ<K>::value, GradGroups<K>::value, GradStages<K>::value>::BYTES + 16 + grad_queue_bytes<K>();
 }
 
 // SINGLE: one solve (B = 1): the K sums stay in registers over all tiles of the CTA and are
 // reduced once at the end; otherwise they are reduced per tile and solve.
 template <int K, bool SINGLE>
-__global__ void __launch_bounds__(GTHREADS, 1)
+__global__ void __launch_bounds__(32 * GradGroups<K>::value * GROUP_WARPS, 1)
 k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
            const unsigned char* __restrict__ cellmap, const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
            const float2* __restrict__ vtab, double* __restrict__ partials) {
     constexpr int P = 3 * (K + 1), GTZ = TileZ<K>::value, GROWS = GTZ / GROUP_WARPS;
     constexpr int RB = GradBatch<K>::value, NB = GROWS / RB;
     static_assert(GROWS % RB == 0 && NB >= 1, "tile rows per thread must be a multiple of the batch");
+    constexpr int GNG = GradGroups<K>::value;
     using Ring = FieldRing<P, GTZ, GNG, GradStages<K>::value>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ int s_cnt[GNG][2][32];                      // double buffered over the batches
@@ -541,6 +548,7 @@ void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, con
             if (e != cudaSuccess) { q.err = e; return; }
             configured = true;
         }
+        constexpr int GNG = GradGroups<K>::value, GTHREADS = 32 * GNG * GROUP_WARPS;
         const int grid = grad_grid(G, fs), nslot = grid * GNG;
         if (B == 1) {
             q.launch(k_grad_tma<K, true>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), G, f0, fs.cellmap, solves, 1, rL, utab, vtab,
@@ -570,7 +578,7 @@ void launch_build_cellmap(cudaStream_t st, const Geom& G, const float* f0, unsig
 }
 // partial-sum slots per solve: two per persistent CTA (TMA kernel), else one per block
 int grad_blocks(const Geom& G, const FieldStream& fs) {
-    if (fs.use_tma) return grad_grid(G, fs) * GNG;
+    if (fs.use_tma) return grad_grid(G, fs) * grad_groups_for(G.K);
     return ((G.nx + TILE - 1) / TILE) * ((G.ny + TILE - 1) / TILE) * G.nz;
 }
 

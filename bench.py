@@ -232,13 +232,15 @@ def run_reference(args, cfg, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def config_dict(cfg, iterations):
+def config_dict(cfg, iterations, fan=1):
     return {"workload": f"{cfg.name}: volume {cfg.nx}x{cfg.ny}x{cfg.nz} @ {cfg.hx} mm, K={cfg.K}, detector "
                         f"{cfg.nu}x{cfg.nv} @ {cfg.pu} mm, consecutive projections 1 deg / (1/6) s apart from frame "
                         f"{FIRST_FRAME}, {cfg.noise} noise, {'irregular' if cfg.irregular else 'regular'} breathing "
                         f"x{cfg.amplitude}",
             "iterations": iterations, "warm_start": "previous frame's w (PAPER.md:L141)",
-            "line_search": "batched 8 candidates" if cfg.batched_linesearch else "sequential Armijo backtracking",
+            "line_search": "Armijo backtracking, all 8 candidate steps per pass" if cfg.batched_linesearch else
+                           ("sequential Armijo backtracking" if fan <= 1 else
+                            f"Armijo backtracking, {fan} candidate steps per pass (same accepted step as sequential)"),
             "l2": "inputs larger than L2: every pass streams the (K+1) vector fields "
                   f"({12 * (cfg.K + 1) * cfg.V / 2**20:.0f} MiB) through a 126 MB L2",
             "parallelism": "replicas"}
@@ -268,7 +270,8 @@ def run_ours(args, cfg, rank, local_rank, world):
     dev = torch.device("cuda", local_rank)
     dist = replicas.init_process_group("nccl")
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(dev)
-    C = 8 if cfg.batched_linesearch else 1
+    fan = 1 if cfg.batched_linesearch else int(args.fan)     # pcamm_opts.batched_linesearch (1 = all 8 at once)
+    C = 8 if cfg.batched_linesearch else max(fan, 1)
     m = pc.Model(nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, hx=cfg.hx, hy=cfg.hy, hz=cfg.hz, K=cfg.K, nu=cfg.nu, nv=cfg.nv,
                  pu=cfg.pu, pv=cfg.pv, f0=t(wl.f0), mean_dvf=t(wl.model.mean), eig_dvf=t(wl.model.eig),
                  landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=C, max_batch=B)
@@ -284,7 +287,7 @@ def run_ours(args, cfg, rank, local_rank, world):
         ys_host.append(torch.from_numpy(y).pin_memory())
         ys_dev.append(t(y))
     angles = [float(wl.frames[fid].angle_rad) for fid in ids]
-    opts = pc.Opts(max_iter=it, batched_linesearch=int(cfg.batched_linesearch), loop_mode=args.loop_mode)
+    opts = pc.Opts(max_iter=it, batched_linesearch=fan if fan > 1 or cfg.batched_linesearch else 0, loop_mode=args.loop_mode)
     if B > 1:   # one stacked [B][nv][nu] tensor per distinct step
         n_distinct = len(ids) // B
         yb_dev = [torch.stack(ys_dev[j * B:(j + 1) * B]) for j in range(n_distinct)]
@@ -350,7 +353,9 @@ def run_ours(args, cfg, rank, local_rank, world):
     i_last = (n - 1) if B == 1 else 0
     tr = m.reconstruct(ys_dev[i_last], angles[i_last], w_after_warmup if B == 1 else np.zeros(cfg.K, np.float32),
                        opts, trace=True)
-    trials = int(np.sum(tr.backtracks + 1)) if tr.backtracks is not None else it
+    width = 8 if cfg.batched_linesearch else max(fan, 1)
+    # candidate steps evaluated (every pass evaluates `width` of them, or what is left of the budget of 8)
+    trials = int(np.sum(np.minimum(width * (tr.backtracks // width + 1), 8))) if tr.backtracks is not None else it
     m.eval(ys_dev[i_last], angles[i_last], tr.w, tr.a, tr.b, want_proj=False)
     for which in (0, 1, 2):
         m.time_kernel(which, 3)
@@ -395,7 +400,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     line = {"metric": METRIC, "value": ms_per_solve, "unit": "ms", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": dict(config_dict(cfg, it), in_flight=B), "projections_per_s": 1e3 * args.steps * world * B / elapsed_ms,
+            "config": dict(config_dict(cfg, it, fan), in_flight=B), "projections_per_s": 1e3 * args.steps * world * B / elapsed_ms,
             "clocks": clocks,
             "e2e": {"value": e2e_ms / (args.steps * world * B), "unit": "ms", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
@@ -413,6 +418,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fan", type=int, default=1,
+                    help="candidate steps evaluated per line-search pass (pcamm_opts.batched_linesearch): the "
+                         "accepted step is the same for every width; 1 = sequential backtracking")
     ap.add_argument("--in-flight", type=int, default=1,
                     help="B > 1: every step advances B independent projection solves in lock step "
                          "(pcamm_reconstruct_batch; BASELINE.json configs[4] sweeps 1, 4, 16, 64), each from w = 0")

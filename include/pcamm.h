@@ -77,8 +77,10 @@ typedef struct {
     float armijo_beta;      /* default 0.5 */
     int32_t max_backtracks; /* default 8 */
     float init_step_vox;    /* first trial moves the DVF by this many voxels rms; default 1 (A7) */
-    int32_t batched_linesearch; /* 0: sequential backtracking; 1: evaluate all candidates at once
-                                   and take the largest passing step (same result; config C3) */
+    int32_t batched_linesearch; /* 0: sequential backtracking; 1: evaluate all max_backtracks candidates
+                                   at once and take the largest passing step (config C3); F >= 2:
+                                   F candidates per pass, the next F if none passes.  The accepted
+                                   step is the same in every mode; needs max_candidates >= the fan */
     int32_t inv_max_iter;   /* default 50 (reading A13) */
     float inv_tol_mm;       /* default 1e-4 */
     int32_t loop_mode;      /* 0 (default): the whole solve is one CUDA graph with device-side

@@ -155,6 +155,14 @@ int check_seq(const Seq& q, const char* what) {
     return PCAMM_OK;
 }
 
+// Candidate steps evaluated per line-search pass: 0 -> 1 (sequential), 1 -> all max_backtracks
+// at once, F >= 2 -> F (the next F follow if none passes).
+int fan_width(const pcamm_opts& o) {
+    if (o.batched_linesearch <= 0) return 1;
+    if (o.batched_linesearch == 1) return o.max_backtracks;
+    return o.batched_linesearch < o.max_backtracks ? o.batched_linesearch : o.max_backtracks;
+}
+
 int resolve_opts(const pcamm_model* m, const pcamm_opts* user, pcamm_opts* o) {
     pcamm_default_opts(o);
     if (user) *o = *user;
@@ -162,8 +170,9 @@ int resolve_opts(const pcamm_model* m, const pcamm_opts* user, pcamm_opts* o) {
     if (o->max_backtracks < 1 || o->max_backtracks > MAXBT) return invalid("opts.max_backtracks out of range");
     if (!(o->armijo_beta > 0.f && o->armijo_beta < 1.f)) return invalid("opts.armijo_beta must be in (0, 1)");
     if (!(o->armijo_c >= 0.f) || !(o->init_step_vox > 0.f)) return invalid("opts.armijo_c / init_step_vox");
-    if (o->batched_linesearch && o->max_backtracks > m->Cmax)
-        return invalid("batched_linesearch needs geometry.max_candidates >= opts.max_backtracks");
+    if (o->batched_linesearch < 0) return invalid("opts.batched_linesearch < 0");
+    if (fan_width(*o) > m->Cmax)
+        return invalid("batched_linesearch needs geometry.max_candidates >= the fan width");
     if (o->inv_max_iter < 0) return invalid("opts.inv_max_iter < 0");
     return PCAMM_OK;
 }
@@ -285,7 +294,7 @@ int solve_impl(pcamm_model* m, int B, const float* y_dev, const float* angles, c
     int rc = resolve_opts(m, user_opts, &o);
     if (rc) return rc;
     const Geom& G = m->G;
-    const int C = o.batched_linesearch ? o.max_backtracks : 1;
+    const int C = fan_width(o);
     fill_call(m, o, B, C);
     SolveIn* in = h_solve_in(m);
     for (int b = 0; b < B; ++b) {

@@ -65,7 +65,7 @@ struct SlabEntry {
 
 // Host -> device, one copy per call.
 struct CallOpts {
-    int B, C;                 // solves in flight, candidate steps evaluated per trial round
+    int B, C;                 // solves in flight, candidate steps evaluated per trial round (the fan width)
     int max_iter, max_backtracks, batched, inv_max_iter;
     double grad_tol, armijo_c, armijo_beta, init_step_vox, inv_tol;
     double hmin_sqrtV;        // min(h) * sqrt(V): the 1-voxel-rms step scale (reading A7)

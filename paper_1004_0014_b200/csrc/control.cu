@@ -52,6 +52,20 @@ __device__ void set_view(const Geom& G, float angle, View* vw) {
     vw->cs = cos(th); vw->sn = sin(th);
 }
 
+// Candidates st.t, st.t + 1, ... (at most C per round, fewer at the end of the backtrack budget) of
+// the Armijo sequence mu0 beta^t into the solve's slots; st.mu is the step of candidate st.t and
+// every later one follows by repeated multiplication, whatever the fan width, so that a fan of
+// any width takes exactly the steps sequential backtracking would.
+__device__ void trial_w(const SolveState& st, int K, double mu, SlotState* sl);
+__device__ void make_round(const SolveState& st, int K, const CallOpts& o, SlotState* slots_b) {
+    double mu = st.mu;
+    for (int cnd = 0; cnd < o.C; ++cnd) {
+        if (st.t + cnd < o.max_backtracks) trial_w(st, K, mu, &slots_b[cnd]);
+        else slots_b[cnd].active = 0;
+        mu *= o.armijo_beta;
+    }
+}
+
 __device__ void trial_w(const SolveState& st, int K, double mu, SlotState* sl) {
     for (int k = 0; k < K; ++k) sl->w[k] = (float)(st.w[k] - mu * st.g[k]);   // Eq. (3), candidate
     sl->mu = mu;
@@ -227,12 +241,7 @@ k_ctl_grad(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_trial, int use_
         st.mu = n == 0 ? o.init_step_vox * o.hmin_sqrtV / gn : 2.0 * st.mu_prev;         // reading A7
         st.t = 0;
         st.trialing = 1;
-        if (o.batched) {
-            for (int cnd = 0; cnd < o.max_backtracks; ++cnd)
-                trial_w(st, K, st.mu * pow(o.armijo_beta, (double)cnd), &c.slots[b * o.C + cnd]);
-        } else {
-            trial_w(st, K, st.mu, &c.slots[b * o.C]);
-        }
+        make_round(st, K, o, &c.slots[b * o.C]);
         any_trial = 1;
         any_running = 1;
         c.solves[b] = st;
@@ -259,38 +268,30 @@ __device__ void ctl_trial_body(const Geom& G, const CtlBufs& c, cudaGraphConditi
         int acc = -1;
         double acc_mu = 0.0, acc_Sp = 0.0, acc_Syp = 0.0;
         bool failed = false;
-        if (o.batched) {
-            // candidates mu beta^c, c = 0..max_backtracks-1, all evaluated: the largest passing
-            // step is the one sequential backtracking would have accepted
-            for (int cnd = 0; cnd < o.max_backtracks; ++cnd) {
-                const int s = b * o.C + cnd;
-                const Sums3 sp = sum_proj(c.proj_part, c.proj_blocks, s, red);
-                if (threadIdx.x != 0) continue;
-                const double mu_s = c.slots[s].mu;
-                c.slots[s].Sp = sp.a; c.slots[s].Syp = sp.b; c.slots[s].J = sp.c;
-                if (acc < 0 && sp.c <= st.Jn - o.armijo_c * mu_s * st.g2) {
-                    acc = s; st.t = cnd; acc_mu = mu_s; acc_Sp = sp.a; acc_Syp = sp.b;
-                }
-                c.slots[s].active = 0;
-            }
-            if (threadIdx.x != 0) continue;
-            if (acc < 0) { failed = true; st.t = o.max_backtracks; }
-        } else {
-            const int s = b * o.C;
+        // the round's candidates st.t .. st.t + C - 1 have been evaluated: the first that passes is
+        // the one sequential backtracking would have accepted (reading A7)
+        int n_cand = o.max_backtracks - st.t;
+        if (n_cand > o.C) n_cand = o.C;
+        double mu_last = st.mu;
+        for (int cnd = 0; cnd < n_cand; ++cnd) {
+            const int s = b * o.C + cnd;
             const Sums3 sp = sum_proj(c.proj_part, c.proj_blocks, s, red);
             if (threadIdx.x != 0) continue;
-            SlotState sl = c.slots[s];
-            sl.Sp = sp.a; sl.Syp = sp.b; sl.J = sp.c;
-            if (sp.c <= st.Jn - o.armijo_c * st.mu * st.g2) {                             // Armijo (L95)
-                acc = s; acc_mu = sl.mu; acc_Sp = sp.a; acc_Syp = sp.b;
-            } else {
-                st.mu *= o.armijo_beta;
-                st.t += 1;
-                if (st.t >= o.max_backtracks) failed = true;
-                else trial_w(st, K, st.mu, &sl);
+            const double mu_s = c.slots[s].mu;
+            c.slots[s].Sp = sp.a; c.slots[s].Syp = sp.b; c.slots[s].J = sp.c;
+            if (acc < 0 && sp.c <= st.Jn - o.armijo_c * mu_s * st.g2) {                   // Armijo (L95)
+                acc = s; acc_mu = mu_s; acc_Sp = sp.a; acc_Syp = sp.b;
+                st.t += cnd;
             }
-            if (acc >= 0 || failed) sl.active = 0;
-            c.slots[s] = sl;
+            c.slots[s].active = 0;
+            mu_last = mu_s;
+        }
+        if (threadIdx.x != 0) continue;
+        if (acc < 0) {
+            st.t += n_cand;
+            st.mu = mu_last * o.armijo_beta;
+            if (st.t >= o.max_backtracks) failed = true;
+            else make_round(st, K, o, &c.slots[b * o.C]);
         }
         if (acc >= 0) {
             const double mu = acc_mu;

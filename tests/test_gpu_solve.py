@@ -125,6 +125,20 @@ def test_batched_linesearch_equals_sequential():
     _compare_with_oracle(g, f0, xbar, u, y, theta, np.zeros(g.K), lm, r2, pc.Opts(max_iter=8, batched_linesearch=1))
 
 
+@pytest.mark.parametrize("fan", [2, 3])
+def test_partial_fan_takes_the_steps_of_sequential_backtracking(fan):
+    """pcamm_opts.batched_linesearch = F >= 2: F candidates per pass, the next F if none passes; the
+    accepted steps are those of sequential backtracking (reading A7), bit for bit."""
+    import paper_1004_0014_b200 as pc
+    g, f0, xbar, u, scale, theta, y, w_star, lm, m = _problem(seed=5, C=3)
+    yd = to_dev(y)
+    r1 = m.reconstruct(yd, theta, np.zeros(g.K), pc.Opts(max_iter=8, init_step_vox=6.0), trace=True)
+    r2 = m.reconstruct(yd, theta, np.zeros(g.K), pc.Opts(max_iter=8, init_step_vox=6.0, batched_linesearch=fan), trace=True)
+    assert r1.backtracks.max() >= 2                      # the runs do backtrack past one fan
+    assert np.array_equal(r1.backtracks, r2.backtracks) and np.array_equal(r1.mu_trace, r2.mu_trace)
+    assert np.array_equal(r1.w, r2.w) and r1.J == r2.J
+
+
 def test_batch_of_solves_equals_single_solves():
     import paper_1004_0014_b200 as pc
     B = 5

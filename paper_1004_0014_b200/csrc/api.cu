@@ -84,6 +84,7 @@ struct pcamm_model {
     FieldStream fs;
     // scratch (device)
     unsigned char* cellmap = nullptr;   // FieldStream::cellmap
+    unsigned char* occ = nullptr;       // occupancy of the trial volumes [S][OCC] (common.cuh)
     float *vol = nullptr, *pseg = nullptr, *p = nullptr, *rL = nullptr;   // vol: trial volumes, ray layout [S][PV]
     ColHdr* col_hdr = nullptr;      // [B][nu]
     SlabEntry* slab_tab = nullptr;  // [B][nu][max_slabs]
@@ -201,8 +202,8 @@ void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     launch_ysums(q, G, m->c, B);
     launch_begin(q, G, m->c, 0);
     launch_view_tables(q, G, m->c.solves, B, m->col_hdr, m->slab_tab);
-    launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV);
-    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_INIT, h_iter, use_cond);
+    launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
+    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_INIT, h_iter, use_cond);
 }
 
 void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial, int use_cond) {
@@ -214,8 +215,8 @@ void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial,
 
 void seq_trial(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_trial, int use_cond) {
     const Geom& G = m->G;
-    launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV);
-    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_TRIAL, h_trial, use_cond);
+    launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
+    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_TRIAL, h_trial, use_cond);
 }
 
 void seq_tail(pcamm_model* m, Seq& q, int B) {
@@ -317,7 +318,7 @@ int solve_impl(pcamm_model* m, int B, const float* y_dev, const float* angles, c
     if (volumes_out) {
         Seq q;
         q.stream = st;
-        launch_warp(q, G, m->fs, m->f0, m->out_slots, B, 0, volumes_out, G.V);
+        launch_warp(q, G, m->fs, m->f0, m->out_slots, B, 0, volumes_out, G.V, nullptr);
         if ((rc = check_seq(q, "final warp"))) return rc;
     }
     CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState) * B, cudaMemcpyDeviceToHost, st));
@@ -448,6 +449,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     Geom& G = m->G;
     G.nx = g->nx; G.ny = g->ny; G.nz = g->nz; G.V = V;
     G.pnx = g->nx + 2; G.pny = g->ny + 2; G.PV = (long long)G.pnx * G.pny * g->nz;
+    G.occ_pitch = ((g->nz + 15) / 16 + 7) / 8 * 8;
+    G.OCC = (long long)G.pnx * G.pny * G.occ_pitch;
     G.hx = g->hx; G.hy = g->hy; G.hz = g->hz;
     G.ihx = 1.f / g->hx; G.ihy = 1.f / g->hy; G.ihz = 1.f / g->hz;
     G.cx = g->cx; G.cy = g->cy; G.cz = g->cz;
@@ -475,7 +478,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return r == cudaSuccess; };
     ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->cellmap, (size_t)(g->nx + 1) * (g->ny + 1) * (g->nz + 1))) && ok(dalloc(m, &m->fields, 3 * (size_t)V * (G.K + 1))) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
-        ok(dalloc(m, &m->vol, S * (size_t)G.PV)) && ok(dalloc(m, &m->col_hdr, B * G.nu)) &&
+        ok(dalloc(m, &m->vol, S * (size_t)G.PV)) && ok(dalloc(m, &m->occ, S * (size_t)G.OCC)) && ok(dalloc(m, &m->col_hdr, B * G.nu)) &&
         ok(dalloc(m, &m->slab_tab, B * G.nu * (size_t)max_slabs(G))) && ok(dalloc(m, &m->p, S * G.npix)) && ok(dalloc(m, &m->pseg, S * G.npix * (size_t)project_segments(G))) &&
         ok(dalloc(m, &m->rL, B * G.npix)) && ok(dalloc(m, &m->utab, B * G.nu)) && ok(dalloc(m, &m->vtab, B * G.nv)) &&
         ok(dalloc(m, &m->in_block, m->in_block_bytes)) && ok(dalloc(m, &m->c.solves, B)) &&
@@ -519,6 +522,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     if (m->M > 0)
         TRY_OR_FAIL(cudaMemcpyAsync(m->lm0, landmarks_mm_host, sizeof(float) * 3 * m->M, cudaMemcpyHostToDevice, st));
     TRY_OR_FAIL(cudaMemsetAsync(m->vol, 0, sizeof(float) * S * (size_t)G.PV, st));   // zero border, never written
+    TRY_OR_FAIL(cudaMemsetAsync(m->occ, 0, S * (size_t)G.OCC, st));                   // likewise
     TRY_OR_FAIL(cudaMemsetAsync(m->nonfinite, 0, sizeof(unsigned long long), st));
     TRY_OR_FAIL(cudaMemsetAsync(m->c.solves, 0, sizeof(SolveState) * B, st));
     TRY_OR_FAIL(cudaMemsetAsync(m->c.slots, 0, sizeof(SlotState) * S, st));
@@ -582,7 +586,7 @@ int pcamm_warp(pcamm_model* m, const float* w_host, float* volume_out_dev, void*
     Seq q;
     int rc = hook_begin(m, nullptr, 0.f, w_host, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
-    launch_warp(q, m->G, m->fs, m->f0, m->c.slots, 1, 0, volume_out_dev, m->G.V);
+    launch_warp(q, m->G, m->fs, m->f0, m->c.slots, 1, 0, volume_out_dev, m->G.V, nullptr);
     if ((rc = check_seq(q, "warp"))) return rc;
     CUDA_TRY(cudaStreamSynchronize(st));
     return PCAMM_OK;
@@ -595,8 +599,8 @@ int pcamm_project(pcamm_model* m, const float* volume_dev, float angle_rad, floa
     int rc = hook_begin(m, nullptr, angle_rad, nullptr, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
     launch_view_tables(q, m->G, m->c.solves, 1, m->col_hdr, m->slab_tab);
-    launch_to_ray_layout(q, m->G, volume_dev, m->vol);
-    launch_project(q, m->G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_NONE, 0, 0);
+    launch_to_ray_layout(q, m->G, volume_dev, m->vol, m->occ);
+    launch_project(q, m->G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0);
     if ((rc = check_seq(q, "project"))) return rc;
     CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * m->G.npix, cudaMemcpyDeviceToDevice, st));
     CUDA_TRY(cudaStreamSynchronize(st));
@@ -626,8 +630,8 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     if (rc) return rc;
     launch_ysums(q2, G, m->c, 1);
     launch_view_tables(q2, G, m->c.solves, 1, m->col_hdr, m->slab_tab);
-    launch_warp(q2, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV);
-    launch_project(q2, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_EVAL, 0, 0);
+    launch_warp(q2, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
+    launch_project(q2, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_EVAL, 0, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
     launch_grad(q2, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
     launch_ctl_eval_grad(q2, G, m->c);
@@ -702,9 +706,9 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
     CUDA_TRY(cudaEventRecord(m->ev0, st));
     for (int i = 0; i < reps; ++i) {
         if (which == 0)
-            launch_warp(q, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV);
+            launch_warp(q, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
         else if (which == 1)
-            launch_project(q, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->pseg, m->p, THEN_NONE, 0, 0);
+            launch_project(q, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0);
         else
             launch_grad(q, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
     }

@@ -22,6 +22,8 @@ struct Geom {
     long long V;
     int pnx, pny;             // in-plane size of a ray-layout volume: nx + 2, ny + 2 (zero border)
     long long PV;             // elements of one ray-layout volume: pnx * pny * nz
+    int occ_pitch;            // occupancy bytes per voxel column of the ray layout (one per 16 z, padded to 8)
+    long long OCC;            // occupancy bytes of one trial volume: pnx * pny * occ_pitch
     float hx, hy, hz;
     float ihx, ihy, ihz;      // 1 / h
     float cx, cy, cz;         // world position of the volume centre
@@ -43,6 +45,25 @@ struct View {
 // neighbouring z, i.e. one or two 128 B lines per load, whatever the gantry angle.
 __host__ __device__ __forceinline__ long long ray_layout_index(const Geom& G, int x, int y, int z) {
     return ((long long)(y + 1) * G.pnx + (x + 1)) * G.nz + z;
+}
+
+// Occupancy of a trial volume: one byte per voxel column (x, y) of the ray layout and range of 16
+// z, non-zero iff some voxel there is non-zero.  Written by whoever writes the volume (every
+// byte exactly once per pass; the border columns stay 0), read by the projector to skip the slabs
+// of a ray that lie in air: their contribution is an exact +0.
+__device__ __forceinline__ long long occ_index(const Geom& G, int x, int y, int zt16) {
+    return ((long long)(y + 1) * G.pnx + (x + 1)) * G.occ_pitch + zt16;
+}
+// A warp holding tz = 16 or 32 consecutive z (lane = z - z0, z0 a multiple of tz) of column (x, y):
+// records the one or two 16-ranges.
+__device__ __forceinline__ void occ_record(const Geom& G, unsigned char* __restrict__ occ, int x, int y, int z0,
+                                           int tz, bool nonzero) {
+    const unsigned bal = __ballot_sync(0xffffffffu, nonzero);
+    if ((threadIdx.x & 31) == 0 && x < G.nx) {
+        const int zt = z0 >> 4;
+        occ[occ_index(G, x, y, zt)] = (bal & 0xffffu) ? 1 : 0;
+        if (tz == 32 && z0 + 16 < G.nz) occ[occ_index(G, x, y, zt + 1)] = (bal >> 16) ? 1 : 0;
+    }
 }
 
 // Per view and detector column: the in-plane part of the slab traversal (project.cu).

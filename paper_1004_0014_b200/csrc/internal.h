@@ -76,8 +76,9 @@ struct Seq {
 // ---- a-1 (warp.cu)
 // f[s] = warp(f0, xbar + U w[s]) for every active slot; ray_layout: the z-fastest layout the
 // projector reads (slot stride G.PV), else the standard [z][y][x] (slot stride G.V).
+// occ: occupancy of the volumes written (ray layout only; common.cuh), else NULL
 void launch_warp(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
-                 int ray_layout, float* vol_out, long long slot_stride);
+                 int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ);
 
 // ---- a-2 (project.cu)
 int project_blocks(const Geom& G);
@@ -92,9 +93,10 @@ struct CtlBufs;
 // [nslots][segments][nu][nv] for the per-segment partial line integrals), the a-3 partial sums
 // {sum p, sum y p, sum (p - a y - b)^2}, and then the control step `then` (THEN_*, common.cuh).
 void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const ColHdr* hdr, const SlabEntry* tab,
-                    const float* vol, float* pseg, float* p, int then, cudaGraphConditionalHandle h, int use_cond);
+                    const float* vol, const unsigned char* occ, float* pseg, float* p, int then,
+                    cudaGraphConditionalHandle h, int use_cond);
 // hooks: standard layout -> ray layout; one ray of the view of solve 0
-void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray);
+void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray, unsigned char* occ);
 void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* tab, int iu, int iv, int cap,
                      int* ijk, float* len, int* n_out);
 

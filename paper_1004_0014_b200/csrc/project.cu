@@ -260,19 +260,50 @@ struct AccSink {
 __global__ void __launch_bounds__(NT)
 k_project(const Geom G, const SlotState* __restrict__ slots, const ColHdr* __restrict__ hdr,
           const SlabEntry* __restrict__ tab, int max_slabs, int n_seg, const float* __restrict__ vol,
-          float* __restrict__ pseg) {
+          const unsigned char* __restrict__ occ, float* __restrict__ pseg) {
     const int s = blockIdx.z / n_seg, seg = blockIdx.z % n_seg;
     if (!slots[s].active) return;
     const int b = slots[s].solve;
     const int iu = blockIdx.x * PW + (threadIdx.x >> 5);
     const int iv = blockIdx.y * 32 + (threadIdx.x & 31);
-    if (iu >= G.nu || iv >= G.nv) return;
+    if (iu >= G.nu) return;                                  // the whole warp
     const ColHdr h = hdr[(long long)b * G.nu + iu];
-    const int n0 = seg * SEG, n = min(h.n_slabs - n0, SEG);
+    int n0 = seg * SEG, n = min(h.n_slabs - n0, SEG);
+    const SlabEntry* row = tab + ((long long)b * G.nu + iu) * max_slabs + n0;
     float p = 0.f;
     if (n > 0) {
+        // Slabs in air add an exact +0: trim the segment to the span of slabs whose voxel columns
+        // hold something (occupancy written with the volume; the lanes share the column, so the
+        // test is split over them and the result is uniform over the warp).
+        {
+            const unsigned long long* ow = reinterpret_cast<const unsigned long long*>(occ + (long long)s * G.OCC);
+            const int words = G.occ_pitch >> 3, lane = threadIdx.x & 31;
+            unsigned long long span = 0ull;
+#pragma unroll
+            for (int part = 0; part < SEG / 32; ++part) {
+                const int sl = part * 32 + lane;
+                bool o = false;
+                if (sl < n) {
+                    const int off0 = __ldg(&row[sl].off0);
+                    const int c0 = off0 / G.nz, c1 = (off0 + h.dT) / G.nz;
+                    for (int wd = 0; wd < words; ++wd)
+                        o |= (__ldg(ow + (long long)c0 * words + wd) | __ldg(ow + (long long)c1 * words + wd)) != 0ull;
+                }
+                span |= (unsigned long long)__ballot_sync(0xffffffffu, o) << (32 * part);
+            }
+            if (span == 0ull) n = 0;
+            else {
+                const int first = (__ffsll((long long)span) - 1) & ~(U - 1);
+                const int last = 63 - __clzll((long long)span);
+                n = min(n, (last & ~(U - 1)) + U) - first;
+                n0 += first;
+                row += first;
+            }
+        }
+    }
+    if (iv >= G.nv) return;                                  // rows beyond the detector (after the warp-wide votes)
+    if (n > 0) {
         const RayZ r = make_ray_z(G, h, iv, n0, n);
-        const SlabEntry* row = tab + ((long long)b * G.nu + iu) * max_slabs + n0;
         const float* base = vol + (long long)s * G.PV;
         asm volatile("" : "+l"(base));       // one base pointer; 32-bit offsets in the loop
         float acc;
@@ -293,7 +324,7 @@ k_project(const Geom G, const SlotState* __restrict__ slots, const ColHdr* __res
 // Standard [z][y][x] -> ray layout (hook path only: the solve's volumes are written in the ray
 // layout by the warp kernel).  Tile: 32 x by 32 z at fixed y.
 __global__ void __launch_bounds__(256)
-k_to_ray_layout(const Geom G, const float* __restrict__ src, float* __restrict__ dst) {
+k_to_ray_layout(const Geom G, const float* __restrict__ src, float* __restrict__ dst, unsigned char* __restrict__ occ) {
     __shared__ float tile[32][33];
     const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
     const int x0 = blockIdx.x * 32, z0 = blockIdx.y * 32, y = blockIdx.z;
@@ -306,7 +337,10 @@ k_to_ray_layout(const Geom G, const float* __restrict__ src, float* __restrict__
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
         const int x = x0 + tw + 8 * r, z = z0 + lane;
-        if (x < G.nx && z < G.nz) dst[ray_layout_index(G, x, y, z)] = tile[lane][tw + 8 * r];
+        const bool st = x < G.nx && z < G.nz;
+        const float v = st ? tile[lane][tw + 8 * r] : 0.f;
+        if (st) dst[ray_layout_index(G, x, y, z)] = v;
+        occ_record(G, occ, x, y, z0, 32, v != 0.f);
     }
 }
 
@@ -364,15 +398,16 @@ void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, 
 }
 
 void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const ColHdr* hdr, const SlabEntry* tab,
-                    const float* vol, float* pseg, float* p, int then, cudaGraphConditionalHandle h, int use_cond) {
+                    const float* vol, const unsigned char* occ, float* pseg, float* p, int then,
+                    cudaGraphConditionalHandle h, int use_cond) {
     const int n_seg = project_segments(G);
     q.launch(k_project, dim3((G.nu + PW - 1) / PW, (G.nv + 31) / 32, nslots * n_seg), dim3(NT), 0, G,
-             (const SlotState*)c.slots, hdr, tab, max_slabs(G), n_seg, vol, pseg);
+             (const SlotState*)c.slots, hdr, tab, max_slabs(G), n_seg, vol, occ, pseg);
     launch_project_finish(q, G, c, nslots, n_seg, pseg, p, then, h, use_cond);
 }
 
-void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray) {
-    q.launch(k_to_ray_layout, dim3((G.nx + 31) / 32, (G.nz + 31) / 32, G.ny), dim3(256), 0, G, vol_std, vol_ray);
+void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray, unsigned char* occ) {
+    q.launch(k_to_ray_layout, dim3((G.nx + 31) / 32, (G.nz + 31) / 32, G.ny), dim3(256), 0, G, vol_std, vol_ray, occ);
 }
 
 void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* tab, int iu, int iv, int cap,

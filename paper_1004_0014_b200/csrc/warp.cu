@@ -47,7 +47,8 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ f0, int nx,
 template <int K, bool RAY>
 __global__ void __launch_bounds__(NTHREADS)
 k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restrict__ xbar, const float* __restrict__ u,
-       const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride) {
+       const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride,
+       unsigned char* __restrict__ occ) {
     __shared__ float tile[TILE][TILE + 1];
     const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
     const int x0 = blockIdx.x * TILE, z0 = blockIdx.y * TILE, y = blockIdx.z;
@@ -104,7 +105,10 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
 #pragma unroll
             for (int r = 0; r < ROWS; ++r) {
                 const int xo = x0 + tw + 8 * r;
-                if (xo < G.nx && zo < G.nz) out[ray_layout_index(G, xo, y, zo)] = tile[lane][tw + 8 * r];
+                const bool st = xo < G.nx && zo < G.nz;
+                const float v = st ? tile[lane][tw + 8 * r] : 0.f;
+                if (st) out[ray_layout_index(G, xo, y, zo)] = v;
+                occ_record(G, occ + (long long)s * G.OCC, xo, y, z0, 32, v != 0.f);
             }
         }
     }
@@ -127,11 +131,13 @@ constexpr size_t warp_smem_bytes() {
 template <int K, bool RAY>
 __global__ void __launch_bounds__(WTHREADS, 1)
 k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
-           const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride) {
+           const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride,
+           unsigned char* __restrict__ occ) {
     constexpr int P = 3 * (K + 1), WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
     using Ring = FieldRing<P, WTZ, WNG, WarpStages<K>::value>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ float tiles[WNG][WTZ][TX + 1];
+    __shared__ int s_occ[WNG][2][TX];                      // per group: column x has something in z block 0 / 1
     __shared__ float s_w[SLOT_CACHE][K];                   // the slots' coefficients (constant during the launch)
     __shared__ int s_active[SLOT_CACHE];
     for (int i = threadIdx.x; i < nslots && i < SLOT_CACHE; i += blockDim.x) {
@@ -204,9 +210,17 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                         if (x < G.nx && z < G.nz) out[((long long)z * G.ny + c.y) * G.nx + x] = val[r];
                     }
                 } else {
+                    // occupancy (common.cuh): is anything non-zero in column x, z block of 16?  Rows
+                    // zz = tw + 8 r: r = 0, 1 lie in the tile's first block, r = 2, 3 in its second.
+                    bool nzb[2] = {false, false};
+#pragma unroll
+                    for (int r = 0; r < WROWS; ++r) nzb[r >> 1] |= val[r] != 0.f && x < G.nx && c.z0 + tw + GROUP_WARPS * r < G.nz;
+                    if (tw < 2) s_occ[group][tw][lane] = 0;
                     group_barrier(group);
 #pragma unroll
                     for (int r = 0; r < WROWS; ++r) tile[tw + GROUP_WARPS * r][lane] = val[r];
+                    if (nzb[0]) s_occ[group][0][lane] = 1;
+                    if (nzb[1]) s_occ[group][1][lane] = 1;
                     group_barrier(group);
                     const int zo = c.z0 + lane;
 #pragma unroll
@@ -215,6 +229,8 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                         if (lane < WTZ && xo < G.nx && zo < G.nz)
                             out[ray_layout_index(G, xo, c.y, zo)] = tile[lane][tw + GROUP_WARPS * r];
                     }
+                    if (tw < WTZ / 16 && x < G.nx && c.z0 + 16 * tw < G.nz)
+                        occ[(long long)sl * G.OCC + occ_index(G, x, c.y, (c.z0 >> 4) + tw)] = (unsigned char)s_occ[group][tw][lane];
                 }
             }
         }
@@ -223,7 +239,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
 
 template <int K, bool RAY>
 void launch_tma(Seq& q, const Geom& G, const CUtensorMap& fmap, int n_sm, const float* f0, const SlotState* slots,
-                int nslots, float* vol_out, long long slot_stride) {
+                int nslots, float* vol_out, long long slot_stride, unsigned char* occ) {
     static bool configured = false;
     constexpr size_t smem = warp_smem_bytes<K>();
     if (!configured) {
@@ -236,32 +252,32 @@ void launch_tma(Seq& q, const Geom& G, const CUtensorMap& fmap, int n_sm, const 
     for (int s0 = 0; s0 < nslots; s0 += SLOT_CACHE) {      // the kernel keeps up to SLOT_CACHE slots' coefficients on chip
         const int ns = nslots - s0 < SLOT_CACHE ? nslots - s0 : SLOT_CACHE;
         q.launch(k_warp_tma<K, RAY>, dim3(grid), dim3(WTHREADS), smem, fmap, G, f0, slots + s0, ns,
-                 vol_out + (long long)s0 * slot_stride, slot_stride);
+                 vol_out + (long long)s0 * slot_stride, slot_stride, occ ? occ + (long long)s0 * G.OCC : occ);
     }
 }
 
 template <int K>
 void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
-              int ray_layout, float* vol_out, long long slot_stride) {
+              int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ) {
     if (fs.use_tma) {
-        if (ray_layout) launch_tma<K, true>(q, G, field_map<K>(fs), fs.n_sm, f0, slots, nslots, vol_out, slot_stride);
-        else launch_tma<K, false>(q, G, field_map<K>(fs), fs.n_sm, f0, slots, nslots, vol_out, slot_stride);
+        if (ray_layout) launch_tma<K, true>(q, G, field_map<K>(fs), fs.n_sm, f0, slots, nslots, vol_out, slot_stride, occ);
+        else launch_tma<K, false>(q, G, field_map<K>(fs), fs.n_sm, f0, slots, nslots, vol_out, slot_stride, occ);
         return;
     }
     const float* xbar = fs.fields;
     const float* u = fs.fields + 3 * G.V;
     dim3 grid((G.nx + TILE - 1) / TILE, (G.nz + TILE - 1) / TILE, G.ny);
-    if (ray_layout) q.launch(k_warp_generic<K, true>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride);
-    else q.launch(k_warp_generic<K, false>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride);
+    if (ray_layout) q.launch(k_warp_generic<K, true>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride, occ);
+    else q.launch(k_warp_generic<K, false>, grid, dim3(NTHREADS), 0, G, f0, xbar, u, slots, nslots, vol_out, slot_stride, occ);
 }
 
 }  // namespace
 
 void launch_warp(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
-                 int ray_layout, float* vol_out, long long slot_stride) {
+                 int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ) {
     switch (G.K) {
 #define PCAMM_CASE(KK) \
-    case KK: launch_k<KK>(q, G, fs, f0, slots, nslots, ray_layout, vol_out, slot_stride); break;
+    case KK: launch_k<KK>(q, G, fs, f0, slots, nslots, ray_layout, vol_out, slot_stride, occ); break;
         PCAMM_CASE(1) PCAMM_CASE(2) PCAMM_CASE(3) PCAMM_CASE(4)
         PCAMM_CASE(5) PCAMM_CASE(6) PCAMM_CASE(7) PCAMM_CASE(8)
 #undef PCAMM_CASE

@@ -119,6 +119,34 @@ def test_projection_matches_oracle(theta):
     assert np.max(np.abs(out - ref)) <= 2e-5 * ref.max()
 
 
+@pytest.mark.parametrize("theta", [0.0, 0.4, np.pi / 4, 1.2, np.pi / 2, 2.8, 4.1])
+def test_projection_skips_air_exactly(theta):
+    """The projector trims every 64-slab segment of a ray to the slabs whose voxel columns hold
+    something non-zero (occupancy bytes written with the volume).  Volumes that are mostly air
+    (an off-centre ellipsoid, a thin slab, a single voxel, nothing at all) long enough for several
+    segments, both through pcamm_project (occupancy from the layout kernel) and through pcamm_eval
+    (occupancy from the warp kernel)."""
+    g = geom(nx=150, ny=140, nz=40, h=(2.0, 2.0, 2.0), K=2, nu=90, nv=36, pitch=(3.6, 3.1), centre=(0.7, 0.2, 0.5))
+    rng = np.random.default_rng(5)
+    zz, yy, xx = np.meshgrid(np.arange(g.nz), np.arange(g.ny), np.arange(g.nx), indexing="ij")
+    blob = ((xx - 95) / 30.0) ** 2 + ((yy - 50) / 22.0) ** 2 + ((zz - 17) / 11.0) ** 2 <= 1.0
+    slab = (np.abs(yy - 100) <= 1) & (zz >= 33)
+    dot = (xx == 3) & (yy == 137) & (zz == 0)
+    f0, xbar, u, scale, m = _model(g, seed=31, disp_vox=1.5)
+    for mask in (blob, blob | slab | dot, dot, np.zeros_like(blob)):
+        f = (rng.random(g.vshape) * mask).astype(np.float32)
+        ref = oracle.project(g, f, theta)
+        out = to_host(m.project(to_dev(f), theta))
+        assert np.max(np.abs(out - ref)) <= 2e-5 * max(ref.max(), 1e-3)
+        assert np.array_equal(out == 0, ref == 0) or np.max(np.abs(ref[out == 0])) <= 1e-6
+    # the same through the warp kernel: the reference image is the masked volume
+    m2 = make_model(g, (f0 * (blob | slab)).astype(np.float32), xbar, u)
+    w = (0.6 * scale * np.array([1.0, -0.7])).astype(np.float32)
+    _, p_ref = oracle.evaluate(g, (f0 * (blob | slab)).astype(np.float32), xbar, u, w, theta)
+    _, _, _, p = m2.eval(to_dev(p_ref.astype(np.float32)), theta, w, 1.0, 0.0)
+    assert rel_l2(to_host(p), p_ref) <= 1e-5
+
+
 @pytest.mark.parametrize("aniso", [((2.0, 3.0, 2.5), (2.5, 2.0)), ((3.0, 2.0, 4.0), (2.0, 3.0))])
 def test_projection_anisotropic_voxels_and_offsets(aniso):
     h, pitch = aniso

@@ -484,7 +484,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         ok(dalloc(m, &m->in_block, m->in_block_bytes)) && ok(dalloc(m, &m->c.solves, B)) &&
         ok(dalloc(m, &m->c.traces, B)) && ok(dalloc(m, &m->c.slots, S)) && ok(dalloc(m, &m->c.flags, 1)) &&
         ok(dalloc(m, &m->c.ysum_part, B * m->c.ysum_blocks * 2)) &&
-        ok(dalloc(m, &m->c.proj_part, S * m->c.proj_blocks * 3)) &&
+        ok(dalloc(m, &m->c.proj_part, S * m->c.proj_blocks * 3)) && ok(dalloc(m, &m->c.seg_ticket, S * m->c.proj_blocks)) &&
         ok(dalloc(m, &m->c.resid_part, B * m->c.resid_blocks)) &&
         ok(dalloc(m, &m->c.grad_part, B * m->c.grad_blocks * KMAX)) && ok(dalloc(m, &m->out_slots, B)) &&
         ok(dalloc(m, &m->lm_out, 3 * B * (size_t)(m->M > 0 ? m->M : 1))) &&
@@ -527,6 +527,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     TRY_OR_FAIL(cudaMemsetAsync(m->c.solves, 0, sizeof(SolveState) * B, st));
     TRY_OR_FAIL(cudaMemsetAsync(m->c.slots, 0, sizeof(SlotState) * S, st));
     TRY_OR_FAIL(cudaMemsetAsync(m->c.flags, 0, sizeof(LoopFlags), st));
+    TRY_OR_FAIL(cudaMemsetAsync(m->c.seg_ticket, 0, sizeof(int) * S * m->c.proj_blocks, st));
     k_count_nonfinite<<<592, 256, 0, st>>>(m->f0, V, m->nonfinite);
     k_count_nonfinite<<<592, 256, 0, st>>>(m->xbar, 3 * V, m->nonfinite);
     k_count_nonfinite<<<592, 256, 0, st>>>(m->u, 3 * V * G.K, m->nonfinite);

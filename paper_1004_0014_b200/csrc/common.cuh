@@ -124,11 +124,11 @@ struct SlotState {
 struct LoopFlags {
     int iter_cond, trial_cond;
     long long n_launch;
-    unsigned ticket;          // blocks of k_project_finish that are done (the last one runs the control step)
+    unsigned ticket;          // unused
     unsigned pad;
 };
 
-// Control step run by the last block of k_project_finish.
+// Control step that follows a projection (k_ctl_after_project).
 constexpr int THEN_NONE = 0, THEN_INIT = 1, THEN_TRIAL = 2, THEN_EVAL = 3;
 
 // In-plane direction D - S of the rays of detector column iu (independent of the row).

@@ -378,66 +378,9 @@ __device__ void ctl_eval_body(const Geom& G, const CtlBufs& c, int stage) {
 __global__ void __launch_bounds__(CT)
 k_ctl_eval_grad(const Geom G, CtlBufs c) { ctl_eval_body(G, c, 1); }
 
-// a-2 (end) and a-3: p = sum of the projector's segments in index order, r_i = p_i - a y_i - b and
-// the per-block partial sums of p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.
-// Tile of 32 detector columns x 32 rows: the partial images are column-major (rows contiguous,
-// as the projector's warps write them), p and y are row-major.
-// The block that finishes last (ticket) then runs the control step that follows this projection
-// (then = THEN_INIT / THEN_TRIAL / THEN_EVAL), which saves a single-block launch per trial.
+// The control step that follows a projection (then = THEN_INIT / THEN_TRIAL / THEN_EVAL): one block.
 __global__ void __launch_bounds__(CT)
-k_project_finish(const Geom G, CtlBufs c, int n_seg, const float* __restrict__ pseg, float* __restrict__ p_out, int then,
-                 cudaGraphConditionalHandle h, int use_cond) {
-    __shared__ float tile[32][33];
-    __shared__ double red[CT / 32];
-    __shared__ int s_last;
-    const int s = blockIdx.z;
-    const int nblk = gridDim.x * gridDim.y;
-    if (c.slots[s].active) {                                             // uniform over the block
-        const int b = c.slots[s].solve;
-        const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
-        const int u0 = blockIdx.x * 32, v0 = blockIdx.y * 32;
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int iu = u0 + tw + 8 * r, iv = v0 + lane;
-            float acc = 0.f;
-            if (iu < G.nu && iv < G.nv)
-                for (int g = 0; g < n_seg; ++g) acc += __ldcg(pseg + (((long long)s * n_seg + g) * G.nu + iu) * G.nv + iv);
-            tile[tw + 8 * r][lane] = acc;
-        }
-        __syncthreads();
-        double vp = 0.0, vyp = 0.0, vrr = 0.0;
-        const float* y = c.in[b].y;
-        const double a = c.solves[b].a, bb = c.solves[b].b;
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int iv = v0 + tw + 8 * r, iu = u0 + lane;
-            if (iu < G.nu && iv < G.nv) {
-                const float p = tile[lane][tw + 8 * r];
-                const int pix = iv * G.nu + iu;
-                p_out[(long long)s * G.npix + pix] = p;
-                const double yv = y ? (double)__ldg(y + pix) : 0.0;
-                const double res = (double)p - a * yv - bb;               // Eq. (2) residual
-                vp += (double)p; vyp += yv * (double)p; vrr += res * res;
-            }
-        }
-        const int blk = blockIdx.y * gridDim.x + blockIdx.x;
-        double* out = c.proj_part + ((long long)s * nblk + blk) * 3;
-        const double sp = block_sum<CT>(vp, red);
-        const double syp = block_sum<CT>(vyp, red);
-        const double srr = block_sum<CT>(vrr, red);
-        if (threadIdx.x == 0) { out[0] = sp; out[1] = syp; out[2] = srr; }
-    }
-    if (then == THEN_NONE) return;
-    if (threadIdx.x == 0) {
-        __threadfence();                                                  // this block's partial sums are visible
-        const unsigned total = (unsigned)nblk * gridDim.z;
-        const unsigned t = atomicAdd(&c.flags->ticket, 1u);
-        s_last = t == total - 1u;
-        if (s_last) c.flags->ticket = 0u;
-    }
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
+k_ctl_after_project(const Geom G, CtlBufs c, int then, cudaGraphConditionalHandle h, int use_cond) {
     if (then == THEN_INIT) ctl_init_body(G, c, h, use_cond);
     else if (then == THEN_TRIAL) ctl_trial_body(G, c, h, use_cond);
     else ctl_eval_body(G, c, 0);
@@ -532,10 +475,10 @@ void launch_ctl_eval_grad(Seq& q, const Geom& G, const CtlBufs& c) {
     q.launch(k_ctl_eval_grad, dim3(1), dim3(CT), 0, G, c);
 }
 
-void launch_project_finish(Seq& q, const Geom& G, const CtlBufs& c, int nslots, int n_seg, const float* pseg, float* p,
-                           int then, cudaGraphConditionalHandle h, int use_cond) {
-    q.launch(k_project_finish, dim3((G.nu + 31) / 32, (G.nv + 31) / 32, nslots), dim3(CT), 0, G, c, n_seg, pseg, p, then, h,
-             use_cond);
+void launch_ctl_after_project(Seq& q, const Geom& G, const CtlBufs& c, int then, cudaGraphConditionalHandle h,
+                              int use_cond) {
+    if (then == THEN_NONE) return;
+    q.launch(k_ctl_after_project, dim3(1), dim3(CT), 0, G, c, then, h, use_cond);
 }
 
 void launch_invert(Seq& q, const Geom& G, const float* xbar, const float* u, const CtlBufs& c, int B, int M,

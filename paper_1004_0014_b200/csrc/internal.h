@@ -124,6 +124,7 @@ struct CtlBufs {
     SolveTrace* traces;
     SlotState* slots;
     LoopFlags* flags;
+    int* seg_ticket;     // [S][proj_blocks]: segment blocks of a ray group that are done (self-resetting)
     double* ysum_part;   // [B][ysum_blocks][2]
     double* proj_part;   // [S][project_blocks][3]
     double* resid_part;  // [B][resid_blocks]
@@ -138,8 +139,8 @@ void launch_ctl_grad(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphCondition
 void launch_ctl_iter_end(Seq& q, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond);
 void launch_ctl_final(Seq& q, const Geom& G, const CtlBufs& c, SlotState* out_slots);
 void launch_ctl_eval_grad(Seq& q, const Geom& G, const CtlBufs& c);
-void launch_project_finish(Seq& q, const Geom& G, const CtlBufs& c, int nslots, int n_seg, const float* pseg, float* p,
-                           int then, cudaGraphConditionalHandle h, int use_cond);
+void launch_ctl_after_project(Seq& q, const Geom& G, const CtlBufs& c, int then, cudaGraphConditionalHandle h,
+                              int use_cond);
 // a-6: landmarks [B][M][3]
 void launch_invert(Seq& q, const Geom& G, const float* xbar, const float* u, const CtlBufs& c, int B, int M,
                    const float* r0, double* r_out);

@@ -27,7 +27,7 @@
 // L2/L1-resident: this kernel is bound by instruction issue, not by HBM.
 //
 // The rays are cut into segments of SEG slabs (one block per segment of 4 columns x 32 rows);
-// k_project_finish (control.cu) adds the segments and forms the a-3 sums.
+// the block of a ray group that finishes last adds the segments and forms the a-3 sums.
 #include "internal.h"
 
 namespace pcamm {
@@ -256,20 +256,25 @@ struct AccSink {
 // (with one block per ray group everything is resident at once and the last third of the
 // kernel runs half empty: profiles/r01).  Segment s of a ray starts from the exact z state at
 // its first slab (double precision set-up) and writes its partial line integral to
-// pseg[slot][s][iu][iv]; k_project_finish (control.cu) adds the segments in index order.
+// pseg[slot][s][iu][iv]; the last block of the ray group adds the segments in index order.
 __global__ void __launch_bounds__(NT)
-k_project(const Geom G, const SlotState* __restrict__ slots, const ColHdr* __restrict__ hdr,
-          const SlabEntry* __restrict__ tab, int max_slabs, int n_seg, const float* __restrict__ vol,
-          const unsigned char* __restrict__ occ, float* __restrict__ pseg) {
+k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* __restrict__ solves,
+          const SolveIn* __restrict__ in, const ColHdr* __restrict__ hdr, const SlabEntry* __restrict__ tab,
+          int max_slabs, int n_seg, const float* __restrict__ vol, const unsigned char* __restrict__ occ,
+          float* pseg, float* __restrict__ p_out, double* __restrict__ partials, int* seg_ticket) {
+    __shared__ double red[NT / 32];
+    __shared__ int s_last;
     const int s = blockIdx.z / n_seg, seg = blockIdx.z % n_seg;
-    if (!slots[s].active) return;
+    if (!slots[s].active) return;                            // uniform over the block
     const int b = slots[s].solve;
     const int iu = blockIdx.x * PW + (threadIdx.x >> 5);
     const int iv = blockIdx.y * 32 + (threadIdx.x & 31);
-    if (iu >= G.nu) return;                                  // the whole warp
-    const ColHdr h = hdr[(long long)b * G.nu + iu];
+    const bool col_ok = iu < G.nu, ray_ok = col_ok && iv < G.nv;
+    ColHdr h;
+    h.n_slabs = 0; h.dT = 0; h.lam0 = 0.0; h.kap = 0.0; h.dxy2 = 0.f; h.axis = 0;
+    if (col_ok) h = hdr[(long long)b * G.nu + iu];
     int n0 = seg * SEG, n = min(h.n_slabs - n0, SEG);
-    const SlabEntry* row = tab + ((long long)b * G.nu + iu) * max_slabs + n0;
+    const SlabEntry* row = tab + ((long long)b * G.nu + (col_ok ? iu : 0)) * max_slabs + n0;
     float p = 0.f;
     if (n > 0) {
         // Slabs in air add an exact +0: trim the segment to the span of slabs whose voxel columns
@@ -301,8 +306,7 @@ k_project(const Geom G, const SlotState* __restrict__ slots, const ColHdr* __res
             }
         }
     }
-    if (iv >= G.nv) return;                                  // rows beyond the detector (after the warp-wide votes)
-    if (n > 0) {
+    if (ray_ok && n > 0) {
         const RayZ r = make_ray_z(G, h, iv, n0, n);
         const float* base = vol + (long long)s * G.PV;
         asm volatile("" : "+l"(base));       // one base pointer; 32-bit offsets in the loop
@@ -318,7 +322,45 @@ k_project(const Geom G, const SlotState* __restrict__ slots, const ColHdr* __res
         }
         p = acc * (r.Ls * 2.3283064365386963e-10f);      // the shares were summed in units of 2^-32
     }
-    pseg[(((long long)s * n_seg + seg) * G.nu + iu) * G.nv + iv] = p;
+    float* my_seg = pseg + (((long long)s * n_seg + seg) * G.nu + (col_ok ? iu : 0)) * G.nv + (ray_ok ? iv : 0);
+    if (ray_ok && n_seg > 1) *my_seg = p;
+
+    // The block of this ray group (PW columns x 32 rows) that finishes last adds the segments in
+    // index order and forms a-3 for its rays: r_i = p_i - a y_i - b with the per-group partial sums
+    // of p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.
+    const int ngroups = gridDim.x * gridDim.y, grp = blockIdx.y * gridDim.x + blockIdx.x;
+    if (n_seg > 1) {
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int* t = seg_ticket + (long long)s * ngroups + grp;
+            const int k = atomicAdd(t, 1);
+            s_last = k == n_seg - 1;
+            if (s_last) *t = 0;
+        }
+        __syncthreads();
+        if (!s_last) return;
+        __threadfence();
+        if (ray_ok) {
+            p = 0.f;
+            for (int g = 0; g < n_seg; ++g)
+                p += __ldcg(pseg + (((long long)s * n_seg + g) * G.nu + iu) * G.nv + iv);
+        }
+    }
+    double vp = 0.0, vyp = 0.0, vrr = 0.0;
+    if (ray_ok) {
+        const int pix = iv * G.nu + iu;
+        p_out[(long long)s * G.npix + pix] = p;
+        const float* y = in[b].y;
+        const double yv = y ? (double)__ldg(y + pix) : 0.0;
+        const double res = (double)p - solves[b].a * yv - solves[b].b;   // Eq. (2) residual
+        vp = (double)p; vyp = yv * (double)p; vrr = res * res;
+    }
+    double* out = partials + ((long long)s * ngroups + grp) * 3;
+    const double sp = block_sum<NT>(vp, red);
+    const double syp = block_sum<NT>(vyp, red);
+    const double srr = block_sum<NT>(vrr, red);
+    if (threadIdx.x == 0) { out[0] = sp; out[1] = syp; out[2] = srr; }
 }
 
 // Standard [z][y][x] -> ray layout (hook path only: the solve's volumes are written in the ray
@@ -388,7 +430,7 @@ __global__ void k_traverse(const Geom G, const ColHdr* __restrict__ hdr, const S
 
 }  // namespace
 
-int project_blocks(const Geom& G) { return ((G.nu + 31) / 32) * ((G.nv + 31) / 32); }
+int project_blocks(const Geom& G) { return ((G.nu + PW - 1) / PW) * ((G.nv + 31) / 32); }
 // slabs per table row: the longest march, rounded up to the group size, plus one group read ahead
 int max_slabs(const Geom& G) { return ((G.nx > G.ny ? G.nx : G.ny) + U - 1) / U * U + U; }
 int project_segments(const Geom& G) { return ((G.nx > G.ny ? G.nx : G.ny) + SEG - 1) / SEG; }
@@ -402,8 +444,9 @@ void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const C
                     cudaGraphConditionalHandle h, int use_cond) {
     const int n_seg = project_segments(G);
     q.launch(k_project, dim3((G.nu + PW - 1) / PW, (G.nv + 31) / 32, nslots * n_seg), dim3(NT), 0, G,
-             (const SlotState*)c.slots, hdr, tab, max_slabs(G), n_seg, vol, occ, pseg);
-    launch_project_finish(q, G, c, nslots, n_seg, pseg, p, then, h, use_cond);
+             (const SlotState*)c.slots, (const SolveState*)c.solves, (const SolveIn*)c.in, hdr, tab, max_slabs(G), n_seg, vol,
+             occ, pseg, p, c.proj_part, c.seg_ticket);
+    launch_ctl_after_project(q, G, c, then, h, use_cond);
 }
 
 void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray, unsigned char* occ) {

@@ -136,3 +136,16 @@ def test_noise_models():
     assert np.array_equal(g, add_noise(y, "gaussian", 0))
     p = add_noise(y, "poisson", 0)
     assert np.all(np.isfinite(p)) and abs(np.mean(p[:, :10] - y[:, :10])) < 0.01
+
+
+def test_bench_ray_slab_count_matches_the_geometry():
+    """bench.py's count of (ray, slab) pairs (the projector's ALU roofline numerator): along an axis
+    every column marches all layers; at 45 degrees the diagonal of the square field of view."""
+    import bench
+    cfg = get_config("C2")
+    assert bench.ray_slab_count(cfg, 0.0) == cfg.nu * cfg.nv * cfg.nx
+    assert bench.ray_slab_count(cfg, np.pi / 2) == cfg.nu * cfg.nv * cfg.ny
+    n45 = bench.ray_slab_count(cfg, np.pi / 4)
+    assert 0.6 * cfg.nu * cfg.nv * cfg.nx < n45 < cfg.nu * cfg.nv * cfg.nx
+    ab = bench.algorithmic_bytes(cfg)
+    assert ab["warp"] == 56 * cfg.V and ab["gradient"] == 52 * cfg.V + 4 * cfg.npix     # SURVEY 8(a), K = 3

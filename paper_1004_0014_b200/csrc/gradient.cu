@@ -110,17 +110,34 @@ __device__ __forceinline__ float gather_voxel(const Geom& G, const GatherView& g
     const int iv0 = max(0, (int)ceilf(vlo - 0.01f)), iv1 = min(G.nv - 1, (int)floorf(vhi + 0.01f));
     const float xl = ex - 0.5f * G.hx, xh = ex + 0.5f * G.hx, yl = ey - 0.5f * G.hy, yh = ey + 0.5f * G.hy;
     float acc = 0.f;
-    for (int iu = iu0; iu <= iu1; ++iu) {
-        const float4 ud = __ldg(utab + iu);
-        const float ax0 = xl * ud.z, ax1 = xh * ud.z, ay0 = yl * ud.w, ay1 = yh * ud.w;
-        const float lo_u = fmaxf(fminf(ax0, ax1), fminf(ay0, ay1));
-        const float hi_u = fminf(fmaxf(ax0, ax1), fmaxf(ay0, ay1));
-        if (!(hi_u > lo_u)) continue;
-        for (int iv = iv0; iv <= iv1; ++iv) {
+    // rows in chunks of NVB (usually one chunk): their z intervals once, then per column the NVB
+    // residual loads are issued together (the gather is a latency chain otherwise)
+    constexpr int NVB = 4;
+    for (int ivb = iv0; ivb <= iv1; ivb += NVB) {
+        float lo_z[NVB], hi_z[NVB];
+#pragma unroll
+        for (int bb = 0; bb < NVB; ++bb) {
+            const int iv = min(ivb + bb, iv1);
             const float2 vd = __ldg(vtab + iv);
             const float az0 = zl * vd.y, az1 = zh * vd.y;
-            const float lo = fmaxf(lo_u, fminf(az0, az1)), hi = fminf(hi_u, fmaxf(az0, az1));
-            acc = fmaf(fmaxf(hi - lo, 0.f), __ldg(rL + iv * G.nu + iu), acc);
+            const bool on = ivb + bb <= iv1;
+            lo_z[bb] = on ? fminf(az0, az1) : 1.f;                 // an empty interval for rows beyond iv1
+            hi_z[bb] = on ? fmaxf(az0, az1) : -1.f;
+        }
+#pragma unroll 2
+        for (int iu = iu0; iu <= iu1; ++iu) {
+            const float4 ud = __ldg(utab + iu);
+            const float ax0 = xl * ud.z, ax1 = xh * ud.z, ay0 = yl * ud.w, ay1 = yh * ud.w;
+            const float lo_u = fmaxf(fminf(ax0, ax1), fminf(ay0, ay1));
+            const float hi_u = fminf(fmaxf(ax0, ax1), fmaxf(ay0, ay1));
+            float rv[NVB];
+#pragma unroll
+            for (int bb = 0; bb < NVB; ++bb) rv[bb] = __ldg(rL + min(ivb + bb, iv1) * G.nu + iu);
+#pragma unroll
+            for (int bb = 0; bb < NVB; ++bb) {
+                const float lo = fmaxf(lo_u, lo_z[bb]), hi = fminf(hi_u, hi_z[bb]);
+                acc = fmaf(fmaxf(hi - lo, 0.f), rv[bb], acc);
+            }
         }
     }
     return acc;

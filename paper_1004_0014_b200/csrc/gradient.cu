@@ -348,30 +348,40 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
 #pragma unroll
                     for (int k = 0; k < K; ++k) acc[k] = 0.f;
                 }
-#pragma unroll 1
+                // 0. light pass over all the thread's voxels of the tile: the displacement (Eq. 1) and
+                //    one byte of the cell map each, the loads of all of them in flight together.
+                float dda[GROWS][3];
+                unsigned char flaga[GROWS];
+#pragma unroll
+                for (int ra = 0; ra < GROWS; ++ra) {
+                    const int zz = tw * GROWS + ra;
+#pragma unroll
+                    for (int cc = 0; cc < 3; ++cc) {
+                        float xs = lds_f32(sf + 4u * ((cc * GTZ + zz) * TX + lane));               // Eq. (1)
+#pragma unroll
+                        for (int k = 0; k < K; ++k)
+                            xs = fmaf(lds_f32(sf + 4u * (((3 + 3 * k + cc) * GTZ + zz) * TX + lane)), w[k], xs);
+                        dda[ra][cc] = xs;
+                    }
+                    const int ci = x + (int)floorf(dda[ra][0]) + 1, cj = c.y + (int)floorf(dda[ra][1]) + 1,
+                              ck = c.z0 + zz + (int)floorf(dda[ra][2]) + 1;
+                    const bool inside = x < G.nx && c.z0 + zz < G.nz && (unsigned)ci <= (unsigned)G.nx &&
+                                        (unsigned)cj <= (unsigned)G.ny && (unsigned)ck <= (unsigned)G.nz;
+                    flaga[ra] = inside ? __ldg(cellmap + ((long long)ck * (G.ny + 1) + cj) * (G.nx + 1) + ci) : (unsigned char)0;
+                }
+#pragma unroll
                 for (int bt = 0; bt < NB; ++bt) {
-                    // 1. G_j and q_kj.  A voxel whose interpolation cell of f0 is constant (cell map,
-                    //    one byte) has G_j = 0 exactly: a warp none of whose voxels of this batch needs
-                    //    more skips the taps, the gathers and the derivative (most of the volume: air,
-                    //    the inside of a homogeneous organ).
+                    // 1. G_j and q_kj.  A voxel whose interpolation cell of f0 is constant (cell map)
+                    //    has G_j = 0 exactly: a warp none of whose voxels of this batch needs more
+                    //    skips the taps, the gathers and the derivative (most of the volume: air, the
+                    //    inside of a homogeneous organ).
                     float dd[RB][3];
                     unsigned char flag[RB];
 #pragma unroll
                     for (int rr = 0; rr < RB; ++rr) {
-                        const int zz = tw * GROWS + bt * RB + rr;
+                        flag[rr] = flaga[bt * RB + rr];
 #pragma unroll
-                        for (int cc = 0; cc < 3; ++cc) {
-                            float xs = lds_f32(sf + 4u * ((cc * GTZ + zz) * TX + lane));           // Eq. (1)
-#pragma unroll
-                            for (int k = 0; k < K; ++k)
-                                xs = fmaf(lds_f32(sf + 4u * (((3 + 3 * k + cc) * GTZ + zz) * TX + lane)), w[k], xs);
-                            dd[rr][cc] = xs;
-                        }
-                        const int ci = x + (int)floorf(dd[rr][0]) + 1, cj = c.y + (int)floorf(dd[rr][1]) + 1,
-                                  ck = c.z0 + zz + (int)floorf(dd[rr][2]) + 1;
-                        const bool inside = x < G.nx && c.z0 + zz < G.nz && (unsigned)ci <= (unsigned)G.nx &&
-                                            (unsigned)cj <= (unsigned)G.ny && (unsigned)ck <= (unsigned)G.nz;
-                        flag[rr] = inside ? __ldg(cellmap + ((long long)ck * (G.ny + 1) + cj) * (G.nx + 1) + ci) : (unsigned char)0;
+                        for (int cc = 0; cc < 3; ++cc) dd[rr][cc] = dda[bt * RB + rr][cc];
                     }
                     bool mine = false;
 #pragma unroll

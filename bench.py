@@ -296,6 +296,8 @@ def run_ours(args, cfg, rank, local_rank, world):
         stage = torch.empty_like(yb_dev[0])
         w_zero = np.zeros((B, cfg.K), np.float32)
 
+    tumour_mm = {}          # frame index in the block -> localised tumour position (device-resident pass)
+
     def run_block(first, count, w, host):
         if B > 1:
             for i in range(first, first + count):
@@ -311,6 +313,8 @@ def run_ours(args, cfg, rank, local_rank, world):
                 r = m.reconstruct(ys_host[i].numpy(), angles[i], w, opts, host_y=True)
             else:
                 r = m.reconstruct(ys_dev[i], angles[i], w, opts)
+                if r.landmarks is not None and len(r.landmarks):
+                    tumour_mm[i] = np.array(r.landmarks[0], np.float64)
             w = r.w
         return w, r
 
@@ -397,6 +401,17 @@ def run_ours(args, cfg, rank, local_rank, world):
                "sample": f"1 projection (frame {ids[args.warmup]}), full {it}-iteration solve from w = 0, "
                          f"OpenMP on {nthr} threads; {time.perf_counter() - tc:.0f} s including its simulated y"}
 
+    # ---- accuracy context (PAPER.md:L119 3D localisation error; not a parity value): the tumour
+    #      position of every timed solve against the fixed point of the analytic test DVF
+    accuracy = None
+    if B == 1 and tumour_mm:
+        from workloads.motion import true_tumour_position
+        errs = [float(np.linalg.norm(tumour_mm[i] - true_tumour_position(cfg, wl.spec, wl.frames[ids[i]], wl.landmarks[0])))
+                for i in sorted(tumour_mm) if i >= args.warmup]
+        if errs:
+            accuracy = {"tumour_error_mm_mean": float(np.mean(errs)), "tumour_error_mm_max": float(np.max(errs)),
+                        "n": len(errs), "note": "synthetic phantom, context only (the paper reports 0.8 +- 0.5 mm on NCAT, L135)"}
+
     line = {"metric": METRIC, "value": ms_per_solve, "unit": "ms", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -406,6 +421,7 @@ def run_ours(args, cfg, rank, local_rank, world):
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
             "last_solve": {"iters": tr.iters, "trials": trials, "status": tr.status, "J0": tr.J0, "J": tr.J},
+            "accuracy": accuracy,
             "context": {"paper_ms_per_projection_tesla_c1060": 240.0}}
     print(json.dumps(line), flush=True)
 

@@ -259,3 +259,58 @@ def solve(g: Geometry, f0, xbar, u, y, theta, w0, opts: Optional[Opts] = None,
     it = res.iters
     return dict(w=w, f=f, p=p, a=res.a, b=res.b, J0=res.J0, J=res.J, iters=it, status=res.status,
                 J_trace=Jt[:it + 1], gnorm_trace=gt[:min(it + 1, n)], mu_trace=mt[:it], backtracks=bt[:it])
+
+
+# ---------------------------------------------------------------- frame stream
+#
+# PAPER.md:L141 (section 4): "We initialized the PCA coefficients to those at its previous frame";
+# PAPER.md:L154 (section 5): "we can also use the predicted PCA coefficients from previous
+# histories to serve as the initial guess for optimization".  The paper names no predictor;
+# DESIGN.md reading B9 takes the polynomial of degree `order` through the last order + 1 frames
+# (order 0 = the previous frame's w, L141), written here as the Lagrange interpolation formula.
+
+def predict_w(times: Sequence[float], ws, t: float, order: int, w0=None) -> np.ndarray:
+    """w predicted for time t from the history (times[i], ws[i]), oldest first.
+
+    order < 0: always w0.  No history: w0.  Otherwise the Lagrange polynomial through the last
+    m = min(order, len(history) - 1) + 1 frames evaluated at t, in float64:
+        w(t) = sum_i w_i prod_{j != i} (t - t_j) / (t_i - t_j).
+    If two of those frames share a time stamp the prediction is the last frame's w.
+    """
+    ws = np.asarray(ws, dtype=np.float64)
+    K = ws.shape[1] if ws.ndim == 2 else (len(w0) if w0 is not None else 0)
+    base = np.zeros(K) if w0 is None else np.asarray(w0, dtype=np.float64)
+    if order < 0 or len(times) == 0:
+        return base.copy()
+    m = min(order, len(times) - 1) + 1
+    ts = [float(x) for x in times[-m:]]
+    wm = ws[-m:]
+    if len(set(ts)) < m:
+        return wm[-1].copy()
+    out = np.zeros(K)
+    for i in range(m):
+        c = 1.0
+        for j in range(m):
+            if j != i:
+                c *= (float(t) - ts[j]) / (ts[i] - ts[j])
+        out += c * wm[i]
+    return out
+
+
+def solve_frames(g: Geometry, f0, xbar, u, ys, thetas, times, order: int, opts: Optional[Opts] = None, w0=None,
+                 history=None):
+    """The per-projection solve over consecutive frames: frame n starts from float32(predict_w(...))
+    of the frames before it (w_init crosses the boundary as float32).  `history`, if given, is
+    a list of (t, w) the first prediction starts from.  Returns the list of solve() results, each
+    with its 'w_init'."""
+    hist_t = [h[0] for h in history] if history else []
+    hist_w = [np.asarray(h[1], dtype=np.float64) for h in history] if history else []
+    out = []
+    for y, th, t in zip(ys, thetas, times):
+        wi = predict_w(hist_t, np.array(hist_w).reshape(len(hist_w), g.K), t, order, w0).astype(np.float32)
+        r = solve(g, f0, xbar, u, y, th, wi, opts, want_volume=False)
+        r["w_init"] = wi
+        out.append(r)
+        hist_t.append(float(t))
+        hist_w.append(np.asarray(r["w"], dtype=np.float32).astype(np.float64))   # w leaves a solve as float32
+    return out

@@ -140,6 +140,49 @@ int pcamm_reconstruct_batch(pcamm_model* model, int32_t B, const float* y_dev, c
                             float* volumes_out_dev, float* landmarks_out_host, pcamm_info* info,
                             void* stream);
 
+/* ---- frame stream: consecutive projections of one treatment ----
+ *
+ * PAPER.md:L141 (section 4): "We initialized the PCA coefficients to those at its previous frame
+ * considering the high-frequency image acquisition (6 Hz) relative to breathing."
+ * PAPER.md:L154 (section 5): "we can also use the predicted PCA coefficients from previous
+ * histories to serve as the initial guess for optimization."  The paper names no predictor;
+ * reading B9: the start of frame n is the polynomial of degree `order` through the last
+ * order + 1 solved frames (their time stamps t and results w), evaluated at the new frame's t:
+ *   order 0 = the previous frame's w (L141); 1 = linear; 2 = quadratic extrapolation;
+ *   PCAMM_PREDICT_NONE = every frame starts from w0.
+ * With fewer solved frames than order + 1 the degree drops to what the history allows; the first
+ * frame starts from w0; equal time stamps among the frames used fall back to order 0.  The
+ * prediction is K scalars of host arithmetic in double, rounded to float (w_init is float).
+ * A fixed-angle sequence (fluoroscopy: "the projection matrix will be constant")
+ * is the same call with a constant angle_rad. */
+#define PCAMM_PREDICT_NONE (-1)
+#define PCAMM_PREDICT_MAX_ORDER 2
+
+/* The predictor alone (host arithmetic, no device): history of n frames, oldest first, time stamps
+ * t_host [n] and results w_host [n][K]; w0_host [K] or NULL (= 0); w_pred_host [K]. */
+int pcamm_predict_w(int32_t order, int32_t K, int32_t n, const double* t_host, const float* w_host,
+                    const float* w0_host, double t, float* w_pred_host);
+
+typedef struct pcamm_frames pcamm_frames; /* opaque; holds the history, refers to (does not own) the model */
+
+/* w0_host [K] or NULL (= 0).  The model must outlive the stream. */
+int pcamm_frames_create(pcamm_model* model, int32_t order, const float* w0_host, pcamm_frames** out);
+void pcamm_frames_destroy(pcamm_frames* frames);
+/* Forget the history (the next frame starts from w0 again). */
+int pcamm_frames_reset(pcamm_frames* frames);
+/* Number of solved frames held (at most PCAMM_PREDICT_MAX_ORDER + 1 are kept). */
+int32_t pcamm_frames_count(const pcamm_frames* frames);
+/* The start the next pcamm_frames_push at time t would use: w_pred_host [K]. */
+int pcamm_frames_predict(const pcamm_frames* frames, double t, float* w_pred_host);
+/* Solve the frame measured at time t (any unit, non-decreasing) from the predicted start and
+ * append (t, w) to the history.  y [nv][nu] is a device pointer, or a host pointer if y_on_host
+ * != 0 (then the host->device copy is part of the call).  w_init_out_host [K] or NULL receives
+ * the start that was used; the other arguments are pcamm_reconstruct's.  A hard error leaves
+ * the history as it was. */
+int pcamm_frames_push(pcamm_frames* frames, const float* y, int32_t y_on_host, float angle_rad, double t,
+                      const pcamm_opts* opts, float* w_out_host, float* w_init_out_host, float* volume_out_dev,
+                      float* landmarks_out_host, pcamm_info* info, void* stream);
+
 /* ---- function-level hooks (parity tests; reading A16 level i) ---- */
 
 /* f = warp(f0, xbar + U w): Eq. 1 + trilinear pull-back. */

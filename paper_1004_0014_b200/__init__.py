@@ -52,7 +52,9 @@ class pcamm_info(C.Structure):
 SYMBOLS = ("pcamm_default_opts", "pcamm_model_create", "pcamm_model_destroy", "pcamm_reconstruct",
            "pcamm_reconstruct_host", "pcamm_reconstruct_batch", "pcamm_warp", "pcamm_project",
            "pcamm_backproject", "pcamm_eval", "pcamm_traverse", "pcamm_localise", "pcamm_time_kernel",
-           "pcamm_launch_count", "pcamm_last_error")
+           "pcamm_launch_count", "pcamm_last_error", "pcamm_predict_w", "pcamm_frames_create",
+           "pcamm_frames_destroy", "pcamm_frames_reset", "pcamm_frames_count", "pcamm_frames_predict",
+           "pcamm_frames_push")
 
 _lib = None
 
@@ -75,6 +77,8 @@ def lib(build_if_missing: bool = True):
         L.pcamm_launch_count.restype = C.c_int64
         L.pcamm_model_destroy.restype = None
         L.pcamm_default_opts.restype = None
+        L.pcamm_frames_destroy.restype = None
+        L.pcamm_frames_count.restype = C.c_int32
         _lib = L
     return _lib
 
@@ -126,6 +130,7 @@ class Result:
     gnorm_trace: Optional[np.ndarray] = None
     mu_trace: Optional[np.ndarray] = None
     backtracks: Optional[np.ndarray] = None
+    w_init: Optional[np.ndarray] = None   # Frames.push: the predicted start
 
 
 def _torch():
@@ -320,3 +325,77 @@ class Model:
         ms = C.c_float(0)
         _check(lib().pcamm_time_kernel(self._h, int(which), int(reps), C.byref(ms), _stream()))
         return float(ms.value)
+
+
+def predict_w(order: int, times, ws, t: float, w0=None, K: Optional[int] = None) -> np.ndarray:
+    """pcamm_predict_w: the start predicted for time t from the history (times[i], ws[i]), oldest first."""
+    ws = np.ascontiguousarray(ws, dtype=np.float32)
+    ts = np.ascontiguousarray(times, dtype=np.float64).reshape(-1)
+    n = ts.size
+    K = K or (ws.shape[1] if ws.ndim == 2 and n else len(w0))
+    ws = ws.reshape(n, K)
+    w0a = _host_f32(w0, K) if w0 is not None else None
+    out = np.zeros(K, np.float32)
+    _check(lib().pcamm_predict_w(int(order), int(K), int(n), ts.ctypes.data_as(C.c_void_p), ws.ctypes.data_as(C.c_void_p),
+                                 w0a.ctypes.data_as(C.c_void_p) if w0a is not None else None, C.c_double(t),
+                                 out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+class Frames:
+    """pcamm_frames_*: consecutive projections of one treatment; each solve starts from the
+    coefficients predicted from the frames before it (order 0: the previous frame's w, 1: linear,
+    2: quadratic extrapolation in the frames' time stamps, -1: always w0)."""
+
+    def __init__(self, model: Model, order: int = 0, w0=None):
+        self.model = model                    # keeps the model alive
+        self._h = C.c_void_p()
+        w0a = _host_f32(w0, model.K) if w0 is not None else None
+        _check(lib().pcamm_frames_create(model._h, int(order), w0a.ctypes.data_as(C.c_void_p) if w0a is not None else None,
+                                         C.byref(self._h)))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().pcamm_frames_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def reset(self) -> None:
+        _check(lib().pcamm_frames_reset(self._h))
+
+    def count(self) -> int:
+        return int(lib().pcamm_frames_count(self._h))
+
+    def predict(self, t: float) -> np.ndarray:
+        w = np.zeros(self.model.K, np.float32)
+        _check(lib().pcamm_frames_predict(self._h, C.c_double(t), w.ctypes.data_as(C.c_void_p)))
+        return w
+
+    def push(self, y, angle_rad: float, t: float, opts: Optional[Opts] = None, volume_out=None, trace: bool = False,
+             host_y: bool = False) -> Result:
+        """Solve the frame measured at time t; the result carries the start that was used as w_init."""
+        m = self.model
+        opts = opts or Opts()
+        w = np.zeros((1, m.K), np.float32)
+        wi = np.zeros(m.K, np.float32)
+        lm = np.zeros((1, m.M, 3), np.float32) if m.M else None
+        infos, keep = m._info(opts, 1, trace)
+        oc = opts._c()
+        vol = _dev_f32(volume_out, m.V, "volume_out") if volume_out is not None else None
+        if host_y:
+            yh = y if isinstance(y, np.ndarray) else y.numpy()
+            assert yh.dtype == np.float32 and yh.flags.c_contiguous and yh.size == m.npix
+            yarg = C.c_void_p(yh.ctypes.data)
+        else:
+            yarg = _dev_f32(y, m.npix, "y")
+        _check(lib().pcamm_frames_push(self._h, yarg, 1 if host_y else 0, C.c_float(angle_rad), C.c_double(t),
+                                       C.byref(oc), w.ctypes.data_as(C.c_void_p), wi.ctypes.data_as(C.c_void_p), vol,
+                                       lm.ctypes.data_as(C.c_void_p) if lm is not None else None, infos, _stream()))
+        r = m._result(0, w, lm, infos, keep, opts.max_iter)
+        r.w_init = wi
+        return r

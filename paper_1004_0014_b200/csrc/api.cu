@@ -380,6 +380,10 @@ int hook_begin(pcamm_model* m, const float* y_dev, float angle, const float* w, 
 
 }  // namespace
 
+namespace pcamm {
+int model_K(const pcamm_model* m) { return m->G.K; }
+}  // namespace pcamm
+
 extern "C" {
 
 void pcamm_default_opts(pcamm_opts* o) {

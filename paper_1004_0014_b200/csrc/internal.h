@@ -10,10 +10,13 @@
 #include "common.cuh"
 #include "stream.cuh"
 
+struct pcamm_model;
+
 namespace pcamm {
 
 void set_error(const std::string& msg);
 void count_launch(long long n);
+int model_K(const pcamm_model* m);   // api.cu
 
 // A linear sequence of kernels.  stream mode: cudaLaunchKernel on `stream`.  graph mode: each
 // kernel becomes a node of `graph` depending on the previous one, so the solve can be replayed

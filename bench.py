@@ -426,6 +426,64 @@ def run_ours(args, cfg, rank, local_rank, world):
     print(json.dumps(line), flush=True)
 
 
+def run_frames_study(args, cfg, rank, local_rank):
+    """--frames-study: the frame stream (pcamm_frames_*) over the
+    same consecutive projections under each start predictor, stopping on the gradient norm
+     instead of after a fixed 10 iterations.  Prints one JSON line (not the bench
+    contract's line): iterations, candidate evaluations, ms per solve and 6 Hz headroom per
+    predictor.  grad_tol, unless given, is the median ||g|| the paper's fixed 10 iterations reach
+    on the warm-up frames started from the previous frame's w."""
+    if rank != 0:
+        return
+    n = args.steps + args.warmup
+    wl = build_workload(cfg)
+    ids = list(range(FIRST_FRAME, FIRST_FRAME + n))
+    gts = ground_truth_volumes(wl, ids)
+    import torch
+    import paper_1004_0014_b200 as pc
+    from workloads.motion import true_tumour_position
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(dev)
+    m = pc.Model(nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, hx=cfg.hx, hy=cfg.hy, hz=cfg.hz, K=cfg.K, nu=cfg.nu, nv=cfg.nv,
+                 pu=cfg.pu, pv=cfg.pv, f0=t(wl.f0), mean_dvf=t(wl.model.mean), eig_dvf=t(wl.model.eig),
+                 landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd)
+    frames = [wl.frames[i] for i in ids]
+    ys = [t(add_noise(m.project(t(gts[fr.index]), fr.angle_rad).cpu().numpy(), cfg.noise, seed=fr.index)) for fr in frames]
+    it = solver_iterations(cfg)
+    tol = args.grad_tol
+    if tol is None:
+        fs = pc.Frames(m, order=0)
+        gn = []
+        for fr, y in zip(frames[:max(args.warmup, 3)], ys):
+            r = fs.push(y, fr.angle_rad, fr.time_s, pc.Opts(max_iter=it), trace=True)
+            gn.append(float(r.gnorm_trace[-1]))
+        tol = float(np.median(gn[1:])) if len(gn) > 1 else gn[0]
+    opts = pc.Opts(max_iter=args.study_max_iter, grad_tol=tol)
+    per = {}
+    for order, name in ((-1, "none (w = 0 every frame)"), (0, "previous frame (L141)"), (1, "linear"), (2, "quadratic")):
+        fs = pc.Frames(m, order=order)
+        for fr, y in zip(frames[:args.warmup], ys):
+            fs.push(y, fr.angle_rad, fr.time_s, opts)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        out = [fs.push(y, fr.angle_rad, fr.time_s, opts, trace=True) for fr, y in zip(frames[args.warmup:], ys[args.warmup:])]
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / len(out)
+        errs = [float(np.linalg.norm(np.array(r.landmarks[0], np.float64) -
+                                     true_tumour_position(cfg, wl.spec, fr, wl.landmarks[0])))
+                for r, fr in zip(out, frames[args.warmup:])]
+        per[str(order)] = {"predictor": name, "ms_per_solve": ms, "mean_iters": float(np.mean([r.iters for r in out])),
+                           "mean_candidate_evaluations": float(np.mean([int(np.sum(r.backtracks + 1)) for r in out])),
+                           "stopped_on_grad_tol": int(sum(r.status == pc.S_GRADTOL for r in out)),
+                           "mean_J": float(np.mean([r.J for r in out])), "tumour_error_mm_mean": float(np.mean(errs)),
+                           "headroom_at_6_hz": (1000.0 / 6.0) / ms}
+    print(json.dumps({"study": "frames", "config": config_dict(cfg, args.study_max_iter), "frames": len(frames) - args.warmup,
+                      "warmup": args.warmup, "grad_tol": tol, "max_iter": args.study_max_iter, "per_order": per}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -443,12 +501,19 @@ def main():
     ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1],
                     help="0: the solve is one CUDA graph with device-side while-loops (default, the timed "
                          "configuration); 1: same kernels launched from the host (for per-launch ncu lists)")
+    ap.add_argument("--frames-study", action="store_true",
+                    help="instead of the bench line: iterations and ms per solve of the frame stream under each "
+                         "start predictor (pcamm_frames_*), stopping on ||g|| <= --grad-tol")
+    ap.add_argument("--grad-tol", type=float, default=None)
+    ap.add_argument("--study-max-iter", type=int, default=30)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     from paper_1004_0014_b200.replicas import env_rank_world
     rank, local_rank, world = env_rank_world()
     cfg = get_config(args.config)
-    if args.impl == "reference":
+    if args.frames_study:
+        run_frames_study(args, cfg, rank, local_rank)
+    elif args.impl == "reference":
         run_reference(args, cfg, rank, world)
     else:
         run_ours(args, cfg, rank, local_rank, world)

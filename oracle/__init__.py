@@ -314,3 +314,36 @@ def solve_frames(g: Geometry, f0, xbar, u, ys, thetas, times, order: int, opts: 
         hist_t.append(float(t))
         hist_w.append(np.asarray(r["w"], dtype=np.float32).astype(np.float64))   # w leaves a solve as float32
     return out
+
+
+# ---------------------------------------------------------------- PCA motion model
+#
+# PAPER.md:L63-69 (section 2.1, Eq. 1): "the DVF ... is approximated by a linear combination of the
+# sample mean vector and a few eigenvectors corresponding to the largest eigenvalues";
+# the training DVFs of the other phases relative to the reference give xbar, u_1..K.
+# Written as the definition: the principal axes of the samples are the right singular vectors of
+# the centred data matrix (library SVD, float64).  Reading A12: unit-norm u_k, eigenvalues of the
+# scatter matrix (no 1/(N-1)), sign of u_k such that u_k . (D_sign_ref - mean) >= 0; reading B10:
+# if that product is exactly 0, the training coefficient of largest magnitude is made positive.
+
+def pca_fit(dvfs, K: int, sign_ref: Optional[int] = None):
+    """dvfs [N][...] float32 samples.  Returns dict(mean [...], eig [K][...], eigenvalues [N]
+    descending, coeffs [N][K] = u_k . (D_i - mean)), all float64."""
+    d32 = np.asarray(dvfs, dtype=np.float32)
+    N = d32.shape[0]
+    shape = d32.shape[1:]
+    D = d32.reshape(N, -1).astype(np.float64)
+    if sign_ref is None:
+        sign_ref = N // 2
+    mean = D.sum(axis=0) / N
+    X = D - mean[None, :]
+    _, S, Vt = np.linalg.svd(X, full_matrices=False)
+    lam = S ** 2
+    u = Vt[:K].copy()
+    coeffs = X @ u.T
+    for k in range(K):
+        c = coeffs[sign_ref, k]
+        if c < 0 or (c == 0 and coeffs[np.argmax(np.abs(coeffs[:, k])), k] < 0):
+            u[k] = -u[k]
+            coeffs[:, k] = -coeffs[:, k]
+    return dict(mean=mean.reshape(shape), eig=u.reshape((K,) + shape), eigenvalues=lam, coeffs=coeffs)

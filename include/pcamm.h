@@ -140,6 +140,28 @@ int pcamm_reconstruct_batch(pcamm_model* model, int32_t B, const float* y_dev, c
                             float* volumes_out_dev, float* landmarks_out_host, pcamm_info* info,
                             void* stream);
 
+/* ---- PCA motion model from training DVFs ----
+ *
+ * PAPER.md:L63-69 (section 2.1, Eq. 1): x(t) ~ xbar + sum_k u_k w_k(t) with xbar "the sample mean
+ * vector" and u_k the "eigenvectors corresponding to the largest eigenvalues"; the
+ * samples are the DVFs of the training phases relative to the reference phase.
+ * dvfs_dev [N][n_per_sample] float32 (n_per_sample = 3 nx ny nz for [3][nz][ny][nx] fields), N in
+ * [2, PCAMM_PCA_MAX_SAMPLES], 1 <= K <= min(PCAMM_KMAX, N - 1).  Outputs, in the layout
+ * pcamm_model_create takes: mean_out_dev [n_per_sample] = (1/N) sum_i D_i; eig_out_dev
+ * [K][n_per_sample], unit L2 norm each, u_k = sum_i v_ik (D_i - xbar) / sqrt(lambda_k) for the
+ * eigenpairs (lambda_k, v_k) of the N x N scatter matrix <D_i - xbar, D_j - xbar> (no 1/(N-1)),
+ * lambda descending (reading A12).  Sign: u_k . (D_sign_ref - xbar) >= 0 (sign_ref = -1: sample
+ * N/2, the end-of-inhale phase of the recipe); if that product is exactly 0 the training
+ * coefficient of largest magnitude is positive (reading B10).  Host outputs or NULL:
+ * eigenvalues_out_host [N] (double), coeffs_out_host [N][K] = u_k . (D_i - xbar) (double).
+ * Errors: PCAMM_E_SINGULAR if lambda_K <= 1e-6 lambda_1 (below what float32 products resolve),
+ * PCAMM_E_NONFINITE for non-finite samples.
+ * Two passes over the samples on `stream`; blocking. */
+#define PCAMM_PCA_MAX_SAMPLES 16
+int pcamm_pca_fit(int64_t n_per_sample, int32_t N, int32_t K, const float* dvfs_dev, int32_t sign_ref,
+                  float* mean_out_dev, float* eig_out_dev, double* eigenvalues_out_host,
+                  double* coeffs_out_host, void* stream);
+
 /* ---- frame stream: consecutive projections of one treatment ----
  *
  * PAPER.md:L141 (section 4): "We initialized the PCA coefficients to those at its previous frame

@@ -52,7 +52,7 @@ class pcamm_info(C.Structure):
 SYMBOLS = ("pcamm_default_opts", "pcamm_model_create", "pcamm_model_destroy", "pcamm_reconstruct",
            "pcamm_reconstruct_host", "pcamm_reconstruct_batch", "pcamm_warp", "pcamm_project",
            "pcamm_backproject", "pcamm_eval", "pcamm_traverse", "pcamm_localise", "pcamm_time_kernel",
-           "pcamm_launch_count", "pcamm_last_error", "pcamm_predict_w", "pcamm_frames_create",
+           "pcamm_launch_count", "pcamm_last_error", "pcamm_pca_fit", "pcamm_predict_w", "pcamm_frames_create",
            "pcamm_frames_destroy", "pcamm_frames_reset", "pcamm_frames_count", "pcamm_frames_predict",
            "pcamm_frames_push")
 
@@ -325,6 +325,25 @@ class Model:
         ms = C.c_float(0)
         _check(lib().pcamm_time_kernel(self._h, int(which), int(reps), C.byref(ms), _stream()))
         return float(ms.value)
+
+
+def pca_fit(dvfs, K: int, sign_ref: int = -1):
+    """pcamm_pca_fit: the PCA motion model of the training DVFs `dvfs` [N][...] (float32 CUDA tensor).
+    Returns (mean [...], eig [K][...]) as CUDA tensors in the layout Model takes, the N eigenvalues of
+    the scatter matrix (descending) and the training coefficients [N][K] (float64 host arrays)."""
+    torch = _torch()
+    if not (dvfs.is_cuda and dvfs.dtype == torch.float32 and dvfs.is_contiguous()):
+        raise ValueError("dvfs must be a contiguous float32 CUDA tensor")
+    N = int(dvfs.shape[0])
+    n = dvfs[0].numel()
+    mean = torch.empty(tuple(dvfs.shape[1:]), dtype=torch.float32, device=dvfs.device)
+    eig = torch.empty((K,) + tuple(dvfs.shape[1:]), dtype=torch.float32, device=dvfs.device)
+    lam = np.zeros(max(N, 1), np.float64)
+    coeffs = np.zeros((max(N, 1), max(K, 1)), np.float64)
+    _check(lib().pcamm_pca_fit(C.c_int64(n), N, int(K), C.c_void_p(dvfs.data_ptr()), int(sign_ref),
+                               C.c_void_p(mean.data_ptr()), C.c_void_p(eig.data_ptr()), lam.ctypes.data_as(C.c_void_p),
+                               coeffs.ctypes.data_as(C.c_void_p), _stream()))
+    return mean, eig, lam, coeffs
 
 
 def predict_w(order: int, times, ws, t: float, w0=None, K: Optional[int] = None) -> np.ndarray:

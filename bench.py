@@ -484,6 +484,53 @@ def run_frames_study(args, cfg, rank, local_rank):
                       "warmup": args.warmup, "grad_tol": tol, "max_iter": args.study_max_iter, "per_order": per}), flush=True)
 
 
+def run_pca_study(args, cfg, rank, local_rank):
+    """--pca-study: pcamm_pca_fit on the config's nine training
+    DVFs: device time of its two streaming passes (CUDA events on the launching stream, inside the
+    library) against their algorithmic bytes, the whole call's wall time, and the distance of the
+    fitted fields from the input recipe's own PCA (context).  One JSON line, not the bench contract's."""
+    if rank != 0:
+        return
+    from workloads.motion import motion_spec, training_dvfs
+    from workloads.pca import fit_pca
+    t0 = time.perf_counter()
+    dvfs = np.ascontiguousarray(training_dvfs(cfg, motion_spec(cfg)), dtype=np.float32)
+    log(f"training DVFs {dvfs.shape} built in {time.perf_counter() - t0:.1f} s")
+    import torch
+    import paper_1004_0014_b200 as pc
+    torch.cuda.set_device(local_rank)
+    d = torch.from_numpy(dvfs).to(torch.device("cuda", local_rank))
+    N, n = dvfs.shape[0], dvfs[0].size
+    for _ in range(max(args.warmup, 1)):
+        pc.pca_fit(d, cfg.K)
+    ms1, ms2, wall = [], [], []
+    for _ in range(args.steps):
+        pm = []
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        mean, eig, lam, coeffs = pc.pca_fit(d, cfg.K, pass_ms=pm)
+        wall.append(1e3 * (time.perf_counter() - t0))
+        ms1.append(pm[0]); ms2.append(pm[1])
+    peak, peak_src = measured_peak_gbs()
+    b1, b2 = 4 * N * n, 4 * N * n + 4 * (cfg.K + 1) * n
+    m1, m2 = float(np.median(ms1)), float(np.median(ms2))
+    t0 = time.perf_counter()
+    ref = fit_pca(dvfs, cfg.K)
+    host_s = time.perf_counter() - t0
+    e = eig.cpu().numpy().astype(np.float64)
+    print(json.dumps({"study": "pca", "workload": f"{cfg.name}: {N} training DVFs of 3 x {cfg.nx}x{cfg.ny}x{cfg.nz} floats, K={cfg.K}",
+                      "reps": args.steps,
+                      "scatter_matrix_pass": {"ms": m1, "algorithmic_bytes": b1, "achieved_gbs": b1 / m1 / 1e6, "frac": b1 / m1 / 1e6 / peak},
+                      "fields_pass": {"ms": m2, "algorithmic_bytes": b2, "achieved_gbs": b2 / m2 / 1e6, "frac": b2 / m2 / 1e6 / peak},
+                      "peak_gbs": peak, "peak_source": peak_src, "call_wall_ms": float(np.median(wall)),
+                      "eigenvalues": [float(x) for x in lam[:N]],
+                      "context": {"input_recipe_pca_numpy_float64_s": host_s,
+                                  "eig_l2_distance_from_recipe": [float(np.linalg.norm(e[k] - ref.eig[k].astype(np.float64)))
+                                                                  for k in range(cfg.K)],
+                                  "mean_max_abs_distance_mm": float(np.abs(mean.cpu().numpy() - ref.mean).max())}}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -504,6 +551,9 @@ def main():
     ap.add_argument("--frames-study", action="store_true",
                     help="instead of the bench line: iterations and ms per solve of the frame stream under each "
                          "start predictor (pcamm_frames_*), stopping on ||g|| <= --grad-tol")
+    ap.add_argument("--pca-study", action="store_true",
+                    help="instead of the bench line: pcamm_pca_fit on the config's training DVFs (device time of its "
+                         "two passes against their algorithmic bytes)")
     ap.add_argument("--grad-tol", type=float, default=None)
     ap.add_argument("--study-max-iter", type=int, default=30)
     args = ap.parse_args()
@@ -513,6 +563,8 @@ def main():
     cfg = get_config(args.config)
     if args.frames_study:
         run_frames_study(args, cfg, rank, local_rank)
+    elif args.pca_study:
+        run_pca_study(args, cfg, rank, local_rank)
     elif args.impl == "reference":
         run_reference(args, cfg, rank, world)
     else:

@@ -156,11 +156,12 @@ int pcamm_reconstruct_batch(pcamm_model* model, int32_t B, const float* y_dev, c
  * eigenvalues_out_host [N] (double), coeffs_out_host [N][K] = u_k . (D_i - xbar) (double).
  * Errors: PCAMM_E_SINGULAR if lambda_K <= 1e-6 lambda_1 (below what float32 products resolve),
  * PCAMM_E_NONFINITE for non-finite samples.
- * Two passes over the samples on `stream`; blocking. */
+ * pass_ms_out_host [2] or NULL: device time in ms of the two passes over the samples (scatter
+ * matrix; fields), CUDA events on `stream` (for bench.py).  Blocking. */
 #define PCAMM_PCA_MAX_SAMPLES 16
 int pcamm_pca_fit(int64_t n_per_sample, int32_t N, int32_t K, const float* dvfs_dev, int32_t sign_ref,
                   float* mean_out_dev, float* eig_out_dev, double* eigenvalues_out_host,
-                  double* coeffs_out_host, void* stream);
+                  double* coeffs_out_host, float* pass_ms_out_host, void* stream);
 
 /* ---- frame stream: consecutive projections of one treatment ----
  *

@@ -327,7 +327,7 @@ class Model:
         return float(ms.value)
 
 
-def pca_fit(dvfs, K: int, sign_ref: int = -1):
+def pca_fit(dvfs, K: int, sign_ref: int = -1, pass_ms: Optional[list] = None):
     """pcamm_pca_fit: the PCA motion model of the training DVFs `dvfs` [N][...] (float32 CUDA tensor).
     Returns (mean [...], eig [K][...]) as CUDA tensors in the layout Model takes, the N eigenvalues of
     the scatter matrix (descending) and the training coefficients [N][K] (float64 host arrays)."""
@@ -340,9 +340,12 @@ def pca_fit(dvfs, K: int, sign_ref: int = -1):
     eig = torch.empty((K,) + tuple(dvfs.shape[1:]), dtype=torch.float32, device=dvfs.device)
     lam = np.zeros(max(N, 1), np.float64)
     coeffs = np.zeros((max(N, 1), max(K, 1)), np.float64)
+    ms = (C.c_float * 2)()
     _check(lib().pcamm_pca_fit(C.c_int64(n), N, int(K), C.c_void_p(dvfs.data_ptr()), int(sign_ref),
                                C.c_void_p(mean.data_ptr()), C.c_void_p(eig.data_ptr()), lam.ctypes.data_as(C.c_void_p),
-                               coeffs.ctypes.data_as(C.c_void_p), _stream()))
+                               coeffs.ctypes.data_as(C.c_void_p), ms if pass_ms is not None else None, _stream()))
+    if pass_ms is not None:
+        pass_ms[:] = [float(ms[0]), float(ms[1])]
     return mean, eig, lam, coeffs
 
 

@@ -234,7 +234,7 @@ using namespace pcamm;
 
 extern "C" int pcamm_pca_fit(int64_t n_per_sample, int32_t N, int32_t K, const float* dvfs_dev, int32_t sign_ref,
                              float* mean_out_dev, float* eig_out_dev, double* eigenvalues_out_host,
-                             double* coeffs_out_host, void* stream) {
+                             double* coeffs_out_host, float* pass_ms_out_host, void* stream) {
     if (!dvfs_dev || !mean_out_dev || !eig_out_dev) return fail(PCAMM_E_INVALID, "NULL argument");
     if (n_per_sample < 1) return fail(PCAMM_E_INVALID, "n_per_sample < 1");
     if (N < 2 || N > PCA_MAXN) return fail(PCAMM_E_INVALID, "number of samples outside [2, PCAMM_PCA_MAX_SAMPLES]");
@@ -250,8 +250,19 @@ extern "C" int pcamm_pca_fit(int64_t n_per_sample, int32_t N, int32_t K, const f
     double* partials = nullptr;
     cudaError_t e = cudaMalloc(&partials, sizeof(double) * (size_t)blocks * NP);
     if (e != cudaSuccess) return cuda_fail("cudaMalloc (scatter-matrix partial sums)", e);
+    cudaEvent_t ev[4] = {};
+    if (pass_ms_out_host) {
+        for (auto& x : ev)
+            if ((e = cudaEventCreate(&x)) != cudaSuccess) { cudaFree(partials); return cuda_fail("cudaEventCreate", e); }
+        cudaEventRecord(ev[0], st);
+    }
+    struct EventGuard {
+        cudaEvent_t* ev;
+        ~EventGuard() { for (int i = 0; i < 4; ++i) if (ev[i]) cudaEventDestroy(ev[i]); }
+    } guard{ev};
     e = cudaErrorInvalidValue;
     PCA_DISPATCH(N, e = launch_gram<NN>(dvfs_dev, n, n, v4, blocks, partials, st));
+    if (pass_ms_out_host) cudaEventRecord(ev[1], st);
     std::vector<double> hp((size_t)blocks * NP);
     if (e == cudaSuccess) e = cudaMemcpyAsync(hp.data(), partials, sizeof(double) * hp.size(), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -295,9 +306,15 @@ extern "C" int pcamm_pca_fit(int64_t n_per_sample, int32_t N, int32_t K, const f
     if (eigenvalues_out_host)
         for (int i = 0; i < N; ++i) eigenvalues_out_host[i] = lam[i];
 
+    if (pass_ms_out_host) cudaEventRecord(ev[2], st);
     e = cudaErrorInvalidValue;
     PCA_DISPATCH(N, e = launch_fields<NN>(dvfs_dev, n, n, v4, blocks, coef, K, mean_out_dev, eig_out_dev, st));
+    if (pass_ms_out_host) cudaEventRecord(ev[3], st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return cuda_fail("eigenvector fields", e);
+    if (pass_ms_out_host) {
+        cudaEventElapsedTime(&pass_ms_out_host[0], ev[0], ev[1]);
+        cudaEventElapsedTime(&pass_ms_out_host[1], ev[2], ev[3]);
+    }
     return PCAMM_OK;
 }

@@ -47,9 +47,9 @@ def test_invalid_arguments_are_reported_without_a_gpu():
     assert lib.pcamm_reconstruct(None, None, C.c_float(0), None, None, None, None, None, None, None) == pc.E_INVALID
     assert pc.launch_count() >= 0
     x = (C.c_float * 4)()
-    assert lib.pcamm_pca_fit(C.c_int64(4), 3, 2, None, -1, x, x, None, None, None) == pc.E_INVALID
-    assert lib.pcamm_pca_fit(C.c_int64(4), 1, 1, x, -1, x, x, None, None, None) == pc.E_INVALID    # N < 2
-    assert lib.pcamm_pca_fit(C.c_int64(4), 3, 3, x, -1, x, x, None, None, None) == pc.E_INVALID    # K > N - 1
+    assert lib.pcamm_pca_fit(C.c_int64(4), 3, 2, None, -1, x, x, None, None, None, None) == pc.E_INVALID
+    assert lib.pcamm_pca_fit(C.c_int64(4), 1, 1, x, -1, x, x, None, None, None, None) == pc.E_INVALID    # N < 2
+    assert lib.pcamm_pca_fit(C.c_int64(4), 3, 3, x, -1, x, x, None, None, None, None) == pc.E_INVALID    # K > N - 1
     assert "K outside" in pc.last_error()
 
 

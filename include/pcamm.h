@@ -68,6 +68,12 @@ typedef struct {
     float off_u, off_v;   /* detector offset in pixels */
     int32_t max_batch;    /* largest B of pcamm_reconstruct_batch (>= 1); scratch is sized for it */
     int32_t max_candidates; /* 1, or >= opts.max_backtracks to allow batched_linesearch */
+    int32_t field_storage;  /* 0 (default): x-bar and u_k kept in float32.  1: u_k kept in
+                               half precision, each scaled by a power of two so that its entries keep 11
+                               significant bits; x-bar stays float32.  Halves the dominant HBM stream of the
+                               warp and gradient kernels; the model then IS the rounded one (every step,
+                               the landmark inversion included, uses the rounded u_k; pcamm_model_fields
+                               returns them).  Needs nx % 8 == 0. */
 } pcamm_geometry;
 
 typedef struct {
@@ -115,6 +121,12 @@ int pcamm_model_create(const pcamm_geometry* geometry, const float* f0_dev, cons
                        const float* eig_dvf_dev, int32_t n_landmarks, const float* landmarks_mm_host,
                        void* stream, pcamm_model** out);
 void pcamm_model_destroy(pcamm_model* model);
+
+/* The motion model as the solve uses it, in mm and in model_create's layout: mean_dvf_out_dev
+ * [3][nz][ny][nx], eig_dvf_out_dev [K][3][nz][ny][nx].  With field_storage = 0 these are the
+ * inputs again (to float rounding of x / h * h); with field_storage = 1 the u_k are the values the
+ * stored halves stand for. */
+int pcamm_model_fields(pcamm_model* model, float* mean_dvf_out_dev, float* eig_dvf_out_dev, void* stream);
 
 /* The per-projection solve (sections 2.2-2.3).  y_dev [nv][nu] is the measured
  * projection, w_init_host [K] the start (the previous frame's w).  Outputs:

@@ -31,7 +31,7 @@ class pcamm_geometry(C.Structure):
                 ("K", C.c_int32), ("nu", C.c_int32), ("nv", C.c_int32),
                 ("pu", C.c_float), ("pv", C.c_float), ("sad", C.c_float), ("sdd", C.c_float),
                 ("off_u", C.c_float), ("off_v", C.c_float),
-                ("max_batch", C.c_int32), ("max_candidates", C.c_int32)]
+                ("max_batch", C.c_int32), ("max_candidates", C.c_int32), ("field_storage", C.c_int32)]
 
 
 class pcamm_opts(C.Structure):
@@ -49,7 +49,8 @@ class pcamm_info(C.Structure):
 
 
 # every symbol include/pcamm.h declares
-SYMBOLS = ("pcamm_default_opts", "pcamm_model_create", "pcamm_model_destroy", "pcamm_reconstruct",
+SYMBOLS = ("pcamm_default_opts", "pcamm_model_create", "pcamm_model_destroy", "pcamm_model_fields",
+           "pcamm_reconstruct",
            "pcamm_reconstruct_host", "pcamm_reconstruct_batch", "pcamm_warp", "pcamm_project",
            "pcamm_backproject", "pcamm_eval", "pcamm_traverse", "pcamm_localise", "pcamm_time_kernel",
            "pcamm_launch_count", "pcamm_last_error", "pcamm_pca_fit", "pcamm_predict_w", "pcamm_frames_create",
@@ -167,12 +168,12 @@ class Model:
 
     def __init__(self, *, nx, ny, nz, hx, hy, hz, K, nu, nv, pu, pv, f0, mean_dvf, eig_dvf,
                  landmarks_mm=None, sad=1000.0, sdd=1500.0, off_u=0.0, off_v=0.0, cx=0.0, cy=0.0, cz=0.0,
-                 max_batch=1, max_candidates=1):
+                 max_batch=1, max_candidates=1, field_storage=0):
         torch = _torch()
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1004_0014_b200 needs a CUDA device (there is no CPU fallback)")
         self.geo = pcamm_geometry(nx, ny, nz, hx, hy, hz, cx, cy, cz, K, nu, nv, pu, pv, sad, sdd, off_u, off_v,
-                                  max_batch, max_candidates)
+                                  max_batch, max_candidates, field_storage)
         self.K, self.V, self.npix = K, nx * ny * nz, nu * nv
         self.vshape, self.pshape = (nz, ny, nx), (nv, nu)
         lm = np.zeros((0, 3), np.float32) if landmarks_mm is None else \
@@ -184,6 +185,14 @@ class Model:
                                         _dev_f32(eig_dvf, 3 * K * self.V, "eig_dvf"), self.M,
                                         lm.ctypes.data_as(C.c_void_p), _stream(), C.byref(self._h)))
         self.device = f0.device
+
+    def fields(self):
+        """pcamm_model_fields: (mean_dvf [3][nz][ny][nx], eig_dvf [K][3][nz][ny][nx]) in mm as the solve uses them."""
+        torch = _torch()
+        mean = torch.empty((3,) + self.vshape, dtype=torch.float32, device=self.device)
+        eig = torch.empty((self.K, 3) + self.vshape, dtype=torch.float32, device=self.device)
+        _check(lib().pcamm_model_fields(self._h, C.c_void_p(mean.data_ptr()), C.c_void_p(eig.data_ptr()), _stream()))
+        return mean, eig
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h:

@@ -45,13 +45,49 @@ __global__ void k_fields_to_voxel_units(float* __restrict__ fields, long long V,
     }
 }
 
+// Reduced-precision storage.  max |u_k| per eigenvector field (bit pattern of a
+// non-negative float orders like an unsigned integer).
+__global__ void k_field_absmax(const float* __restrict__ u, long long n_per_k, int K, unsigned int* __restrict__ out) {
+    for (int k = 0; k < K; ++k) {
+        float mx = 0.f;
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_per_k; i += (long long)gridDim.x * blockDim.x)
+            mx = fmaxf(mx, fabsf(u[(long long)k * n_per_k + i]));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        if ((threadIdx.x & 31) == 0) atomicMax(out + k, __float_as_uint(mx));
+    }
+}
+// u16 = half(u * scale[k]); u is overwritten by the value the half stands for, u16 / scale[k]
+// (exact in float), so that every other reader of the fields sees what the streaming kernels see.
+__global__ void k_quantise_fields(float* __restrict__ u, __half* __restrict__ u16, long long n_per_k, int K,
+                                  FieldScale scale, FieldScale inv) {
+    const long long n = n_per_k * K;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int k = (int)(i / n_per_k);
+        const __half h = __float2half_rn(u[i] * scale.inv[k]);
+        u16[i] = h;
+        u[i] = __half2float(h) * inv.inv[k];
+    }
+}
+// Fields as the solve uses them, back in mm.
+__global__ void k_fields_to_mm(const float* __restrict__ fields, long long V, int planes, float hx, float hy, float hz,
+                               float* __restrict__ out) {
+    const long long n = V * planes;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int c = (int)((i / V) % 3);
+        out[i] = fields[i] * (c == 0 ? hx : (c == 1 ? hy : hz));
+    }
+}
+
 }  // namespace
 
-bool make_field_map(const Geom& G, const float* fields, int planes, int tz, CUtensorMap* out, std::string* why) {
+bool make_field_map(const Geom& G, const void* fields, int planes, int tz, int elem_bytes, CUtensorMap* out,
+                    std::string* why) {
     typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-    if (G.nx % 4 != 0) { if (why) *why = "nx * 4 bytes is not a multiple of 16"; return false; }
+    const cuuint64_t eb = (cuuint64_t)elem_bytes;
+    if ((G.nx * eb) % 16 != 0) { if (why) *why = "a row of nx elements is not a multiple of 16 bytes"; return false; }
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
@@ -61,10 +97,11 @@ bool make_field_map(const Geom& G, const float* fields, int planes, int tz, CUte
         return false;
     }
     const cuuint64_t dims[4] = {(cuuint64_t)G.nx, (cuuint64_t)G.ny, (cuuint64_t)G.nz, (cuuint64_t)planes};
-    const cuuint64_t strides[3] = {(cuuint64_t)G.nx * 4, (cuuint64_t)G.nx * G.ny * 4, (cuuint64_t)G.V * 4};
+    const cuuint64_t strides[3] = {(cuuint64_t)G.nx * eb, (cuuint64_t)G.nx * G.ny * eb, (cuuint64_t)G.V * eb};
     const cuuint32_t box[4] = {(cuuint32_t)TX, 1u, (cuuint32_t)tz, (cuuint32_t)planes};
     const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
-    const CUresult r = ((EncodeFn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)fields, dims, strides, box, estr,
+    const CUresult r = ((EncodeFn)fn)(out, elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                                      4, (void*)fields, dims, strides, box, estr,
                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                       CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { if (why) *why = "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")"; return false; }
@@ -81,6 +118,7 @@ struct pcamm_model {
     int M = 0, Bmax = 1, Cmax = 1, S = 1;
     // model (device)
     float *f0 = nullptr, *fields = nullptr, *xbar = nullptr, *u = nullptr, *lm0 = nullptr;   // xbar, u: views of fields
+    __half* u16 = nullptr;          // reduced-precision copy of u (geometry.field_storage = 1), else NULL
     FieldStream fs;
     // scratch (device)
     unsigned char* cellmap = nullptr;   // FieldStream::cellmap
@@ -552,10 +590,62 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     // the streaming kernels' view of the fields: TMA tensor map (else the generic kernels)
     m->fs.fields = m->fields;
     std::string why;
-    m->fs.use_tma = make_field_map(G, m->fields, 3 * (G.K + 1), 32, &m->fs.map32, &why) &&
-                    make_field_map(G, m->fields, 3 * (G.K + 1), 16, &m->fs.map16, &why);
+    m->fs.use_tma = make_field_map(G, m->fields, 3 * (G.K + 1), 32, 4, &m->fs.map32, &why) &&
+                    make_field_map(G, m->fields, 3 * (G.K + 1), 16, 4, &m->fs.map16, &why);
+    if (g->field_storage == 1) {
+        // u_k in half: scale[k] = the power of two that puts max |u_k| (voxel units) into [8192, 16384),
+        // so that entries down to 2^-28 of the largest stay normal halves with 11 significant bits
+        if (G.nx % 8 != 0) { set_error("field_storage = 1 needs nx to be a multiple of 8"); return fail(PCAMM_E_INVALID); }
+        unsigned int* d_max = nullptr;
+        unsigned int h_max[KMAX] = {};
+        cudaError_t e2 = dalloc(m, &m->u16, 3 * (size_t)V * G.K);
+        if (e2 == cudaSuccess) e2 = dalloc(m, &d_max, (size_t)KMAX);
+        if (e2 == cudaSuccess) e2 = cudaMemsetAsync(d_max, 0, sizeof(unsigned int) * KMAX, st);
+        if (e2 == cudaSuccess) {
+            k_field_absmax<<<1184, 256, 0, st>>>(m->u, 3 * V, G.K, d_max);
+            e2 = cudaMemcpyAsync(h_max, d_max, sizeof(unsigned int) * KMAX, cudaMemcpyDeviceToHost, st);
+        }
+        if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(st);
+        if (e2 != cudaSuccess) { set_error(std::string("field quantisation: ") + cudaGetErrorString(e2)); return fail(PCAMM_E_CUDA); }
+        FieldScale scale = {}, inv = {};
+        for (int k = 0; k < KMAX; ++k) {
+            float mx;
+            std::memcpy(&mx, &h_max[k], sizeof(float));
+            int ex = 0;
+            if (k < G.K && mx > 0.f) std::frexp(mx, &ex);       // mx = f * 2^ex, f in [0.5, 1)
+            scale.inv[k] = (k < G.K && mx > 0.f) ? std::ldexp(1.f, 14 - ex) : 1.f;
+            inv.inv[k] = 1.f / scale.inv[k];
+        }
+        k_quantise_fields<<<1184, 256, 0, st>>>(m->u, m->u16, 3 * V, G.K, scale, inv);
+        m->fs.scale = inv;
+        m->fs.u16 = m->u16;
+        m->fs.half_u = make_field_map(G, m->fields, 3, 32, 4, &m->fs.xmap32, &why) &&
+                       make_field_map(G, m->fields, 3, 16, 4, &m->fs.xmap16, &why) &&
+                       make_field_map(G, m->u16, 3 * G.K, 32, 2, &m->fs.umap32, &why) &&
+                       make_field_map(G, m->u16, 3 * G.K, 16, 2, &m->fs.umap16, &why);
+        e2 = cudaStreamSynchronize(st);
+        if (e2 != cudaSuccess || !m->fs.half_u || !m->fs.use_tma) {
+            set_error("field_storage = 1: " + (e2 != cudaSuccess ? std::string(cudaGetErrorString(e2)) : why));
+            return fail(e2 != cudaSuccess ? PCAMM_E_CUDA : PCAMM_E_INVALID);
+        }
+    } else if (g->field_storage != 0) {
+        set_error("geometry.field_storage must be 0 or 1");
+        return fail(PCAMM_E_INVALID);
+    }
     m->c.grad_blocks = grad_blocks(G, m->fs);
     *out = m;
+    return PCAMM_OK;
+}
+
+int pcamm_model_fields(pcamm_model* m, float* mean_dvf_out_dev, float* eig_dvf_out_dev, void* stream) {
+    if (!m || !mean_dvf_out_dev || !eig_dvf_out_dev) return invalid("NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom& G = m->G;
+    k_fields_to_mm<<<1184, 256, 0, st>>>(m->xbar, G.V, 3, G.hx, G.hy, G.hz, mean_dvf_out_dev);
+    k_fields_to_mm<<<1184, 256, 0, st>>>(m->u, G.V, 3 * G.K, G.hx, G.hy, G.hz, eig_dvf_out_dev);
+    count_launch(2);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaStreamSynchronize(st));
     return PCAMM_OK;
 }
 

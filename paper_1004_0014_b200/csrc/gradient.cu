@@ -271,23 +271,25 @@ constexpr size_t grad_queue_bytes() { return (size_t)GradGroups<K>::value * Grad
 template <int K> struct GradStages {
     static constexpr int value = stages_per_group<K>(GradGroups<K>::value, 2, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
 };
-template <int K>
+template <int K, bool H>
 constexpr size_t grad_smem_bytes() {
-    return FieldRing<3 * (K + 1), TileZ<K>::value, GradGroups<K>::value, GradStages<K>::value>::BYTES + 16 + grad_queue_bytes<K>();
+    return FieldRing<3 * (K + 1), TileZ<K>::value, GradGroups<K>::value, GradStages<K>::value, H>::BYTES + 16 + grad_queue_bytes<K>();
 }
 
 // SINGLE: one solve (B = 1): the K sums stay in registers over all tiles of the CTA and are
 // reduced once at the end; otherwise they are reduced per tile and solve.
-template <int K, bool SINGLE>
+// H: u_k stored in half (stream.cuh FieldRing, FieldScale).
+template <int K, bool SINGLE, bool H>
 __global__ void __launch_bounds__(32 * GradGroups<K>::value * GROUP_WARPS, 1)
-k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
+k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
+           const Geom G, const float* __restrict__ f0,
            const unsigned char* __restrict__ cellmap, const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
            const float2* __restrict__ vtab, double* __restrict__ partials) {
     constexpr int P = 3 * (K + 1), GTZ = TileZ<K>::value, GROWS = GTZ / GROUP_WARPS;
     constexpr int RB = GradBatch<K>::value, NB = GROWS / RB;
     static_assert(GROWS % RB == 0 && NB >= 1, "tile rows per thread must be a multiple of the batch");
     constexpr int GNG = GradGroups<K>::value;
-    using Ring = FieldRing<P, GTZ, GNG, GradStages<K>::value>;
+    using Ring = FieldRing<P, GTZ, GNG, GradStages<K>::value, H>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ int s_cnt[GNG][2][32];                      // double buffered over the batches
     __shared__ float s_red[GNG][GROUP_WARPS][K];
@@ -298,7 +300,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
         s_running[b] = solves[b].running;
         s_gv[b] = make_gather_view(G, solves[b].view);
 #pragma unroll
-        for (int k = 0; k < K; ++k) s_w[b][k] = (float)solves[b].w[k];
+        for (int k = 0; k < K; ++k) s_w[b][k] = H ? (float)solves[b].w[k] * scale.inv[k] : (float)solves[b].w[k];
     }
     Ring ring;
     ring.bind(smem_raw);
@@ -322,7 +324,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     if (!any_running) return;                              // uniform over the grid
     const bool leader = gtid == 0;
     const uint64_t policy = l2_evict_first_policy();
-    if (leader) ring.prologue(&fmap, G, n_tiles, group, policy);
+    if (leader) ring.prologue(&fmap, &umap, G, n_tiles, group, policy);
 
     float acc[K];
 #pragma unroll
@@ -357,10 +359,10 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     const int zz = tw * GROWS + ra;
 #pragma unroll
                     for (int cc = 0; cc < 3; ++cc) {
-                        float xs = lds_f32(sf + 4u * ((cc * GTZ + zz) * TX + lane));               // Eq. (1)
+                        float xs = Ring::xbar_at(sf, cc, zz, lane);                                // Eq. (1)
 #pragma unroll
                         for (int k = 0; k < K; ++k)
-                            xs = fmaf(lds_f32(sf + 4u * (((3 + 3 * k + cc) * GTZ + zz) * TX + lane)), w[k], xs);
+                            xs = fmaf(Ring::u_at(sf, k, cc, zz, lane), w[k], xs);
                         dda[ra][cc] = xs;
                     }
                     const int ci = x + (int)floorf(dda[ra][0]) + 1, cj = c.y + (int)floorf(dda[ra][1]) + 1,
@@ -409,10 +411,11 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                             float gx, gy, gz;
                             grad8(taps[rr], cv[rr], &gx, &gy, &gz);
 #pragma unroll
-                            for (int k = 0; k < K; ++k)
-                                q[rr][k] = gx * lds_f32(sf + 4u * (((3 + 3 * k + 0) * GTZ + zz) * TX + lane)) +
-                                           gy * lds_f32(sf + 4u * (((3 + 3 * k + 1) * GTZ + zz) * TX + lane)) +
-                                           gz * lds_f32(sf + 4u * (((3 + 3 * k + 2) * GTZ + zz) * TX + lane));
+                            for (int k = 0; k < K; ++k) {
+                                q[rr][k] = gx * Ring::u_at(sf, k, 0, zz, lane) + gy * Ring::u_at(sf, k, 1, zz, lane) +
+                                           gz * Ring::u_at(sf, k, 2, zz, lane);
+                                if (H) q[rr][k] *= scale.inv[k];      // power of two: exact
+                            }
                             const bool active = flag[rr] != 0 && (gx != 0.f || gy != 0.f || gz != 0.f);
                             masks[rr] = __ballot_sync(0xffffffffu, active);
                         }
@@ -423,7 +426,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     }
                     group_barrier(group);
                     if (SINGLE && bt == NB - 1 && leader)                   // no more reads of the stage: refill it
-                        ring.issue(&fmap, G, n_tiles, group, j + GradStages<K>::value, policy);
+                        ring.issue(&fmap, &umap, G, n_tiles, group, j + GradStages<K>::value, policy);
                     // 2. compaction in the fixed order (row, warp, lane), appended to the queue
                     int cnt = lane < RB * GROUP_WARPS ? s_cnt[group][parity][lane] : 0, incl = cnt;
                     parity ^= 1;
@@ -489,7 +492,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
             }
             if (!SINGLE) {
                 group_barrier(group);                       // every thread of the group is done with the stage
-                if (leader) ring.issue(&fmap, G, n_tiles, group, j + GradStages<K>::value, policy);
+                if (leader) ring.issue(&fmap, &umap, G, n_tiles, group, j + GradStages<K>::value, policy);
             }
         }
     }
@@ -562,32 +565,39 @@ k_backproject(const Geom G, const SolveState* __restrict__ solves, const float* 
     out[lin] = gather_voxel(G, gv, rL, utab, vtab, xw, yw, zw);
 }
 
+template <int K, bool H>
+void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
+                const float* rL, const float4* utab, const float2* vtab, double* partials) {
+    static bool configured = false;
+    constexpr size_t smem = grad_smem_bytes<K, H>();
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_grad_tma<K, true, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_grad_tma<K, false, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) { q.err = e; return; }
+        configured = true;
+    }
+    constexpr int GNG = GradGroups<K>::value, GTHREADS = 32 * GNG * GROUP_WARPS;
+    const int grid = grad_grid(G, fs), nslot = grid * GNG;
+    if (B == 1) {
+        q.launch(k_grad_tma<K, true, H>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, G, f0,
+                 fs.cellmap, solves, 1, rL, utab, vtab, partials);
+        return;
+    }
+    for (int b0 = 0; b0 < B; b0 += SOLVE_CACHE) {       // the kernel keeps up to SOLVE_CACHE solves' constants on chip
+        const int nb = B - b0 < SOLVE_CACHE ? B - b0 : SOLVE_CACHE;
+        q.launch(k_grad_tma<K, false, H>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, G, f0,
+                 fs.cellmap, solves + b0, nb, rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu,
+                 vtab + (long long)b0 * G.nv, partials + (long long)b0 * nslot * KMAX);
+    }
+}
+
 template <int K>
 void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
               const float* rL, const float4* utab, const float2* vtab, double* partials) {
     if (fs.use_tma) {
-        static bool configured = false;
-        constexpr size_t smem = grad_smem_bytes<K>();
-        if (!configured) {
-            cudaError_t e = cudaFuncSetAttribute(k_grad_tma<K, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e == cudaSuccess)
-                e = cudaFuncSetAttribute(k_grad_tma<K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) { q.err = e; return; }
-            configured = true;
-        }
-        constexpr int GNG = GradGroups<K>::value, GTHREADS = 32 * GNG * GROUP_WARPS;
-        const int grid = grad_grid(G, fs), nslot = grid * GNG;
-        if (B == 1) {
-            q.launch(k_grad_tma<K, true>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), G, f0, fs.cellmap, solves, 1, rL, utab, vtab,
-                     partials);
-            return;
-        }
-        for (int b0 = 0; b0 < B; b0 += SOLVE_CACHE) {       // the kernel keeps up to SOLVE_CACHE solves' constants on chip
-            const int nb = B - b0 < SOLVE_CACHE ? B - b0 : SOLVE_CACHE;
-            q.launch(k_grad_tma<K, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), G, f0, fs.cellmap, solves + b0, nb,
-                     rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu, vtab + (long long)b0 * G.nv,
-                     partials + (long long)b0 * nslot * KMAX);
-        }
+        if (fs.half_u) launch_tma<K, true>(q, G, fs, f0, solves, B, rL, utab, vtab, partials);
+        else launch_tma<K, false>(q, G, fs, f0, solves, B, rL, utab, vtab, partials);
         return;
     }
     dim3 grid((G.nx + TILE - 1) / TILE, (G.ny + TILE - 1) / TILE, G.nz);

@@ -14,6 +14,7 @@
 #pragma once
 
 #include <cuda.h>
+#include <cuda_fp16.h>
 
 #include <string>
 
@@ -97,6 +98,11 @@ __device__ __forceinline__ float lds_f32(uint32_t addr) {
     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
     return v;
 }
+__device__ __forceinline__ float lds_f16(uint32_t addr) {
+    unsigned short h;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(h) : "r"(addr));
+    return __half2float(__ushort_as_half(h));
+}
 __device__ __forceinline__ void group_barrier(int group) {
     asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(GROUP_THREADS) : "memory");
 }
@@ -110,25 +116,38 @@ __device__ __forceinline__ void group_barrier(int group) {
 // "empty" barrier and no producer warp are needed, and waiting on the phase parity of the "full"
 // barrier is sound (a group sharing stages with others could be a whole ring cycle ahead of the
 // barrier it polls and mistake the previous phase for its own).
-template <int P, int TZ, int NG, int SPG>
+//
+// H (reduced-precision storage): the stage holds xbar's three planes in float and
+// the 3K planes of u_1 .. u_K in half (each u_k scaled by a power of two, common.cuh FieldScale),
+// filled by two TMA loads from two tensors that complete on the same barrier.
+template <int P, int TZ, int NG, int SPG, bool H = false>
 struct FieldRing {
     static constexpr int NS = NG * SPG;
-    static constexpr int STAGE_FLOATS = P * TZ * TX;
-    static constexpr uint32_t STAGE_BYTES = STAGE_FLOATS * 4u;
+    static constexpr uint32_t XBAR_BYTES = 3u * TZ * TX * 4u;
+    static constexpr uint32_t STAGE_BYTES = H ? XBAR_BYTES + (uint32_t)(P - 3) * TZ * TX * 2u : (uint32_t)P * TZ * TX * 4u;
     static constexpr size_t BYTES = (size_t)NS * STAGE_BYTES + NS * sizeof(uint64_t);
 
-    float* data;        // 128 B aligned
-    uint64_t* full;     // [NS] TMA completion
+    unsigned char* data;   // 128 B aligned
+    uint64_t* full;        // [NS] TMA completion
 
     __device__ __forceinline__ void bind(unsigned char* smem) {
-        data = reinterpret_cast<float*>(smem);
+        data = smem;
         full = reinterpret_cast<uint64_t*>(smem + (size_t)NS * STAGE_BYTES);
     }
     __device__ __forceinline__ void init() {   // one thread
         for (int s = 0; s < NS; ++s) mbar_init(full + s, 1);
         mbar_fence_init();
     }
-    __device__ __forceinline__ const float* stage(int s) const { return data + (size_t)s * STAGE_FLOATS; }
+    __device__ __forceinline__ const unsigned char* stage(int s) const { return data + (size_t)s * STAGE_BYTES; }
+
+    // Shared-memory reads of a stage at byte address sf: component cc of xbar / of u_k at row zz, column x.
+    __device__ __forceinline__ static float xbar_at(uint32_t sf, int cc, int zz, int x) {
+        return lds_f32(sf + 4u * ((cc * TZ + zz) * TX + x));
+    }
+    __device__ __forceinline__ static float u_at(uint32_t sf, int k, int cc, int zz, int x) {
+        if (H) return lds_f16(sf + XBAR_BYTES + 2u * (((3 * k + cc) * TZ + zz) * TX + x));
+        return lds_f32(sf + 4u * (((3 + 3 * k + cc) * TZ + zz) * TX + x));
+    }
 
     // Tile of the volume that is group g's j-th tile in this CTA (may be >= the tile count).
     __device__ __forceinline__ static long long tile_of(int g, int j) {
@@ -138,20 +157,29 @@ struct FieldRing {
     __device__ __forceinline__ static uint32_t parity_of(int j) { return (uint32_t)(j / SPG) & 1u; }
 
     // Group leader: start the load of the group's j-th tile (nothing if the volume has no such tile).
-    __device__ __forceinline__ void issue(const CUtensorMap* map, const Geom& G, long long n_tiles, int g, int j,
-                                          uint64_t policy) const {
+    // map: all P planes in float (H = false) or xbar's three planes; umap: the half planes (H only).
+    __device__ __forceinline__ void issue(const CUtensorMap* map, const CUtensorMap* umap, const Geom& G,
+                                          long long n_tiles, int g, int j, uint64_t policy) const {
         const long long t = tile_of(g, j);
         if (t >= n_tiles) return;
         const int s = stage_of(g, j);
         const TileCoord c = tile_coord(G, TZ, t);
         mbar_arrive_expect_tx(full + s, STAGE_BYTES);
-        tma_load_4d(data + (size_t)s * STAGE_FLOATS, map, full + s, c.x0, c.y, c.z0, 0, policy);
+        tma_load_4d(data + (size_t)s * STAGE_BYTES, map, full + s, c.x0, c.y, c.z0, 0, policy);
+        if (H) tma_load_4d(data + (size_t)s * STAGE_BYTES + XBAR_BYTES, umap, full + s, c.x0, c.y, c.z0, 0, policy);
     }
     // Group leader, once: the first SPG tiles.
-    __device__ __forceinline__ void prologue(const CUtensorMap* map, const Geom& G, long long n_tiles, int g,
-                                             uint64_t policy) const {
-        for (int j = 0; j < SPG; ++j) issue(map, G, n_tiles, g, j, policy);
+    __device__ __forceinline__ void prologue(const CUtensorMap* map, const CUtensorMap* umap, const Geom& G,
+                                             long long n_tiles, int g, uint64_t policy) const {
+        for (int j = 0; j < SPG; ++j) issue(map, umap, G, n_tiles, g, j, policy);
     }
+};
+
+// Reduced-precision storage of u_k: half(u_k / h * scale[k]), scale a power of two chosen at
+// model_create so that the largest entry of u_k lands in [0.25, 0.5); inv[k] = 1 / scale[k].
+// Eq. (1) then uses w_k * inv[k] (exact), and the K gradient sums are multiplied by inv[k].
+struct FieldScale {
+    float inv[KMAX];
 };
 
 // What the streaming kernels need to know about the model's fields.
@@ -160,6 +188,12 @@ struct FieldStream {
     bool use_tma = false;            // false: register-staged generic kernels
     int n_sm = 1;                    // persistent grid size
     CUtensorMap map32, map16;        // boxes {TX, 1, 32 | 16, 3(K+1)}
+    // reduced-precision storage: u_k in half, xbar in float
+    bool half_u = false;
+    const __half* u16 = nullptr;     // [3K][V]
+    CUtensorMap xmap32, xmap16;      // xbar alone, boxes {TX, 1, 32 | 16, 3} of float
+    CUtensorMap umap32, umap16;      // u16, boxes {TX, 1, 32 | 16, 3K} of half
+    FieldScale scale = {};
     // one byte per interpolation cell (i0, j0, k0) in [-1, n-1]^3, element
     // ((k0+1)(ny+1) + (j0+1))(nx+1) + (i0+1): 0 if the cell's eight zero-padded taps of f0 are all
     // equal (then the image gradient is exactly 0 anywhere in the cell), else 1 (gradient.cu)
@@ -178,12 +212,20 @@ constexpr int stages_per_group(int n_groups, int max_spg, int budget_bytes) {
 }
 template <int K>
 __host__ __device__ __forceinline__ const CUtensorMap& field_map(const FieldStream& fs) {
+    if (fs.half_u) return TileZ<K>::value == 32 ? fs.xmap32 : fs.xmap16;
     return TileZ<K>::value == 32 ? fs.map32 : fs.map16;
+}
+template <int K>
+__host__ __device__ __forceinline__ const CUtensorMap& half_map(const FieldStream& fs) {
+    if (!fs.half_u) return field_map<K>(fs);      // unused by the kernels then
+    return TileZ<K>::value == 32 ? fs.umap32 : fs.umap16;
 }
 
 // Host: the tensor map of the fields [P][nz][ny][nx] (xbar's three planes first, then u_1 .. u_K)
 // with box {TX, 1, tz, P}.  Returns false if the driver entry point is missing or the shape
 // cannot be described (nx * 4 must be a multiple of 16 bytes).
-bool make_field_map(const Geom& G, const float* fields, int planes, int tz, CUtensorMap* out, std::string* why);
+// elem_bytes 4: float planes; 2: half planes.
+bool make_field_map(const Geom& G, const void* fields, int planes, int tz, int elem_bytes, CUtensorMap* out,
+                    std::string* why);
 
 }  // namespace pcamm

@@ -123,18 +123,20 @@ constexpr int WTHREADS = 32 * WNG * GROUP_WARPS;
 constexpr int WSTATIC = 16 * 1024; // static shared memory of the kernel (transposition tiles, slot cache), rounded up
 template <int K> struct WarpStages { static constexpr int value = stages_per_group<K>(WNG, 2, 227 * 1024 - WSTATIC - 64); };
 
-template <int K>
+template <int K, bool H>
 constexpr size_t warp_smem_bytes() {
-    return FieldRing<3 * (K + 1), TileZ<K>::value, WNG, WarpStages<K>::value>::BYTES;
+    return FieldRing<3 * (K + 1), TileZ<K>::value, WNG, WarpStages<K>::value, H>::BYTES;
 }
 
-template <int K, bool RAY>
+// H: u_k stored in half (stream.cuh FieldRing, FieldScale)
+template <int K, bool RAY, bool H>
 __global__ void __launch_bounds__(WTHREADS, 1)
-k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* __restrict__ f0,
+k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
+           const Geom G, const float* __restrict__ f0,
            const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride,
            unsigned char* __restrict__ occ) {
     constexpr int P = 3 * (K + 1), WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
-    using Ring = FieldRing<P, WTZ, WNG, WarpStages<K>::value>;
+    using Ring = FieldRing<P, WTZ, WNG, WarpStages<K>::value, H>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ float tiles[WNG][WTZ][TX + 1];
     __shared__ int s_occ[WNG][2][TX];                      // per group: column x has something in z block 0 / 1
@@ -143,7 +145,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     for (int i = threadIdx.x; i < nslots && i < SLOT_CACHE; i += blockDim.x) {
         s_active[i] = slots[i].active;
 #pragma unroll
-        for (int k = 0; k < K; ++k) s_w[i][k] = slots[i].w[k];
+        for (int k = 0; k < K; ++k) s_w[i][k] = H ? slots[i].w[k] * scale.inv[k] : slots[i].w[k];
     }
     Ring ring;
     ring.bind(smem_raw);
@@ -162,7 +164,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     const bool leader = tw == 0 && lane == 0;
     const uint64_t policy = l2_evict_first_policy();
     float(*tile)[TX + 1] = tiles[group];
-    if (leader) ring.prologue(&fmap, G, n_tiles, group, policy);
+    if (leader) ring.prologue(&fmap, &umap, G, n_tiles, group, policy);
     int j = 0;                                             // this group's tile counter
     for (long long t = Ring::tile_of(group, 0); t < n_tiles; t += (long long)WNG * gridDim.x, ++j) {
         {
@@ -187,16 +189,16 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
                     float d[3];
 #pragma unroll
                     for (int cc = 0; cc < 3; ++cc) {
-                        float xs = lds_f32(sf + 4u * ((cc * WTZ + zz) * TX + lane));               // Eq. (1)
+                        float xs = Ring::xbar_at(sf, cc, zz, lane);                                // Eq. (1)
 #pragma unroll
-                        for (int k = 0; k < K; ++k) xs = fmaf(lds_f32(sf + 4u * (((3 + 3 * k + cc) * WTZ + zz) * TX + lane)), w[k], xs);
+                        for (int k = 0; k < K; ++k) xs = fmaf(Ring::u_at(sf, k, cc, zz, lane), w[k], xs);
                         d[cc] = xs;
                     }
                     taps[r] = make_taps(G.nx, G.ny, G.nz, x, c.y, z, d[0], d[1], d[2]);
                 }
                 if (sl == last_active) {                    // the fields of this tile are in registers: refill the
                     group_barrier(group);                   // stage while the gathers are under way
-                    if (leader) ring.issue(&fmap, G, n_tiles, group, j + WarpStages<K>::value, policy);
+                    if (leader) ring.issue(&fmap, &umap, G, n_tiles, group, j + WarpStages<K>::value, policy);
                 }
                 float cv[WROWS][8];
 #pragma unroll
@@ -237,13 +239,16 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const Geom G, const float* 
     }
 }
 
-template <int K, bool RAY>
-void launch_tma(Seq& q, const Geom& G, const CUtensorMap& fmap, int n_sm, const float* f0, const SlotState* slots,
+template <int K, bool RAY, bool H>
+void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots,
                 int nslots, float* vol_out, long long slot_stride, unsigned char* occ) {
     static bool configured = false;
-    constexpr size_t smem = warp_smem_bytes<K>();
+    constexpr size_t smem = warp_smem_bytes<K, H>();
+    const CUtensorMap& fmap = field_map<K>(fs);
+    const CUtensorMap& umap = half_map<K>(fs);
+    const int n_sm = fs.n_sm;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_warp_tma<K, RAY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(k_warp_tma<K, RAY, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) { q.err = e; return; }
         configured = true;
     }
@@ -251,7 +256,7 @@ void launch_tma(Seq& q, const Geom& G, const CUtensorMap& fmap, int n_sm, const 
     const int grid = (int)(nt < n_sm ? nt : n_sm);
     for (int s0 = 0; s0 < nslots; s0 += SLOT_CACHE) {      // the kernel keeps up to SLOT_CACHE slots' coefficients on chip
         const int ns = nslots - s0 < SLOT_CACHE ? nslots - s0 : SLOT_CACHE;
-        q.launch(k_warp_tma<K, RAY>, dim3(grid), dim3(WTHREADS), smem, fmap, G, f0, slots + s0, ns,
+        q.launch(k_warp_tma<K, RAY, H>, dim3(grid), dim3(WTHREADS), smem, fmap, umap, fs.scale, G, f0, slots + s0, ns,
                  vol_out + (long long)s0 * slot_stride, slot_stride, occ ? occ + (long long)s0 * G.OCC : occ);
     }
 }
@@ -260,8 +265,13 @@ template <int K>
 void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
               int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ) {
     if (fs.use_tma) {
-        if (ray_layout) launch_tma<K, true>(q, G, field_map<K>(fs), fs.n_sm, f0, slots, nslots, vol_out, slot_stride, occ);
-        else launch_tma<K, false>(q, G, field_map<K>(fs), fs.n_sm, f0, slots, nslots, vol_out, slot_stride, occ);
+        if (fs.half_u) {
+            if (ray_layout) launch_tma<K, true, true>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ);
+            else launch_tma<K, false, true>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ);
+        } else {
+            if (ray_layout) launch_tma<K, true, false>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ);
+            else launch_tma<K, false, false>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ);
+        }
         return;
     }
     const float* xbar = fs.fields;

@@ -74,12 +74,14 @@ def solver_iterations(cfg) -> int:
     return cfg.iterations
 
 
-def algorithmic_bytes(cfg):
-    """what the method must move per launch, f0 gathers counted once."""
+def algorithmic_bytes(cfg, field_storage=0):
+    """what the method must move per launch, f0 gathers counted once.
+    field_storage = 1: the u_k planes are halves (6 K bytes per voxel instead of 12 K)."""
     V, K, npix = cfg.V, cfg.K, cfg.npix
-    return {"warp": (12 * (K + 1) + 4 + 4) * V,
+    fields = 12 * (K + 1) if field_storage == 0 else 12 + 6 * K
+    return {"warp": (fields + 4 + 4) * V,
             "project": 4 * V + 4 * npix,
-            "gradient": (12 * (K + 1) + 4) * V + 4 * npix}
+            "gradient": (fields + 4) * V + 4 * npix}
 
 
 def measured_traffic():
@@ -232,7 +234,7 @@ def run_reference(args, cfg, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def config_dict(cfg, iterations, fan=1):
+def config_dict(cfg, iterations, fan=1, field_storage=0):
     return {"workload": f"{cfg.name}: volume {cfg.nx}x{cfg.ny}x{cfg.nz} @ {cfg.hx} mm, K={cfg.K}, detector "
                         f"{cfg.nu}x{cfg.nv} @ {cfg.pu} mm, consecutive projections 1 deg / (1/6) s apart from frame "
                         f"{FIRST_FRAME}, {cfg.noise} noise, {'irregular' if cfg.irregular else 'regular'} breathing "
@@ -242,7 +244,7 @@ def config_dict(cfg, iterations, fan=1):
                            ("sequential Armijo backtracking" if fan <= 1 else
                             f"Armijo backtracking, {fan} candidate steps per pass (same accepted step as sequential)"),
             "l2": "inputs larger than L2: every pass streams the (K+1) vector fields "
-                  f"({12 * (cfg.K + 1) * cfg.V / 2**20:.0f} MiB) through a 126 MB L2",
+                  f"({(12 * (cfg.K + 1) if field_storage == 0 else 12 + 6 * cfg.K) * cfg.V / 2**20:.0f} MiB) through a 126 MB L2",
             "parallelism": "replicas"}
 
 
@@ -274,7 +276,8 @@ def run_ours(args, cfg, rank, local_rank, world):
     C = 8 if cfg.batched_linesearch else max(fan, 1)
     m = pc.Model(nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, hx=cfg.hx, hy=cfg.hy, hz=cfg.hz, K=cfg.K, nu=cfg.nu, nv=cfg.nv,
                  pu=cfg.pu, pv=cfg.pv, f0=t(wl.f0), mean_dvf=t(wl.model.mean), eig_dvf=t(wl.model.eig),
-                 landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=C, max_batch=B)
+                 landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=C, max_batch=B,
+                 field_storage=args.field_storage)
     # measured projections: the scanner is simulated with the library's own projector applied to
     # the ground-truth volume, plus seeded noise (the CPU arm simulates its own with the oracle)
     ys_host, ys_dev = [], []
@@ -365,9 +368,9 @@ def run_ours(args, cfg, rank, local_rank, world):
         m.time_kernel(which, 3)
     kt = {name: m.time_kernel(which, 20) for which, name in ((0, "warp"), (1, "project"), (2, "gradient"))}
     nl = {"warp": trials + 1, "project": trials + 1, "gradient": tr.iters}
-    ab = algorithmic_bytes(cfg)
+    ab = algorithmic_bytes(cfg, args.field_storage)
     peak, peak_src = measured_peak_gbs()
-    traffic = measured_traffic().get(cfg.name, {})
+    traffic = measured_traffic().get(cfg.name if args.field_storage == 0 else cfg.name + "_half_u", {})
     per_kernel = {k: {"bound": "hbm", "ms": kt[k], "launches_per_solve": nl[k], "algorithmic_bytes": ab[k],
                       "achieved": ab[k] / (kt[k] * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                       "frac": ab[k] / (kt[k] * 1e-3) / 1e9 / peak, "traffic": traffic.get(k)}
@@ -415,7 +418,10 @@ def run_ours(args, cfg, rank, local_rank, world):
     line = {"metric": METRIC, "value": ms_per_solve, "unit": "ms", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": dict(config_dict(cfg, it, fan), in_flight=B), "projections_per_s": 1e3 * args.steps * world * B / elapsed_ms,
+            "config": dict(config_dict(cfg, it, fan, args.field_storage), in_flight=B,
+                           field_storage="float32" if args.field_storage == 0 else
+                           "u_k stored as float16 with a power-of-two scale per field, x-bar float32, arithmetic float32 "
+                           "(SURVEY 8(f).4; NOT the headline configuration)"), "projections_per_s": 1e3 * args.steps * world * B / elapsed_ms,
             "clocks": clocks,
             "e2e": {"value": e2e_ms / (args.steps * world * B), "unit": "ms", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
@@ -551,6 +557,8 @@ def main():
     ap.add_argument("--frames-study", action="store_true",
                     help="instead of the bench line: iterations and ms per solve of the frame stream under each "
                          "start predictor (pcamm_frames_*), stopping on ||g|| <= --grad-tol")
+    ap.add_argument("--field-storage", type=int, default=0, choices=[0, 1],
+                    help="pcamm_geometry.field_storage: 0 float32 fields (the headline configuration), 1 u_k in half")
     ap.add_argument("--pca-study", action="store_true",
                     help="instead of the bench line: pcamm_pca_fit on the config's training DVFs (device time of its "
                          "two passes against their algorithmic bytes)")

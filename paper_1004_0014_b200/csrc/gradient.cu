@@ -268,12 +268,12 @@ struct QueueEntry {
 template <int K> struct GradQueueCap { static constexpr int value = GROUP_THREADS * (GradBatch<K>::value + 1); };
 template <int K>
 constexpr size_t grad_queue_bytes() { return (size_t)GradGroups<K>::value * GradQueueCap<K>::value * sizeof(QueueEntry<K>); }
-template <int K> struct GradStages {
-    static constexpr int value = stages_per_group<K>(GradGroups<K>::value, 2, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
+template <int K, bool H> struct GradStages {
+    static constexpr int value = stages_per_group<K, H>(GradGroups<K>::value, 2, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
 };
 template <int K, bool H>
 constexpr size_t grad_smem_bytes() {
-    return FieldRing<3 * (K + 1), TileZ<K>::value, GradGroups<K>::value, GradStages<K>::value, H>::BYTES + 16 + grad_queue_bytes<K>();
+    return FieldRing<3 * (K + 1), TileZ<K>::value, GradGroups<K>::value, GradStages<K, H>::value, H>::BYTES + 16 + grad_queue_bytes<K>();
 }
 
 // SINGLE: one solve (B = 1): the K sums stay in registers over all tiles of the CTA and are
@@ -289,7 +289,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     constexpr int RB = GradBatch<K>::value, NB = GROWS / RB;
     static_assert(GROWS % RB == 0 && NB >= 1, "tile rows per thread must be a multiple of the batch");
     constexpr int GNG = GradGroups<K>::value;
-    using Ring = FieldRing<P, GTZ, GNG, GradStages<K>::value, H>;
+    using Ring = FieldRing<P, GTZ, GNG, GradStages<K, H>::value, H>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ int s_cnt[GNG][2][32];                      // double buffered over the batches
     __shared__ float s_red[GNG][GROUP_WARPS][K];
@@ -426,7 +426,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                     }
                     group_barrier(group);
                     if (SINGLE && bt == NB - 1 && leader)                   // no more reads of the stage: refill it
-                        ring.issue(&fmap, &umap, G, n_tiles, group, j + GradStages<K>::value, policy);
+                        ring.issue(&fmap, &umap, G, n_tiles, group, j + GradStages<K, H>::value, policy);
                     // 2. compaction in the fixed order (row, warp, lane), appended to the queue
                     int cnt = lane < RB * GROUP_WARPS ? s_cnt[group][parity][lane] : 0, incl = cnt;
                     parity ^= 1;
@@ -492,7 +492,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
             }
             if (!SINGLE) {
                 group_barrier(group);                       // every thread of the group is done with the stage
-                if (leader) ring.issue(&fmap, &umap, G, n_tiles, group, j + GradStages<K>::value, policy);
+                if (leader) ring.issue(&fmap, &umap, G, n_tiles, group, j + GradStages<K, H>::value, policy);
             }
         }
     }

@@ -204,9 +204,9 @@ struct FieldStream {
 // ring has to fit in 227 KB of shared memory next to the kernel's own buffers.
 template <int K> struct TileZ { static constexpr int value = K <= 4 ? 32 : 16; };
 // stages per consumer group that fit into budget_bytes, at most max_spg
-template <int K>
+template <int K, bool H = false>
 constexpr int stages_per_group(int n_groups, int max_spg, int budget_bytes) {
-    const int stage = 3 * (K + 1) * TileZ<K>::value * TX * 4;
+    const int stage = (H ? 12 + 6 * K : 12 * (K + 1)) * TileZ<K>::value * TX;
     const int n = budget_bytes / stage / n_groups;
     return n < max_spg ? (n < 1 ? 1 : n) : max_spg;
 }

@@ -121,11 +121,11 @@ constexpr int SLOT_CACHE = 64;     // slots whose coefficients are kept in share
 constexpr int WTHREADS = 32 * WNG * GROUP_WARPS;
 
 constexpr int WSTATIC = 16 * 1024; // static shared memory of the kernel (transposition tiles, slot cache), rounded up
-template <int K> struct WarpStages { static constexpr int value = stages_per_group<K>(WNG, 2, 227 * 1024 - WSTATIC - 64); };
+template <int K, bool H> struct WarpStages { static constexpr int value = stages_per_group<K, H>(WNG, 2, 227 * 1024 - WSTATIC - 64); };
 
 template <int K, bool H>
 constexpr size_t warp_smem_bytes() {
-    return FieldRing<3 * (K + 1), TileZ<K>::value, WNG, WarpStages<K>::value, H>::BYTES;
+    return FieldRing<3 * (K + 1), TileZ<K>::value, WNG, WarpStages<K, H>::value, H>::BYTES;
 }
 
 // H: u_k stored in half (stream.cuh FieldRing, FieldScale)
@@ -136,7 +136,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
            const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride,
            unsigned char* __restrict__ occ) {
     constexpr int P = 3 * (K + 1), WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
-    using Ring = FieldRing<P, WTZ, WNG, WarpStages<K>::value, H>;
+    using Ring = FieldRing<P, WTZ, WNG, WarpStages<K, H>::value, H>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ float tiles[WNG][WTZ][TX + 1];
     __shared__ int s_occ[WNG][2][TX];                      // per group: column x has something in z block 0 / 1
@@ -198,7 +198,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                 }
                 if (sl == last_active) {                    // the fields of this tile are in registers: refill the
                     group_barrier(group);                   // stage while the gathers are under way
-                    if (leader) ring.issue(&fmap, &umap, G, n_tiles, group, j + WarpStages<K>::value, policy);
+                    if (leader) ring.issue(&fmap, &umap, G, n_tiles, group, j + WarpStages<K, H>::value, policy);
                 }
                 float cv[WROWS][8];
 #pragma unroll

@@ -45,6 +45,14 @@ __global__ void k_fields_to_voxel_units(float* __restrict__ fields, long long V,
     }
 }
 
+// f0 with a border of two zero voxels on every side (trilinear.cuh); out is zeroed beforehand.
+__global__ void k_pad_f0(const float* __restrict__ f0, Geom G, float* __restrict__ out) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < G.V; i += (long long)gridDim.x * blockDim.x) {
+        const int x = (int)(i % G.nx), y = (int)((i / G.nx) % G.ny), z = (int)(i / ((long long)G.nx * G.ny));
+        out[((long long)(z + 2) * G.fny + (y + 2)) * G.fnx + (x + 2)] = f0[i];
+    }
+}
+
 // Reduced-precision storage.  max |u_k| per eigenvector field (bit pattern of a
 // non-negative float orders like an unsigned integer).
 __global__ void k_field_absmax(const float* __restrict__ u, long long n_per_k, int K, unsigned int* __restrict__ out) {
@@ -117,6 +125,7 @@ struct pcamm_model {
     Geom G;
     int M = 0, Bmax = 1, Cmax = 1, S = 1;
     // model (device)
+    float* f0p = nullptr;           // f0 with its zero border: what the warp and gradient kernels gather from
     float *f0 = nullptr, *fields = nullptr, *xbar = nullptr, *u = nullptr, *lm0 = nullptr;   // xbar, u: views of fields
     __half* u16 = nullptr;          // reduced-precision copy of u (geometry.field_storage = 1), else NULL
     FieldStream fs;
@@ -240,20 +249,20 @@ void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     launch_ysums(q, G, m->c, B);
     launch_begin(q, G, m->c, 0);
     launch_view_tables(q, G, m->c.solves, B, m->col_hdr, m->slab_tab);
-    launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
+    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
     launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_INIT, h_iter, use_cond);
 }
 
 void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial, int use_cond) {
     const Geom& G = m->G;
     launch_resid(q, G, m->c.solves, m->c.in, B, 0, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_grad(q, G, m->fs, m->f0, m->c.solves, B, m->rL, m->utab, m->vtab, m->c.grad_part);
+    launch_grad(q, G, m->fs, m->f0p, m->c.solves, B, m->rL, m->utab, m->vtab, m->c.grad_part);
     launch_ctl_grad(q, G, m->c, h_trial, use_cond);
 }
 
 void seq_trial(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_trial, int use_cond) {
     const Geom& G = m->G;
-    launch_warp(q, G, m->fs, m->f0, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
+    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
     launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_TRIAL, h_trial, use_cond);
 }
 
@@ -356,7 +365,7 @@ int solve_impl(pcamm_model* m, int B, const float* y_dev, const float* angles, c
     if (volumes_out) {
         Seq q;
         q.stream = st;
-        launch_warp(q, G, m->fs, m->f0, m->out_slots, B, 0, volumes_out, G.V, nullptr);
+        launch_warp(q, G, m->fs, m->f0p, m->out_slots, B, 0, volumes_out, G.V, nullptr);
         if ((rc = check_seq(q, "final warp"))) return rc;
     }
     CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState) * B, cudaMemcpyDeviceToHost, st));
@@ -468,7 +477,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     if (g->K < 1 || g->K > KMAX) return invalid("K outside [1, PCAMM_KMAX]");
     if (n_landmarks < 0 || (n_landmarks > 0 && !landmarks_mm_host)) return invalid("landmarks");
     const long long V = (long long)g->nx * g->ny * g->nz;
-    if ((long long)(g->nx + 2) * (g->ny + 2) * g->nz >= (1LL << 31) || (long long)g->nu * g->nv >= (1LL << 31)) return invalid("volume or detector too large");
+    if ((long long)(g->nx + 4) * (g->ny + 4) * (g->nz + 4) >= (1LL << 31) || (long long)g->nu * g->nv >= (1LL << 31)) return invalid("volume or detector too large");
     const int Bmax = g->max_batch < 1 ? 1 : g->max_batch;
     const int Cmax = g->max_candidates < 1 ? 1 : g->max_candidates;
     if (Cmax > MAXBT || Bmax > 4096) return invalid("max_batch / max_candidates too large");
@@ -491,6 +500,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     Geom& G = m->G;
     G.nx = g->nx; G.ny = g->ny; G.nz = g->nz; G.V = V;
     G.pnx = g->nx + 2; G.pny = g->ny + 2; G.PV = (long long)G.pnx * G.pny * g->nz;
+    G.fnx = g->nx + 4; G.fny = g->ny + 4; G.fpp = G.fnx * G.fny;
     G.occ_pitch = ((g->nz + 15) / 16 + 7) / 8 * 8;
     G.OCC = (long long)G.pnx * G.pny * G.occ_pitch;
     G.hx = g->hx; G.hy = g->hy; G.hz = g->hz;
@@ -519,7 +529,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     m->trav_cap = G.nx + G.ny + G.nz + 8;
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return r == cudaSuccess; };
-    ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->cellmap, (size_t)(g->nx + 1) * (g->ny + 1) * (g->nz + 1))) && ok(dalloc(m, &m->fields, 3 * (size_t)V * (G.K + 1))) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
+    ok(dalloc(m, &m->f0, (size_t)V)) && ok(dalloc(m, &m->f0p, (size_t)(g->nx + 4) * (g->ny + 4) * (g->nz + 4))) && ok(dalloc(m, &m->cellmap, (size_t)(g->nx + 1) * (g->ny + 1) * (g->nz + 1))) && ok(dalloc(m, &m->fields, 3 * (size_t)V * (G.K + 1))) && ok(dalloc(m, &m->lm0, 3 * (size_t)(m->M > 0 ? m->M : 1))) &&
         ok(dalloc(m, &m->vol, S * (size_t)G.PV)) && ok(dalloc(m, &m->occ, S * (size_t)G.OCC)) && ok(dalloc(m, &m->col_hdr, B * G.nu)) &&
         ok(dalloc(m, &m->slab_tab, B * G.nu * (size_t)max_slabs(G))) && ok(dalloc(m, &m->p, S * G.npix)) && ok(dalloc(m, &m->pseg, S * G.npix * (size_t)project_segments(G))) &&
         ok(dalloc(m, &m->rL, B * G.npix)) && ok(dalloc(m, &m->utab, B * G.nu)) && ok(dalloc(m, &m->vtab, B * G.nv)) &&
@@ -574,6 +584,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     k_count_nonfinite<<<592, 256, 0, st>>>(m->xbar, 3 * V, m->nonfinite);
     k_count_nonfinite<<<592, 256, 0, st>>>(m->u, 3 * V * G.K, m->nonfinite);
     k_fields_to_voxel_units<<<1184, 256, 0, st>>>(m->fields, V, 3 * (G.K + 1), G.hx, G.hy, G.hz);
+    TRY_OR_FAIL(cudaMemsetAsync(m->f0p, 0, sizeof(float) * (size_t)G.fpp * (g->nz + 4), st));
+    k_pad_f0<<<1184, 256, 0, st>>>(m->f0, G, m->f0p);
     launch_build_cellmap(st, G, m->f0, m->cellmap);
     m->fs.cellmap = m->cellmap;
     unsigned long long bad = 0;
@@ -681,7 +693,7 @@ int pcamm_warp(pcamm_model* m, const float* w_host, float* volume_out_dev, void*
     Seq q;
     int rc = hook_begin(m, nullptr, 0.f, w_host, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
-    launch_warp(q, m->G, m->fs, m->f0, m->c.slots, 1, 0, volume_out_dev, m->G.V, nullptr);
+    launch_warp(q, m->G, m->fs, m->f0p, m->c.slots, 1, 0, volume_out_dev, m->G.V, nullptr);
     if ((rc = check_seq(q, "warp"))) return rc;
     CUDA_TRY(cudaStreamSynchronize(st));
     return PCAMM_OK;
@@ -725,10 +737,10 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     if (rc) return rc;
     launch_ysums(q2, G, m->c, 1);
     launch_view_tables(q2, G, m->c.solves, 1, m->col_hdr, m->slab_tab);
-    launch_warp(q2, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
+    launch_warp(q2, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
     launch_project(q2, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_EVAL, 0, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_grad(q2, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
+    launch_grad(q2, G, m->fs, m->f0p, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
     launch_ctl_eval_grad(q2, G, m->c);
     if ((rc = check_seq(q2, "eval"))) return rc;
     if (proj_out_dev) CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * G.npix, cudaMemcpyDeviceToDevice, st));
@@ -801,11 +813,11 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
     CUDA_TRY(cudaEventRecord(m->ev0, st));
     for (int i = 0; i < reps; ++i) {
         if (which == 0)
-            launch_warp(q, G, m->fs, m->f0, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
+            launch_warp(q, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
         else if (which == 1)
             launch_project(q, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0);
         else
-            launch_grad(q, G, m->fs, m->f0, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
+            launch_grad(q, G, m->fs, m->f0p, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
     }
     CUDA_TRY(cudaEventRecord(m->ev1, st));
     int rc = check_seq(q, "time_kernel");

@@ -24,6 +24,7 @@ struct Geom {
     long long PV;             // elements of one ray-layout volume: pnx * pny * nz
     int occ_pitch;            // occupancy bytes per voxel column of the ray layout (one per 16 z, padded to 8)
     long long OCC;            // occupancy bytes of one trial volume: pnx * pny * occ_pitch
+    int fnx, fny, fpp;        // padded f0 (two zero voxels on every side): nx + 4, ny + 4, fnx * fny (trilinear.cuh)
     float hx, hy, hz;
     float ihx, ihy, ihz;      // 1 / h
     float cx, cy, cz;         // world position of the volume centre

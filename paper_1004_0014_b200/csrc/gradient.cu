@@ -147,9 +147,9 @@ __device__ __forceinline__ float gather_voxel(const Geom& G, const GatherView& g
 // displacement (the model's fields are in voxel units, so G . u_k needs no 1/h: (G/h) . (u h) = G . u).
 __device__ __forceinline__ void trilinear_grad(const Geom& G, const float* __restrict__ f0, int i, int j, int k,
                                                float dx, float dy, float dz, float* gx, float* gy, float* gz) {
-    const Taps t = make_taps(G.nx, G.ny, G.nz, i, j, k, dx, dy, dz);
+    const Taps t = make_taps(G, i, j, k, dx, dy, dz);
     float c[8];
-    gather8(f0, t, c);
+    gather8(G, f0, t, c);
     grad8(t, c, gx, gy, gz);
 }
 
@@ -400,11 +400,11 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                         Taps taps[RB];
 #pragma unroll
                         for (int rr = 0; rr < RB; ++rr)
-                            taps[rr] = make_taps(G.nx, G.ny, G.nz, x, c.y, c.z0 + tw * GROWS + bt * RB + rr,
+                            taps[rr] = make_taps(G, x, c.y, c.z0 + tw * GROWS + bt * RB + rr,
                                                  dd[rr][0], dd[rr][1], dd[rr][2]);
                         float cv[RB][8];
 #pragma unroll
-                        for (int rr = 0; rr < RB; ++rr) gather8(f0, taps[rr], cv[rr]);
+                        for (int rr = 0; rr < RB; ++rr) gather8(G, f0, taps[rr], cv[rr]);
 #pragma unroll
                         for (int rr = 0; rr < RB; ++rr) {
                             const int zz = tw * GROWS + bt * RB + rr;

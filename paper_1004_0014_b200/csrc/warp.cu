@@ -32,11 +32,11 @@ constexpr int ROWS = 4;        // voxels per thread (z rows tw, tw+8, tw+16, tw+
 constexpr int NTHREADS = 256;  // 32 x 8
 
 // Trilinear interpolation of f0 at voxel (i,j,k) displaced by d voxels (d = x / h).
-__device__ __forceinline__ float trilinear(const float* __restrict__ f0, int nx, int ny, int nz, int i, int j, int k,
+__device__ __forceinline__ float trilinear(const Geom& G, const float* __restrict__ f0, int i, int j, int k,
                                            float dx, float dy, float dz) {
-    const Taps t = make_taps(nx, ny, nz, i, j, k, dx, dy, dz);
+    const Taps t = make_taps(G, i, j, k, dx, dy, dz);
     float c[8];
-    gather8(f0, t, c);
+    gather8(G, f0, t, c);
     return combine8(t, c);
 }
 
@@ -89,7 +89,7 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
                     for (int k = 0; k < K; ++k) xs = fmaf(uu[r][k][c], w[k], xs);
                     d[c] = xs;
                 }
-                val[r] = trilinear(f0, G.nx, G.ny, G.nz, x, y, z0 + tw + 8 * r, d[0], d[1], d[2]);
+                val[r] = trilinear(G, f0, x, y, z0 + tw + 8 * r, d[0], d[1], d[2]);
             }
         }
         if (!RAY) {
@@ -194,7 +194,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                         for (int k = 0; k < K; ++k) xs = fmaf(Ring::u_at(sf, k, cc, zz, lane), w[k], xs);
                         d[cc] = xs;
                     }
-                    taps[r] = make_taps(G.nx, G.ny, G.nz, x, c.y, z, d[0], d[1], d[2]);
+                    taps[r] = make_taps(G, x, c.y, z, d[0], d[1], d[2]);
                 }
                 if (sl == last_active) {                    // the fields of this tile are in registers: refill the
                     group_barrier(group);                   // stage while the gathers are under way
@@ -202,7 +202,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                 }
                 float cv[WROWS][8];
 #pragma unroll
-                for (int r = 0; r < WROWS; ++r) gather8(f0, taps[r], cv[r]);    // 8 WROWS gathers in flight
+                for (int r = 0; r < WROWS; ++r) gather8(G, f0, taps[r], cv[r]);    // 8 WROWS gathers in flight
 #pragma unroll
                 for (int r = 0; r < WROWS; ++r) val[r] = combine8(taps[r], cv[r]);
                 if (!RAY) {

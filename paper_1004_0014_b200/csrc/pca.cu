@@ -28,7 +28,7 @@ namespace {
 
 constexpr int PCA_NT = 256;
 constexpr int PCA_MAXN = PCAMM_PCA_MAX_SAMPLES;
-constexpr int PCA_RUN = 256;   // elements a thread sums in float before the double reduction
+constexpr int PCA_RUN = 32;    // items (of 1 or 4 elements) a thread sums in float before the double reduction
 
 struct PcaCoef {
     float c[PCAMM_KMAX][PCA_MAXN];   // v_ik / sqrt(lambda_k)

@@ -3,7 +3,7 @@ PCA (SVD of the centred samples in float64) on the training DVFs of the DESIGN.m
 on ragged synthetic samples.
 
 Bars: eigenvalues to 1e-5 relative to the largest; mean to 2 float32 ulp of the
-largest sample value; u_k to 2e-5 in relative L2 (float32 products summed over <= 256-element runs,
+largest sample value; u_k to 2e-5 in relative L2 (float32 products summed over <= 128-element runs,
 double above: rounding errors of random sign, so the scatter matrix is good to about 1e-7 sqrt(n) / n
 of lambda_1, and an eigenvector moves by that error over its eigenvalue gap); training coefficients
 to 2e-5 of sqrt(lambda_1).

@@ -116,26 +116,29 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
 
 // ---------------------------------------------------------------- the TMA-fed kernel
 
-constexpr int WNG = 3;             // consumer groups
+// consumer groups: four where the stages of the 16-slice tiles (K = 5, 6) leave room for them
+// and for the L1 lines of the f0 gathers, else three
+template <int K> struct WarpGroups { static constexpr int value = (K == 5 || K == 6) ? 4 : 3; };
 constexpr int SLOT_CACHE = 64;     // slots whose coefficients are kept in shared memory
-constexpr int WTHREADS = 32 * WNG * GROUP_WARPS;
+template <int K> struct WarpThreads { static constexpr int value = 32 * WarpGroups<K>::value * GROUP_WARPS; };
 
 constexpr int WSTATIC = 16 * 1024; // static shared memory of the kernel (transposition tiles, slot cache), rounded up
-template <int K, bool H> struct WarpStages { static constexpr int value = stages_per_group<K, H>(WNG, 2, 227 * 1024 - WSTATIC - 64); };
+template <int K, bool H> struct WarpStages { static constexpr int value = stages_per_group<K, H>(WarpGroups<K>::value, 2, 227 * 1024 - WSTATIC - 64); };
 
 template <int K, bool H>
 constexpr size_t warp_smem_bytes() {
-    return FieldRing<3 * (K + 1), TileZ<K>::value, WNG, WarpStages<K, H>::value, H>::BYTES;
+    return FieldRing<3 * (K + 1), TileZ<K>::value, WarpGroups<K>::value, WarpStages<K, H>::value, H>::BYTES;
 }
 
 // H: u_k stored in half (stream.cuh FieldRing, FieldScale)
 template <int K, bool RAY, bool H>
-__global__ void __launch_bounds__(WTHREADS, 1)
+__global__ void __launch_bounds__(WarpThreads<K>::value, 1)
 k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
            const Geom G, const float* __restrict__ f0,
            const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride,
            unsigned char* __restrict__ occ) {
     constexpr int P = 3 * (K + 1), WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
+    constexpr int WNG = WarpGroups<K>::value;
     using Ring = FieldRing<P, WTZ, WNG, WarpStages<K, H>::value, H>;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ float tiles[WNG][WTZ][TX + 1];
@@ -256,7 +259,7 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     const int grid = (int)(nt < n_sm ? nt : n_sm);
     for (int s0 = 0; s0 < nslots; s0 += SLOT_CACHE) {      // the kernel keeps up to SLOT_CACHE slots' coefficients on chip
         const int ns = nslots - s0 < SLOT_CACHE ? nslots - s0 : SLOT_CACHE;
-        q.launch(k_warp_tma<K, RAY, H>, dim3(grid), dim3(WTHREADS), smem, fmap, umap, fs.scale, G, f0, slots + s0, ns,
+        q.launch(k_warp_tma<K, RAY, H>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, G, f0, slots + s0, ns,
                  vol_out + (long long)s0 * slot_stride, slot_stride, occ ? occ + (long long)s0 * G.OCC : occ);
     }
 }

@@ -10,6 +10,8 @@ solve consecutive projections of the rotation (1 degree, 1/6 s apart) and each s
 previous frame's coefficients.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config C2]
+    python bench.py --frames-study | --pca-study     (SURVEY 8(f).2 / 8(f).3 measurements; their own JSON line)
+    python bench.py --field-storage 1                (u_k stored in half; not the headline)
 
 N > 1 (under torchrun): replicas only -- every rank holds the model and solves its own contiguous
 block of K projections; no data-path collective; scaling is weak.

@@ -77,6 +77,18 @@ __global__ void k_quantise_fields(float* __restrict__ u, __half* __restrict__ u1
         u[i] = __half2float(h) * inv.inv[k];
     }
 }
+// max |value| of every plane of the fields (voxel units).
+__global__ void k_plane_absmax(const float* __restrict__ fields, long long V, int planes, unsigned int* __restrict__ out) {
+    for (int p = 0; p < planes; ++p) {
+        float mx = 0.f;
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long long)gridDim.x * blockDim.x)
+            mx = fmaxf(mx, fabsf(fields[(long long)p * V + i]));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        if ((threadIdx.x & 31) == 0) atomicMax(out + p, __float_as_uint(mx));
+    }
+}
+
 // Fields as the solve uses them, back in mm.
 __global__ void k_fields_to_mm(const float* __restrict__ fields, long long V, int planes, float hx, float hy, float hz,
                                float* __restrict__ out) {
@@ -131,6 +143,7 @@ struct pcamm_model {
     FieldStream fs;
     // scratch (device)
     unsigned char* cellmap = nullptr;   // FieldStream::cellmap
+    unsigned *f0_integral = nullptr, *cell_integral = nullptr;   // summed-volume tables (stream.cuh box_count)
     unsigned char* occ = nullptr;       // occupancy of the trial volumes [S][OCC] (common.cuh)
     float *vol = nullptr, *pseg = nullptr, *p = nullptr, *rL = nullptr;   // vol: trial volumes, ray layout [S][PV]
     ColHdr* col_hdr = nullptr;      // [B][nu]
@@ -643,6 +656,59 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     } else if (g->field_storage != 0) {
         set_error("geometry.field_storage must be 0 or 1");
         return fail(PCAMM_E_INVALID);
+    }
+    if (m->fs.use_tma) {
+        // what lets the streaming kernels skip tiles that can only see zeros (reading B8): the
+        // largest magnitude of every field plane (bounds the displacement for any w) and the
+        // summed-volume tables of f0 != 0 and of the cell map, built on the host once
+        const int planes = 3 * (G.K + 1);
+        unsigned int* d_max = nullptr;
+        unsigned int h_max[3 * (KMAX + 1)] = {};
+        std::vector<float> h_f0((size_t)V);
+        const size_t ncell = (size_t)(g->nx + 1) * (g->ny + 1) * (g->nz + 1);
+        std::vector<unsigned char> h_cell(ncell);
+        cudaError_t e3 = dalloc(m, &d_max, (size_t)planes);
+        if (e3 == cudaSuccess) e3 = dalloc(m, &m->f0_integral, ncell);
+        if (e3 == cudaSuccess) e3 = dalloc(m, &m->cell_integral, (size_t)(g->nx + 2) * (g->ny + 2) * (g->nz + 2));
+        if (e3 == cudaSuccess) e3 = cudaMemsetAsync(d_max, 0, sizeof(unsigned int) * planes, st);
+        if (e3 == cudaSuccess) {
+            k_plane_absmax<<<1184, 256, 0, st>>>(m->fields, V, planes, d_max);
+            e3 = cudaMemcpyAsync(h_max, d_max, sizeof(unsigned int) * planes, cudaMemcpyDeviceToHost, st);
+        }
+        if (e3 == cudaSuccess) e3 = cudaMemcpyAsync(h_f0.data(), m->f0, sizeof(float) * (size_t)V, cudaMemcpyDeviceToHost, st);
+        if (e3 == cudaSuccess) e3 = cudaMemcpyAsync(h_cell.data(), m->cellmap, ncell, cudaMemcpyDeviceToHost, st);
+        if (e3 == cudaSuccess) e3 = cudaStreamSynchronize(st);
+        if (e3 == cudaSuccess) {
+            for (int p = 0; p < planes; ++p) std::memcpy(&m->fs.fmax.v[p], &h_max[p], sizeof(float));
+            // table over [0, ex) x [0, ey) x [0, ez) of a 0/1 map given by `one(x, y, z)`
+            auto build = [](int ex, int ey, int ez, auto one) {
+                const size_t px = (size_t)ex + 1, pp = px * ((size_t)ey + 1);
+                std::vector<unsigned> I(pp * ((size_t)ez + 1), 0u);
+                for (int z = 0; z < ez; ++z)
+                    for (int y = 0; y < ey; ++y) {
+                        unsigned row = 0;                 // ones in [0, x] of this row
+                        for (int x = 0; x < ex; ++x) {
+                            row += one(x, y, z) ? 1u : 0u;
+                            I[(z + 1) * pp + (y + 1) * px + (x + 1)] =
+                                row + I[(z + 1) * pp + y * px + (x + 1)] + I[z * pp + (y + 1) * px + (x + 1)] - I[z * pp + y * px + (x + 1)];
+                        }
+                    }
+                return I;
+            };
+            const int nx = g->nx, ny = g->ny;
+            const std::vector<unsigned> If = build(g->nx, g->ny, g->nz, [&](int x, int y, int z) {
+                return h_f0[((size_t)z * ny + y) * nx + x] != 0.f;
+            });
+            const std::vector<unsigned> Ic = build(g->nx + 1, g->ny + 1, g->nz + 1, [&](int x, int y, int z) {
+                return h_cell[((size_t)z * (ny + 1) + y) * (nx + 1) + x] != 0;
+            });
+            e3 = cudaMemcpyAsync(m->f0_integral, If.data(), sizeof(unsigned) * If.size(), cudaMemcpyHostToDevice, st);
+            if (e3 == cudaSuccess) e3 = cudaMemcpyAsync(m->cell_integral, Ic.data(), sizeof(unsigned) * Ic.size(), cudaMemcpyHostToDevice, st);
+            if (e3 == cudaSuccess) e3 = cudaStreamSynchronize(st);
+        }
+        if (e3 != cudaSuccess) { set_error(std::string("summed-volume tables: ") + cudaGetErrorString(e3)); return fail(PCAMM_E_CUDA); }
+        m->fs.f0_integral = m->f0_integral;
+        m->fs.cell_integral = m->cell_integral;
     }
     m->c.grad_blocks = grad_blocks(G, m->fs);
     *out = m;

@@ -168,6 +168,14 @@ struct FieldRing {
         tma_load_4d(data + (size_t)s * STAGE_BYTES, map, full + s, c.x0, c.y, c.z0, 0, policy);
         if (H) tma_load_4d(data + (size_t)s * STAGE_BYTES + XBAR_BYTES, umap, full + s, c.x0, c.y, c.z0, 0, policy);
     }
+    // Group leader: start the load of tile t of the volume into stage s of the ring.
+    __device__ __forceinline__ void issue_tile(const CUtensorMap* map, const CUtensorMap* umap, const Geom& G,
+                                               long long t, int s, uint64_t policy) const {
+        const TileCoord c = tile_coord(G, TZ, t);
+        mbar_arrive_expect_tx(full + s, STAGE_BYTES);
+        tma_load_4d(data + (size_t)s * STAGE_BYTES, map, full + s, c.x0, c.y, c.z0, 0, policy);
+        if (H) tma_load_4d(data + (size_t)s * STAGE_BYTES + XBAR_BYTES, umap, full + s, c.x0, c.y, c.z0, 0, policy);
+    }
     // Group leader, once: the first SPG tiles.
     __device__ __forceinline__ void prologue(const CUtensorMap* map, const CUtensorMap* umap, const Geom& G,
                                              long long n_tiles, int g, uint64_t policy) const {
@@ -181,6 +189,28 @@ struct FieldRing {
 struct FieldScale {
     float inv[KMAX];
 };
+
+// Largest magnitude of every plane of the fields (voxel units; as the kernels read them):
+// |d_c| <= v[c] + sum_k |w_k| v[3 + 3k + c] bounds the displacement of Eq. (1) anywhere.
+struct FieldMax {
+    float v[3 * (KMAX + 1)];
+};
+
+// Summed-volume table of a 0/1 map over [0, ex) x [0, ey) x [0, ez): element ((z (ey + 1)) + y)(ex + 1) + x
+// holds the number of ones in [0, x) x [0, y) x [0, z) (mod 2^32).  Ones in the inclusive box
+// [xl, xh] x [yl, yh] x [zl, zh] (already clipped to the map, non-empty):
+__device__ __forceinline__ unsigned box_count(const unsigned* __restrict__ I, int ex, int ey, int xl, int xh, int yl,
+                                              int yh, int zl, int zh) {
+    const unsigned px = (unsigned)(ex + 1), pp = px * (unsigned)(ey + 1);
+    const unsigned x0 = (unsigned)xl, x1 = (unsigned)xh + 1u, y0 = (unsigned)yl * px, y1 = ((unsigned)yh + 1u) * px;
+    const unsigned z0 = (unsigned)zl * pp, z1 = ((unsigned)zh + 1u) * pp;
+    return __ldg(I + z1 + y1 + x1) - __ldg(I + z1 + y1 + x0) - __ldg(I + z1 + y0 + x1) - __ldg(I + z0 + y1 + x1) +
+           __ldg(I + z1 + y0 + x0) + __ldg(I + z0 + y1 + x0) + __ldg(I + z0 + y0 + x1) - __ldg(I + z0 + y0 + x0);
+}
+
+// Reach of a tile's interpolation stencils: per axis the largest |floor(d)| any voxel can have,
+// from the bound on |d| (a small margin covers the float rounding of Eq. (1)).
+__device__ __forceinline__ int reach_of(float dmax) { return (int)ceilf(dmax * 1.0001f + 0.001f); }
 
 // What the streaming kernels need to know about the model's fields.
 struct FieldStream {
@@ -198,6 +228,11 @@ struct FieldStream {
     // ((k0+1)(ny+1) + (j0+1))(nx+1) + (i0+1): 0 if the cell's eight zero-padded taps of f0 are all
     // equal (then the image gradient is exactly 0 anywhere in the cell), else 1 (gradient.cu)
     const unsigned char* cellmap = nullptr;
+    // summed-volume tables (box_count): of f0 != 0 over the voxel grid [nx][ny][nz], and of the
+    // cell map over [nx + 1][ny + 1][nz + 1]; NULL: no tile is ever skipped (reading B8)
+    const unsigned* f0_integral = nullptr;
+    const unsigned* cell_integral = nullptr;
+    FieldMax fmax = {};
 };
 
 // Tile extent along z and ring depth by K: a stage is 3(K+1) planes x TZ x TX floats and the

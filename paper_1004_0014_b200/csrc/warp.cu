@@ -119,6 +119,7 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
 // consumer groups: four where the stages of the 16-slice tiles (K = 5, 6) leave room for them
 // and for the L1 lines of the f0 gathers, else three
 template <int K> struct WarpGroups { static constexpr int value = (K == 5 || K == 6) ? 4 : 3; };
+constexpr int AIR_WORDS = 64;      // air flags of up to 2048 tiles per consumer group (beyond: never skipped)
 constexpr int SLOT_CACHE = 64;     // slots whose coefficients are kept in shared memory
 template <int K> struct WarpThreads { static constexpr int value = 32 * WarpGroups<K>::value * GROUP_WARPS; };
 
@@ -134,7 +135,7 @@ constexpr size_t warp_smem_bytes() {
 template <int K, bool RAY, bool H>
 __global__ void __launch_bounds__(WarpThreads<K>::value, 1)
 k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
-           const Geom G, const float* __restrict__ f0,
+           const FieldMax fmax, const unsigned* __restrict__ f0_integral, const Geom G, const float* __restrict__ f0,
            const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride,
            unsigned char* __restrict__ occ) {
     constexpr int P = 3 * (K + 1), WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
@@ -145,6 +146,18 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     __shared__ int s_occ[WNG][2][TX];                      // per group: column x has something in z block 0 / 1
     __shared__ float s_w[SLOT_CACHE][K];                   // the slots' coefficients (constant during the launch)
     __shared__ int s_active[SLOT_CACHE];
+    __shared__ int s_reach[3];                             // reach of the stencils, max over the active slots
+    __shared__ unsigned s_air[WarpGroups<K>::value][AIR_WORDS];   // per group: bit jt set = its jt-th tile is air
+    if (threadIdx.x < 3) {
+        float dmax = 0.f;
+        for (int i = 0; i < nslots && i < SLOT_CACHE; ++i) {
+            if (!slots[i].active) continue;
+            float d = fmax.v[threadIdx.x];
+            for (int k = 0; k < K; ++k) d = fmaf(fabsf(slots[i].w[k]), fmax.v[3 + 3 * k + threadIdx.x], d);
+            dmax = fmaxf(dmax, d);
+        }
+        s_reach[threadIdx.x] = reach_of(dmax);
+    }
     for (int i = threadIdx.x; i < nslots && i < SLOT_CACHE; i += blockDim.x) {
         s_active[i] = slots[i].active;
 #pragma unroll
@@ -167,13 +180,83 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     const bool leader = tw == 0 && lane == 0;
     const uint64_t policy = l2_evict_first_policy();
     float(*tile)[TX + 1] = tiles[group];
-    if (leader) ring.prologue(&fmap, &umap, G, n_tiles, group, policy);
-    int j = 0;                                             // this group's tile counter
+    // A tile whose stencils can only reach zeros of f0 (summed-volume table of f0 != 0 over the
+    // box the tile's voxels can be displaced into) is all zero whatever the fields say: its
+    // fields are neither loaded nor read, it is written as zeros (reading B8: exact).
+    // The flags of the group's tiles are worked out up front (one tile per thread, eight loads of
+    // the table each) and kept as bit masks in shared memory, off the tiles' critical path.
+    {
+        const int Rx = s_reach[0], Ry = s_reach[1], Rz = s_reach[2];
+        const int gtid = threadIdx.x - group * GROUP_THREADS;
+        for (int base = 0; base < AIR_WORDS * 32; base += GROUP_THREADS) {
+            const int jt = base + gtid;
+            const long long t = Ring::tile_of(group, jt);
+            bool air = false;
+            if (f0_integral != nullptr && t < n_tiles) {
+                const TileCoord c = tile_coord(G, WTZ, t);
+                const int xl = max(c.x0 - Rx, 0), xh = min(c.x0 + TX + Rx, G.nx - 1);
+                const int yl = max(c.y - Ry, 0), yh = min(c.y + 1 + Ry, G.ny - 1);
+                const int zl = max(c.z0 - Rz, 0), zh = min(c.z0 + WTZ + Rz, G.nz - 1);
+                air = xl > xh || yl > yh || zl > zh || box_count(f0_integral, G.nx, G.ny, xl, xh, yl, yh, zl, zh) == 0u;
+            }
+            const unsigned mask = __ballot_sync(0xffffffffu, air);
+            if (lane == 0) s_air[group][jt >> 5] = mask;
+            if (Ring::tile_of(group, base + GROUP_THREADS) >= n_tiles) break;     // uniform over the group
+        }
+        group_barrier(group);
+    }
+    auto tile_is_air = [&](int jt) -> bool {               // jt: the group's tile counter
+        return jt < AIR_WORDS * 32 && ((s_air[group][jt >> 5] >> (jt & 31)) & 1u) != 0u;
+    };
+    // The group's loads go through its stages in the order of its tiles that are not air.
+    constexpr int SPG = WarpStages<K, H>::value;
+    int n_issued = 0, j_issue = 0;                         // leader: loads started, next tile counter to look at
+    auto issue_next = [&]() {
+        for (;;) {
+            const long long t2 = Ring::tile_of(group, j_issue);
+            if (t2 >= n_tiles) return;
+            if (tile_is_air(j_issue++)) continue;
+            ring.issue_tile(&fmap, &umap, G, t2, group * SPG + n_issued % SPG, policy);
+            ++n_issued;
+            return;
+        }
+    };
+    if (leader)
+        for (int i = 0; i < SPG; ++i) issue_next();
+    int n_loaded = 0, j = 0;                               // loads this group has consumed; its tile counter
     for (long long t = Ring::tile_of(group, 0); t < n_tiles; t += (long long)WNG * gridDim.x, ++j) {
+        const bool air = tile_is_air(j);                   // uniform over the group
+        if (air) {                                         // zeros, straight to their places
+            const TileCoord c = tile_coord(G, WTZ, t);
+            for (int sl = 0; sl < nslots; ++sl) {
+                if (!s_active[sl]) continue;
+                float* out = vol_out + (long long)sl * slot_stride;
+                if (!RAY) {
+#pragma unroll
+                    for (int r = 0; r < WROWS; ++r) {
+                        const int x = c.x0 + lane, z = c.z0 + tw + GROUP_WARPS * r;
+                        if (x < G.nx && z < G.nz) out[((long long)z * G.ny + c.y) * G.nx + x] = 0.f;
+                    }
+                } else {
+                    const int zo = c.z0 + lane;
+#pragma unroll
+                    for (int r = 0; r < TX / GROUP_WARPS; ++r) {
+                        const int xo = c.x0 + tw + GROUP_WARPS * r;
+                        if (lane < WTZ && xo < G.nx && zo < G.nz) out[ray_layout_index(G, xo, c.y, zo)] = 0.f;
+                    }
+                    if (tw < WTZ / 16 && c.x0 + lane < G.nx && c.z0 + 16 * tw < G.nz)
+                        occ[(long long)sl * G.OCC + occ_index(G, c.x0 + lane, c.y, (c.z0 >> 4) + tw)] = (unsigned char)0;
+                }
+            }
+            continue;
+        }
         {
-            const int s = Ring::stage_of(group, j);
-            mbar_wait(ring.full + s, Ring::parity_of(j));
-            const uint32_t sf = smem_u32(ring.stage(s));   // [P][WTZ][TX]
+            uint32_t sf = 0;
+            if (!air) {
+                const int s = group * SPG + n_loaded % SPG;
+                mbar_wait(ring.full + s, (uint32_t)(n_loaded / SPG) & 1u);
+                sf = smem_u32(ring.stage(s));              // [P][WTZ][TX]
+            }
             const TileCoord c = tile_coord(G, WTZ, t);
             const int x = c.x0 + lane;
             for (int sl = 0; sl < nslots; ++sl) {
@@ -185,6 +268,9 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                 // voxels of a ragged tile beyond the grid: TMA filled their fields with zeros, the
                 // taps are clamped, the value is computed and not stored
                 float val[WROWS];
+#pragma unroll
+                for (int r = 0; r < WROWS; ++r) val[r] = 0.f;
+                if (!air) {
                 Taps taps[WROWS];
 #pragma unroll
                 for (int r = 0; r < WROWS; ++r) {
@@ -201,13 +287,14 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                 }
                 if (sl == last_active) {                    // the fields of this tile are in registers: refill the
                     group_barrier(group);                   // stage while the gathers are under way
-                    if (leader) ring.issue(&fmap, &umap, G, n_tiles, group, j + WarpStages<K, H>::value, policy);
+                    if (leader) issue_next();
                 }
                 float cv[WROWS][8];
 #pragma unroll
                 for (int r = 0; r < WROWS; ++r) gather8(G, f0, taps[r], cv[r]);    // 8 WROWS gathers in flight
 #pragma unroll
                 for (int r = 0; r < WROWS; ++r) val[r] = combine8(taps[r], cv[r]);
+                }
                 if (!RAY) {
 #pragma unroll
                     for (int r = 0; r < WROWS; ++r) {
@@ -238,6 +325,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                         occ[(long long)sl * G.OCC + occ_index(G, x, c.y, (c.z0 >> 4) + tw)] = (unsigned char)s_occ[group][tw][lane];
                 }
             }
+            if (!air) ++n_loaded;
         }
     }
 }
@@ -259,7 +347,7 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     const int grid = (int)(nt < n_sm ? nt : n_sm);
     for (int s0 = 0; s0 < nslots; s0 += SLOT_CACHE) {      // the kernel keeps up to SLOT_CACHE slots' coefficients on chip
         const int ns = nslots - s0 < SLOT_CACHE ? nslots - s0 : SLOT_CACHE;
-        q.launch(k_warp_tma<K, RAY, H>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, G, f0, slots + s0, ns,
+        q.launch(k_warp_tma<K, RAY, H>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax, fs.f0_integral, G, f0, slots + s0, ns,
                  vol_out + (long long)s0 * slot_stride, slot_stride, occ ? occ + (long long)s0 * G.OCC : occ);
     }
 }

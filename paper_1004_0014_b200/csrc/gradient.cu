@@ -254,6 +254,7 @@ constexpr int grad_groups_for(int K) {
 }
 template <int K> struct GradGroups { static constexpr int value = grad_groups_for(K); };
 constexpr int GSTATIC = 12 * 1024;                  // static shared memory of the kernel, rounded up
+constexpr int GRAD_SKIP_WORDS = 64;                 // skip flags of up to 2048 tiles per consumer group (beyond: never skipped)
 constexpr int SOLVE_CACHE = 64;                     // solves whose constants are kept in shared memory
 
 template <int K> struct GradBatch { static constexpr int value = 2; };     // RB
@@ -282,7 +283,7 @@ constexpr size_t grad_smem_bytes() {
 template <int K, bool SINGLE, bool H>
 __global__ void __launch_bounds__(32 * GradGroups<K>::value * GROUP_WARPS, 1)
 k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
-           const Geom G, const float* __restrict__ f0,
+           const FieldMax fmax, const unsigned* __restrict__ cell_integral, const Geom G, const float* __restrict__ f0,
            const unsigned char* __restrict__ cellmap, const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
            const float2* __restrict__ vtab, double* __restrict__ partials) {
     constexpr int P = 3 * (K + 1), GTZ = TileZ<K>::value, GROWS = GTZ / GROUP_WARPS;
@@ -296,6 +297,18 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     __shared__ GatherView s_gv[SOLVE_CACHE];               // per solve, constant during the launch
     __shared__ float s_w[SOLVE_CACHE][K];
     __shared__ int s_running[SOLVE_CACHE];
+    __shared__ int s_reach[3];                             // reach of the stencils, max over the running solves
+    __shared__ unsigned s_skip[GNG][GRAD_SKIP_WORDS];      // per group: bit jt set = nothing to do in its jt-th tile
+    if (threadIdx.x < 3) {
+        float dmax = 0.f;
+        for (int b = 0; b < B; ++b) {
+            if (!solves[b].running) continue;
+            float d = fmax.v[threadIdx.x];
+            for (int k = 0; k < K; ++k) d = fmaf(fabsf((float)solves[b].w[k]) * 1.000001f, fmax.v[3 + 3 * k + threadIdx.x], d);
+            dmax = fmaxf(dmax, d);
+        }
+        s_reach[threadIdx.x] = reach_of(dmax);
+    }
     for (int b = threadIdx.x; b < B; b += blockDim.x) {    // B <= SOLVE_CACHE (the launcher chunks)
         s_running[b] = solves[b].running;
         s_gv[b] = make_gather_view(G, solves[b].view);
@@ -324,16 +337,59 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     if (!any_running) return;                              // uniform over the grid
     const bool leader = gtid == 0;
     const uint64_t policy = l2_evict_first_policy();
-    if (leader) ring.prologue(&fmap, &umap, G, n_tiles, group, policy);
+    // A tile all of whose voxels can only land in constant cells of f0 (summed-volume table of the
+    // cell map over the box of cells the tile's voxels can be displaced into) has G_j = 0
+    // everywhere: its fields are neither loaded nor read (reading B8: exact).  The flags of the
+    // group's tiles are worked out up front, one tile per thread, and kept as bit masks.
+    {
+        const int Rx = s_reach[0], Ry = s_reach[1], Rz = s_reach[2];
+        for (int base = 0; base < GRAD_SKIP_WORDS * 32; base += GROUP_THREADS) {
+            const int jt = base + gtid;
+            const long long t = Ring::tile_of(group, jt);
+            bool skip = false;
+            if (cell_integral != nullptr && t < n_tiles) {
+                const TileCoord c = tile_coord(G, GTZ, t);
+                const int xl = max(c.x0 - Rx + 1, 0), xh = min(c.x0 + TX + Rx, G.nx);
+                const int yl = max(c.y - Ry + 1, 0), yh = min(c.y + 1 + Ry, G.ny);
+                const int zl = max(c.z0 - Rz + 1, 0), zh = min(c.z0 + GTZ + Rz, G.nz);
+                skip = xl > xh || yl > yh || zl > zh ||
+                       box_count(cell_integral, G.nx + 1, G.ny + 1, xl, xh, yl, yh, zl, zh) == 0u;
+            }
+            const unsigned mask = __ballot_sync(0xffffffffu, skip);
+            if (lane == 0) s_skip[group][jt >> 5] = mask;
+            if (Ring::tile_of(group, base + GROUP_THREADS) >= n_tiles) break;     // uniform over the group
+        }
+        group_barrier(group);
+    }
+    auto tile_is_skipped = [&](int jt) -> bool {           // jt: the group's tile counter
+        return jt < GRAD_SKIP_WORDS * 32 && ((s_skip[group][jt >> 5] >> (jt & 31)) & 1u) != 0u;
+    };
+    // The group's loads go through its stages in the order of its tiles that are not skipped.
+    constexpr int SPG = GradStages<K, H>::value;
+    int n_issued = 0, j_issue = 0;                         // leader: loads started, next tile counter to look at
+    auto issue_next = [&]() {
+        for (;;) {
+            const long long t2 = Ring::tile_of(group, j_issue);
+            if (t2 >= n_tiles) return;
+            if (tile_is_skipped(j_issue++)) continue;
+            ring.issue_tile(&fmap, &umap, G, t2, group * SPG + n_issued % SPG, policy);
+            ++n_issued;
+            return;
+        }
+    };
+    if (leader)
+        for (int i = 0; i < SPG; ++i) issue_next();
 
     float acc[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) acc[k] = 0.f;
-    int j = 0;                                             // this group's tile counter
+    int j = 0, n_loaded = 0;                               // this group's tile counter; loads it has consumed
     for (long long t = Ring::tile_of(group, 0); t < n_tiles; t += (long long)GNG * gridDim.x, ++j) {
+        if (tile_is_skipped(j)) continue;                  // uniform over the group
         {
-            const int s = Ring::stage_of(group, j);
-            mbar_wait(ring.full + s, Ring::parity_of(j));
+            const int s = group * SPG + n_loaded % SPG;
+            mbar_wait(ring.full + s, (uint32_t)(n_loaded / SPG) & 1u);
+            ++n_loaded;
             const uint32_t sf = smem_u32(ring.stage(s));   // [P][GTZ][TX]
             const TileCoord c = tile_coord(G, GTZ, t);
             const int x = c.x0 + lane;
@@ -425,8 +481,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                         for (int rr = 0; rr < RB; ++rr) s_cnt[group][parity][rr * GROUP_WARPS + tw] = __popc(masks[rr]);
                     }
                     group_barrier(group);
-                    if (SINGLE && bt == NB - 1 && leader)                   // no more reads of the stage: refill it
-                        ring.issue(&fmap, &umap, G, n_tiles, group, j + GradStages<K, H>::value, policy);
+                    if (SINGLE && bt == NB - 1 && leader) issue_next();    // no more reads of the stage: refill it
                     // 2. compaction in the fixed order (row, warp, lane), appended to the queue
                     int cnt = lane < RB * GROUP_WARPS ? s_cnt[group][parity][lane] : 0, incl = cnt;
                     parity ^= 1;
@@ -492,7 +547,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
             }
             if (!SINGLE) {
                 group_barrier(group);                       // every thread of the group is done with the stage
-                if (leader) ring.issue(&fmap, &umap, G, n_tiles, group, j + GradStages<K, H>::value, policy);
+                if (leader) issue_next();
             }
         }
     }
@@ -580,13 +635,13 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     constexpr int GNG = GradGroups<K>::value, GTHREADS = 32 * GNG * GROUP_WARPS;
     const int grid = grad_grid(G, fs), nslot = grid * GNG;
     if (B == 1) {
-        q.launch(k_grad_tma<K, true, H>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, G, f0,
+        q.launch(k_grad_tma<K, true, H>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, fs.cell_integral, G, f0,
                  fs.cellmap, solves, 1, rL, utab, vtab, partials);
         return;
     }
     for (int b0 = 0; b0 < B; b0 += SOLVE_CACHE) {       // the kernel keeps up to SOLVE_CACHE solves' constants on chip
         const int nb = B - b0 < SOLVE_CACHE ? B - b0 : SOLVE_CACHE;
-        q.launch(k_grad_tma<K, false, H>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, G, f0,
+        q.launch(k_grad_tma<K, false, H>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, fs.cell_integral, G, f0,
                  fs.cellmap, solves + b0, nb, rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu,
                  vtab + (long long)b0 * G.nv, partials + (long long)b0 * nslot * KMAX);
     }

@@ -377,6 +377,10 @@ def run_ours(args, cfg, rank, local_rank, world):
                       "achieved": ab[k] / (kt[k] * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                       "frac": ab[k] / (kt[k] * 1e-3) / 1e9 / peak, "traffic": traffic.get(k)}
                   for k in kt}
+    for k in per_kernel:        # what the launch really moved (ncu, profiles/), against the same peak
+        if per_kernel[k]["traffic"]:
+            per_kernel[k]["traffic_gbs"] = per_kernel[k]["traffic"] / (kt[k] * 1e-3) / 1e9
+            per_kernel[k]["traffic_frac"] = per_kernel[k]["traffic_gbs"] / peak
     # the projector against the SMs' fp32 lane-operation rate as well (it is not an HBM kernel)
     n_rs = ray_slab_count(cfg, angles[i_last])
     ops = PROJECT_OPS_PER_RAY_SLAB * n_rs
@@ -390,6 +394,9 @@ def run_ours(args, cfg, rank, local_rank, world):
     d = per_kernel[dom]
     roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],
                 "frac": d["frac"], "traffic": d["traffic"],
+                "note": "achieved = SURVEY 8(a) algorithmic bytes (every voxel's fields counted) / launch time; the warp and "
+                        "gradient kernels skip, exactly, the tiles whose stencils can only see zeros / constant cells of f0 "
+                        "(DESIGN.md reading B8), so they move fewer bytes than that (traffic, traffic_frac) and frac may exceed 1",
                 "peak_source": peak_src if d["bound"] == "hbm" else
                 "148 SMs x 128 fp32 lanes x 1.965 GHz (B200_PROFILING.md unit counts and clocks; DESIGN.md section 6)",
                 "per_kernel": per_kernel,

@@ -74,6 +74,10 @@ typedef struct {
                                warp and gradient kernels; the model then IS the rounded one (every step,
                                the landmark inversion included, uses the rounded u_k; pcamm_model_fields
                                returns them).  Needs nx % 8 == 0. */
+    int32_t tile_skipping;  /* the warp and gradient kernels skip, exactly, the tiles of the volume that can only
+                               see zeros / constant cells of f0 (reading B8): 0 (default) where the
+                               volume has tiles enough per SM to win back the flags' set-up (a few dependent
+                               loads per launch), 1 always, 2 never */
 } pcamm_geometry;
 
 typedef struct {

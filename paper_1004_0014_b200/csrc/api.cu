@@ -657,7 +657,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         set_error("geometry.field_storage must be 0 or 1");
         return fail(PCAMM_E_INVALID);
     }
-    if (m->fs.use_tma) {
+    if (g->tile_skipping < 0 || g->tile_skipping > 2) { set_error("geometry.tile_skipping must be 0, 1 or 2"); return fail(PCAMM_E_INVALID); }
+    if (m->fs.use_tma && g->tile_skipping != 2) {
         // what lets the streaming kernels skip tiles that can only see zeros (reading B8): the
         // largest magnitude of every field plane (bounds the displacement for any w) and the
         // summed-volume tables of f0 != 0 and of the cell map, built on the host once
@@ -709,6 +710,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         if (e3 != cudaSuccess) { set_error(std::string("summed-volume tables: ") + cudaGetErrorString(e3)); return fail(PCAMM_E_CUDA); }
         m->fs.f0_integral = m->f0_integral;
         m->fs.cell_integral = m->cell_integral;
+        m->fs.skip_min_tiles_per_sm = g->tile_skipping == 1 ? 0 : (g->tile_skipping == 2 ? (1 << 30) : SKIP_MIN_TILES_PER_SM);
     }
     m->c.grad_blocks = grad_blocks(G, m->fs);
     *out = m;

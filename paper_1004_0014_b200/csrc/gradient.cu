@@ -279,8 +279,9 @@ constexpr size_t grad_smem_bytes() {
 
 // SINGLE: one solve (B = 1): the K sums stay in registers over all tiles of the CTA and are
 // reduced once at the end; otherwise they are reduced per tile and solve.
-// H: u_k stored in half (stream.cuh FieldRing, FieldScale).
-template <int K, bool SINGLE, bool H>
+// H: u_k stored in half (stream.cuh FieldRing, FieldScale).  SKIP: with the tile flags of reading
+// B8 (cell_integral != NULL); without them the loads simply follow the tile counter.
+template <int K, bool SINGLE, bool H, bool SKIP>
 __global__ void __launch_bounds__(32 * GradGroups<K>::value * GROUP_WARPS, 1)
 k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
            const FieldMax fmax, const unsigned* __restrict__ cell_integral, const Geom G, const float* __restrict__ f0,
@@ -298,8 +299,9 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     __shared__ float s_w[SOLVE_CACHE][K];
     __shared__ int s_running[SOLVE_CACHE];
     __shared__ int s_reach[3];                             // reach of the stencils, max over the running solves
+    __shared__ int s_issue[GNG][2];
     __shared__ unsigned s_skip[GNG][GRAD_SKIP_WORDS];      // per group: bit jt set = nothing to do in its jt-th tile
-    if (threadIdx.x < 3) {
+    if (SKIP && threadIdx.x < 3) {
         float dmax = 0.f;
         for (int b = 0; b < B; ++b) {
             if (!solves[b].running) continue;
@@ -341,13 +343,13 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     // cell map over the box of cells the tile's voxels can be displaced into) has G_j = 0
     // everywhere: its fields are neither loaded nor read (reading B8: exact).  The flags of the
     // group's tiles are worked out up front, one tile per thread, and kept as bit masks.
-    {
+    if (SKIP) {
         const int Rx = s_reach[0], Ry = s_reach[1], Rz = s_reach[2];
         for (int base = 0; base < GRAD_SKIP_WORDS * 32; base += GROUP_THREADS) {
             const int jt = base + gtid;
             const long long t = Ring::tile_of(group, jt);
             bool skip = false;
-            if (cell_integral != nullptr && t < n_tiles) {
+            if (t < n_tiles) {
                 const TileCoord c = tile_coord(G, GTZ, t);
                 const int xl = max(c.x0 - Rx + 1, 0), xh = min(c.x0 + TX + Rx, G.nx);
                 const int yl = max(c.y - Ry + 1, 0), yh = min(c.y + 1 + Ry, G.ny);
@@ -362,20 +364,28 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
         group_barrier(group);
     }
     auto tile_is_skipped = [&](int jt) -> bool {           // jt: the group's tile counter
-        return jt < GRAD_SKIP_WORDS * 32 && ((s_skip[group][jt >> 5] >> (jt & 31)) & 1u) != 0u;
+        return SKIP && jt < GRAD_SKIP_WORDS * 32 && ((s_skip[group][jt >> 5] >> (jt & 31)) & 1u) != 0u;
     };
     // The group's loads go through its stages in the order of its tiles that are not skipped.
     constexpr int SPG = GradStages<K, H>::value;
-    int n_issued = 0, j_issue = 0;                         // leader: loads started, next tile counter to look at
+    // (the leader's two counters live in shared memory: registers are what limits this kernel)
+    if (leader) { s_issue[group][0] = 0; s_issue[group][1] = 0; }      // loads started, next tile counter to look at
     auto issue_next = [&]() {
+        if (!SKIP) {                                       // the group's tiles in turn
+            const int j_issue = s_issue[group][1]++;
+            ring.issue(&fmap, &umap, G, n_tiles, group, j_issue, policy);
+            return;
+        }
+        int n_issued = s_issue[group][0], j_issue = s_issue[group][1];
         for (;;) {
             const long long t2 = Ring::tile_of(group, j_issue);
-            if (t2 >= n_tiles) return;
+            if (t2 >= n_tiles) break;
             if (tile_is_skipped(j_issue++)) continue;
             ring.issue_tile(&fmap, &umap, G, t2, group * SPG + n_issued % SPG, policy);
             ++n_issued;
-            return;
+            break;
         }
+        s_issue[group][0] = n_issued; s_issue[group][1] = j_issue;
     };
     if (leader)
         for (int i = 0; i < SPG; ++i) issue_next();
@@ -387,9 +397,10 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     for (long long t = Ring::tile_of(group, 0); t < n_tiles; t += (long long)GNG * gridDim.x, ++j) {
         if (tile_is_skipped(j)) continue;                  // uniform over the group
         {
-            const int s = group * SPG + n_loaded % SPG;
-            mbar_wait(ring.full + s, (uint32_t)(n_loaded / SPG) & 1u);
-            ++n_loaded;
+            const int nl = SKIP ? n_loaded : j;
+            const int s = group * SPG + nl % SPG;
+            mbar_wait(ring.full + s, (uint32_t)(nl / SPG) & 1u);
+            if (SKIP) ++n_loaded;
             const uint32_t sf = smem_u32(ring.stage(s));   // [P][GTZ][TX]
             const TileCoord c = tile_coord(G, GTZ, t);
             const int x = c.x0 + lane;
@@ -626,22 +637,25 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     static bool configured = false;
     constexpr size_t smem = grad_smem_bytes<K, H>();
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_grad_tma<K, true, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(k_grad_tma<K, false, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaSuccess;
+        auto set = [&](auto kernel) { if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); };
+        set(k_grad_tma<K, true, H, true>); set(k_grad_tma<K, true, H, false>);
+        set(k_grad_tma<K, false, H, true>); set(k_grad_tma<K, false, H, false>);
         if (e != cudaSuccess) { q.err = e; return; }
         configured = true;
     }
     constexpr int GNG = GradGroups<K>::value, GTHREADS = 32 * GNG * GROUP_WARPS;
     const int grid = grad_grid(G, fs), nslot = grid * GNG;
+    // the flags cost a few dependent loads per launch: only where a CTA has tiles enough to win them back
+    const unsigned* skip_table = tile_count(G, TileZ<K>::value) >= fs.skip_min_tiles_per_sm * (long long)fs.n_sm ? fs.cell_integral : nullptr;
     if (B == 1) {
-        q.launch(k_grad_tma<K, true, H>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, fs.cell_integral, G, f0,
+        q.launch(skip_table ? k_grad_tma<K, true, H, true> : k_grad_tma<K, true, H, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, skip_table, G, f0,
                  fs.cellmap, solves, 1, rL, utab, vtab, partials);
         return;
     }
     for (int b0 = 0; b0 < B; b0 += SOLVE_CACHE) {       // the kernel keeps up to SOLVE_CACHE solves' constants on chip
         const int nb = B - b0 < SOLVE_CACHE ? B - b0 : SOLVE_CACHE;
-        q.launch(k_grad_tma<K, false, H>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, fs.cell_integral, G, f0,
+        q.launch(skip_table ? k_grad_tma<K, false, H, true> : k_grad_tma<K, false, H, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, skip_table, G, f0,
                  fs.cellmap, solves + b0, nb, rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu,
                  vtab + (long long)b0 * G.nv, partials + (long long)b0 * nslot * KMAX);
     }

@@ -208,6 +208,10 @@ __device__ __forceinline__ unsigned box_count(const unsigned* __restrict__ I, in
            __ldg(I + z1 + y0 + x0) + __ldg(I + z0 + y1 + x0) + __ldg(I + z0 + y0 + x1) - __ldg(I + z0 + y0 + x0);
 }
 
+// The tile flags cost a few dependent loads at the start of a launch: they are used where a CTA
+// has at least this many tiles to win them back on.
+constexpr int SKIP_MIN_TILES_PER_SM = 12;
+
 // Reach of a tile's interpolation stencils: per axis the largest |floor(d)| any voxel can have,
 // from the bound on |d| (a small margin covers the float rounding of Eq. (1)).
 __device__ __forceinline__ int reach_of(float dmax) { return (int)ceilf(dmax * 1.0001f + 0.001f); }
@@ -233,6 +237,7 @@ struct FieldStream {
     const unsigned* f0_integral = nullptr;
     const unsigned* cell_integral = nullptr;
     FieldMax fmax = {};
+    int skip_min_tiles_per_sm = SKIP_MIN_TILES_PER_SM;     // geometry.tile_skipping: 0 always, INT_MAX never
 };
 
 // Tile extent along z and ring depth by K: a stage is 3(K+1) planes x TZ x TX floats and the

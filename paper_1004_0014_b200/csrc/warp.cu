@@ -131,8 +131,9 @@ constexpr size_t warp_smem_bytes() {
     return FieldRing<3 * (K + 1), TileZ<K>::value, WarpGroups<K>::value, WarpStages<K, H>::value, H>::BYTES;
 }
 
-// H: u_k stored in half (stream.cuh FieldRing, FieldScale)
-template <int K, bool RAY, bool H>
+// H: u_k stored in half (stream.cuh FieldRing, FieldScale).  SKIP: with the tile flags of reading
+// B8 (f0_integral != NULL); without them the loads simply follow the tile counter.
+template <int K, bool RAY, bool H, bool SKIP>
 __global__ void __launch_bounds__(WarpThreads<K>::value, 1)
 k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
            const FieldMax fmax, const unsigned* __restrict__ f0_integral, const Geom G, const float* __restrict__ f0,
@@ -147,8 +148,9 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     __shared__ float s_w[SLOT_CACHE][K];                   // the slots' coefficients (constant during the launch)
     __shared__ int s_active[SLOT_CACHE];
     __shared__ int s_reach[3];                             // reach of the stencils, max over the active slots
+    __shared__ int s_issue[WarpGroups<K>::value][2];
     __shared__ unsigned s_air[WarpGroups<K>::value][AIR_WORDS];   // per group: bit jt set = its jt-th tile is air
-    if (threadIdx.x < 3) {
+    if (SKIP && threadIdx.x < 3) {
         float dmax = 0.f;
         for (int i = 0; i < nslots && i < SLOT_CACHE; ++i) {
             if (!slots[i].active) continue;
@@ -185,14 +187,14 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     // fields are neither loaded nor read, it is written as zeros (reading B8: exact).
     // The flags of the group's tiles are worked out up front (one tile per thread, eight loads of
     // the table each) and kept as bit masks in shared memory, off the tiles' critical path.
-    {
+    if (SKIP) {
         const int Rx = s_reach[0], Ry = s_reach[1], Rz = s_reach[2];
         const int gtid = threadIdx.x - group * GROUP_THREADS;
         for (int base = 0; base < AIR_WORDS * 32; base += GROUP_THREADS) {
             const int jt = base + gtid;
             const long long t = Ring::tile_of(group, jt);
             bool air = false;
-            if (f0_integral != nullptr && t < n_tiles) {
+            if (t < n_tiles) {
                 const TileCoord c = tile_coord(G, WTZ, t);
                 const int xl = max(c.x0 - Rx, 0), xh = min(c.x0 + TX + Rx, G.nx - 1);
                 const int yl = max(c.y - Ry, 0), yh = min(c.y + 1 + Ry, G.ny - 1);
@@ -206,20 +208,28 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
         group_barrier(group);
     }
     auto tile_is_air = [&](int jt) -> bool {               // jt: the group's tile counter
-        return jt < AIR_WORDS * 32 && ((s_air[group][jt >> 5] >> (jt & 31)) & 1u) != 0u;
+        return SKIP && jt < AIR_WORDS * 32 && ((s_air[group][jt >> 5] >> (jt & 31)) & 1u) != 0u;
     };
     // The group's loads go through its stages in the order of its tiles that are not air.
     constexpr int SPG = WarpStages<K, H>::value;
-    int n_issued = 0, j_issue = 0;                         // leader: loads started, next tile counter to look at
+    // (the leader's two counters live in shared memory: registers are what limits this kernel)
+    if (leader) { s_issue[group][0] = 0; s_issue[group][1] = 0; }      // loads started, next tile counter to look at
     auto issue_next = [&]() {
+        if (!SKIP) {                                       // the group's tiles in turn
+            const int j_issue = s_issue[group][1]++;
+            ring.issue(&fmap, &umap, G, n_tiles, group, j_issue, policy);
+            return;
+        }
+        int n_issued = s_issue[group][0], j_issue = s_issue[group][1];
         for (;;) {
             const long long t2 = Ring::tile_of(group, j_issue);
-            if (t2 >= n_tiles) return;
+            if (t2 >= n_tiles) break;
             if (tile_is_air(j_issue++)) continue;
             ring.issue_tile(&fmap, &umap, G, t2, group * SPG + n_issued % SPG, policy);
             ++n_issued;
-            return;
+            break;
         }
+        s_issue[group][0] = n_issued; s_issue[group][1] = j_issue;
     };
     if (leader)
         for (int i = 0; i < SPG; ++i) issue_next();
@@ -253,8 +263,9 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
         {
             uint32_t sf = 0;
             if (!air) {
-                const int s = group * SPG + n_loaded % SPG;
-                mbar_wait(ring.full + s, (uint32_t)(n_loaded / SPG) & 1u);
+                const int nl = SKIP ? n_loaded : j;
+                const int s = group * SPG + nl % SPG;
+                mbar_wait(ring.full + s, (uint32_t)(nl / SPG) & 1u);
                 sf = smem_u32(ring.stage(s));              // [P][WTZ][TX]
             }
             const TileCoord c = tile_coord(G, WTZ, t);
@@ -325,7 +336,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                         occ[(long long)sl * G.OCC + occ_index(G, x, c.y, (c.z0 >> 4) + tw)] = (unsigned char)s_occ[group][tw][lane];
                 }
             }
-            if (!air) ++n_loaded;
+            if (SKIP && !air) ++n_loaded;
         }
     }
 }
@@ -339,16 +350,26 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     const CUtensorMap& umap = half_map<K>(fs);
     const int n_sm = fs.n_sm;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_warp_tma<K, RAY, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) { q.err = e; return; }
         configured = true;
     }
     const long long nt = tile_count(G, TileZ<K>::value);
     const int grid = (int)(nt < n_sm ? nt : n_sm);
+    // the tile flags cost a few dependent loads per launch: used where a CTA has tiles enough to win them back
+    const unsigned* table = nt >= fs.skip_min_tiles_per_sm * (long long)n_sm ? fs.f0_integral : nullptr;
     for (int s0 = 0; s0 < nslots; s0 += SLOT_CACHE) {      // the kernel keeps up to SLOT_CACHE slots' coefficients on chip
         const int ns = nslots - s0 < SLOT_CACHE ? nslots - s0 : SLOT_CACHE;
-        q.launch(k_warp_tma<K, RAY, H>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax, fs.f0_integral, G, f0, slots + s0, ns,
-                 vol_out + (long long)s0 * slot_stride, slot_stride, occ ? occ + (long long)s0 * G.OCC : occ);
+        float* out = vol_out + (long long)s0 * slot_stride;
+        unsigned char* oc = occ ? occ + (long long)s0 * G.OCC : occ;
+        if (table)
+            q.launch(k_warp_tma<K, RAY, H, true>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
+                     table, G, f0, slots + s0, ns, out, slot_stride, oc);
+        else
+            q.launch(k_warp_tma<K, RAY, H, false>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
+                     table, G, f0, slots + s0, ns, out, slot_stride, oc);
     }
 }
 

@@ -294,3 +294,42 @@ def test_localisation_matches_oracle_and_closed_forms():
     m1 = make_model(g1, f0, xb, uc, landmarks=lm[:2])
     np.testing.assert_allclose(m1.localise(np.array([2.0])), lm[:2] - 2.0 * np.array([0.5, -1.25, 2.0]), atol=1e-6)
     np.testing.assert_array_equal(m1.localise(np.array([0.0])), lm[:2])
+
+
+@pytest.mark.parametrize("disp_vox", [0.4, 3.0, 9.0])
+def test_tiles_that_cannot_contribute_are_skipped_exactly(disp_vox):
+    """DESIGN.md reading B8, per tile: the warp kernel writes a tile as zeros without reading its
+    fields when f0 is 0 on everything its stencils can reach, the gradient kernel does not visit a
+    tile whose voxels can only land in constant cells.  Both rest on a bound of the displacement
+    from the field maxima; a reference image that is a few small bodies in a lot of air, with
+    displacements from a fraction of a voxel to well beyond a tile's neighbours, through grids
+    with ragged tiles.  Where f0's support cannot reach, the result is exactly 0 on both sides."""
+    g = geom(nx=136, ny=70, nz=75, h=(2.0, 2.0, 2.0), K=3, nu=96, nv=64, pitch=(3.4, 2.6), centre=(0.3, -0.4, 0.2))
+    rng = np.random.default_rng(int(disp_vox * 10))
+    zz, yy, xx = np.meshgrid(np.arange(g.nz), np.arange(g.ny), np.arange(g.nx), indexing="ij")
+    body = ((xx - 100) / 14.0) ** 2 + ((yy - 20) / 9.0) ** 2 + ((zz - 50) / 12.0) ** 2 <= 1.0
+    plate = (np.abs(xx - 30) <= 2) & (yy >= 50) & (zz <= 20)          # constant inside: gradient only at its faces
+    dot = (xx == 70) & (yy == 35) & (zz == 37)
+    f0, xbar, u, scale, _ = _model(g, seed=17, disp_vox=disp_vox)
+    f0 = (np.where(body, 0.5 + f0, 0.0) + 0.7 * plate + 1.3 * dot).astype(np.float32)
+    m = make_model(g, f0, xbar, u, tile_skipping=1)
+    m_all = make_model(g, f0, xbar, u, tile_skipping=2)               # visits every tile
+    theta = 0.9
+    for wf in (0.0, 1.0, -1.7):
+        w = (wf * scale * np.array([1.0, -0.6, 0.8])).astype(np.float32)
+        f_ref = oracle.warp(g, f0, xbar, u, w)
+        f_gpu = to_host(m.warp(w))
+        assert np.array_equal(f_gpu, to_host(m_all.warp(w)))          # the shortcut changes no bit
+        assert np.max(np.abs(f_gpu - f_ref)) <= 2e-5 * np.abs(f_ref).max()
+        assert np.all(f_gpu[f_ref == 0] == 0)
+        _, p_ref = oracle.evaluate(g, f0, xbar, u, w, theta)
+        y = (p_ref * (1 + 0.05 * rng.standard_normal(p_ref.shape))).astype(np.float32)
+        J, grad, ab, p = m.eval(to_dev(y), theta, w, 0.9, 0.01)
+        assert rel_l2(to_host(p), p_ref) <= 1e-5
+        g_ref = oracle.gradient(g, f0, xbar, u, w, 0.9, 0.01, p_ref, y, theta)
+        assert np.linalg.norm(grad - g_ref) <= 1e-4 * np.linalg.norm(g_ref)
+        J2, grad2, _, p2 = m_all.eval(to_dev(y), theta, w, 0.9, 0.01)
+        assert J2 == J and np.array_equal(grad2, grad) and np.array_equal(to_host(p2), to_host(p))
+    # nothing but air: every tile goes the short way
+    m0 = make_model(g, np.zeros(g.vshape, np.float32), xbar, u)
+    assert not to_host(m0.warp(w)).any()

@@ -270,6 +270,9 @@ def run_ours(args, cfg, rank, local_rank, world):
 
     import torch
     import paper_1004_0014_b200 as pc
+    for kv in args.tune:
+        name, _, value = kv.partition("=")
+        pc.tune(name, int(value))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     dist = replicas.init_process_group("nccl")
@@ -571,6 +574,8 @@ def main():
     ap.add_argument("--pca-study", action="store_true",
                     help="instead of the bench line: pcamm_pca_fit on the config's training DVFs (device time of its "
                          "two passes against their algorithmic bytes)")
+    ap.add_argument("--tune", action="append", default=[], metavar="NAME=VALUE",
+                    help="pcamm_tune measurement knob, set before the model is created (repeatable)")
     ap.add_argument("--grad-tol", type=float, default=None)
     ap.add_argument("--study-max-iter", type=int, default=30)
     args = ap.parse_args()

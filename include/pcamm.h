@@ -259,6 +259,13 @@ int pcamm_localise(pcamm_model* model, const float* w_host, int32_t inv_max_iter
  * which: 0 = warp (a-1), 1 = project (a-2), 2 = gradient (a-4). */
 int pcamm_time_kernel(pcamm_model* model, int32_t which, int32_t reps, float* ms_out, void* stream);
 
+/* Measurement knob (process-wide; set it before pcamm_model_create: a model's solve graphs keep the
+ * launch configuration they were built with).  Returns PCAMM_E_INVALID for an unknown name.
+ *   "project_chunks_per_segment"  chunks of the projector's march a block works through
+ *                                 (0 = automatic, the default);
+ *   "project_scan_slabs"          slabs per scan of the projector: 1, 2 or 4 (0 = automatic). */
+int pcamm_tune(const char* name, int32_t value);
+
 /* Number of kernels launched by this library on the calling thread since the last reset
  * (host-side launch count; kernels inside device-side loops are counted from the device's
  * iteration counters after each solve). */

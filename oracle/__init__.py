@@ -181,13 +181,6 @@ def traverse(g: Geometry, theta, iu: int, iv: int):
     return ijk[:n.value].copy(), ln[:n.value].copy(), gap.value
 
 
-def min_gaps(g: Geometry, theta) -> np.ndarray:
-    out = np.empty(g.pshape, dtype=np.float64)
-    gc = g._c()
-    lib().orc_min_gaps(C.byref(gc), C.c_double(_angle(theta)), _p(out))
-    return out
-
-
 def lsfit(p, y):
     p, y = _f64(p), _f32(y)
     a, b = C.c_double(0), C.c_double(0)

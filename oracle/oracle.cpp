@@ -287,21 +287,6 @@ int orc_traverse(const OrcGeom* g, double theta, int iu, int iv, int cap, int32_
     return (int)segs.size() <= cap ? 0 : 1;
 }
 
-// Smallest crossing gap of every ray (mm), [nv][nu]; INFINITY for rays that miss.
-void orc_min_gaps(const OrcGeom* g, double theta, double* gap_out) {
-    const OrcGeom& G = *g;
-#pragma omp parallel num_threads(g_threads)
-    {
-        std::vector<Seg> segs;
-#pragma omp for schedule(static)
-        for (int64_t pix = 0; pix < npix(G); ++pix) {
-            double mg;
-            siddon(G, make_ray(G, theta, (int)(pix % G.nu), (int)(pix / G.nu)), segs, &mg);
-            gap_out[pix] = mg;
-        }
-    }
-}
-
 // p = P_theta f: p_i = sum_j l_ij f_j (Eq. 2; reading A3).
 void orc_project(const OrcGeom* g, const double* f, double theta, double* p_out) {
     const OrcGeom& G = *g;

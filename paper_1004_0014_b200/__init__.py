@@ -53,7 +53,7 @@ SYMBOLS = ("pcamm_default_opts", "pcamm_model_create", "pcamm_model_destroy", "p
            "pcamm_reconstruct",
            "pcamm_reconstruct_host", "pcamm_reconstruct_batch", "pcamm_warp", "pcamm_project",
            "pcamm_backproject", "pcamm_eval", "pcamm_traverse", "pcamm_localise", "pcamm_time_kernel",
-           "pcamm_launch_count", "pcamm_last_error", "pcamm_pca_fit", "pcamm_predict_w", "pcamm_frames_create",
+           "pcamm_tune", "pcamm_launch_count", "pcamm_last_error", "pcamm_pca_fit", "pcamm_predict_w", "pcamm_frames_create",
            "pcamm_frames_destroy", "pcamm_frames_reset", "pcamm_frames_count", "pcamm_frames_predict",
            "pcamm_frames_push")
 
@@ -90,6 +90,11 @@ def last_error() -> str:
 
 def launch_count(reset: bool = False) -> int:
     return int(lib().pcamm_launch_count(1 if reset else 0))
+
+
+def tune(name: str, value: int) -> None:
+    """pcamm_tune: a measurement knob (set before creating the Model)."""
+    _check(lib().pcamm_tune(name.encode(), int(value)))
 
 
 def _check(rc: int) -> int:

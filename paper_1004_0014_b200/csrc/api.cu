@@ -491,6 +491,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     if (n_landmarks < 0 || (n_landmarks > 0 && !landmarks_mm_host)) return invalid("landmarks");
     const long long V = (long long)g->nx * g->ny * g->nz;
     if ((long long)(g->nx + 4) * (g->ny + 4) * (g->nz + 4) >= (1LL << 31) || (long long)g->nu * g->nv >= (1LL << 31)) return invalid("volume or detector too large");
+    // the gradient kernel's voxel queue packs (x, y) into 16 + 15 bits
+    if (g->nx >= 65536 || g->ny >= 32768) return invalid("nx must be < 65536 and ny < 32768");
     const int Bmax = g->max_batch < 1 ? 1 : g->max_batch;
     const int Cmax = g->max_candidates < 1 ? 1 : g->max_candidates;
     if (Cmax > MAXBT || Bmax > 4096) return invalid("max_batch / max_candidates too large");
@@ -506,6 +508,11 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     if (!(vmax / g->hz <= (double)g->sdd / std::sqrt((double)g->hx * g->hx + (double)g->hy * g->hy)))
         return invalid("cone angle too steep for the voxel aspect ratio (z-slope > 1 voxel per slab)");
 
+    {
+        Geom Gz = {};
+        Gz.nz = g->nz;
+        if (!project_fits(Gz)) return invalid("nz too large for the projector's shared-memory knots");
+    }
     pcamm_model* m = new (std::nothrow) pcamm_model();
     if (!m) { set_error("out of host memory"); return PCAMM_E_NOMEM; }
     m->geo = *g;
@@ -520,6 +527,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     G.ihx = 1.f / g->hx; G.ihy = 1.f / g->hy; G.ihz = 1.f / g->hz;
     G.cx = g->cx; G.cy = g->cy; G.cz = g->cz;
     G.lox = (double)g->cx - ex; G.loy = (double)g->cy - ey; G.loz = (double)g->cz - ez;
+    G.ihz_d = 1.0 / (double)g->hz; G.Szi = (0.0 - G.loz) / (double)g->hz;
     G.K = g->K; G.nu = g->nu; G.nv = g->nv; G.npix = g->nu * g->nv;
     G.pu = g->pu; G.pv = g->pv; G.sad = g->sad; G.sdd = g->sdd; G.off_u = g->off_u; G.off_v = g->off_v;
 
@@ -870,6 +878,14 @@ int pcamm_localise(pcamm_model* m, const float* w_host, int32_t inv_max_iter, fl
     CUDA_TRY(cudaStreamSynchronize(st));
     for (int i = 0; i < 3 * m->M; ++i) landmarks_out_host[i] = (float)m->h_lm[i];
     return PCAMM_OK;
+}
+
+int pcamm_tune(const char* name, int32_t value) {
+    if (!name) return invalid("NULL argument");
+    const std::string n(name);
+    if (n == "project_chunks_per_segment") { g_chunks_per_segment = value < 0 ? 0 : value; return PCAMM_OK; }
+    if (n == "project_scan_slabs") { g_scan_slabs = value < 0 ? 0 : value; return PCAMM_OK; }
+    return invalid("unknown knob: " + n);
 }
 
 int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out, void* stream) {

@@ -29,6 +29,7 @@ struct Geom {
     float ihx, ihy, ihz;      // 1 / h
     float cx, cy, cz;         // world position of the volume centre
     double lox, loy, loz;     // world position of the volume's low corner
+    double ihz_d, Szi;        // 1 / hz and the source plane z = 0 in voxel-corner units, -loz / hz (project.cu)
     int K;
     int nu, nv, npix;
     float pu, pv, sad, sdd, off_u, off_v;
@@ -73,15 +74,16 @@ struct ColHdr {
     double kap;               // 1 / |g_m|: ray parameter per slab, in units of (D - S) per voxel
     float dxy2;               // in-plane part of |D - S|^2, mm^2
     int n_slabs;              // slabs in which the column's rays can be inside the volume in-plane
-    int dT;                   // element offset to the next voxel across a transverse plane
+    int dT;                   // voxel-column offset ((y + 1) pnx + (x + 1) units) to the next column across a transverse plane
     int axis;                 // 0: marches along x, 1: along y
 };
 
-// Per view, column and slab: element offset of the voxel column (i, j) the ray is in when it
-// enters the slab, and the share tt of the slab's path before the transverse plane crossing
-// (1 if none in this slab), stored in units of 2^-32 of the slab like the z crossing counters.
+// Per view, column and slab: the voxel column (i, j) the ray is in when it enters the slab, as the
+// column index (j + 1) pnx + (i + 1) of the ray layout, and the share tt of the slab's path before
+// the transverse plane crossing (1 if none in this slab), stored in units of 2^-32 of the slab
+// like the z crossing counters.
 struct SlabEntry {
-    int off0;
+    int col;
     float tt;
 };
 

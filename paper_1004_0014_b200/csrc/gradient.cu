@@ -634,15 +634,17 @@ k_backproject(const Geom G, const SolveState* __restrict__ solves, const float* 
 template <int K, bool H>
 void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
                 const float* rL, const float4* utab, const float2* vtab, double* partials) {
-    static bool configured = false;
+    static DeviceOnce configured;
     constexpr size_t smem = grad_smem_bytes<K, H>();
-    if (!configured) {
-        cudaError_t e = cudaSuccess;
-        auto set = [&](auto kernel) { if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); };
-        set(k_grad_tma<K, true, H, true>); set(k_grad_tma<K, true, H, false>);
-        set(k_grad_tma<K, false, H, true>); set(k_grad_tma<K, false, H, false>);
-        if (e != cudaSuccess) { q.err = e; return; }
-        configured = true;
+    {
+        const cudaError_t e0 = configured.run([&] {
+            cudaError_t e = cudaSuccess;
+            auto set = [&](auto kernel) { if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); };
+            set(k_grad_tma<K, true, H, true>); set(k_grad_tma<K, true, H, false>);
+            set(k_grad_tma<K, false, H, true>); set(k_grad_tma<K, false, H, false>);
+            return e;
+        });
+        if (e0 != cudaSuccess) { q.err = e0; return; }
     }
     constexpr int GNG = GradGroups<K>::value, GTHREADS = 32 * GNG * GROUP_WARPS;
     const int grid = grad_grid(G, fs), nslot = grid * GNG;

@@ -5,7 +5,9 @@
 
 #include <cuda_runtime.h>
 
+#include <mutex>
 #include <string>
+#include <vector>
 
 #include "common.cuh"
 #include "stream.cuh"
@@ -17,6 +19,29 @@ namespace pcamm {
 void set_error(const std::string& msg);
 void count_launch(long long n);
 int model_K(const pcamm_model* m);   // api.cu
+
+// Function attributes (the opt-in to more than 48 KB of dynamic shared memory) are per device:
+// runs fn() the first time it is called while a given device is current (thread safe).
+class DeviceOnce {
+    std::mutex mu_;
+    std::vector<char> done_;
+
+  public:
+    template <class F>
+    cudaError_t run(F fn) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        std::lock_guard<std::mutex> lock(mu_);
+        if ((int)done_.size() > dev && done_[dev]) return cudaSuccess;
+        e = fn();
+        if (e == cudaSuccess) {
+            if ((int)done_.size() <= dev) done_.resize(dev + 1, 0);
+            done_[dev] = 1;
+        }
+        return e;
+    }
+};
 
 // A linear sequence of kernels.  stream mode: cudaLaunchKernel on `stream`.  graph mode: each
 // kernel becomes a node of `graph` depending on the previous one, so the solve can be replayed
@@ -86,10 +111,10 @@ void launch_warp(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, 
 // ---- a-2 (project.cu)
 int project_blocks(const Geom& G);
 int max_slabs(const Geom& G);
+extern int g_chunks_per_segment, g_scan_slabs;     // measurement knobs (pcamm_tune): 0 = automatic
+bool project_fits(const Geom& G);    // the knots of one scan row set fit into shared memory (nz up to ~ 4000)
 // in-plane traversal tables of the views of solves 0..B-1 (once per solve: the angle is fixed)
 void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, ColHdr* hdr, SlabEntry* tab);
-// p[s] = P f[s] for every active slot (volumes in the ray layout); per-block partial sums
-// {sum p, sum y p, sum (p - a y - b)^2}.
 int project_segments(const Geom& G);
 struct CtlBufs;
 // p[s] = P f[s] for every active slot (volumes in the ray layout; pseg: scratch

@@ -3,40 +3,44 @@
 //
 // Reading A3: p_i = sum_j l_ij f_j with l_ij the exact length of the source -> pixel-centre
 // segment inside voxel box j (Siddon's radiological path).  The oracle merges and sorts all plane
-// crossings; this kernel computes the same sum slab by slab:
+// crossings of every ray; this file computes the same sums from the structure of a flat detector
+// whose columns are parallel to the rotation axis:
 //
 //   the ray marches along its dominant in-plane axis m (|d_m|/h_m largest; t = the other in-plane
-//   axis).  Between the planes M = i and M = i+1 (voxel-corner index units) it moves by
-//   |sT| <= 1 voxels in t and |sZ| <= 1 voxels in z, so it crosses at most one t-plane and one
-//   z-plane inside the slab: at most three voxels, whose shares tau of the slab length follow
-//   from where those two crossings fall.  Summed over slabs this is exactly Siddon's sum.
+//   axis) through the slabs between the planes M = i and M = i+1 (voxel-corner index units).  ALL
+//   rays of one detector column share their in-plane path: in slab n they are in voxel column A_n
+//   for the share tt_n of the slab and in the transverse neighbour B_n for the rest (|sT| <= 1:
+//   at most one transverse crossing per slab).  The rows of the column differ only in WHERE they
+//   cross the axial (z) planes.  With the per-level path integral
 //
-// Split of the work.  On a flat detector whose rows are parallel to the rotation axis, all rays
-// of one detector column share their in-plane path; the gantry angle is fixed for the whole
-// solve (P varies per angle, not per iteration).  So the in-plane traversal is
-// tabulated ONCE per solve (k_view_tables: per column and slab the voxel column the ray is in
-// and the share tt of the slab before its t-plane crossing, evaluated directly in double), and
-// the projector, which runs once per line-search trial, only tracks the z crossings per ray (32.32
-// fixed-point counters set up in double) and accumulates at most three pieces per slab.
+//       S_k(q) = integral_0^q f[column(s)][k] ds       (q in slabs; piecewise linear in q)
 //
-// Mapping: one thread per ray, one warp per 32 consecutive detector rows of ONE column.  The
-// lanes of a warp are in the same (x, y) voxel column and ~11 neighbouring z, so with the
-// z-fastest ray layout of the trial volumes (common.cuh) every load of a warp falls into one or
-// two 128 B lines at any gantry angle; the table entry of a slab is one broadcast 8-byte load;
-// the trip count is uniform over the warp.  The volume was just written by the warp kernel and is
-// L2/L1-resident: this kernel is bound by instruction issue, not by HBM.
+//   the line integral of a ray that is in level k_0 until its crossing q_1, in k_1 until q_2, ...
+//   is  Ls * sum_m [ S_{k_m}(q_{m+1}) - S_{k_m}(q_m) ]  (Ls = mm of path per slab): exactly
+//   Siddon's sum, regrouped.
 //
-// The rays are cut into segments of SEG slabs (one block per segment of 4 columns x 32 rows);
-// the block of a ray group that finishes last adds the segments and forms the a-3 sums.
+// Split of the work.  The gantry angle is fixed for the whole solve (P varies per
+// angle, not per iteration), so the in-plane traversal is tabulated ONCE per solve (k_view_tables:
+// per column and slab the voxel column A_n and the share tt_n, evaluated directly in double).
+// The projector, which runs once per line-search trial, takes one block per (detector column,
+// segment of CH slabs):
+//   phase 1  each warp scans SC slabs for every level at once (lanes = z, coalesced 128-bit loads
+//            of the z-fastest ray layout, all loads of the scan in flight together) and leaves the
+//            knots of S_k (slab entry, transverse crossing, slab exit; prefix restarted per warp)
+//            in shared memory: (levels x slabs) work, shared by all rows of the column, instead of
+//            (rows x slabs) gathers;
+//   phase 2  one thread per row: the z crossings of its ray (32.32 fixed-point counters set up in
+//            double) are walked in order; each costs one interpolated look-up of two levels'
+//            knots, each scan adds its end knot at the ray's current level.
+// The block of a column that finishes last adds the segments and forms the a-3 sums.
 #include "internal.h"
 
 namespace pcamm {
 
 namespace {
 
-constexpr int PW = 4;             // warps (= detector columns) per block
-constexpr int NT = 32 * PW;
-constexpr int SEG = 64;           // slabs per block (a multiple of the march's group size)
+constexpr int PT = 384;           // threads of a projector block
+constexpr int PWARPS = PT / 32;   // = scans per block (one per warp)
 
 constexpr double FIX = 4294967296.0;            // 2^32
 constexpr double QMAX = 1073741824.0;           // crossings beyond any volume are parked here (2^30 slabs)
@@ -96,7 +100,7 @@ k_view_tables(const Geom G, const SolveState* __restrict__ solves, ColHdr* __res
     const View vw = solves[b].view;
     double dxy2;
     const ColSetup c = col_setup(G, vw, iu, &dxy2);
-    const int strideT = (c.axis == 0 ? G.pnx : 1) * G.nz;
+    const int strideT = c.axis == 0 ? G.pnx : 1;
     if (threadIdx.x == 0) {
         ColHdr h;
         h.lam0 = (c.Mb - c.Sm) / c.gm;
@@ -121,21 +125,21 @@ k_view_tables(const Geom G, const SolveState* __restrict__ solves, ColHdr* __res
         tt = fmin(fmax(tt, 0.0), 1.0);
         const int jx = c.axis == 0 ? i : j, jy = c.axis == 0 ? j : i;
         SlabEntry e;
-        e.off0 = ((jy + 1) * G.pnx + (jx + 1)) * G.nz;
-        e.tt = (float)(tt * 4294967296.0);       // in units of 2^-32 of the slab (see march)
+        e.col = (jy + 1) * G.pnx + (jx + 1);
+        e.tt = (float)(tt * 4294967296.0);       // in units of 2^-32 of the slab
         row[n] = e;
     }
     // null entries up to the end of the (padded) row: a zero-valued border column whose
     // transverse neighbours are inside the buffer, no crossing
     for (int n = c.n_slabs + threadIdx.x; n < max_slabs; n += blockDim.x) {
         SlabEntry e;
-        e.off0 = G.pnx * G.nz;            // (x, y) = (-1, 0)
+        e.col = G.pnx;                    // (x, y) = (-1, 0)
         e.tt = 4294967296.f;
         row[n] = e;
     }
 }
 
-// ------------------------------------------------------------------ per-ray z tracking and the march
+// ------------------------------------------------------------------ per-ray z tracking
 
 // The crossings of axial (z) voxel planes are tracked as 32.32 fixed-point values of the slab
 // coordinate q: hi word = slab in which the crossing falls, lo word = share of that slab's path
@@ -144,222 +148,357 @@ k_view_tables(const Geom G, const SolveState* __restrict__ solves, ColHdr* __res
 // almost parallel to the planes that rounding, divided by the slope, would misplace the crossing
 // by whole slabs).
 struct RayZ {
-    int k, dirZ;
-    unsigned long long QZ, dQZ;
-    float Ls;                       // mm of path per slab
-    int kmin, kmax;                 // bounds of the axial indices met in n_slabs slabs
+    int k, dirZ;                    // level at the entry of the first slab; +1 / -1 / 0 per crossing
+    unsigned long long QZ, dQZ;     // next crossing and the spacing of the crossings
 };
 
-__device__ __forceinline__ void first_crossing(double P0, double s, int* idx0, int* dir, unsigned long long* Q,
-                                               unsigned long long* dQ) {
-    const double fl = floor(P0);
-    *idx0 = (int)fl;
-    if (s == 0.0) { *dir = 0; *Q = (unsigned long long)(QMAX * FIX); *dQ = 0ull; return; }
-    *dir = s > 0.0 ? 1 : -1;
-    const double plane = s > 0.0 ? fl + 1.0 : fl;
-    const double q = fmin(fmax((plane - P0) / s, 0.0), QMAX);
-    const double d = fmin(1.0 / fabs(s), QMAX);
-    *Q = (unsigned long long)(q * FIX + 0.5);
-    *dQ = (unsigned long long)(d * FIX + 0.5);
-    if (*dQ < (1ull << 32)) *dQ = 1ull << 32;   // |s| <= 1: never two crossings in one slab
-}
-
 // z state of the ray of row iv at the entry of slab n0 of its column (slabs are then counted
-// from there), for a march of n slabs.
-__device__ __forceinline__ RayZ make_ray_z(const Geom& G, const ColHdr& h, int iv, int n0, int n) {
+// from there).  first_crossing() with the divisions by the slope replaced by one reciprocal.
+__device__ __forceinline__ RayZ make_ray_z(const Geom& G, const ColHdr& h, int iv, int n0) {
     RayZ r;
     const double dz = ((double)iv - 0.5 * (G.nv - 1) + (double)G.off_v) * (double)G.pv;
-    const double gz = dz / (double)G.hz;
-    const double Szi = (0.0 - G.loz) / (double)G.hz;                      // the source is in the plane z = 0
+    const double gz = dz * G.ihz_d;
     const double sz = gz * h.kap;                                         // z per slab
-    first_crossing(fma(gz, fma(h.kap, (double)n0, h.lam0), Szi), sz, &r.k, &r.dirZ, &r.QZ, &r.dQZ);
-    r.Ls = (float)(sqrt((double)h.dxy2 + dz * dz) * h.kap);            // mm per slab
-    const int ncross = (int)(fabs(sz) * (double)n) + 2;                   // conservative
-    r.kmin = r.dirZ < 0 ? r.k - ncross : r.k;
-    r.kmax = r.dirZ > 0 ? r.k + ncross : r.k;
+    const double P0 = fma(gz, fma(h.kap, (double)n0, h.lam0), G.Szi);     // z (voxel-corner units) at the slab's entry
+    const double fl = floor(P0);
+    r.k = (int)fl;
+    if (sz == 0.0) { r.dirZ = 0; r.QZ = (unsigned long long)(QMAX * FIX); r.dQZ = 0ull; return r; }
+    r.dirZ = sz > 0.0 ? 1 : -1;
+    const double inv = 1.0 / fabs(sz);
+    const double dist = sz > 0.0 ? fl + 1.0 - P0 : P0 - fl;               // to the next plane, in voxels
+    const double q = fmin(dist * inv, QMAX), d = fmin(inv, QMAX);
+    r.QZ = (unsigned long long)(q * FIX + 0.5);
+    r.dQZ = (unsigned long long)(d * FIX + 0.5);
+    if (r.dQZ < (1ull << 32)) r.dQZ = 1ull << 32;                         // |sz| <= 1 (reading B2)
     return r;
 }
 
-// Runs the slabs of one ray, source side first, U at a time.  Per piece the sink is asked first
-// to fetch (off = element offset of the voxel column (i, j), k = axial index) and later to add
-// (off, k, tau = share of the slab's path length, fetched value): all fetches of a group of U
-// slabs are issued before the first add, and the table entries of the next group are loaded
-// while this one is worked on.  Rows are padded with null entries (zero-valued border column,
-// tt = 1) to a multiple of U plus one group, so there is no remainder loop.  Pieces of zero
-// share are passed on (the sink ignores or drops them).
-constexpr int U = 4;
+// mm of path per slab of the ray of row iv in the column of header h
+__device__ __forceinline__ float ray_slab_length(const Geom& G, const ColHdr& h, int iv) {
+    const double dz = ((double)iv - 0.5 * (G.nv - 1) + (double)G.off_v) * (double)G.pv;
+    return (float)(sqrt((double)h.dxy2 + dz * dz) * h.kap);
+}
 
-template <class Sink>
-__device__ __forceinline__ void march(const SlabEntry* __restrict__ row, int n_slabs, int dT, RayZ r, Sink& sink) {
-    const int4* row4 = reinterpret_cast<const int4*>(row);          // two entries per 16 B
+// ------------------------------------------------------------------ the pieces of one ray, in order
+//
+// pcamm_traverse: the ordered voxels and lengths of one ray, from the same table entries and the
+// same crossing counters the projector integrates over.  Per slab at most three pieces: the
+// transverse crossing (share tt of the table) and the z crossing (share tz of the counter) cut it.
+struct RecSink {
+    int cap, n;
+    int nx, ny, nz, pnx;
+    float Ls, eps;
+    int* ijk;
+    float* len;
+    __device__ __forceinline__ void add(int col, int k, float tau_raw) {
+        if (!((unsigned)k < (unsigned)nz)) return;
+        const float tau = tau_raw * 2.3283064365386963e-10f;                // shares come in units of 2^-32
+        const int jy = col / pnx - 1, jx = col % pnx - 1;
+        if (!((unsigned)jx < (unsigned)nx && (unsigned)jy < (unsigned)ny)) return;      // zero border
+        const float l = tau * Ls;
+        if (!(l > eps)) return;     // zero-length pieces are dropped (reading A22)
+        if (n < cap) {
+            ijk[3 * n + 0] = jx;
+            ijk[3 * n + 1] = jy;
+            ijk[3 * n + 2] = k;
+            len[n] = l;
+        }
+        ++n;
+    }
+};
+
+__device__ __forceinline__ void walk_pieces(const SlabEntry* __restrict__ row, int n_slabs, int dT, RayZ r, RecSink& sink) {
     int k = r.k;
-    unsigned qlo = (unsigned)r.QZ, qhi = (unsigned)(r.QZ >> 32);     // next z crossing: slab, share * 2^32
-    const unsigned dlo = (unsigned)r.dQZ, dhi = (unsigned)(r.dQZ >> 32);
-    int4 ea = __ldg(row4), eb = __ldg(row4 + 1);
-    for (int n0 = 0; n0 < n_slabs; n0 += U) {
-        const int4 na = __ldg(row4 + (n0 >> 1) + 2), nb = __ldg(row4 + (n0 >> 1) + 3);   // next group
-        const int off0s[U] = {ea.x, ea.z, eb.x, eb.z};
-        const float tts[U] = {__int_as_float(ea.y), __int_as_float(ea.w), __int_as_float(eb.y), __int_as_float(eb.w)};
-        int pi[U][3], pk[U][3];
-        float pt[U][3], pv[U][3];
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            // shares are kept in units of 2^-32 of a slab (the table's tt is stored that way and the
-            // crossing counter's low word is one already): the caller scales the sum once
-            const float tt = tts[u];
-            const bool cz = qhi == (unsigned)(n0 + u);
-            const float tz = cz ? __uint2float_rn(qlo) : 4294967296.f;
-            const int dk = cz ? r.dirZ : 0;
-            const float t1 = fminf(tt, tz), t2 = fmaxf(tt, tz);
-            const bool tfirst = tt < tz;
-            const int i0 = off0s[u] + k;
-            pi[u][0] = i0;                          pk[u][0] = k;                    pt[u][0] = t1;
-            pi[u][1] = i0 + (tfirst ? dT : dk);     pk[u][1] = tfirst ? k : k + dk;  pt[u][1] = t2 - t1;
-            pi[u][2] = i0 + dT + dk;                pk[u][2] = k + dk;               pt[u][2] = 4294967296.f - t2;
-#pragma unroll
-            for (int i = 0; i < 3; ++i) pv[u][i] = sink.fetch(pi[u][i], pk[u][i]);
-            k += dk;
-            asm("{\n"
-                ".reg .pred p;\n"
-                "setp.ne.s32 p, %2, 0;\n"
-                "@p add.cc.u32 %0, %0, %3;\n"
-                "@p addc.u32 %1, %1, %4;\n"
-                "}\n"
-                : "+r"(qlo), "+r"(qhi)
-                : "r"((int)cz), "r"(dlo), "r"(dhi));
-        }
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-#pragma unroll
-            for (int i = 0; i < 3; ++i) sink.add(pi[u][i], pk[u][i], pt[u][i], pv[u][i]);
-        }
-        ea = na; eb = nb;
+    unsigned long long Q = r.QZ;
+    for (int n = 0; n < n_slabs; ++n) {
+        const SlabEntry e = row[n];
+        const float tt = e.tt;                                        // units of 2^-32 of the slab
+        const bool cz = (unsigned)(Q >> 32) == (unsigned)n;
+        const float tz = cz ? __uint2float_rn((unsigned)Q) : 4294967296.f;
+        const int dk = cz ? r.dirZ : 0;
+        const float t1 = fminf(tt, tz), t2 = fmaxf(tt, tz);
+        const bool tfirst = tt < tz;
+        sink.add(e.col, k, t1);
+        sink.add(tfirst ? e.col + dT : e.col, tfirst ? k : k + dk, t2 - t1);
+        sink.add(e.col + dT, k + dk, 4294967296.f - t2);
+        k += dk;
+        if (cz) Q += r.dQZ;
     }
 }
 
-// CHECK = false: the caller has established that the ray stays inside [0, nz) for the whole
-// march (no per-piece test).
-template <bool CHECK>
-struct AccSink {
-    const float* __restrict__ vol;
-    int Nz;
-    float acc;
-    __device__ __forceinline__ float fetch(int idx, int k) const {      // idx = column offset + k
-        return (!CHECK || (unsigned)k < (unsigned)Nz) ? __ldg(vol + (unsigned)idx) : 0.f;
-    }
-    __device__ __forceinline__ void add(int, int, float tau, float v) { acc = fmaf(tau, v, acc); }
-};
+// ------------------------------------------------------------------ the projector
 
-// Grid: (columns / PW, row groups of 32, slots x segments).  A block marches SEG slabs of its
-// rays: the rows of the grid are cut into segments so that there are several times more blocks
-// than fit on the GPU at once and the hardware block scheduler keeps every SM busy to the end
-// (with one block per ray group everything is resident at once and the last third of the
-// kernel runs half empty: profiles/r01).  Segment s of a ray starts from the exact z state at
-// its first slab (double precision set-up) and writes its partial line integral to
-// pseg[slot][s][iu][iv]; the last block of the ray group adds the segments in index order.
-__global__ void __launch_bounds__(NT)
+// Knots of one scan: 2 SC + 1 rows (entry of slab 0, its transverse crossing, entry of slab 1, ...,
+// exit of slab SC - 1) of NZP floats: level k at element 4 + k, four zero floats in front (level -1
+// and alignment) and at least four behind (level nz): a ray outside the volume in z reads zeros.
+__host__ __device__ __forceinline__ int knot_pitch(int nz) { return (nz + 3) / 4 * 4 + 8; }
+
+// chunks per segment: their air masks (2 SC bits each) share one 32-bit ballot
+__host__ __device__ constexpr int max_cps(int sc) { return 32 / (2 * sc); }
+
+__device__ __forceinline__ void add64(unsigned& lo, unsigned& hi, unsigned dlo, unsigned dhi) {
+    asm("add.cc.u32 %0, %0, %2;\n\taddc.u32 %1, %1, %3;" : "+r"(lo), "+r"(hi) : "r"(dlo), "r"(dhi));
+}
+
+// Grid: (detector columns, segments x row blocks, slots).  A block takes the rows
+// rb RPT PT .. + RPT PT - 1 of its column through the n_chunks chunks (of CH = PWARPS SC slabs) of
+// its segment; the ray state lives in registers from chunk to chunk.  VEC: levels per lane and load
+// (4 where nz is a multiple of 4, else 1).  Segment g writes the sums of all its rows (in slabs,
+// not yet mm) to pseg[slot][g][iu][iv]; the block of the column that finishes last adds the
+// segments in index order and multiplies by the path length per slab.
+//
+// Per chunk: (1) the scans, one per warp; (2) the prefix of the scans' end knots over the chunk,
+// P[c][k] = S_k at the entry of scan c, so that S_k(q) = P[c][k] + (the scan's own knots); (3) per
+// ray the crossings that fall into the chunk, in order: S_k(q) - S_{k+dirZ}(q) each, and S at the
+// chunk's exit at the level the ray has by then.
+template <int VEC, int SC, int RPT>
+__global__ void __launch_bounds__(PT, SC == 4 ? 3 : 4)
 k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* __restrict__ solves,
           const SolveIn* __restrict__ in, const ColHdr* __restrict__ hdr, const SlabEntry* __restrict__ tab,
-          int max_slabs, int n_seg, const float* __restrict__ vol, const unsigned char* __restrict__ occ,
-          float* pseg, float* __restrict__ p_out, double* __restrict__ partials, int* seg_ticket) {
-    __shared__ double red[NT / 32];
+          int max_slabs, int n_seg, int n_chunks, int NZP, const float* __restrict__ vol,
+          const unsigned char* __restrict__ occ, float* pseg, float* __restrict__ p_out, double* __restrict__ partials,
+          int* seg_ticket) {
+    constexpr int CH = PWARPS * SC, NKNOT = 2 * SC + 1;
+    constexpr int LOG_SC = SC == 4 ? 2 : (SC == 2 ? 1 : 0);
+    extern __shared__ __align__(16) float s_knots[];        // [PWARPS][NKNOT][NZP], then P [PWARPS + 1][NZP]
+    __shared__ float s_tt[CH];
+    __shared__ float2 s_inv[CH];                             // 1 / tt and 1 / (1 - tt) (0 where there is nothing to divide)
+    __shared__ int s_air[PWARPS];
+    __shared__ double red[PT / 32];
     __shared__ int s_last;
-    const int s = blockIdx.z / n_seg, seg = blockIdx.z % n_seg;
+    int seg = blockIdx.y, rb = 0;
+    if (seg >= n_seg) { rb = seg / n_seg; seg -= rb * n_seg; }
+    const int iu = blockIdx.x, s = blockIdx.z;
     if (!slots[s].active) return;                            // uniform over the block
     const int b = slots[s].solve;
-    const int iu = blockIdx.x * PW + (threadIdx.x >> 5);
-    const int iv = blockIdx.y * 32 + (threadIdx.x & 31);
-    const bool col_ok = iu < G.nu, ray_ok = col_ok && iv < G.nv;
-    ColHdr h;
-    h.n_slabs = 0; h.dT = 0; h.lam0 = 0.0; h.kap = 0.0; h.dxy2 = 0.f; h.axis = 0;
-    if (col_ok) h = hdr[(long long)b * G.nu + iu];
-    int n0 = seg * SEG, n = min(h.n_slabs - n0, SEG);
-    const SlabEntry* row = tab + ((long long)b * G.nu + (col_ok ? iu : 0)) * max_slabs + n0;
-    float p = 0.f;
-    if (n > 0) {
-        // Slabs in air add an exact +0: trim the segment to the span of slabs whose voxel columns
-        // hold something (occupancy written with the volume; the lanes share the column, so the
-        // test is split over them and the result is uniform over the warp).
-        {
-            const unsigned long long* ow = reinterpret_cast<const unsigned long long*>(occ + (long long)s * G.OCC);
-            const int words = G.occ_pitch >> 3, lane = threadIdx.x & 31;
-            unsigned long long span = 0ull;
-#pragma unroll
-            for (int part = 0; part < SEG / 32; ++part) {
-                const int sl = part * 32 + lane;
-                bool o = false;
-                if (sl < n) {
-                    const int off0 = __ldg(&row[sl].off0);
-                    const int c0 = off0 / G.nz, c1 = (off0 + h.dT) / G.nz;
-                    for (int wd = 0; wd < words; ++wd)
-                        o |= (__ldg(ow + (long long)c0 * words + wd) | __ldg(ow + (long long)c1 * words + wd)) != 0ull;
-                }
-                span |= (unsigned long long)__ballot_sync(0xffffffffu, o) << (32 * part);
-            }
-            if (span == 0ull) n = 0;
-            else {
-                const int first = (__ffsll((long long)span) - 1) & ~(U - 1);
-                const int last = 63 - __clzll((long long)span);
-                n = min(n, (last & ~(U - 1)) + U) - first;
-                n0 += first;
-                row += first;
-            }
-        }
-    }
-    if (ray_ok && n > 0) {
-        const RayZ r = make_ray_z(G, h, iv, n0, n);
-        const float* base = vol + (long long)s * G.PV;
-        asm volatile("" : "+l"(base));       // one base pointer; 32-bit offsets in the loop
-        float acc;
-        if (r.kmin >= 0 && r.kmax < G.nz) {
-            AccSink<false> sink{base, G.nz, 0.f};
-            march(row, n, h.dT, r, sink);
-            acc = sink.acc;
-        } else {
-            AccSink<true> sink{base, G.nz, 0.f};
-            march(row, n, h.dT, r, sink);
-            acc = sink.acc;
-        }
-        p = acc * (r.Ls * 2.3283064365386963e-10f);      // the shares were summed in units of 2^-32
-    }
-    float* my_seg = pseg + (((long long)s * n_seg + seg) * G.nu + (col_ok ? iu : 0)) * G.nv + (ray_ok ? iv : 0);
-    if (ray_ok && n_seg > 1) *my_seg = p;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int p_off = PWARPS * NKNOT * NZP;                  // start of P in s_knots
+    const int kw = warp * NKNOT * NZP;                       // this warp's knot rows
+    const ColHdr h = hdr[b * G.nu + iu];
+    const int n0 = seg * n_chunks * CH;
+    const SlabEntry* rows = tab + ((long long)b * G.nu + iu) * max_slabs + n0 + warp * SC;   // this warp's first scan
+    const float* base = vol + (long long)s * G.PV;
+    const int dTe = h.dT * G.nz;                             // element offset of the transverse neighbour
 
-    // The block of this ray group (PW columns x 32 rows) that finishes last adds the segments in
-    // index order and forms a-3 for its rays: r_i = p_i - a y_i - b with the per-group partial sums
-    // of p, y p and r^2 (Eq. 2, L91-93 Eq. 4) in double.
-    const int ngroups = gridDim.x * gridDim.y, grp = blockIdx.y * gridDim.x + blockIdx.x;
-    if (n_seg > 1) {
-        __threadfence();
-        __syncthreads();
+    // the rays of this thread: level (+ 4: index into a knot row), next crossing (relative to slab n0), running sum
+    int rk[RPT], rdir[RPT];
+    unsigned rqlo[RPT], rqhi[RPT], rdlo[RPT], rdhi[RPT];
+    float racc[RPT];
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) {
+        const int iv = (rb * RPT + r) * PT + threadIdx.x;
+        rk[r] = 4; rdir[r] = 0; rqlo[r] = 0u; rqhi[r] = 0xffffffffu; rdlo[r] = rdhi[r] = 0u; racc[r] = 0.f;
+        if (iv < G.nv && n0 < h.n_slabs) {
+            const RayZ z = make_ray_z(G, h, iv, n0);
+            rk[r] = z.k + 4; rdir[r] = z.dirZ;
+            rqlo[r] = (unsigned)z.QZ; rqhi[r] = (unsigned)(z.QZ >> 32);
+            rdlo[r] = (unsigned)z.dQZ; rdhi[r] = (unsigned)(z.dQZ >> 32);
+        }
+    }
+    // Slabs in air add an exact +0 (reading B8).  Per scan of this warp in every chunk of the segment:
+    // the occupancy of the column the ray is in and, if it crosses into the transverse neighbour,
+    // of that one.  Lane = (chunk, slab, A | B): bit 2 SC j + 2 i of the mask says that slab i of the
+    // warp's scan in chunk j has something in A, the next bit the same for B.
+    unsigned masks;
+    {
+        const int words = G.occ_pitch >> 3;
+        const unsigned long long* ow = reinterpret_cast<const unsigned long long*>(occ + (long long)s * G.OCC);
+        const int j = lane / (2 * SC), i = (lane / 2) % SC;
+        bool has = false;
+        if (j < n_chunks && n0 + j * CH < h.n_slabs) {
+            const SlabEntry e = rows[j * CH + i];
+            if ((lane & 1) == 0 || e.tt < 4294967296.f) {
+                const unsigned long long* o = ow + (e.col + (lane & 1) * h.dT) * words;
+                for (int wd = 0; wd < words; ++wd) has |= __ldg(o + wd) != 0ull;
+            }
+        }
+        masks = __ballot_sync(0xffffffffu, has);
+    }
+    {   // the zero levels -1 and nz of this warp's knot rows (and the padding), never written again
+        const int wpad = NZP - 4 - G.nz;
+        if (lane < 4 + wpad) {
+            const int e = lane < 4 ? lane : G.nz + lane;
+#pragma unroll
+            for (int i = 0; i < NKNOT; ++i) s_knots[kw + i * NZP + e] = 0.f;
+        }
+        if (warp == 0 && lane < 4 + wpad) {                  // and of the prefix rows
+            const int e = lane < 4 ? lane : G.nz + lane;
+            for (int i = 0; i <= PWARPS; ++i) s_knots[p_off + i * NZP + e] = 0.f;
+        }
+    }
+
+    for (int j = 0; j < n_chunks; ++j) {
+        if (n0 + j * CH >= h.n_slabs) break;                 // uniform over the block
+        // ---- (1) warp w scans slabs n0 + j CH + w SC .. + SC - 1 (null entries behind the column's
+        //      last slab: a zero-valued border column without occupancy)
+        const unsigned m = (masks >> (2 * SC * j)) & ((1u << (2 * SC)) - 1u);
+        const SlabEntry* row = rows + j * CH;
+        if (lane < SC) {
+            const float tt = row[lane].tt, ot = 4294967296.f - tt;
+            s_tt[warp * SC + lane] = tt;
+            s_inv[warp * SC + lane] = make_float2(tt > 0.f ? __fdividef(1.f, tt) : 0.f, ot > 0.f ? __fdividef(1.f, ot) : 0.f);
+        }
+        if (lane == 0) s_air[warp] = m == 0u;
+        if (m != 0u) {                                       // uniform over the warp
+            for (int zp = 0; zp < G.nz; zp += 32 * VEC) {
+                const int z = zp + lane * VEC;
+                const bool ok = z < G.nz;
+                const float* bz = base + (ok ? z : 0);       // lanes beyond the last level load level 0 and store nothing
+                float A[SC][VEC], Bv[SC][VEC];
+#pragma unroll
+                for (int i = 0; i < SC; ++i) {               // every load of the scan before the first use
+                    const float* pa = bz + __ldg(&row[i].col) * G.nz;       // broadcast load
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) { A[i][v] = 0.f; Bv[i][v] = 0.f; }
+                    if ((m >> (2 * i)) & 1u) {               // uniform over the warp
+                        if (VEC == 4) {
+                            const float4 va = __ldg(reinterpret_cast<const float4*>(pa));
+                            A[i][0] = va.x; A[i][1 % VEC] = va.y; A[i][2 % VEC] = va.z; A[i][3 % VEC] = va.w;
+                        } else A[i][0] = __ldg(pa);
+                    }
+                    if ((m >> (2 * i + 1)) & 1u) {
+                        if (VEC == 4) {
+                            const float4 vb = __ldg(reinterpret_cast<const float4*>(pa + dTe));
+                            Bv[i][0] = vb.x; Bv[i][1 % VEC] = vb.y; Bv[i][2 % VEC] = vb.z; Bv[i][3 % VEC] = vb.w;
+                        } else Bv[i][0] = __ldg(pa + dTe);
+                    }
+                }
+                __syncwarp();                                // s_tt of this warp's slabs (written above)
+                float S[VEC];
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) S[v] = 0.f;
+                float* dst = s_knots + kw + 4 + z;
+                auto put = [&]() {
+                    if (ok) {
+                        if (VEC == 4) *reinterpret_cast<float4*>(dst) = make_float4(S[0], S[1 % VEC], S[2 % VEC], S[3 % VEC]);
+                        else dst[0] = S[0];
+                    }
+                    dst += NZP;
+                };
+#pragma unroll
+                for (int i = 0; i < SC; ++i) {
+                    const float tt = s_tt[warp * SC + i];
+                    const float ta = tt * 2.3283064365386963e-10f;          // the table's shares are in units of 2^-32
+                    const float tb = (4294967296.f - tt) * 2.3283064365386963e-10f;
+                    put();
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) S[v] = fmaf(ta, A[i][v], S[v]);
+                    put();
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) S[v] = fmaf(tb, Bv[i][v], S[v]);
+                }
+                put();
+            }
+        } else {                                             // an air scan: its end knots are zeros (for the prefix)
+            for (int i = lane; i < G.nz; i += 32) s_knots[kw + 2 * SC * NZP + 4 + i] = 0.f;
+        }
+        const int any = __syncthreads_or(m != 0u);
+        // ---- (2) prefix of the scans' end knots, per level
+        if (any) {                                           // uniform over the block
+            for (int i = threadIdx.x; i < G.nz; i += PT) {
+                float run = 0.f;
+                const float* e = s_knots + 2 * SC * NZP + 4 + i;
+                float* pp = s_knots + p_off + 4 + i;
+                pp[0] = 0.f;
+#pragma unroll
+                for (int c = 0; c < PWARPS; ++c) {
+                    run += e[c * NKNOT * NZP];
+                    pp[(c + 1) * NZP] = run;
+                }
+            }
+            __syncthreads();
+        }
+        // ---- (3) the crossings of this thread's rays that fall into the chunk
+        const unsigned end = (unsigned)((j + 1) * CH);
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) {
+            if (!any) {                                      // nothing to add: the crossings only move the level
+                while (rqhi[r] < end) { rk[r] += rdir[r]; add64(rqlo[r], rqhi[r], rdlo[r], rdhi[r]); }
+                continue;
+            }
+            int k = rk[r];
+            unsigned qlo = rqlo[r], qhi = rqhi[r];
+            float acc = racc[r];
+            const int dir = rdir[r], ktop = G.nz + 4;
+            while (qhi < end) {
+                // crossing from level k to k + dir at share tz of slab qhi: S_k(q) - S_{k + dir}(q),
+                // S linear between the knots on either side of q
+                const int rel = (int)qhi - j * CH, c = rel >> LOG_SC;
+                const int ka = min(max(k, 3), ktop), kb = min(max(k + dir, 3), ktop);
+                const int pc = p_off + c * NZP;
+                float dv = s_knots[pc + ka] - s_knots[pc + kb];
+                if (!s_air[c]) {
+                    const float tz = __uint2float_rn(qlo), tt = s_tt[rel];
+                    const float2 inv = s_inv[rel];
+                    const bool before = tz < tt;
+                    const float lam = before ? tz * inv.x : (tz - tt) * inv.y;
+                    const int k0 = (c * NKNOT + 2 * (rel & (SC - 1)) + (before ? 0 : 1)) * NZP;
+                    const float a0 = s_knots[k0 + ka], a1 = s_knots[k0 + NZP + ka];
+                    const float b0 = s_knots[k0 + kb], b1 = s_knots[k0 + NZP + kb];
+                    dv += (a0 - b0) + ((a1 - a0) - (b1 - b0)) * lam;
+                }
+                acc += dv;
+                k += dir;
+                add64(qlo, qhi, rdlo[r], rdhi[r]);
+            }
+            acc += s_knots[p_off + PWARPS * NZP + min(max(k, 3), ktop)];
+            rk[r] = k; rqlo[r] = qlo; rqhi[r] = qhi; racc[r] = acc;
+        }
+        __syncthreads();                                     // the next chunk's scans overwrite the knots
+    }
+
+    // The block of this column that finishes last adds the segments in index order and forms a-3
+    // for its rays: r_i = p_i - a y_i - b with the per-column partial sums of p, y p and r^2
+    // (Eq. 2, L91-93 Eq. 4) in double.
+    const int n_part = gridDim.y;                            // segments x row blocks of this column
+    if (n_part > 1) {
+        float* my = pseg + (((long long)s * n_seg + seg) * G.nu + iu) * G.nv;
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) {
+            const int iv = (rb * RPT + r) * PT + threadIdx.x;
+            if (iv < G.nv) my[iv] = racc[r];
+        }
+        __syncthreads();                                     // the block's stores are ordered before thread 0's fence
         if (threadIdx.x == 0) {
-            int* t = seg_ticket + (long long)s * ngroups + grp;
+            __threadfence();
+            int* t = seg_ticket + s * G.nu + iu;
             const int k = atomicAdd(t, 1);
-            s_last = k == n_seg - 1;
-            if (s_last) *t = 0;
+            s_last = k == n_part - 1;
+            if (s_last) { *t = 0; __threadfence(); }
         }
         __syncthreads();
         if (!s_last) return;
-        __threadfence();
-        if (ray_ok) {
-            p = 0.f;
-            for (int g = 0; g < n_seg; ++g)
-                p += __ldcg(pseg + (((long long)s * n_seg + g) * G.nu + iu) * G.nv + iv);
-        }
     }
     double vp = 0.0, vyp = 0.0, vrr = 0.0;
-    if (ray_ok) {
-        const int pix = iv * G.nu + iu;
+    const float* y = in[b].y;
+    const double fa = solves[b].a, fb = solves[b].b;
+    auto finish = [&](int iv, float acc) {
+        const long long pix = (long long)iv * G.nu + iu;
+        const float p = acc * ray_slab_length(G, h, iv);
         p_out[(long long)s * G.npix + pix] = p;
-        const float* y = in[b].y;
         const double yv = y ? (double)__ldg(y + pix) : 0.0;
-        const double res = (double)p - solves[b].a * yv - solves[b].b;   // Eq. (2) residual
-        vp = (double)p; vyp = yv * (double)p; vrr = res * res;
+        const double res = (double)p - fa * yv - fb;                      // Eq. (2) residual
+        vp += (double)p; vyp += yv * (double)p; vrr += res * res;
+    };
+    if (n_part > 1) {
+        const float* ps = pseg + ((long long)s * n_seg * G.nu + iu) * G.nv;
+        const long long gstride = (long long)G.nu * G.nv;
+        for (int iv = threadIdx.x; iv < G.nv; iv += PT) {
+            float acc = 0.f;
+            for (int g = 0; g < n_seg; ++g) acc += __ldcg(ps + g * gstride + iv);
+            finish(iv, acc);
+        }
+    } else {                                                 // this block had the whole column
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) {
+            const int iv = r * PT + threadIdx.x;
+            if (iv < G.nv) finish(iv, racc[r]);
+        }
     }
-    double* out = partials + ((long long)s * ngroups + grp) * 3;
-    const double sp = block_sum<NT>(vp, red);
-    const double syp = block_sum<NT>(vyp, red);
-    const double srr = block_sum<NT>(vrr, red);
+    double* out = partials + ((long long)s * G.nu + iu) * 3;
+    const double sp = block_sum<PT>(vp, red);
+    const double syp = block_sum<PT>(vyp, red);
+    const double srr = block_sum<PT>(vrr, red);
     if (threadIdx.x == 0) { out[0] = sp; out[1] = syp; out[2] = srr; }
 }
 
@@ -386,31 +525,7 @@ k_to_ray_layout(const Geom G, const float* __restrict__ src, float* __restrict__
     }
 }
 
-struct RecSink {
-    int cap, n;
-    int nx, ny, nz, pnx;
-    float Ls, eps;
-    int* ijk;
-    float* len;
-    __device__ __forceinline__ float fetch(int, int) const { return 0.f; }
-    __device__ __forceinline__ void add(int idx, int k, float tau_raw, float) {
-        if (!((unsigned)k < (unsigned)nz)) return;
-        const float tau = tau_raw * 2.3283064365386963e-10f;                // shares come in units of 2^-32
-        const int col = (idx - k) / nz, jy = col / pnx - 1, jx = col % pnx - 1;
-        if (!((unsigned)jx < (unsigned)nx && (unsigned)jy < (unsigned)ny)) return;      // zero border
-        const float l = tau * Ls;
-        if (!(l > eps)) return;     // zero-length pieces are dropped (reading A22)
-        if (n < cap) {
-            ijk[3 * n + 0] = jx;
-            ijk[3 * n + 1] = jy;
-            ijk[3 * n + 2] = k;
-            len[n] = l;
-        }
-        ++n;
-    }
-};
-
-// One ray through the projector's own tables and march (pcamm_traverse).
+// One ray through the projector's own tables and crossing counters (pcamm_traverse).
 __global__ void k_traverse(const Geom G, const ColHdr* __restrict__ hdr, const SlabEntry* __restrict__ tab,
                            int max_slabs, int iu, int iv, int cap, int* ijk, float* len, int* n_out) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
@@ -421,31 +536,91 @@ __global__ void k_traverse(const Geom G, const ColHdr* __restrict__ hdr, const S
     sink.Ls = 0.f;
     sink.ijk = ijk; sink.len = len;
     if (h.n_slabs > 0) {
-        const RayZ r = make_ray_z(G, h, iv, 0, h.n_slabs);
-        sink.Ls = r.Ls;
-        march(tab + (long long)iu * max_slabs, h.n_slabs, h.dT, r, sink);
+        const RayZ r = make_ray_z(G, h, iv, 0);
+        sink.Ls = ray_slab_length(G, h, iv);
+        walk_pieces(tab + (long long)iu * max_slabs, h.n_slabs, h.dT, r, sink);
     }
     *n_out = sink.n;
 }
 
 }  // namespace
 
-int project_blocks(const Geom& G) { return ((G.nu + PW - 1) / PW) * ((G.nv + 31) / 32); }
-// slabs per table row: the longest march, rounded up to the group size, plus one group read ahead
-int max_slabs(const Geom& G) { return ((G.nx > G.ny ? G.nx : G.ny) + U - 1) / U * U + U; }
-int project_segments(const Geom& G) { return ((G.nx > G.ny ? G.nx : G.ny) + SEG - 1) / SEG; }
+// Slabs per scan: the most whose knots leave room for three blocks per SM (the block's shared memory
+// is PWARPS (2 SC + 1) knot rows and PWARPS + 1 prefix rows of knot_pitch(nz) floats).
+int g_scan_slabs = 0;                                       // 0: automatic (pcamm_tune "project_scan_slabs")
+int scan_slabs(const Geom& G) {
+    const size_t row = sizeof(float) * (size_t)knot_pitch(G.nz);
+    if (g_scan_slabs == 1 || g_scan_slabs == 2 || g_scan_slabs == 4) {
+        if (row * (PWARPS * (2 * g_scan_slabs + 2) + 1) <= 200 * 1024) return g_scan_slabs;
+    }
+    if (row * (PWARPS * 10 + 1) <= 75 * 1024) return 4;
+    if (row * (PWARPS * 6 + 1) <= 75 * 1024) return 2;
+    return 1;
+}
+size_t project_smem(const Geom& G) {
+    return sizeof(float) * (size_t)knot_pitch(G.nz) * (PWARPS * (2 * scan_slabs(G) + 2) + 1);
+}
+bool project_fits(const Geom& G) { return project_smem(G) <= 200 * 1024; }
+
+// partial-sum groups per slot: one per detector column
+int project_blocks(const Geom& G) { return G.nu; }
+// chunks (of PWARPS scans) of the longest march
+int project_chunks(const Geom& G) {
+    const int ch = PWARPS * scan_slabs(G);
+    return ((G.nx > G.ny ? G.nx : G.ny) + ch - 1) / ch;
+}
+// Chunks per block: a column's march is cut into segments so that the grid has several waves of
+// blocks (the ray set-up is paid once per segment and ray).
+int g_chunks_per_segment = 0;                              // 0: automatic (pcamm_tune "project_chunks_per_segment")
+int chunks_per_segment(const Geom& G) {
+    const int nc = project_chunks(G);
+    const int mc = max_cps(scan_slabs(G)), cap = nc < mc ? nc : mc;
+    if (g_chunks_per_segment > 0) return g_chunks_per_segment < cap ? g_chunks_per_segment : cap;
+    int cps = cap;                                         // the fewest segments that still give >= 1024 blocks
+    while (cps > 1 && (long long)G.nu * ((nc + cps - 1) / cps) * ((G.nv + 2 * PT - 1) / (2 * PT)) < 1024) --cps;
+    return cps;
+}
+// upper bound (scratch is sized for one chunk per segment)
+int project_segments(const Geom& G) { return project_chunks(G); }
+// slabs per table row: whole chunks (null entries behind the column's last slab)
+int max_slabs(const Geom& G) { return project_chunks(G) * PWARPS * scan_slabs(G); }
 
 void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, ColHdr* hdr, SlabEntry* tab) {
     q.launch(k_view_tables, dim3(G.nu, B), dim3(128), 0, G, solves, hdr, tab, max_slabs(G));
 }
 
+template <int VEC, int SC, int RPT>
+void launch_project_t(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const ColHdr* hdr, const SlabEntry* tab,
+                      const float* vol, const unsigned char* occ, float* pseg, float* p) {
+    static DeviceOnce configured;
+    const size_t smem = project_smem(G);
+    const cudaError_t e = configured.run([&] {
+        return cudaFuncSetAttribute(k_project<VEC, SC, RPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    });
+    if (e != cudaSuccess) { q.err = e; return; }
+    const int cps = chunks_per_segment(G), n_seg = (project_chunks(G) + cps - 1) / cps;
+    const int row_blocks = (G.nv + RPT * PT - 1) / (RPT * PT);
+    for (int s0 = 0; s0 < nslots; s0 += 65535) {              // gridDim.z
+        const int ns = nslots - s0 < 65535 ? nslots - s0 : 65535;
+        q.launch(k_project<VEC, SC, RPT>, dim3(G.nu, n_seg * row_blocks, ns), dim3(PT), smem, G, (const SlotState*)c.slots + s0,
+                 (const SolveState*)c.solves, (const SolveIn*)c.in, hdr, tab, max_slabs(G), n_seg, cps, knot_pitch(G.nz),
+                 vol + (long long)s0 * G.PV, occ + (long long)s0 * G.OCC, pseg + (long long)s0 * n_seg * G.npix,
+                 p + (long long)s0 * G.npix, c.proj_part + (long long)s0 * G.nu * 3, c.seg_ticket + (long long)s0 * G.nu);
+    }
+}
+
 void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const ColHdr* hdr, const SlabEntry* tab,
                     const float* vol, const unsigned char* occ, float* pseg, float* p, int then,
                     cudaGraphConditionalHandle h, int use_cond) {
-    const int n_seg = project_segments(G);
-    q.launch(k_project, dim3((G.nu + PW - 1) / PW, (G.nv + 31) / 32, nslots * n_seg), dim3(NT), 0, G,
-             (const SlotState*)c.slots, (const SolveState*)c.solves, (const SolveIn*)c.in, hdr, tab, max_slabs(G), n_seg, vol,
-             occ, pseg, p, c.proj_part, c.seg_ticket);
+    const int sc = scan_slabs(G);
+    const bool v4 = G.nz % 4 == 0, one = G.nv <= PT;
+#define PCAMM_PROJ(VEC, SC) \
+    do { if (one) launch_project_t<VEC, SC, 1>(q, G, c, nslots, hdr, tab, vol, occ, pseg, p); \
+         else launch_project_t<VEC, SC, 2>(q, G, c, nslots, hdr, tab, vol, occ, pseg, p); } while (0)
+    if (sc == 4) { if (v4) PCAMM_PROJ(4, 4); else PCAMM_PROJ(1, 4); }
+    else if (sc == 2) { if (v4) PCAMM_PROJ(4, 2); else PCAMM_PROJ(1, 2); }
+    else { if (v4) PCAMM_PROJ(4, 1); else PCAMM_PROJ(1, 1); }
+#undef PCAMM_PROJ
     launch_ctl_after_project(q, G, c, then, h, use_cond);
 }
 

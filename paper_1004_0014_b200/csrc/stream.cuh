@@ -214,7 +214,9 @@ constexpr int SKIP_MIN_TILES_PER_SM = 12;
 
 // Reach of a tile's interpolation stencils: per axis the largest |floor(d)| any voxel can have,
 // from the bound on |d| (a small margin covers the float rounding of Eq. (1)).
-__device__ __forceinline__ int reach_of(float dmax) { return (int)ceilf(dmax * 1.0001f + 0.001f); }
+// Clamped to 2^20 voxels (beyond any grid every stencil is outside anyway; a huge or non-finite
+// bound must not wrap the int box arithmetic of the tile flags: it then simply covers the volume).
+__device__ __forceinline__ int reach_of(float dmax) { return (int)ceilf(fminf(dmax * 1.0001f + 0.001f, 1048576.f)); }
 
 // What the streaming kernels need to know about the model's fields.
 struct FieldStream {

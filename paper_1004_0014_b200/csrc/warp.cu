@@ -344,17 +344,19 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
 template <int K, bool RAY, bool H>
 void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots,
                 int nslots, float* vol_out, long long slot_stride, unsigned char* occ) {
-    static bool configured = false;
+    static DeviceOnce configured;
     constexpr size_t smem = warp_smem_bytes<K, H>();
     const CUtensorMap& fmap = field_map<K>(fs);
     const CUtensorMap& umap = half_map<K>(fs);
     const int n_sm = fs.n_sm;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    {
+        const cudaError_t e = configured.run([&] {
+            cudaError_t r = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (r == cudaSuccess)
+                r = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            return r;
+        });
         if (e != cudaSuccess) { q.err = e; return; }
-        configured = true;
     }
     const long long nt = tile_count(G, TileZ<K>::value);
     const int grid = (int)(nt < n_sm ? nt : n_sm);

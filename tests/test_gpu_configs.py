@@ -4,8 +4,8 @@ phantom, PCA of the training DVFs, measured projection from the oracle's project
 noise), CUDA path against the oracle through the C ABI.
 
 C0 and C1 run at full size.  C3 (K = 5 with hysteresis, all 8 candidate steps per line-search pass)
-and C4 (fine detector, several solves in flight) run on reduced grids with the same recipe, so that
-the oracle finishes in seconds; their full sizes are measured by bench.py.
+and C4 (fine detector, several solves in flight) run here on reduced grids with the same recipe and
+more iterations; their FULL sizes are tests/test_gpu_fullsize_c3c4.py.
 
 Bars (north_star; reading A16): w within 1e-3 ||w||, tumour position <= 0.05 mm, J and (a, b) to
 1e-3 / 1e-4; trajectories compared when the backtrack counts agree, else the oracle replays the

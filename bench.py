@@ -502,6 +502,72 @@ def run_frames_study(args, cfg, rank, local_rank):
                       "warmup": args.warmup, "grad_tol": tol, "max_iter": args.study_max_iter, "per_order": per}), flush=True)
 
 
+TL_KINDS = ("ysums", "begin", "view_tables", "warp", "project", "ctl_after_project", "resid", "gradient", "ctl_grad",
+            "iter_end", "final", "invert")
+
+
+def run_timeline(args, cfg, rank, local_rank):
+    """--timeline: the kernels of one solve of the timed workload, as the device saw them: start (first
+    block in) and end (last block out) of every kernel on the global timer, recorded inside the kernels
+    (pcamm_tune "timeline"; nsys is not installed in this image).  Prints one JSON line (not the bench
+    contract's): per kernel kind the count, the summed duration and the summed gap to the previous
+    kernel's end; with --timeline-out FILE also the event list as text."""
+    if rank != 0:
+        return
+    n = args.warmup + 1
+    wl = build_workload(cfg)
+    ids = list(range(FIRST_FRAME, FIRST_FRAME + n))
+    gts = ground_truth_volumes(wl, ids)
+    import torch
+    import paper_1004_0014_b200 as pc
+    for kv in args.tune:
+        name, _, value = kv.partition("=")
+        pc.tune(name, int(value))
+    pc.tune("timeline", 1)
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(dev)
+    m = pc.Model(nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, hx=cfg.hx, hy=cfg.hy, hz=cfg.hz, K=cfg.K, nu=cfg.nu, nv=cfg.nv,
+                 pu=cfg.pu, pv=cfg.pv, f0=t(wl.f0), mean_dvf=t(wl.model.mean), eig_dvf=t(wl.model.eig),
+                 landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=8 if cfg.batched_linesearch else 1)
+    opts = pc.Opts(max_iter=solver_iterations(cfg), batched_linesearch=1 if cfg.batched_linesearch else 0)
+    w = np.zeros(cfg.K, np.float32)
+    for i, fid in enumerate(ids):
+        fr = wl.frames[fid]
+        y = t(add_noise(m.project(t(gts[fid]), fr.angle_rad).cpu().numpy(), cfg.noise, seed=fid))
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        r = m.reconstruct(y, fr.angle_rad, w, opts)
+        e1.record()
+        torch.cuda.synchronize()
+        w = r.w
+    kind, t0, t1 = m.timeline()
+    per = {}
+    prev_end = None
+    for k, a, b in zip(kind, t0, t1):
+        d = per.setdefault(TL_KINDS[k], {"count": 0, "busy_us": 0.0, "gap_before_us": 0.0})
+        d["count"] += 1
+        d["busy_us"] += float(b - a)
+        if prev_end is not None:
+            d["gap_before_us"] += float(a - prev_end)
+        prev_end = b
+    busy = sum(d["busy_us"] for d in per.values())
+    span = float(t1[-1] - t0[0]) if len(t0) else 0.0
+    if args.timeline_out:
+        with open(args.timeline_out, "w") as f:
+            f.write("# kernel timeline of one solve (us on the device's global timer, relative to the first kernel's start)\n")
+            f.write("# index kind start end duration gap_before\n")
+            pe = None
+            for i, (k, a, b) in enumerate(zip(kind, t0, t1)):
+                f.write(f"{i:4d} {TL_KINDS[k]:18s} {a:10.2f} {b:10.2f} {b - a:8.2f} {0.0 if pe is None else a - pe:8.2f}\n")
+                pe = b
+    print(json.dumps({"study": "timeline", "config": config_dict(cfg, solver_iterations(cfg)), "kernels": int(len(kind)),
+                      "span_us": span, "busy_us": busy, "busy_frac": busy / span if span else None,
+                      "solve_ms_cuda_events_with_timeline_on": e0.elapsed_time(e1),
+                      "per_kind": per, "iters": int(r.iters)}), flush=True)
+
+
 def run_pca_study(args, cfg, rank, local_rank):
     """--pca-study: pcamm_pca_fit on the config's nine training
     DVFs: device time of its two streaming passes (CUDA events on the launching stream, inside the
@@ -576,6 +642,9 @@ def main():
                          "two passes against their algorithmic bytes)")
     ap.add_argument("--tune", action="append", default=[], metavar="NAME=VALUE",
                     help="pcamm_tune measurement knob, set before the model is created (repeatable)")
+    ap.add_argument("--timeline", action="store_true",
+                    help="instead of the bench line: the kernel timeline of one solve, recorded inside the kernels")
+    ap.add_argument("--timeline-out", default=None, help="with --timeline: write the event list to this text file")
     ap.add_argument("--grad-tol", type=float, default=None)
     ap.add_argument("--study-max-iter", type=int, default=30)
     args = ap.parse_args()
@@ -587,6 +656,8 @@ def main():
         run_frames_study(args, cfg, rank, local_rank)
     elif args.pca_study:
         run_pca_study(args, cfg, rank, local_rank)
+    elif args.timeline:
+        run_timeline(args, cfg, rank, local_rank)
     elif args.impl == "reference":
         run_reference(args, cfg, rank, world)
     else:

@@ -259,12 +259,30 @@ int pcamm_localise(pcamm_model* model, const float* w_host, int32_t inv_max_iter
  * which: 0 = warp (a-1), 1 = project (a-2), 2 = gradient (a-4). */
 int pcamm_time_kernel(pcamm_model* model, int32_t which, int32_t reps, float* ms_out, void* stream);
 
+/* What the two streaming kernels really loaded (reading B8: tiles whose stencils can only see zeros
+ * of f0 / constant cells are skipped, exactly).  out[0], out[1] = field tiles loaded by the warp and
+ * by the gradient kernel in all launches since the counters were last reset (one tile = out[3]
+ * voxels, all 3(K+1) field planes); out[2] = tiles of the whole volume (0: the generic kernels are
+ * in use, which visit everything and count nothing).  reset != 0 clears the counters. */
+int pcamm_tile_counts(pcamm_model* model, int32_t reset, int64_t* out /* [4] */, void* stream);
+
 /* Measurement knob (process-wide; set it before pcamm_model_create: a model's solve graphs keep the
  * launch configuration they were built with).  Returns PCAMM_E_INVALID for an unknown name.
  *   "project_chunks_per_segment"  chunks of the projector's march a block works through
  *                                 (0 = automatic, the default);
- *   "project_scan_slabs"          slabs per scan of the projector: 1, 2 or 4 (0 = automatic). */
+ *   "project_scan_slabs"          slabs per scan of the projector: 1, 2 or 4 (0 = automatic);
+ *   "timeline"                    1: models created from now on record, inside their kernels, the
+ *                                 start and end of every kernel of a solve (pcamm_timeline). */
 int pcamm_tune(const char* name, int32_t value);
+
+/* Kernel timeline of the model's last solve (timeline knob): per kernel, in launch order, its kind
+ * (0 ysums, 1 begin, 2 view tables, 3 warp, 4 project, 5 control after a projection, 6 residual,
+ * 7 gradient, 8 control after the gradient, 9 unused, 10 final, 11 tumour inversion) and
+ * its start (first block in) and end (last block out) in microseconds on the device's global timer,
+ * relative to the first kernel's start.  *n_out = kernels recorded (at most 2048; arrays filled up
+ * to cap). */
+int pcamm_timeline(pcamm_model* model, int32_t cap, int32_t* kind_out, double* start_us_out, double* end_us_out,
+                   int32_t* n_out, void* stream);
 
 /* Number of kernels launched by this library on the calling thread since the last reset
  * (host-side launch count; kernels inside device-side loops are counted from the device's

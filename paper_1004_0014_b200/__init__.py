@@ -53,7 +53,7 @@ SYMBOLS = ("pcamm_default_opts", "pcamm_model_create", "pcamm_model_destroy", "p
            "pcamm_reconstruct",
            "pcamm_reconstruct_host", "pcamm_reconstruct_batch", "pcamm_warp", "pcamm_project",
            "pcamm_backproject", "pcamm_eval", "pcamm_traverse", "pcamm_localise", "pcamm_time_kernel",
-           "pcamm_tune", "pcamm_launch_count", "pcamm_last_error", "pcamm_pca_fit", "pcamm_predict_w", "pcamm_frames_create",
+           "pcamm_tune", "pcamm_tile_counts", "pcamm_timeline", "pcamm_launch_count", "pcamm_last_error", "pcamm_pca_fit", "pcamm_predict_w", "pcamm_frames_create",
            "pcamm_frames_destroy", "pcamm_frames_reset", "pcamm_frames_count", "pcamm_frames_predict",
            "pcamm_frames_push")
 
@@ -332,6 +332,24 @@ class Model:
         _check(lib().pcamm_localise(self._h, w.ctypes.data_as(C.c_void_p), int(inv_max_iter), C.c_float(inv_tol_mm),
                                     out.ctypes.data_as(C.c_void_p), _stream()))
         return out
+
+    def timeline(self):
+        """pcamm_timeline: (kind, start_us, end_us) arrays of the kernels of the last solve (timeline knob)."""
+        cap = 2048
+        kind = np.zeros(cap, np.int32)
+        t0 = np.zeros(cap, np.float64)
+        t1 = np.zeros(cap, np.float64)
+        n = C.c_int32(0)
+        _check(lib().pcamm_timeline(self._h, cap, kind.ctypes.data_as(C.c_void_p), t0.ctypes.data_as(C.c_void_p),
+                                    t1.ctypes.data_as(C.c_void_p), C.byref(n), _stream()))
+        k = min(n.value, cap)
+        return kind[:k].copy(), t0[:k].copy(), t1[:k].copy()
+
+    def tile_counts(self, reset: bool = False):
+        """pcamm_tile_counts: (warp tiles loaded, gradient tiles loaded, tiles of the volume, voxels per tile)."""
+        out = (C.c_int64 * 4)()
+        _check(lib().pcamm_tile_counts(self._h, 1 if reset else 0, out, _stream()))
+        return tuple(int(v) for v in out)
 
     def time_kernel(self, which: int, reps: int = 20) -> float:
         """Average device milliseconds per launch of kernel 0 warp / 1 project / 2 gradient on the

@@ -17,6 +17,7 @@ namespace pcamm {
 
 static thread_local std::string g_error;
 static thread_local long long g_launches = 0;
+int g_timeline = 0;
 
 void set_error(const std::string& msg) { g_error = msg; }
 void count_launch(long long n) { g_launches += n; }
@@ -160,6 +161,8 @@ struct pcamm_model {
     int* trav_n = nullptr;
     int trav_cap = 0;
     unsigned long long* nonfinite = nullptr;
+    unsigned long long* visited = nullptr;   // FieldStream::visited
+    Timeline* tl = nullptr;                  // kernel timeline of the last solve (timeline knob), else NULL
     float* y_stage = nullptr;   // device copy of a host-side measured projection (pcamm_reconstruct_host)
     // pinned host staging
     char* h_in = nullptr;
@@ -256,33 +259,38 @@ int push_call(pcamm_model* m, int B, cudaStream_t st) {
 }
 
 // ---- the kernel sequences of a solve (shared by the graph and the host-driven mode)
+//
+//   head:       sums of y, begin, per-view tables, warp + projection at w0 (-> first fit)
+//   loop body:  residual, gradient (-> J_n, g, first candidates), warp, projection (-> Armijo test,
+//               Eq. 3 update, Eq. 4 fit); a solve in the middle of a line search skips the first two
+//   tail:       closing residual (J at exit), final, landmark inversion
+// A single-block control step (control.cuh) follows every projection and every gradient pass.
 
-void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_iter, int use_cond) {
+void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_loop, int use_cond) {
     const Geom& G = m->G;
     launch_ysums(q, G, m->c, B);
     launch_begin(q, G, m->c, 0);
     launch_view_tables(q, G, m->c.solves, B, m->col_hdr, m->slab_tab);
     launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
-    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_INIT, h_iter, use_cond);
+    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_INIT, h_loop, use_cond,
+                   q.n_kernels);
 }
 
-void seq_grad(pcamm_model* m, Seq& q, int B, cudaGraphConditionalHandle h_trial, int use_cond) {
+void seq_body(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_loop, int use_cond) {
     const Geom& G = m->G;
+    const int n0 = q.n_kernels;
     launch_resid(q, G, m->c.solves, m->c.in, B, 0, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_grad(q, G, m->fs, m->f0p, m->c.solves, B, m->rL, m->utab, m->vtab, m->c.grad_part);
-    launch_ctl_grad(q, G, m->c, h_trial, use_cond);
-}
-
-void seq_trial(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_trial, int use_cond) {
-    const Geom& G = m->G;
+    launch_grad(q, G, m->fs, m->f0p, m->c, B, m->rL, m->utab, m->vtab, GRAD_SOLVE);
     launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
-    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_TRIAL, h_trial, use_cond);
+    launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_TRIAL, h_loop, use_cond,
+                   q.n_kernels - n0);
 }
 
 void seq_tail(pcamm_model* m, Seq& q, int B) {
     const Geom& G = m->G;
+    const int n0 = q.n_kernels;
     launch_resid(q, G, m->c.solves, m->c.in, B, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_ctl_final(q, G, m->c, m->out_slots);
+    launch_ctl_final(q, G, m->c, m->out_slots, q.n_kernels - n0 + 1 + (m->M > 0 ? 1 : 0));
     launch_invert(q, G, m->xbar, m->u, m->c, B, m->M, m->lm0, m->lm_out);
 }
 
@@ -292,21 +300,16 @@ int get_graph(pcamm_model* m, int B, int C, GraphRec** out) {
     if (it != m->graphs.end()) { *out = &it->second; return PCAMM_OK; }
     GraphRec rec;
     CUDA_TRY(cudaGraphCreate(&rec.graph, 0));
-    cudaGraphConditionalHandle h_iter, h_trial;
-    CUDA_TRY(cudaGraphConditionalHandleCreate(&h_iter, rec.graph, 0, cudaGraphCondAssignDefault));
-    CUDA_TRY(cudaGraphConditionalHandleCreate(&h_trial, rec.graph, 0, cudaGraphCondAssignDefault));
+    cudaGraphConditionalHandle h_loop;
+    CUDA_TRY(cudaGraphConditionalHandleCreate(&h_loop, rec.graph, 0, cudaGraphCondAssignDefault));
     Seq q;
     q.graph = rec.graph;
-    seq_head(m, q, B, C, h_iter, 1);
-    Seq it_body = q.add_while(h_iter);          // iterations n = 0 ..
-    seq_grad(m, it_body, B, h_trial, 1);
-    Seq tr_body = it_body.add_while(h_trial);   // Armijo backtracking (Eq. 3)
-    seq_trial(m, tr_body, B, C, h_trial, 1);
-    launch_ctl_iter_end(it_body, m->c, h_iter, 1);
+    seq_head(m, q, B, C, h_loop, 1);
+    Seq body = q.add_while(h_loop);             // iterations and their line searches
+    seq_body(m, body, B, C, h_loop, 1);
     seq_tail(m, q, B);
     int rc;
-    if ((rc = check_seq(q, "graph build")) || (rc = check_seq(it_body, "graph build (iteration body)")) ||
-        (rc = check_seq(tr_body, "graph build (trial body)"))) {
+    if ((rc = check_seq(q, "graph build")) || (rc = check_seq(body, "graph build (loop body)"))) {
         cudaGraphDestroy(rec.graph);
         return rc;
     }
@@ -333,13 +336,9 @@ int run_host_loop(pcamm_model* m, int B, int C, cudaStream_t st) {
     int rc;
     seq_head(m, q, B, C, 0, 0);
     if ((rc = check_seq(q, "solve head")) || (rc = read_flags(m, st))) return rc;
-    while (m->h_flags->iter_cond) {
-        seq_grad(m, q, B, 0, 0);
-        if ((rc = check_seq(q, "gradient step")) || (rc = read_flags(m, st))) return rc;
-        while (m->h_flags->trial_cond) {
-            seq_trial(m, q, B, C, 0, 0);
-            if ((rc = check_seq(q, "trial step")) || (rc = read_flags(m, st))) return rc;
-        }
+    while (m->h_flags->loop_cond) {
+        seq_body(m, q, B, C, 0, 0);
+        if ((rc = check_seq(q, "loop body")) || (rc = read_flags(m, st))) return rc;
     }
     seq_tail(m, q, B);
     return check_seq(q, "solve tail");
@@ -368,6 +367,10 @@ int solve_impl(pcamm_model* m, int B, const float* y_dev, const float* angles, c
         in[b].a = in[b].b = 0.f;
     }
     if ((rc = push_call(m, B, st))) return rc;
+    if (m->tl) {       // fresh timeline: no events, starts at the largest time, ends at 0
+        CUDA_TRY(cudaMemsetAsync(m->tl, 0, sizeof(Timeline), st));
+        CUDA_TRY(cudaMemsetAsync(m->tl->t0, 0xff, sizeof(m->tl->t0), st));
+    }
     if (o.loop_mode == 0) {
         GraphRec* g = nullptr;
         if ((rc = get_graph(m, B, C, &g))) return rc;
@@ -515,6 +518,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     }
     pcamm_model* m = new (std::nothrow) pcamm_model();
     if (!m) { set_error("out of host memory"); return PCAMM_E_NOMEM; }
+    m->G.tl = nullptr;
     m->geo = *g;
     m->M = n_landmarks; m->Bmax = Bmax; m->Cmax = Cmax; m->S = Bmax * Cmax;
     Geom& G = m->G;
@@ -562,7 +566,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         ok(dalloc(m, &m->c.grad_part, B * m->c.grad_blocks * KMAX)) && ok(dalloc(m, &m->out_slots, B)) &&
         ok(dalloc(m, &m->lm_out, 3 * B * (size_t)(m->M > 0 ? m->M : 1))) &&
         ok(dalloc(m, &m->trav_ijk, 3 * (size_t)m->trav_cap)) && ok(dalloc(m, &m->trav_len, (size_t)m->trav_cap)) &&
-        ok(dalloc(m, &m->trav_n, 1)) && ok(dalloc(m, &m->nonfinite, 1)) && ok(dalloc(m, &m->y_stage, (size_t)G.npix)) &&
+        ok(dalloc(m, &m->trav_n, 1)) && ok(dalloc(m, &m->nonfinite, 1)) && ok(dalloc(m, &m->visited, 2)) && ok(dalloc(m, &m->y_stage, (size_t)G.npix)) &&
         ok(halloc(m, &m->h_in, m->in_block_bytes)) && ok(halloc(m, &m->h_solves, B)) &&
         ok(halloc(m, &m->h_traces, B)) && ok(halloc(m, &m->h_flags, 1)) &&
         ok(halloc(m, &m->h_lm, 3 * B * (size_t)(m->M > 0 ? m->M : 1))) &&
@@ -573,6 +577,11 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         cudaGetLastError();
         pcamm_model_destroy(m);
         return e == cudaErrorMemoryAllocation ? PCAMM_E_NOMEM : PCAMM_E_CUDA;
+    }
+    if (g_timeline) {
+        e = dalloc(m, &m->tl, 1);
+        if (e != cudaSuccess) { set_error("allocation failed (timeline)"); pcamm_model_destroy(m); return PCAMM_E_NOMEM; }
+        G.tl = m->tl;
     }
     m->xbar = m->fields;
     m->u = m->fields + 3 * (size_t)V;
@@ -597,6 +606,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     TRY_OR_FAIL(cudaMemsetAsync(m->vol, 0, sizeof(float) * S * (size_t)G.PV, st));   // zero border, never written
     TRY_OR_FAIL(cudaMemsetAsync(m->occ, 0, S * (size_t)G.OCC, st));                   // likewise
     TRY_OR_FAIL(cudaMemsetAsync(m->nonfinite, 0, sizeof(unsigned long long), st));
+    TRY_OR_FAIL(cudaMemsetAsync(m->visited, 0, 2 * sizeof(unsigned long long), st));
+    m->fs.visited = m->visited;
     TRY_OR_FAIL(cudaMemsetAsync(m->c.solves, 0, sizeof(SolveState) * B, st));
     TRY_OR_FAIL(cudaMemsetAsync(m->c.slots, 0, sizeof(SlotState) * S, st));
     TRY_OR_FAIL(cudaMemsetAsync(m->c.flags, 0, sizeof(LoopFlags), st));
@@ -783,7 +794,7 @@ int pcamm_project(pcamm_model* m, const float* volume_dev, float angle_rad, floa
     if (rc) return rc;
     launch_view_tables(q, m->G, m->c.solves, 1, m->col_hdr, m->slab_tab);
     launch_to_ray_layout(q, m->G, volume_dev, m->vol, m->occ);
-    launch_project(q, m->G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0);
+    launch_project(q, m->G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0, 0);
     if ((rc = check_seq(q, "project"))) return rc;
     CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * m->G.npix, cudaMemcpyDeviceToDevice, st));
     CUDA_TRY(cudaStreamSynchronize(st));
@@ -814,10 +825,9 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     launch_ysums(q2, G, m->c, 1);
     launch_view_tables(q2, G, m->c.solves, 1, m->col_hdr, m->slab_tab);
     launch_warp(q2, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
-    launch_project(q2, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_EVAL, 0, 0);
+    launch_project(q2, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_EVAL, 0, 0, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_grad(q2, G, m->fs, m->f0p, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
-    launch_ctl_eval_grad(q2, G, m->c);
+    launch_grad(q2, G, m->fs, m->f0p, m->c, 1, m->rL, m->utab, m->vtab, GRAD_EVAL);
     if ((rc = check_seq(q2, "eval"))) return rc;
     if (proj_out_dev) CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * G.npix, cudaMemcpyDeviceToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState), cudaMemcpyDeviceToHost, st));
@@ -880,11 +890,45 @@ int pcamm_localise(pcamm_model* m, const float* w_host, int32_t inv_max_iter, fl
     return PCAMM_OK;
 }
 
+int pcamm_tile_counts(pcamm_model* m, int32_t reset, int64_t* out, void* stream) {
+    if (!m || !out) return invalid("NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long h[2] = {0ull, 0ull};
+    CUDA_TRY(cudaMemcpyAsync(h, m->visited, sizeof(h), cudaMemcpyDeviceToHost, st));
+    if (reset) CUDA_TRY(cudaMemsetAsync(m->visited, 0, sizeof(h), st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    const int tz = m->G.K <= PCAMM_TZ_SMALL_K ? 32 : 16;                  // TileZ<K>
+    out[0] = (int64_t)h[0]; out[1] = (int64_t)h[1];
+    out[2] = m->fs.use_tma ? (int64_t)tile_count(m->G, tz) : 0;
+    out[3] = (int64_t)TX * tz;
+    return PCAMM_OK;
+}
+
+int pcamm_timeline(pcamm_model* m, int32_t cap, int32_t* kind_out, double* start_us_out, double* end_us_out,
+                   int32_t* n_out, void* stream) {
+    if (!m || !n_out || cap < 0 || (cap > 0 && (!kind_out || !start_us_out || !end_us_out))) return invalid("NULL argument");
+    *n_out = 0;
+    if (!m->tl) return invalid("the model was created without the timeline knob");
+    std::vector<Timeline> h(1);
+    CUDA_TRY(cudaMemcpyAsync(h.data(), m->tl, sizeof(Timeline), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    const Timeline& t = h[0];
+    const int n = (int)(t.n < (unsigned)TL_CAP ? t.n : (unsigned)TL_CAP);
+    *n_out = n;
+    for (int i = 0; i < n && i < cap; ++i) {
+        kind_out[i] = t.kind[i];
+        start_us_out[i] = 1e-3 * (double)(t.t0[i] - t.t0[0]);
+        end_us_out[i] = 1e-3 * (double)(t.t1[i] - t.t0[0]);
+    }
+    return PCAMM_OK;
+}
+
 int pcamm_tune(const char* name, int32_t value) {
     if (!name) return invalid("NULL argument");
     const std::string n(name);
     if (n == "project_chunks_per_segment") { g_chunks_per_segment = value < 0 ? 0 : value; return PCAMM_OK; }
     if (n == "project_scan_slabs") { g_scan_slabs = value < 0 ? 0 : value; return PCAMM_OK; }
+    if (n == "timeline") { g_timeline = value != 0; return PCAMM_OK; }
     return invalid("unknown knob: " + n);
 }
 
@@ -899,9 +943,9 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
         if (which == 0)
             launch_warp(q, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
         else if (which == 1)
-            launch_project(q, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0);
+            launch_project(q, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0, 0);
         else
-            launch_grad(q, G, m->fs, m->f0p, m->c.solves, 1, m->rL, m->utab, m->vtab, m->c.grad_part);
+            launch_grad(q, G, m->fs, m->f0p, m->c, 1, m->rL, m->utab, m->vtab, GRAD_NONE);
     }
     CUDA_TRY(cudaEventRecord(m->ev1, st));
     int rc = check_seq(q, "time_kernel");

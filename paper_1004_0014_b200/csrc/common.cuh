@@ -16,8 +16,52 @@ constexpr int KMAX = PCAMM_KMAX;
 constexpr int MAXBT = PCAMM_MAX_BACKTRACKS;
 constexpr int TRACE_CAP = 1024;  // iterations recorded in the device-side traces
 
+// Measurement (pcamm_tune "timeline"): start and end of every kernel of a solve on the device's
+// global timer, taken inside the kernels (first block in, last block out).  The kernels of a solve
+// run strictly one after the other, so one running event index serves them all.
+constexpr int TL_CAP = 2048;
+enum { TLK_YSUMS = 0, TLK_BEGIN, TLK_VIEW, TLK_WARP, TLK_PROJECT, TLK_CTL_PROJ, TLK_RESID, TLK_GRAD, TLK_CTL_GRAD,
+       TLK_ITER_END, TLK_FINAL, TLK_INVERT };
+struct Timeline {
+    unsigned n, done;
+    unsigned pad[2];
+    unsigned long long t0[TL_CAP], t1[TL_CAP];      // ns; t0 preset to ~0, t1 to 0
+    int kind[TL_CAP];
+};
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ bool tl_first_thread() { return (threadIdx.x | threadIdx.y | threadIdx.z) == 0; }
+// at the top of a kernel, by every block
+__device__ __forceinline__ void tl_begin(Timeline* tl) {
+    if (tl && tl_first_thread()) {
+        const unsigned e = *(volatile unsigned*)&tl->n;
+        if (e < TL_CAP) atomicMin(&tl->t0[e], global_timer_ns());
+    }
+}
+// wherever a block leaves the kernel (uniform over the block)
+__device__ __forceinline__ void tl_end(Timeline* tl, int kind) {
+    if (!tl) return;
+    __syncthreads();
+    if (tl_first_thread()) {
+        const unsigned e = *(volatile unsigned*)&tl->n;
+        if (e < TL_CAP) atomicMax(&tl->t1[e], global_timer_ns());
+        __threadfence();
+        const unsigned nblk = gridDim.x * gridDim.y * gridDim.z;
+        if (atomicAdd(&tl->done, 1u) == nblk - 1u) {
+            tl->done = 0u;
+            if (e < TL_CAP) tl->kind[e] = kind;
+            __threadfence();
+            *(volatile unsigned*)&tl->n = e + 1u;
+        }
+    }
+}
+
 // Model-constant geometry (passed to kernels by value).
 struct Geom {
+    Timeline* tl;             // NULL unless the timeline knob was on when the model was created
     int nx, ny, nz;
     long long V;
     int pnx, pny;             // in-plane size of a ray-layout volume: nx + 2, ny + 2 (zero border)
@@ -116,6 +160,11 @@ struct SolveTrace {
     int bt[TRACE_CAP];
 };
 
+// The loop of a solve is flat: its body is {residual, gradient, warp, projection}.  A solve in the
+// middle of a line search (trialing) skips the first two; one whose step has just been accepted
+// needs the residual and the gradient of its next iteration.
+__device__ __forceinline__ bool needs_gradient(const SolveState& st) { return st.running && !st.trialing; }
+
 // One trial evaluation: candidate c of solve b, slot s = b * C + c.
 struct SlotState {
     float w[KMAX];
@@ -123,16 +172,33 @@ struct SlotState {
     double mu, J, Sp, Syp;
 };
 
-// Loop conditions mirrored to plain memory so that the host-driven mode can read them.
+// Loop condition mirrored to plain memory so that the host-driven mode can read it, and the
+// number of kernels the device-side loop has launched.
 struct LoopFlags {
-    int iter_cond, trial_cond;
+    int loop_cond, pad0;
     long long n_launch;
-    unsigned ticket;          // unused
-    unsigned pad;
 };
 
-// Control step that follows a projection (k_ctl_after_project).
+// Control step run by the last block of a projection (control.cuh) ...
 constexpr int THEN_NONE = 0, THEN_INIT = 1, THEN_TRIAL = 2, THEN_EVAL = 3;
+// ... and of a gradient pass.
+constexpr int GRAD_NONE = 0, GRAD_SOLVE = 1, GRAD_EVAL = 2;
+
+// Device buffers of the control steps.
+struct CtlBufs {
+    CallOpts* opts;
+    SolveIn* in;
+    SolveState* solves;
+    SolveTrace* traces;
+    SlotState* slots;
+    LoopFlags* flags;
+    int* seg_ticket;     // [S][nu]: blocks of a detector column that are done (self-resetting)
+    double* ysum_part;   // [B][ysum_blocks][2]
+    double* proj_part;   // [S][project_blocks][3]
+    double* resid_part;  // [B][resid_blocks]
+    double* grad_part;   // [B][grad_blocks][K]
+    int ysum_blocks, proj_blocks, resid_blocks, grad_blocks;
+};
 
 // In-plane direction D - S of the rays of detector column iu (independent of the row).
 __device__ __forceinline__ void ray_dir_inplane(const Geom& G, double cs, double sn, int iu, double* dx, double* dy) {

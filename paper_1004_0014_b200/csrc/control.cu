@@ -1,28 +1,24 @@
-// a-3 (second half), a-5 and a-6: the scalar side of the alternating algorithm, kept on the device.
+// The single-block kernels of a solve that are not folded into a streaming kernel: sums of y, the
+// start of a call, the closing step, and a-6:
 //
-//   step 1 (Eq. 3):  w_{n+1} = w_n - mu_n dJ/dw_n, mu_n by Armijo's rule (L95)
-//   step 2 (Eq. 4):  (a, b)^T = (Y^T Y)^-1 Y^T P f_{n+1},  Y = [y, 1]
-//   stop:         ||dJ/dw|| small or max_iter reached
 //   tumour:     r_{m+1} = r0 - x(r_m)  (fixed-point inverse of the pull-back DVF)
 //
-// Readings A7 (Armijo constants, first step = init_step_vox voxels rms, later 2 x the accepted
-// step), A8 (initial (a, b) = fit at w0; singular fit), A9, A13 are listed in DESIGN.md.
-//
-// Each control kernel is one block; thread b owns solve b.  All scalars are double.  The kernels
-// also decide whether the enclosing device-side while-loops of the solve graph continue
-// (cudaGraphSetConditional) and mirror those decisions into LoopFlags for the host-driven mode.
+// The control steps of the alternating algorithm (Armijo test, Eq. 3 update, Eq. 4 fit, stopping
+// rule) are the device functions of control.cuh, run by the last block of the projector / of the
+// gradient kernel.  Reading A13 (landmark inversion) is listed in DESIGN.md.
 #include "internal.h"
+#include "control.cuh"
 
 namespace pcamm {
 
 namespace {
 
-constexpr int CT = 256;   // threads of a control block
 constexpr int YT = 256;
 
 __global__ void __launch_bounds__(YT)
 k_ysums(const Geom G, const SolveIn* __restrict__ in, double* __restrict__ part) {
     __shared__ double red[YT / 32];
+    tl_begin(G.tl);
     const int b = blockIdx.y;
     const float* y = in[b].y;
     double s = 0.0, ss = 0.0;
@@ -36,15 +32,7 @@ k_ysums(const Geom G, const SolveIn* __restrict__ in, double* __restrict__ part)
         double* o = part + ((long long)b * gridDim.x + blockIdx.x) * 2;
         o[0] = S; o[1] = SS;
     }
-}
-
-// Step 2, Eq. (4) as the 2x2 normal equations of Y = [y, 1].  false: y constant (reading A8).
-__device__ bool lsfit(double n, double Sy, double Syy, double Sp, double Syp, double* a, double* b) {
-    const double det = Syy * n - Sy * Sy;
-    if (!(det > 1e-12 * Syy * n)) return false;
-    *a = (Syp * n - Sy * Sp) / det;
-    *b = (Syy * Sp - Sy * Syp) / det;
-    return true;
+    tl_end(G.tl, TLK_YSUMS);
 }
 
 __device__ void set_view(const Geom& G, float angle, View* vw) {
@@ -52,31 +40,12 @@ __device__ void set_view(const Geom& G, float angle, View* vw) {
     vw->cs = cos(th); vw->sn = sin(th);
 }
 
-// Candidates st.t, st.t + 1, ... (at most C per round, fewer at the end of the backtrack budget) of
-// the Armijo sequence mu0 beta^t into the solve's slots; st.mu is the step of candidate st.t and
-// every later one follows by repeated multiplication, whatever the fan width, so that a fan of
-// any width takes exactly the steps sequential backtracking would.
-__device__ void trial_w(const SolveState& st, int K, double mu, SlotState* sl);
-__device__ void make_round(const SolveState& st, int K, const CallOpts& o, SlotState* slots_b) {
-    double mu = st.mu;
-    for (int cnd = 0; cnd < o.C; ++cnd) {
-        if (st.t + cnd < o.max_backtracks) trial_w(st, K, mu, &slots_b[cnd]);
-        else slots_b[cnd].active = 0;
-        mu *= o.armijo_beta;
-    }
-}
-
-__device__ void trial_w(const SolveState& st, int K, double mu, SlotState* sl) {
-    for (int k = 0; k < K; ++k) sl->w[k] = (float)(st.w[k] - mu * st.g[k]);   // Eq. (3), candidate
-    sl->mu = mu;
-    sl->active = 1;
-}
-
 // mode 0: start of a solve.  mode 1: pcamm_eval (a, b given).  mode 2: hooks that only need the
 // view and w in slot 0.
 __global__ void __launch_bounds__(CT)
 k_begin(const Geom G, const CallOpts* __restrict__ opts, const SolveIn* __restrict__ in, SolveState* solves,
         SlotState* slots, LoopFlags* flags, int mode) {
+    tl_begin(G.tl);
     const int B = opts->B, C = opts->C;
     for (int b = threadIdx.x; b < B; b += CT) {
         SolveState& st = solves[b];
@@ -99,291 +68,61 @@ k_begin(const Geom G, const CallOpts* __restrict__ opts, const SolveIn* __restri
         for (int k = 0; k < G.K; ++k) s0.w[k] = in[b].w_init[k];
         s0.active = 1;
     }
-    if (threadIdx.x == 0) { flags->iter_cond = 0; flags->trial_cond = 0; flags->n_launch = 0; flags->ticket = 0u; }
+    if (threadIdx.x == 0) { flags->loop_cond = 0; flags->n_launch = 0; }
+    tl_end(G.tl, TLK_BEGIN);
 }
 
-// Sum of n partials with the given stride, by the whole control block (fixed order); the result
-// is broadcast to all threads.
-__device__ double coop_sum(const double* part, int n, int stride, double* red /* [CT/32 + 1] */) {
-    double v = 0.0;
-    for (int i = threadIdx.x; i < n; i += CT) v += __ldcg(part + (long long)i * stride);   // written by other blocks
-    const double s = block_sum<CT>(v, red);
-    if (threadIdx.x == 0) red[CT / 32] = s;
-    __syncthreads();
-    return red[CT / 32];
-}
-
-struct Sums3 { double a, b, c; };
-
-// The three projection sums of slot s in one pass (one round trip to L2, one exchange).
-__device__ Sums3 sum_proj(const double* part, int nblk, int s, double* red /* unused */) {
-    __shared__ double ex[3][CT / 32];
-    __shared__ double tot[3];
-    (void)red;
-    const double* p = part + (long long)s * nblk * 3;
-    double v0 = 0.0, v1 = 0.0, v2 = 0.0;
-    for (int i = threadIdx.x; i < nblk; i += CT) {
-        v0 += __ldcg(p + 3 * i); v1 += __ldcg(p + 3 * i + 1); v2 += __ldcg(p + 3 * i + 2);
-    }
-    v0 = warp_sum(v0); v1 = warp_sum(v1); v2 = warp_sum(v2);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    __syncthreads();                       // ex / tot may still be read from a previous call
-    if (lane == 0) { ex[0][wid] = v0; ex[1][wid] = v1; ex[2][wid] = v2; }
-    __syncthreads();
-    if (threadIdx.x < 3) {
-        double t = 0.0;
-#pragma unroll
-        for (int i = 0; i < CT / 32; ++i) t += ex[threadIdx.x][i];
-        tot[threadIdx.x] = t;
-    }
-    __syncthreads();
-    Sums3 r;
-    r.a = tot[0]; r.b = tot[1]; r.c = tot[2];
-    return r;
-}
-
-__device__ void publish(LoopFlags* flags, int iter_cond, int trial_cond, int launched) {
-    flags->iter_cond = iter_cond;
-    flags->trial_cond = trial_cond;
-    flags->n_launch += launched;
-}
-
-// After the initial evaluation at w0: Sy, Syy, the first fit (reading A8), loop start.
-__device__ void ctl_init_body(const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond) {
-    __shared__ double red[CT / 32 + 1];
-    int any_running = 0;
-    const CallOpts& o = *c.opts;
-    for (int b = 0; b < o.B; ++b) {
-        SolveState& st = c.solves[b];
-        const double* yp = c.ysum_part + (long long)b * c.ysum_blocks * 2;
-        const double Sy = coop_sum(yp, c.ysum_blocks, 2, red), Syy = coop_sum(yp + 1, c.ysum_blocks, 2, red);
-        const int s0 = b * o.C;
-        const Sums3 sp = sum_proj(c.proj_part, c.proj_blocks, s0, red);
-        if (threadIdx.x != 0) continue;
-        st.Sy = Sy; st.Syy = Syy;
-        c.slots[s0].Sp = sp.a; c.slots[s0].Syp = sp.b;
-        c.slots[s0].active = 0;
-        if (!isfinite(Sy) || !isfinite(Syy)) st.status = PCAMM_E_NONFINITE;
-        else if (!lsfit((double)G.npix, Sy, Syy, sp.a, sp.b, &st.a, &st.b)) st.status = PCAMM_E_SINGULAR;
-        st.acc_slot = s0;
-        st.iter = 0;
-        if (st.status == 0 && o.max_iter <= 0) st.status = PCAMM_S_MAXITER;
-        st.running = st.status == 0;
-        any_running |= st.running;
-    }
-    if (threadIdx.x == 0) {
-        publish(c.flags, any_running, 0, 6);
-        if (use_cond) cudaGraphSetConditional(h_iter, any_running);
-    }
-}
-
-// After the residual and gradient kernels of iteration n: J_n, g, stopping rule, first candidate(s).
+// The control step that follows a projection (then = THEN_INIT / THEN_TRIAL / THEN_EVAL): one block.
+// In graph mode the decision it leaves in LoopFlags becomes the condition of the solve graph's
+// while-node.
 __global__ void __launch_bounds__(CT)
-k_ctl_grad(const Geom G, CtlBufs c, cudaGraphConditionalHandle h_trial, int use_cond) {
-    __shared__ double ex[KMAX + 1][CT / 32];
-    __shared__ double tot[KMAX + 1];
-    int any_trial = 0, any_running = 0;
-    const CallOpts o = *c.opts;
-    const int K = G.K;
-    for (int b = 0; b < o.B; ++b) {
-        SolveState st = c.solves[b];                   // worked on in registers; thread 0 writes it back
-        if (!st.running) continue;                                                        // uniform
-        const int n = st.iter;
-        // J_n and the K gradient sums in one pass over the partial sums (fixed order)
-        {
-            double v[KMAX + 1];
-#pragma unroll
-            for (int k = 0; k <= KMAX; ++k) v[k] = 0.0;
-            const double* rp = c.resid_part + (long long)b * c.resid_blocks;
-            for (int i = threadIdx.x; i < c.resid_blocks; i += CT) v[KMAX] += __ldcg(rp + i);
-            const double* gp = c.grad_part + (long long)b * c.grad_blocks * KMAX;
-            for (int i = threadIdx.x; i < c.grad_blocks; i += CT) {
-#pragma unroll
-                for (int k = 0; k < KMAX; ++k)
-                    if (k < K) v[k] += __ldcg(gp + (long long)i * KMAX + k);
-            }
-            const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-            __syncthreads();
-#pragma unroll
-            for (int k = 0; k <= KMAX; ++k) {
-                const double w = warp_sum(v[k]);
-                if (lane == 0) ex[k][wid] = w;
-            }
-            __syncthreads();
-            if (threadIdx.x <= KMAX) {
-                double t = 0.0;
-#pragma unroll
-                for (int i = 0; i < CT / 32; ++i) t += ex[threadIdx.x][i];
-                tot[threadIdx.x] = t;
-            }
-            __syncthreads();
-        }
-        if (threadIdx.x != 0) continue;
-        const double Jn = tot[KMAX];
-        double gk[KMAX];
-        for (int k = 0; k < K; ++k) gk[k] = tot[k];
-        st.Jn = Jn;                                                                       // Eq. (2)
-        if (n == 0) st.J0 = st.Jn;
-        double g2 = 0.0;
-        for (int k = 0; k < K; ++k) {
-            st.g[k] = 2.0 * gk[k];
-            g2 += st.g[k] * st.g[k];
-        }
-        st.g2 = g2;
-        const double gn = sqrt(g2);
-        if (n < TRACE_CAP) { c.traces[b].J[n] = st.Jn; c.traces[b].gnorm[n] = gn; }
-        if (gn <= o.grad_tol || !isfinite(gn)) {
-            st.status = isfinite(gn) ? PCAMM_S_GRADTOL : PCAMM_E_NONFINITE;
-            st.running = 0; st.trialing = 0;
-            c.solves[b] = st;
-            continue;
-        }
-        st.mu = n == 0 ? o.init_step_vox * o.hmin_sqrtV / gn : 2.0 * st.mu_prev;         // reading A7
-        st.t = 0;
-        st.trialing = 1;
-        make_round(st, K, o, &c.slots[b * o.C]);
-        any_trial = 1;
-        any_running = 1;
-        c.solves[b] = st;
-    }
-    if (threadIdx.x == 0) {
-        publish(c.flags, any_running, any_trial, 3);
-        if (use_cond) cudaGraphSetConditional(h_trial, any_trial);
-    }
+k_ctl_after_project(const Geom G, CtlBufs c, int then, cudaGraphConditionalHandle h_loop, int use_cond, int n_seq) {
+    __shared__ CtlShared sh;
+    tl_begin(G.tl);
+    put_word(&sh.o, get_word((const CallOpts*)c.opts));
+    __syncthreads();
+    if (then == THEN_INIT) ctl_init_body(sh, G, c, n_seq);
+    else if (then == THEN_TRIAL) ctl_trial_body(sh, G, c, n_seq);
+    else ctl_eval_body(sh, G, c, 0);
+    if (use_cond && threadIdx.x == 0) cudaGraphSetConditional(h_loop, c.flags->loop_cond);
+    tl_end(G.tl, TLK_CTL_PROJ);
 }
 
-// After warp + projection of the candidate(s): Armijo's inequality, Eq. (3) update, Eq. (4) fit.
-__device__ void ctl_trial_body(const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond) {
-    __shared__ double red[CT / 32 + 1];
-    int any_trial = 0, any_running = 0;
-    const CallOpts o = *c.opts;
-    const int K = G.K;
-    for (int b = 0; b < o.B; ++b) {
-        // the state is worked on in registers (one round trip to L2 each way, instead of one per
-        // field touched); thread 0 writes it back
-        SolveState st = c.solves[b];
-        if (st.running && !st.trialing) any_running = 1;
-        if (!st.trialing) continue;                                                       // uniform
-        const int n = st.iter;
-        int acc = -1;
-        double acc_mu = 0.0, acc_Sp = 0.0, acc_Syp = 0.0;
-        bool failed = false;
-        // the round's candidates st.t .. st.t + C - 1 have been evaluated: the first that passes is
-        // the one sequential backtracking would have accepted (reading A7)
-        int n_cand = o.max_backtracks - st.t;
-        if (n_cand > o.C) n_cand = o.C;
-        double mu_last = st.mu;
-        for (int cnd = 0; cnd < n_cand; ++cnd) {
-            const int s = b * o.C + cnd;
-            const Sums3 sp = sum_proj(c.proj_part, c.proj_blocks, s, red);
-            if (threadIdx.x != 0) continue;
-            const double mu_s = c.slots[s].mu;
-            c.slots[s].Sp = sp.a; c.slots[s].Syp = sp.b; c.slots[s].J = sp.c;
-            if (acc < 0 && sp.c <= st.Jn - o.armijo_c * mu_s * st.g2) {                   // Armijo (L95)
-                acc = s; acc_mu = mu_s; acc_Sp = sp.a; acc_Syp = sp.b;
-                st.t += cnd;
-            }
-            c.slots[s].active = 0;
-            mu_last = mu_s;
-        }
-        if (threadIdx.x != 0) continue;
-        if (acc < 0) {
-            st.t += n_cand;
-            st.mu = mu_last * o.armijo_beta;
-            if (st.t >= o.max_backtracks) failed = true;
-            else make_round(st, K, o, &c.slots[b * o.C]);
-        }
-        if (acc >= 0) {
-            const double mu = acc_mu;
-            for (int k = 0; k < K; ++k) st.w[k] -= mu * st.g[k];                          // Eq. (3)
-            st.mu_prev = mu;
-            st.acc_slot = acc;
-            if (n < TRACE_CAP) { c.traces[b].mu[n] = mu; c.traces[b].bt[n] = st.t; }
-            st.iter = n + 1;
-            st.trialing = 0;
-            if (!lsfit((double)G.npix, st.Sy, st.Syy, acc_Sp, acc_Syp, &st.a, &st.b)) {   // Eq. (4)
-                st.status = PCAMM_E_SINGULAR; st.running = 0;
-            } else if (st.iter >= o.max_iter) { st.status = PCAMM_S_MAXITER; st.running = 0; }
-        } else if (failed) {
-            if (n < TRACE_CAP) { c.traces[b].mu[n] = 0.0; c.traces[b].bt[n] = st.t; }
-            st.status = PCAMM_S_LINESEARCH;
-            st.running = 0; st.trialing = 0;
-        }
-        if (st.trialing) any_trial = 1;
-        if (st.running) any_running = 1;
-        c.solves[b] = st;                                                                 // thread 0 only gets here
-    }
-    if (threadIdx.x == 0) {
-        publish(c.flags, any_running, any_trial, 3);
-        if (use_cond) cudaGraphSetConditional(h_trial, any_trial);
-    }
-}
-
-// Last kernel of the iteration body: decides whether the outer while-loop runs again.
-__global__ void k_ctl_iter_end(CtlBufs c, cudaGraphConditionalHandle h_iter, int use_cond) {
-    if (threadIdx.x == 0) {
-        c.flags->n_launch += 1;
-        if (use_cond) cudaGraphSetConditional(h_iter, c.flags->iter_cond);
-    }
+// The control step that follows a gradient pass (mode = GRAD_SOLVE / GRAD_EVAL): one block.  (The
+// loop condition it may change is handed over by the step after the projection, which always
+// follows in the same loop body.)
+__global__ void __launch_bounds__(CT)
+k_ctl_after_grad(const Geom G, CtlBufs c, int mode) {
+    __shared__ CtlShared sh;
+    tl_begin(G.tl);
+    put_word(&sh.o, get_word((const CallOpts*)c.opts));
+    __syncthreads();
+    if (mode == GRAD_SOLVE) ctl_grad_body(sh, G, c);
+    else ctl_eval_body(sh, G, c, 1);
+    tl_end(G.tl, TLK_CTL_GRAD);
 }
 
 // After the closing residual pass: J at exit, final w into the output slots.
 __global__ void __launch_bounds__(CT)
-k_ctl_final(const Geom G, CtlBufs c, SlotState* out_slots) {
-    __shared__ double red[CT / 32 + 1];
-    const CallOpts& o = *c.opts;
-    for (int b = 0; b < o.B; ++b) {
+k_ctl_final(const Geom G, CtlBufs c, SlotState* out_slots, int n_seq) {
+    __shared__ CtlShared sh;
+    tl_begin(G.tl);
+    const int B = c.opts->B;
+    for (int b = 0; b < B; ++b) {
         SolveState& st = c.solves[b];
-        const double J = coop_sum(c.resid_part + (long long)b * c.resid_blocks, c.resid_blocks, 1, red);
+        double vj[1];
+        load_partials<1, 4>(c.resid_part + (long long)b * c.resid_blocks, c.resid_blocks, 1, vj);
+        reduce_partials<1>(sh, vj, 0);
         if (threadIdx.x != 0) continue;
-        st.J = J;
+        st.J = sh.res[0][0];
         if (isnan(st.J0)) st.J0 = st.J;
         if (st.iter <= TRACE_CAP) c.traces[b].J[st.iter] = st.J;
         SlotState& sl = out_slots[b];
         for (int k = 0; k < KMAX; ++k) sl.w[k] = k < G.K ? (float)st.w[k] : 0.f;
         sl.active = 1; sl.solve = b; sl.mu = 0.0; sl.J = st.J; sl.Sp = sl.Syp = 0.0;
     }
-    if (threadIdx.x == 0) c.flags->n_launch += 3;
-}
-
-// pcamm_eval: stage 0 after the projection (J at the given (a, b), fit of Eq. 4), stage 1 after
-// the gradient.
-__device__ void ctl_eval_body(const Geom& G, const CtlBufs& c, int stage) {
-    __shared__ double red[CT / 32 + 1];
-    const CallOpts& o = *c.opts;
-    for (int b = 0; b < o.B; ++b) {
-        SolveState& st = c.solves[b];
-        if (stage == 0) {
-            const double* yp = c.ysum_part + (long long)b * c.ysum_blocks * 2;
-            const double Sy = coop_sum(yp, c.ysum_blocks, 2, red), Syy = coop_sum(yp + 1, c.ysum_blocks, 2, red);
-            const Sums3 sp = sum_proj(c.proj_part, c.proj_blocks, b * o.C, red);
-            if (threadIdx.x != 0) continue;
-            st.Sy = Sy; st.Syy = Syy;
-            st.J = sp.c;
-            st.fit_a = st.fit_b = nan("");
-            lsfit((double)G.npix, Sy, Syy, sp.a, sp.b, &st.fit_a, &st.fit_b);
-            st.acc_slot = b * o.C;
-        } else {
-            const double Jn = coop_sum(c.resid_part + (long long)b * c.resid_blocks, c.resid_blocks, 1, red);
-            double gk[KMAX];
-            for (int k = 0; k < G.K; ++k)
-                gk[k] = coop_sum(c.grad_part + (long long)b * c.grad_blocks * KMAX + k, c.grad_blocks, KMAX, red);
-            if (threadIdx.x != 0) continue;
-            st.Jn = Jn;
-            for (int k = 0; k < G.K; ++k) st.g[k] = 2.0 * gk[k];
-        }
-    }
-}
-
-__global__ void __launch_bounds__(CT)
-k_ctl_eval_grad(const Geom G, CtlBufs c) { ctl_eval_body(G, c, 1); }
-
-// The control step that follows a projection (then = THEN_INIT / THEN_TRIAL / THEN_EVAL): one block.
-__global__ void __launch_bounds__(CT)
-k_ctl_after_project(const Geom G, CtlBufs c, int then, cudaGraphConditionalHandle h, int use_cond) {
-    if (then == THEN_INIT) ctl_init_body(G, c, h, use_cond);
-    else if (then == THEN_TRIAL) ctl_trial_body(G, c, h, use_cond);
-    else ctl_eval_body(G, c, 0);
+    if (threadIdx.x == 0) c.flags->n_launch += n_seq;
+    tl_end(G.tl, TLK_FINAL);
 }
 
 // a-6.  One warp per (landmark, solve).  x(r) is the trilinear interpolation of the synthesised
@@ -392,6 +131,7 @@ k_ctl_after_project(const Geom G, CtlBufs c, int then, cudaGraphConditionalHandl
 __global__ void __launch_bounds__(32)
 k_invert(const Geom G, const float* __restrict__ xbar, const float* __restrict__ u, const CallOpts* __restrict__ opts,
          const SolveState* __restrict__ solves, int M, const float* __restrict__ r0s, double* __restrict__ r_out) {
+    tl_begin(G.tl);
     const int m = blockIdx.x, b = blockIdx.y, lane = threadIdx.x;
     const int K = G.K;
     const long long V = G.V;
@@ -444,6 +184,7 @@ k_invert(const Geom G, const float* __restrict__ xbar, const float* __restrict__
         double* o = r_out + ((long long)b * M + m) * 3;
         o[0] = r[0]; o[1] = r[1]; o[2] = r[2];
     }
+    tl_end(G.tl, TLK_INVERT);
 }
 
 }  // namespace
@@ -459,26 +200,19 @@ void launch_begin(Seq& q, const Geom& G, const CtlBufs& c, int mode) {
              c.flags, mode);
 }
 
-void launch_ctl_grad(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond) {
-    q.launch(k_ctl_grad, dim3(1), dim3(CT), 0, G, c, h_trial, use_cond);
-}
-
-void launch_ctl_iter_end(Seq& q, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond) {
-    q.launch(k_ctl_iter_end, dim3(1), dim3(32), 0, c, h_iter, use_cond);
-}
-
-void launch_ctl_final(Seq& q, const Geom& G, const CtlBufs& c, SlotState* out_slots) {
-    q.launch(k_ctl_final, dim3(1), dim3(CT), 0, G, c, out_slots);
-}
-
-void launch_ctl_eval_grad(Seq& q, const Geom& G, const CtlBufs& c) {
-    q.launch(k_ctl_eval_grad, dim3(1), dim3(CT), 0, G, c);
-}
-
 void launch_ctl_after_project(Seq& q, const Geom& G, const CtlBufs& c, int then, cudaGraphConditionalHandle h,
-                              int use_cond) {
+                              int use_cond, int n_before) {
     if (then == THEN_NONE) return;
-    q.launch(k_ctl_after_project, dim3(1), dim3(CT), 0, G, c, then, h, use_cond);
+    q.launch(k_ctl_after_project, dim3(1), dim3(CT), 0, G, c, then, h, use_cond, n_before + 1);
+}
+
+void launch_ctl_after_grad(Seq& q, const Geom& G, const CtlBufs& c, int mode) {
+    if (mode == GRAD_NONE) return;
+    q.launch(k_ctl_after_grad, dim3(1), dim3(CT), 0, G, c, mode);
+}
+
+void launch_ctl_final(Seq& q, const Geom& G, const CtlBufs& c, SlotState* out_slots, int n_seq) {
+    q.launch(k_ctl_final, dim3(1), dim3(CT), 0, G, c, out_slots, n_seq);
 }
 
 void launch_invert(Seq& q, const Geom& G, const float* xbar, const float* u, const CtlBufs& c, int B, int M,

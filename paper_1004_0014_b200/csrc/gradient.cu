@@ -39,9 +39,10 @@ k_resid(const Geom G, const SolveState* __restrict__ solves, const SolveIn* __re
         int force, const float* __restrict__ p_slots, const float* __restrict__ r_direct, float* __restrict__ rL,
         float4* __restrict__ utab, float2* __restrict__ vtab, double* __restrict__ partials) {
     __shared__ double red[RT / 32];
+    tl_begin(G.tl);
     const int b = blockIdx.y;
     const SolveState& st = solves[b];
-    if (!st.running && !force) return;
+    if (!needs_gradient(st) && !force) { tl_end(G.tl, TLK_RESID); return; }
     const View vw = st.view;
     const int pix = blockIdx.x * RT + threadIdx.x;
     double rr = 0.0;
@@ -72,6 +73,7 @@ k_resid(const Geom G, const SolveState* __restrict__ solves, const SolveIn* __re
     }
     const double s = block_sum<RT>(rr, red);
     if (threadIdx.x == 0) partials[(long long)b * gridDim.x + blockIdx.x] = s;
+    tl_end(G.tl, TLK_RESID);
 }
 
 // Per-view constants of the gather, in float.
@@ -156,9 +158,12 @@ __device__ __forceinline__ void trilinear_grad(const Geom& G, const float* __res
 template <int K>
 __global__ void __launch_bounds__(GT)
 k_grad_generic(const Geom G, const float* __restrict__ f0, const float* __restrict__ xbar, const float* __restrict__ u,
-       const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
-       const float2* __restrict__ vtab, double* __restrict__ partials) {
+       const CtlBufs c, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
+       const float2* __restrict__ vtab) {
     __shared__ double red[GT / 32];
+    tl_begin(G.tl);
+    const SolveState* __restrict__ solves = c.solves;
+    double* __restrict__ partials = c.grad_part;
     const int lane = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int x0 = blockIdx.x * TILE, y0 = blockIdx.y * TILE, z = blockIdx.z;
     const int x = x0 + lane;
@@ -184,7 +189,7 @@ k_grad_generic(const Geom G, const float* __restrict__ f0, const float* __restri
     const float zw = G.cz + ((float)z - 0.5f * (G.nz - 1)) * G.hz;
 
     for (int b = 0; b < B; ++b) {
-        if (!solves[b].running) continue;               // uniform over the grid
+        if (!needs_gradient(solves[b])) continue;       // uniform over the grid
         float w[K];
 #pragma unroll
         for (int k = 0; k < K; ++k) w[k] = (float)solves[b].w[k];
@@ -222,10 +227,11 @@ k_grad_generic(const Geom G, const float* __restrict__ f0, const float* __restri
             if (threadIdx.x == 0) partials[((long long)b * nblk + blk) * KMAX + k] = s;
         }
     }
+    tl_end(G.tl, TLK_GRAD);
 }
 
 int grad_grid(const Geom& G, const FieldStream& fs) {
-    const long long nt = tile_count(G, G.K <= 4 ? 32 : 16);      // TileZ<K>
+    const long long nt = tile_count(G, G.K <= PCAMM_TZ_SMALL_K ? 32 : 16);      // TileZ<K>
     return (int)(nt < fs.n_sm ? nt : fs.n_sm);
 }
 
@@ -247,7 +253,7 @@ int grad_grid(const Geom& G, const FieldStream& fs) {
 
 // Consumer groups per CTA: three where their stages and queues fit into shared memory, else two.
 constexpr int grad_groups_for(int K) {
-    const int tz = K <= 4 ? 32 : 16;                                      // TileZ<K>
+    const int tz = K <= PCAMM_TZ_SMALL_K ? 32 : 16;                       // TileZ<K>
     const int stage = 3 * (K + 1) * tz * TX * 4;
     const int queue = GROUP_THREADS * 3 * (8 + 4 * K);                    // GradQueueCap x sizeof(QueueEntry)
     return 3 * (stage + queue) + 16 * 1024 <= 227 * 1024 ? 3 : 2;
@@ -270,7 +276,7 @@ template <int K> struct GradQueueCap { static constexpr int value = GROUP_THREAD
 template <int K>
 constexpr size_t grad_queue_bytes() { return (size_t)GradGroups<K>::value * GradQueueCap<K>::value * sizeof(QueueEntry<K>); }
 template <int K, bool H> struct GradStages {
-    static constexpr int value = stages_per_group<K, H>(GradGroups<K>::value, 2, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
+    static constexpr int value = stages_per_group<K, H>(GradGroups<K>::value, PCAMM_MAX_SPG, 227 * 1024 - GSTATIC - (int)grad_queue_bytes<K>() - 64);
 };
 template <int K, bool H>
 constexpr size_t grad_smem_bytes() {
@@ -285,9 +291,10 @@ template <int K, bool SINGLE, bool H, bool SKIP>
 __global__ void __launch_bounds__(32 * GradGroups<K>::value * GROUP_WARPS, 1)
 k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
            const FieldMax fmax, const unsigned* __restrict__ cell_integral, const Geom G, const float* __restrict__ f0,
-           const unsigned char* __restrict__ cellmap, const SolveState* __restrict__ solves, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
-           const float2* __restrict__ vtab, double* __restrict__ partials) {
+           const unsigned char* __restrict__ cellmap, const CtlBufs c, int b0, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
+           const float2* __restrict__ vtab, unsigned long long* __restrict__ visited) {
     constexpr int P = 3 * (K + 1), GTZ = TileZ<K>::value, GROWS = GTZ / GROUP_WARPS;
+    const SolveState* __restrict__ solves = c.solves + b0;                 // solves b0 .. b0 + B - 1 in this launch
     constexpr int RB = GradBatch<K>::value, NB = GROWS / RB;
     static_assert(GROWS % RB == 0 && NB >= 1, "tile rows per thread must be a multiple of the batch");
     constexpr int GNG = GradGroups<K>::value;
@@ -301,10 +308,11 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     __shared__ int s_reach[3];                             // reach of the stencils, max over the running solves
     __shared__ int s_issue[GNG][2];
     __shared__ unsigned s_skip[GNG][GRAD_SKIP_WORDS];      // per group: bit jt set = nothing to do in its jt-th tile
+    tl_begin(G.tl);
     if (SKIP && threadIdx.x < 3) {
         float dmax = 0.f;
         for (int b = 0; b < B; ++b) {
-            if (!solves[b].running) continue;
+            if (!needs_gradient(solves[b])) continue;
             float d = fmax.v[threadIdx.x];
             for (int k = 0; k < K; ++k) d = fmaf(fabsf((float)solves[b].w[k]) * 1.000001f, fmax.v[3 + 3 * k + threadIdx.x], d);
             dmax = fmaxf(dmax, d);
@@ -312,7 +320,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
         s_reach[threadIdx.x] = reach_of(dmax);
     }
     for (int b = threadIdx.x; b < B; b += blockDim.x) {    // B <= SOLVE_CACHE (the launcher chunks)
-        s_running[b] = solves[b].running;
+        s_running[b] = needs_gradient(solves[b]);
         s_gv[b] = make_gather_view(G, solves[b].view);
 #pragma unroll
         for (int k = 0; k < K; ++k) s_w[b][k] = H ? (float)solves[b].w[k] * scale.inv[k] : (float)solves[b].w[k];
@@ -332,11 +340,12 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     QueueEntry<K>* queue = queues + (size_t)group * QCAP;   // ring buffer: q_head .. q_head + q_n - 1 (mod QCAP)
     int q_head = 0, q_n = 0, parity = 0;                    // identical in every thread of the group
     const int nslot = gridDim.x * GNG, slot = blockIdx.x * GNG + group;   // this group's partial-sum slot
+    double* __restrict__ partials = c.grad_part + (long long)b0 * nslot * KMAX;
     if (gtid < K)
         for (int b = 0; b < B; ++b) partials[((long long)b * nslot + slot) * KMAX + gtid] = 0.0;
     bool any_running = false;
     for (int b = 0; b < B; ++b) any_running |= s_running[b] != 0;
-    if (!any_running) return;                              // uniform over the grid
+    if (!any_running) { tl_end(G.tl, TLK_GRAD); return; }  // uniform over the grid
     const bool leader = gtid == 0;
     const uint64_t policy = l2_evict_first_policy();
     // A tile all of whose voxels can only land in constant cells of f0 (summed-volume table of the
@@ -562,6 +571,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
             }
         }
     }
+    if (leader && visited) atomicAdd(visited + 1, (unsigned long long)(SKIP ? n_loaded : j));
     if (SINGLE) {                                           // the group's K sums over all its tiles
         if (s_running[0]) {                                 // what is left in the queue
             group_barrier(group);
@@ -594,6 +604,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
             partials[(long long)slot * KMAX + gtid] = tot;
         }
     }
+    tl_end(G.tl, TLK_GRAD);
 }
 
 // The cell map of FieldStream: one thread per interpolation cell.
@@ -632,8 +643,8 @@ k_backproject(const Geom G, const SolveState* __restrict__ solves, const float* 
 }
 
 template <int K, bool H>
-void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
-                const float* rL, const float4* utab, const float2* vtab, double* partials) {
+void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const CtlBufs& c, int B,
+                const float* rL, const float4* utab, const float2* vtab) {
     static DeviceOnce configured;
     constexpr size_t smem = grad_smem_bytes<K, H>();
     {
@@ -647,33 +658,32 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
         if (e0 != cudaSuccess) { q.err = e0; return; }
     }
     constexpr int GNG = GradGroups<K>::value, GTHREADS = 32 * GNG * GROUP_WARPS;
-    const int grid = grad_grid(G, fs), nslot = grid * GNG;
+    const int grid = grad_grid(G, fs);
     // the flags cost a few dependent loads per launch: only where a CTA has tiles enough to win them back
     const unsigned* skip_table = tile_count(G, TileZ<K>::value) >= fs.skip_min_tiles_per_sm * (long long)fs.n_sm ? fs.cell_integral : nullptr;
     if (B == 1) {
         q.launch(skip_table ? k_grad_tma<K, true, H, true> : k_grad_tma<K, true, H, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, skip_table, G, f0,
-                 fs.cellmap, solves, 1, rL, utab, vtab, partials);
+                 fs.cellmap, c, 0, 1, rL, utab, vtab, fs.visited);
         return;
     }
     for (int b0 = 0; b0 < B; b0 += SOLVE_CACHE) {       // the kernel keeps up to SOLVE_CACHE solves' constants on chip
         const int nb = B - b0 < SOLVE_CACHE ? B - b0 : SOLVE_CACHE;
         q.launch(skip_table ? k_grad_tma<K, false, H, true> : k_grad_tma<K, false, H, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, skip_table, G, f0,
-                 fs.cellmap, solves + b0, nb, rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu,
-                 vtab + (long long)b0 * G.nv, partials + (long long)b0 * nslot * KMAX);
+                 fs.cellmap, c, b0, nb, rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu,
+                 vtab + (long long)b0 * G.nv, fs.visited);
     }
 }
 
 template <int K>
-void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
-              const float* rL, const float4* utab, const float2* vtab, double* partials) {
+void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const CtlBufs& c, int B,
+              const float* rL, const float4* utab, const float2* vtab) {
     if (fs.use_tma) {
-        if (fs.half_u) launch_tma<K, true>(q, G, fs, f0, solves, B, rL, utab, vtab, partials);
-        else launch_tma<K, false>(q, G, fs, f0, solves, B, rL, utab, vtab, partials);
+        if (fs.half_u) launch_tma<K, true>(q, G, fs, f0, c, B, rL, utab, vtab);
+        else launch_tma<K, false>(q, G, fs, f0, c, B, rL, utab, vtab);
         return;
     }
     dim3 grid((G.nx + TILE - 1) / TILE, (G.ny + TILE - 1) / TILE, G.nz);
-    q.launch(k_grad_generic<K>, grid, dim3(GT), 0, G, f0, fs.fields, fs.fields + 3 * G.V, solves, B, rL, utab, vtab,
-             partials);
+    q.launch(k_grad_generic<K>, grid, dim3(GT), 0, G, f0, fs.fields, fs.fields + 3 * G.V, c, B, rL, utab, vtab);
 }
 
 }  // namespace
@@ -696,16 +706,17 @@ void launch_resid(Seq& q, const Geom& G, const SolveState* solves, const SolveIn
              partials);
 }
 
-void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
-                 const float* rL, const float4* utab, const float2* vtab, double* partials) {
+void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const CtlBufs& c, int B,
+                 const float* rL, const float4* utab, const float2* vtab, int mode) {
     switch (G.K) {
 #define PCAMM_CASE(KK) \
-    case KK: launch_k<KK>(q, G, fs, f0, solves, B, rL, utab, vtab, partials); break;
+    case KK: launch_k<KK>(q, G, fs, f0, c, B, rL, utab, vtab); break;
         PCAMM_CASE(1) PCAMM_CASE(2) PCAMM_CASE(3) PCAMM_CASE(4)
         PCAMM_CASE(5) PCAMM_CASE(6) PCAMM_CASE(7) PCAMM_CASE(8)
 #undef PCAMM_CASE
         default: break;
     }
+    launch_ctl_after_grad(q, G, c, mode);       // the control step that follows the gradient (control.cu)
 }
 
 void launch_backproject(Seq& q, const Geom& G, const SolveState* solves, const float* rL, const float4* utab,

@@ -52,6 +52,7 @@ struct Seq {
     cudaGraphNode_t last = nullptr;
     bool has_last = false;
     cudaError_t err = cudaSuccess;
+    int n_kernels = 0;        // kernels appended so far (not counting the bodies of while-loops)
 
     bool graph_mode() const { return graph != nullptr; }
 
@@ -83,6 +84,7 @@ struct Seq {
     template <class... KArgs>
     void launch_impl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, KArgs... args) {
         void* argv[] = {(void*)&args...};
+        ++n_kernels;
         if (graph) {
             cudaKernelNodeParams kp = {};
             kp.func = (void*)kernel;
@@ -112,17 +114,18 @@ void launch_warp(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, 
 int project_blocks(const Geom& G);
 int max_slabs(const Geom& G);
 extern int g_chunks_per_segment, g_scan_slabs;     // measurement knobs (pcamm_tune): 0 = automatic
+extern int g_timeline;                             // 1: models record the kernel timeline of their solves
 bool project_fits(const Geom& G);    // the knots of one scan row set fit into shared memory (nz up to ~ 4000)
 // in-plane traversal tables of the views of solves 0..B-1 (once per solve: the angle is fixed)
 void launch_view_tables(Seq& q, const Geom& G, const SolveState* solves, int B, ColHdr* hdr, SlabEntry* tab);
 int project_segments(const Geom& G);
-struct CtlBufs;
 // p[s] = P f[s] for every active slot (volumes in the ray layout; pseg: scratch
 // [nslots][segments][nu][nv] for the per-segment partial line integrals), the a-3 partial sums
-// {sum p, sum y p, sum (p - a y - b)^2}, and then the control step `then` (THEN_*, common.cuh).
+// {sum p, sum y p, sum (p - a y - b)^2}, and then the control step `then` (THEN_*, common.cuh);
+// n_before: kernels of the sequence in front of this launch.
 void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const ColHdr* hdr, const SlabEntry* tab,
                     const float* vol, const unsigned char* occ, float* pseg, float* p, int then,
-                    cudaGraphConditionalHandle h, int use_cond);
+                    cudaGraphConditionalHandle h, int use_cond, int n_before);
 // hooks: standard layout -> ray layout; one ray of the view of solve 0
 void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray, unsigned char* occ);
 void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* tab, int iu, int iv, int cap,
@@ -137,38 +140,26 @@ void launch_build_cellmap(cudaStream_t st, const Geom& G, const float* f0, unsig
 // force: also for solves that are no longer running (closing pass); r_direct: take r from there.
 void launch_resid(Seq& q, const Geom& G, const SolveState* solves, const SolveIn* in, int B, int force,
                   const float* p, const float* r_direct, float* rL, float4* utab, float2* vtab, double* partials);
-// g = 2 U^T (df/dx) P^T r, per-block partial sums [B][blocks][K].
-void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SolveState* solves, int B,
-                 const float* rL, const float4* utab, const float2* vtab, double* partials);
+// g = 2 U^T (df/dx) P^T r for the solves that need it (control.cuh needs_gradient), per-block partial
+// sums [B][blocks][K], and then the control step `mode` (GRAD_*).
+void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const CtlBufs& c, int B,
+                 const float* rL, const float4* utab, const float2* vtab, int mode);
 // hook: B = P^T r as a volume for solve 0's view (rL/utab/vtab as written by launch_resid).
 void launch_backproject(Seq& q, const Geom& G, const SolveState* solves, const float* rL, const float4* utab,
                         const float2* vtab, float* vol_out);
 
-// ---- control (control.cu)
-struct CtlBufs {
-    CallOpts* opts;
-    SolveIn* in;
-    SolveState* solves;
-    SolveTrace* traces;
-    SlotState* slots;
-    LoopFlags* flags;
-    int* seg_ticket;     // [S][proj_blocks]: segment blocks of a ray group that are done (self-resetting)
-    double* ysum_part;   // [B][ysum_blocks][2]
-    double* proj_part;   // [S][project_blocks][3]
-    double* resid_part;  // [B][resid_blocks]
-    double* grad_part;   // [B][grad_blocks][K]
-    int ysum_blocks, proj_blocks, resid_blocks, grad_blocks;
-};
+// ---- control (control.cu; the steps themselves are device functions of control.cuh)
 int ysum_blocks(const Geom& G);
 void launch_ysums(Seq& q, const Geom& G, const CtlBufs& c, int B);
 // begin: views, w = w_init, slot 0 of every solve = w_init.  mode 0 solve, 1 eval hook.
 void launch_begin(Seq& q, const Geom& G, const CtlBufs& c, int mode);
-void launch_ctl_grad(Seq& q, const Geom& G, const CtlBufs& c, cudaGraphConditionalHandle h_trial, int use_cond);
-void launch_ctl_iter_end(Seq& q, const CtlBufs& c, cudaGraphConditionalHandle h_iter, int use_cond);
-void launch_ctl_final(Seq& q, const Geom& G, const CtlBufs& c, SlotState* out_slots);
-void launch_ctl_eval_grad(Seq& q, const Geom& G, const CtlBufs& c);
+// the single-block control steps (control.cuh) behind a projection / a gradient pass; in graph mode
+// the first also hands LoopFlags::loop_cond to the while-node.  n_before: kernels of the sequence
+// in front of it (launch accounting)
 void launch_ctl_after_project(Seq& q, const Geom& G, const CtlBufs& c, int then, cudaGraphConditionalHandle h,
-                              int use_cond);
+                              int use_cond, int n_before);
+void launch_ctl_after_grad(Seq& q, const Geom& G, const CtlBufs& c, int mode);
+void launch_ctl_final(Seq& q, const Geom& G, const CtlBufs& c, SlotState* out_slots, int n_seq);
 // a-6: landmarks [B][M][3]
 void launch_invert(Seq& q, const Geom& G, const float* xbar, const float* u, const CtlBufs& c, int B, int M,
                    const float* r0, double* r_out);

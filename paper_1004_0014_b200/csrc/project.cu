@@ -96,6 +96,7 @@ __device__ __forceinline__ ColSetup col_setup(const Geom& G, const View& vw, int
 __global__ void __launch_bounds__(128)
 k_view_tables(const Geom G, const SolveState* __restrict__ solves, ColHdr* __restrict__ hdr,
               SlabEntry* __restrict__ tab, int max_slabs) {
+    tl_begin(G.tl);
     const int iu = blockIdx.x, b = blockIdx.y;
     const View vw = solves[b].view;
     double dxy2;
@@ -137,6 +138,7 @@ k_view_tables(const Geom G, const SolveState* __restrict__ solves, ColHdr* __res
         e.tt = 4294967296.f;
         row[n] = e;
     }
+    tl_end(G.tl, TLK_VIEW);
 }
 
 // ------------------------------------------------------------------ per-ray z tracking
@@ -253,11 +255,9 @@ __device__ __forceinline__ void add64(unsigned& lo, unsigned& hi, unsigned dlo, 
 // chunk's exit at the level the ray has by then.
 template <int VEC, int SC, int RPT>
 __global__ void __launch_bounds__(PT, SC == 4 ? 3 : 4)
-k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* __restrict__ solves,
-          const SolveIn* __restrict__ in, const ColHdr* __restrict__ hdr, const SlabEntry* __restrict__ tab,
+k_project(const Geom G, const CtlBufs c, int slot0, const ColHdr* __restrict__ hdr, const SlabEntry* __restrict__ tab,
           int max_slabs, int n_seg, int n_chunks, int NZP, const float* __restrict__ vol,
-          const unsigned char* __restrict__ occ, float* pseg, float* __restrict__ p_out, double* __restrict__ partials,
-          int* seg_ticket) {
+          const unsigned char* __restrict__ occ, float* pseg, float* __restrict__ p_out) {
     constexpr int CH = PWARPS * SC, NKNOT = 2 * SC + 1;
     constexpr int LOG_SC = SC == 4 ? 2 : (SC == 2 ? 1 : 0);
     extern __shared__ __align__(16) float s_knots[];        // [PWARPS][NKNOT][NZP], then P [PWARPS + 1][NZP]
@@ -266,10 +266,15 @@ k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* _
     __shared__ int s_air[PWARPS];
     __shared__ double red[PT / 32];
     __shared__ int s_last;
+    tl_begin(G.tl);
     int seg = blockIdx.y, rb = 0;
     if (seg >= n_seg) { rb = seg / n_seg; seg -= rb * n_seg; }
-    const int iu = blockIdx.x, s = blockIdx.z;
-    if (!slots[s].active) return;                            // uniform over the block
+    const int iu = blockIdx.x, s = slot0 + blockIdx.z;
+    const SlotState* __restrict__ slots = c.slots;
+    const SolveState* __restrict__ solves = c.solves;
+    int* seg_ticket = c.seg_ticket;
+    double* __restrict__ partials = c.proj_part;
+    if (!slots[s].active) { tl_end(G.tl, TLK_PROJECT); return; }     // uniform over the block
     const int b = slots[s].solve;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int p_off = PWARPS * NKNOT * NZP;                  // start of P in s_knots
@@ -467,10 +472,10 @@ k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* _
             if (s_last) { *t = 0; __threadfence(); }
         }
         __syncthreads();
-        if (!s_last) return;
+        if (!s_last) { tl_end(G.tl, TLK_PROJECT); return; }
     }
     double vp = 0.0, vyp = 0.0, vrr = 0.0;
-    const float* y = in[b].y;
+    const float* y = c.in[b].y;
     const double fa = solves[b].a, fb = solves[b].b;
     auto finish = [&](int iv, float acc) {
         const long long pix = (long long)iv * G.nu + iu;
@@ -500,6 +505,7 @@ k_project(const Geom G, const SlotState* __restrict__ slots, const SolveState* _
     const double syp = block_sum<PT>(vyp, red);
     const double srr = block_sum<PT>(vrr, red);
     if (threadIdx.x == 0) { out[0] = sp; out[1] = syp; out[2] = srr; }
+    tl_end(G.tl, TLK_PROJECT);
 }
 
 // Standard [z][y][x] -> ray layout (hook path only: the solve's volumes are written in the ray
@@ -602,16 +608,15 @@ void launch_project_t(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const
     const int row_blocks = (G.nv + RPT * PT - 1) / (RPT * PT);
     for (int s0 = 0; s0 < nslots; s0 += 65535) {              // gridDim.z
         const int ns = nslots - s0 < 65535 ? nslots - s0 : 65535;
-        q.launch(k_project<VEC, SC, RPT>, dim3(G.nu, n_seg * row_blocks, ns), dim3(PT), smem, G, (const SlotState*)c.slots + s0,
-                 (const SolveState*)c.solves, (const SolveIn*)c.in, hdr, tab, max_slabs(G), n_seg, cps, knot_pitch(G.nz),
-                 vol + (long long)s0 * G.PV, occ + (long long)s0 * G.OCC, pseg + (long long)s0 * n_seg * G.npix,
-                 p + (long long)s0 * G.npix, c.proj_part + (long long)s0 * G.nu * 3, c.seg_ticket + (long long)s0 * G.nu);
+        q.launch(k_project<VEC, SC, RPT>, dim3(G.nu, n_seg * row_blocks, ns), dim3(PT), smem, G, c, s0, hdr, tab,
+                 max_slabs(G), n_seg, cps, knot_pitch(G.nz), vol, occ, pseg, p);
     }
 }
 
 void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const ColHdr* hdr, const SlabEntry* tab,
                     const float* vol, const unsigned char* occ, float* pseg, float* p, int then,
-                    cudaGraphConditionalHandle h, int use_cond) {
+                    cudaGraphConditionalHandle h, int use_cond, int n_before) {
+    const int n_mark = q.n_kernels;
     const int sc = scan_slabs(G);
     const bool v4 = G.nz % 4 == 0, one = G.nv <= PT;
 #define PCAMM_PROJ(VEC, SC) \
@@ -621,7 +626,8 @@ void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const C
     else if (sc == 2) { if (v4) PCAMM_PROJ(4, 2); else PCAMM_PROJ(1, 2); }
     else { if (v4) PCAMM_PROJ(4, 1); else PCAMM_PROJ(1, 1); }
 #undef PCAMM_PROJ
-    launch_ctl_after_project(q, G, c, then, h, use_cond);
+    // the control step that follows the projection (control.cu); n_before + the kernels launched here
+    launch_ctl_after_project(q, G, c, then, h, use_cond, q.n_kernels - n_mark + n_before);
 }
 
 void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray, unsigned char* occ) {

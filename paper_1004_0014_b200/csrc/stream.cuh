@@ -37,12 +37,15 @@ __host__ __device__ __forceinline__ int tiles_z(const Geom& G, int tz) { return 
 __host__ __device__ __forceinline__ long long tile_count(const Geom& G, int tz) {
     return (long long)tiles_x(G) * G.ny * tiles_z(G, tz);
 }
-__device__ __forceinline__ TileCoord tile_coord(const Geom& G, int tz, long long t) {
-    const int ntx = tiles_x(G);
+// (t < 2^31: pcamm_model_create bounds the volume; 32-bit divisions)
+__device__ __forceinline__ TileCoord tile_coord(const Geom& G, int tz, long long t64) {
+    const unsigned t = (unsigned)t64, ntx = (unsigned)tiles_x(G);
+    const unsigned row = t / ntx;                       // (y, z tile)
+    const unsigned zt = row / (unsigned)G.ny;
     TileCoord c;
-    c.x0 = (int)(t % ntx) * TX;
-    c.y = (int)((t / ntx) % G.ny);
-    c.z0 = (int)(t / ((long long)ntx * G.ny)) * tz;
+    c.x0 = (int)(t - row * ntx) * TX;
+    c.y = (int)(row - zt * (unsigned)G.ny);
+    c.z0 = (int)zt * tz;
     return c;
 }
 
@@ -240,11 +243,20 @@ struct FieldStream {
     const unsigned* cell_integral = nullptr;
     FieldMax fmax = {};
     int skip_min_tiles_per_sm = SKIP_MIN_TILES_PER_SM;     // geometry.tile_skipping: 0 always, INT_MAX never
+    // measurement: tiles whose fields the warp / gradient kernels really loaded, summed over the
+    // launches since the host last cleared them ([0] warp, [1] gradient; one atomic per consumer group)
+    unsigned long long* visited = nullptr;
 };
 
 // Tile extent along z and ring depth by K: a stage is 3(K+1) planes x TZ x TX floats and the
 // ring has to fit in 227 KB of shared memory next to the kernel's own buffers.
-template <int K> struct TileZ { static constexpr int value = K <= 4 ? 32 : 16; };
+#ifndef PCAMM_TZ_SMALL_K
+#define PCAMM_TZ_SMALL_K 4      // largest K with 32-slice tiles (experiments: 0 = 16 slices for every K)
+#endif
+#ifndef PCAMM_MAX_SPG
+#define PCAMM_MAX_SPG 2         // stages per consumer group, at most
+#endif
+template <int K> struct TileZ { static constexpr int value = K <= PCAMM_TZ_SMALL_K ? 32 : 16; };
 // stages per consumer group that fit into budget_bytes, at most max_spg
 template <int K, bool H = false>
 constexpr int stages_per_group(int n_groups, int max_spg, int budget_bytes) {

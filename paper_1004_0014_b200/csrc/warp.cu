@@ -50,6 +50,7 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
        const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride,
        unsigned char* __restrict__ occ) {
     __shared__ float tile[TILE][TILE + 1];
+    tl_begin(G.tl);
     const int lane = threadIdx.x & 31, tw = threadIdx.x >> 5;
     const int x0 = blockIdx.x * TILE, z0 = blockIdx.y * TILE, y = blockIdx.z;
     const int x = x0 + lane;
@@ -112,19 +113,23 @@ k_warp_generic(const Geom G, const float* __restrict__ f0, const float* __restri
             }
         }
     }
+    tl_end(G.tl, TLK_WARP);
 }
 
 // ---------------------------------------------------------------- the TMA-fed kernel
 
 // consumer groups: four where the stages of the 16-slice tiles (K = 5, 6) leave room for them
 // and for the L1 lines of the f0 gathers, else three
-template <int K> struct WarpGroups { static constexpr int value = (K == 5 || K == 6) ? 4 : 3; };
+#ifndef PCAMM_WARP_GROUPS
+#define PCAMM_WARP_GROUPS 3
+#endif
+template <int K> struct WarpGroups { static constexpr int value = (K == 5 || K == 6) ? 4 : PCAMM_WARP_GROUPS; };
 constexpr int AIR_WORDS = 64;      // air flags of up to 2048 tiles per consumer group (beyond: never skipped)
 constexpr int SLOT_CACHE = 64;     // slots whose coefficients are kept in shared memory
 template <int K> struct WarpThreads { static constexpr int value = 32 * WarpGroups<K>::value * GROUP_WARPS; };
 
 constexpr int WSTATIC = 16 * 1024; // static shared memory of the kernel (transposition tiles, slot cache), rounded up
-template <int K, bool H> struct WarpStages { static constexpr int value = stages_per_group<K, H>(WarpGroups<K>::value, 2, 227 * 1024 - WSTATIC - 64); };
+template <int K, bool H> struct WarpStages { static constexpr int value = stages_per_group<K, H>(WarpGroups<K>::value, PCAMM_MAX_SPG, 227 * 1024 - WSTATIC - 64); };
 
 template <int K, bool H>
 constexpr size_t warp_smem_bytes() {
@@ -138,7 +143,7 @@ __global__ void __launch_bounds__(WarpThreads<K>::value, 1)
 k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
            const FieldMax fmax, const unsigned* __restrict__ f0_integral, const Geom G, const float* __restrict__ f0,
            const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride,
-           unsigned char* __restrict__ occ) {
+           unsigned char* __restrict__ occ, unsigned long long* __restrict__ visited) {
     constexpr int P = 3 * (K + 1), WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
     constexpr int WNG = WarpGroups<K>::value;
     using Ring = FieldRing<P, WTZ, WNG, WarpStages<K, H>::value, H>;
@@ -150,6 +155,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     __shared__ int s_reach[3];                             // reach of the stencils, max over the active slots
     __shared__ int s_issue[WarpGroups<K>::value][2];
     __shared__ unsigned s_air[WarpGroups<K>::value][AIR_WORDS];   // per group: bit jt set = its jt-th tile is air
+    tl_begin(G.tl);
     if (SKIP && threadIdx.x < 3) {
         float dmax = 0.f;
         for (int i = 0; i < nslots && i < SLOT_CACHE; ++i) {
@@ -177,7 +183,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     int last_active = -1;                                  // the last slot that reads the stage
     for (int i = 0; i < nslots; ++i)
         if (s_active[i]) last_active = i;
-    if (last_active < 0) return;                           // nothing to warp
+    if (last_active < 0) { tl_end(G.tl, TLK_WARP); return; }   // nothing to warp
     const int group = warp / GROUP_WARPS, tw = warp % GROUP_WARPS;
     const bool leader = tw == 0 && lane == 0;
     const uint64_t policy = l2_evict_first_policy();
@@ -339,6 +345,8 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
             if (SKIP && !air) ++n_loaded;
         }
     }
+    if (leader && visited) atomicAdd(visited, (unsigned long long)(SKIP ? n_loaded : j));
+    tl_end(G.tl, TLK_WARP);
 }
 
 template <int K, bool RAY, bool H>
@@ -368,10 +376,10 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
         unsigned char* oc = occ ? occ + (long long)s0 * G.OCC : occ;
         if (table)
             q.launch(k_warp_tma<K, RAY, H, true>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
-                     table, G, f0, slots + s0, ns, out, slot_stride, oc);
+                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited);
         else
             q.launch(k_warp_tma<K, RAY, H, false>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
-                     table, G, f0, slots + s0, ns, out, slot_stride, oc);
+                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited);
     }
 }
 

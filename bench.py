@@ -76,56 +76,30 @@ def solver_iterations(cfg) -> int:
     return cfg.iterations
 
 
+def field_bytes_per_voxel(cfg, field_storage=0):
+    """12 (K + 1) bytes of float fields per voxel; with field_storage = 1 the u_k planes
+    are halves (6 K bytes instead of 12 K)."""
+    return 12 * (cfg.K + 1) if field_storage == 0 else 12 + 6 * cfg.K
+
+
 def algorithmic_bytes(cfg, field_storage=0):
-    """what the method must move per launch, f0 gathers counted once.
-    field_storage = 1: the u_k planes are halves (6 K bytes per voxel instead of 12 K)."""
-    V, K, npix = cfg.V, cfg.K, cfg.npix
-    fields = 12 * (K + 1) if field_storage == 0 else 12 + 6 * K
+    """what the dense method must move per launch, every voxel's fields counted,
+    f0 gathers counted once."""
+    V, npix = cfg.V, cfg.npix
+    fields = field_bytes_per_voxel(cfg, field_storage)
     return {"warp": (fields + 4 + 4) * V,
             "project": 4 * V + 4 * npix,
             "gradient": (fields + 4) * V + 4 * npix}
 
 
-def measured_traffic():
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel, from the committed
-    `ncu --set full` capture of this round (profiles/r01_traffic.json; null if absent)."""
-    try:
-        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
-            return json.load(f)
-    except Exception:
-        return {}
-
-
-# The projector is bound by instruction issue, not by HBM (its volume is L2-resident, DESIGN.md):
-# it is reported against the fp32 lane-operation rate of the SMs.  Algorithmic operations per
-# (ray, slab) of the exact slab march (DESIGN.md "Kernels", a-2): 15.
-PROJECT_OPS_PER_RAY_SLAB = 15
-ALU_PEAK_TOPS = 148 * 128 * 1.965e9 / 1e12      # 148 SMs x 128 fp32 lanes x 1.965 GHz (B200_PROFILING.md)
-
-
-def ray_slab_count(cfg, angle_rad: float) -> int:
-    """(ray, slab) pairs the projector marches at this gantry angle: per detector column the voxel
-    layers along its dominant in-plane axis in which the ray overlaps the volume (the in-plane
-    clipping of DESIGN.md a-2), times the detector rows."""
-    cs, sn = np.cos(angle_rad), np.sin(angle_rad)
-    uu = (np.arange(cfg.nu) - 0.5 * (cfg.nu - 1)) * cfg.pu
-    dx, dy = -cfg.sdd * cs - uu * sn, -cfg.sdd * sn + uu * cs
-    gx, gy = dx / cfg.hx, dy / cfg.hy
-    sx = (cfg.sad * cs + 0.5 * cfg.nx * cfg.hx) / cfg.hx
-    sy = (cfg.sad * sn + 0.5 * cfg.ny * cfg.hy) / cfg.hy
-    along_x = np.abs(gx) >= np.abs(gy)
-    gm, gt = np.where(along_x, gx, gy), np.where(along_x, gy, gx)
-    sm, st = np.where(along_x, sx, sy), np.where(along_x, sy, sx)
-    nm, nt = np.where(along_x, cfg.nx, cfg.ny), np.where(along_x, cfg.ny, cfg.nx)
-    slope = gt / gm
-    t0 = st - sm * slope
-    with np.errstate(divide="ignore", invalid="ignore"):
-        m0, m1 = (0.0 - t0) / slope, (nt - t0) / slope
-    lo = np.where(slope != 0, np.minimum(m0, m1), 0.0)
-    hi = np.where(slope != 0, np.maximum(m0, m1), nm.astype(float))
-    lo, hi = np.clip(lo, 0, nm), np.clip(hi, 0, nm)
-    n = np.maximum(np.ceil(hi) - np.floor(lo), 0)
-    return int(n.sum()) * cfg.nv
+def moved_bytes(cfg, field_storage, tiles_loaded, vox_per_tile):
+    """What one launch really had to move, from the tiles the timed launches loaded (counted inside the
+    kernels, pcamm_tile_counts; reading B8: tiles that can only see zeros / constant cells are skipped).
+    A loaded tile costs its fields and its f0 gathers (4 B per voxel, counted once); the warp kernel
+    writes every voxel of the volume (skipped tiles as zeros), the gradient kernel reads the residual."""
+    fields = field_bytes_per_voxel(cfg, field_storage)
+    return {"warp": tiles_loaded["warp"] * vox_per_tile * (fields + 4) + 4 * cfg.V,
+            "gradient": tiles_loaded["gradient"] * vox_per_tile * (fields + 4) + 4 * cfg.npix}
 
 
 def measured_peak_gbs():
@@ -224,16 +198,26 @@ def run_reference(args, cfg, rank, world):
     secs, nthr = time_oracle_solves(wl, gts, cyc, it)
     timed = secs[args.warmup:]
     ms = 1e3 * float(np.mean(timed))
+    fan = 1 if cfg.batched_linesearch else int(args.fan)
     line = {"impl": "reference", "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_median": 1e3 * float(np.median(timed)),
+            "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_dict(cfg, it),
+            "config": full_config(cfg, it, fan, args.field_storage, max(int(args.in_flight), 1)),
             "cpu_baseline": {"value": ms, "unit": "ms", "cores": nthr, "kind": "oracle",
                              "sample": f"full {it}-iteration oracle solves, {n_distinct} distinct projections "
                                        f"cycled over {n} steps, OpenMP on {nthr} threads"},
             "e2e": {"value": ms, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def full_config(cfg, iterations, fan, field_storage, in_flight):
+    """The config object of the bench line (identical in both arms)."""
+    return dict(config_dict(cfg, iterations, fan, field_storage), in_flight=in_flight,
+                field_storage="float32" if field_storage == 0 else
+                "u_k stored as float16 with a power-of-two scale per field, x-bar float32, arithmetic float32 "
+                "(SURVEY 8(f).4; NOT the headline configuration)")
 
 
 def config_dict(cfg, iterations, fan=1, field_storage=0):
@@ -244,7 +228,8 @@ def config_dict(cfg, iterations, fan=1, field_storage=0):
             "iterations": iterations, "warm_start": "previous frame's w (PAPER.md:L141)",
             "line_search": "Armijo backtracking, all 8 candidate steps per pass" if cfg.batched_linesearch else
                            ("sequential Armijo backtracking" if fan <= 1 else
-                            f"Armijo backtracking, {fan} candidate steps per pass (same accepted step as sequential)"),
+                            f"Armijo backtracking, {fan} candidate steps evaluated per pass: the accepted steps are those of "
+                            "sequential backtracking, bit for bit (DESIGN.md reading B7)"),
             "l2": "inputs larger than L2: every pass streams the (K+1) vector fields "
                   f"({(12 * (cfg.K + 1) if field_storage == 0 else 12 + 6 * cfg.K) * cfg.V / 2**20:.0f} MiB) through a 126 MB L2",
             "parallelism": "replicas"}
@@ -305,25 +290,29 @@ def run_ours(args, cfg, rank, local_rank, world):
         w_zero = np.zeros((B, cfg.K), np.float32)
 
     tumour_mm = {}          # frame index in the block -> localised tumour position (device-resident pass)
+    step_events = []        # one CUDA event behind every step of the device-resident pass
 
-    def run_block(first, count, w, host):
-        if B > 1:
-            for i in range(first, first + count):
+    def run_block(first, count, w, host, events=None):
+        for i in range(first, first + count):
+            if B > 1:
                 j = i % n_distinct
                 if host:
                     stage.copy_(yb_host[j], non_blocking=True)
                     r = m.reconstruct_batch(stage, ab[j], w_zero, opts)[-1]
                 else:
                     r = m.reconstruct_batch(yb_dev[j], ab[j], w_zero, opts)[-1]
-            return w, r
-        for i in range(first, first + count):
-            if host:
+            elif host:
                 r = m.reconstruct(ys_host[i].numpy(), angles[i], w, opts, host_y=True)
+                w = r.w
             else:
                 r = m.reconstruct(ys_dev[i], angles[i], w, opts)
                 if r.landmarks is not None and len(r.landmarks):
                     tumour_mm[i] = np.array(r.landmarks[0], np.float64)
-            w = r.w
+                w = r.w
+            if events is not None:
+                ev = torch.cuda.Event(enable_timing=True)
+                ev.record()
+                events.append(ev)
         return w, r
 
     # ---- device-resident timing: y already in HBM
@@ -336,9 +325,11 @@ def run_ours(args, cfg, rank, local_rank, world):
     pc.launch_count(reset=True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    w, last = run_block(args.warmup, args.steps, w, host=False)
+    w, last = run_block(args.warmup, args.steps, w, host=False, events=step_events)
     e1.record()
     torch.cuda.synchronize()
+    marks = [e0] + step_events
+    step_ms = [marks[i].elapsed_time(marks[i + 1]) for i in range(len(step_events))]
     launches = pc.launch_count(reset=True)
     replicas.barrier(dist)
     clocks = sampler.stop() if sampler else None
@@ -366,55 +357,84 @@ def run_ours(args, cfg, rank, local_rank, world):
     tr = m.reconstruct(ys_dev[i_last], angles[i_last], w_after_warmup if B == 1 else np.zeros(cfg.K, np.float32),
                        opts, trace=True)
     width = 8 if cfg.batched_linesearch else max(fan, 1)
-    # candidate steps evaluated (every pass evaluates `width` of them, or what is left of the budget of 8)
+    # line-search passes (each one warp + one projection launch over `width` candidates), candidates evaluated
+    passes = int(np.sum(tr.backtracks // width + 1)) if tr.backtracks is not None else it
     trials = int(np.sum(np.minimum(width * (tr.backtracks // width + 1), 8))) if tr.backtracks is not None else it
     m.eval(ys_dev[i_last], angles[i_last], tr.w, tr.a, tr.b, want_proj=False)
+    # the warp and projection kernels are timed over as many candidate steps as a line-search pass
+    # evaluates (nearby coefficient vectors: the candidates of a pass differ by one step)
+    m.time_slots(np.stack([tr.w * (1.0 + 0.02 * c) for c in range(width)]))
     for which in (0, 1, 2):
         m.time_kernel(which, 3)
-    kt = {name: m.time_kernel(which, 20) for which, name in ((0, "warp"), (1, "project"), (2, "gradient"))}
-    nl = {"warp": trials + 1, "project": trials + 1, "gradient": tr.iters}
+    REPS = 20
+    kt, tiles_loaded = {}, {}
+    for which, name in ((0, "warp"), (1, "project"), (2, "gradient")):
+        m.tile_counts(reset=True)
+        kt[name] = m.time_kernel(which, REPS)
+        tc = m.tile_counts(reset=True)               # tiles the timed launches loaded, counted in the kernels
+        tiles_loaded[name] = tc[0 if which == 0 else 1] / REPS
+    n_tiles, vox_per_tile = tc[2], tc[3]
+    nl = {"warp": passes + 1, "project": passes + 1, "gradient": tr.iters}
     ab = algorithmic_bytes(cfg, args.field_storage)
     peak, peak_src = measured_peak_gbs()
-    traffic = measured_traffic().get(cfg.name if args.field_storage == 0 else cfg.name + "_half_u", {})
-    per_kernel = {k: {"bound": "hbm", "ms": kt[k], "launches_per_solve": nl[k], "algorithmic_bytes": ab[k],
-                      "achieved": ab[k] / (kt[k] * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                      "frac": ab[k] / (kt[k] * 1e-3) / 1e9 / peak, "traffic": traffic.get(k)}
-                  for k in kt}
-    for k in per_kernel:        # what the launch really moved (ncu, profiles/), against the same peak
-        if per_kernel[k]["traffic"]:
-            per_kernel[k]["traffic_gbs"] = per_kernel[k]["traffic"] / (kt[k] * 1e-3) / 1e9
-            per_kernel[k]["traffic_frac"] = per_kernel[k]["traffic_gbs"] / peak
-    # the projector against the SMs' fp32 lane-operation rate as well (it is not an HBM kernel)
-    n_rs = ray_slab_count(cfg, angles[i_last])
-    ops = PROJECT_OPS_PER_RAY_SLAB * n_rs
-    per_kernel["project"].update({"hbm_gbs": per_kernel["project"]["achieved"], "hbm_frac": per_kernel["project"]["frac"],
-                                  "bound": "alu", "ray_slabs": n_rs, "algorithmic_ops": ops,
-                                  "achieved": ops / (kt["project"] * 1e-3) / 1e12, "peak": ALU_PEAK_TOPS,
-                                  "unit": "Tlane-op/s", "frac": ops / (kt["project"] * 1e-3) / 1e12 / ALU_PEAK_TOPS,
-                                  "ray_slabs_per_s": n_rs / (kt["project"] * 1e-3)})
+    # per launch over `width` candidates: the fields once, the f0 gathers, the volume and the projection per candidate
+    ab["warp"] += (width - 1) * 8 * cfg.V
+    ab["project"] *= width
+    if n_tiles:
+        mv = moved_bytes(cfg, args.field_storage, tiles_loaded, vox_per_tile)
+        mv["warp"] += (width - 1) * (tiles_loaded["warp"] * vox_per_tile * 4 + 4 * cfg.V)
+    else:                                            # generic kernels (shapes TMA cannot describe): every tile
+        mv = {"warp": ab["warp"], "gradient": ab["gradient"]}
+    mv["project"] = ab["project"]
+    per_kernel = {}
+    for k in kt:
+        sec = kt[k] * 1e-3
+        per_kernel[k] = {"bound": "hbm", "ms": kt[k], "launches_per_solve": nl[k],
+                         "candidates_per_launch": 1 if k == "gradient" else width,
+                         "moved_bytes": mv[k], "achieved": mv[k] / sec / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": mv[k] / sec / 1e9 / peak,
+                         "dense_algorithmic_bytes": ab[k], "speedup_vs_dense_bytes": ab[k] / sec / 1e9 / peak}
+        if k != "project" and n_tiles:
+            per_kernel[k]["tiles_loaded_per_launch"] = tiles_loaded[k]
+            per_kernel[k]["tiles_total"] = n_tiles
+    # the projector's volume was just written and is L2-resident: it is not an HBM kernel.
+    # What it does per launch: one pass over (detector column, slab, level) and one look-up per z crossing.
+    per_kernel["project"].update({
+        "note": "L2-resident input: bound by issue and shared-memory latency, not by HBM (DESIGN.md section 5a); "
+                "frac = SURVEY 8(d) bytes (4 V + 4 Npix) / time / HBM peak, as BASELINE.json asks",
+        "rays_per_s": width * cfg.npix / (kt["project"] * 1e-3)})
     dom = max(kt, key=lambda k: kt[k] * nl[k])
-    wp_gbs = (ab["warp"] + ab["project"]) / ((kt["warp"] + kt["project"]) * 1e-3) / 1e9
+    wp_gbs = (mv["warp"] + mv["project"]) / ((kt["warp"] + kt["project"]) * 1e-3) / 1e9
     d = per_kernel[dom]
     roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],
-                "frac": d["frac"], "traffic": d["traffic"],
-                "note": "achieved = SURVEY 8(a) algorithmic bytes (every voxel's fields counted) / launch time; the warp and "
-                        "gradient kernels skip, exactly, the tiles whose stencils can only see zeros / constant cells of f0 "
-                        "(DESIGN.md reading B8), so they move fewer bytes than that (traffic, traffic_frac) and frac may exceed 1",
-                "peak_source": peak_src if d["bound"] == "hbm" else
-                "148 SMs x 128 fp32 lanes x 1.965 GHz (B200_PROFILING.md unit counts and clocks; DESIGN.md section 6)",
+                "frac": d["frac"], "traffic": None,
+                "note": "achieved = bytes the launch had to move / CUDA-event time of the launch (pcamm_time_kernel, on the "
+                        "launching stream): fields and f0 of the tiles the kernel loaded (counted in the kernel for the same "
+                        "launches), the volume written, the residual read.  speedup_vs_dense_bytes puts SURVEY 8(a)'s dense "
+                        "bytes (every voxel's fields) over the same time: the kernels skip, exactly, tiles that can only "
+                        "see zeros / constant cells of f0 (DESIGN.md reading B8).  traffic (ncu DRAM bytes): profiles/",
+                "peak_source": peak_src,
                 "per_kernel": per_kernel,
-                "warp_plus_project": {"gbs": wp_gbs, "frac": wp_gbs / peak,
-                                      "frac_of_nominal_8000": wp_gbs / 8000.0},
+                "warp_plus_project": {"gbs": wp_gbs, "frac": wp_gbs / peak, "frac_of_nominal_8000": wp_gbs / 8000.0,
+                                      "dense_gbs": (ab["warp"] + ab["project"]) / ((kt["warp"] + kt["project"]) * 1e-3) / 1e9},
                 "kernel_share_of_step": {k: kt[k] * nl[k] / (elapsed_ms / args.steps / B) for k in kt}}
 
-    # ---- the oracle on this box's host cores, one full solve of the same workload
+    # ---- the oracle on this box's host cores (a baseline, not the target): one full solve of the same
+    #      workload on all cores, and a short one on a single core
     cpu = None
     if not args.no_cpu_baseline:
-        tc = time.perf_counter()
+        tc0 = time.perf_counter()
         secs, nthr = time_oracle_solves(wl, gts, [ids[args.warmup]], it)
         cpu = {"value": 1e3 * secs[0], "unit": "ms", "cores": nthr, "kind": "oracle",
                "sample": f"1 projection (frame {ids[args.warmup]}), full {it}-iteration solve from w = 0, "
-                         f"OpenMP on {nthr} threads; {time.perf_counter() - tc:.0f} s including its simulated y"}
+                         f"OpenMP on {nthr} threads; {time.perf_counter() - tc0:.0f} s including its simulated y"}
+        it1 = min(it, args.cpu_single_iters)
+        if it1 > 0:
+            secs1, _ = time_oracle_solves(wl, gts, [ids[args.warmup]], it1, threads=1)
+            cpu["single_thread"] = {"value": 1e3 * secs1[0], "unit": "ms", "cores": 1, "iterations": it1,
+                                    "ms_per_iteration": 1e3 * secs1[0] / it1,
+                                    "sample": f"the same projection, {it1}-iteration solve from w = 0 on one thread "
+                                              f"(bounded: a full {it}-iteration solve takes about {it / it1:.0f}x as long)"}
 
     # ---- accuracy context (PAPER.md:L119 3D localisation error; not a parity value): the tumour
     #      position of every timed solve against the fixed point of the analytic test DVF
@@ -428,17 +448,16 @@ def run_ours(args, cfg, rank, local_rank, world):
                         "n": len(errs), "note": "synthetic phantom, context only (the paper reports 0.8 +- 0.5 mm on NCAT, L135)"}
 
     line = {"metric": METRIC, "value": ms_per_solve, "unit": "ms", "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": False,
+            "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps,
+            "ms_per_step_median": float(np.median(step_ms)) if step_ms else None, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": dict(config_dict(cfg, it, fan, args.field_storage), in_flight=B,
-                           field_storage="float32" if args.field_storage == 0 else
-                           "u_k stored as float16 with a power-of-two scale per field, x-bar float32, arithmetic float32 "
-                           "(SURVEY 8(f).4; NOT the headline configuration)"), "projections_per_s": 1e3 * args.steps * world * B / elapsed_ms,
+            "config": full_config(cfg, it, fan, args.field_storage, B), "projections_per_s": 1e3 * args.steps * world * B / elapsed_ms,
             "clocks": clocks,
             "e2e": {"value": e2e_ms / (args.steps * world * B), "unit": "ms", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-            "last_solve": {"iters": tr.iters, "trials": trials, "status": tr.status, "J0": tr.J0, "J": tr.J},
+            "last_solve": {"iters": tr.iters, "line_search_passes": passes, "candidates_evaluated": trials,
+                           "status": tr.status, "J0": tr.J0, "J": tr.J},
             "accuracy": accuracy,
             "context": {"paper_ms_per_projection_tesla_c1060": 240.0}}
     print(json.dumps(line), flush=True)
@@ -619,13 +638,15 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--fan", type=int, default=1,
+    ap.add_argument("--fan", type=int, default=2,
                     help="candidate steps evaluated per line-search pass (pcamm_opts.batched_linesearch): the "
-                         "accepted step is the same for every width; 1 = sequential backtracking")
+                         "accepted step is the same for every width, bit for bit; 1 = sequential backtracking")
+    ap.add_argument("--cpu-single-iters", type=int, default=1,
+                    help="iterations of the single-thread oracle leg (0: skip it)")
     ap.add_argument("--in-flight", type=int, default=1,
                     help="B > 1: every step advances B independent projection solves in lock step "
                          "(pcamm_reconstruct_batch; BASELINE.json configs[4] sweeps 1, 4, 16, 64), each from w = 0")

@@ -259,6 +259,12 @@ int pcamm_localise(pcamm_model* model, const float* w_host, int32_t inv_max_iter
  * which: 0 = warp (a-1), 1 = project (a-2), 2 = gradient (a-4). */
 int pcamm_time_kernel(pcamm_model* model, int32_t which, int32_t reps, float* ms_out, void* stream);
 
+/* For pcamm_time_kernel: makes the first nslots (<= max_batch * max_candidates) trial slots active
+ * with the coefficients w_host [nslots][K], so that the warp and projection kernels are timed over
+ * as many candidate steps per launch as the solve evaluates per line-search pass.  Call it after
+ * pcamm_eval (which leaves one slot active and resets this to 1). */
+int pcamm_time_slots(pcamm_model* model, int32_t nslots, const float* w_host, void* stream);
+
 /* What the two streaming kernels really loaded (reading B8: tiles whose stencils can only see zeros
  * of f0 / constant cells are skipped, exactly).  out[0], out[1] = field tiles loaded by the warp and
  * by the gradient kernel in all launches since the counters were last reset (one tile = out[3]

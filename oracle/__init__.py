@@ -115,6 +115,19 @@ def max_threads() -> int:
     return int(lib().orc_max_threads())
 
 
+SIDDON, RAY_MARCHING = 0, 1
+
+
+def set_projector(kind: int, step_mm: float = 1.0) -> None:
+    """Which discretisation of P project / backproject / gradient / solve use from now on: SIDDON (reading
+    A3, the default) or RAY_MARCHING with the nominal step `step_mm` (reading C1)."""
+    lib().orc_set_projector(int(kind), C.c_double(float(step_mm)))
+
+
+def get_projector() -> int:
+    return int(lib().orc_get_projector())
+
+
 def _f32(a):
     a = np.ascontiguousarray(a)
     assert a.dtype == np.float32, "oracle inputs are the float32 arrays the GPU path consumes"

@@ -15,7 +15,9 @@
 // Pins (tests/test_oracle_*.py): brute-force ray/box intersection, chord closed
 // forms, adjoint dot-product, identity / integer-shift / affine-ramp warps,
 // finite differences of J, exact intensity fits, planted coefficients, closed-
-// form DVF inversion.  No function here is "parity unpinned".
+// form DVF inversion; for the ray-marching variant of P (reading C1): uniform and
+// affine volumes in closed form, a dense matrix built separately, the adjoint
+// identity, finite differences of J.  No function here is "parity unpinned".
 //
 // Inputs are the float32 arrays the GPU path consumes, up-cast to double.
 #include <algorithm>
@@ -58,6 +60,15 @@ struct OrcResult {
 
 static int g_threads = 1;
 void orc_set_threads(int n) { g_threads = n < 1 ? 1 : n; }
+
+// Which discretisation of P the projector, the backprojector and everything built on them use
+// (PAPER.md:L82 says only "projection matrix"): 0 = Siddon's exact radiological path (reading A3,
+// the default), 1 = fixed-step trilinear ray marching (reading C1 below) with
+// the nominal step step_mm.
+static int g_projector = 0;
+static double g_step_mm = 1.0;
+void orc_set_projector(int kind, double step_mm) { g_projector = kind == 1 ? 1 : 0; if (step_mm > 0) g_step_mm = step_mm; }
+int orc_get_projector() { return g_projector; }
 int orc_get_threads() { return g_threads; }
 int orc_max_threads() {
 #ifdef _OPENMP
@@ -233,6 +244,63 @@ void dvf_at_point(const OrcGeom& g, const float* xbar, const float* u, const dou
             }
 }
 
+// ---- fixed-step trilinear ray marching (north_star "fixed-step or Siddon
+// traversal"; PAPER.md:L82 leaves the discretisation of P open).  Reading C1:
+//
+//   p_i = d_i sum_{m = 0}^{M_i - 1} (T f)(E_i + (m + 1/2) d_i e_i)
+//
+// where [E_i, X_i] is the part of the ray source -> pixel centre i inside the box spanned by the
+// voxel CENTRES (where trilinear interpolation T f of the voxel-centre values is defined without
+// any padding rule), L_i its length, e_i the unit direction, M_i = ceil(L_i / step) and
+// d_i = L_i / M_i <= step: the midpoint rule on M_i equal steps.  A ray that misses the box, or an
+// axis with a single voxel layer (a box of no thickness), gives 0.
+//
+// The matrix entries are l_ij = d_i sum_m (weight of voxel j in T at sample m); both P and P^T walk
+// the same samples through this one enumerator, so P^T is the exact transpose.
+// fn(lin, weight): called for each of the 8 taps of each sample, weight = d_i * trilinear weight.
+template <class Fn>
+void rm_samples(const OrcGeom& g, const Ray& r, double step_mm, Fn fn) {
+    const int N[3] = {g.nx, g.ny, g.nz};
+    const double h[3] = {g.hx, g.hy, g.hz};
+    const double ctr[3] = {g.cx, g.cy, g.cz};
+    double lo[3], amin = 0.0, amax = 1.0;
+    for (int c = 0; c < 3; ++c) {
+        if (N[c] < 2) return;
+        lo[c] = ctr[c] - (N[c] - 1) / 2.0 * h[c];                        // centre of voxel 0
+        const double hi = ctr[c] + (N[c] - 1) / 2.0 * h[c];              // centre of voxel N - 1
+        if (std::fabs(r.d[c]) < 1e-12 * r.L) {
+            if (r.S[c] < lo[c] || r.S[c] > hi) return;
+            continue;
+        }
+        const double a0 = (lo[c] - r.S[c]) / r.d[c], a1 = (hi - r.S[c]) / r.d[c];
+        amin = std::max(amin, std::min(a0, a1));
+        amax = std::min(amax, std::max(a0, a1));
+    }
+    if (!(amin < amax)) return;
+    const double L = (amax - amin) * r.L;
+    const int64_t M = (int64_t)std::ceil(L / step_mm);
+    if (M < 1) return;
+    const double d = L / (double)M, da = (amax - amin) / (double)M;
+    for (int64_t m = 0; m < M; ++m) {
+        const double al = amin + ((double)m + 0.5) * da;
+        int64_t i0[3];
+        double t[3];
+        for (int c = 0; c < 3; ++c) {
+            const double q = (r.S[c] + al * r.d[c] - lo[c]) / h[c];      // index coordinates, in [0, N - 1]
+            int64_t f = (int64_t)std::floor(q);
+            f = std::min<int64_t>(std::max<int64_t>(f, 0), N[c] - 2);
+            i0[c] = f;
+            t[c] = q - (double)f;
+        }
+        for (int a = 0; a < 2; ++a)
+            for (int b = 0; b < 2; ++b)
+                for (int cc = 0; cc < 2; ++cc) {
+                    const double wgt = (a ? t[0] : 1.0 - t[0]) * (b ? t[1] : 1.0 - t[1]) * (cc ? t[2] : 1.0 - t[2]);
+                    fn(((i0[2] + cc) * g.ny + (i0[1] + b)) * g.nx + (i0[0] + a), d * wgt);
+                }
+    }
+}
+
 }  // namespace
 
 extern "C" {
@@ -290,6 +358,16 @@ int orc_traverse(const OrcGeom* g, double theta, int iu, int iv, int cap, int32_
 // p = P_theta f: p_i = sum_j l_ij f_j (Eq. 2; reading A3).
 void orc_project(const OrcGeom* g, const double* f, double theta, double* p_out) {
     const OrcGeom& G = *g;
+    if (g_projector == 1) {                            // reading C1: p_i = sum_j l_ij f_j with the ray-marching l_ij
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+        for (int64_t pix = 0; pix < npix(G); ++pix) {
+            double s = 0.0;
+            rm_samples(G, make_ray(G, theta, (int)(pix % G.nu), (int)(pix / G.nu)), g_step_mm,
+                       [&](int64_t lin, double wgt) { s += wgt * f[lin]; });
+            p_out[pix] = s;
+        }
+        return;
+    }
 #pragma omp parallel num_threads(g_threads)
     {
         std::vector<Seg> segs;
@@ -321,6 +399,12 @@ void orc_backproject(const OrcGeom* g, const double* r, double theta, double* B_
         std::vector<Seg> segs;
 #pragma omp for schedule(static)
         for (int64_t pix = 0; pix < npix(G); ++pix) {
+            if (g_projector == 1) {                    // reading C1: the transpose of the same ray-marching l_ij
+                const double ri = r[pix];
+                rm_samples(G, make_ray(G, theta, (int)(pix % G.nu), (int)(pix / G.nu)), g_step_mm,
+                           [&](int64_t lin, double wgt) { acc[lin] += wgt * ri; });
+                continue;
+            }
             siddon(G, make_ray(G, theta, (int)(pix % G.nu), (int)(pix / G.nu)), segs, nullptr);
             for (const Seg& sg : segs) acc[((int64_t)sg.k * G.ny + sg.j) * G.nx + sg.i] += sg.len * r[pix];
         }

@@ -52,7 +52,7 @@ class pcamm_info(C.Structure):
 SYMBOLS = ("pcamm_default_opts", "pcamm_model_create", "pcamm_model_destroy", "pcamm_model_fields",
            "pcamm_reconstruct",
            "pcamm_reconstruct_host", "pcamm_reconstruct_batch", "pcamm_warp", "pcamm_project",
-           "pcamm_backproject", "pcamm_eval", "pcamm_traverse", "pcamm_localise", "pcamm_time_kernel",
+           "pcamm_backproject", "pcamm_eval", "pcamm_traverse", "pcamm_localise", "pcamm_time_kernel", "pcamm_time_slots",
            "pcamm_tune", "pcamm_tile_counts", "pcamm_timeline", "pcamm_launch_count", "pcamm_last_error", "pcamm_pca_fit", "pcamm_predict_w", "pcamm_frames_create",
            "pcamm_frames_destroy", "pcamm_frames_reset", "pcamm_frames_count", "pcamm_frames_predict",
            "pcamm_frames_push")
@@ -350,6 +350,11 @@ class Model:
         out = (C.c_int64 * 4)()
         _check(lib().pcamm_tile_counts(self._h, 1 if reset else 0, out, _stream()))
         return tuple(int(v) for v in out)
+
+    def time_slots(self, w) -> None:
+        """pcamm_time_slots: the candidate coefficient vectors [n][K] the warp / projection timings run over."""
+        w = np.ascontiguousarray(w, np.float32).reshape(-1, self.K)
+        _check(lib().pcamm_time_slots(self._h, int(w.shape[0]), w.ctypes.data_as(C.c_void_p), _stream()))
 
     def time_kernel(self, which: int, reps: int = 20) -> float:
         """Average device milliseconds per launch of kernel 0 warp / 1 project / 2 gradient on the

@@ -163,6 +163,7 @@ struct pcamm_model {
     unsigned long long* nonfinite = nullptr;
     unsigned long long* visited = nullptr;   // FieldStream::visited
     Timeline* tl = nullptr;                  // kernel timeline of the last solve (timeline knob), else NULL
+    int time_slots = 1;                      // trial slots pcamm_time_kernel launches over (pcamm_time_slots)
     float* y_stage = nullptr;   // device copy of a host-side measured projection (pcamm_reconstruct_host)
     // pinned host staging
     char* h_in = nullptr;
@@ -822,6 +823,7 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     Seq q2;
     int rc = hook_begin(m, y_dev, angle_rad, w_host, a, b, 1, st, q2);
     if (rc) return rc;
+    m->time_slots = 1;
     launch_ysums(q2, G, m->c, 1);
     launch_view_tables(q2, G, m->c.solves, 1, m->col_hdr, m->slab_tab);
     launch_warp(q2, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
@@ -932,6 +934,22 @@ int pcamm_tune(const char* name, int32_t value) {
     return invalid("unknown knob: " + n);
 }
 
+int pcamm_time_slots(pcamm_model* m, int32_t nslots, const float* w_host, void* stream) {
+    if (!m || !w_host) return invalid("NULL argument");
+    if (nslots < 1 || nslots > m->S) return invalid("nslots outside [1, max_batch * max_candidates]");
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<SlotState> h((size_t)nslots);
+    for (int s = 0; s < nslots; ++s) {
+        std::memset(&h[s], 0, sizeof(SlotState));
+        for (int k = 0; k < m->G.K; ++k) h[s].w[k] = w_host[s * m->G.K + k];
+        h[s].active = 1; h[s].solve = 0;
+    }
+    CUDA_TRY(cudaMemcpyAsync(m->c.slots, h.data(), sizeof(SlotState) * nslots, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    m->time_slots = nslots;
+    return PCAMM_OK;
+}
+
 int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out, void* stream) {
     if (!m || !ms_out || reps < 1 || which < 0 || which > 2) return invalid("invalid argument");
     cudaStream_t st = (cudaStream_t)stream;
@@ -941,9 +959,9 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
     CUDA_TRY(cudaEventRecord(m->ev0, st));
     for (int i = 0; i < reps; ++i) {
         if (which == 0)
-            launch_warp(q, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
+            launch_warp(q, G, m->fs, m->f0p, m->c.slots, m->time_slots, 1, m->vol, G.PV, m->occ);
         else if (which == 1)
-            launch_project(q, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0, 0);
+            launch_project(q, G, m->c, m->time_slots, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0, 0);
         else
             launch_grad(q, G, m->fs, m->f0p, m->c, 1, m->rL, m->utab, m->vtab, GRAD_NONE);
     }

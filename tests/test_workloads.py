@@ -138,14 +138,20 @@ def test_noise_models():
     assert np.all(np.isfinite(p)) and abs(np.mean(p[:, :10] - y[:, :10])) < 0.01
 
 
-def test_bench_ray_slab_count_matches_the_geometry():
-    """bench.py's count of (ray, slab) pairs (the projector's ALU roofline numerator): along an axis
-    every column marches all layers; at 45 degrees the diagonal of the square field of view."""
+def test_bench_moved_bytes_model():
+    """bench.py's bytes-moved model (the roofline numerators): with every tile loaded it equals SURVEY 8(a)'s
+    dense algorithmic bytes, and a skipped tile saves its fields and its f0 gathers but not the warp
+    kernel's store."""
     import bench
     cfg = get_config("C2")
-    assert bench.ray_slab_count(cfg, 0.0) == cfg.nu * cfg.nv * cfg.nx
-    assert bench.ray_slab_count(cfg, np.pi / 2) == cfg.nu * cfg.nv * cfg.ny
-    n45 = bench.ray_slab_count(cfg, np.pi / 4)
-    assert 0.6 * cfg.nu * cfg.nv * cfg.nx < n45 < cfg.nu * cfg.nv * cfg.nx
-    ab = bench.algorithmic_bytes(cfg)
-    assert ab["warp"] == 56 * cfg.V and ab["gradient"] == 52 * cfg.V + 4 * cfg.npix     # SURVEY 8(a), K = 3
+    vox = 32 * 32
+    n_tiles = cfg.V // vox
+    dense = bench.algorithmic_bytes(cfg)
+    full = bench.moved_bytes(cfg, 0, {"warp": n_tiles, "gradient": n_tiles}, vox)
+    assert full["warp"] == dense["warp"] == 56 * cfg.V
+    assert full["gradient"] == dense["gradient"] == 52 * cfg.V + 4 * cfg.npix
+    half = bench.moved_bytes(cfg, 0, {"warp": n_tiles // 2, "gradient": n_tiles // 2}, vox)
+    assert half["warp"] == 26 * cfg.V + 4 * cfg.V and half["gradient"] == 26 * cfg.V + 4 * cfg.npix
+    assert bench.moved_bytes(cfg, 1, {"warp": n_tiles, "gradient": n_tiles}, vox)["warp"] == (12 + 18 + 8) * cfg.V
+
+

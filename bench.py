@@ -195,6 +195,9 @@ def run_reference(args, cfg, rank, world):
     gts = ground_truth_volumes(wl, ids[:n_distinct])
     it = solver_iterations(cfg)
     cyc = [ids[i % n_distinct] for i in range(n)]
+    if args.projector == 1:
+        import oracle
+        oracle.set_projector(oracle.RAY_MARCHING, (args.ray_step_vox or 0.5) * min(cfg.hx, cfg.hy, cfg.hz))
     secs, nthr = time_oracle_solves(wl, gts, cyc, it)
     timed = secs[args.warmup:]
     ms = 1e3 * float(np.mean(timed))
@@ -203,13 +206,22 @@ def run_reference(args, cfg, rank, world):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_median": 1e3 * float(np.median(timed)),
             "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": full_config(cfg, it, fan, args.field_storage, max(int(args.in_flight), 1)),
+            "config": dict(full_config(cfg, it, fan, args.field_storage, max(int(args.in_flight), 1)), **projector_config(args)),
             "cpu_baseline": {"value": ms, "unit": "ms", "cores": nthr, "kind": "oracle",
                              "sample": f"full {it}-iteration oracle solves, {n_distinct} distinct projections "
                                        f"cycled over {n} steps, OpenMP on {nthr} threads"},
             "e2e": {"value": ms, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def projector_config(args):
+    """Extra config key of the runs that use the ray-marching variant of P: none for the
+    headline configuration (Siddon)."""
+    if args.projector == 0:
+        return {}
+    return {"projector": f"fixed-step trilinear ray marching, nominal step {args.ray_step_vox or 0.5} x the smallest voxel "
+                         "edge (DESIGN.md reading C1; NOT the headline configuration, which is Siddon's exact path)"}
 
 
 def full_config(cfg, iterations, fan, field_storage, in_flight):
@@ -267,7 +279,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     m = pc.Model(nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, hx=cfg.hx, hy=cfg.hy, hz=cfg.hz, K=cfg.K, nu=cfg.nu, nv=cfg.nv,
                  pu=cfg.pu, pv=cfg.pv, f0=t(wl.f0), mean_dvf=t(wl.model.mean), eig_dvf=t(wl.model.eig),
                  landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=C, max_batch=B,
-                 field_storage=args.field_storage)
+                 field_storage=args.field_storage, projector=args.projector, ray_step_vox=args.ray_step_vox)
     # measured projections: the scanner is simulated with the library's own projector applied to
     # the ground-truth volume, plus seeded noise (the CPU arm simulates its own with the oracle)
     ys_host, ys_dev = [], []
@@ -424,6 +436,9 @@ def run_ours(args, cfg, rank, local_rank, world):
     cpu = None
     if not args.no_cpu_baseline:
         tc0 = time.perf_counter()
+        if args.projector == 1:
+            import oracle
+            oracle.set_projector(oracle.RAY_MARCHING, (args.ray_step_vox or 0.5) * min(cfg.hx, cfg.hy, cfg.hz))
         secs, nthr = time_oracle_solves(wl, gts, [ids[args.warmup]], it)
         cpu = {"value": 1e3 * secs[0], "unit": "ms", "cores": nthr, "kind": "oracle",
                "sample": f"1 projection (frame {ids[args.warmup]}), full {it}-iteration solve from w = 0, "
@@ -451,7 +466,8 @@ def run_ours(args, cfg, rank, local_rank, world):
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps,
             "ms_per_step_median": float(np.median(step_ms)) if step_ms else None, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": full_config(cfg, it, fan, args.field_storage, B), "projections_per_s": 1e3 * args.steps * world * B / elapsed_ms,
+            "config": dict(full_config(cfg, it, fan, args.field_storage, B), **projector_config(args)),
+            "projections_per_s": 1e3 * args.steps * world * B / elapsed_ms,
             "clocks": clocks,
             "e2e": {"value": e2e_ms / (args.steps * world * B), "unit": "ms", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h},
@@ -663,6 +679,10 @@ def main():
                          "two passes against their algorithmic bytes)")
     ap.add_argument("--tune", action="append", default=[], metavar="NAME=VALUE",
                     help="pcamm_tune measurement knob, set before the model is created (repeatable)")
+    ap.add_argument("--projector", type=int, default=0, choices=[0, 1],
+                    help="pcamm_geometry.projector: 0 Siddon's exact path (the headline configuration), 1 fixed-step "
+                         "trilinear ray marching (SURVEY 8(f) row 1)")
+    ap.add_argument("--ray-step-vox", type=float, default=0.0, help="projector 1: nominal step in voxels (0 = 0.5)")
     ap.add_argument("--timeline", action="store_true",
                     help="instead of the bench line: the kernel timeline of one solve, recorded inside the kernels")
     ap.add_argument("--timeline-out", default=None, help="with --timeline: write the event list to this text file")

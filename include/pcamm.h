@@ -78,6 +78,14 @@ typedef struct {
                                see zeros / constant cells of f0 (reading B8): 0 (default) where the
                                volume has tiles enough per SM to win back the flags' set-up (a few dependent
                                loads per launch), 1 always, 2 never */
+    int32_t projector;      /* discretisation of P (PAPER.md:L82 says only "projection matrix"): 0 (default)
+                               Siddon's exact radiological path (reading A3); 1 fixed-step trilinear ray
+                               marching (reading C1): p_i = d_i sum_m (T f)(sample m), the
+                               midpoint rule on M_i = ceil(L_i / step) equal steps d_i = L_i / M_i over the part
+                               of the ray inside the box spanned by the voxel centres, T f the trilinear
+                               interpolant; P^T is the exact transpose (scattered with atomic adds: results
+                               reproducible to rounding, not bitwise).  pcamm_traverse needs projector 0 */
+    float ray_step_vox;     /* projector 1: nominal step in units of the smallest voxel edge; 0 = default 0.5 */
 } pcamm_geometry;
 
 typedef struct {

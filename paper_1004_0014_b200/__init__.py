@@ -31,7 +31,8 @@ class pcamm_geometry(C.Structure):
                 ("K", C.c_int32), ("nu", C.c_int32), ("nv", C.c_int32),
                 ("pu", C.c_float), ("pv", C.c_float), ("sad", C.c_float), ("sdd", C.c_float),
                 ("off_u", C.c_float), ("off_v", C.c_float),
-                ("max_batch", C.c_int32), ("max_candidates", C.c_int32), ("field_storage", C.c_int32), ("tile_skipping", C.c_int32)]
+                ("max_batch", C.c_int32), ("max_candidates", C.c_int32), ("field_storage", C.c_int32), ("tile_skipping", C.c_int32),
+                ("projector", C.c_int32), ("ray_step_vox", C.c_float)]
 
 
 class pcamm_opts(C.Structure):
@@ -173,12 +174,12 @@ class Model:
 
     def __init__(self, *, nx, ny, nz, hx, hy, hz, K, nu, nv, pu, pv, f0, mean_dvf, eig_dvf,
                  landmarks_mm=None, sad=1000.0, sdd=1500.0, off_u=0.0, off_v=0.0, cx=0.0, cy=0.0, cz=0.0,
-                 max_batch=1, max_candidates=1, field_storage=0, tile_skipping=0):
+                 max_batch=1, max_candidates=1, field_storage=0, tile_skipping=0, projector=0, ray_step_vox=0.0):
         torch = _torch()
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1004_0014_b200 needs a CUDA device (there is no CPU fallback)")
         self.geo = pcamm_geometry(nx, ny, nz, hx, hy, hz, cx, cy, cz, K, nu, nv, pu, pv, sad, sdd, off_u, off_v,
-                                  max_batch, max_candidates, field_storage, tile_skipping)
+                                  max_batch, max_candidates, field_storage, tile_skipping, projector, ray_step_vox)
         self.K, self.V, self.npix = K, nx * ny * nz, nu * nv
         self.vshape, self.pshape = (nz, ny, nx), (nv, nu)
         lm = np.zeros((0, 3), np.float32) if landmarks_mm is None else \

@@ -147,6 +147,7 @@ struct pcamm_model {
     unsigned *f0_integral = nullptr, *cell_integral = nullptr;   // summed-volume tables (stream.cuh box_count)
     unsigned char* occ = nullptr;       // occupancy of the trial volumes [S][OCC] (common.cuh)
     float *vol = nullptr, *pseg = nullptr, *p = nullptr, *rL = nullptr;   // vol: trial volumes, ray layout [S][PV]
+    float* bvol = nullptr;          // projector 1: backprojection volumes P^T r, [B][V] (raymarch.cu), else NULL
     ColHdr* col_hdr = nullptr;      // [B][nu]
     SlabEntry* slab_tab = nullptr;  // [B][nu][max_slabs]
     float4* utab = nullptr;
@@ -281,7 +282,8 @@ void seq_body(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     const Geom& G = m->G;
     const int n0 = q.n_kernels;
     launch_resid(q, G, m->c.solves, m->c.in, B, 0, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_grad(q, G, m->fs, m->f0p, m->c, B, m->rL, m->utab, m->vtab, GRAD_SOLVE);
+    if (G.projector == 1) launch_backproject_rm(q, G, m->c.solves, B, 0, m->rL, m->bvol);
+    launch_grad(q, G, m->fs, m->f0p, m->c, B, m->rL, m->utab, m->vtab, m->bvol, GRAD_SOLVE);
     launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
     launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_TRIAL, h_loop, use_cond,
                    q.n_kernels - n0);
@@ -492,6 +494,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     if (g->nx < 1 || g->ny < 1 || g->nz < 1 || g->nu < 1 || g->nv < 1) return invalid("sizes must be positive");
     if (!(g->hx > 0 && g->hy > 0 && g->hz > 0 && g->pu > 0 && g->pv > 0)) return invalid("voxel / pixel sizes must be positive");
     if (g->K < 1 || g->K > KMAX) return invalid("K outside [1, PCAMM_KMAX]");
+    if (g->projector != 0 && g->projector != 1) return invalid("geometry.projector must be 0 or 1");
+    if (!(g->ray_step_vox >= 0.f) || !std::isfinite(g->ray_step_vox)) return invalid("geometry.ray_step_vox must be >= 0");
     if (n_landmarks < 0 || (n_landmarks > 0 && !landmarks_mm_host)) return invalid("landmarks");
     const long long V = (long long)g->nx * g->ny * g->nz;
     if ((long long)(g->nx + 4) * (g->ny + 4) * (g->nz + 4) >= (1LL << 31) || (long long)g->nu * g->nv >= (1LL << 31)) return invalid("volume or detector too large");
@@ -533,6 +537,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     G.cx = g->cx; G.cy = g->cy; G.cz = g->cz;
     G.lox = (double)g->cx - ex; G.loy = (double)g->cy - ey; G.loz = (double)g->cz - ez;
     G.ihz_d = 1.0 / (double)g->hz; G.Szi = (0.0 - G.loz) / (double)g->hz;
+    G.projector = g->projector;
+    G.rm_step_mm = (g->ray_step_vox > 0.f ? g->ray_step_vox : 0.5f) * std::fmin(g->hx, std::fmin(g->hy, g->hz));
     G.K = g->K; G.nu = g->nu; G.nv = g->nv; G.npix = g->nu * g->nv;
     G.pu = g->pu; G.pv = g->pv; G.sad = g->sad; G.sdd = g->sdd; G.off_u = g->off_u; G.off_v = g->off_v;
 
@@ -578,6 +584,10 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         cudaGetLastError();
         pcamm_model_destroy(m);
         return e == cudaErrorMemoryAllocation ? PCAMM_E_NOMEM : PCAMM_E_CUDA;
+    }
+    if (g->projector == 1) {
+        e = dalloc(m, &m->bvol, B * (size_t)V);
+        if (e != cudaSuccess) { set_error("allocation failed (backprojection volumes)"); cudaGetLastError(); pcamm_model_destroy(m); return PCAMM_E_NOMEM; }
     }
     if (g_timeline) {
         e = dalloc(m, &m->tl, 1);
@@ -809,7 +819,8 @@ int pcamm_backproject(pcamm_model* m, const float* r_dev, float angle_rad, float
     int rc = hook_begin(m, nullptr, angle_rad, nullptr, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
     launch_resid(q, m->G, m->c.solves, m->c.in, 1, 1, m->p, r_dev, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_backproject(q, m->G, m->c.solves, m->rL, m->utab, m->vtab, volume_out_dev);
+    if (m->G.projector == 1) launch_backproject_rm(q, m->G, m->c.solves, 1, 1, m->rL, volume_out_dev);
+    else launch_backproject(q, m->G, m->c.solves, m->rL, m->utab, m->vtab, volume_out_dev);
     if ((rc = check_seq(q, "backproject"))) return rc;
     CUDA_TRY(cudaStreamSynchronize(st));
     return PCAMM_OK;
@@ -829,7 +840,8 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     launch_warp(q2, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
     launch_project(q2, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_EVAL, 0, 0, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    launch_grad(q2, G, m->fs, m->f0p, m->c, 1, m->rL, m->utab, m->vtab, GRAD_EVAL);
+    if (G.projector == 1) launch_backproject_rm(q2, G, m->c.solves, 1, 1, m->rL, m->bvol);
+    launch_grad(q2, G, m->fs, m->f0p, m->c, 1, m->rL, m->utab, m->vtab, m->bvol, GRAD_EVAL);
     if ((rc = check_seq(q2, "eval"))) return rc;
     if (proj_out_dev) CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * G.npix, cudaMemcpyDeviceToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState), cudaMemcpyDeviceToHost, st));
@@ -845,6 +857,7 @@ int pcamm_traverse(pcamm_model* m, float angle_rad, int32_t iu, int32_t iv, int3
                    float* len_out_host, int32_t* n_out, void* stream) {
     if (!m || !ijk_out_host || !len_out_host || !n_out) return invalid("NULL argument");
     if (iu < 0 || iu >= m->G.nu || iv < 0 || iv >= m->G.nv || cap < 0) return invalid("pixel outside the detector");
+    if (m->G.projector != 0) return invalid("pcamm_traverse lists Siddon's segments: it needs geometry.projector = 0");
     cudaStream_t st = (cudaStream_t)stream;
     Seq q;
     int rc = hook_begin(m, nullptr, angle_rad, nullptr, 0.f, 0.f, 2, st, q);
@@ -963,7 +976,7 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
         else if (which == 1)
             launch_project(q, G, m->c, m->time_slots, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0, 0);
         else
-            launch_grad(q, G, m->fs, m->f0p, m->c, 1, m->rL, m->utab, m->vtab, GRAD_NONE);
+            launch_grad(q, G, m->fs, m->f0p, m->c, 1, m->rL, m->utab, m->vtab, m->bvol, GRAD_NONE);
     }
     CUDA_TRY(cudaEventRecord(m->ev1, st));
     int rc = check_seq(q, "time_kernel");

@@ -77,6 +77,8 @@ struct Geom {
     int K;
     int nu, nv, npix;
     float pu, pv, sad, sdd, off_u, off_v;
+    int projector;            // 0: Siddon's exact path lengths (project.cu), 1: fixed-step ray marching (raymarch.cu)
+    float rm_step_mm;         // nominal step of the ray marching
 };
 
 // Angle-dependent part of the geometry of one solve, computed on the device in double.

@@ -159,7 +159,7 @@ template <int K>
 __global__ void __launch_bounds__(GT)
 k_grad_generic(const Geom G, const float* __restrict__ f0, const float* __restrict__ xbar, const float* __restrict__ u,
        const CtlBufs c, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
-       const float2* __restrict__ vtab) {
+       const float2* __restrict__ vtab, const float* __restrict__ bvol) {
     __shared__ double red[GT / 32];
     tl_begin(G.tl);
     const SolveState* __restrict__ solves = c.solves;
@@ -216,7 +216,8 @@ k_grad_generic(const Geom G, const float* __restrict__ f0, const float* __restri
             trilinear_grad(G, f0, x, y, z, d[0], d[1], d[2], &gx, &gy, &gz);
             if (gx == 0.f && gy == 0.f && gz == 0.f) continue;
             const float yw = G.cy + ((float)y - 0.5f * (G.ny - 1)) * G.hy;
-            const float Bj = gather_voxel(G, gv, rLb, ub, vb, xw, yw, zw);
+            const float Bj = bvol ? __ldg(bvol + (long long)b * V + ((long long)z * G.ny + y) * G.nx + x)
+                                  : gather_voxel(G, gv, rLb, ub, vb, xw, yw, zw);
 #pragma unroll
             for (int k = 0; k < K; ++k)
                 acc[k] = fmaf(Bj, gx * uu[r][k][0] + gy * uu[r][k][1] + gz * uu[r][k][2], acc[k]);
@@ -292,7 +293,7 @@ __global__ void __launch_bounds__(32 * GradGroups<K>::value * GROUP_WARPS, 1)
 k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
            const FieldMax fmax, const unsigned* __restrict__ cell_integral, const Geom G, const float* __restrict__ f0,
            const unsigned char* __restrict__ cellmap, const CtlBufs c, int b0, int B, const float* __restrict__ rL, const float4* __restrict__ utab,
-           const float2* __restrict__ vtab, unsigned long long* __restrict__ visited) {
+           const float2* __restrict__ vtab, const float* __restrict__ bvol, unsigned long long* __restrict__ visited) {
     constexpr int P = 3 * (K + 1), GTZ = TileZ<K>::value, GROWS = GTZ / GROUP_WARPS;
     const SolveState* __restrict__ solves = c.solves + b0;                 // solves b0 .. b0 + B - 1 in this launch
     constexpr int RB = GradBatch<K>::value, NB = GROWS / RB;
@@ -537,7 +538,8 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                         const float xw = G.cx + ((float)(en.xy & 0xffff) - 0.5f * (G.nx - 1)) * G.hx;
                         const float yw = G.cy + ((float)(en.xy >> 16) - 0.5f * (G.ny - 1)) * G.hy;
                         const float zw = G.cz + ((float)en.z - 0.5f * (G.nz - 1)) * G.hz;
-                        const float Bj = gather_voxel(G, gv, rLb, ub, vb, xw, yw, zw);
+                        const float Bj = bvol ? __ldg(bvol + (long long)b * G.V + ((long long)en.z * G.ny + (en.xy >> 16)) * G.nx + (en.xy & 0xffff))
+                                              : gather_voxel(G, gv, rLb, ub, vb, xw, yw, zw);
 #pragma unroll
                         for (int k = 0; k < K; ++k) acc[k] = fmaf(Bj, en.q[k], acc[k]);
                     }
@@ -583,7 +585,8 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                 const float xw = G.cx + ((float)(en.xy & 0xffff) - 0.5f * (G.nx - 1)) * G.hx;
                 const float yw = G.cy + ((float)(en.xy >> 16) - 0.5f * (G.ny - 1)) * G.hy;
                 const float zw = G.cz + ((float)en.z - 0.5f * (G.nz - 1)) * G.hz;
-                const float Bj = gather_voxel(G, gv, rL, utab, vtab, xw, yw, zw);
+                const float Bj = bvol ? __ldg(bvol + ((long long)en.z * G.ny + (en.xy >> 16)) * G.nx + (en.xy & 0xffff))
+                                      : gather_voxel(G, gv, rL, utab, vtab, xw, yw, zw);
 #pragma unroll
                 for (int k = 0; k < K; ++k) acc[k] = fmaf(Bj, en.q[k], acc[k]);
             }
@@ -644,7 +647,7 @@ k_backproject(const Geom G, const SolveState* __restrict__ solves, const float* 
 
 template <int K, bool H>
 void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const CtlBufs& c, int B,
-                const float* rL, const float4* utab, const float2* vtab) {
+                const float* rL, const float4* utab, const float2* vtab, const float* bvol) {
     static DeviceOnce configured;
     constexpr size_t smem = grad_smem_bytes<K, H>();
     {
@@ -663,27 +666,27 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     const unsigned* skip_table = tile_count(G, TileZ<K>::value) >= fs.skip_min_tiles_per_sm * (long long)fs.n_sm ? fs.cell_integral : nullptr;
     if (B == 1) {
         q.launch(skip_table ? k_grad_tma<K, true, H, true> : k_grad_tma<K, true, H, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, skip_table, G, f0,
-                 fs.cellmap, c, 0, 1, rL, utab, vtab, fs.visited);
+                 fs.cellmap, c, 0, 1, rL, utab, vtab, bvol, fs.visited);
         return;
     }
     for (int b0 = 0; b0 < B; b0 += SOLVE_CACHE) {       // the kernel keeps up to SOLVE_CACHE solves' constants on chip
         const int nb = B - b0 < SOLVE_CACHE ? B - b0 : SOLVE_CACHE;
         q.launch(skip_table ? k_grad_tma<K, false, H, true> : k_grad_tma<K, false, H, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, skip_table, G, f0,
                  fs.cellmap, c, b0, nb, rL + (long long)b0 * G.npix, utab + (long long)b0 * G.nu,
-                 vtab + (long long)b0 * G.nv, fs.visited);
+                 vtab + (long long)b0 * G.nv, bvol ? bvol + (long long)b0 * G.V : bvol, fs.visited);
     }
 }
 
 template <int K>
 void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const CtlBufs& c, int B,
-              const float* rL, const float4* utab, const float2* vtab) {
+              const float* rL, const float4* utab, const float2* vtab, const float* bvol) {
     if (fs.use_tma) {
-        if (fs.half_u) launch_tma<K, true>(q, G, fs, f0, c, B, rL, utab, vtab);
-        else launch_tma<K, false>(q, G, fs, f0, c, B, rL, utab, vtab);
+        if (fs.half_u) launch_tma<K, true>(q, G, fs, f0, c, B, rL, utab, vtab, bvol);
+        else launch_tma<K, false>(q, G, fs, f0, c, B, rL, utab, vtab, bvol);
         return;
     }
     dim3 grid((G.nx + TILE - 1) / TILE, (G.ny + TILE - 1) / TILE, G.nz);
-    q.launch(k_grad_generic<K>, grid, dim3(GT), 0, G, f0, fs.fields, fs.fields + 3 * G.V, c, B, rL, utab, vtab);
+    q.launch(k_grad_generic<K>, grid, dim3(GT), 0, G, f0, fs.fields, fs.fields + 3 * G.V, c, B, rL, utab, vtab, bvol);
 }
 
 }  // namespace
@@ -707,10 +710,10 @@ void launch_resid(Seq& q, const Geom& G, const SolveState* solves, const SolveIn
 }
 
 void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const CtlBufs& c, int B,
-                 const float* rL, const float4* utab, const float2* vtab, int mode) {
+                 const float* rL, const float4* utab, const float2* vtab, const float* bvol, int mode) {
     switch (G.K) {
 #define PCAMM_CASE(KK) \
-    case KK: launch_k<KK>(q, G, fs, f0, c, B, rL, utab, vtab); break;
+    case KK: launch_k<KK>(q, G, fs, f0, c, B, rL, utab, vtab, bvol); break;
         PCAMM_CASE(1) PCAMM_CASE(2) PCAMM_CASE(3) PCAMM_CASE(4)
         PCAMM_CASE(5) PCAMM_CASE(6) PCAMM_CASE(7) PCAMM_CASE(8)
 #undef PCAMM_CASE

@@ -126,6 +126,11 @@ int project_segments(const Geom& G);
 void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const ColHdr* hdr, const SlabEntry* tab,
                     const float* vol, const unsigned char* occ, float* pseg, float* p, int then,
                     cudaGraphConditionalHandle h, int use_cond, int n_before);
+// the ray-marching variant (raymarch.cu; pcamm_geometry.projector = 1): p[s] and the a-3 partial sums
+// (no control step: launch_project adds it), and B[b] = P^T r for the solves that need a gradient
+// (force: for all), r taken from rL = r |D - S|
+void launch_project_rm(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const float* vol, float* p);
+void launch_backproject_rm(Seq& q, const Geom& G, const SolveState* solves, int B, int force, const float* rL, float* bvol);
 // hooks: standard layout -> ray layout; one ray of the view of solve 0
 void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray, unsigned char* occ);
 void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* tab, int iu, int iv, int cap,
@@ -142,8 +147,10 @@ void launch_resid(Seq& q, const Geom& G, const SolveState* solves, const SolveIn
                   const float* p, const float* r_direct, float* rL, float4* utab, float2* vtab, double* partials);
 // g = 2 U^T (df/dx) P^T r for the solves that need it (control.cuh needs_gradient), per-block partial
 // sums [B][blocks][K], and then the control step `mode` (GRAD_*).
+// bvol: NULL (Siddon: B_j is gathered from rL with the exact path lengths) or the backprojection
+// volumes [B][V] of launch_backproject_rm
 void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const CtlBufs& c, int B,
-                 const float* rL, const float4* utab, const float2* vtab, int mode);
+                 const float* rL, const float4* utab, const float2* vtab, const float* bvol, int mode);
 // hook: B = P^T r as a volume for solve 0's view (rL/utab/vtab as written by launch_resid).
 void launch_backproject(Seq& q, const Geom& G, const SolveState* solves, const float* rL, const float4* utab,
                         const float2* vtab, float* vol_out);

@@ -617,6 +617,11 @@ void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const C
                     const float* vol, const unsigned char* occ, float* pseg, float* p, int then,
                     cudaGraphConditionalHandle h, int use_cond, int n_before) {
     const int n_mark = q.n_kernels;
+    if (G.projector == 1) {                                  // the ray-marching variant (raymarch.cu)
+        launch_project_rm(q, G, c, nslots, vol, p);
+        launch_ctl_after_project(q, G, c, then, h, use_cond, q.n_kernels - n_mark + n_before);
+        return;
+    }
     const int sc = scan_slabs(G);
     const bool v4 = G.nz % 4 == 0, one = G.nv <= PT;
 #define PCAMM_PROJ(VEC, SC) \

@@ -8,7 +8,8 @@ import numpy as np
 import oracle
 
 
-def make_model(g: oracle.Geometry, f0, xbar, u, landmarks=None, max_batch=1, max_candidates=1, tile_skipping=1):
+def make_model(g: oracle.Geometry, f0, xbar, u, landmarks=None, max_batch=1, max_candidates=1, tile_skipping=1,
+               projector=0, ray_step_vox=0.0):
     # tile_skipping=1: the parity grids are too small for the library's default to turn the tile flags on
     import torch
     import paper_1004_0014_b200 as pc
@@ -17,7 +18,8 @@ def make_model(g: oracle.Geometry, f0, xbar, u, landmarks=None, max_batch=1, max
     return pc.Model(nx=g.nx, ny=g.ny, nz=g.nz, hx=g.hx, hy=g.hy, hz=g.hz, K=g.K, nu=g.nu, nv=g.nv, pu=g.pu,
                     pv=g.pv, f0=t(f0), mean_dvf=t(xbar), eig_dvf=t(u), landmarks_mm=landmarks, sad=g.sad,
                     sdd=g.sdd, off_u=g.off_u, off_v=g.off_v, cx=g.cx, cy=g.cy, cz=g.cz, max_batch=max_batch,
-                    max_candidates=max_candidates, tile_skipping=tile_skipping)
+                    max_candidates=max_candidates, tile_skipping=tile_skipping, projector=projector,
+                    ray_step_vox=ray_step_vox)
 
 
 def to_dev(a):

@@ -33,7 +33,7 @@ def test_default_opts_and_struct_layout():
     d = pc.Opts()
     for f, _ in pc.pcamm_opts._fields_:
         assert getattr(o, f) == pytest.approx(getattr(d, f)), f
-    assert C.sizeof(pc.pcamm_geometry) == 22 * 4
+    assert C.sizeof(pc.pcamm_geometry) == 24 * 4
     assert C.sizeof(pc.pcamm_opts) == 10 * 4
     assert C.sizeof(pc.pcamm_info) == 8 + 4 * 8 + 4 * 8
 

@@ -564,8 +564,10 @@ def run_timeline(args, cfg, rank, local_rank):
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(dev)
     m = pc.Model(nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, hx=cfg.hx, hy=cfg.hy, hz=cfg.hz, K=cfg.K, nu=cfg.nu, nv=cfg.nv,
                  pu=cfg.pu, pv=cfg.pv, f0=t(wl.f0), mean_dvf=t(wl.model.mean), eig_dvf=t(wl.model.eig),
-                 landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=8 if cfg.batched_linesearch else 1)
-    opts = pc.Opts(max_iter=solver_iterations(cfg), batched_linesearch=1 if cfg.batched_linesearch else 0)
+                 landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd,
+                 max_candidates=8 if cfg.batched_linesearch else max(int(args.fan), 1))
+    fan = 1 if cfg.batched_linesearch else int(args.fan)
+    opts = pc.Opts(max_iter=solver_iterations(cfg), batched_linesearch=1 if cfg.batched_linesearch else (fan if fan > 1 else 0))
     w = np.zeros(cfg.K, np.float32)
     for i, fid in enumerate(ids):
         fr = wl.frames[fid]
@@ -597,7 +599,7 @@ def run_timeline(args, cfg, rank, local_rank):
             for i, (k, a, b) in enumerate(zip(kind, t0, t1)):
                 f.write(f"{i:4d} {TL_KINDS[k]:18s} {a:10.2f} {b:10.2f} {b - a:8.2f} {0.0 if pe is None else a - pe:8.2f}\n")
                 pe = b
-    print(json.dumps({"study": "timeline", "config": config_dict(cfg, solver_iterations(cfg)), "kernels": int(len(kind)),
+    print(json.dumps({"study": "timeline", "config": config_dict(cfg, solver_iterations(cfg), fan), "kernels": int(len(kind)),
                       "span_us": span, "busy_us": busy, "busy_frac": busy / span if span else None,
                       "solve_ms_cuda_events_with_timeline_on": e0.elapsed_time(e1),
                       "per_kind": per, "iters": int(r.iters)}), flush=True)

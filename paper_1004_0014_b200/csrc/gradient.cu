@@ -446,7 +446,7 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                               ck = c.z0 + zz + (int)floorf(dda[ra][2]) + 1;
                     const bool inside = x < G.nx && c.z0 + zz < G.nz && (unsigned)ci <= (unsigned)G.nx &&
                                         (unsigned)cj <= (unsigned)G.ny && (unsigned)ck <= (unsigned)G.nz;
-                    flaga[ra] = inside ? __ldg(cellmap + ((long long)ck * (G.ny + 1) + cj) * (G.nx + 1) + ci) : (unsigned char)0;
+                    flaga[ra] = inside ? __ldg(cellmap + ((unsigned)ck * (unsigned)(G.ny + 1) + (unsigned)cj) * (unsigned)(G.nx + 1) + (unsigned)ci) : (unsigned char)0;   // (< 2^31 cells)
                 }
 #pragma unroll
                 for (int bt = 0; bt < NB; ++bt) {

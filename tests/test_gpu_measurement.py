@@ -1,0 +1,128 @@
+"""The measurement hooks of the C ABI (they feed bench.py's roofline block and the timeline under
+profiles/): the tile counters of the two streaming kernels, the in-kernel timeline, the timing hooks
+over several candidate slots, the tuning knobs.  No parity claims here; what is checked is that the
+numbers mean what bench.py takes them to mean.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from tests.gpu_util import make_model, to_dev
+from tests.util import geom, smooth_model
+
+pytestmark = pytest.mark.gpu
+
+
+def _setup(tile_skipping=1, **kw):
+    g = geom(nx=96, ny=70, nz=64, h=(2.0, 2.0, 2.0), K=3, nu=96, nv=64, pitch=(3.4, 2.6))
+    f0, xbar, u, scale = smooth_model(g, seed=5, disp_vox=1.0)
+    zz, yy, xx = np.meshgrid(np.arange(g.nz), np.arange(g.ny), np.arange(g.nx), indexing="ij")
+    body = ((xx - 60) / 20.0) ** 2 + ((yy - 30) / 14.0) ** 2 + ((zz - 30) / 18.0) ** 2 <= 1.0
+    f0 = np.where(body, 0.5 + f0, 0.0).astype(np.float32)            # a body in a lot of air: tiles to skip
+    m = make_model(g, f0, xbar, u, tile_skipping=tile_skipping, **kw)
+    w = (0.4 * scale * np.array([1.0, -0.6, 0.8])).astype(np.float32)
+    _, p = oracle.evaluate(g, f0, xbar, u, w, 0.9)
+    return g, m, w, to_dev(p.astype(np.float32))
+
+
+def test_tile_counters_count_the_tiles_the_timed_launches_loaded():
+    g, m, w, y = _setup(tile_skipping=1)
+    m.eval(y, 0.9, w, 1.0, 0.0, want_proj=False)
+    m.tile_counts(reset=True)
+    m.time_kernel(0, 5)
+    warp_tiles, grad_tiles, total, vox = m.tile_counts(reset=True)
+    assert vox == 32 * 32 and total == 3 * g.ny * 2
+    assert grad_tiles == 0 and warp_tiles % 5 == 0 and 0 < warp_tiles // 5 < total
+    m.time_kernel(2, 4)
+    warp_tiles, grad_tiles, _, _ = m.tile_counts(reset=True)
+    assert warp_tiles == 0 and grad_tiles % 4 == 0 and 0 < grad_tiles // 4 < total
+    # with skipping off every tile is loaded
+    g2, m2, w2, y2 = _setup(tile_skipping=2)
+    m2.eval(y2, 0.9, w2, 1.0, 0.0, want_proj=False)
+    m2.tile_counts(reset=True)
+    m2.time_kernel(0, 3)
+    m2.time_kernel(2, 3)
+    a, b, total2, _ = m2.tile_counts()
+    assert a == 3 * total2 and b == 3 * total2
+
+
+def test_timing_over_two_candidate_slots():
+    """pcamm_time_slots: the warp and projection timings then run over two candidates per launch; the fields
+    are still loaded once per tile."""
+    g, m, w, y = _setup(max_candidates=2)
+    m.eval(y, 0.9, w, 1.0, 0.0, want_proj=False)
+    m.tile_counts(reset=True)
+    m.time_kernel(0, 4)
+    one = m.tile_counts(reset=True)[0]
+    m.time_slots(np.stack([w, 1.05 * w]))
+    t_warp, t_proj = m.time_kernel(0, 4), m.time_kernel(1, 4)
+    two = m.tile_counts(reset=True)[0]
+    assert t_warp > 0 and t_proj > 0
+    assert one > 0 and two >= one                  # the same tiles (a few more where the larger w reaches further)
+    assert two <= 1.2 * one
+    with pytest.raises(Exception):
+        m.time_slots(np.stack([w, w, w]))          # more slots than the model has
+
+
+def test_timeline_lists_the_kernels_of_a_solve_in_order():
+    import paper_1004_0014_b200 as pc
+    pc.tune("timeline", 1)
+    try:
+        g, m, w, y = _setup(landmarks=np.array([[5.0, -4.0, 3.0]], np.float32))
+    finally:
+        pc.tune("timeline", 0)
+    res = m.reconstruct(y, 0.9, np.zeros(3, np.float32), pc.Opts(max_iter=3), trace=True)
+    kind, t0, t1 = m.timeline()
+    names = ("ysums", "begin", "view", "warp", "project", "ctl_proj", "resid", "grad", "ctl_grad", "-", "final", "invert")
+    seq = [names[k] for k in kind]
+    assert seq[:6] == ["ysums", "begin", "view", "warp", "project", "ctl_proj"]
+    assert seq[-3:] == ["resid", "final", "invert"]
+    body = seq[6:-3]
+    assert len(body) % 6 == 0 and len(body) // 6 >= res.iters
+    for i in range(0, len(body), 6):
+        assert body[i:i + 6] == ["resid", "grad", "ctl_grad", "warp", "project", "ctl_proj"]
+    assert np.all(t1 >= t0) and np.all(t0[1:] >= t1[:-1])          # one after the other
+    assert pc.launch_count() >= len(kind)
+    # a model created without the knob has no timeline
+    g2, m2, _, _ = _setup()
+    with pytest.raises(pc.PcammError):
+        m2.timeline()
+
+
+def test_unknown_knob_is_an_error():
+    import paper_1004_0014_b200 as pc
+    with pytest.raises(pc.PcammError):
+        pc.tune("no_such_knob", 1)
+
+
+def test_projector_knobs_change_the_launch_not_the_result():
+    import paper_1004_0014_b200 as pc
+    g, m, w, y = _setup()
+    _, _, _, p_ref = m.eval(y, 0.9, w, 1.0, 0.0)
+    p_ref = p_ref.cpu().numpy()
+    try:
+        for sc, cps in ((2, 1), (1, 3), (4, 2)):
+            pc.tune("project_scan_slabs", sc)
+            pc.tune("project_chunks_per_segment", cps)
+            g2, m2, _, _ = _setup()
+            p = m2.eval(y, 0.9, w, 1.0, 0.0)[3].cpu().numpy()
+            assert np.max(np.abs(p - p_ref)) <= 2e-6 * np.max(np.abs(p_ref))
+    finally:
+        pc.tune("project_scan_slabs", 0)
+        pc.tune("project_chunks_per_segment", 0)
+
+
+def test_model_on_a_second_device():
+    """The opt-in to large dynamic shared memory is per device."""
+    import torch
+    import paper_1004_0014_b200 as pc
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two visible GPUs")
+    g, m, w, y = _setup()
+    with torch.cuda.device(1):
+        f0, xbar, u, scale = smooth_model(g, seed=5, disp_vox=1.0)
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to("cuda:1")
+        m1 = pc.Model(nx=g.nx, ny=g.ny, nz=g.nz, hx=g.hx, hy=g.hy, hz=g.hz, K=g.K, nu=g.nu, nv=g.nv, pu=g.pu, pv=g.pv,
+                      f0=t(f0), mean_dvf=t(xbar), eig_dvf=t(u), sad=g.sad, sdd=g.sdd)
+        out = m1.warp(w)
+        assert out.device.index == 1

@@ -92,14 +92,24 @@ def algorithmic_bytes(cfg, field_storage=0):
             "gradient": (fields + 4) * V + 4 * npix}
 
 
-def moved_bytes(cfg, field_storage, tiles_loaded, vox_per_tile):
+RECORD_BYTES = 20       # one gradient record: x | y << 16, z, G_x, G_y, G_z (stream.cuh GradRecords)
+
+
+def moved_bytes(cfg, field_storage, tiles_loaded, vox_per_tile, records=None, n_tiles=0):
     """What one launch really had to move, from the tiles the timed launches loaded (counted inside the
     kernels, pcamm_tile_counts; reading B8: tiles that can only see zeros / constant cells are skipped).
     A loaded tile costs its fields and its f0 gathers (4 B per voxel, counted once); the warp kernel
-    writes every voxel of the volume (skipped tiles as zeros), the gradient kernel reads the residual."""
+    writes every voxel of the volume (skipped tiles as zeros), the gradient kernel reads the residual.
+    With gradient records (the default for one solve) the warp kernel also writes 20 B per voxel with
+    G_j != 0 and a count per sub-tile (8 per tile); the gradient reads those and 12 K bytes of u per record
+    (scattered 4-byte loads: the sectors they touch are not counted) and the residual."""
     fields = field_bytes_per_voxel(cfg, field_storage)
-    return {"warp": tiles_loaded["warp"] * vox_per_tile * (fields + 4) + 4 * cfg.V,
-            "gradient": tiles_loaded["gradient"] * vox_per_tile * (fields + 4) + 4 * cfg.npix}
+    out = {"warp": tiles_loaded["warp"] * vox_per_tile * (fields + 4) + 4 * cfg.V,
+           "gradient": tiles_loaded["gradient"] * vox_per_tile * (fields + 4) + 4 * cfg.npix}
+    if records and records["gathered"] > 0:
+        out["warp"] += RECORD_BYTES * records["written"] + 4 * 8 * n_tiles
+        out["gradient"] = (RECORD_BYTES + 12 * cfg.K) * records["gathered"] + 4 * 8 * n_tiles + 4 * cfg.npix
+    return out
 
 
 def measured_peak_gbs():
@@ -379,13 +389,18 @@ def run_ours(args, cfg, rank, local_rank, world):
     for which in (0, 1, 2):
         m.time_kernel(which, 3)
     REPS = 20
-    kt, tiles_loaded = {}, {}
+    kt, tiles_loaded, records = {}, {}, {"written": 0.0, "gathered": 0.0}
     for which, name in ((0, "warp"), (1, "project"), (2, "gradient")):
         m.tile_counts(reset=True)
         kt[name] = m.time_kernel(which, REPS)
         tc = m.tile_counts(reset=True)               # tiles the timed launches loaded, counted in the kernels
         tiles_loaded[name] = tc[0 if which == 0 else 1] / REPS
+        if which == 0:
+            records["written"] = tc[5] / REPS        # gradient records, all candidates of the launch
+        if which == 2:
+            records["gathered"] = tc[4] / REPS       # those of the accepted candidate
     n_tiles, vox_per_tile = tc[2], tc[3]
+    by_records = records["gathered"] > 0
     nl = {"warp": passes + 1, "project": passes + 1, "gradient": tr.iters}
     ab = algorithmic_bytes(cfg, args.field_storage)
     peak, peak_src = measured_peak_gbs()
@@ -393,7 +408,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     ab["warp"] += (width - 1) * 8 * cfg.V
     ab["project"] *= width
     if n_tiles:
-        mv = moved_bytes(cfg, args.field_storage, tiles_loaded, vox_per_tile)
+        mv = moved_bytes(cfg, args.field_storage, tiles_loaded, vox_per_tile, records, n_tiles)
         mv["warp"] += (width - 1) * (tiles_loaded["warp"] * vox_per_tile * 4 + 4 * cfg.V)
     else:                                            # generic kernels (shapes TMA cannot describe): every tile
         mv = {"warp": ab["warp"], "gradient": ab["gradient"]}
@@ -409,6 +424,14 @@ def run_ours(args, cfg, rank, local_rank, world):
         if k != "project" and n_tiles:
             per_kernel[k]["tiles_loaded_per_launch"] = tiles_loaded[k]
             per_kernel[k]["tiles_total"] = n_tiles
+    if by_records:
+        per_kernel["warp"]["gradient_records_written_per_launch"] = records["written"]
+        per_kernel["gradient"].update({
+            "kernel": "k_grad_gather", "records_per_launch": records["gathered"],
+            "records_per_voxel": records["gathered"] / cfg.V,
+            "note": "a gather over the records the warp kernel left for the voxels with G_j != 0 (DESIGN.md section 5b): "
+                    "latency- and sector-bound scattered loads, not a stream; moved_bytes counts 20 B per record, "
+                    "12 K B of u per record, the counts and the residual, not the 32-byte sectors touched"})
     # the projector's volume was just written and is L2-resident: it is not an HBM kernel.
     # What it does per launch: one pass over (detector column, slab, level) and one look-up per z crossing.
     per_kernel["project"].update({

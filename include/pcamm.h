@@ -277,14 +277,21 @@ int pcamm_time_slots(pcamm_model* model, int32_t nslots, const float* w_host, vo
  * of f0 / constant cells are skipped, exactly).  out[0], out[1] = field tiles loaded by the warp and
  * by the gradient kernel in all launches since the counters were last reset (one tile = out[3]
  * voxels, all 3(K+1) field planes); out[2] = tiles of the whole volume (0: the generic kernels are
- * in use, which visit everything and count nothing).  reset != 0 clears the counters. */
-int pcamm_tile_counts(pcamm_model* model, int32_t reset, int64_t* out /* [4] */, void* stream);
+ * in use, which visit everything and count nothing).  With gradient records (pcamm_tune
+ * "grad_records", the default for a single solve) the gradient loads no field tiles: out[4] = records
+ * its gather went through, out[5] = records the warp kernel wrote (20 bytes each), same launches.
+ * reset != 0 clears the counters. */
+int pcamm_tile_counts(pcamm_model* model, int32_t reset, int64_t* out /* [6] */, void* stream);
 
 /* Measurement knob (process-wide; set it before pcamm_model_create: a model's solve graphs keep the
  * launch configuration they were built with).  Returns PCAMM_E_INVALID for an unknown name.
  *   "project_chunks_per_segment"  chunks of the projector's march a block works through
  *                                 (0 = automatic, the default);
  *   "project_scan_slabs"          slabs per scan of the projector: 1, 2 or 4 (0 = automatic);
+ *   "grad_records"                0: the gradient of a single solve makes its own pass over the K+1 fields
+ *                                 (1, the default: the warp kernel leaves records of the voxels with a
+ *                                 non-zero image gradient and the gradient is a gather over them;
+ *                                 DESIGN.md section 5a);
  *   "timeline"                    1: models created from now on record, inside their kernels, the
  *                                 start and end of every kernel of a solve (pcamm_timeline). */
 int pcamm_tune(const char* name, int32_t value);

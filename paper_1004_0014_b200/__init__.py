@@ -347,8 +347,9 @@ class Model:
         return kind[:k].copy(), t0[:k].copy(), t1[:k].copy()
 
     def tile_counts(self, reset: bool = False):
-        """pcamm_tile_counts: (warp tiles loaded, gradient tiles loaded, tiles of the volume, voxels per tile)."""
-        out = (C.c_int64 * 4)()
+        """pcamm_tile_counts: (warp tiles loaded, gradient tiles loaded, tiles of the volume, voxels per tile,
+        gradient records gathered, gradient records written by the warp kernel)."""
+        out = (C.c_int64 * 6)()
         _check(lib().pcamm_tile_counts(self._h, 1 if reset else 0, out, _stream()))
         return tuple(int(v) for v in out)
 

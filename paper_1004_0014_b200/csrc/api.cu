@@ -18,6 +18,7 @@ namespace pcamm {
 static thread_local std::string g_error;
 static thread_local long long g_launches = 0;
 int g_timeline = 0;
+int g_grad_records = 1;   // pcamm_tune "grad_records": 0 = the gradient of a single solve makes its own pass over the fields
 
 void set_error(const std::string& msg) { g_error = msg; }
 void count_launch(long long n) { g_launches += n; }
@@ -273,7 +274,7 @@ void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     launch_ysums(q, G, m->c, B);
     launch_begin(q, G, m->c, 0);
     launch_view_tables(q, G, m->c.solves, B, m->col_hdr, m->slab_tab);
-    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
+    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ, B == 1 ? m->fs.grad_rec : nullptr);
     launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_INIT, h_loop, use_cond,
                    q.n_kernels);
 }
@@ -284,7 +285,7 @@ void seq_body(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     launch_resid(q, G, m->c.solves, m->c.in, B, 0, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
     if (G.projector == 1) launch_backproject_rm(q, G, m->c.solves, B, 0, m->rL, m->bvol);
     launch_grad(q, G, m->fs, m->f0p, m->c, B, m->rL, m->utab, m->vtab, m->bvol, GRAD_SOLVE);
-    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ);
+    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ, B == 1 ? m->fs.grad_rec : nullptr);
     launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_TRIAL, h_loop, use_cond,
                    q.n_kernels - n0);
 }
@@ -384,7 +385,7 @@ int solve_impl(pcamm_model* m, int B, const float* y_dev, const float* angles, c
     if (volumes_out) {
         Seq q;
         q.stream = st;
-        launch_warp(q, G, m->fs, m->f0p, m->out_slots, B, 0, volumes_out, G.V, nullptr);
+        launch_warp(q, G, m->fs, m->f0p, m->out_slots, B, 0, volumes_out, G.V, nullptr, nullptr);
         if ((rc = check_seq(q, "final warp"))) return rc;
     }
     CUDA_TRY(cudaMemcpyAsync(m->h_solves, m->c.solves, sizeof(SolveState) * B, cudaMemcpyDeviceToHost, st));
@@ -573,7 +574,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         ok(dalloc(m, &m->c.grad_part, B * m->c.grad_blocks * KMAX)) && ok(dalloc(m, &m->out_slots, B)) &&
         ok(dalloc(m, &m->lm_out, 3 * B * (size_t)(m->M > 0 ? m->M : 1))) &&
         ok(dalloc(m, &m->trav_ijk, 3 * (size_t)m->trav_cap)) && ok(dalloc(m, &m->trav_len, (size_t)m->trav_cap)) &&
-        ok(dalloc(m, &m->trav_n, 1)) && ok(dalloc(m, &m->nonfinite, 1)) && ok(dalloc(m, &m->visited, 2)) && ok(dalloc(m, &m->y_stage, (size_t)G.npix)) &&
+        ok(dalloc(m, &m->trav_n, 1)) && ok(dalloc(m, &m->nonfinite, 1)) && ok(dalloc(m, &m->visited, 4)) && ok(dalloc(m, &m->y_stage, (size_t)G.npix)) &&
         ok(halloc(m, &m->h_in, m->in_block_bytes)) && ok(halloc(m, &m->h_solves, B)) &&
         ok(halloc(m, &m->h_traces, B)) && ok(halloc(m, &m->h_flags, 1)) &&
         ok(halloc(m, &m->h_lm, 3 * B * (size_t)(m->M > 0 ? m->M : 1))) &&
@@ -617,7 +618,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     TRY_OR_FAIL(cudaMemsetAsync(m->vol, 0, sizeof(float) * S * (size_t)G.PV, st));   // zero border, never written
     TRY_OR_FAIL(cudaMemsetAsync(m->occ, 0, S * (size_t)G.OCC, st));                   // likewise
     TRY_OR_FAIL(cudaMemsetAsync(m->nonfinite, 0, sizeof(unsigned long long), st));
-    TRY_OR_FAIL(cudaMemsetAsync(m->visited, 0, 2 * sizeof(unsigned long long), st));
+    TRY_OR_FAIL(cudaMemsetAsync(m->visited, 0, 4 * sizeof(unsigned long long), st));
     m->fs.visited = m->visited;
     TRY_OR_FAIL(cudaMemsetAsync(m->c.solves, 0, sizeof(SolveState) * B, st));
     TRY_OR_FAIL(cudaMemsetAsync(m->c.slots, 0, sizeof(SlotState) * S, st));
@@ -743,6 +744,22 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         m->fs.skip_min_tiles_per_sm = g->tile_skipping == 1 ? 0 : (g->tile_skipping == 2 ? (1 << 30) : SKIP_MIN_TILES_PER_SM);
     }
     m->c.grad_blocks = grad_blocks(G, m->fs);
+    if (m->fs.use_tma && g_grad_records) {
+        // gradient records of the trial slots of a single solve (stream.cuh GradRecords): 20 bytes per voxel and slot
+        const int tz = G.K <= PCAMM_TZ_SMALL_K ? 32 : 16;                     // TileZ<K>
+        const long long n_tiles = tile_count(G, tz), n_sub = n_tiles * GROUP_WARPS, plane = n_tiles * (TX * tz);
+        const size_t words = (size_t)grad_record_words(n_sub, plane) * (size_t)Cmax;
+        int* rec = nullptr;
+        cudaError_t e4 = dalloc(m, &rec, words);
+        if (e4 == cudaSuccess) e4 = cudaMemsetAsync(rec, 0, sizeof(int) * words, st);
+        if (e4 == cudaSuccess) e4 = cudaStreamSynchronize(st);
+        if (e4 != cudaSuccess) {
+            set_error(std::string("gradient records: ") + cudaGetErrorString(e4));
+            cudaGetLastError();
+            return fail(e4 == cudaErrorMemoryAllocation ? PCAMM_E_NOMEM : PCAMM_E_CUDA);
+        }
+        m->fs.grad_rec = rec;
+    }
     *out = m;
     return PCAMM_OK;
 }
@@ -791,7 +808,7 @@ int pcamm_warp(pcamm_model* m, const float* w_host, float* volume_out_dev, void*
     Seq q;
     int rc = hook_begin(m, nullptr, 0.f, w_host, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
-    launch_warp(q, m->G, m->fs, m->f0p, m->c.slots, 1, 0, volume_out_dev, m->G.V, nullptr);
+    launch_warp(q, m->G, m->fs, m->f0p, m->c.slots, 1, 0, volume_out_dev, m->G.V, nullptr, nullptr);
     if ((rc = check_seq(q, "warp"))) return rc;
     CUDA_TRY(cudaStreamSynchronize(st));
     return PCAMM_OK;
@@ -837,7 +854,7 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     m->time_slots = 1;
     launch_ysums(q2, G, m->c, 1);
     launch_view_tables(q2, G, m->c.solves, 1, m->col_hdr, m->slab_tab);
-    launch_warp(q2, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ);
+    launch_warp(q2, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ, m->fs.grad_rec);
     launch_project(q2, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_EVAL, 0, 0, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
     if (G.projector == 1) launch_backproject_rm(q2, G, m->c.solves, 1, 1, m->rL, m->bvol);
@@ -908,7 +925,7 @@ int pcamm_localise(pcamm_model* m, const float* w_host, int32_t inv_max_iter, fl
 int pcamm_tile_counts(pcamm_model* m, int32_t reset, int64_t* out, void* stream) {
     if (!m || !out) return invalid("NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned long long h[2] = {0ull, 0ull};
+    unsigned long long h[4] = {0ull, 0ull, 0ull, 0ull};
     CUDA_TRY(cudaMemcpyAsync(h, m->visited, sizeof(h), cudaMemcpyDeviceToHost, st));
     if (reset) CUDA_TRY(cudaMemsetAsync(m->visited, 0, sizeof(h), st));
     CUDA_TRY(cudaStreamSynchronize(st));
@@ -916,6 +933,7 @@ int pcamm_tile_counts(pcamm_model* m, int32_t reset, int64_t* out, void* stream)
     out[0] = (int64_t)h[0]; out[1] = (int64_t)h[1];
     out[2] = m->fs.use_tma ? (int64_t)tile_count(m->G, tz) : 0;
     out[3] = (int64_t)TX * tz;
+    out[4] = (int64_t)h[2]; out[5] = (int64_t)h[3];
     return PCAMM_OK;
 }
 
@@ -944,6 +962,7 @@ int pcamm_tune(const char* name, int32_t value) {
     if (n == "project_chunks_per_segment") { g_chunks_per_segment = value < 0 ? 0 : value; return PCAMM_OK; }
     if (n == "project_scan_slabs") { g_scan_slabs = value < 0 ? 0 : value; return PCAMM_OK; }
     if (n == "timeline") { g_timeline = value != 0; return PCAMM_OK; }
+    if (n == "grad_records") { g_grad_records = value != 0; return PCAMM_OK; }
     return invalid("unknown knob: " + n);
 }
 
@@ -972,7 +991,7 @@ int pcamm_time_kernel(pcamm_model* m, int32_t which, int32_t reps, float* ms_out
     CUDA_TRY(cudaEventRecord(m->ev0, st));
     for (int i = 0; i < reps; ++i) {
         if (which == 0)
-            launch_warp(q, G, m->fs, m->f0p, m->c.slots, m->time_slots, 1, m->vol, G.PV, m->occ);
+            launch_warp(q, G, m->fs, m->f0p, m->c.slots, m->time_slots, 1, m->vol, G.PV, m->occ, m->fs.grad_rec);
         else if (which == 1)
             launch_project(q, G, m->c, m->time_slots, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_NONE, 0, 0, 0);
         else

@@ -610,6 +610,106 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     tl_end(G.tl, TLK_GRAD);
 }
 
+// ---------------------------------------------------------------- one solve: the gather over the records
+//
+// For a single solve the streaming pass above is not needed at all: the warp kernel that wrote the
+// accepted candidate's trial volume had the eight taps of every voxel in registers and left a record
+// (x, y, z, G_j) for every voxel with G_j != 0 (stream.cuh GradRecords; warp.cu).  What remains of
+// a-4 is, per record: B_j by the voxel-driven detector gather (the same exact l_ij; or from the
+// backprojection volume of the ray-marching variant), u_kj from the fields (3 K scattered loads),
+// and acc_k += B_j (G_j . u_kj); per thread over its records, then warp -> block -> partial sums, all
+// in fixed order.  No V-sized gradient volume exists at any point, and the K+1 fields are streamed
+// once per line-search pass instead of once more per iteration.
+constexpr int GG_WARPS = 8;        // warps of a gather block
+constexpr int GG_THREADS = 32 * GG_WARPS;
+constexpr int GG_ROUND = 64;       // sub-tiles whose records a block flattens at a time
+
+// grid: as many blocks as the fused kernel has consumer groups (the same partial-sum slots).  Block
+// v takes sub-tiles v, v + grid, ...; their records are flattened (prefix of the counts, GG_ROUND
+// sub-tiles at a time) and dealt one per thread, so that every lane has work whatever the counts.
+template <int K>
+__global__ void __launch_bounds__(GG_THREADS, 4)
+k_grad_gather(const Geom G, const SolveState* __restrict__ solves, int* __restrict__ rec_base, long long n_sub, int cap,
+              const float* __restrict__ fields, const float* __restrict__ rL, const float4* __restrict__ utab,
+              const float2* __restrict__ vtab, const float* __restrict__ bvol, double* __restrict__ partials,
+              unsigned long long* __restrict__ visited) {
+    __shared__ double red[GG_WARPS][K];
+    __shared__ int s_pref[GG_ROUND + 1];
+    tl_begin(G.tl);
+    if (!needs_gradient(solves[0])) { tl_end(G.tl, TLK_GRAD); return; }    // uniform over the grid
+    const GradRecords rec = grad_records(rec_base, n_sub, n_sub * cap, solves[0].acc_slot);   // of the accepted candidate
+    const GatherView gv = make_gather_view(G, solves[0].view);
+    const float* __restrict__ u = fields + 3 * G.V;                          // u_1 .. u_K, planar, voxel units
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float acc[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) acc[k] = 0.f;
+    long long n_gathered = 0;
+    for (long long t0 = blockIdx.x; t0 < n_sub; t0 += (long long)gridDim.x * GG_ROUND) {
+        // the counts of this round's sub-tiles t0, t0 + grid, ... and their exclusive prefix
+        __syncthreads();
+        if (threadIdx.x < GG_ROUND) {
+            const long long t = t0 + (long long)threadIdx.x * gridDim.x;
+            int cnt = t < n_sub ? __ldcg(rec.count + t) : 0, incl = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += v;
+            }
+            s_pref[threadIdx.x + 1] = incl;                // per half of 32; the second half is shifted below
+            if (threadIdx.x == 0) s_pref[0] = 0;
+        }
+        __syncthreads();
+        const int half = s_pref[32];
+        __syncthreads();
+        if (threadIdx.x >= 32 && threadIdx.x < GG_ROUND) s_pref[threadIdx.x + 1] += half;
+        __syncthreads();
+        const int total = s_pref[GG_ROUND];
+        n_gathered += total;
+        for (int e = threadIdx.x; e < total; e += GG_THREADS) {
+            int lo = 0, hi = GG_ROUND;                      // sub-tile index i with pref[i] <= e < pref[i + 1]
+#pragma unroll
+            for (int step = 0; step < 6; ++step) {
+                const int mid = (lo + hi) >> 1;
+                if (s_pref[mid] <= e) lo = mid; else hi = mid;
+            }
+            const long long idx = (t0 + (long long)lo * gridDim.x) * cap + (e - s_pref[lo]);
+            const int xy = __ldcg(rec.xy + idx), z = __ldcg(rec.z + idx);
+            const float gx = __ldcg(rec.g + idx), gy = __ldcg(rec.g + rec.plane + idx), gz = __ldcg(rec.g + 2 * rec.plane + idx);
+            const int x = xy & 0xffff, y = xy >> 16;
+            const long long lin = ((long long)z * G.ny + y) * G.nx + x;
+            float q[K];
+#pragma unroll
+            for (int k = 0; k < K; ++k)                     // q_kj = G_j . u_kj (fields in voxel units: no 1/h, reading B4)
+                q[k] = gx * __ldg(u + (3 * k) * G.V + lin) + gy * __ldg(u + (3 * k + 1) * G.V + lin) + gz * __ldg(u + (3 * k + 2) * G.V + lin);
+            float Bj;
+            if (bvol) Bj = __ldg(bvol + lin);
+            else {
+                const float xw = G.cx + ((float)x - 0.5f * (G.nx - 1)) * G.hx;
+                const float yw = G.cy + ((float)y - 0.5f * (G.ny - 1)) * G.hy;
+                const float zw = G.cz + ((float)z - 0.5f * (G.nz - 1)) * G.hz;
+                Bj = gather_voxel(G, gv, rL, utab, vtab, xw, yw, zw);
+            }
+#pragma unroll
+            for (int k = 0; k < K; ++k) acc[k] = fmaf(Bj, q[k], acc[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const double sv = warp_sum((double)acc[k]);
+        if (lane == 0) red[warp][k] = sv;
+    }
+    __syncthreads();
+    if (threadIdx.x < K) {
+        double tot = 0.0;
+#pragma unroll
+        for (int i = 0; i < GG_WARPS; ++i) tot += red[i][threadIdx.x];
+        partials[(long long)blockIdx.x * KMAX + threadIdx.x] = tot;
+    }
+    if (threadIdx.x == 0 && visited) atomicAdd(visited + 2, (unsigned long long)n_gathered);
+    tl_end(G.tl, TLK_GRAD);
+}
+
 // The cell map of FieldStream: one thread per interpolation cell.
 __global__ void __launch_bounds__(256)
 k_build_cellmap(const Geom G, const float* __restrict__ f0, unsigned char* __restrict__ cellmap) {
@@ -664,6 +764,12 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     const int grid = grad_grid(G, fs);
     // the flags cost a few dependent loads per launch: only where a CTA has tiles enough to win them back
     const unsigned* skip_table = tile_count(G, TileZ<K>::value) >= fs.skip_min_tiles_per_sm * (long long)fs.n_sm ? fs.cell_integral : nullptr;
+    if (B == 1 && fs.grad_rec) {                        // one solve: the warp kernel left the records, gather only
+        const long long n_sub = tile_count(G, TileZ<K>::value) * GROUP_WARPS;
+        q.launch(k_grad_gather<K>, dim3(grid * GNG), dim3(GG_THREADS), 0, G, (const SolveState*)c.solves, fs.grad_rec, n_sub,
+                 TX * TileZ<K>::value / GROUP_WARPS, fs.fields, rL, utab, vtab, bvol, c.grad_part, fs.visited);
+        return;
+    }
     if (B == 1) {
         q.launch(skip_table ? k_grad_tma<K, true, H, true> : k_grad_tma<K, true, H, false>, dim3(grid), dim3(GTHREADS), smem, field_map<K>(fs), half_map<K>(fs), fs.scale, fs.fmax, skip_table, G, f0,
                  fs.cellmap, c, 0, 1, rL, utab, vtab, bvol, fs.visited);

@@ -107,8 +107,10 @@ struct Seq {
 // f[s] = warp(f0, xbar + U w[s]) for every active slot; ray_layout: the z-fastest layout the
 // projector reads (slot stride G.PV), else the standard [z][y][x] (slot stride G.V).
 // occ: occupancy of the volumes written (ray layout only; common.cuh), else NULL
+// rec: base of the slots' gradient records (stream.cuh GradRecords; written with the ray layout
+// only) or NULL
 void launch_warp(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
-                 int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ);
+                 int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ, int* rec);
 
 // ---- a-2 (project.cu)
 int project_blocks(const Geom& G);

@@ -221,6 +221,33 @@ constexpr int SKIP_MIN_TILES_PER_SM = 12;
 // bound must not wrap the int box arithmetic of the tile flags: it then simply covers the volume).
 __device__ __forceinline__ int reach_of(float dmax) { return (int)ceilf(fminf(dmax * 1.0001f + 0.001f, 1048576.f)); }
 
+// Records of the voxels with a non-zero image gradient (single-solve path; warp.cu writes them,
+// gradient.cu k_grad_gather reads them).  The warp kernel has, for every voxel of a trial volume,
+// the eight taps of f0 in registers: their differences are G_j = df_j / dx_j, exactly what a-4 needs
+// at the same coefficients.  So it writes, per trial slot, one record (x, y, z, G_j) for every voxel
+// with G_j != 0 (boundary voxels: 6 % at C2), and the gradient of the accepted candidate needs no
+// second pass over the K+1 fields: only B_j and u_kj at the recorded voxels.
+// Layout per slot: a tile is cut into GROUP_WARPS sub-tiles (the voxels one warp of the consumer
+// group handles: TX x TZ / GROUP_WARPS = `cap` of them, so a sub-tile cannot overflow); sub-tile s
+// owns records s cap .. s cap + count[s] - 1, in the fixed order (row, lane).
+struct GradRecords {
+    int* count;        // [n_sub]
+    int* xy;           // [plane]  x | y << 16
+    int* z;            // [plane]
+    float* g;          // [3][plane]
+    long long plane;   // n_sub * cap
+};
+__host__ __device__ __forceinline__ long long grad_record_words(long long n_sub, long long plane) { return n_sub + 5 * plane; }
+__host__ __device__ __forceinline__ GradRecords grad_records(int* base, long long n_sub, long long plane, int slot) {
+    GradRecords r;
+    r.count = base + (long long)slot * grad_record_words(n_sub, plane);
+    r.xy = r.count + n_sub;
+    r.z = r.xy + plane;
+    r.g = reinterpret_cast<float*>(r.z + plane);
+    r.plane = plane;
+    return r;
+}
+
 // What the streaming kernels need to know about the model's fields.
 struct FieldStream {
     const float* fields = nullptr;   // [3(K+1)][V]: xbar's planes, then u_1 .. u_K
@@ -243,6 +270,8 @@ struct FieldStream {
     const unsigned* cell_integral = nullptr;
     FieldMax fmax = {};
     int skip_min_tiles_per_sm = SKIP_MIN_TILES_PER_SM;     // geometry.tile_skipping: 0 always, INT_MAX never
+    // gradient records of the trial slots (GradRecords; NULL: none, the gradient makes its own pass)
+    int* grad_rec = nullptr;
     // measurement: tiles whose fields the warp / gradient kernels really loaded, summed over the
     // launches since the host last cleared them ([0] warp, [1] gradient; one atomic per consumer group)
     unsigned long long* visited = nullptr;

@@ -137,13 +137,14 @@ constexpr size_t warp_smem_bytes() {
 }
 
 // H: u_k stored in half (stream.cuh FieldRing, FieldScale).  SKIP: with the tile flags of reading
-// B8 (f0_integral != NULL); without them the loads simply follow the tile counter.
-template <int K, bool RAY, bool H, bool SKIP>
+// B8 (f0_integral != NULL); without them the loads simply follow the tile counter.  REC: also
+// writes the gradient records of every slot (stream.cuh GradRecords; rec = their base).
+template <int K, bool RAY, bool H, bool SKIP, bool REC>
 __global__ void __launch_bounds__(WarpThreads<K>::value, 1)
 k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUtensorMap umap, const FieldScale scale,
            const FieldMax fmax, const unsigned* __restrict__ f0_integral, const Geom G, const float* __restrict__ f0,
            const SlotState* __restrict__ slots, int nslots, float* __restrict__ vol_out, long long slot_stride,
-           unsigned char* __restrict__ occ, unsigned long long* __restrict__ visited) {
+           unsigned char* __restrict__ occ, unsigned long long* __restrict__ visited, int* __restrict__ rec) {
     constexpr int P = 3 * (K + 1), WTZ = TileZ<K>::value, WROWS = WTZ / GROUP_WARPS;
     constexpr int WNG = WarpGroups<K>::value;
     using Ring = FieldRing<P, WTZ, WNG, WarpStages<K, H>::value, H>;
@@ -179,6 +180,8 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     }
     __syncthreads();
     const long long n_tiles = tile_count(G, WTZ);
+    const long long n_sub = n_tiles * GROUP_WARPS, rec_plane = n_tiles * (TX * WTZ);
+    constexpr int SUBCAP = TX * WROWS;                     // records a sub-tile (one warp's voxels of a tile) can hold
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int last_active = -1;                                  // the last slot that reads the stage
     for (int i = 0; i < nslots; ++i)
@@ -240,6 +243,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     if (leader)
         for (int i = 0; i < SPG; ++i) issue_next();
     int n_loaded = 0, j = 0;                               // loads this group has consumed; its tile counter
+    int n_written = 0;                                     // records this warp wrote (REC)
     for (long long t = Ring::tile_of(group, 0); t < n_tiles; t += (long long)WNG * gridDim.x, ++j) {
         const bool air = tile_is_air(j);                   // uniform over the group
         if (air) {                                         // zeros, straight to their places
@@ -247,6 +251,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
             for (int sl = 0; sl < nslots; ++sl) {
                 if (!s_active[sl]) continue;
                 float* out = vol_out + (long long)sl * slot_stride;
+                if (REC && lane == 0) grad_records(rec, n_sub, rec_plane, sl).count[t * GROUP_WARPS + tw] = 0;   // f0 = 0 all around: G = 0
                 if (!RAY) {
 #pragma unroll
                     for (int r = 0; r < WROWS; ++r) {
@@ -311,6 +316,34 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                 for (int r = 0; r < WROWS; ++r) gather8(G, f0, taps[r], cv[r]);    // 8 WROWS gathers in flight
 #pragma unroll
                 for (int r = 0; r < WROWS; ++r) val[r] = combine8(taps[r], cv[r]);
+                if (REC) {
+                    // G_j from the same taps (reading A6): the voxels of this warp with
+                    // G_j != 0, in the order (row, lane), into its sub-tile's records
+                    const GradRecords R = grad_records(rec, n_sub, rec_plane, sl);
+                    const long long sub = t * GROUP_WARPS + tw, base = sub * SUBCAP;
+                    int n_rec = 0;
+#pragma unroll
+                    for (int r = 0; r < WROWS; ++r) {
+                        const int z = c.z0 + tw + GROUP_WARPS * r;
+                        // a cell whose eight taps are equal has G = 0 exactly: most warps stop here
+                        const bool varies = (cv[r][1] != cv[r][0] || cv[r][2] != cv[r][0] || cv[r][3] != cv[r][0] || cv[r][4] != cv[r][0] ||
+                                             cv[r][5] != cv[r][0] || cv[r][6] != cv[r][0] || cv[r][7] != cv[r][0]) && x < G.nx && z < G.nz;
+                        if (!__any_sync(0xffffffffu, varies)) continue;          // uniform over the warp
+                        float gx, gy, gz;
+                        grad8(taps[r], cv[r], &gx, &gy, &gz);
+                        const bool active = varies && (gx != 0.f || gy != 0.f || gz != 0.f);
+                        const unsigned mask = __ballot_sync(0xffffffffu, active);
+                        if (active) {
+                            const long long pos = base + n_rec + __popc(mask & ((1u << lane) - 1u));
+                            R.xy[pos] = x | c.y << 16;
+                            R.z[pos] = z;
+                            R.g[pos] = gx; R.g[R.plane + pos] = gy; R.g[2 * R.plane + pos] = gz;
+                        }
+                        n_rec += __popc(mask);
+                    }
+                    if (lane == 0) R.count[sub] = n_rec;
+                    n_written += n_rec;
+                }
                 }
                 if (!RAY) {
 #pragma unroll
@@ -346,12 +379,13 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
         }
     }
     if (leader && visited) atomicAdd(visited, (unsigned long long)(SKIP ? n_loaded : j));
+    if (REC && lane == 0 && visited && n_written) atomicAdd(visited + 3, (unsigned long long)n_written);
     tl_end(G.tl, TLK_WARP);
 }
 
-template <int K, bool RAY, bool H>
+template <int K, bool RAY, bool H, bool REC>
 void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots,
-                int nslots, float* vol_out, long long slot_stride, unsigned char* occ) {
+                int nslots, float* vol_out, long long slot_stride, unsigned char* occ, int* rec) {
     static DeviceOnce configured;
     constexpr size_t smem = warp_smem_bytes<K, H>();
     const CUtensorMap& fmap = field_map<K>(fs);
@@ -359,9 +393,9 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     const int n_sm = fs.n_sm;
     {
         const cudaError_t e = configured.run([&] {
-            cudaError_t r = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaError_t r = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, true, REC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (r == cudaSuccess)
-                r = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                r = cudaFuncSetAttribute(k_warp_tma<K, RAY, H, false, REC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             return r;
         });
         if (e != cudaSuccess) { q.err = e; return; }
@@ -375,24 +409,28 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
         float* out = vol_out + (long long)s0 * slot_stride;
         unsigned char* oc = occ ? occ + (long long)s0 * G.OCC : occ;
         if (table)
-            q.launch(k_warp_tma<K, RAY, H, true>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
-                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited);
+            q.launch(k_warp_tma<K, RAY, H, true, REC>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
+                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited, rec);
         else
-            q.launch(k_warp_tma<K, RAY, H, false>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
-                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited);
+            q.launch(k_warp_tma<K, RAY, H, false, REC>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
+                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited, rec);
     }
 }
 
 template <int K>
 void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
-              int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ) {
+              int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ, int* rec) {
     if (fs.use_tma) {
+        // records only with the ray layout (the solve's trial volumes) and at most SLOT_CACHE slots in one launch
+        const bool with_rec = rec && ray_layout && nslots <= SLOT_CACHE;
         if (fs.half_u) {
-            if (ray_layout) launch_tma<K, true, true>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ);
-            else launch_tma<K, false, true>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ);
+            if (with_rec) launch_tma<K, true, true, true>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ, rec);
+            else if (ray_layout) launch_tma<K, true, true, false>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ, nullptr);
+            else launch_tma<K, false, true, false>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ, nullptr);
         } else {
-            if (ray_layout) launch_tma<K, true, false>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ);
-            else launch_tma<K, false, false>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ);
+            if (with_rec) launch_tma<K, true, false, true>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ, rec);
+            else if (ray_layout) launch_tma<K, true, false, false>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ, nullptr);
+            else launch_tma<K, false, false, false>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ, nullptr);
         }
         return;
     }
@@ -406,10 +444,10 @@ void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, con
 }  // namespace
 
 void launch_warp(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
-                 int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ) {
+                 int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ, int* rec) {
     switch (G.K) {
 #define PCAMM_CASE(KK) \
-    case KK: launch_k<KK>(q, G, fs, f0, slots, nslots, ray_layout, vol_out, slot_stride, occ); break;
+    case KK: launch_k<KK>(q, G, fs, f0, slots, nslots, ray_layout, vol_out, slot_stride, occ, rec); break;
         PCAMM_CASE(1) PCAMM_CASE(2) PCAMM_CASE(3) PCAMM_CASE(4)
         PCAMM_CASE(5) PCAMM_CASE(6) PCAMM_CASE(7) PCAMM_CASE(8)
 #undef PCAMM_CASE

@@ -13,6 +13,9 @@ from tests.util import geom, smooth_model
 pytestmark = pytest.mark.gpu
 
 
+_FIELDS = []          # (f0, xbar, u) of the last _setup, for the oracle
+
+
 def _setup(tile_skipping=1, **kw):
     g = geom(nx=96, ny=70, nz=64, h=(2.0, 2.0, 2.0), K=3, nu=96, nv=64, pitch=(3.4, 2.6))
     f0, xbar, u, scale = smooth_model(g, seed=5, disp_vox=1.0)
@@ -20,30 +23,75 @@ def _setup(tile_skipping=1, **kw):
     body = ((xx - 60) / 20.0) ** 2 + ((yy - 30) / 14.0) ** 2 + ((zz - 30) / 18.0) ** 2 <= 1.0
     f0 = np.where(body, 0.5 + f0, 0.0).astype(np.float32)            # a body in a lot of air: tiles to skip
     m = make_model(g, f0, xbar, u, tile_skipping=tile_skipping, **kw)
+    _FIELDS.append((f0, xbar, u))
     w = (0.4 * scale * np.array([1.0, -0.6, 0.8])).astype(np.float32)
     _, p = oracle.evaluate(g, f0, xbar, u, w, 0.9)
     return g, m, w, to_dev(p.astype(np.float32))
 
 
 def test_tile_counters_count_the_tiles_the_timed_launches_loaded():
+    import paper_1004_0014_b200 as pc
+    # default: the warp kernel leaves gradient records, the gradient of one solve gathers over them
     g, m, w, y = _setup(tile_skipping=1)
     m.eval(y, 0.9, w, 1.0, 0.0, want_proj=False)
     m.tile_counts(reset=True)
     m.time_kernel(0, 5)
-    warp_tiles, grad_tiles, total, vox = m.tile_counts(reset=True)
+    warp_tiles, grad_tiles, total, vox, gathered, written = m.tile_counts(reset=True)
     assert vox == 32 * 32 and total == 3 * g.ny * 2
-    assert grad_tiles == 0 and warp_tiles % 5 == 0 and 0 < warp_tiles // 5 < total
+    assert grad_tiles == 0 and gathered == 0 and warp_tiles % 5 == 0 and 0 < warp_tiles // 5 < total
+    assert written % 5 == 0 and 0 < written // 5 < g.V
     m.time_kernel(2, 4)
-    warp_tiles, grad_tiles, _, _ = m.tile_counts(reset=True)
-    assert warp_tiles == 0 and grad_tiles % 4 == 0 and 0 < grad_tiles // 4 < total
-    # with skipping off every tile is loaded
-    g2, m2, w2, y2 = _setup(tile_skipping=2)
-    m2.eval(y2, 0.9, w2, 1.0, 0.0, want_proj=False)
-    m2.tile_counts(reset=True)
-    m2.time_kernel(0, 3)
-    m2.time_kernel(2, 3)
-    a, b, total2, _ = m2.tile_counts()
-    assert a == 3 * total2 and b == 3 * total2
+    warp_tiles, grad_tiles, _, _, gathered, w2 = m.tile_counts(reset=True)
+    assert warp_tiles == 0 and grad_tiles == 0 and w2 == 0
+    assert gathered == 4 * (written // 5)                       # the records of the accepted slot, all of them
+    # the number of records is the number of voxels with G_j != 0 (oracle: the warped volume's gradient)
+    # (float against double: a voxel whose G cancels to zero in one of the two is counted differently)
+    Gf = oracle.warp_grad(g, *_FIELDS[-1], w)
+    n_ref = int(np.count_nonzero(np.any(np.asarray(Gf).reshape(3, -1) != 0, axis=0)))
+    assert abs(written // 5 - n_ref) <= 0.002 * n_ref and n_ref < 0.5 * g.V
+    try:
+        pc.tune("grad_records", 0)                              # the gradient streams the fields itself
+        g, m, w, y = _setup(tile_skipping=1)
+        m.eval(y, 0.9, w, 1.0, 0.0, want_proj=False)
+        m.tile_counts(reset=True)
+        m.time_kernel(0, 5)
+        warp_tiles, grad_tiles, total, vox, gathered, written = m.tile_counts(reset=True)
+        assert grad_tiles == 0 and written == 0 and warp_tiles % 5 == 0 and 0 < warp_tiles // 5 < total
+        m.time_kernel(2, 4)
+        warp_tiles, grad_tiles, _, _, gathered, _ = m.tile_counts(reset=True)
+        assert warp_tiles == 0 and gathered == 0 and grad_tiles % 4 == 0 and 0 < grad_tiles // 4 < total
+        # with skipping off every tile is loaded
+        g2, m2, w2, y2 = _setup(tile_skipping=2)
+        m2.eval(y2, 0.9, w2, 1.0, 0.0, want_proj=False)
+        m2.tile_counts(reset=True)
+        m2.time_kernel(0, 3)
+        m2.time_kernel(2, 3)
+        a, b, total2 = m2.tile_counts()[:3]
+        assert a == 3 * total2 and b == 3 * total2
+    finally:
+        pc.tune("grad_records", 1)
+
+
+def test_gradient_from_records_and_streamed_gradient_agree():
+    """pcamm_tune("grad_records"): the same a-4 either from the records the warp kernel left or by a pass of
+    its own over the fields; the sums differ in order only."""
+    import paper_1004_0014_b200 as pc
+    g, m, w, y = _setup(max_candidates=2)
+    J1, g1, fit1, _ = m.eval(y, 0.9, 0.7 * w, 0.95, 0.01)
+    r1 = m.reconstruct(y, 0.9, np.zeros(3, np.float32), pc.Opts(max_iter=5), trace=True)
+    f1 = m.reconstruct(y, 0.9, np.zeros(3, np.float32), pc.Opts(max_iter=5, batched_linesearch=2), trace=True)
+    try:
+        pc.tune("grad_records", 0)
+        g, m0, w, y = _setup()
+        J0, g0, fit0, _ = m0.eval(y, 0.9, 0.7 * w, 0.95, 0.01)
+        r0 = m0.reconstruct(y, 0.9, np.zeros(3, np.float32), pc.Opts(max_iter=5), trace=True)
+    finally:
+        pc.tune("grad_records", 1)
+    assert J1 == J0 and fit1 == fit0
+    assert np.linalg.norm(g1 - g0) <= 1e-5 * np.linalg.norm(g0)
+    assert np.array_equal(r1.backtracks, r0.backtracks) and np.array_equal(f1.backtracks, r0.backtracks)
+    assert np.linalg.norm(r1.w - r0.w) <= 1e-4 * np.linalg.norm(r0.w)
+    assert np.array_equal(f1.w, r1.w)                           # reading B7 holds with the records too
 
 
 def test_timing_over_two_candidate_slots():

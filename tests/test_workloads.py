@@ -155,3 +155,7 @@ def test_bench_moved_bytes_model():
     assert bench.moved_bytes(cfg, 1, {"warp": n_tiles, "gradient": n_tiles}, vox)["warp"] == (12 + 18 + 8) * cfg.V
 
 
+    # gradient records (one solve): the warp kernel writes them, the gradient gathers over the accepted slot's
+    rec = bench.moved_bytes(cfg, 0, {"warp": n_tiles, "gradient": 0}, vox, {"written": 2000.0, "gathered": 1000.0}, n_tiles)
+    assert rec["warp"] == 56 * cfg.V + 20 * 2000 + 32 * n_tiles
+    assert rec["gradient"] == (20 + 12 * cfg.K) * 1000 + 32 * n_tiles + 4 * cfg.npix

@@ -92,7 +92,7 @@ def algorithmic_bytes(cfg, field_storage=0):
             "gradient": (fields + 4) * V + 4 * npix}
 
 
-RECORD_BYTES = 20       # one gradient record: x | y << 16, z, G_x, G_y, G_z (stream.cuh GradRecords)
+RECORD_BYTES = 48       # one gradient record: packed voxel coordinates, three fractions, eight taps of f0 (stream.cuh GradRecord)
 
 
 def moved_bytes(cfg, field_storage, tiles_loaded, vox_per_tile, records=None, n_tiles=0):
@@ -100,8 +100,8 @@ def moved_bytes(cfg, field_storage, tiles_loaded, vox_per_tile, records=None, n_
     kernels, pcamm_tile_counts; reading B8: tiles that can only see zeros / constant cells are skipped).
     A loaded tile costs its fields and its f0 gathers (4 B per voxel, counted once); the warp kernel
     writes every voxel of the volume (skipped tiles as zeros), the gradient kernel reads the residual.
-    With gradient records (the default for one solve) the warp kernel also writes 20 B per voxel with
-    G_j != 0 and a count per sub-tile (8 per tile); the gradient reads those and 12 K bytes of u per record
+    With gradient records (the default for one solve) the warp kernel also writes 48 B per voxel with
+    a non-constant cell and a count per sub-tile (8 per tile); the gradient reads those and 12 K bytes of u per record
     (scattered 4-byte loads: the sectors they touch are not counted) and the residual."""
     fields = field_bytes_per_voxel(cfg, field_storage)
     out = {"warp": tiles_loaded["warp"] * vox_per_tile * (fields + 4) + 4 * cfg.V,
@@ -430,7 +430,7 @@ def run_ours(args, cfg, rank, local_rank, world):
             "kernel": "k_grad_gather", "records_per_launch": records["gathered"],
             "records_per_voxel": records["gathered"] / cfg.V,
             "note": "a gather over the records the warp kernel left for the voxels with G_j != 0 (DESIGN.md section 5b): "
-                    "latency- and sector-bound scattered loads, not a stream; moved_bytes counts 20 B per record, "
+                    "latency- and sector-bound scattered loads, not a stream; moved_bytes counts 48 B per record, "
                     "12 K B of u per record, the counts and the residual, not the 32-byte sectors touched"})
     # the projector's volume was just written and is L2-resident: it is not an HBM kernel.
     # What it does per launch: one pass over (detector column, slab, level) and one look-up per z crossing.

@@ -279,7 +279,7 @@ int pcamm_time_slots(pcamm_model* model, int32_t nslots, const float* w_host, vo
  * voxels, all 3(K+1) field planes); out[2] = tiles of the whole volume (0: the generic kernels are
  * in use, which visit everything and count nothing).  With gradient records (pcamm_tune
  * "grad_records", the default for a single solve) the gradient loads no field tiles: out[4] = records
- * its gather went through, out[5] = records the warp kernel wrote (20 bytes each), same launches.
+ * its gather went through, out[5] = records the warp kernel wrote (48 bytes each), same launches.
  * reset != 0 clears the counters. */
 int pcamm_tile_counts(pcamm_model* model, int32_t reset, int64_t* out /* [6] */, void* stream);
 
@@ -289,9 +289,13 @@ int pcamm_tile_counts(pcamm_model* model, int32_t reset, int64_t* out /* [6] */,
  *                                 (0 = automatic, the default);
  *   "project_scan_slabs"          slabs per scan of the projector: 1, 2 or 4 (0 = automatic);
  *   "grad_records"                0: the gradient of a single solve makes its own pass over the K+1 fields
- *                                 (1, the default: the warp kernel leaves records of the voxels with a
- *                                 non-zero image gradient and the gradient is a gather over them;
- *                                 DESIGN.md section 5a);
+ *                                 (1, the default: the warp kernel leaves records of the voxels whose
+ *                                 interpolation cell is not constant and the gradient is a gather over
+ *                                 them);
+ *   "pdl"                         0: plain kernel -> kernel edges in the solve graphs (1, the default:
+ *                                 programmatic dependent launch, the next kernel's blocks are launched
+ *                                 while the previous kernel drains and wait for its completion on the
+ *                                 device; same order of memory effects);
  *   "timeline"                    1: models created from now on record, inside their kernels, the
  *                                 start and end of every kernel of a solve (pcamm_timeline). */
 int pcamm_tune(const char* name, int32_t value);

@@ -18,6 +18,7 @@ namespace pcamm {
 static thread_local std::string g_error;
 static thread_local long long g_launches = 0;
 int g_timeline = 0;
+int g_pdl = 1;            // pcamm_tune "pdl": programmatic kernel -> kernel edges in the solve graphs built from then on
 int g_grad_records = 1;   // pcamm_tune "grad_records": 0 = the gradient of a single solve makes its own pass over the fields
 
 void set_error(const std::string& msg) { g_error = msg; }
@@ -308,6 +309,7 @@ int get_graph(pcamm_model* m, int B, int C, GraphRec** out) {
     CUDA_TRY(cudaGraphConditionalHandleCreate(&h_loop, rec.graph, 0, cudaGraphCondAssignDefault));
     Seq q;
     q.graph = rec.graph;
+    q.pdl = g_pdl != 0;
     seq_head(m, q, B, C, h_loop, 1);
     Seq body = q.add_while(h_loop);             // iterations and their line searches
     seq_body(m, body, B, C, h_loop, 1);
@@ -538,6 +540,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     G.cx = g->cx; G.cy = g->cy; G.cz = g->cz;
     G.lox = (double)g->cx - ex; G.loy = (double)g->cy - ey; G.loz = (double)g->cz - ez;
     G.ihz_d = 1.0 / (double)g->hz; G.Szi = (0.0 - G.loz) / (double)g->hz;
+    tile_multipliers(G);
     G.projector = g->projector;
     G.rm_step_mm = (g->ray_step_vox > 0.f ? g->ray_step_vox : 0.5f) * std::fmin(g->hx, std::fmin(g->hy, g->hz));
     G.K = g->K; G.nu = g->nu; G.nv = g->nv; G.npix = g->nu * g->nv;
@@ -557,7 +560,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         m->fs.n_sm = n_sm > 0 ? n_sm : 1;
         FieldStream generic = m->fs, tma = m->fs;
         generic.use_tma = false; tma.use_tma = true;
-        m->c.grad_blocks = std::max(grad_blocks(G, generic), grad_blocks(G, tma));
+        m->c.grad_blocks = std::max(std::max(grad_blocks(G, generic), grad_blocks(G, tma)), grad_gather_blocks(G, m->fs));
     }
     m->trav_cap = G.nx + G.ny + G.nz + 8;
     cudaError_t e = cudaSuccess;
@@ -744,8 +747,8 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         m->fs.skip_min_tiles_per_sm = g->tile_skipping == 1 ? 0 : (g->tile_skipping == 2 ? (1 << 30) : SKIP_MIN_TILES_PER_SM);
     }
     m->c.grad_blocks = grad_blocks(G, m->fs);
-    if (m->fs.use_tma && g_grad_records) {
-        // gradient records of the trial slots of a single solve (stream.cuh GradRecords): 20 bytes per voxel and slot
+    if (m->fs.use_tma && g_grad_records && G.nx <= RECORD_MAX_XY && G.ny <= RECORD_MAX_XY && G.nz <= RECORD_MAX_Z) {
+        // gradient records of the trial slots of a single solve (stream.cuh GradRecords): 48 bytes per voxel and slot
         const int tz = G.K <= PCAMM_TZ_SMALL_K ? 32 : 16;                     // TileZ<K>
         const long long n_tiles = tile_count(G, tz), n_sub = n_tiles * GROUP_WARPS, plane = n_tiles * (TX * tz);
         const size_t words = (size_t)grad_record_words(n_sub, plane) * (size_t)Cmax;
@@ -963,6 +966,7 @@ int pcamm_tune(const char* name, int32_t value) {
     if (n == "project_scan_slabs") { g_scan_slabs = value < 0 ? 0 : value; return PCAMM_OK; }
     if (n == "timeline") { g_timeline = value != 0; return PCAMM_OK; }
     if (n == "grad_records") { g_grad_records = value != 0; return PCAMM_OK; }
+    if (n == "pdl") { g_pdl = value != 0; return PCAMM_OK; }
     return invalid("unknown knob: " + n);
 }
 

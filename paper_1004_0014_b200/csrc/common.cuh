@@ -34,8 +34,20 @@ __device__ __forceinline__ unsigned long long global_timer_ns() {
     return t;
 }
 __device__ __forceinline__ bool tl_first_thread() { return (threadIdx.x | threadIdx.y | threadIdx.z) == 0; }
+// Programmatic dependent launch (internal.h Seq, pcamm_tune "pdl"): inside the solve graph a kernel
+// may be launched, and its blocks become resident, while its predecessor drains; the blocks wait here
+// until the predecessor has completed and its writes are visible.  Nothing a previous kernel wrote
+// may be read, and nothing it read may be overwritten, before this; every kernel of the graph calls
+// it first thing (through tl_begin), so the order of all memory effects is that of the plain graph.
+// The kernel's own dependents may be launched at once: they wait the same way.  (Launched without a
+// programmatic edge both instructions do nothing.)
+__device__ __forceinline__ void grid_dependency_wait() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
 // at the top of a kernel, by every block
 __device__ __forceinline__ void tl_begin(Timeline* tl) {
+    grid_dependency_wait();
     if (tl && tl_first_thread()) {
         const unsigned e = *(volatile unsigned*)&tl->n;
         if (e < TL_CAP) atomicMin(&tl->t0[e], global_timer_ns());
@@ -77,6 +89,7 @@ struct Geom {
     int K;
     int nu, nv, npix;
     float pu, pv, sad, sdd, off_u, off_v;
+    unsigned tile_mx, tile_my; // ceil(2^32 / tiles along x), ceil(2^32 / ny): tile index -> coordinates without divisions (stream.cuh tile_coord; 0: divide)
     int projector;            // 0: Siddon's exact path lengths (project.cu), 1: fixed-step ray marching (raymarch.cu)
     float rm_step_mm;         // nominal step of the ray marching
 };

@@ -622,19 +622,22 @@ k_grad_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
 // once per line-search pass instead of once more per iteration.
 constexpr int GG_WARPS = 8;        // warps of a gather block
 constexpr int GG_THREADS = 32 * GG_WARPS;
-constexpr int GG_ROUND = 64;       // sub-tiles whose records a block flattens at a time
+constexpr int GG_ROUND = GG_THREADS;   // sub-tiles whose records a block flattens at a time: one count per thread
+// blocks per SM (64 registers per thread for K <= 4, 80 beyond): the kernel lives on warps in flight
+__host__ __device__ constexpr int gather_per_sm(int K) { return K <= 4 ? 4 : 3; }
 
-// grid: as many blocks as the fused kernel has consumer groups (the same partial-sum slots).  Block
-// v takes sub-tiles v, v + grid, ...; their records are flattened (prefix of the counts, GG_ROUND
-// sub-tiles at a time) and dealt one per thread, so that every lane has work whatever the counts.
+// Block v takes sub-tiles v, v + grid, ...; their records are flattened (prefix of the counts,
+// GG_ROUND sub-tiles at a time: usually all of the block's) and dealt one per thread, so that every
+// lane has work whatever the counts.  One partial sum per block and k.
 template <int K>
-__global__ void __launch_bounds__(GG_THREADS, 4)
+__global__ void __launch_bounds__(GG_THREADS, gather_per_sm(K))
 k_grad_gather(const Geom G, const SolveState* __restrict__ solves, int* __restrict__ rec_base, long long n_sub, int cap,
               const float* __restrict__ fields, const float* __restrict__ rL, const float4* __restrict__ utab,
               const float2* __restrict__ vtab, const float* __restrict__ bvol, double* __restrict__ partials,
               unsigned long long* __restrict__ visited) {
     __shared__ double red[GG_WARPS][K];
     __shared__ int s_pref[GG_ROUND + 1];
+    __shared__ int s_wsum[GG_WARPS];
     tl_begin(G.tl);
     if (!needs_gradient(solves[0])) { tl_end(G.tl, TLK_GRAD); return; }    // uniform over the grid
     const GradRecords rec = grad_records(rec_base, n_sub, n_sub * cap, solves[0].acc_slot);   // of the accepted candidate
@@ -647,36 +650,47 @@ k_grad_gather(const Geom G, const SolveState* __restrict__ solves, int* __restri
     long long n_gathered = 0;
     for (long long t0 = blockIdx.x; t0 < n_sub; t0 += (long long)gridDim.x * GG_ROUND) {
         // the counts of this round's sub-tiles t0, t0 + grid, ... and their exclusive prefix
-        __syncthreads();
-        if (threadIdx.x < GG_ROUND) {
-            const long long t = t0 + (long long)threadIdx.x * gridDim.x;
-            int cnt = t < n_sub ? __ldcg(rec.count + t) : 0, incl = cnt;
+        const long long t = t0 + (long long)threadIdx.x * gridDim.x;
+        int incl = t < n_sub ? __ldcg(rec.count + t) : 0;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int v = __shfl_up_sync(0xffffffffu, incl, o);
-                if (lane >= o) incl += v;
-            }
-            s_pref[threadIdx.x + 1] = incl;                // per half of 32; the second half is shifted below
-            if (threadIdx.x == 0) s_pref[0] = 0;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
         }
+        if (lane == 31) s_wsum[warp] = incl;
+        __syncthreads();                                   // (every thread is done with the previous round's prefix)
+        int before = 0, total = 0;
+#pragma unroll
+        for (int i = 0; i < GG_WARPS; ++i) {
+            const int v = s_wsum[i];
+            before += i < warp ? v : 0;
+            total += v;
+        }
+        s_pref[threadIdx.x + 1] = before + incl;
+        if (threadIdx.x == 0) s_pref[0] = 0;
         __syncthreads();
-        const int half = s_pref[32];
-        __syncthreads();
-        if (threadIdx.x >= 32 && threadIdx.x < GG_ROUND) s_pref[threadIdx.x + 1] += half;
-        __syncthreads();
-        const int total = s_pref[GG_ROUND];
         n_gathered += total;
         for (int e = threadIdx.x; e < total; e += GG_THREADS) {
             int lo = 0, hi = GG_ROUND;                      // sub-tile index i with pref[i] <= e < pref[i + 1]
 #pragma unroll
-            for (int step = 0; step < 6; ++step) {
+            for (int step = 0; step < 8; ++step) {
                 const int mid = (lo + hi) >> 1;
                 if (s_pref[mid] <= e) lo = mid; else hi = mid;
             }
             const long long idx = (t0 + (long long)lo * gridDim.x) * cap + (e - s_pref[lo]);
-            const int xy = __ldcg(rec.xy + idx), z = __ldcg(rec.z + idx);
-            const float gx = __ldcg(rec.g + idx), gy = __ldcg(rec.g + rec.plane + idx), gz = __ldcg(rec.g + 2 * rec.plane + idx);
-            const int x = xy & 0xffff, y = xy >> 16;
+            const int4* rp = reinterpret_cast<const int4*>(rec.r + idx);             // one 48-byte record
+            const int4 rw = __ldcg(rp), c03 = __ldcg(rp + 1), c47 = __ldcg(rp + 2);
+            const int x = record_x(rw.x), y = record_y(rw.x), z = record_z(rw.x);
+            // G_j from the taps and fractions the warp kernel had (trilinear.cuh: the same arithmetic)
+            Taps tp;
+            tp.base = 0u;
+            tp.wx1 = __int_as_float(rw.y); tp.wy1 = __int_as_float(rw.z); tp.wz1 = __int_as_float(rw.w);
+            tp.wx0 = 1.f - tp.wx1; tp.wy0 = 1.f - tp.wy1; tp.wz0 = 1.f - tp.wz1;
+            const float cv[8] = {__int_as_float(c03.x), __int_as_float(c03.y), __int_as_float(c03.z), __int_as_float(c03.w),
+                                 __int_as_float(c47.x), __int_as_float(c47.y), __int_as_float(c47.z), __int_as_float(c47.w)};
+            float gx, gy, gz;
+            grad8(tp, cv, &gx, &gy, &gz);
+            if (gx == 0.f && gy == 0.f && gz == 0.f) continue;                       // contributes an exact 0
             const long long lin = ((long long)z * G.ny + y) * G.nx + x;
             float q[K];
 #pragma unroll
@@ -766,7 +780,7 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     const unsigned* skip_table = tile_count(G, TileZ<K>::value) >= fs.skip_min_tiles_per_sm * (long long)fs.n_sm ? fs.cell_integral : nullptr;
     if (B == 1 && fs.grad_rec) {                        // one solve: the warp kernel left the records, gather only
         const long long n_sub = tile_count(G, TileZ<K>::value) * GROUP_WARPS;
-        q.launch(k_grad_gather<K>, dim3(grid * GNG), dim3(GG_THREADS), 0, G, (const SolveState*)c.solves, fs.grad_rec, n_sub,
+        q.launch(k_grad_gather<K>, dim3(grad_gather_blocks(G, fs)), dim3(GG_THREADS), 0, G, (const SolveState*)c.solves, fs.grad_rec, n_sub,
                  TX * TileZ<K>::value / GROUP_WARPS, fs.fields, rL, utab, vtab, bvol, c.grad_part, fs.visited);
         return;
     }
@@ -804,6 +818,8 @@ void launch_build_cellmap(cudaStream_t st, const Geom& G, const float* f0, unsig
     k_build_cellmap<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, f0, cellmap);
 }
 // partial-sum slots per solve: two per persistent CTA (TMA kernel), else one per block
+int grad_gather_blocks(const Geom& G, const FieldStream& fs) { return fs.n_sm * gather_per_sm(G.K); }
+
 int grad_blocks(const Geom& G, const FieldStream& fs) {
     if (fs.use_tma) return grad_grid(G, fs) * grad_groups_for(G.K);
     return ((G.nx + TILE - 1) / TILE) * ((G.ny + TILE - 1) / TILE) * G.nz;
@@ -825,7 +841,9 @@ void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, 
 #undef PCAMM_CASE
         default: break;
     }
-    launch_ctl_after_grad(q, G, c, mode);       // the control step that follows the gradient (control.cu)
+    CtlBufs cc = c;                             // the control step that follows the gradient (control.cu) adds as many
+    if (fs.use_tma && B == 1 && fs.grad_rec) cc.grad_blocks = grad_gather_blocks(G, fs);     // partial sums as the kernel left
+    launch_ctl_after_grad(q, G, cc, mode);
 }
 
 void launch_backproject(Seq& q, const Geom& G, const SolveState* solves, const float* rL, const float4* utab,

@@ -53,6 +53,8 @@ struct Seq {
     bool has_last = false;
     cudaError_t err = cudaSuccess;
     int n_kernels = 0;        // kernels appended so far (not counting the bodies of while-loops)
+    bool pdl = false;         // graph mode: kernel -> kernel edges are programmatic (common.cuh grid_dependency_wait)
+    bool last_is_kernel = false;
 
     bool graph_mode() const { return graph != nullptr; }
 
@@ -65,6 +67,7 @@ struct Seq {
     // Appends a while-loop node; the kernels of its body go to the returned sequence.
     Seq add_while(cudaGraphConditionalHandle handle) {
         Seq body;
+        body.pdl = pdl;
         if (err != cudaSuccess) { body.err = err; return body; }
         cudaGraphNodeParams p = {};
         p.type = cudaGraphNodeTypeConditional;
@@ -76,6 +79,7 @@ struct Seq {
         if (err != cudaSuccess) { body.err = err; return body; }
         last = node;
         has_last = true;
+        last_is_kernel = false;
         body.graph = p.conditional.phGraph_out[0];
         return body;
     }
@@ -93,9 +97,25 @@ struct Seq {
             kp.sharedMemBytes = (unsigned)smem;
             kp.kernelParams = argv;
             cudaGraphNode_t node;
-            err = cudaGraphAddKernelNode(&node, graph, has_last ? &last : nullptr, has_last ? 1 : 0, &kp);
+            if (pdl && has_last && last_is_kernel) {
+                cudaGraphNodeParams np = {};
+                np.type = cudaGraphNodeTypeKernel;
+                np.kernel.func = kp.func;
+                np.kernel.gridDim = grid;
+                np.kernel.blockDim = block;
+                np.kernel.sharedMemBytes = (unsigned)smem;
+                np.kernel.kernelParams = argv;
+                cudaGraphEdgeData ed = {};
+                ed.from_port = cudaGraphKernelNodePortProgrammatic;
+                ed.to_port = cudaGraphKernelNodePortDefault;
+                ed.type = cudaGraphDependencyTypeProgrammatic;
+                err = cudaGraphAddNode_v2(&node, graph, &last, &ed, 1, &np);
+            } else {
+                err = cudaGraphAddKernelNode(&node, graph, has_last ? &last : nullptr, has_last ? 1 : 0, &kp);
+            }
             last = node;
             has_last = true;
+            last_is_kernel = true;
         } else {
             err = cudaLaunchKernel((const void*)kernel, grid, block, argv, smem, stream);
             count_launch(1);
@@ -116,6 +136,7 @@ void launch_warp(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, 
 int project_blocks(const Geom& G);
 int max_slabs(const Geom& G);
 extern int g_chunks_per_segment, g_scan_slabs;     // measurement knobs (pcamm_tune): 0 = automatic
+extern int g_pdl;                                  // 1: programmatic kernel -> kernel edges in the solve graphs
 extern int g_timeline;                             // 1: models record the kernel timeline of their solves
 bool project_fits(const Geom& G);    // the knots of one scan row set fit into shared memory (nz up to ~ 4000)
 // in-plane traversal tables of the views of solves 0..B-1 (once per solve: the angle is fixed)
@@ -141,6 +162,7 @@ void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* 
 // ---- a-3 / a-4 (gradient.cu)
 int resid_blocks(const Geom& G);
 int grad_blocks(const Geom& G, const FieldStream& fs);
+int grad_gather_blocks(const Geom& G, const FieldStream& fs);      // partial sums of the gather over the gradient records (one solve)
 void launch_build_cellmap(cudaStream_t st, const Geom& G, const float* f0, unsigned char* cellmap);
 // r = p - a y - b, rL = r * |D - S|, per-view tables, partial sums of r^2; p of solve b is read
 // from its accepted slot.

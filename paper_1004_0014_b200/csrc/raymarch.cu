@@ -162,6 +162,7 @@ k_backproject_rm(const Geom G, const SolveState* __restrict__ solves, int force,
 __global__ void __launch_bounds__(256)
 k_zero_bvol(const Geom G, const SolveState* __restrict__ solves, int force, float4* __restrict__ bvol4, long long n4_per_solve,
             float* __restrict__ bvol, long long V) {
+    grid_dependency_wait();
     const int b = blockIdx.y;
     if (!needs_gradient(solves[b]) && !force) return;
     const long long i = (long long)blockIdx.x * 256 + threadIdx.x;

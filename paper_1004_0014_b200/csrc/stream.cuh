@@ -37,16 +37,23 @@ __host__ __device__ __forceinline__ int tiles_z(const Geom& G, int tz) { return 
 __host__ __device__ __forceinline__ long long tile_count(const Geom& G, int tz) {
     return (long long)tiles_x(G) * G.ny * tiles_z(G, tz);
 }
-// (t < 2^31: pcamm_model_create bounds the volume; 32-bit divisions)
+// (t < 2^31: pcamm_model_create bounds the volume.)  The two divisions are multiplications by
+// M = ceil(2^32 / d), exact for every t with t d < 2^32 (t M / 2^32 = t / d + t r / (d 2^32) with
+// r = M d - 2^32 < d); the host sets the multipliers to 0 where that does not hold (tile_multipliers).
 __device__ __forceinline__ TileCoord tile_coord(const Geom& G, int tz, long long t64) {
     const unsigned t = (unsigned)t64, ntx = (unsigned)tiles_x(G);
-    const unsigned row = t / ntx;                       // (y, z tile)
-    const unsigned zt = row / (unsigned)G.ny;
+    const unsigned row = G.tile_mx ? __umulhi(t, G.tile_mx) : t / ntx;                   // (y, z tile)
+    const unsigned zt = G.tile_my ? __umulhi(row, G.tile_my) : row / (unsigned)G.ny;
     TileCoord c;
     c.x0 = (int)(t - row * ntx) * TX;
     c.y = (int)(row - zt * (unsigned)G.ny);
     c.z0 = (int)zt * tz;
     return c;
+}
+inline void tile_multipliers(Geom& G) {
+    const unsigned long long n_max = (unsigned long long)tile_count(G, 16), ntx = (unsigned long long)tiles_x(G), ny = (unsigned long long)G.ny;
+    G.tile_mx = (ntx >= 2 && n_max * ntx < (1ull << 32)) ? (unsigned)(((1ull << 32) + ntx - 1) / ntx) : 0u;
+    G.tile_my = (ny >= 2 && n_max * ny < (1ull << 32)) ? (unsigned)(((1ull << 32) + ny - 1) / ny) : 0u;
 }
 
 // ---------------------------------------------------------------- mbarrier / TMA (PTX)
@@ -221,30 +228,40 @@ constexpr int SKIP_MIN_TILES_PER_SM = 12;
 // bound must not wrap the int box arithmetic of the tile flags: it then simply covers the volume).
 __device__ __forceinline__ int reach_of(float dmax) { return (int)ceilf(fminf(dmax * 1.0001f + 0.001f, 1048576.f)); }
 
-// Records of the voxels with a non-zero image gradient (single-solve path; warp.cu writes them,
-// gradient.cu k_grad_gather reads them).  The warp kernel has, for every voxel of a trial volume,
-// the eight taps of f0 in registers: their differences are G_j = df_j / dx_j, exactly what a-4 needs
-// at the same coefficients.  So it writes, per trial slot, one record (x, y, z, G_j) for every voxel
-// with G_j != 0 (boundary voxels: 6 % at C2), and the gradient of the accepted candidate needs no
-// second pass over the K+1 fields: only B_j and u_kj at the recorded voxels.
+// Records of the voxels whose interpolation cell is not constant (single-solve path; warp.cu writes
+// them, gradient.cu k_grad_gather reads them).  The warp kernel has, for every voxel of a trial
+// volume, the eight taps of f0 and the three fractions in registers: G_j = df_j / dx_j is a function of
+// those eleven numbers, and it is exactly 0 where the eight taps are equal.  So it writes, per trial
+// slot, one record for every voxel whose taps differ (boundary voxels: 6 % at C2), and the gradient of
+// the accepted candidate needs no second pass over the K+1 fields: G_j from the record, B_j and u_kj
+// at the recorded voxels.  (The record holds the taps, not G_j: a warp row usually has one or two such
+// voxels, and forming G_j there would cost the whole warp its 40 instructions for them; the gather
+// forms it with every lane busy.)
 // Layout per slot: a tile is cut into GROUP_WARPS sub-tiles (the voxels one warp of the consumer
 // group handles: TX x TZ / GROUP_WARPS = `cap` of them, so a sub-tile cannot overflow); sub-tile s
-// owns records s cap .. s cap + count[s] - 1, in the fixed order (row, lane).
+// owns records s cap .. s cap + count[s] - 1, in the fixed order (row, lane).  A record is 48 bytes
+// (three 16-byte stores / loads).
+struct GradRecord {
+    int xyz;           // x | y << 11 | z << 22 (pcamm_model_create: records only for nx, ny <= 2048, nz <= 1024)
+    float tx, ty, tz;  // fractions of the displaced position in its cell (trilinear.cuh Taps: w1 = t, w0 = 1 - t)
+    float c[8];        // the cell's taps of f0, in gather8's order
+};
+constexpr int RECORD_WORDS = 12;
+constexpr int RECORD_MAX_XY = 2048, RECORD_MAX_Z = 1024;
+__device__ __forceinline__ int record_xyz(int x, int y, int z) { return x | y << 11 | z << 22; }
+__device__ __forceinline__ int record_x(int w) { return w & 2047; }
+__device__ __forceinline__ int record_y(int w) { return (w >> 11) & 2047; }
+__device__ __forceinline__ int record_z(int w) { return (int)((unsigned)w >> 22); }
 struct GradRecords {
     int* count;        // [n_sub]
-    int* xy;           // [plane]  x | y << 16
-    int* z;            // [plane]
-    float* g;          // [3][plane]
-    long long plane;   // n_sub * cap
+    GradRecord* r;     // [n_sub * cap]
 };
-__host__ __device__ __forceinline__ long long grad_record_words(long long n_sub, long long plane) { return n_sub + 5 * plane; }
+// (n_sub is a multiple of GROUP_WARPS = 8: the records start 16-byte aligned)
+__host__ __device__ __forceinline__ long long grad_record_words(long long n_sub, long long plane) { return n_sub + RECORD_WORDS * plane; }
 __host__ __device__ __forceinline__ GradRecords grad_records(int* base, long long n_sub, long long plane, int slot) {
     GradRecords r;
     r.count = base + (long long)slot * grad_record_words(n_sub, plane);
-    r.xy = r.count + n_sub;
-    r.z = r.xy + plane;
-    r.g = reinterpret_cast<float*>(r.z + plane);
-    r.plane = plane;
+    r.r = reinterpret_cast<GradRecord*>(r.count + n_sub);
     return r;
 }
 

@@ -48,10 +48,13 @@ __device__ __forceinline__ Taps make_taps(const Geom& G, int i, int j, int k, fl
 
 // c[0..7]: taps (x0,y0,z0), (x1,y0,z0), (x0,y1,z0), (x1,y1,z0), (x0,y0,z1), ...; f0p: the padded copy.
 __device__ __forceinline__ void gather8(const Geom& G, const float* __restrict__ f0p, const Taps& t, float* c) {
+    // 32-bit element offsets (the padded copy has fewer than 2^31 elements): one add and one widening
+    // multiply-add per tap pair instead of 64-bit pointer sums
+    const unsigned b10 = t.base + (unsigned)G.fnx, b01 = t.base + (unsigned)G.fpp, b11 = b01 + (unsigned)G.fnx;
     const float* p00 = f0p + t.base;
-    const float* p10 = p00 + G.fnx;
-    const float* p01 = p00 + G.fpp;
-    const float* p11 = p01 + G.fnx;
+    const float* p10 = f0p + b10;
+    const float* p01 = f0p + b01;
+    const float* p11 = f0p + b11;
     c[0] = __ldg(p00); c[1] = __ldg(p00 + 1);
     c[2] = __ldg(p10); c[3] = __ldg(p10 + 1);
     c[4] = __ldg(p01); c[5] = __ldg(p01 + 1);

@@ -182,6 +182,9 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
     const long long n_tiles = tile_count(G, WTZ);
     const long long n_sub = n_tiles * GROUP_WARPS, rec_plane = n_tiles * (TX * WTZ);
     constexpr int SUBCAP = TX * WROWS;                     // records a sub-tile (one warp's voxels of a tile) can hold
+    const long long rec_stride_w = grad_record_words(n_sub, rec_plane);            // words per slot
+    int* const rec_count = rec;                            // slot 0's counts and records (GradRecords)
+    int* const rec_w = REC ? reinterpret_cast<int*>(grad_records(rec, n_sub, rec_plane, 0).r) : nullptr;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int last_active = -1;                                  // the last slot that reads the stage
     for (int i = 0; i < nslots; ++i)
@@ -251,7 +254,7 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
             for (int sl = 0; sl < nslots; ++sl) {
                 if (!s_active[sl]) continue;
                 float* out = vol_out + (long long)sl * slot_stride;
-                if (REC && lane == 0) grad_records(rec, n_sub, rec_plane, sl).count[t * GROUP_WARPS + tw] = 0;   // f0 = 0 all around: G = 0
+                if (REC && lane == 0) rec_count[(long long)sl * rec_stride_w + t * GROUP_WARPS + tw] = 0;   // f0 = 0 all around: G = 0
                 if (!RAY) {
 #pragma unroll
                     for (int r = 0; r < WROWS; ++r) {
@@ -281,6 +284,10 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
             }
             const TileCoord c = tile_coord(G, WTZ, t);
             const int x = c.x0 + lane;
+            // which of the thread's rows are voxels of the grid
+            unsigned in_grid = 0u;
+#pragma unroll
+            for (int r = 0; r < WROWS; ++r) in_grid |= (x < G.nx && c.z0 + tw + GROUP_WARPS * r < G.nz) ? 1u << r : 0u;
             for (int sl = 0; sl < nslots; ++sl) {
                 if (!s_active[sl]) continue;               // uniform over the grid
                 float w[K];
@@ -317,46 +324,41 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
 #pragma unroll
                 for (int r = 0; r < WROWS; ++r) val[r] = combine8(taps[r], cv[r]);
                 if (REC) {
-                    // G_j from the same taps (reading A6): the voxels of this warp with
-                    // G_j != 0, in the order (row, lane), into its sub-tile's records
-                    const GradRecords R = grad_records(rec, n_sub, rec_plane, sl);
-                    const long long sub = t * GROUP_WARPS + tw, base = sub * SUBCAP;
+                    // the voxels of this warp whose cell is not constant (only they can have G_j != 0;
+                    // PAPER.md:L95, reading A6), in the order (row, lane), into its sub-tile's records
+                    const int sub = (int)t * GROUP_WARPS + tw;
+                    GradRecord* R = reinterpret_cast<GradRecord*>(rec_w + (long long)sl * rec_stride_w) + sub * SUBCAP;
+                    const int xyz0 = record_xyz(x, c.y, c.z0 + tw);
                     int n_rec = 0;
 #pragma unroll
                     for (int r = 0; r < WROWS; ++r) {
-                        const int z = c.z0 + tw + GROUP_WARPS * r;
-                        // a cell whose eight taps are equal has G = 0 exactly: most warps stop here
-                        const bool varies = (cv[r][1] != cv[r][0] || cv[r][2] != cv[r][0] || cv[r][3] != cv[r][0] || cv[r][4] != cv[r][0] ||
-                                             cv[r][5] != cv[r][0] || cv[r][6] != cv[r][0] || cv[r][7] != cv[r][0]) && x < G.nx && z < G.nz;
-                        if (!__any_sync(0xffffffffu, varies)) continue;          // uniform over the warp
-                        float gx, gy, gz;
-                        grad8(taps[r], cv[r], &gx, &gy, &gz);
-                        const bool active = varies && (gx != 0.f || gy != 0.f || gz != 0.f);
-                        const unsigned mask = __ballot_sync(0xffffffffu, active);
-                        if (active) {
-                            const long long pos = base + n_rec + __popc(mask & ((1u << lane) - 1u));
-                            R.xy[pos] = x | c.y << 16;
-                            R.z[pos] = z;
-                            R.g[pos] = gx; R.g[R.plane + pos] = gy; R.g[2 * R.plane + pos] = gz;
+                        const bool diff = cv[r][1] != cv[r][0] || cv[r][2] != cv[r][0] || cv[r][3] != cv[r][0] || cv[r][4] != cv[r][0] ||
+                                          cv[r][5] != cv[r][0] || cv[r][6] != cv[r][0] || cv[r][7] != cv[r][0];
+                        const bool varies = diff && ((in_grid >> r) & 1u);
+                        const unsigned mask = __ballot_sync(0xffffffffu, varies);
+                        if (mask == 0u) continue;                                // most warp rows: uniform
+                        if (varies) {
+                            int4* dst = reinterpret_cast<int4*>(R + n_rec + __popc(mask & ((1u << lane) - 1u)));
+                            dst[0] = make_int4(xyz0 + (GROUP_WARPS * r << 22), __float_as_int(taps[r].wx1), __float_as_int(taps[r].wy1), __float_as_int(taps[r].wz1));
+                            dst[1] = make_int4(__float_as_int(cv[r][0]), __float_as_int(cv[r][1]), __float_as_int(cv[r][2]), __float_as_int(cv[r][3]));
+                            dst[2] = make_int4(__float_as_int(cv[r][4]), __float_as_int(cv[r][5]), __float_as_int(cv[r][6]), __float_as_int(cv[r][7]));
                         }
                         n_rec += __popc(mask);
                     }
-                    if (lane == 0) R.count[sub] = n_rec;
+                    if (lane == 0) rec_count[(long long)sl * rec_stride_w + sub] = n_rec;
                     n_written += n_rec;
                 }
                 }
                 if (!RAY) {
 #pragma unroll
-                    for (int r = 0; r < WROWS; ++r) {
-                        const int z = c.z0 + tw + GROUP_WARPS * r;
-                        if (x < G.nx && z < G.nz) out[((long long)z * G.ny + c.y) * G.nx + x] = val[r];
-                    }
+                    for (int r = 0; r < WROWS; ++r)
+                        if ((in_grid >> r) & 1u) out[((c.z0 + tw + GROUP_WARPS * r) * G.ny + c.y) * G.nx + x] = val[r];     // (V < 2^31)
                 } else {
                     // occupancy (common.cuh): is anything non-zero in column x, z block of 16?  Rows
                     // zz = tw + 8 r: r = 0, 1 lie in the tile's first block, r = 2, 3 in its second.
                     bool nzb[2] = {false, false};
 #pragma unroll
-                    for (int r = 0; r < WROWS; ++r) nzb[r >> 1] |= val[r] != 0.f && x < G.nx && c.z0 + tw + GROUP_WARPS * r < G.nz;
+                    for (int r = 0; r < WROWS; ++r) nzb[r >> 1] |= val[r] != 0.f && ((in_grid >> r) & 1u);
                     if (tw < 2) s_occ[group][tw][lane] = 0;
                     group_barrier(group);
 #pragma unroll
@@ -364,13 +366,12 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                     if (nzb[0]) s_occ[group][0][lane] = 1;
                     if (nzb[1]) s_occ[group][1][lane] = 1;
                     group_barrier(group);
-                    const int zo = c.z0 + lane;
+                    // this thread's transposed stores: column c.x0 + tw + 8 r, level c.z0 + lane (elements < 2^31)
+                    const int ray0 = (int)ray_layout_index(G, c.x0 + tw, c.y, c.z0 + lane), ray_step = GROUP_WARPS * G.nz;
+                    const bool z_ok = lane < WTZ && c.z0 + lane < G.nz;
 #pragma unroll
-                    for (int r = 0; r < TX / GROUP_WARPS; ++r) {
-                        const int xo = c.x0 + tw + GROUP_WARPS * r;
-                        if (lane < WTZ && xo < G.nx && zo < G.nz)
-                            out[ray_layout_index(G, xo, c.y, zo)] = tile[lane][tw + GROUP_WARPS * r];
-                    }
+                    for (int r = 0; r < TX / GROUP_WARPS; ++r)
+                        if (z_ok && c.x0 + tw + GROUP_WARPS * r < G.nx) out[ray0 + r * ray_step] = tile[lane][tw + GROUP_WARPS * r];
                     if (tw < WTZ / 16 && x < G.nx && c.z0 + 16 * tw < G.nz)
                         occ[(long long)sl * G.OCC + occ_index(G, x, c.y, (c.z0 >> 4) + tw)] = (unsigned char)s_occ[group][tw][lane];
                 }

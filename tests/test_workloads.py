@@ -157,5 +157,5 @@ def test_bench_moved_bytes_model():
 
     # gradient records (one solve): the warp kernel writes them, the gradient gathers over the accepted slot's
     rec = bench.moved_bytes(cfg, 0, {"warp": n_tiles, "gradient": 0}, vox, {"written": 2000.0, "gathered": 1000.0}, n_tiles)
-    assert rec["warp"] == 56 * cfg.V + 20 * 2000 + 32 * n_tiles
-    assert rec["gradient"] == (20 + 12 * cfg.K) * 1000 + 32 * n_tiles + 4 * cfg.npix
+    assert rec["warp"] == 56 * cfg.V + 48 * 2000 + 32 * n_tiles
+    assert rec["gradient"] == (48 + 12 * cfg.K) * 1000 + 32 * n_tiles + 4 * cfg.npix

@@ -289,7 +289,8 @@ int pcamm_tile_counts(pcamm_model* model, int32_t reset, int64_t* out /* [6] */,
  *                                 (0 = automatic, the default);
  *   "project_scan_slabs"          slabs per scan of the projector: 1, 2 or 4 (0 = automatic);
  *   "grad_records"                0: the gradient of a single solve makes its own pass over the K+1 fields
- *                                 (1, the default: the warp kernel leaves records of the voxels whose
+ *                                 (1, the default: in models created with max_batch = 1 and
+ *                                 max_candidates <= 2 the warp kernel leaves records of the voxels whose
  *                                 interpolation cell is not constant and the gradient is a gather over
  *                                 them);
  *   "pdl"                         0: plain kernel -> kernel edges in the solve graphs (1, the default:

@@ -312,6 +312,8 @@ int get_graph(pcamm_model* m, int B, int C, GraphRec** out) {
     q.pdl = g_pdl != 0;
     seq_head(m, q, B, C, h_loop, 1);
     Seq body = q.add_while(h_loop);             // iterations and their line searches
+    // (two or more passes per evaluation of the loop condition were measured and are slower: 2.81 / 2.84 / 2.87 ms
+    // per C2 solve with 2 / 3 / 4 against 2.74 ms with one)
     seq_body(m, body, B, C, h_loop, 1);
     seq_tail(m, q, B);
     int rc;
@@ -747,7 +749,11 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
         m->fs.skip_min_tiles_per_sm = g->tile_skipping == 1 ? 0 : (g->tile_skipping == 2 ? (1 << 30) : SKIP_MIN_TILES_PER_SM);
     }
     m->c.grad_blocks = grad_blocks(G, m->fs);
-    if (m->fs.use_tma && g_grad_records && G.nx <= RECORD_MAX_XY && G.ny <= RECORD_MAX_XY && G.nz <= RECORD_MAX_Z) {
+    // Records pay where few candidates share a pass (each candidate slot costs the warp kernel about a sixth
+    // more, the gather saves one pass over the fields per iteration: a win for one or two candidates, a loss
+    // for the fan of eight) and serve single solves only: models made for them get the records.
+    if (m->fs.use_tma && g_grad_records && Bmax == 1 && Cmax <= RECORD_MAX_FAN && G.nx <= RECORD_MAX_XY && G.ny <= RECORD_MAX_XY &&
+        G.nz <= RECORD_MAX_Z) {
         // gradient records of the trial slots of a single solve (stream.cuh GradRecords): 48 bytes per voxel and slot
         const int tz = G.K <= PCAMM_TZ_SMALL_K ? 32 : 16;                     // TileZ<K>
         const long long n_tiles = tile_count(G, tz), n_sub = n_tiles * GROUP_WARPS, plane = n_tiles * (TX * tz);

@@ -248,6 +248,7 @@ struct GradRecord {
 };
 constexpr int RECORD_WORDS = 12;
 constexpr int RECORD_MAX_XY = 2048, RECORD_MAX_Z = 1024;
+constexpr int RECORD_MAX_FAN = 2;      // candidate slots per pass up to which the records are written (api.cu)
 __device__ __forceinline__ int record_xyz(int x, int y, int z) { return x | y << 11 | z << 22; }
 __device__ __forceinline__ int record_x(int w) { return w & 2047; }
 __device__ __forceinline__ int record_y(int w) { return (w >> 11) & 2047; }

@@ -315,6 +315,27 @@ int pcamm_timeline(pcamm_model* model, int32_t cap, int32_t* kind_out, double* s
  * iteration counters after each solve). */
 int64_t pcamm_launch_count(int32_t reset);
 
+/* a-3 for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the intensity fit of Eq. 4 and the cost of Eq. 2
+ * of one projection pair, with no model and no allocation of any kind: every
+ * intermediate lives in one file-scope device array of 41 216 bytes (csrc/noalloc.cu), which every
+ * GPU that loads the library holds until the process exits.
+ *   p_dev, y_dev  [npix] float, device: the computed and the measured projection (any layout, the
+ *                 same for both); read only
+ *   npix          1 .. PCAMM_STATIC_MAX_PIXELS; beyond that PCAMM_E_INVALID (the array holds no more)
+ *   out_dev       [8] double, device, owned by the caller: a, b (Eq. 4), J = sum (p - a y - b)^2 at
+ *                 that (a, b), sum p, sum y, sum y^2, sum y p, status (PCAMM_OK, PCAMM_E_SINGULAR: y is
+ *                 constant, then a = b = 0; PCAMM_E_NONFINITE: a sum is not finite) as a double
+ * Asynchronous on `stream` (one memset and two kernels; nothing is synchronised, nothing read back):
+ * out_dev is valid once the stream has reached the end of the call.  Sums in double in a fixed
+ * order: the same inputs give the same bits.  The scratch array is shared by every call on a device
+ * and keeps the last call's contents; what must start at zero is cleared on the stream at the start
+ * of each call.  Calls that overlap on the GPU (different streams or threads, same device) race on it
+ * and give wrong results: serialise them.  Returns PCAMM_OK, PCAMM_E_INVALID (NULL argument, size) or
+ * PCAMM_E_CUDA. */
+#define PCAMM_STATIC_MAX_PIXELS (1 << 22)
+int pcamm_fit_cost_static(const float* p_dev, const float* y_dev, int64_t npix, double* out_dev, void* stream);
+
 const char* pcamm_last_error(void);
 
 #ifdef __cplusplus

@@ -54,7 +54,7 @@ SYMBOLS = ("pcamm_default_opts", "pcamm_model_create", "pcamm_model_destroy", "p
            "pcamm_reconstruct",
            "pcamm_reconstruct_host", "pcamm_reconstruct_batch", "pcamm_warp", "pcamm_project",
            "pcamm_backproject", "pcamm_eval", "pcamm_traverse", "pcamm_localise", "pcamm_time_kernel", "pcamm_time_slots",
-           "pcamm_tune", "pcamm_tile_counts", "pcamm_timeline", "pcamm_launch_count", "pcamm_last_error", "pcamm_pca_fit", "pcamm_predict_w", "pcamm_frames_create",
+           "pcamm_tune", "pcamm_tile_counts", "pcamm_timeline", "pcamm_fit_cost_static", "pcamm_launch_count", "pcamm_last_error", "pcamm_pca_fit", "pcamm_predict_w", "pcamm_frames_create",
            "pcamm_frames_destroy", "pcamm_frames_reset", "pcamm_frames_count", "pcamm_frames_predict",
            "pcamm_frames_push")
 
@@ -364,6 +364,27 @@ class Model:
         ms = C.c_float(0)
         _check(lib().pcamm_time_kernel(self._h, int(which), int(reps), C.byref(ms), _stream()))
         return float(ms.value)
+
+
+STATIC_MAX_PIXELS = 1 << 22     # PCAMM_STATIC_MAX_PIXELS
+
+
+def fit_cost_static(p, y, out=None):
+    """pcamm_fit_cost_static: the intensity fit (Eq. 4) and cost (Eq. 2) of the projection pair (p, y)
+    (float32 CUDA tensors of the same size, at most STATIC_MAX_PIXELS pixels) without a model and
+    without any allocation inside the library (its scratch is a static device array; calls that
+    overlap on the GPU race on it).  `out`: a float64 CUDA tensor of 8 elements to receive the results
+    (allocated here if None; pass one where nothing may allocate).  Asynchronous: returns `out`
+    = (a, b, J, sum p, sum y, sum y^2, sum y p, status), valid once the current stream reaches it."""
+    torch = _torch()
+    n = int(p.numel())
+    pp, yy = _dev_f32(p, n, "p"), _dev_f32(y, n, "y")
+    if out is None:
+        out = torch.empty(8, dtype=torch.float64, device=p.device)
+    if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 8):
+        raise TypeError("out: expected a contiguous float64 CUDA tensor of 8 elements")
+    _check(lib().pcamm_fit_cost_static(pp, yy, C.c_int64(n), C.c_void_p(out.data_ptr()), _stream()))
+    return out
 
 
 def pca_fit(dvfs, K: int, sign_ref: int = -1, pass_ms: Optional[list] = None):

@@ -10,7 +10,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpcamm.so")
-SOURCES = ["api.cu", "frames.cu", "pca.cu", "warp.cu", "project.cu", "raymarch.cu", "gradient.cu", "control.cu"]
+SOURCES = ["api.cu", "frames.cu", "pca.cu", "warp.cu", "project.cu", "raymarch.cu", "gradient.cu", "control.cu", "noalloc.cu"]
 # every header of csrc/ (globbed, so that a new one cannot be forgotten) and the public one
 HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))) + [os.path.join("..", "..", "include", "pcamm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -297,6 +297,10 @@ int pcamm_tile_counts(pcamm_model* model, int32_t reset, int64_t* out /* [6] */,
  *                                 programmatic dependent launch, the next kernel's blocks are launched
  *                                 while the previous kernel drains and wait for its completion on the
  *                                 device; same order of memory effects);
+ *   "static_passes"               line-search passes laid out as plain kernel nodes in front of the solve
+ *                                 graph's while-loop (the loop takes the passes beyond): -1, the default,
+ *                                 = min(max_iter, 16) when opts.grad_tol = 0 (a solve then takes max_iter
+ *                                 iterations of at least one pass each) and 0 otherwise; 0 .. 64 forces it;
  *   "timeline"                    1: models created from now on record, inside their kernels, the
  *                                 start and end of every kernel of a solve (pcamm_timeline). */
 int pcamm_tune(const char* name, int32_t value);

@@ -18,6 +18,8 @@ namespace pcamm {
 static thread_local std::string g_error;
 static thread_local long long g_launches = 0;
 int g_timeline = 0;
+constexpr int STATIC_PASSES_MAX = 16;
+int g_static_passes = -1; // pcamm_tune "static_passes": -1 automatic (get_graph's caller)
 int g_pdl = 1;            // pcamm_tune "pdl": programmatic kernel -> kernel edges in the solve graphs built from then on
 int g_grad_records = 1;   // pcamm_tune "grad_records": 0 = the gradient of a single solve makes its own pass over the fields
 
@@ -299,8 +301,11 @@ void seq_tail(pcamm_model* m, Seq& q, int B) {
     launch_invert(q, G, m->xbar, m->u, m->c, B, m->M, m->lm0, m->lm_out);
 }
 
-int get_graph(pcamm_model* m, int B, int C, GraphRec** out) {
-    const long long key = (long long)B * 1024 + C;
+// n_static: line-search passes laid out as plain kernel nodes in front of the while-loop (pcamm_tune
+// "static_passes"); the loop then takes whatever passes remain.  Every kernel of a pass looks at its
+// solves' state first, so a pass behind the end of a solve does nothing.
+int get_graph(pcamm_model* m, int B, int C, int n_static, GraphRec** out) {
+    const long long key = ((long long)n_static * 8192 + B) * 1024 + C;
     auto it = m->graphs.find(key);
     if (it != m->graphs.end()) { *out = &it->second; return PCAMM_OK; }
     GraphRec rec;
@@ -311,6 +316,7 @@ int get_graph(pcamm_model* m, int B, int C, GraphRec** out) {
     q.graph = rec.graph;
     q.pdl = g_pdl != 0;
     seq_head(m, q, B, C, h_loop, 1);
+    for (int i = 0; i < n_static; ++i) seq_body(m, q, B, C, h_loop, 1);
     Seq body = q.add_while(h_loop);             // iterations and their line searches
     // (two or more passes per evaluation of the loop condition were measured and are slower: 2.81 / 2.84 / 2.87 ms
     // per C2 solve with 2 / 3 / 4 against 2.74 ms with one)
@@ -381,7 +387,14 @@ int solve_impl(pcamm_model* m, int B, const float* y_dev, const float* angles, c
     }
     if (o.loop_mode == 0) {
         GraphRec* g = nullptr;
-        if ((rc = get_graph(m, B, C, &g))) return rc;
+        // Passes in front of the loop: with the stopping rule off (grad_tol = 0) a solve takes max_iter iterations,
+        // each at least one line-search pass, so that many passes can be plain nodes (2 us from kernel to kernel
+        // instead of the 7 to 9 us an evaluation of the loop condition costs); the loop takes the passes beyond.
+        // With grad_tol on, the count is not known and a pass behind the end of a solve still costs its six
+        // launches (about 20 us): none then.  (A line search that fails ends a solve early too: rare.)
+        const int auto_static = o.grad_tol > 0.f ? 0 : (o.max_iter < STATIC_PASSES_MAX ? o.max_iter : STATIC_PASSES_MAX);
+        const int n_static = g_static_passes < 0 ? auto_static : (g_static_passes < o.max_iter ? g_static_passes : o.max_iter);
+        if ((rc = get_graph(m, B, C, n_static, &g))) return rc;
         CUDA_TRY(cudaGraphLaunch(g->exec, st));
     } else {
         if ((rc = run_host_loop(m, B, C, st))) return rc;
@@ -973,6 +986,11 @@ int pcamm_tune(const char* name, int32_t value) {
     if (n == "timeline") { g_timeline = value != 0; return PCAMM_OK; }
     if (n == "grad_records") { g_grad_records = value != 0; return PCAMM_OK; }
     if (n == "pdl") { g_pdl = value != 0; return PCAMM_OK; }
+    if (n == "static_passes") {
+        if (value < -1 || value > 64) return invalid("static_passes must be -1 .. 64");
+        g_static_passes = value;
+        return PCAMM_OK;
+    }
     return invalid("unknown knob: " + n);
 }
 

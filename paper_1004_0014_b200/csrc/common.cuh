@@ -39,11 +39,12 @@ __device__ __forceinline__ bool tl_first_thread() { return (threadIdx.x | thread
 // until the predecessor has completed and its writes are visible.  Nothing a previous kernel wrote
 // may be read, and nothing it read may be overwritten, before this; every kernel of the graph calls
 // it first thing (through tl_begin), so the order of all memory effects is that of the plain graph.
-// The kernel's own dependents may be launched at once: they wait the same way.  (Launched without a
-// programmatic edge both instructions do nothing.)
+// Once through, the kernel lets its own dependents be launched: they wait the same way, and at most
+// one kernel is ever resident ahead of the running one.  (Launched without a programmatic edge both
+// instructions do nothing.)
 __device__ __forceinline__ void grid_dependency_wait() {
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 // at the top of a kernel, by every block
 __device__ __forceinline__ void tl_begin(Timeline* tl) {

@@ -780,6 +780,9 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     const unsigned* skip_table = tile_count(G, TileZ<K>::value) >= fs.skip_min_tiles_per_sm * (long long)fs.n_sm ? fs.cell_integral : nullptr;
     if (B == 1 && fs.grad_rec) {                        // one solve: the warp kernel left the records, gather only
         const long long n_sub = tile_count(G, TileZ<K>::value) * GROUP_WARPS;
+        // a plain edge into the gather: launched programmatically behind k_resid at the top level of the graph it
+        // took 65 us instead of 38 (timeline; the other kernels are indifferent or gain)
+        q.plain_next = true;
         q.launch(k_grad_gather<K>, dim3(grad_gather_blocks(G, fs)), dim3(GG_THREADS), 0, G, (const SolveState*)c.solves, fs.grad_rec, n_sub,
                  TX * TileZ<K>::value / GROUP_WARPS, fs.fields, rL, utab, vtab, bvol, c.grad_part, fs.visited);
         return;

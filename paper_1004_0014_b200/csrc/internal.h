@@ -55,6 +55,7 @@ struct Seq {
     int n_kernels = 0;        // kernels appended so far (not counting the bodies of while-loops)
     bool pdl = false;         // graph mode: kernel -> kernel edges are programmatic (common.cuh grid_dependency_wait)
     bool last_is_kernel = false;
+    bool plain_next = false;  // the next kernel takes a plain edge whatever pdl says (then reset)
 
     bool graph_mode() const { return graph != nullptr; }
 
@@ -97,7 +98,9 @@ struct Seq {
             kp.sharedMemBytes = (unsigned)smem;
             kp.kernelParams = argv;
             cudaGraphNode_t node;
-            if (pdl && has_last && last_is_kernel) {
+            const bool programmatic = pdl && has_last && last_is_kernel && !plain_next;
+            plain_next = false;
+            if (programmatic) {
                 cudaGraphNodeParams np = {};
                 np.type = cudaGraphNodeTypeKernel;
                 np.kernel.func = kp.func;

@@ -160,6 +160,27 @@ def test_projector_knobs_change_the_launch_not_the_result():
         pc.tune("project_chunks_per_segment", 0)
 
 
+def test_graph_knobs_change_the_launch_not_the_result():
+    """pcamm_tune("pdl") and ("static_passes"): the same kernels in the same order with the same memory effects,
+    so a solve gives the same bits whatever the edges of its graph are and wherever its while-loop starts."""
+    import paper_1004_0014_b200 as pc
+    g, m, w, y = _setup(max_candidates=2)
+    opts = pc.Opts(max_iter=5, batched_linesearch=2)
+    ref = m.reconstruct(y, 0.9, np.zeros(3, np.float32), opts, trace=True)
+    try:
+        for knob, value in (("pdl", 0), ("static_passes", 0), ("static_passes", 3), ("static_passes", 9)):
+            pc.tune(knob, value)
+            g2, m2, _, _ = _setup(max_candidates=2)
+            r = m2.reconstruct(y, 0.9, np.zeros(3, np.float32), opts, trace=True)
+            assert r.iters == ref.iters and np.array_equal(r.backtracks, ref.backtracks)
+            assert np.array_equal(r.w, ref.w) and r.J == ref.J and r.a == ref.a and r.b == ref.b
+            pc.tune("pdl", 1)
+            pc.tune("static_passes", -1)
+    finally:
+        pc.tune("pdl", 1)
+        pc.tune("static_passes", -1)
+
+
 def test_model_on_a_second_device():
     """The opt-in to large dynamic shared memory is per device."""
     import torch

@@ -239,7 +239,7 @@ __device__ __forceinline__ int reach_of(float dmax) { return (int)ceilf(fminf(dm
 // forms it with every lane busy.)
 // Layout per slot: a tile is cut into GROUP_WARPS sub-tiles (the voxels one warp of the consumer
 // group handles: TX x TZ / GROUP_WARPS = `cap` of them, so a sub-tile cannot overflow); sub-tile s
-// owns records s cap .. s cap + count[s] - 1, in the fixed order (row, lane).  A record is 48 bytes
+// owns records s cap .. s cap + count[s] - 1, in the fixed order (lane, row).  A record is 48 bytes
 // (three 16-byte stores / loads).
 struct GradRecord {
     int xyz;           // x | y << 11 | z << 22 (pcamm_model_create: records only for nx, ny <= 2048, nz <= 1024)

@@ -325,25 +325,41 @@ k_warp_tma(const __grid_constant__ CUtensorMap fmap, const __grid_constant__ CUt
                 for (int r = 0; r < WROWS; ++r) val[r] = combine8(taps[r], cv[r]);
                 if (REC) {
                     // the voxels of this warp whose cell is not constant (only they can have G_j != 0;
-                    // PAPER.md:L95, reading A6), in the order (row, lane), into its sub-tile's records
-                    const int sub = (int)t * GROUP_WARPS + tw;
-                    GradRecord* R = reinterpret_cast<GradRecord*>(rec_w + (long long)sl * rec_stride_w) + sub * SUBCAP;
-                    const int xyz0 = record_xyz(x, c.y, c.z0 + tw);
-                    int n_rec = 0;
+                    // PAPER.md:L95, reading A6), in the order (lane, row), into its sub-tile's records:
+                    // a lane's rows with such a cell, the warp's running count of them, then each lane
+                    // stores its records one behind the other
+                    unsigned vmask = 0u;
 #pragma unroll
                     for (int r = 0; r < WROWS; ++r) {
                         const bool diff = cv[r][1] != cv[r][0] || cv[r][2] != cv[r][0] || cv[r][3] != cv[r][0] || cv[r][4] != cv[r][0] ||
                                           cv[r][5] != cv[r][0] || cv[r][6] != cv[r][0] || cv[r][7] != cv[r][0];
-                        const bool varies = diff && ((in_grid >> r) & 1u);
-                        const unsigned mask = __ballot_sync(0xffffffffu, varies);
-                        if (mask == 0u) continue;                                // most warp rows: uniform
-                        if (varies) {
-                            int4* dst = reinterpret_cast<int4*>(R + n_rec + __popc(mask & ((1u << lane) - 1u)));
-                            dst[0] = make_int4(xyz0 + (GROUP_WARPS * r << 22), __float_as_int(taps[r].wx1), __float_as_int(taps[r].wy1), __float_as_int(taps[r].wz1));
-                            dst[1] = make_int4(__float_as_int(cv[r][0]), __float_as_int(cv[r][1]), __float_as_int(cv[r][2]), __float_as_int(cv[r][3]));
-                            dst[2] = make_int4(__float_as_int(cv[r][4]), __float_as_int(cv[r][5]), __float_as_int(cv[r][6]), __float_as_int(cv[r][7]));
+                        vmask |= diff ? 1u << r : 0u;
+                    }
+                    vmask &= in_grid;
+                    const int sub = (int)t * GROUP_WARPS + tw;
+                    int n_rec = 0;
+                    if (__any_sync(0xffffffffu, vmask != 0u)) {                  // uniform over the warp
+                        const int cnt = __popc(vmask);
+                        int incl = cnt;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+                            if (lane >= o) incl += v;
                         }
-                        n_rec += __popc(mask);
+                        n_rec = __shfl_sync(0xffffffffu, incl, 31);
+                        if (vmask != 0u) {
+                            int4* dst = reinterpret_cast<int4*>(reinterpret_cast<GradRecord*>(rec_w + (long long)sl * rec_stride_w) + sub * SUBCAP + (incl - cnt));
+                            const int xyz0 = record_xyz(x, c.y, c.z0 + tw);
+#pragma unroll
+                            for (int r = 0; r < WROWS; ++r) {
+                                if ((vmask >> r) & 1u) {
+                                    dst[0] = make_int4(xyz0 + (GROUP_WARPS * r << 22), __float_as_int(taps[r].wx1), __float_as_int(taps[r].wy1), __float_as_int(taps[r].wz1));
+                                    dst[1] = make_int4(__float_as_int(cv[r][0]), __float_as_int(cv[r][1]), __float_as_int(cv[r][2]), __float_as_int(cv[r][3]));
+                                    dst[2] = make_int4(__float_as_int(cv[r][4]), __float_as_int(cv[r][5]), __float_as_int(cv[r][6]), __float_as_int(cv[r][7]));
+                                    dst += 3;
+                                }
+                            }
+                        }
                     }
                     if (lane == 0) rec_count[(long long)sl * rec_stride_w + sub] = n_rec;
                     n_written += n_rec;

@@ -152,6 +152,7 @@ struct pcamm_model {
     unsigned char* occ = nullptr;       // occupancy of the trial volumes [S][OCC] (common.cuh)
     float *vol = nullptr, *pseg = nullptr, *p = nullptr, *rL = nullptr;   // vol: trial volumes, ray layout [S][PV]
     float* bvol = nullptr;          // projector 1: backprojection volumes P^T r, [B][V] (raymarch.cu), else NULL
+    unsigned* rec_mask = nullptr;   // projector 1 with gradient records: one bit per voxel, record_mask_words(G) words
     ColHdr* col_hdr = nullptr;      // [B][nu]
     SlabEntry* slab_tab = nullptr;  // [B][nu][max_slabs]
     float4* utab = nullptr;
@@ -272,6 +273,16 @@ int push_call(pcamm_model* m, int B, cudaStream_t st) {
 //   tail:       closing residual (J at exit), final, landmark inversion
 // A single-block control step (control.cuh) follows every projection and every gradient pass.
 
+// P^T r of the ray-marching variant for the solves that need a gradient; where the gradient of the one solve
+// gathers over the records, only at the recorded voxels (raymarch.cu)
+void backproject_rm(pcamm_model* m, Seq& q, int B, int force, float* bvol, bool all_voxels) {
+    const Geom& G = m->G;
+    const int tz = G.K <= PCAMM_TZ_SMALL_K ? 32 : 16;                     // TileZ<K>
+    const bool masked = !all_voxels && B == 1 && m->fs.grad_rec;
+    launch_backproject_rm(q, G, m->c.solves, B, force, m->rL, bvol, masked ? m->fs.grad_rec : nullptr,
+                          tile_count(G, tz) * GROUP_WARPS, TX * tz / GROUP_WARPS, masked ? m->rec_mask : nullptr);
+}
+
 void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h_loop, int use_cond) {
     const Geom& G = m->G;
     launch_ysums(q, G, m->c, B);
@@ -286,7 +297,7 @@ void seq_body(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     const Geom& G = m->G;
     const int n0 = q.n_kernels;
     launch_resid(q, G, m->c.solves, m->c.in, B, 0, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    if (G.projector == 1) launch_backproject_rm(q, G, m->c.solves, B, 0, m->rL, m->bvol);
+    if (G.projector == 1) backproject_rm(m, q, B, 0, m->bvol, false);
     launch_grad(q, G, m->fs, m->f0p, m->c, B, m->rL, m->utab, m->vtab, m->bvol, GRAD_SOLVE);
     launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ, B == 1 ? m->fs.grad_rec : nullptr);
     launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_TRIAL, h_loop, use_cond,
@@ -606,6 +617,7 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     }
     if (g->projector == 1) {
         e = dalloc(m, &m->bvol, B * (size_t)V);
+        if (e == cudaSuccess) e = dalloc(m, &m->rec_mask, (size_t)record_mask_words(G));
         if (e != cudaSuccess) { set_error("allocation failed (backprojection volumes)"); cudaGetLastError(); pcamm_model_destroy(m); return PCAMM_E_NOMEM; }
     }
     if (g_timeline) {
@@ -858,7 +870,7 @@ int pcamm_backproject(pcamm_model* m, const float* r_dev, float angle_rad, float
     int rc = hook_begin(m, nullptr, angle_rad, nullptr, 0.f, 0.f, 2, st, q);
     if (rc) return rc;
     launch_resid(q, m->G, m->c.solves, m->c.in, 1, 1, m->p, r_dev, m->rL, m->utab, m->vtab, m->c.resid_part);
-    if (m->G.projector == 1) launch_backproject_rm(q, m->G, m->c.solves, 1, 1, m->rL, volume_out_dev);
+    if (m->G.projector == 1) backproject_rm(m, q, 1, 1, volume_out_dev, true);          // the hook wants every voxel
     else launch_backproject(q, m->G, m->c.solves, m->rL, m->utab, m->vtab, volume_out_dev);
     if ((rc = check_seq(q, "backproject"))) return rc;
     CUDA_TRY(cudaStreamSynchronize(st));
@@ -879,7 +891,7 @@ int pcamm_eval(pcamm_model* m, const float* y_dev, float angle_rad, const float*
     launch_warp(q2, G, m->fs, m->f0p, m->c.slots, 1, 1, m->vol, G.PV, m->occ, m->fs.grad_rec);
     launch_project(q2, G, m->c, 1, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_EVAL, 0, 0, 0);
     launch_resid(q2, G, m->c.solves, m->c.in, 1, 1, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
-    if (G.projector == 1) launch_backproject_rm(q2, G, m->c.solves, 1, 1, m->rL, m->bvol);
+    if (G.projector == 1) backproject_rm(m, q2, 1, 1, m->bvol, false);
     launch_grad(q2, G, m->fs, m->f0p, m->c, 1, m->rL, m->utab, m->vtab, m->bvol, GRAD_EVAL);
     if ((rc = check_seq(q2, "eval"))) return rc;
     if (proj_out_dev) CUDA_TRY(cudaMemcpyAsync(proj_out_dev, m->p, sizeof(float) * G.npix, cudaMemcpyDeviceToDevice, st));

@@ -156,7 +156,12 @@ void launch_project(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const C
 // (no control step: launch_project adds it), and B[b] = P^T r for the solves that need a gradient
 // (force: for all), r taken from rL = r |D - S|
 void launch_project_rm(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const float* vol, float* p);
-void launch_backproject_rm(Seq& q, const Geom& G, const SolveState* solves, int B, int force, const float* rL, float* bvol);
+// rec, n_sub, cap, mask: the gradient records of the slots (stream.cuh GradRecords) and a scratch of
+// record_mask_words(G) words, where the gradient of the one solve will read B at the recorded voxels
+// only (the scatter then skips every other voxel); else NULL / 0
+long long record_mask_words(const Geom& G);
+void launch_backproject_rm(Seq& q, const Geom& G, const SolveState* solves, int B, int force, const float* rL, float* bvol,
+                           int* rec, long long n_sub, int cap, unsigned* mask);
 // hooks: standard layout -> ray layout; one ray of the view of solve 0
 void launch_to_ray_layout(Seq& q, const Geom& G, const float* vol_std, float* vol_ray, unsigned char* occ);
 void launch_traverse(Seq& q, const Geom& G, const ColHdr* hdr, const SlabEntry* tab, int iu, int iv, int cap,

@@ -16,6 +16,11 @@
 // gathering (the order of the adds is not fixed: results of this variant are reproducible to
 // rounding, not bitwise).  This variant is the simple ray-driven form; the regrouping that makes
 // the Siddon projector fast (project.cu) is not applied to it.
+//
+// Where the gradient of a single solve is a gather over the records the warp kernel left
+// (stream.cuh GradRecords), B is read at the recorded voxels only: k_record_mask turns the records
+// of the accepted candidate into one bit per voxel, and the scatter then skips every add to a voxel
+// nobody will read (at C2 94 % of them; the sums at the others are what they would have been).
 #include "internal.h"
 
 namespace pcamm {
@@ -130,7 +135,7 @@ k_project_rm(const Geom G, const CtlBufs c, int slot0, const float* __restrict__
 // k_resid leaves it.  r_direct: one view, solve 0 (the pcamm_backproject hook).  grid (nu, B).
 __global__ void __launch_bounds__(RT)
 k_backproject_rm(const Geom G, const SolveState* __restrict__ solves, int force, const float* __restrict__ rL,
-                 float* __restrict__ bvol) {
+                 float* __restrict__ bvol, const unsigned* __restrict__ mask) {
     tl_begin(G.tl);
     const int iu = blockIdx.x, b = blockIdx.y;
     if (!needs_gradient(solves[b]) && !force) { tl_end(G.tl, TLK_RESID); return; }
@@ -148,8 +153,20 @@ k_backproject_rm(const Geom G, const SolveState* __restrict__ solves, int force,
         if (rd == 0.f) continue;
         for (int m = 0; m < r.M; ++m) {
             const RmSample q = rm_sample(G, r, m);
-            float* p0 = B + ((long long)q.k * G.ny + q.j) * G.nx + q.i;
+            const long long l0 = ((long long)q.k * G.ny + q.j) * G.nx + q.i;
+            float* p0 = B + l0;
             const float wx0 = 1.f - q.tx, wy0 = 1.f - q.ty, wz0 = (1.f - q.tz) * rd, wz1 = q.tz * rd;
+            if (mask) {                                                    // uniform over the grid
+                auto add = [&](long long off, float v) {
+                    const long long l = l0 + off;
+                    if ((__ldg(mask + (l >> 5)) >> (unsigned)(l & 31)) & 1u) atomicAdd(p0 + off, v);
+                };
+                add(0, wx0 * wy0 * wz0);            add(sx, q.tx * wy0 * wz0);
+                add(sy, wx0 * q.ty * wz0);          add(sy + sx, q.tx * q.ty * wz0);
+                add(sz, wx0 * wy0 * wz1);           add(sz + sx, q.tx * wy0 * wz1);
+                add(sz + sy, wx0 * q.ty * wz1);     add(sz + sy + sx, q.tx * q.ty * wz1);
+                continue;
+            }
             atomicAdd(p0, wx0 * wy0 * wz0);           atomicAdd(p0 + sx, q.tx * wy0 * wz0);
             atomicAdd(p0 + sy, wx0 * q.ty * wz0);     atomicAdd(p0 + sy + sx, q.tx * q.ty * wz0);
             atomicAdd(p0 + sz, wx0 * wy0 * wz1);      atomicAdd(p0 + sz + sx, q.tx * wy0 * wz1);
@@ -171,6 +188,33 @@ k_zero_bvol(const Geom G, const SolveState* __restrict__ solves, int force, floa
     } else if (i < V) bvol[b * V + i] = 0.f;
 }
 
+// One bit per voxel (bit lin & 31 of word lin >> 5, lin = (z ny + y) nx + x): set where the accepted
+// candidate of solve 0 has a gradient record.  One warp per sub-tile of records; the words are
+// cleared beforehand (k_zero_words).
+__global__ void __launch_bounds__(256)
+k_record_mask(const Geom G, const SolveState* __restrict__ solves, int force, int* __restrict__ rec_base, long long n_sub, int cap,
+              unsigned* __restrict__ mask) {
+    grid_dependency_wait();
+    if (!needs_gradient(solves[0]) && !force) return;
+    const GradRecords rec = grad_records(rec_base, n_sub, n_sub * cap, solves[0].acc_slot);
+    const long long sub = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (sub >= n_sub) return;
+    const int n = __ldcg(rec.count + sub);
+    for (int e = threadIdx.x & 31; e < n; e += 32) {
+        const int w = __ldcg(&rec.r[sub * cap + e].xyz);
+        const long long lin = ((long long)record_z(w) * G.ny + record_y(w)) * G.nx + record_x(w);
+        atomicOr(mask + (lin >> 5), 1u << (unsigned)(lin & 31));
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_zero_words(const SolveState* __restrict__ solves, int force, unsigned* __restrict__ words, long long n) {
+    grid_dependency_wait();
+    if (!needs_gradient(solves[0]) && !force) return;
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i < n) words[i] = 0u;
+}
+
 }  // namespace
 
 void launch_project_rm(Seq& q, const Geom& G, const CtlBufs& c, int nslots, const float* vol, float* p) {
@@ -180,15 +224,24 @@ void launch_project_rm(Seq& q, const Geom& G, const CtlBufs& c, int nslots, cons
     }
 }
 
-void launch_backproject_rm(Seq& q, const Geom& G, const SolveState* solves, int B, int force, const float* rL, float* bvol) {
+long long record_mask_words(const Geom& G) { return (G.V + 31) / 32; }
+
+void launch_backproject_rm(Seq& q, const Geom& G, const SolveState* solves, int B, int force, const float* rL, float* bvol,
+                           int* rec, long long n_sub, int cap, unsigned* mask) {
     const bool v4 = G.V % 4 == 0;
     const long long n = v4 ? G.V / 4 : G.V;
+    const bool masked = B == 1 && rec && mask;          // one solve whose gradient gathers over the records
+    if (masked) {
+        const long long nw = record_mask_words(G);
+        q.launch(k_zero_words, dim3((unsigned)((nw + 255) / 256)), dim3(256), 0, solves, force, mask, nw);
+        q.launch(k_record_mask, dim3((unsigned)((n_sub + 7) / 8)), dim3(256), 0, G, solves, force, rec, n_sub, cap, mask);
+    }
     for (int b0 = 0; b0 < B; b0 += 65535) {
         const int nb = B - b0 < 65535 ? B - b0 : 65535;
         q.launch(k_zero_bvol, dim3((unsigned)((n + 255) / 256), nb), dim3(256), 0, G, solves + b0, force,
                  reinterpret_cast<float4*>(bvol + (long long)b0 * G.V), v4 ? n : 0LL, bvol + (long long)b0 * G.V, G.V);
         q.launch(k_backproject_rm, dim3(G.nu, nb), dim3(RT), 0, G, solves + b0, force, rL + (long long)b0 * G.npix,
-                 bvol + (long long)b0 * G.V);
+                 bvol + (long long)b0 * G.V, (const unsigned*)(masked ? mask : nullptr));
     }
 }
 

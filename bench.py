@@ -101,8 +101,8 @@ def moved_bytes(cfg, field_storage, tiles_loaded, vox_per_tile, records=None, n_
     A loaded tile costs its fields and its f0 gathers (4 B per voxel, counted once); the warp kernel
     writes every voxel of the volume (skipped tiles as zeros), the gradient kernel reads the residual.
     With gradient records (the default for one solve) the warp kernel also writes 48 B per voxel with
-    a non-constant cell and a count per sub-tile (8 per tile); the gradient reads those and 12 K bytes of u per record
-    (scattered 4-byte loads: the sectors they touch are not counted) and the residual."""
+    a non-constant cell and a count per sub-tile (8 per tile); the gradient reads those, the voxel's 3 K values of
+    u (12 K bytes, from the copy that holds them side by side) per record, and the residual."""
     fields = field_bytes_per_voxel(cfg, field_storage)
     out = {"warp": tiles_loaded["warp"] * vox_per_tile * (fields + 4) + 4 * cfg.V,
            "gradient": tiles_loaded["gradient"] * vox_per_tile * (fields + 4) + 4 * cfg.npix}
@@ -430,8 +430,8 @@ def run_ours(args, cfg, rank, local_rank, world):
             "kernel": "k_grad_gather", "records_per_launch": records["gathered"],
             "records_per_voxel": records["gathered"] / cfg.V,
             "note": "a gather over the records the warp kernel left for the voxels with G_j != 0 (DESIGN.md section 5b): "
-                    "latency- and sector-bound scattered loads, not a stream; moved_bytes counts 48 B per record, "
-                    "12 K B of u per record, the counts and the residual, not the 32-byte sectors touched"})
+                    "latency-bound scattered loads, not a stream; moved_bytes counts 48 B per record, "
+                    "12 K B of u per record, the counts and the residual"})
     # the projector's volume was just written and is L2-resident: it is not an HBM kernel.
     # What it does per launch: one pass over (detector column, slab, level) and one look-up per z crossing.
     per_kernel["project"].update({

@@ -293,6 +293,9 @@ int pcamm_tile_counts(pcamm_model* model, int32_t reset, int64_t* out /* [6] */,
  *                                 max_candidates <= 2 the warp kernel leaves records of the voxels whose
  *                                 interpolation cell is not constant and the gradient is a gather over
  *                                 them);
+ *   "grad_aos"                    0: the gather over the records reads u_k from the field planes (1, the
+ *                                 default: models with records also hold u_1 .. u_K with a voxel's 3 K values
+ *                                 side by side, 4 ceil(3 K / 4) floats per voxel, which the gather reads);
  *   "pdl"                         0: plain kernel -> kernel edges in the solve graphs (1, the default:
  *                                 programmatic dependent launch, the next kernel's blocks are launched
  *                                 while the previous kernel drains and wait for its completion on the

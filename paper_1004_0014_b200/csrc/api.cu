@@ -21,6 +21,7 @@ int g_timeline = 0;
 constexpr int STATIC_PASSES_MAX = 16;
 int g_static_passes = -1; // pcamm_tune "static_passes": -1 automatic (get_graph's caller)
 int g_pdl = 1;            // pcamm_tune "pdl": programmatic kernel -> kernel edges in the solve graphs built from then on
+int g_grad_aos = 1;       // pcamm_tune "grad_aos": 0 = the gather over the records reads u_k from the planes
 int g_grad_records = 1;   // pcamm_tune "grad_records": 0 = the gradient of a single solve makes its own pass over the fields
 
 void set_error(const std::string& msg) { g_error = msg; }
@@ -47,6 +48,16 @@ __global__ void k_fields_to_voxel_units(float* __restrict__ fields, long long V,
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         const int c = (int)((i / V) % 3);
         fields[i] = __fdiv_rn(fields[i], c == 0 ? hx : (c == 1 ? hy : hz));
+    }
+}
+
+// u_1 .. u_K, planar [3 K][V], to [V][pitch] with a voxel's 3 K values side by side (FieldStream::u_aos).
+__global__ void k_u_to_aos(const float* __restrict__ u, long long V, int K, int pitch, float* __restrict__ out) {
+    const long long n = V * pitch;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const long long v = i / pitch;
+        const int c = (int)(i - v * pitch);
+        out[i] = c < 3 * K ? u[(long long)c * V + v] : 0.f;
     }
 }
 
@@ -793,6 +804,20 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
             return fail(e4 == cudaErrorMemoryAllocation ? PCAMM_E_NOMEM : PCAMM_E_CUDA);
         }
         m->fs.grad_rec = rec;
+        if (g_grad_aos) {
+            float* aos = nullptr;
+            e4 = dalloc(m, &aos, (size_t)V * aos_pitch(G.K));
+            if (e4 == cudaSuccess) {
+                k_u_to_aos<<<1184, 256, 0, st>>>(m->u, V, G.K, aos_pitch(G.K), aos);
+                e4 = cudaStreamSynchronize(st);
+            }
+            if (e4 != cudaSuccess) {
+                set_error(std::string("gradient records (u side by side): ") + cudaGetErrorString(e4));
+                cudaGetLastError();
+                return fail(e4 == cudaErrorMemoryAllocation ? PCAMM_E_NOMEM : PCAMM_E_CUDA);
+            }
+            m->fs.u_aos = aos;
+        }
     }
     *out = m;
     return PCAMM_OK;
@@ -998,6 +1023,7 @@ int pcamm_tune(const char* name, int32_t value) {
     if (n == "timeline") { g_timeline = value != 0; return PCAMM_OK; }
     if (n == "grad_records") { g_grad_records = value != 0; return PCAMM_OK; }
     if (n == "pdl") { g_pdl = value != 0; return PCAMM_OK; }
+    if (n == "grad_aos") { g_grad_aos = value != 0; return PCAMM_OK; }
     if (n == "static_passes") {
         if (value < -1 || value > 64) return invalid("static_passes must be -1 .. 64");
         g_static_passes = value;

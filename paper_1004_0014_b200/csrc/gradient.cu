@@ -632,7 +632,7 @@ __host__ __device__ constexpr int gather_per_sm(int K) { return K <= 4 ? 4 : 3; 
 template <int K>
 __global__ void __launch_bounds__(GG_THREADS, gather_per_sm(K))
 k_grad_gather(const Geom G, const SolveState* __restrict__ solves, int* __restrict__ rec_base, long long n_sub, int cap,
-              const float* __restrict__ fields, const float* __restrict__ rL, const float4* __restrict__ utab,
+              const float* __restrict__ fields, const float* __restrict__ u_aos, const float* __restrict__ rL, const float4* __restrict__ utab,
               const float2* __restrict__ vtab, const float* __restrict__ bvol, double* __restrict__ partials,
               unsigned long long* __restrict__ visited) {
     __shared__ double red[GG_WARPS][K];
@@ -692,10 +692,23 @@ k_grad_gather(const Geom G, const SolveState* __restrict__ solves, int* __restri
             grad8(tp, cv, &gx, &gy, &gz);
             if (gx == 0.f && gy == 0.f && gz == 0.f) continue;                       // contributes an exact 0
             const long long lin = ((long long)z * G.ny + y) * G.nx + x;
-            float q[K];
+            float q[K];                                     // q_kj = G_j . u_kj (fields in voxel units: no 1/h, reading B4)
+            if (u_aos) {                                    // uniform over the grid
+                constexpr int P = aos_pitch(K);
+                float uu[P];
+                const float4* ua = reinterpret_cast<const float4*>(u_aos + lin * P);
 #pragma unroll
-            for (int k = 0; k < K; ++k)                     // q_kj = G_j . u_kj (fields in voxel units: no 1/h, reading B4)
-                q[k] = gx * __ldg(u + (3 * k) * G.V + lin) + gy * __ldg(u + (3 * k + 1) * G.V + lin) + gz * __ldg(u + (3 * k + 2) * G.V + lin);
+                for (int i = 0; i < P / 4; ++i) {
+                    const float4 v = __ldg(ua + i);
+                    uu[4 * i] = v.x; uu[4 * i + 1] = v.y; uu[4 * i + 2] = v.z; uu[4 * i + 3] = v.w;
+                }
+#pragma unroll
+                for (int k = 0; k < K; ++k) q[k] = gx * uu[3 * k] + gy * uu[3 * k + 1] + gz * uu[3 * k + 2];
+            } else {
+#pragma unroll
+                for (int k = 0; k < K; ++k)
+                    q[k] = gx * __ldg(u + (3 * k) * G.V + lin) + gy * __ldg(u + (3 * k + 1) * G.V + lin) + gz * __ldg(u + (3 * k + 2) * G.V + lin);
+            }
             float Bj;
             if (bvol) Bj = __ldg(bvol + lin);
             else {
@@ -784,7 +797,7 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
         // took 65 us instead of 38 (timeline; the other kernels are indifferent or gain)
         q.plain_next = true;
         q.launch(k_grad_gather<K>, dim3(grad_gather_blocks(G, fs)), dim3(GG_THREADS), 0, G, (const SolveState*)c.solves, fs.grad_rec, n_sub,
-                 TX * TileZ<K>::value / GROUP_WARPS, fs.fields, rL, utab, vtab, bvol, c.grad_part, fs.visited);
+                 TX * TileZ<K>::value / GROUP_WARPS, fs.fields, fs.u_aos, rL, utab, vtab, bvol, c.grad_part, fs.visited);
         return;
     }
     if (B == 1) {

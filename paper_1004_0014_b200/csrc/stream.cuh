@@ -266,6 +266,8 @@ __host__ __device__ __forceinline__ GradRecords grad_records(int* base, long lon
     return r;
 }
 
+__host__ __device__ constexpr int aos_pitch(int K) { return (3 * K + 3) / 4 * 4; }
+
 // What the streaming kernels need to know about the model's fields.
 struct FieldStream {
     const float* fields = nullptr;   // [3(K+1)][V]: xbar's planes, then u_1 .. u_K
@@ -290,6 +292,10 @@ struct FieldStream {
     int skip_min_tiles_per_sm = SKIP_MIN_TILES_PER_SM;     // geometry.tile_skipping: 0 always, INT_MAX never
     // gradient records of the trial slots (GradRecords; NULL: none, the gradient makes its own pass)
     int* grad_rec = nullptr;
+    // with the records: a copy of u_1 .. u_K with a voxel's 3 K values side by side, [V][aos_pitch(K)]
+    // floats (zero padded), so that the gather over the records fetches them from two or three 32-byte
+    // sectors instead of 3 K
+    const float* u_aos = nullptr;
     // measurement: tiles whose fields the warp / gradient kernels really loaded, summed over the
     // launches since the host last cleared them ([0] warp, [1] gradient; one atomic per consumer group)
     unsigned long long* visited = nullptr;

@@ -99,3 +99,34 @@ def test_c2_solve_and_tumour_position(c2):
     m.reconstruct(to_dev(y), fr.angle_rad, w0, opts, volume_out=vol_dev)
     vol = to_host(vol_dev)
     assert rel_l2(vol, oracle.warp(g, wl.f0, wl.model.mean, wl.model.eig, ref["w"].astype(np.float32))) <= 2e-5
+
+
+def test_c2_solve_in_the_bench_configuration(c2):
+    """What bench.py times by default: a model with two candidate slots, two Armijo candidates per
+    line-search pass (reading B7), the gradient from the records the warp kernel leaves, the certain
+    passes in front of the graph's loop.  Against the sequential solve of the default model (the same
+    accepted steps, bit for bit) and against the oracle."""
+    import paper_1004_0014_b200 as pc
+    cfg, wl, g, m, fr, y = c2
+    m2 = pc.Model(nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, hx=cfg.hx, hy=cfg.hy, hz=cfg.hz, K=cfg.K, nu=cfg.nu, nv=cfg.nv,
+                  pu=cfg.pu, pv=cfg.pv, f0=to_dev(wl.f0), mean_dvf=to_dev(wl.model.mean), eig_dvf=to_dev(wl.model.eig),
+                  landmarks_mm=wl.landmarks, sad=cfg.sad, sdd=cfg.sdd, max_candidates=2)
+    w0 = np.zeros(cfg.K, np.float32)
+    seq = m.reconstruct(to_dev(y), fr.angle_rad, w0, pc.Opts(max_iter=4), trace=True)
+    opts = pc.Opts(max_iter=4, batched_linesearch=2)
+    res = m2.reconstruct(to_dev(y), fr.angle_rad, w0, opts, trace=True)
+    assert res.iters == 4 and np.array_equal(res.backtracks, seq.backtracks)
+    assert np.array_equal(res.w, seq.w) and res.J == seq.J and res.a == seq.a and res.b == seq.b
+    assert np.array_equal(res.landmarks, seq.landmarks)
+    ref = oracle.solve(g, wl.f0, wl.model.mean, wl.model.eig, y, fr.angle_rad, w0, oracle_opts(pc.Opts(max_iter=4)),
+                       forced_mu=np.concatenate([res.mu_trace, np.zeros(4)]), want_volume=False)
+    assert np.linalg.norm(res.w - ref["w"]) <= 1e-3 * np.linalg.norm(ref["w"]), (res.w, ref["w"])
+    assert abs(res.J - ref["J"]) <= 1e-3 * ref["J"]
+    r_ref, _ = oracle.invert(g, wl.model.mean, wl.model.eig, ref["w"], wl.landmarks)
+    assert np.max(np.linalg.norm(res.landmarks - r_ref, axis=1)) <= 0.05           # mm
+    # the records really were in use: the gradient loaded no field tiles
+    m2.eval(to_dev(y), fr.angle_rad, res.w, res.a, res.b, want_proj=False)
+    m2.tile_counts(reset=True)
+    m2.time_kernel(2, 1)
+    tc = m2.tile_counts(reset=True)
+    assert tc[1] == 0 and tc[4] > 0

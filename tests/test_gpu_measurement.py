@@ -181,6 +181,31 @@ def test_graph_knobs_change_the_launch_not_the_result():
         pc.tune("static_passes", -1)
 
 
+def test_passes_behind_the_end_of_a_solve_do_nothing():
+    """A solve that stops early (here: it starts at the minimiser of a noise-free problem, so its first line
+    searches find no decreasing step) leaves the passes laid out in front of the loop with nothing to do: the
+    result is that of a graph without them, bit for bit, and the launch count says they ran."""
+    import paper_1004_0014_b200 as pc
+    g, m, w, y = _setup(max_candidates=2)               # y = P f(w), noise-free
+    opts = pc.Opts(max_iter=8, batched_linesearch=2)
+    pc.launch_count(reset=True)
+    res = m.reconstruct(y, 0.9, w, opts, trace=True)
+    assert res.iters < 8 and res.status == 3            # PCAMM_S_LINESEARCH
+    n_auto = pc.launch_count(reset=True)
+    try:
+        pc.tune("static_passes", 0)
+        g2, m2, _, _ = _setup(max_candidates=2)
+        pc.launch_count(reset=True)
+        ref = m2.reconstruct(y, 0.9, w, opts, trace=True)
+        n_loop = pc.launch_count(reset=True)
+    finally:
+        pc.tune("static_passes", -1)
+    assert ref.iters == res.iters and ref.status == res.status and np.array_equal(ref.backtracks, res.backtracks)
+    assert np.array_equal(ref.w, res.w) and ref.J == res.J and ref.a == res.a and ref.b == res.b
+    assert np.array_equal(ref.landmarks, res.landmarks) if res.landmarks is not None else True
+    assert n_auto > n_loop                              # the idle passes were launched (and counted)
+
+
 def test_model_on_a_second_device():
     """The opt-in to large dynamic shared memory is per device."""
     import torch

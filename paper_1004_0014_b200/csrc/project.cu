@@ -465,11 +465,14 @@ k_project(const Geom G, const CtlBufs c, int slot0, const ColHdr* __restrict__ h
         }
         __syncthreads();                                     // the block's stores are ordered before thread 0's fence
         if (threadIdx.x == 0) {
-            __threadfence();
+            // release: the block's stores (ordered before this thread by the barrier) are visible to whoever
+            // reads the ticket after it; acquire: the last block sees the other blocks' stores.  One
+            // acq_rel atomic instead of a full fence on either side of a relaxed one.
             int* t = seg_ticket + s * G.nu + iu;
-            const int k = atomicAdd(t, 1);
+            int k;
+            asm volatile("atom.add.acq_rel.gpu.s32 %0, [%1], 1;" : "=r"(k) : "l"(t) : "memory");
             s_last = k == n_part - 1;
-            if (s_last) { *t = 0; __threadfence(); }
+            if (s_last) *t = 0;                              // for the next launch (kernel boundaries order it)
         }
         __syncthreads();
         if (!s_last) { tl_end(G.tl, TLK_PROJECT); return; }

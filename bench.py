@@ -683,9 +683,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--fan", type=int, default=2,
+    ap.add_argument("--fan", type=int, default=None,
                     help="candidate steps evaluated per line-search pass (pcamm_opts.batched_linesearch): the "
-                         "accepted step is the same for every width, bit for bit; 1 = sequential backtracking")
+                         "accepted step is the same for every width, bit for bit; 1 = sequential backtracking.  "
+                         "Default: 2 for one solve in flight (a pass then shares the field stream and the launches "
+                         "between its candidates), 1 for --in-flight > 1 (the solves in flight share them already; "
+                         "a second candidate per pass only adds candidates that are evaluated and thrown away)")
     ap.add_argument("--cpu-single-iters", type=int, default=1,
                     help="iterations of the single-thread oracle leg (0: skip it)")
     ap.add_argument("--in-flight", type=int, default=1,
@@ -714,6 +717,8 @@ def main():
     ap.add_argument("--grad-tol", type=float, default=None)
     ap.add_argument("--study-max-iter", type=int, default=30)
     args = ap.parse_args()
+    if args.fan is None:
+        args.fan = 2 if max(int(args.in_flight), 1) == 1 else 1
     args.warmup = max(args.warmup, 0)
     from paper_1004_0014_b200.replicas import env_rank_world
     rank, local_rank, world = env_rank_world()

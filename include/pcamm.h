@@ -289,10 +289,11 @@ int pcamm_tile_counts(pcamm_model* model, int32_t reset, int64_t* out /* [6] */,
  *                                 (0 = automatic, the default);
  *   "project_scan_slabs"          slabs per scan of the projector: 1, 2 or 4 (0 = automatic);
  *   "grad_records"                0: the gradient of a single solve makes its own pass over the K+1 fields
- *                                 (1, the default: in models created with max_batch = 1 and
- *                                 max_candidates <= 2 the warp kernel leaves records of the voxels whose
- *                                 interpolation cell is not constant and the gradient is a gather over
- *                                 them);
+ *                                 (1, the default: in models created with max_candidates <= 2 whose
+ *                                 records (48 bytes per voxel, trial slot and solve in flight) fit into
+ *                                 three fifths of the free device memory, the warp kernel leaves records of
+ *                                 the voxels whose interpolation cell is not constant and the gradient is
+ *                                 a gather over them);
  *   "grad_aos"                    0: the gather over the records reads u_k from the field planes (1, the
  *                                 default: models with records also hold u_1 .. u_K with a voxel's 3 K values
  *                                 side by side, 4 ceil(3 K / 4) floats per voxel, which the gather reads);

@@ -299,7 +299,7 @@ void seq_head(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     launch_ysums(q, G, m->c, B);
     launch_begin(q, G, m->c, 0);
     launch_view_tables(q, G, m->c.solves, B, m->col_hdr, m->slab_tab);
-    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ, B == 1 ? m->fs.grad_rec : nullptr);
+    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ, m->fs.grad_rec);
     launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_INIT, h_loop, use_cond,
                    q.n_kernels);
 }
@@ -310,7 +310,7 @@ void seq_body(pcamm_model* m, Seq& q, int B, int C, cudaGraphConditionalHandle h
     launch_resid(q, G, m->c.solves, m->c.in, B, 0, m->p, nullptr, m->rL, m->utab, m->vtab, m->c.resid_part);
     if (G.projector == 1) backproject_rm(m, q, B, 0, m->bvol, false);
     launch_grad(q, G, m->fs, m->f0p, m->c, B, m->rL, m->utab, m->vtab, m->bvol, GRAD_SOLVE);
-    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ, B == 1 ? m->fs.grad_rec : nullptr);
+    launch_warp(q, G, m->fs, m->f0p, m->c.slots, B * C, 1, m->vol, G.PV, m->occ, m->fs.grad_rec);
     launch_project(q, G, m->c, B * C, m->col_hdr, m->slab_tab, m->vol, m->occ, m->pseg, m->p, THEN_TRIAL, h_loop, use_cond,
                    q.n_kernels - n0);
 }
@@ -786,14 +786,22 @@ int pcamm_model_create(const pcamm_geometry* g, const float* f0_dev, const float
     }
     m->c.grad_blocks = grad_blocks(G, m->fs);
     // Records pay where few candidates share a pass (each candidate slot costs the warp kernel about a sixth
-    // more, the gather saves one pass over the fields per iteration: a win for one or two candidates, a loss
-    // for the fan of eight) and serve single solves only: models made for them get the records.
-    if (m->fs.use_tma && g_grad_records && Bmax == 1 && Cmax <= RECORD_MAX_FAN && G.nx <= RECORD_MAX_XY && G.ny <= RECORD_MAX_XY &&
-        G.nz <= RECORD_MAX_Z) {
+    // more, the gather saves one pass over the fields per iteration and solve: a win for one or two candidates,
+    // a loss for the fan of eight), and they take 48 V bytes per trial slot: models with max_candidates <= 2
+    // get them if all their slots' records fit into three fifths of what is free on the device now.
+    size_t rec_bytes = 0, free_b = 0, total_b = 0;
+    {
+        const int tz = G.K <= PCAMM_TZ_SMALL_K ? 32 : 16;                     // TileZ<K>
+        const long long n_tiles = tile_count(G, tz);
+        rec_bytes = sizeof(int) * (size_t)grad_record_words(n_tiles * GROUP_WARPS, n_tiles * (TX * tz)) * (size_t)m->S;
+        if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { free_b = 0; cudaGetLastError(); }
+    }
+    if (m->fs.use_tma && g_grad_records && Cmax <= RECORD_MAX_FAN && rec_bytes <= free_b / 5 * 3 && G.nx <= RECORD_MAX_XY &&
+        G.ny <= RECORD_MAX_XY && G.nz <= RECORD_MAX_Z) {
         // gradient records of the trial slots of a single solve (stream.cuh GradRecords): 48 bytes per voxel and slot
         const int tz = G.K <= PCAMM_TZ_SMALL_K ? 32 : 16;                     // TileZ<K>
         const long long n_tiles = tile_count(G, tz), n_sub = n_tiles * GROUP_WARPS, plane = n_tiles * (TX * tz);
-        const size_t words = (size_t)grad_record_words(n_sub, plane) * (size_t)Cmax;
+        const size_t words = (size_t)grad_record_words(n_sub, plane) * (size_t)m->S;          // every trial slot of every solve in flight
         int* rec = nullptr;
         cudaError_t e4 = dalloc(m, &rec, words);
         if (e4 == cudaSuccess) e4 = cudaMemsetAsync(rec, 0, sizeof(int) * words, st);

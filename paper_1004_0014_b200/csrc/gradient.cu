@@ -632,16 +632,20 @@ __host__ __device__ constexpr int gather_per_sm(int K) { return K <= 4 ? 4 : 3; 
 template <int K>
 __global__ void __launch_bounds__(GG_THREADS, gather_per_sm(K))
 k_grad_gather(const Geom G, const SolveState* __restrict__ solves, int* __restrict__ rec_base, long long n_sub, int cap,
-              const float* __restrict__ fields, const float* __restrict__ u_aos, const float* __restrict__ rL, const float4* __restrict__ utab,
-              const float2* __restrict__ vtab, const float* __restrict__ bvol, double* __restrict__ partials,
+              const float* __restrict__ fields, const float* __restrict__ u_aos, const float* rL, const float4* utab,
+              const float2* vtab, const float* bvol, double* partials,
               unsigned long long* __restrict__ visited) {
     __shared__ double red[GG_WARPS][K];
     __shared__ int s_pref[GG_ROUND + 1];
     __shared__ int s_wsum[GG_WARPS];
     tl_begin(G.tl);
-    if (!needs_gradient(solves[0])) { tl_end(G.tl, TLK_GRAD); return; }    // uniform over the grid
-    const GradRecords rec = grad_records(rec_base, n_sub, n_sub * cap, solves[0].acc_slot);   // of the accepted candidate
-    const GatherView gv = make_gather_view(G, solves[0].view);
+    const int b = blockIdx.y;                                               // the solve (grid.y solves in flight)
+    if (!needs_gradient(solves[b])) { tl_end(G.tl, TLK_GRAD); return; }    // uniform over the block
+    const GradRecords rec = grad_records(rec_base, n_sub, n_sub * cap, solves[b].acc_slot);   // of the accepted candidate
+    const GatherView gv = make_gather_view(G, solves[b].view);
+    rL += (long long)b * G.npix; utab += (long long)b * G.nu; vtab += (long long)b * G.nv;
+    if (bvol) bvol += (long long)b * G.V;
+    partials += (long long)b * gridDim.x * KMAX;
     const float* __restrict__ u = fields + 3 * G.V;                          // u_1 .. u_K, planar, voxel units
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float acc[K];
@@ -791,12 +795,13 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
     const int grid = grad_grid(G, fs);
     // the flags cost a few dependent loads per launch: only where a CTA has tiles enough to win them back
     const unsigned* skip_table = tile_count(G, TileZ<K>::value) >= fs.skip_min_tiles_per_sm * (long long)fs.n_sm ? fs.cell_integral : nullptr;
-    if (B == 1 && fs.grad_rec) {                        // one solve: the warp kernel left the records, gather only
+    if (fs.grad_rec) {                                  // the warp kernel left the records: gather only
+        if (B > 65535) { q.err = cudaErrorInvalidValue; return; }
         const long long n_sub = tile_count(G, TileZ<K>::value) * GROUP_WARPS;
         // a plain edge into the gather: launched programmatically behind k_resid at the top level of the graph it
         // took 65 us instead of 38 (timeline; the other kernels are indifferent or gain)
         q.plain_next = true;
-        q.launch(k_grad_gather<K>, dim3(grad_gather_blocks(G, fs)), dim3(GG_THREADS), 0, G, (const SolveState*)c.solves, fs.grad_rec, n_sub,
+        q.launch(k_grad_gather<K>, dim3(grad_gather_blocks(G, fs), B), dim3(GG_THREADS), 0, G, (const SolveState*)c.solves, fs.grad_rec, n_sub,
                  TX * TileZ<K>::value / GROUP_WARPS, fs.fields, fs.u_aos, rL, utab, vtab, bvol, c.grad_part, fs.visited);
         return;
     }
@@ -858,7 +863,7 @@ void launch_grad(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, 
         default: break;
     }
     CtlBufs cc = c;                             // the control step that follows the gradient (control.cu) adds as many
-    if (fs.use_tma && B == 1 && fs.grad_rec) cc.grad_blocks = grad_gather_blocks(G, fs);     // partial sums as the kernel left
+    if (fs.use_tma && fs.grad_rec) cc.grad_blocks = grad_gather_blocks(G, fs);     // partial sums as the kernel left
     launch_ctl_after_grad(q, G, cc, mode);
 }
 

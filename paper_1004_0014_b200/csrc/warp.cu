@@ -425,12 +425,14 @@ void launch_tma(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, c
         const int ns = nslots - s0 < SLOT_CACHE ? nslots - s0 : SLOT_CACHE;
         float* out = vol_out + (long long)s0 * slot_stride;
         unsigned char* oc = occ ? occ + (long long)s0 * G.OCC : occ;
+        // the records of slot s0 onwards (GradRecords: one block of words per slot)
+        int* rec_s0 = rec ? rec + (long long)s0 * grad_record_words(nt * GROUP_WARPS, nt * (TX * TileZ<K>::value)) : rec;
         if (table)
             q.launch(k_warp_tma<K, RAY, H, true, REC>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
-                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited, rec);
+                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited, rec_s0);
         else
             q.launch(k_warp_tma<K, RAY, H, false, REC>, dim3(grid), dim3(WarpThreads<K>::value), smem, fmap, umap, fs.scale, fs.fmax,
-                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited, rec);
+                     table, G, f0, slots + s0, ns, out, slot_stride, oc, fs.visited, rec_s0);
     }
 }
 
@@ -438,8 +440,8 @@ template <int K>
 void launch_k(Seq& q, const Geom& G, const FieldStream& fs, const float* f0, const SlotState* slots, int nslots,
               int ray_layout, float* vol_out, long long slot_stride, unsigned char* occ, int* rec) {
     if (fs.use_tma) {
-        // records only with the ray layout (the solve's trial volumes) and at most SLOT_CACHE slots in one launch
-        const bool with_rec = rec && ray_layout && nslots <= SLOT_CACHE;
+        // records only with the ray layout (the solve's trial volumes)
+        const bool with_rec = rec && ray_layout;
         if (fs.half_u) {
             if (with_rec) launch_tma<K, true, true, true>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ, rec);
             else if (ray_layout) launch_tma<K, true, true, false>(q, G, fs, f0, slots, nslots, vol_out, slot_stride, occ, nullptr);

@@ -686,9 +686,10 @@ def main():
     ap.add_argument("--fan", type=int, default=None,
                     help="candidate steps evaluated per line-search pass (pcamm_opts.batched_linesearch): the "
                          "accepted step is the same for every width, bit for bit; 1 = sequential backtracking.  "
-                         "Default: 2 for one solve in flight (a pass then shares the field stream and the launches "
-                         "between its candidates), 1 for --in-flight > 1 (the solves in flight share them already; "
-                         "a second candidate per pass only adds candidates that are evaluated and thrown away)")
+                         "Default: 2 for one solve in flight on volumes up to C2's size (a pass then shares the field "
+                         "stream and the launches between its candidates), else 1 (larger volumes, and --in-flight > 1 "
+                         "where the solves in flight share them already: a second candidate per pass then only adds "
+                         "candidates that are evaluated and thrown away)")
     ap.add_argument("--cpu-single-iters", type=int, default=1,
                     help="iterations of the single-thread oracle leg (0: skip it)")
     ap.add_argument("--in-flight", type=int, default=1,
@@ -717,12 +718,14 @@ def main():
     ap.add_argument("--grad-tol", type=float, default=None)
     ap.add_argument("--study-max-iter", type=int, default=30)
     args = ap.parse_args()
-    if args.fan is None:
-        args.fan = 2 if max(int(args.in_flight), 1) == 1 else 1
     args.warmup = max(args.warmup, 0)
     from paper_1004_0014_b200.replicas import env_rank_world
     rank, local_rank, world = env_rank_world()
     cfg = get_config(args.config)
+    if args.fan is None:
+        # measured: two candidates per pass win up to C2's size for one solve in flight (C1 0.95 against 1.06 ms,
+        # C2 2.55 against 2.68), one candidate wins beyond (C4: 8.45 against 9.11) and for solves in flight
+        args.fan = 2 if max(int(args.in_flight), 1) == 1 and cfg.V <= (1 << 23) else 1
     if args.frames_study:
         run_frames_study(args, cfg, rank, local_rank)
     elif args.pca_study:

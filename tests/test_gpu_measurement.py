@@ -160,6 +160,40 @@ def test_projector_knobs_change_the_launch_not_the_result():
         pc.tune("project_chunks_per_segment", 0)
 
 
+def test_solves_in_flight_from_records_and_from_the_streamed_gradient_agree():
+    """Several solves in flight take their gradients from the records as well (one gather over the solves):
+    against the streamed kernel, which sums in another order, and against the same solves one at a time."""
+    import torch
+    import paper_1004_0014_b200 as pc
+    g, m, w, y0 = _setup(max_batch=3, max_candidates=2)
+    f0, xbar, u = _FIELDS[-1]
+    thetas = np.array([0.9, 2.3, 4.0], np.float32)
+    ys = []
+    for i, th in enumerate(thetas):
+        _, p = oracle.evaluate(g, f0, xbar, u, (0.6 + 0.3 * i) * w, float(th))
+        ys.append(p.astype(np.float32))
+    yd = to_dev(np.stack(ys))
+    w0 = np.zeros((3, 3), np.float32)
+    for fan in (1, 2):
+        opts = pc.Opts(max_iter=4, batched_linesearch=fan if fan > 1 else 0)
+        rec = m.reconstruct_batch(yd, thetas, w0, opts, trace=True)
+        assert m.tile_counts(reset=True)[4] > 0                      # records were gathered
+        one = [m.reconstruct(yd[b], float(thetas[b]), w0[b], opts, trace=True) for b in range(3)]
+        try:
+            pc.tune("grad_records", 0)
+            g2, m0, _, _ = _setup(max_batch=3, max_candidates=2)
+            ref = m0.reconstruct_batch(yd, thetas, w0, opts, trace=True)
+            assert m0.tile_counts(reset=True)[4] == 0
+        finally:
+            pc.tune("grad_records", 1)
+        for b in range(3):
+            assert np.array_equal(rec[b].backtracks, ref[b].backtracks) and rec[b].iters == ref[b].iters
+            assert np.linalg.norm(rec[b].w - ref[b].w) <= 1e-4 * np.linalg.norm(ref[b].w)
+            assert abs(rec[b].J - ref[b].J) <= 1e-5 * ref[b].J
+            # in flight or alone: the same gather in the same order, the same bits
+            assert np.array_equal(rec[b].w, one[b].w) and rec[b].J == one[b].J
+
+
 def test_graph_knobs_change_the_launch_not_the_result():
     """pcamm_tune("pdl") and ("static_passes"): the same kernels in the same order with the same memory effects,
     so a solve gives the same bits whatever the edges of its graph are and wherever its while-loop starts."""
